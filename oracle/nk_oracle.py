@@ -1,0 +1,163 @@
+"""ORACLE — test infrastructure, NOT the product.
+
+Plain, slow, float64 / complex128 CPU restatement of the batched local-energy estimator of NetKet 3
+(arxiv 2112.10526) for an RBM ansatz, written from the paper's definitions.  It shares no code with the
+CUDA path (`paper_2112_10526_b200/csrc`), and only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s
+cpu_baseline / `--impl reference` legs may import it.
+
+What it computes, in the paper's order and notation (citations are PAPER.md lines):
+  * `log_cosh(z)`            stable ln cosh z                       (Eq. (41) L1292 names ln cosh; L1298 `logcosh`)
+  * `rbm_logpsi`             ln psi(s) = a.s + sum_j ln cosh(W s + b)_j   (RBM: L575; W in C^{MxN}, b in C^M: Eq. (7);
+                                                                    formula and visible bias a: BASELINE.json north_star, Q1/Q2)
+  * `connected`              get_conn(s) -> (eta, mels): all eta with <s|H|eta> != 0  (Eq. (3))
+        Heisenberg  H = sum_b J_c(b) sigma_i . sigma_j   (Eq. (50); Pauli matrices, not S = sigma/2, cf. L1624 "/400")
+        Ising       H = J sum_b sz_i sz_j - h sum_i sx_i (Eq. (54))
+  * `local_energy`           A~(s) = sum_s' psi(s')/psi(s) <s|A|s'>  (Eq. (12)) — every ln psi(s') FROM SCRATCH
+  * `stats`                  E[A~] ~ (1/N_s) sum A~(s_i)            (Eq. (17)) and the population variance (Q10)
+
+Pins (tests/test_oracle_pins.py, `-m "not gpu"`): dense Kronecker-product Hamiltonians built independently in
+tests/dense_ref.py (Born identity Eq. (11) L646 over the full space; row-by-row equality of the connected list),
+Eq. (2), closed forms (W = 0; M = 1 with np.cosh; uniform psi), known ring spectra, symmetries.
+No function here is "parity unpinned".
+"""
+from __future__ import annotations
+
+import numpy as np
+
+KIND_HEISENBERG = 0
+KIND_ISING = 1
+FLAG_MARSHALL = 1  # off-diagonal Heisenberg element -2J instead of +2J (Q6; default off)
+
+LN2 = float(np.log(2.0))
+
+
+def log_cosh(z):
+    """ln cosh z, stable for large |Re z|; real or complex input (float64 / complex128).
+
+    cosh is even, so flip z to Re z >= 0, then ln cosh z = z + log1p(exp(-2z)) - ln 2 (principal log1p;
+    its argument has |exp(-2z)| <= 1).  DESIGN.md Q11.
+    """
+    z = np.asarray(z)
+    if np.iscomplexobj(z):
+        z = z.astype(np.complex128)
+        z = np.where(z.real < 0, -z, z)
+        return z + np.log1p(np.exp(-2.0 * z)) - LN2
+    z = np.abs(z.astype(np.float64))
+    return z + np.log1p(np.exp(-2.0 * z)) - LN2
+
+
+def _up(x, cplx):
+    """Exact up-cast of fp32 / complex64 stored parameters (Q12)."""
+    return np.asarray(x).astype(np.complex128 if cplx else np.float64)
+
+
+def rbm_logpsi(sigma, W, a=None, b=None):
+    """ln psi for a batch.  sigma [B][N] (+-1), W [M][N], a [N] or None, b [M] or None -> [B]."""
+    sigma = np.atleast_2d(np.asarray(sigma))
+    cplx = np.iscomplexobj(W)
+    W = _up(W, cplx)
+    s = sigma.astype(np.complex128 if cplx else np.float64)
+    theta = s @ W.T                                   # theta = W s        (Eq. (7))
+    if b is not None:
+        theta = theta + _up(b, cplx)[None, :]         #       + b
+    out = log_cosh(theta).sum(axis=1)                 # sum_j ln cosh theta_j
+    if a is not None:
+        out = out + s @ _up(a, cplx)                  # + sum_i a_i s_i
+    return out
+
+
+def rbm_theta(sigma, W, b=None):
+    """theta = W s + b for a batch, float64/complex128 [B][M]."""
+    cplx = np.iscomplexobj(W)
+    theta = np.atleast_2d(np.asarray(sigma)).astype(np.complex128 if cplx else np.float64) @ _up(W, cplx).T
+    if b is not None:
+        theta = theta + _up(b, cplx)[None, :]
+    return theta
+
+
+def max_conn(kind, n_sites, n_bonds):
+    """Fixed width C of the connected list: slot 0 diagonal + one slot per bond (Heisenberg) / per site (Ising)."""
+    return (n_bonds if kind == KIND_HEISENBERG else n_sites) + 1
+
+
+def connected(kind, sigma_row, bonds, colors, J, h=0.0, flags=0):
+    """get_conn for ONE basis state (Eq. (3)), fixed-width convention of DESIGN.md Q9.
+
+    Returns (sigma_prime int8 [C][N], mels float64 [C], flips int32 [C][2], n_conn int):
+      slot 0        diagonal: sigma itself, H_ss, flips (-1,-1) — always present, even if 0
+      Heisenberg    slot 1+b <-> bond b=(i,j): if s_i != s_j the two spins are exchanged, element 2*J_c(b)
+                    (-2*J_c(b) with FLAG_MARSHALL), flips (i,j); if s_i == s_j a PADDED slot: sigma itself,
+                    element 0, flips (-1,-1)
+      Ising         slot 1+k <-> site k: spin k negated, element -h, flips (k,-1)
+      n_conn        number of non-padded slots (diagonal included)
+    """
+    s = np.asarray(sigma_row, dtype=np.int8)
+    N = s.shape[0]
+    bonds = np.asarray(bonds)
+    J = np.asarray(J, dtype=np.float64)
+    colors = np.zeros(len(bonds), dtype=np.int64) if colors is None else np.asarray(colors)
+    C = max_conn(kind, N, len(bonds))
+    sp = np.tile(s, (C, 1))
+    mels = np.zeros(C, dtype=np.float64)
+    flips = np.full((C, 2), -1, dtype=np.int32)
+    diag = 0.0
+    for bnd, (i, j) in enumerate(bonds):              # sz_i sz_j term of every bond (both models)
+        diag += J[colors[bnd]] * float(s[i]) * float(s[j])
+    mels[0] = diag
+    n_conn = 1
+    if kind == KIND_HEISENBERG:
+        # sx sx + sy sy = 2 (s+ s- + s- s+): exchanges antiparallel spins with element 2 (Pauli convention)
+        off = -2.0 if (flags & FLAG_MARSHALL) else 2.0
+        for bnd, (i, j) in enumerate(bonds):
+            if s[i] != s[j]:
+                sp[1 + bnd, i], sp[1 + bnd, j] = s[j], s[i]
+                mels[1 + bnd] = off * J[colors[bnd]]
+                flips[1 + bnd] = (i, j)
+                n_conn += 1
+    elif kind == KIND_ISING:
+        for k in range(N):                            # -h sx_k flips spin k
+            sp[1 + k, k] = -s[k]
+            mels[1 + k] = -h
+            flips[1 + k] = (k, -1)
+            n_conn += 1
+    else:
+        raise ValueError("unknown operator kind")
+    return sp, mels, flips, n_conn
+
+
+def local_energy(kind, sigma, bonds, colors, J, h, W, a=None, b=None, flags=0):
+    """Local estimator Eq. (12) L652 for every row of sigma: sum over the connected list of
+    mel * exp(ln psi(s') - ln psi(s)), with EVERY ln psi(s') evaluated from scratch by `rbm_logpsi`.
+    Returns (eloc [B] float64|complex128, logpsi [B])."""
+    sigma = np.atleast_2d(np.asarray(sigma, dtype=np.int8))
+    cplx = np.iscomplexobj(W)
+    B = sigma.shape[0]
+    eloc = np.zeros(B, dtype=np.complex128 if cplx else np.float64)
+    logpsi = rbm_logpsi(sigma, W, a, b)
+    for n in range(B):
+        sp, mels, _, _ = connected(kind, sigma[n], bonds, colors, J, h, flags)
+        lp = rbm_logpsi(sp, W, a, b)                  # all C configurations, nothing incremental
+        eloc[n] = np.sum(mels * np.exp(lp - logpsi[n]))
+    return eloc, logpsi
+
+
+def stats(eloc):
+    """Eq. (17): mean over the batch; population variance mean |E - mean|^2 (ddof = 0).
+    Returns (mean_re, mean_im, variance, count) as float64."""
+    e = np.asarray(eloc).astype(np.complex128)
+    m = e.sum() / e.size
+    var = float(np.sum(np.abs(e - m) ** 2) / e.size)
+    return float(m.real), float(m.imag), var, float(e.size)
+
+
+def count_amplitudes(kind, sigma, bonds, colors, J, h=0.0):
+    """Number of off-diagonal connected entries with non-zero matrix element, summed over the batch
+    (the numerator of 'connected-amplitude evaluations/s')."""
+    sigma = np.atleast_2d(np.asarray(sigma, dtype=np.int8))
+    bonds = np.asarray(bonds)
+    if kind == KIND_ISING:
+        return int(sigma.shape[0] * sigma.shape[1]) if h != 0.0 else 0
+    J = np.asarray(J, dtype=np.float64)
+    colors = np.zeros(len(bonds), dtype=np.int64) if colors is None else np.asarray(colors)
+    anti = sigma[:, bonds[:, 0]] != sigma[:, bonds[:, 1]]
+    return int(anti[:, J[colors] != 0.0].sum())
