@@ -1,0 +1,299 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the batched local-energy path (BASELINE.json metric: local energies/s and
+connected-amplitude evaluations/s, with the fraction of the binding roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (pack, theta contraction, ln psi, fused local energy, statistics) over
+one synthetic batch of BASELINE.json configs[--config - 1]; default config 5, the largest single-GPU workload
+(65536 samples, N = 1024, chunks of 4096).  Under torchrun (N > 1) every rank processes its own batch (weak
+scaling; the only exchange is an all-gather of the 4-double statistics).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+CONFIG_TEXT = {
+    1: "configs[0]: 1D Heisenberg L=10, real RBM alpha=1, 1024 samples",
+    2: "configs[1]: 2D Heisenberg 10x10, real RBM alpha=1, 4096 samples",
+    3: "configs[2]: 2D TFIM 20x20 h=3, real RBM alpha=2, 8192 samples",
+    4: "configs[3]: 2D J1-J2 10x10, complex RBM alpha=4, 16384 samples",
+    5: "configs[4]: 2D Heisenberg 32x32, real RBM alpha=2, 65536 samples in chunks of 4096",
+}
+MUFU_LANES_PER_CLK_PER_SM = 16      # 4 SMSPs x 4 lanes
+N_SMS = 148
+
+
+def measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return {}
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], threading.Event()
+
+    def run(self):
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
+                f = [x.strip() for x in out.stdout.strip().split(",")]
+                if len(f) >= 7:
+                    self.rows.append(f)
+            except Exception:
+                pass
+            self.stop_flag.wait(0.1)
+
+    def summary(self):
+        self.stop_flag.set()
+        self.join(timeout=6)
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = sorted(float(r[0]) for r in self.rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons,
+                "samples": len(self.rows), "power_w_max": max(float(r[2]) for r in self.rows)}
+
+
+def oracle_rate(p, n_rows, repeat=1):
+    """Times the float64 oracle (as it stands) on the first n_rows samples; returns (local energies/s, seconds)."""
+    from oracle import nk_oracle as orc
+    t0 = time.perf_counter()
+    for _ in range(repeat):
+        orc.local_energy(p.kind, p.sigma[:n_rows], p.bonds, p.colors, p.J, p.h, p.W, p.a, p.b)
+    dt = time.perf_counter() - t0
+    return n_rows * repeat / dt, dt
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [i.get("num_threads", 1) for i in threadpool_info() if i.get("user_api") == "blas"]
+        return max(n) if n else 1
+    except Exception:
+        return os.cpu_count() or 1
+
+
+ORACLE_ROWS_PER_STEP = {1: 1024, 2: 256, 3: 16, 4: 64, 5: 4}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same config / metric; each step is a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import nk_oracle as orc
+    from paper_2112_10526_b200 import inputs as inp
+    n = ORACLE_ROWS_PER_STEP[args.config]
+    p = inp.make_config(args.config, n_samples=n)
+    for _ in range(args.warmup):
+        oracle_rate(p, n)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_rate(p, n)
+    dt = time.perf_counter() - t0
+    rate = n * args.steps / dt
+    amps = orc.count_amplitudes(p.kind, p.sigma, p.bonds, p.colors, p.J, p.h) / n
+    sample = f"first {n} samples of the batch per step (work is linear in samples)"
+    line = {"impl": "reference", "metric": "local_energies_per_sec", "value": rate, "unit": "local energies/s",
+            "amplitudes_per_sec": rate * amps, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic (seeded, BASELINE.json recipe)",
+            "config": {"workload": CONFIG_TEXT[args.config], "sample": sample},
+            "cpu_baseline": {"value": rate, "unit": "local energies/s", "cores": blas_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": rate, "unit": "local energies/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2112_10526_b200 as nk
+    from paper_2112_10526_b200 import inputs as inp
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    nk.load()
+
+    p = inp.make_config(args.config, sample_seed_offset=rank)           # weak scaling: own batch per rank
+    B, N, M = p.n_samples, p.n_sites, p.n_hidden
+    dt_code = nk.NK_C64 if p.complex_params else nk.NK_F32
+    op = nk.Operator.from_problem(p)
+    sigma_h = torch.from_numpy(p.sigma).pin_memory()
+    W_h, a_h, b_h = (torch.from_numpy(x).pin_memory() for x in (p.W, p.a, p.b))
+    sigma, W, a, b = (t.to(dev) for t in (sigma_h, W_h, a_h, b_h))
+    plan = nk.LocalEnergyPlan(op, B, N, M, dt_code, p.chunk_size, device=dev)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)         # > 126 MB L2
+    gathered = [torch.zeros(4, dtype=torch.float64, device=dev) for _ in range(world)]
+
+    def step():
+        _, _, stats = plan.run(sigma, W, a, b)
+        if world > 1:
+            dist.all_gather(gathered, stats)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+
+    # ---- device-resident timing: K steps, per-step CUDA events, L2 flushed between steps -------------------
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    nk.launch_count(reset=True)
+    nk.profile_enable(True)
+    nk.profile_read()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    for s in range(args.steps):
+        flush.zero_()
+        ev[s][0].record()
+        step()
+        ev[s][1].record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.summary()
+    launches = nk.launch_count(reset=True)
+    phases = nk.profile_read()
+    nk.profile_enable(False)
+    step_ms = [a_.elapsed_time(b_) for a_, b_ in ev]
+    total_ms = float(sum(step_ms))
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+
+    # ---- end to end through the host-buffer C call (pinned inputs, H2D + D2H inside the timed region) -------
+    hplan = nk.HostPlan(op, B, N, M, dt_code, p.chunk_size, device=dev)
+    cdt = torch.complex64 if p.complex_params else torch.float32
+    out = (torch.empty(B, dtype=cdt).pin_memory().numpy(), torch.empty(B, dtype=cdt).pin_memory().numpy(),
+           torch.empty(4, dtype=torch.float64).pin_memory().numpy())
+    host_args = (sigma_h.numpy(), W_h.numpy(), a_h.numpy(), b_h.numpy())
+    for _ in range(2):
+        nk.local_energy_host(op, *host_args, chunk_size=p.chunk_size, plan=hplan, out=out)
+    e2e_steps = max(3, min(args.steps, 10))
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(e2e_steps):
+        nk.local_energy_host(op, *host_args, chunk_size=p.chunk_size, plan=hplan, out=out)
+    e1.record()
+    torch.cuda.synchronize()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item()) / e2e_steps
+    esz = 8 if p.complex_params else 4
+    h2d = B * N + (M * N + N + M) * esz
+    d2h = 2 * B * esz + 32
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- accounting -----------------------------------------------------------------------------------------
+    anti = p.sigma[:, p.bonds[:, 0]] != p.sigma[:, p.bonds[:, 1]]
+    if p.kind == inp.KIND_HEISENBERG:
+        amps = int(anti[:, p.J[p.colors] != 0].sum())
+    else:
+        amps = B * N if p.h != 0 else 0
+    pairs = amps * M                                                     # (amplitude, hidden unit) evaluations
+    fused_ms, fused_n = phases["fused"]
+    fused_ms_per_step = fused_ms / args.steps
+    peaks = measured_peaks()
+    sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0)
+    mufu_per_pair = 3 if p.complex_params else 1
+    peak_pairs = N_SMS * MUFU_LANES_PER_CLK_PER_SM * sm_max * 1e6 / mufu_per_pair / 1e9       # Gpair/s at max clock
+    ach_pairs = pairs / (fused_ms_per_step * 1e-3) / 1e9 if fused_ms_per_step > 0 else 0.0
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", f"fused_dram_bytes_cfg{args.config}.txt")
+    if os.path.exists(tpath):
+        try:
+            traffic = float(open(tpath).read().split()[0])
+        except Exception:
+            traffic = None
+    roofline = {"bound": "alu", "kernel": "fused_eloc_kernel", "achieved": ach_pairs, "peak": peak_pairs,
+                "unit": "Gpair/s", "frac": ach_pairs / peak_pairs if peak_pairs else None, "traffic": traffic,
+                "peak_basis": f"MUFU pipe: {N_SMS} SMs x {MUFU_LANES_PER_CLK_PER_SM} lanes/clk x {sm_max:.0f} MHz / "
+                              f"{mufu_per_pair} MUFU per (amplitude, hidden unit) pair (DESIGN.md)",
+                "ms_per_launch": fused_ms / fused_n if fused_n else None, "launches_per_step": fused_n / args.steps,
+                "frac_at_measured_clock": (ach_pairs / (peak_pairs * clocks["sm_mhz"] / sm_max)
+                                           if clocks.get("sm_mhz") else None),
+                "phase_ms_per_step": {k: v[0] / args.steps for k, v in phases.items()}}
+
+    n_or = ORACLE_ROWS_PER_STEP[args.config] * 4
+    n_or = min(n_or, B)
+    cpu_rate, cpu_s = oracle_rate(p, n_or)
+    cpu = {"value": cpu_rate, "unit": "local energies/s", "cores": blas_threads(), "kind": "oracle",
+           "sample": f"first {n_or} samples of the batch, {cpu_s:.1f} s (work is linear in samples)",
+           "host_cpus": os.cpu_count()}
+
+    value = world * B / (ms_per_step * 1e-3)
+    line = {"metric": "local_energies_per_sec", "value": value, "unit": "local energies/s",
+            "amplitudes_per_sec": world * amps / (ms_per_step * 1e-3), "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "c64" if p.complex_params else "f32",
+            "data": "synthetic (seeded, BASELINE.json recipe)",
+            "config": {"workload": CONFIG_TEXT[args.config], "samples_per_gpu": B, "n_sites": N, "n_hidden": M,
+                       "chunk_size": p.chunk_size, "amplitudes_per_step_per_gpu": amps,
+                       "l2": "flushed between steps (512 MiB memset outside the per-step CUDA events)",
+                       "parallelism": f"samples sharded over {world} rank(s), statistics all-gathered"},
+            "clocks": clocks, "e2e": {"value": world * B / (e2e_ms * 1e-3), "unit": "local energies/s",
+                                      "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms},
+            "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+            "step_ms": [round(x, 4) for x in step_ms], "inputs_sha256": p.sha256()}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,137 @@
+/* nkb200.h — C ABI of libnkb200.so: batched RBM local energies for lattice spin Hamiltonians on one B200.
+ *
+ * The calls follow the paper's statement of the problem (citations: PAPER.md lines of arxiv 2112.10526):
+ *   get_conn(sigma) -> (eta, mels)                         Eq. (3)  L215-219      -> nk_connected
+ *   apply(params, sigma_batch) -> ln psi, batched           Eq. (6)  L273, L410    -> nk_rbm_logpsi
+ *   local estimator A~(s) = sum_s' psi(s')/psi(s) <s|A|s'>  Eq. (12) L652          -> nk_local_energy
+ *   sample mean over the batch                              Eq. (17) L675          -> nk_local_energy (stats_out)
+ *   chunk_size bounds the configurations evaluated at once  Sec. 3.3.1 L689-695    -> nk_local_energy (chunk_size)
+ * Ansatz (RBM, L575; ln cosh form Eq. (41); shapes W in C^{MxN}, b in C^M from Eq. (7)):
+ *   ln psi(s) = sum_i a_i s_i + sum_j ln cosh(theta_j),  theta = W s + b.
+ * Operators (hard-coded matrix elements, the style of L201-203):
+ *   NK_HEISENBERG  H = sum_b J_c(b) sigma_i . sigma_j (Pauli matrices, Eq. (50)): diagonal J s_i s_j,
+ *                  antiparallel bond -> exchanged configuration with element 2 J  (-2 J with NK_FLAG_MARSHALL)
+ *   NK_ISING       H = J sum_b sz_i sz_j - h sum_i sx_i (Eq. (54)): diagonal J s_i s_j, every single-spin
+ *                  flip with element -h
+ *
+ * Conventions
+ *   - "dev" pointers are CUDA device pointers, "host" pointers are ordinary host memory.  All buffers belong to
+ *     the caller.  The library allocates device memory only inside nk_operator_create and frees it only in
+ *     nk_operator_destroy.
+ *   - Every call that takes a stream is asynchronous on that stream (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream) and never synchronises the device, except nk_local_energy_host (see there).
+ *   - Spins are int8 with values +1 / -1, row-major [B][N].  W is row-major [M][N] (theta = W s + b); a is [N],
+ *     b is [M].  dtype NK_F32: float; NK_C64: interleaved (re, im) float pairs.  a and b may be NULL (= zeros).
+ *   - Return value: NK_OK (0) or a negative nk_status.  Argument errors are detected on the host before any
+ *     launch.  No exceptions, no exit(), no CPU fallback: without a CUDA device every compute call returns
+ *     NK_ERR_CUDA.
+ *   - Limits of this version: M <= 2048 (NK_F32) or M <= 1024 (NK_C64); N <= 65535; larger -> NK_ERR_UNSUPPORTED.
+ */
+#ifndef NKB200_H
+#define NKB200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nk_operator_s* nk_operator_t;   /* opaque; device-resident bond table + couplings */
+typedef void* nk_stream_t;                      /* a cudaStream_t */
+
+enum nk_status {
+    NK_OK = 0,
+    NK_ERR_INVALID_ARG = -1,   /* NULL / out-of-range / inconsistent argument */
+    NK_ERR_BAD_SPIN = -2,      /* reserved: sigma value not in {+1,-1} (validation is opt-in, not yet wired) */
+    NK_ERR_WORKSPACE = -3,     /* workspace NULL, misaligned (256 B) or smaller than the *_workspace_bytes query */
+    NK_ERR_UNSUPPORTED = -4,   /* sizes beyond the limits above */
+    NK_ERR_CUDA = -5           /* a CUDA runtime call failed; see nk_last_cuda_error() */
+};
+enum nk_kind { NK_HEISENBERG = 0, NK_ISING = 1 };
+enum nk_dtype { NK_F32 = 0, NK_C64 = 1 };
+enum nk_flags {
+    NK_FLAG_MARSHALL = 1u,     /* nk_operator_create: off-diagonal Heisenberg element -2J (default +2J, Eq. (50)) */
+    NK_OUT_F64 = 2u            /* nk_rbm_logpsi: logpsi_out is double / (re,im) double instead of float */
+};
+
+/* Static, never-NULL description of a status code. */
+const char* nk_status_string(int status);
+/* The cudaError_t (as int) of the most recent NK_ERR_CUDA on this thread, 0 if none. */
+int nk_last_cuda_error(void);
+/* Library version, e.g. 100 = 0.1.0. */
+int nk_version(void);
+
+/* ---- operator ------------------------------------------------------------------------------------------
+ * Copies the bond table to the device.  bonds_host [n_bonds][2] with 0 <= i,j < n_sites and i != j (each
+ * undirected pair listed once; the ORDER of the table fixes the order of the connected list).  colors_host
+ * [n_bonds] in [0, n_colors) or NULL (all 0).  J_host [n_colors].  h is used by NK_ISING only.
+ * Synchronous (cudaMalloc + cudaMemcpy).  Errors: NK_ERR_INVALID_ARG on a bad table, NK_ERR_CUDA. */
+int nk_operator_create(nk_operator_t* out, int kind, int n_sites, int n_bonds, const int32_t* bonds_host,
+                       const int32_t* colors_host, int n_colors, const double* J_host, double h, unsigned flags);
+int nk_operator_destroy(nk_operator_t op);
+/* Width C of the connected list: n_bonds + 1 (Heisenberg) or n_sites + 1 (Ising). */
+int nk_operator_max_conn(nk_operator_t op, int* C_out);
+
+/* ---- ln psi ---------------------------------------------------------------------------------------------
+ * logpsi_out dev [B]: float | (re,im) float, or double | (re,im) double with NK_OUT_F64.  The imaginary part
+ * is returned modulo 2 pi (a sum of principal logs).  theta_out: NULL, or dev [B][M] (float | (re,im) float)
+ * receiving theta = W s + b.  theta is contracted with exact +-1 products and fp32 accumulation; the ln cosh
+ * terms and their sum are evaluated in fp64 (Q12).  workspace: dev, 256-B aligned, at least
+ * nk_rbm_logpsi_workspace_bytes(B, N, M, dtype) bytes. */
+size_t nk_rbm_logpsi_workspace_bytes(int64_t B, int N, int M, int dtype);
+int nk_rbm_logpsi(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* a,
+                  const void* b, void* logpsi_out, void* theta_out, unsigned flags, void* workspace,
+                  size_t workspace_bytes, nk_stream_t stream);
+
+/* ---- connected configurations (inspection / parity call; the fused path never materialises sigma') --------
+ * Fixed-width list per sample, C = nk_operator_max_conn:
+ *   slot 0      diagonal: flips (-1,-1), mel = H_ss (always present)
+ *   Heisenberg  slot 1+b <-> bond b = (i,j): antiparallel -> flips (i,j), mel = +-2 J_c(b), sigma' = sigma with
+ *               s_i, s_j exchanged; parallel -> PADDED: flips (-1,-1), mel 0, sigma' = sigma
+ *   Ising       slot 1+k <-> site k: flips (k,-1), mel = -h, sigma' = sigma with s_k negated
+ * flips_out dev int32 [B][C][2]; mels_out dev float [B][C]; n_conn_out dev int32 [B] = number of non-padded
+ * slots; sigma_prime_out NULL or dev int8 [B][C][N].  Any of the three outputs flips/mels/n_conn may be NULL. */
+int nk_connected(nk_operator_t op, const int8_t* sigma, int64_t B, int32_t* flips_out, float* mels_out,
+                 int32_t* n_conn_out, int8_t* sigma_prime_out, nk_stream_t stream);
+
+/* ---- local energy ---------------------------------------------------------------------------------------
+ * E_loc(s) = H_ss + sum_{s' != s} H_ss' psi(s')/psi(s) for every row of sigma, evaluated chunk_size samples at a
+ * time (0 = whole batch) inside a workspace whose size depends on min(B, chunk_size), not on B.  Per-sample
+ * results do not depend on chunk_size.
+ *   eloc_out    dev [B] float | (re,im) float
+ *   logpsi_out  NULL or dev [B] float | (re,im) float  (ln psi(s), as nk_rbm_logpsi)
+ *   stats_out   NULL or dev double[4]: mean_re, mean_im, population variance mean|E - mean|^2, count
+ * W/a/b packing (transposes, bond-difference table) is redone on every call — the parameters change every VMC
+ * step — and is part of the call's time. */
+size_t nk_local_energy_workspace_bytes(nk_operator_t op, int64_t B, int N, int M, int dtype, int64_t chunk_size);
+int nk_local_energy(nk_operator_t op, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
+                    const void* a, const void* b, int64_t chunk_size, void* eloc_out, void* logpsi_out,
+                    double* stats_out, void* workspace, size_t workspace_bytes, nk_stream_t stream);
+
+/* Same computation with HOST inputs and outputs (the end-to-end call): copies sigma/W/a/b host->device into
+ * `scratch`, runs nk_local_energy, copies eloc / logpsi / stats back and SYNCHRONISES `stream` before returning.
+ * Host buffers should be pinned for the copies to be asynchronous.  scratch: dev, 256-B aligned, at least
+ * nk_local_energy_host_scratch_bytes(...) bytes (inputs + outputs + workspace).  eloc_host [B], logpsi_host [B]
+ * or NULL, stats_host double[4] or NULL. */
+size_t nk_local_energy_host_scratch_bytes(nk_operator_t op, int64_t B, int N, int M, int dtype, int64_t chunk_size);
+int nk_local_energy_host(nk_operator_t op, const int8_t* sigma_host, int64_t B, int N, int M, int dtype,
+                         const void* W_host, const void* a_host, const void* b_host, int64_t chunk_size,
+                         void* eloc_host, void* logpsi_host, double* stats_host, void* scratch,
+                         size_t scratch_bytes, nk_stream_t stream);
+
+/* Per-phase device timing (bench accounting).  With nk_profile_enable(1), nk_local_energy brackets each phase
+ * of each chunk with CUDA events on the call's stream (a few microseconds of timeline each).  nk_profile_read
+ * synchronises on those events, adds up the elapsed milliseconds per phase since the last read and writes
+ * out[0..4] = ms in {pack, theta contraction, ln psi, fused local energy, statistics}, out[5..9] = the number of
+ * bracketed launches groups per phase; then clears the record.  Thread-local, like nk_launch_count. */
+int nk_profile_enable(int on);
+int nk_profile_read(double* out10_host);
+
+/* Number of kernels the library launched on this thread since the last call with reset != 0 (bench accounting). */
+int64_t nk_launch_count(int reset);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NKB200_H */

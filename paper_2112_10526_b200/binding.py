@@ -1,1 +1,297 @@
-__all__ = []
+"""ctypes binding over libnkb200.so (include/nkb200.h).  Argument marshalling only: every step of the path runs
+in the library's CUDA kernels.  torch is used to allocate device memory and to supply the current stream.
+
+There is no CPU fallback: if the shared library is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+__all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host",
+           "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
+           "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "EXPORTS"]
+
+NK_HEISENBERG, NK_ISING = 0, 1
+NK_F32, NK_C64 = 0, 1
+NK_FLAG_MARSHALL, NK_OUT_F64 = 1, 2
+LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libnkb200.so")
+
+_vp, _i64, _int, _sz, _u32, _dbl = C.c_void_p, C.c_int64, C.c_int, C.c_size_t, C.c_uint, C.c_double
+# name -> (restype, argtypes): every symbol include/nkb200.h declares
+EXPORTS = {
+    "nk_status_string": (C.c_char_p, [_int]),
+    "nk_last_cuda_error": (_int, []),
+    "nk_version": (_int, []),
+    "nk_operator_create": (_int, [C.POINTER(_vp), _int, _int, _int, _vp, _vp, _int, _vp, _dbl, _u32]),
+    "nk_operator_destroy": (_int, [_vp]),
+    "nk_operator_max_conn": (_int, [_vp, C.POINTER(_int)]),
+    "nk_rbm_logpsi_workspace_bytes": (_sz, [_i64, _int, _int, _int]),
+    "nk_rbm_logpsi": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _vp, _u32, _vp, _sz, _vp]),
+    "nk_connected": (_int, [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp]),
+    "nk_local_energy_workspace_bytes": (_sz, [_vp, _i64, _int, _int, _int, _i64]),
+    "nk_local_energy": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "nk_local_energy_host_scratch_bytes": (_sz, [_vp, _i64, _int, _int, _int, _i64]),
+    "nk_local_energy_host": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "nk_launch_count": (_i64, [_int]),
+    "nk_profile_enable": (_int, [_int]),
+    "nk_profile_read": (_int, [_vp]),
+}
+
+_lib = None
+
+
+class NkError(RuntimeError):
+    pass
+
+
+def load():
+    """Open libnkb200.so (built in-tree by `python -m paper_2112_10526_b200.build`).  Raises if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise NkError(f"{LIB_PATH} not found: build it with `python -m paper_2112_10526_b200.build` "
+                          "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        for name, (res, args) in EXPORTS.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        lib = load()
+        msg = lib.nk_status_string(rc).decode()
+        raise NkError(f"{what}: {msg} (status {rc}, cudaError {lib.nk_last_cuda_error()})")
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _stream():
+    return _torch().cuda.current_stream().cuda_stream
+
+
+def _ptr(t):
+    return None if t is None else t.data_ptr()
+
+
+def _dtype_code(W) -> int:
+    torch = _torch()
+    if W.dtype == torch.float32:
+        return NK_F32
+    if W.dtype == torch.complex64:
+        return NK_C64
+    raise NkError("W must be float32 or complex64")
+
+
+def _check_params(sigma, W, a, b):
+    torch = _torch()
+    if sigma.dtype != torch.int8 or sigma.dim() != 2 or not sigma.is_contiguous() or not sigma.is_cuda:
+        raise NkError("sigma must be a contiguous CUDA int8 tensor [B][N]")
+    if W.dim() != 2 or not W.is_contiguous() or not W.is_cuda or W.shape[1] != sigma.shape[1]:
+        raise NkError("W must be a contiguous CUDA tensor [M][N]")
+    for name, t, n in (("a", a, W.shape[1]), ("b", b, W.shape[0])):
+        if t is not None and (t.dtype != W.dtype or tuple(t.shape) != (n,) or not t.is_contiguous() or not t.is_cuda):
+            raise NkError(f"{name} must be a contiguous CUDA tensor of W's dtype and length {n}")
+
+
+class Operator:
+    """nk_operator_t: device-resident bond table + couplings (nk_operator_create / nk_operator_destroy)."""
+
+    def __init__(self, kind: int, n_sites: int, bonds, colors=None, J=(1.0,), h: float = 0.0, flags: int = 0):
+        lib = load()
+        bonds = np.ascontiguousarray(np.asarray(bonds, dtype=np.int32).reshape(-1, 2))
+        J = np.ascontiguousarray(np.asarray(J, dtype=np.float64).reshape(-1))
+        col = None if colors is None else np.ascontiguousarray(np.asarray(colors, dtype=np.int32))
+        if col is not None and col.shape != (len(bonds),):
+            raise NkError("colors must have one entry per bond")
+        self.kind, self.n_sites, self.n_bonds = int(kind), int(n_sites), len(bonds)
+        h_ = _vp()
+        rc = lib.nk_operator_create(C.byref(h_), self.kind, self.n_sites, self.n_bonds,
+                                    bonds.ctypes.data if len(bonds) else None,
+                                    None if col is None else col.ctypes.data, len(J), J.ctypes.data, float(h),
+                                    int(flags))
+        _check(rc, "nk_operator_create")
+        self.handle = h_
+        c = _int()
+        _check(lib.nk_operator_max_conn(self.handle, C.byref(c)), "nk_operator_max_conn")
+        self.max_conn = c.value
+
+    @classmethod
+    def from_problem(cls, p, flags: int = 0):
+        return cls(p.kind, p.n_sites, p.bonds, p.colors, p.J, p.h, flags)
+
+    def close(self):
+        if getattr(self, "handle", None) is not None and _lib is not None:
+            _lib.nk_operator_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def rbm_logpsi(sigma, W, a=None, b=None, *, out_f64: bool = False, return_theta: bool = False):
+    """nk_rbm_logpsi: ln psi [B] (and theta [B][M]) for device tensors."""
+    torch = _torch()
+    lib = load()
+    _check_params(sigma, W, a, b)
+    B, N = sigma.shape
+    M = W.shape[0]
+    dt = _dtype_code(W)
+    cplx = dt == NK_C64
+    odt = (torch.complex128 if cplx else torch.float64) if out_f64 else (torch.complex64 if cplx else torch.float32)
+    out = torch.empty(B, dtype=odt, device=sigma.device)
+    theta = torch.empty((B, M), dtype=W.dtype, device=sigma.device) if return_theta else None
+    nbytes = lib.nk_rbm_logpsi_workspace_bytes(B, N, M, dt)
+    ws = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=sigma.device)
+    rc = lib.nk_rbm_logpsi(_ptr(sigma), B, N, M, dt, _ptr(W), _ptr(a), _ptr(b), _ptr(out), _ptr(theta),
+                           NK_OUT_F64 if out_f64 else 0, _ptr(ws), ws.numel(), _stream())
+    _check(rc, "nk_rbm_logpsi")
+    return (out, theta) if return_theta else out
+
+
+def connected(op: Operator, sigma, *, materialize: bool = False):
+    """nk_connected: (flips [B][C][2] int32, mels [B][C] f32, n_conn [B] int32, sigma' [B][C][N] int8 | None)."""
+    torch = _torch()
+    lib = load()
+    if sigma.dtype != torch.int8 or sigma.dim() != 2 or not sigma.is_contiguous() or sigma.shape[1] != op.n_sites:
+        raise NkError("sigma must be a contiguous CUDA int8 tensor [B][n_sites]")
+    B, N = sigma.shape
+    Cw = op.max_conn
+    flips = torch.empty((B, Cw, 2), dtype=torch.int32, device=sigma.device)
+    mels = torch.empty((B, Cw), dtype=torch.float32, device=sigma.device)
+    n_conn = torch.empty(B, dtype=torch.int32, device=sigma.device)
+    sp = torch.empty((B, Cw, N), dtype=torch.int8, device=sigma.device) if materialize else None
+    rc = lib.nk_connected(op.handle, _ptr(sigma), B, _ptr(flips), _ptr(mels), _ptr(n_conn), _ptr(sp), _stream())
+    _check(rc, "nk_connected")
+    return flips, mels, n_conn, sp
+
+
+class LocalEnergyPlan:
+    """Pre-allocated outputs + workspace for repeated nk_local_energy calls of one shape (used by bench.py so
+    that the timed region contains nothing but the C call)."""
+
+    def __init__(self, op: Operator, B: int, N: int, M: int, dtype_code: int, chunk_size: int = 0, device="cuda",
+                 want_logpsi: bool = True):
+        torch = _torch()
+        lib = load()
+        self.op, self.B, self.N, self.M, self.dt, self.chunk = op, int(B), int(N), int(M), dtype_code, int(chunk_size)
+        cdt = torch.complex64 if dtype_code == NK_C64 else torch.float32
+        self.eloc = torch.empty(B, dtype=cdt, device=device)
+        self.logpsi = torch.empty(B, dtype=cdt, device=device) if want_logpsi else None
+        self.stats = torch.zeros(4, dtype=torch.float64, device=device)
+        self.ws_bytes = lib.nk_local_energy_workspace_bytes(op.handle, B, N, M, dtype_code, self.chunk)
+        if self.ws_bytes == 0:
+            raise NkError("nk_local_energy_workspace_bytes rejected the arguments")
+        self.ws = torch.empty(self.ws_bytes, dtype=torch.uint8, device=device)
+
+    def run(self, sigma, W, a, b):
+        rc = load().nk_local_energy(self.op.handle, _ptr(sigma), self.B, self.N, self.M, self.dt, _ptr(W), _ptr(a),
+                                    _ptr(b), self.chunk, _ptr(self.eloc), _ptr(self.logpsi), _ptr(self.stats),
+                                    _ptr(self.ws), self.ws_bytes, _stream())
+        _check(rc, "nk_local_energy")
+        return self.eloc, self.logpsi, self.stats
+
+
+def local_energy(op: Operator, sigma, W, a=None, b=None, *, chunk_size: int = 0, want_logpsi: bool = True):
+    """nk_local_energy on device tensors -> (eloc [B], logpsi [B] | None, stats double[4])."""
+    _check_params(sigma, W, a, b)
+    plan = LocalEnergyPlan(op, sigma.shape[0], sigma.shape[1], W.shape[0], _dtype_code(W), chunk_size,
+                           device=sigma.device, want_logpsi=want_logpsi)
+    return plan.run(sigma, W, a, b)
+
+
+class HostPlan:
+    """Device scratch for nk_local_energy_host (inputs + outputs + workspace), reusable across calls."""
+
+    def __init__(self, op, B, N, M, dtype_code, chunk_size=0, device="cuda"):
+        torch = _torch()
+        self.bytes = load().nk_local_energy_host_scratch_bytes(op.handle, B, N, M, dtype_code, int(chunk_size))
+        if self.bytes == 0:
+            raise NkError("nk_local_energy_host_scratch_bytes rejected the arguments")
+        self.scratch = torch.empty(self.bytes, dtype=torch.uint8, device=device)
+
+
+def local_energy_host(op: Operator, sigma, W, a=None, b=None, *, chunk_size: int = 0, want_logpsi: bool = True,
+                      plan: HostPlan | None = None, out=None):
+    """nk_local_energy_host on HOST numpy arrays (ideally views of pinned torch tensors).
+    Returns (eloc, logpsi | None, stats[4]) as numpy arrays; synchronises the stream."""
+    lib = load()
+    sigma = np.ascontiguousarray(sigma, dtype=np.int8)
+    W = np.ascontiguousarray(W)
+    if W.dtype not in (np.float32, np.complex64):
+        raise NkError("W must be float32 or complex64")
+    dt = NK_C64 if W.dtype == np.complex64 else NK_F32
+    B, N = sigma.shape
+    M = W.shape[0]
+    a = None if a is None else np.ascontiguousarray(a, dtype=W.dtype)
+    b = None if b is None else np.ascontiguousarray(b, dtype=W.dtype)
+    if plan is None:
+        plan = HostPlan(op, B, N, M, dt, chunk_size)
+    if out is None:
+        out = (np.empty(B, dtype=W.dtype), np.empty(B, dtype=W.dtype) if want_logpsi else None,
+               np.empty(4, dtype=np.float64))
+    eloc, logpsi, stats = out
+    p = lambda x: None if x is None else x.ctypes.data
+    rc = lib.nk_local_energy_host(op.handle, p(sigma), B, N, M, dt, p(W), p(a), p(b), int(chunk_size), p(eloc),
+                                  p(logpsi), p(stats), _ptr(plan.scratch), plan.bytes, _stream())
+    _check(rc, "nk_local_energy_host")
+    return eloc, logpsi, stats
+
+
+def launch_count(reset: bool = False) -> int:
+    return int(load().nk_launch_count(1 if reset else 0))
+
+
+PHASES = ("pack", "theta", "logpsi", "fused", "stats")
+
+
+def profile_enable(on: bool = True):
+    _check(load().nk_profile_enable(1 if on else 0), "nk_profile_enable")
+
+
+def profile_read() -> dict:
+    """{phase: (total ms, bracketed launch groups)} since the last read (synchronises on the recorded events)."""
+    out = np.zeros(10, dtype=np.float64)
+    _check(load().nk_profile_read(out.ctypes.data), "nk_profile_read")
+    return {ph: (float(out[i]), int(out[5 + i])) for i, ph in enumerate(PHASES)}
+
+
+# ---- multi-GPU: samples shard across ranks, the only exchange is the statistics ----------
+def combine_stats(parts):
+    """Combine per-shard (mean_re, mean_im, variance, count) into the statistics of the union (Chan et al.
+    pairwise update).  Host arithmetic on 4 doubles per shard; used after an all-gather of the stats."""
+    n_tot, mr, mi, m2 = 0.0, 0.0, 0.0, 0.0
+    for p in parts:
+        pr, pi, pv, n = (float(x) for x in p)
+        if n == 0:
+            continue
+        d_r, d_i = pr - mr, pi - mi
+        new_n = n_tot + n
+        m2 += pv * n + (d_r * d_r + d_i * d_i) * n_tot * n / new_n
+        mr += d_r * n / new_n
+        mi += d_i * n / new_n
+        n_tot = new_n
+    return np.array([mr, mi, m2 / n_tot if n_tot else 0.0, n_tot])
+
+
+def allreduce_stats(stats):
+    """All-gather the 4-double statistics over torch.distributed (NCCL on GPUs, gloo on CPU) and combine."""
+    torch = _torch()
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return combine_stats([stats.detach().cpu().numpy() if hasattr(stats, "detach") else stats])
+    t = stats if hasattr(stats, "detach") else torch.as_tensor(np.asarray(stats, dtype=np.float64))
+    gathered = [torch.empty_like(t) for _ in range(dist.get_world_size())]
+    dist.all_gather(gathered, t.contiguous())
+    return combine_stats([g.cpu().numpy() for g in gathered])

@@ -1,0 +1,368 @@
+// C ABI of libnkb200.so (include/nkb200.h): argument validation, workspace carving, the chunked driver
+// (Sec. 3.3.1: chunk_size bounds the configurations evaluated at once).
+#include <new>
+#include <vector>
+
+#include "nk_internal.h"
+
+namespace nk {
+
+static thread_local int tl_last_cuda = 0;
+static thread_local int64_t tl_launches = 0;
+void count_launch(int n) { tl_launches += n; }
+
+// ---- optional per-phase event timing ----
+enum Phase { PH_PACK = 0, PH_GEMM, PH_LOGPSI, PH_FUSED, PH_STATS, PH_COUNT };
+struct Span { int phase; cudaEvent_t a, b; };
+static thread_local bool tl_prof = false;
+static thread_local std::vector<Span> tl_spans;
+struct Scope {
+    cudaStream_t st; Span sp; bool on;
+    Scope(int phase, cudaStream_t s) : st(s), on(tl_prof) {
+        if (!on) return;
+        sp.phase = phase;
+        if (cudaEventCreate(&sp.a) != cudaSuccess || cudaEventCreate(&sp.b) != cudaSuccess) { on = false; return; }
+        cudaEventRecord(sp.a, st);
+    }
+    ~Scope() {
+        if (!on) return;
+        cudaEventRecord(sp.b, st);
+        tl_spans.push_back(sp);
+    }
+};
+
+static int cuda_fail(cudaError_t e) {
+    tl_last_cuda = (int)e;
+    return NK_ERR_CUDA;
+}
+#define NK_CUDA(x)                                   \
+    do {                                             \
+        cudaError_t e__ = (x);                       \
+        if (e__ != cudaSuccess) return cuda_fail(e__); \
+    } while (0)
+
+Geometry make_geometry(const Operator* op, int N, int M, int dtype) {
+    Geometry g{};
+    const bool cplx = dtype == NK_C64;
+    g.N = N; g.N_pad = round_up(N, 16);
+    g.M = M; g.M_pad = round_up(M, MPAD_ALIGN);
+    g.planes = cplx ? 2 : 1;
+    g.M_eff = g.planes * g.M_pad;
+    g.n_rows = op ? (op->kind == NK_HEISENBERG ? op->n_bonds : op->n_sites) : 0;
+    g.ok = g.M_pad / MPAD_ALIGN <= (cplx ? MAX_V_CPLX : MAX_V_REAL) && N <= 65535 && g.n_rows <= 65535;
+    g.ctas_per_sm = fused_ctas_per_sm(g.M_pad, cplx);
+    // shared-memory plan of the fused kernel: [stages x tile][sigma rows][2 x stages mbarriers]
+    const size_t budget = (size_t)(227 * 1024) / g.ctas_per_sm - 1024;
+    const size_t sig = (size_t)fused_consumer_warps() * g.N_pad;
+    const size_t row_bytes = (size_t)g.M_eff * 4;
+    if (sig + 2 * row_bytes + 64 > budget) { g.ok = false; g.tile_rows = 1; g.stages = 2; }
+    else {
+        size_t target = (budget - sig - 64) / 3;
+        if (target > 64 * 1024) target = 64 * 1024;
+        int tr = (int)(target / row_bytes);
+        if (tr < 1) tr = 1;
+        if (tr > 32) tr = 32;
+        g.tile_rows = tr;
+        int stages = (int)((budget - sig - 64) / (tr * row_bytes));
+        if (stages > 4) stages = 4;
+        g.stages = stages;       // >= 2 by the check above (tr = 1) or >= 3 by construction
+    }
+    g.n_tiles = (g.n_rows + g.tile_rows - 1) / g.tile_rows;
+    g.n_rows_pad = g.n_tiles * g.tile_rows;
+    if (g.n_rows_pad == 0) g.n_rows_pad = g.tile_rows;   // keep the tables non-empty
+    g.smem_bytes = (size_t)g.stages * g.tile_rows * row_bytes + sig + 2 * 8 * (size_t)g.stages;
+    return g;
+}
+
+// workspace carving: a bump allocator over the caller's buffer (256-B aligned pieces)
+struct Carver {
+    uint8_t* base;
+    size_t off = 0;
+    explicit Carver(void* p) : base((uint8_t*)p) {}
+    template <typename T>
+    T* take(size_t count) {
+        T* r = (T*)(base ? base + off : nullptr);
+        off += align256(count * sizeof(T));
+        return r;
+    }
+};
+
+struct LogpsiWs {
+    float *Wg, *bg, *theta;
+    size_t bytes;
+};
+static LogpsiWs carve_logpsi(void* ws, const Geometry& g, int64_t rows) {
+    Carver c(ws);
+    LogpsiWs w;
+    w.Wg = c.take<float>((size_t)g.M_eff * g.N);
+    w.bg = c.take<float>(g.M_eff);
+    w.theta = c.take<float>((size_t)rows * g.M_eff);
+    w.bytes = c.off;
+    return w;
+}
+struct ElocWs {
+    float *Wg, *bg, *Wt, *Dtab, *theta;
+    RowInfo* rows;
+    size_t bytes;
+};
+static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk) {
+    Carver c(ws);
+    ElocWs w;
+    w.Wg = c.take<float>((size_t)g.M_eff * g.N);
+    w.bg = c.take<float>(g.M_eff);
+    w.Wt = c.take<float>((size_t)g.N * g.M_eff);
+    w.Dtab = c.take<float>((size_t)g.n_rows_pad * g.M_eff);
+    w.rows = c.take<RowInfo>(g.n_rows_pad);
+    w.theta = c.take<float>((size_t)chunk * g.M_eff);
+    w.bytes = c.off;
+    return w;
+}
+
+static bool bad_dims(int64_t B, int N, int M, int dtype) {
+    return B < 0 || N <= 0 || M <= 0 || (dtype != NK_F32 && dtype != NK_C64);
+}
+
+}  // namespace nk
+
+using namespace nk;
+
+extern "C" {
+
+const char* nk_status_string(int status) {
+    switch (status) {
+        case NK_OK: return "NK_OK";
+        case NK_ERR_INVALID_ARG: return "NK_ERR_INVALID_ARG: null, out-of-range or inconsistent argument";
+        case NK_ERR_BAD_SPIN: return "NK_ERR_BAD_SPIN: spin value not in {+1,-1}";
+        case NK_ERR_WORKSPACE: return "NK_ERR_WORKSPACE: workspace null, misaligned or too small";
+        case NK_ERR_UNSUPPORTED: return "NK_ERR_UNSUPPORTED: sizes beyond this version's limits";
+        case NK_ERR_CUDA: return "NK_ERR_CUDA: a CUDA runtime call failed (see nk_last_cuda_error)";
+        default: return "unknown nk_status";
+    }
+}
+int nk_last_cuda_error(void) { return tl_last_cuda; }
+int nk_version(void) { return 100; }
+int64_t nk_launch_count(int reset) {
+    const int64_t v = tl_launches;
+    if (reset) tl_launches = 0;
+    return v;
+}
+
+int nk_profile_enable(int on) {
+    tl_prof = on != 0;
+    return NK_OK;
+}
+int nk_profile_read(double* out) {
+    if (!out) return NK_ERR_INVALID_ARG;
+    for (int i = 0; i < 2 * PH_COUNT; ++i) out[i] = 0.0;
+    int rc = NK_OK;
+    for (const Span& sp : tl_spans) {
+        float ms = 0.f;
+        cudaError_t e = cudaEventSynchronize(sp.b);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, sp.a, sp.b);
+        if (e != cudaSuccess) rc = cuda_fail(e);
+        else { out[sp.phase] += ms; out[PH_COUNT + sp.phase] += 1.0; }
+        cudaEventDestroy(sp.a); cudaEventDestroy(sp.b);
+    }
+    tl_spans.clear();
+    return rc;
+}
+
+int nk_operator_create(nk_operator_t* out, int kind, int n_sites, int n_bonds, const int32_t* bonds_host,
+                       const int32_t* colors_host, int n_colors, const double* J_host, double h, unsigned flags) {
+    if (!out) return NK_ERR_INVALID_ARG;
+    *out = nullptr;
+    if ((kind != NK_HEISENBERG && kind != NK_ISING) || n_sites <= 0 || n_bonds < 0 || n_colors <= 0 || !J_host ||
+        (n_bonds > 0 && !bonds_host) || (flags & ~NK_FLAG_MARSHALL))
+        return NK_ERR_INVALID_ARG;
+    for (int b = 0; b < n_bonds; ++b) {
+        const int i = bonds_host[2 * b], j = bonds_host[2 * b + 1];
+        if (i < 0 || j < 0 || i >= n_sites || j >= n_sites || i == j) return NK_ERR_INVALID_ARG;
+        if (colors_host && (colors_host[b] < 0 || colors_host[b] >= n_colors)) return NK_ERR_INVALID_ARG;
+    }
+    Operator* op = new (std::nothrow) Operator();
+    if (!op) return NK_ERR_INVALID_ARG;
+    op->kind = kind; op->n_sites = n_sites; op->n_bonds = n_bonds; op->n_colors = n_colors; op->flags = flags; op->h = h;
+    op->d_bonds = nullptr; op->d_colors = nullptr; op->d_Jf = nullptr; op->d_Jd = nullptr;
+    std::vector<int32_t> colors(n_bonds > 0 ? n_bonds : 1, 0);
+    if (colors_host) for (int b = 0; b < n_bonds; ++b) colors[b] = colors_host[b];
+    std::vector<float> Jf(n_colors);
+    for (int c = 0; c < n_colors; ++c) Jf[c] = (float)J_host[c];
+    const size_t nb = n_bonds > 0 ? n_bonds : 1;
+    cudaError_t e = cudaMalloc(&op->d_bonds, nb * 2 * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc(&op->d_colors, nb * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc(&op->d_Jf, n_colors * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&op->d_Jd, n_colors * sizeof(double));
+    if (e == cudaSuccess && n_bonds > 0)
+        e = cudaMemcpy(op->d_bonds, bonds_host, (size_t)n_bonds * 2 * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(op->d_colors, colors.data(), nb * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(op->d_Jf, Jf.data(), n_colors * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(op->d_Jd, J_host, n_colors * sizeof(double), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        nk_operator_destroy((nk_operator_t)op);
+        return cuda_fail(e);
+    }
+    *out = (nk_operator_t)op;
+    return NK_OK;
+}
+
+int nk_operator_destroy(nk_operator_t h) {
+    if (!h) return NK_ERR_INVALID_ARG;
+    Operator* op = (Operator*)h;
+    cudaFree(op->d_bonds); cudaFree(op->d_colors); cudaFree(op->d_Jf); cudaFree(op->d_Jd);
+    delete op;
+    return NK_OK;
+}
+
+int nk_operator_max_conn(nk_operator_t h, int* C_out) {
+    if (!h || !C_out) return NK_ERR_INVALID_ARG;
+    const Operator* op = (const Operator*)h;
+    *C_out = (op->kind == NK_HEISENBERG ? op->n_bonds : op->n_sites) + 1;
+    return NK_OK;
+}
+
+size_t nk_rbm_logpsi_workspace_bytes(int64_t B, int N, int M, int dtype) {
+    if (bad_dims(B, N, M, dtype)) return 0;
+    const Geometry g = make_geometry(nullptr, N, M, dtype);
+    return carve_logpsi(nullptr, g, B).bytes;
+}
+
+int nk_rbm_logpsi(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* a,
+                  const void* b, void* logpsi_out, void* theta_out, unsigned flags, void* workspace,
+                  size_t workspace_bytes, nk_stream_t stream) {
+    if (bad_dims(B, N, M, dtype) || !W || (flags & ~NK_OUT_F64) || (B > 0 && (!sigma || !logpsi_out)))
+        return NK_ERR_INVALID_ARG;
+    const Geometry g = make_geometry(nullptr, N, M, dtype);
+    if (g.M_pad / MPAD_ALIGN > (dtype == NK_C64 ? MAX_V_CPLX : MAX_V_REAL) || N > 65535) return NK_ERR_UNSUPPORTED;
+    if (B == 0) return NK_OK;
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_logpsi(nullptr, g, B).bytes)
+        return NK_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const LogpsiWs w = carve_logpsi(workspace, g, B);
+    NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.Wg, w.bg, st));
+    NK_CUDA(launch_theta_gemm(sigma, B, N, g.M_eff, w.Wg, w.bg, w.theta, st));
+    NK_CUDA(launch_logpsi(sigma, B, g, dtype, w.theta, a, logpsi_out, (flags & NK_OUT_F64) != 0, theta_out, st));
+    return NK_OK;
+}
+
+int nk_connected(nk_operator_t h, const int8_t* sigma, int64_t B, int32_t* flips_out, float* mels_out,
+                 int32_t* n_conn_out, int8_t* sigma_prime_out, nk_stream_t stream) {
+    if (!h || B < 0 || (B > 0 && !sigma)) return NK_ERR_INVALID_ARG;
+    const Operator* op = (const Operator*)h;
+    if (op->n_sites > 48 * 1024) return NK_ERR_UNSUPPORTED;
+    NK_CUDA(launch_connected(op, sigma, B, flips_out, mels_out, n_conn_out, sigma_prime_out, (cudaStream_t)stream));
+    return NK_OK;
+}
+
+static int64_t eff_chunk(int64_t B, int64_t chunk_size) {
+    if (chunk_size <= 0 || chunk_size > B) return B > 0 ? B : 1;
+    return chunk_size;
+}
+
+size_t nk_local_energy_workspace_bytes(nk_operator_t h, int64_t B, int N, int M, int dtype, int64_t chunk_size) {
+    if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0) return 0;
+    const Operator* op = (const Operator*)h;
+    const Geometry g = make_geometry(op, N, M, dtype);
+    return carve_eloc(nullptr, g, eff_chunk(B, chunk_size)).bytes;
+}
+
+int nk_local_energy(nk_operator_t h, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
+                    const void* a, const void* b, int64_t chunk_size, void* eloc_out, void* logpsi_out,
+                    double* stats_out, void* workspace, size_t workspace_bytes, nk_stream_t stream) {
+    if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0 || !W || (B > 0 && (!sigma || !eloc_out)))
+        return NK_ERR_INVALID_ARG;
+    const Operator* op = (const Operator*)h;
+    if (N != op->n_sites) return NK_ERR_INVALID_ARG;
+    const Geometry g = make_geometry(op, N, M, dtype);
+    if (!g.ok) return NK_ERR_UNSUPPORTED;
+    const int64_t chunk = eff_chunk(B, chunk_size);
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_eloc(nullptr, g, chunk).bytes)
+        return NK_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const ElocWs w = carve_eloc(workspace, g, chunk);
+    NK_CUDA(fused_eloc_init());
+    {
+        Scope sc(PH_PACK, st);
+        NK_CUDA(launch_pack(op, g, dtype, W, a, b, w.Wg, w.bg, w.Wt, w.Dtab, w.rows, st));
+    }
+    const size_t esz = dtype == NK_C64 ? 8 : 4;
+    for (int64_t s0 = 0; s0 < B; s0 += chunk) {
+        const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
+        const int8_t* sg = sigma + s0 * N;
+        {
+            Scope sc(PH_GEMM, st);
+            NK_CUDA(launch_theta_gemm(sg, nb, N, g.M_eff, w.Wg, w.bg, w.theta, st));
+        }
+        if (logpsi_out) {
+            Scope sc(PH_LOGPSI, st);
+            NK_CUDA(launch_logpsi(sg, nb, g, dtype, w.theta, a, (uint8_t*)logpsi_out + s0 * esz, false, nullptr, st));
+        }
+        {
+            Scope sc(PH_FUSED, st);
+            NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Dtab, w.rows, (uint8_t*)eloc_out + s0 * esz, st));
+        }
+    }
+    if (stats_out) {
+        Scope sc(PH_STATS, st);
+        NK_CUDA(launch_stats(eloc_out, B, dtype, stats_out, st));
+    }
+    return NK_OK;
+}
+
+// ---- host-buffer entry point ---------------------------------------------------------------------------
+namespace {
+struct HostScratch {
+    int8_t* sigma;
+    void *W, *a, *b, *eloc, *logpsi, *ws;
+    double* stats;
+    size_t ws_bytes, bytes;
+};
+HostScratch carve_host(void* scratch, nk_operator_t h, int64_t B, int N, int M, int dtype, int64_t chunk_size) {
+    const size_t esz = dtype == NK_C64 ? 8 : 4;
+    Carver c(scratch);
+    HostScratch s;
+    s.sigma = c.take<int8_t>((size_t)B * N);
+    s.W = c.take<uint8_t>((size_t)M * N * esz);
+    s.a = c.take<uint8_t>((size_t)N * esz);
+    s.b = c.take<uint8_t>((size_t)M * esz);
+    s.eloc = c.take<uint8_t>((size_t)B * esz);
+    s.logpsi = c.take<uint8_t>((size_t)B * esz);
+    s.stats = c.take<double>(4);
+    s.ws_bytes = nk_local_energy_workspace_bytes(h, B, N, M, dtype, chunk_size);
+    s.ws = c.take<uint8_t>(s.ws_bytes);
+    s.bytes = c.off;
+    return s;
+}
+}  // namespace
+
+size_t nk_local_energy_host_scratch_bytes(nk_operator_t h, int64_t B, int N, int M, int dtype, int64_t chunk_size) {
+    if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0) return 0;
+    return carve_host(nullptr, h, B, N, M, dtype, chunk_size).bytes;
+}
+
+int nk_local_energy_host(nk_operator_t h, const int8_t* sigma_host, int64_t B, int N, int M, int dtype,
+                         const void* W_host, const void* a_host, const void* b_host, int64_t chunk_size,
+                         void* eloc_host, void* logpsi_host, double* stats_host, void* scratch, size_t scratch_bytes,
+                         nk_stream_t stream) {
+    if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0 || !W_host || (B > 0 && (!sigma_host || !eloc_host)))
+        return NK_ERR_INVALID_ARG;
+    if (!scratch || ((uintptr_t)scratch & 255)) return NK_ERR_WORKSPACE;
+    const HostScratch s = carve_host(scratch, h, B, N, M, dtype, chunk_size);
+    if (scratch_bytes < s.bytes) return NK_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t esz = dtype == NK_C64 ? 8 : 4;
+    if (B > 0) NK_CUDA(cudaMemcpyAsync(s.sigma, sigma_host, (size_t)B * N, cudaMemcpyHostToDevice, st));
+    NK_CUDA(cudaMemcpyAsync(s.W, W_host, (size_t)M * N * esz, cudaMemcpyHostToDevice, st));
+    if (a_host) NK_CUDA(cudaMemcpyAsync(s.a, a_host, (size_t)N * esz, cudaMemcpyHostToDevice, st));
+    if (b_host) NK_CUDA(cudaMemcpyAsync(s.b, b_host, (size_t)M * esz, cudaMemcpyHostToDevice, st));
+    const int rc = nk_local_energy(h, s.sigma, B, N, M, dtype, s.W, a_host ? s.a : nullptr, b_host ? s.b : nullptr,
+                                   chunk_size, s.eloc, logpsi_host ? s.logpsi : nullptr, stats_host ? s.stats : nullptr,
+                                   s.ws, s.ws_bytes, stream);
+    if (rc != NK_OK) return rc;
+    if (B > 0) NK_CUDA(cudaMemcpyAsync(eloc_host, s.eloc, (size_t)B * esz, cudaMemcpyDeviceToHost, st));
+    if (B > 0 && logpsi_host) NK_CUDA(cudaMemcpyAsync(logpsi_host, s.logpsi, (size_t)B * esz, cudaMemcpyDeviceToHost, st));
+    if (stats_host) NK_CUDA(cudaMemcpyAsync(stats_host, s.stats, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    NK_CUDA(cudaStreamSynchronize(st));
+    return NK_OK;
+}
+
+}  // extern "C"

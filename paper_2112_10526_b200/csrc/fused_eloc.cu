@@ -1,0 +1,350 @@
+// Fused incremental local-energy kernel (SURVEY.md §8 a1 + a4): for every sample, enumerate the connected
+// configurations from the device bond table (never materialising sigma'), update theta by one row of the
+// bond-difference table, and accumulate  E_loc(s) = H_ss + sum_s' H_ss' psi(s')/psi(s)   (Eq. (12)).
+//
+// Mapping: one warp owns one sample; lane l holds hidden units {128 v + 4 l + c : v < V, c < 4} of theta in
+// registers.  A CTA = FW consumer warps + 1 producer warp.  The producer streams tiles of the table Dtab through a
+// shared-memory ring with 1-D bulk async copies (TMA engine) and mbarriers; every consumer warp walks the same
+// tiles, tests its own sample's bonds (ballot), and for each active row does, per hidden unit,
+//      theta_s' = theta_s + s D                      (theta_s = 2 log2(e) theta, s = -sigma_i)
+//      e'  = 2^(-|theta_s'|) = exp(-2|theta'|)       (1 MUFU)
+//      P  *= (1 + e')                                (FMA)
+//      acc += |theta_s'| - |theta_s|                 (per-term difference: no cancellation of O(100) sums)
+// which is the stable form ln cosh x = |x| + ln(1 + e^{-2|x|}) - ln 2 with the logarithm hoisted out of the sum
+// over hidden units (sum_j ln(1+e_j) = ln prod_j (1+e_j)) and cancelled against the final exp:
+//      psi'/psi = 2^(acc/2 + s a2) * prod_j (1+e'_j) / prod_j (1+e_j).
+// Complex parameters: cosh(x+iy) = (e^{|x|}/2) [(1+e) cos u + i (1-e) sin u], u = sign(x) y, and the product runs
+// over complex factors.
+#include <type_traits>
+
+#include "nk_internal.h"
+#include "ptx_helpers.cuh"
+
+namespace nk {
+
+constexpr int FW = 15;                       // consumer warps (samples in flight) per CTA; +1 producer = 512 threads
+constexpr int FTHREADS = (FW + 1) * 32;
+
+struct FusedParams {
+    const int8_t* sigma;
+    int64_t B;
+    int N, N_pad;
+    const float* theta;
+    int M_pad, M_eff;
+    const float* Dtab;
+    const RowInfo* rows;
+    int n_rows, tile_rows, n_tiles, stages;
+    const int32_t* bonds;
+    const int32_t* colors;
+    const float* Jf;
+    int n_bonds, kind;
+    float* eloc;
+};
+
+__device__ __forceinline__ float warp_sum_f(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ float warp_prod_f(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v *= __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// ---- per-row inner loops ---------------------------------------------------------------------------------
+template <int V>
+struct RealState {
+    float4 th[V];      // theta_s
+    float qinv;        // 1 / prod_{j in lane} (1 + e_j)
+
+    __device__ __forceinline__ void load(const float* __restrict__ row, int lane, int /*M_pad*/) {
+        float p0 = 1.f, p1 = 1.f, p2 = 1.f, p3 = 1.f;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            float4 t = *reinterpret_cast<const float4*>(row + (v * 32 + lane) * 4);
+            t.x *= KAPPA; t.y *= KAPPA; t.z *= KAPPA; t.w *= KAPPA;
+            th[v] = t;
+            p0 = fmaf(p0, ex2_approx(-fabsf(t.x)), p0);
+            p1 = fmaf(p1, ex2_approx(-fabsf(t.y)), p1);
+            p2 = fmaf(p2, ex2_approx(-fabsf(t.z)), p2);
+            p3 = fmaf(p3, ex2_approx(-fabsf(t.w)), p3);
+        }
+        qinv = 1.f / ((p0 * p1) * (p2 * p3));
+    }
+    // returns psi'/psi without the visible-bias factor, identical on all lanes
+    __device__ __forceinline__ float ratio(const float* __restrict__ drow, int lane, float s, float a2) const {
+        float p0 = 1.f, p1 = 1.f, p2 = 1.f, p3 = 1.f, acc0 = 0.f, acc1 = 0.f;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            const float4 d = *reinterpret_cast<const float4*>(drow + (v * 32 + lane) * 4);
+            const float4 t = th[v];
+            const float x0 = fmaf(s, d.x, t.x), x1 = fmaf(s, d.y, t.y);
+            const float x2 = fmaf(s, d.z, t.z), x3 = fmaf(s, d.w, t.w);
+            p0 = fmaf(p0, ex2_approx(-fabsf(x0)), p0);
+            p1 = fmaf(p1, ex2_approx(-fabsf(x1)), p1);
+            p2 = fmaf(p2, ex2_approx(-fabsf(x2)), p2);
+            p3 = fmaf(p3, ex2_approx(-fabsf(x3)), p3);
+            acc0 += fabsf(x0) - fabsf(t.x);
+            acc1 += fabsf(x1) - fabsf(t.y);
+            acc0 += fabsf(x2) - fabsf(t.z);
+            acc1 += fabsf(x3) - fabsf(t.w);
+        }
+        float r = ((p0 * p1) * (p2 * p3)) * qinv;
+        float acc = acc0 + acc1;
+        r = warp_prod_f(r);
+        acc = warp_sum_f(acc);
+        return r * ex2_approx(fmaf(0.5f, acc, s * a2));
+    }
+};
+
+template <int V>
+struct CplxState {
+    float4 tx[V], ty[V];   // Re theta_s (scaled), Im theta (radians)
+    float qr, qi;          // 1 / prod_{j in lane} f_j
+
+    static __device__ __forceinline__ void factor(float x, float y, float& p, float& q) {
+        const float e = ex2_approx(-fabsf(x));
+        float sn, cs;
+        __sincosf(y, &sn, &cs);
+        p = fmaf(e, cs, cs);                      // (1+e) cos y
+        q = fmaf(-e, sn, sn);                     // (1-e) sin y
+        q = __int_as_float(__float_as_int(q) ^ (__float_as_int(x) & 0x80000000));   // times sign(x)
+    }
+    static __device__ __forceinline__ void cmul(float& ar, float& ai, float br, float bi) {
+        const float r = fmaf(ar, br, -ai * bi), i = fmaf(ar, bi, ai * br);
+        ar = r; ai = i;
+    }
+    __device__ __forceinline__ void load(const float* __restrict__ row, int lane, int M_pad) {
+        float ar = 1.f, ai = 0.f, br = 1.f, bi = 0.f;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            float4 x = *reinterpret_cast<const float4*>(row + (v * 32 + lane) * 4);
+            const float4 y = *reinterpret_cast<const float4*>(row + M_pad + (v * 32 + lane) * 4);
+            x.x *= KAPPA; x.y *= KAPPA; x.z *= KAPPA; x.w *= KAPPA;
+            tx[v] = x; ty[v] = y;
+            float p, q;
+            factor(x.x, y.x, p, q); cmul(ar, ai, p, q);
+            factor(x.y, y.y, p, q); cmul(br, bi, p, q);
+            factor(x.z, y.z, p, q); cmul(ar, ai, p, q);
+            factor(x.w, y.w, p, q); cmul(br, bi, p, q);
+        }
+        cmul(ar, ai, br, bi);
+        const float inv = 1.f / fmaf(ar, ar, ai * ai);
+        qr = ar * inv; qi = -ai * inv;
+    }
+    __device__ __forceinline__ void ratio(const float* __restrict__ drow, int lane, int M_pad, float s, float a2re,
+                                          float a2im, float& out_re, float& out_im) const {
+        float ar = 1.f, ai = 0.f, br = 1.f, bi = 0.f, acc = 0.f;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            const float4 dx = *reinterpret_cast<const float4*>(drow + (v * 32 + lane) * 4);
+            const float4 dy = *reinterpret_cast<const float4*>(drow + M_pad + (v * 32 + lane) * 4);
+            const float4 x = tx[v], y = ty[v];
+            float p, q;
+            const float x0 = fmaf(s, dx.x, x.x), x1 = fmaf(s, dx.y, x.y);
+            const float x2 = fmaf(s, dx.z, x.z), x3 = fmaf(s, dx.w, x.w);
+            factor(x0, fmaf(s, dy.x, y.x), p, q); cmul(ar, ai, p, q);
+            factor(x1, fmaf(s, dy.y, y.y), p, q); cmul(br, bi, p, q);
+            factor(x2, fmaf(s, dy.z, y.z), p, q); cmul(ar, ai, p, q);
+            factor(x3, fmaf(s, dy.w, y.w), p, q); cmul(br, bi, p, q);
+            acc += (fabsf(x0) - fabsf(x.x)) + (fabsf(x1) - fabsf(x.y));
+            acc += (fabsf(x2) - fabsf(x.z)) + (fabsf(x3) - fabsf(x.w));
+        }
+        cmul(ar, ai, br, bi);
+        cmul(ar, ai, qr, qi);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const float orr = __shfl_xor_sync(0xffffffffu, ar, o), oi = __shfl_xor_sync(0xffffffffu, ai, o);
+            cmul(ar, ai, orr, oi);
+            acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        }
+        const float mag = ex2_approx(fmaf(0.5f, acc, s * a2re));
+        float sn, cs;
+        __sincosf(s * a2im, &sn, &cs);
+        cmul(ar, ai, mag * cs, mag * sn);
+        out_re = ar; out_im = ai;
+    }
+};
+
+// ---- kernel ----------------------------------------------------------------------------------------------
+template <int V, bool CPLX, int MINB>
+__global__ void __launch_bounds__(FTHREADS, MINB) fused_eloc_kernel(const FusedParams p) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t stage_bytes = (uint32_t)p.tile_rows * p.M_eff * 4u;
+    float* ring = reinterpret_cast<float*>(smem);
+    int8_t* sig_all = reinterpret_cast<int8_t*>(smem + (size_t)p.stages * stage_bytes);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sig_all + (size_t)FW * p.N_pad);   // full[stages], empty[stages]
+    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + p.stages);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < p.stages; ++s) {
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, FW);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const int64_t n_groups = (p.B + FW - 1) / FW;
+    const int64_t my_groups = (n_groups > blockIdx.x) ? (n_groups - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    const int64_t total_tiles = my_groups * p.n_tiles;
+
+    if (warp == FW) {
+        // ===== producer: one lane streams Dtab tiles round-robin, tile index = g mod n_tiles =====
+        if (lane == 0) {
+            int stage = 0, tile = 0;
+            uint32_t parity = 1;                      // first pass over the ring: slots are free
+            for (int64_t g = 0; g < total_tiles; ++g) {
+                mbar_wait(empty0 + 8 * stage, parity);
+                mbar_arrive_expect_tx(full0 + 8 * stage, stage_bytes);
+                bulk_g2s(smem_u32(ring) + stage * stage_bytes, p.Dtab + (size_t)tile * p.tile_rows * p.M_eff,
+                         stage_bytes, full0 + 8 * stage);
+                if (++stage == p.stages) { stage = 0; parity ^= 1; }
+                if (++tile == p.n_tiles) tile = 0;
+            }
+        }
+        return;
+    }
+
+    // ===== consumers =====
+    int8_t* sg = sig_all + warp * p.N_pad;
+    int stage = 0;
+    uint32_t parity = 0;
+    typename std::conditional<CPLX, CplxState<V>, RealState<V>>::type st;
+
+    for (int64_t grp = blockIdx.x; grp < n_groups; grp += gridDim.x) {
+        const int64_t sample = grp * FW + warp;
+        const bool valid = sample < p.B;
+        const int64_t srow = valid ? sample : 0;      // tail warps shadow sample 0 (results discarded)
+        __syncwarp();
+        for (int i = lane; i < p.N; i += 32) sg[i] = p.sigma[srow * p.N + i];
+        st.load(p.theta + srow * p.M_eff, lane, p.M_pad);
+        __syncwarp();
+
+        float diag = 0.f, e_re = 0.f, e_im = 0.f;
+        if (p.kind == NK_ISING) {
+            for (int b = lane; b < p.n_bonds; b += 32) {
+                const int i = p.bonds[2 * b], j = p.bonds[2 * b + 1];
+                diag += p.Jf[p.colors[b]] * (float)(sg[i] * sg[j]);
+            }
+        }
+        for (int t = 0; t < p.n_tiles; ++t) {
+            // enumerate this tile's rows for this sample: lane r <-> row t*tile_rows + r
+            bool active = false;
+            float sgn = 0.f, coef = 0.f, a2re = 0.f, a2im = 0.f;
+            if (lane < p.tile_rows) {
+                const RowInfo ri = p.rows[t * p.tile_rows + lane];
+                if (ri.i >= 0) {
+                    const int si = sg[ri.i];
+                    const int sj = (ri.j >= 0) ? (int)sg[ri.j] : -si;
+                    active = valid && (si != sj);
+                    diag += ri.jdiag * (float)(si * sj);
+                    sgn = (float)(-si); coef = ri.coef; a2re = ri.a2_re; a2im = ri.a2_im;
+                }
+            }
+            unsigned mask = __ballot_sync(0xffffffffu, active);
+            mbar_wait(full0 + 8 * stage, parity);
+            const float* tile = ring + (size_t)stage * (stage_bytes / 4);
+            while (mask) {
+                const int r = __ffs(mask) - 1;
+                mask &= mask - 1;
+                const float s = __shfl_sync(0xffffffffu, sgn, r);
+                const float c = __shfl_sync(0xffffffffu, coef, r);
+                const float ar = __shfl_sync(0xffffffffu, a2re, r);
+                if constexpr (!CPLX) {
+                    e_re = fmaf(c, st.ratio(tile + (size_t)r * p.M_eff, lane, s, ar), e_re);
+                } else {
+                    const float ai = __shfl_sync(0xffffffffu, a2im, r);
+                    float rr, rim;
+                    st.ratio(tile + (size_t)r * p.M_eff, lane, p.M_pad, s, ar, ai, rr, rim);
+                    e_re = fmaf(c, rr, e_re);
+                    e_im = fmaf(c, rim, e_im);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+            if (++stage == p.stages) { stage = 0; parity ^= 1; }
+        }
+        diag = warp_sum_f(diag);
+        if (valid && lane == 0) {
+            if constexpr (!CPLX) p.eloc[sample] = diag + e_re;
+            else { p.eloc[2 * sample] = diag + e_re; p.eloc[2 * sample + 1] = e_im; }
+        }
+    }
+}
+
+// ---- dispatch ----------------------------------------------------------------------------------------------
+using KernelFn = void (*)(const FusedParams);
+
+template <int V, bool CPLX>
+constexpr int min_blocks() { return ((CPLX ? 8 : 4) * V <= 16) ? 2 : 1; }
+
+template <int V>
+static KernelFn pick_real(int v) {
+    if (v == V) return fused_eloc_kernel<V, false, min_blocks<V, false>()>;
+    if constexpr (V < MAX_V_REAL) return pick_real<V + 1>(v);
+    return nullptr;
+}
+template <int V>
+static KernelFn pick_cplx(int v) {
+    if (v == V) return fused_eloc_kernel<V, true, min_blocks<V, true>()>;
+    if constexpr (V < MAX_V_CPLX) return pick_cplx<V + 1>(v);
+    return nullptr;
+}
+
+static int g_num_sms = 0;
+static bool g_attr_done = false;
+
+cudaError_t fused_eloc_init() {
+    if (g_attr_done) return cudaSuccess;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    for (int v = 1; v <= MAX_V_REAL; ++v) {
+        e = cudaFuncSetAttribute((const void*)pick_real<1>(v), cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+    }
+    for (int v = 1; v <= MAX_V_CPLX; ++v) {
+        e = cudaFuncSetAttribute((const void*)pick_cplx<1>(v), cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+    }
+    g_attr_done = true;
+    return cudaSuccess;
+}
+
+int fused_ctas_per_sm(int M_pad, bool cplx) {
+    const int V = M_pad / MPAD_ALIGN;
+    return ((cplx ? 8 : 4) * V <= 16) ? 2 : 1;
+}
+int fused_consumer_warps() { return FW; }
+
+cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
+                              const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,
+                              cudaStream_t st) {
+    if (B <= 0) return cudaSuccess;
+    cudaError_t e = fused_eloc_init();
+    if (e != cudaSuccess) return e;
+    const bool cplx = dtype == NK_C64;
+    const int V = g.M_pad / MPAD_ALIGN;
+    KernelFn fn = cplx ? pick_cplx<1>(V) : pick_real<1>(V);
+    if (fn == nullptr) return cudaErrorInvalidValue;
+    FusedParams p;
+    p.sigma = sigma; p.B = B; p.N = g.N; p.N_pad = g.N_pad;
+    p.theta = theta; p.M_pad = g.M_pad; p.M_eff = g.M_eff;
+    p.Dtab = Dtab; p.rows = rows; p.n_rows = g.n_rows; p.tile_rows = g.tile_rows; p.n_tiles = g.n_tiles;
+    p.stages = g.stages;
+    p.bonds = op->d_bonds; p.colors = op->d_colors; p.Jf = op->d_Jf; p.n_bonds = op->n_bonds; p.kind = op->kind;
+    p.eloc = (float*)eloc_out;
+    const int64_t n_groups = (B + FW - 1) / FW;
+    const int64_t max_ctas = (int64_t)g_num_sms * g.ctas_per_sm;
+    const unsigned grid = (unsigned)(n_groups < max_ctas ? n_groups : max_ctas);
+    fn<<<grid, FTHREADS, g.smem_bytes, st>>>(p);
+    count_launch();
+    return cudaGetLastError();
+}
+
+}  // namespace nk

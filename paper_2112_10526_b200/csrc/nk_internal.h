@@ -1,0 +1,81 @@
+// Internal declarations shared by the translation units of libnkb200.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "nkb200.h"
+
+namespace nk {
+
+// theta is kept in the fused kernel as theta_s = KAPPA * theta, so that exp(-2|theta|) = 2^(-|theta_s|)
+// is a bare MUFU.EX2 (no multiply).  KAPPA = 2 log2(e).
+constexpr float KAPPA = 2.8853900817779268f;
+constexpr float LOG2E = 1.4426950408889634f;
+
+constexpr int MPAD_ALIGN = 128;      // hidden units padded to a multiple of 128: one float4 per lane per 128
+constexpr int MAX_V_REAL = 16;       // M_pad <= 2048 (real)
+constexpr int MAX_V_CPLX = 8;        // M_pad <= 1024 (complex, two planes)
+
+// One row of the bond-difference table D: which sites it touches and the scalar data the fused kernel needs.
+struct __align__(32) RowInfo {
+    int32_t i;        // site whose spin gives the sign (s = -sigma_i)
+    int32_t j;        // exchange partner, or -1 for a single flip / padded row
+    float coef;       // matrix element of the connected configuration (+-2 J_c, or -h)
+    float jdiag;      // Heisenberg: J_c of the bond (diagonal term J s_i s_j); Ising: 0
+    float a2_re;      // log2(e) * 2 (a_i - a_j)   [or 2 a_i]: exponent contribution of the visible bias
+    float a2_im;      // complex: 2 Im(a_i - a_j) in radians; real: 0
+    int32_t pad0, pad1;
+};
+
+struct Operator {
+    int kind, n_sites, n_bonds, n_colors;
+    unsigned flags;
+    double h;
+    int32_t* d_bonds;    // [n_bonds][2]
+    int32_t* d_colors;   // [n_bonds]
+    float* d_Jf;         // [n_colors]
+    double* d_Jd;        // [n_colors]
+};
+
+inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+inline size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
+
+// Geometry derived from (op, N, M, dtype).
+struct Geometry {
+    int N, N_pad, M, M_pad, M_eff, planes;   // M_eff = planes * M_pad; N_pad = N rounded up to 16
+    int n_rows, tile_rows, n_tiles, n_rows_pad;
+    int stages, ctas_per_sm;                 // shared-memory ring plan of the fused kernel
+    size_t smem_bytes;
+    bool ok;                                 // false: sizes beyond what this version supports
+};
+int fused_ctas_per_sm(int M_pad, bool cplx);
+int fused_consumer_warps();
+Geometry make_geometry(const Operator* op, int N, int M, int dtype);
+
+// ---- launchers (each returns cudaGetLastError() of its launches) -----------------------------------------
+// pack.cu
+cudaError_t launch_pack(const Operator* op, const Geometry& g, int dtype, const void* W, const void* a, const void* b,
+                        float* Wg, float* bg, float* Wt, float* Dtab, RowInfo* rows, cudaStream_t st);
+cudaError_t launch_pack_gemm_only(const Geometry& g, int dtype, const void* W, const void* b, float* Wg, float* bg,
+                                  cudaStream_t st);
+// theta_gemm.cu : theta[s][m] = bg[m] + sum_k sigma[s][k] Wg[m][k]
+cudaError_t launch_theta_gemm(const int8_t* sigma, int64_t B, int N, int M_eff, const float* Wg, const float* bg,
+                              float* theta, cudaStream_t st);
+// logpsi.cu
+cudaError_t launch_logpsi(const int8_t* sigma, int64_t B, const Geometry& g, int dtype, const float* theta,
+                          const void* a, void* logpsi_out, bool out_f64, void* theta_out, cudaStream_t st);
+// connected.cu
+cudaError_t launch_connected(const Operator* op, const int8_t* sigma, int64_t B, int32_t* flips, float* mels,
+                             int32_t* n_conn, int8_t* sigma_prime, cudaStream_t st);
+// fused_eloc.cu
+cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
+                              const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,
+                              cudaStream_t st);
+cudaError_t fused_eloc_init();   // one-time cudaFuncSetAttribute calls
+// stats.cu
+cudaError_t launch_stats(const void* eloc, int64_t B, int dtype, double* stats_out, cudaStream_t st);
+
+void count_launch(int n = 1);
+
+}  // namespace nk

@@ -1,0 +1,249 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by element, on the same
+seeded inputs.  Tolerances (BASELINE.json north_star; Q13):
+    connected lists      bit-exact
+    ln psi               |gpu - oracle| <= 1e-5 (fp32 output; Im compared modulo 2 pi)
+    E_loc                |gpu - oracle| <= 1e-4 |oracle| + 1e-6
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import nk_oracle as orc
+from paper_2112_10526_b200 import inputs as inp
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+LOGPSI_ATOL = 1e-5
+ELOC_RTOL, ELOC_ATOL = 1e-4, 1e-6
+
+
+def dev(x):
+    return None if x is None else torch.from_numpy(np.ascontiguousarray(x)).to(DEV)
+
+
+def run_gpu(nk, p, chunk=None, flags=0, a=True, b=True):
+    op = nk.Operator.from_problem(p, flags)
+    e, lp, st = nk.local_energy(op, dev(p.sigma), dev(p.W), dev(p.a) if a else None, dev(p.b) if b else None,
+                                chunk_size=p.chunk_size if chunk is None else chunk)
+    torch.cuda.synchronize()
+    out = e.cpu().numpy(), lp.cpu().numpy(), st.cpu().numpy()
+    op.close()
+    return out
+
+
+def run_oracle(p, rows=None, flags=0, a=True, b=True):
+    sig = p.sigma if rows is None else p.sigma[rows]
+    return orc.local_energy(p.kind, sig, p.bonds, p.colors, p.J, p.h, p.W, p.a if a else None, p.b if b else None,
+                            flags)
+
+
+def assert_eloc(e_gpu, e_ref):
+    e_gpu = np.asarray(e_gpu).astype(np.complex128)
+    e_ref = np.asarray(e_ref).astype(np.complex128)
+    err = np.abs(e_gpu - e_ref)
+    tol = ELOC_RTOL * np.abs(e_ref) + ELOC_ATOL
+    assert np.all(np.isfinite(e_gpu.view(np.float64)))
+    worst = int(np.argmax(err - tol))
+    assert np.all(err <= tol), f"E_loc mismatch at {worst}: gpu {e_gpu[worst]} oracle {e_ref[worst]}"
+    return float(np.max(err / (np.abs(e_ref) + 1e-30)))
+
+
+def assert_logpsi(lp_gpu, lp_ref, atol=LOGPSI_ATOL):
+    lp_gpu = np.asarray(lp_gpu).astype(np.complex128)
+    lp_ref = np.asarray(lp_ref).astype(np.complex128)
+    dre = np.abs(lp_gpu.real - lp_ref.real)
+    dim = np.abs((lp_gpu.imag - lp_ref.imag + np.pi) % (2 * np.pi) - np.pi)
+    assert dre.max() <= atol, f"Re ln psi err {dre.max()}"
+    assert dim.max() <= atol, f"Im ln psi err {dim.max()} (mod 2 pi)"
+    return float(max(dre.max(), dim.max()))
+
+
+# ------------------------------------------------------------------ nk_connected: bit-exact
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (2, 96), (3, 24), (4, 64), (5, 6)])
+def test_connected_bit_exact(nk, cfg, n):
+    p = inp.make_config(cfg, n_samples=n)
+    op = nk.Operator.from_problem(p)
+    flips, mels, n_conn, sp = nk.connected(op, dev(p.sigma), materialize=True)
+    torch.cuda.synchronize()
+    flips, mels, n_conn, sp = (t.cpu().numpy() for t in (flips, mels, n_conn, sp))
+    assert flips.shape == (n, p.max_conn, 2) and sp.shape == (n, p.max_conn, p.n_sites)
+    for s in range(n):
+        sp_r, mels_r, flips_r, nc_r = orc.connected(p.kind, p.sigma[s], p.bonds, p.colors, p.J, p.h)
+        assert np.array_equal(sp[s], sp_r), f"sigma' differs for sample {s}"
+        assert np.array_equal(flips[s], flips_r)
+        assert np.array_equal(mels[s], mels_r.astype(np.float32))
+        assert n_conn[s] == nc_r
+    op.close()
+
+
+def test_connected_marshall_and_coloured_couplings(nk):
+    p = inp.make_problem(inp.KIND_HEISENBERG, "square", 4, 8, 37, seed=21, order=2, J=(0.75, -1.25))
+    op = nk.Operator.from_problem(p, flags=nk.NK_FLAG_MARSHALL)
+    flips, mels, n_conn, sp = nk.connected(op, dev(p.sigma), materialize=False)
+    torch.cuda.synchronize()
+    assert sp is None
+    for s in range(37):
+        _, mels_r, flips_r, nc_r = orc.connected(p.kind, p.sigma[s], p.bonds, p.colors, p.J, p.h, orc.FLAG_MARSHALL)
+        assert np.array_equal(flips[s].cpu().numpy(), flips_r)
+        assert np.array_equal(mels[s].cpu().numpy(), mels_r.astype(np.float32))
+        assert int(n_conn[s]) == nc_r
+
+
+# ------------------------------------------------------------------ nk_rbm_logpsi
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (2, 1024), (3, 512), (4, 1024), (5, 384)])
+def test_logpsi_parity(nk, cfg, n):
+    p = inp.make_config(cfg, n_samples=n)
+    ref = orc.rbm_logpsi(p.sigma, p.W, p.a, p.b)
+    lp32, theta = nk.rbm_logpsi(dev(p.sigma), dev(p.W), dev(p.a), dev(p.b), return_theta=True)
+    lp64 = nk.rbm_logpsi(dev(p.sigma), dev(p.W), dev(p.a), dev(p.b), out_f64=True)
+    torch.cuda.synchronize()
+    e32 = assert_logpsi(lp32.cpu().numpy(), ref)
+    e64 = assert_logpsi(lp64.cpu().numpy(), ref)
+    th_ref = orc.rbm_theta(p.sigma, p.W, p.b)
+    th_err = np.abs(theta.cpu().numpy().astype(th_ref.dtype) - th_ref).max()
+    assert th_err < 2e-6, th_err
+    print(f"cfg{cfg}: ln psi err fp32-out {e32:.2e}, f64-out {e64:.2e}, theta err {th_err:.2e}, |ln psi| max "
+          f"{np.abs(ref).max():.1f}")
+
+
+def test_logpsi_without_biases_and_tiny_shapes(nk):
+    for (N, M, B, cplx) in [(3, 1, 1, False), (5, 7, 33, True), (17, 130, 9, False), (6, 129, 40, True)]:
+        rng = np.random.default_rng(N * 100 + M)
+        W, a, b = inp.draw_params(rng, N, M, 0.5, cplx)
+        sigma = inp.draw_samples(rng, B, N, False)
+        lp = nk.rbm_logpsi(dev(sigma), dev(W), None, None, out_f64=True)
+        torch.cuda.synchronize()
+        assert_logpsi(lp.cpu().numpy(), orc.rbm_logpsi(sigma, W, None, None), atol=2e-6)
+        lp = nk.rbm_logpsi(dev(sigma), dev(W), dev(a), None)
+        assert_logpsi(lp.cpu().numpy(), orc.rbm_logpsi(sigma, W, a, None))
+
+
+# ------------------------------------------------------------------ nk_local_energy: element-by-element
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (2, 512), (3, 96), (4, 160), (5, 47)])
+def test_local_energy_parity(nk, cfg, n):
+    p = inp.make_config(cfg, n_samples=n)
+    e, lp, st = run_gpu(nk, p, chunk=0)
+    e_ref, lp_ref = run_oracle(p)
+    worst = assert_eloc(e, e_ref)
+    lerr = assert_logpsi(lp, lp_ref)
+    m = orc.stats(e_ref)
+    assert abs(st[0] - m[0]) <= 1e-4 * abs(m[0]) + 1e-6 and abs(st[1] - m[1]) <= 1e-4 * abs(m[0]) + 1e-6
+    assert abs(st[2] - m[2]) <= 1e-3 * m[2] + 1e-9 and st[3] == n
+    # the statistics are exactly those of the returned E_loc (fp64 reduction)
+    np.testing.assert_allclose(st[:3], orc.stats(e.astype(np.complex128))[:3], rtol=1e-12, atol=1e-12)
+    print(f"cfg{cfg}: max rel err E_loc {worst:.2e}, ln psi {lerr:.2e}")
+
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_launch_configuration_sampled(nk, cfg):
+    """BASELINE.json's full batch in the launch configuration bench.py times (config 5: 16 chunks of 4096);
+    the oracle checks a fixed sample of outputs (first and last rows of several chunks)."""
+    p = inp.make_config(cfg)
+    e, lp, st = run_gpu(nk, p)
+    B = p.n_samples
+    chunk = p.chunk_size or B
+    rows = sorted({c * chunk + o for c in range(0, B // chunk, max(1, B // chunk // 4)) for o in (0, chunk - 1)}
+                  | {B - 1, B // 2 + 1})
+    if cfg != 5:
+        rows = sorted(set(rows) | set(range(17, B, B // 24)))
+    e_ref, lp_ref = run_oracle(p, rows)
+    assert_eloc(e[rows], e_ref)
+    assert_logpsi(lp[rows], lp_ref)
+    assert np.all(np.isfinite(e.view(np.float32))) and st[3] == B
+    np.testing.assert_allclose(st[:3], orc.stats(e.astype(np.complex128))[:3], rtol=1e-11, atol=1e-11)
+    # property that holds at any size: uniform psi => E_loc = sum_c J_c n_{b,c} (Heisenberg) / diag - h N (Ising)
+    q = inp.make_config(cfg)
+    q.W = np.zeros_like(q.W); q.a = np.zeros_like(q.a)
+    e0, _, _ = run_gpu(nk, q)
+    if q.kind == inp.KIND_HEISENBERG:
+        expect = float(sum(q.J[c] for c in q.colors))
+        np.testing.assert_allclose(e0.real, expect, rtol=2e-6)
+    else:
+        s = q.sigma.astype(np.float64)
+        diag = (s[:, q.bonds[:, 0]] * s[:, q.bonds[:, 1]]).sum(axis=1) * q.J[0]
+        np.testing.assert_allclose(e0, diag - q.h * q.n_sites, rtol=2e-6, atol=1e-3)
+    if q.complex_params:
+        assert np.abs(e0.imag).max() < 1e-3
+
+
+def test_chunking_does_not_change_results(nk):
+    p = inp.make_config(2, n_samples=1000)
+    ref, lref, sref = run_gpu(nk, p, chunk=0)
+    for chunk in (1000, 512, 333, 15, 1, 4096):
+        e, lp, st = run_gpu(nk, p, chunk=chunk)
+        assert np.array_equal(e, ref) and np.array_equal(lp, lref), f"chunk {chunk}"
+        assert np.array_equal(st, sref)
+
+
+# ------------------------------------------------------------------ edge and degenerate cases
+@pytest.mark.parametrize("case", [
+    dict(kind=0, lattice="chain", L=4, M=1, B=1),                      # smallest everything
+    dict(kind=0, lattice="chain", L=6, M=3, B=16, sz0=False),          # outside the S^z=0 sector, incl. all-up rows
+    dict(kind=1, lattice="chain", L=7, M=5, B=31, h=0.8),              # odd N, Ising, ragged batch
+    dict(kind=1, lattice="square", L=3, M=130, B=29, h=3.0),           # M just above one 128-block
+    dict(kind=0, lattice="square", L=4, M=257, B=77, order=2, J=(1.0, 0.5)),
+    dict(kind=0, lattice="square", L=4, M=40, B=45, order=2, J=(0.3, -0.7), complex_params=True),
+    dict(kind=1, lattice="square", L=4, M=129, B=20, h=1.1, complex_params=True),
+    dict(kind=1, lattice="chain", L=5, M=4, B=8, h=0.0),               # no off-diagonal element at all
+    dict(kind=0, lattice="square", L=6, M=640, B=33),                  # V = 5: one CTA per SM variant
+    dict(kind=0, lattice="square", L=6, M=300, B=33, complex_params=True),
+])
+def test_edge_cases(nk, case):
+    case = dict(case)
+    p = inp.make_problem(case.pop("kind"), case.pop("lattice"), case.pop("L"), case.pop("M"), case.pop("B"),
+                         seed=33, scale=0.2, **case)
+    if p.name.startswith("chain6"):
+        p.sigma[0] = 1; p.sigma[1] = -1                                # fully polarised rows: no active bond
+    e, lp, _ = run_gpu(nk, p)
+    e_ref, lp_ref = run_oracle(p)
+    assert_eloc(e, e_ref)
+    assert_logpsi(lp, lp_ref)
+
+
+def test_null_biases_marshall_flag_and_empty_batch(nk):
+    p = inp.make_problem(inp.KIND_HEISENBERG, "square", 4, 24, 50, seed=5, scale=0.3)
+    e, lp, _ = run_gpu(nk, p, a=False, b=False)
+    e_ref, lp_ref = run_oracle(p, a=False, b=False)
+    assert_eloc(e, e_ref); assert_logpsi(lp, lp_ref)
+    e, _, _ = run_gpu(nk, p, flags=nk.NK_FLAG_MARSHALL)
+    assert_eloc(e, run_oracle(p, flags=orc.FLAG_MARSHALL)[0])
+    op = nk.Operator.from_problem(p)
+    empty = torch.empty((0, p.n_sites), dtype=torch.int8, device=DEV)
+    e, lp, st = nk.local_energy(op, empty, dev(p.W), dev(p.a), dev(p.b))
+    torch.cuda.synchronize()
+    assert e.numel() == 0 and st.cpu().tolist() == [0.0, 0.0, 0.0, 0.0]
+
+
+def test_larger_parameters_stress(nk):
+    """Trained states have larger |theta| (Q17): parameters x10, ratios spanning orders of magnitude."""
+    p = inp.make_config(2, n_samples=200)
+    p.W = (p.W * 10).astype(np.float32); p.a = (p.a * 10).astype(np.float32); p.b = (p.b * 10).astype(np.float32)
+    e, lp, _ = run_gpu(nk, p)
+    e_ref, lp_ref = run_oracle(p)
+    assert_eloc(e, e_ref)
+    assert_logpsi(lp, lp_ref, atol=5e-5)     # |ln psi| ~ 300 here: fp32 output ulp is 3e-5
+
+
+def test_host_entry_point_matches_device_entry_point(nk):
+    p = inp.make_config(4, n_samples=300)
+    e_d, lp_d, st_d = run_gpu(nk, p, chunk=128)
+    op = nk.Operator.from_problem(p)
+    e_h, lp_h, st_h = nk.local_energy_host(op, p.sigma, p.W, p.a, p.b, chunk_size=128)
+    assert np.array_equal(e_h, e_d) and np.array_equal(lp_h, lp_d) and np.array_equal(st_h, st_d)
+
+
+def test_errors_are_loud(nk):
+    p = inp.make_problem(inp.KIND_HEISENBERG, "chain", 6, 4, 4, seed=1)
+    op = nk.Operator.from_problem(p)
+    with pytest.raises(nk.NkError, match="INVALID_ARG"):                 # N does not match the operator
+        nk.local_energy(op, dev(np.ones((4, 8), np.int8)), dev(np.zeros((4, 8), np.float32)))
+    big = inp.draw_params(np.random.default_rng(0), 6, 2049, 0.1, False)
+    with pytest.raises(nk.NkError):                                      # M beyond the supported width
+        nk.local_energy(op, dev(p.sigma), dev(big[0]), None, None)
+    lib = nk.load()
+    ws = torch.empty(1024, dtype=torch.uint8, device=DEV)
+    out = torch.empty(4, dtype=torch.float32, device=DEV)
+    rc = lib.nk_local_energy(op.handle, dev(p.sigma).data_ptr(), 4, 6, 4, 0, dev(p.W).data_ptr(), None, None, 0,
+                             out.data_ptr(), None, None, ws.data_ptr() + 1, 1023, None)
+    assert rc == -3                                                      # misaligned / short workspace

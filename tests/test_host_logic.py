@@ -1,0 +1,124 @@
+"""CPU-only tests: the C-ABI library loads and exports every symbol the header declares, host-side argument
+checks fail loudly without a GPU, input generators, and the multi-rank statistics combine (gloo, world_size 2)."""
+import ctypes
+import os
+import re
+import socket
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2112_10526_b200 as nk
+from oracle import nk_oracle as orc
+from paper_2112_10526_b200 import inputs as inp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    import __graft_entry__ as ge
+    ge.build()
+    return nk.load()
+
+
+def test_header_and_binding_declare_the_same_symbols(lib):
+    hdr = open(os.path.join(ROOT, "include", "nkb200.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(nk_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(nk.EXPORTS), declared ^ set(nk.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), f"{name} not exported by libnkb200.so"
+
+
+def test_status_strings_and_version(lib):
+    assert lib.nk_status_string(0) == b"NK_OK"
+    for code in (-1, -2, -3, -4, -5):
+        assert lib.nk_status_string(code).startswith(b"NK_ERR_")
+    assert lib.nk_status_string(12345) == b"unknown nk_status"
+    assert lib.nk_version() >= 100
+
+
+def test_argument_errors_are_reported_before_any_launch(lib):
+    h = ctypes.c_void_p()
+    J = np.array([1.0])
+    bonds = np.array([[0, 1], [1, 1]], dtype=np.int32)          # i == j: invalid
+    rc = lib.nk_operator_create(ctypes.byref(h), 0, 4, 2, bonds.ctypes.data, None, 1, J.ctypes.data, 0.0, 0)
+    assert rc == -1 and not h.value
+    bonds = np.array([[0, 7]], dtype=np.int32)                  # out of range
+    assert lib.nk_operator_create(ctypes.byref(h), 0, 4, 1, bonds.ctypes.data, None, 1, J.ctypes.data, 0.0, 0) == -1
+    assert lib.nk_operator_create(ctypes.byref(h), 5, 4, 0, None, None, 1, J.ctypes.data, 0.0, 0) == -1
+    assert lib.nk_rbm_logpsi_workspace_bytes(16, 10, 10, 7) == 0        # bad dtype
+    assert lib.nk_rbm_logpsi_workspace_bytes(16, 10, 10, 0) > 0
+    assert lib.nk_rbm_logpsi(None, 4, 10, 10, 0, None, None, None, None, None, 0, None, 0, None) == -1
+    assert lib.nk_local_energy(None, None, 4, 10, 10, 0, None, None, None, 0, None, None, None, None, 0, None) == -1
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
+def test_no_cpu_fallback_without_a_gpu(lib):
+    b, c = inp.chain_bonds(4)
+    with pytest.raises(nk.NkError, match="NK_ERR_CUDA"):
+        nk.Operator(nk.NK_HEISENBERG, 4, b, c, [1.0])
+
+
+def test_input_generators_match_the_config_table():
+    sizes = {1: (10, 10, 1024, 10), 2: (100, 100, 4096, 200), 4: (100, 400, 16384, 400)}
+    for c, (N, M, B, nb) in sizes.items():
+        p = inp.make_config(c, n_samples=32)
+        assert (p.n_sites, p.n_hidden, len(p.bonds)) == (N, M, nb)
+        assert p.W.shape == (M, N) and p.sigma.shape == (32, N) and p.sigma.dtype == np.int8
+        assert np.all(p.sigma.sum(axis=1) == 0) and set(np.unique(p.sigma)) == {-1, 1}
+        pairs = {(min(i, j), max(i, j)) for i, j in p.bonds}
+        assert len(pairs) == nb                                        # each undirected pair once
+        deg = np.bincount(p.bonds.ravel(), minlength=N)
+        assert np.all(deg == 2 * nb // N)
+    p3 = inp.make_config(3, n_samples=8)
+    assert (p3.n_sites, p3.n_hidden, len(p3.bonds), p3.h, p3.max_conn) == (400, 800, 800, 3.0, 401)
+    p4 = inp.make_config(4, n_samples=8)
+    assert p4.W.dtype == np.complex64 and list(p4.J) == [1.0, 0.5] and np.bincount(p4.colors).tolist() == [200, 200]
+    # same seed -> same arrays; different rank offset -> different samples, same parameters
+    q = inp.make_config(2, n_samples=32)
+    r = inp.make_config(2, n_samples=32, sample_seed_offset=1)
+    assert np.array_equal(q.W, inp.make_config(2, n_samples=4).W) and np.array_equal(q.W, r.W)
+    assert not np.array_equal(q.sigma, r.sigma)
+
+
+def test_combine_stats_equals_stats_of_the_union():
+    rng = np.random.default_rng(0)
+    e = rng.normal(size=1000) + 1j * rng.normal(size=1000)
+    parts = [orc.stats(e[:100]), orc.stats(e[100:650]), orc.stats(e[650:]), (0.0, 0.0, 0.0, 0.0)]
+    np.testing.assert_allclose(nk.combine_stats(parts), orc.stats(e), rtol=1e-12, atol=1e-14)
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    return port
+
+
+def _rank_main(rank, world, port, q):
+    import torch.distributed as dist
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    rng = np.random.default_rng(0)
+    e = rng.normal(size=1000)
+    shard = e[rank::world]                                             # each rank owns a slice of the samples
+    out = nk.allreduce_stats(torch.tensor(orc.stats(shard), dtype=torch.float64))
+    q.put((rank, out.tolist()))
+    dist.destroy_process_group()
+
+
+def test_allreduce_stats_gloo_world_size_2():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_rank_main, args=(r, 2, port, q)) for r in range(2)]
+    [p.start() for p in procs]
+    res = dict(q.get(timeout=120) for _ in procs)
+    [p.join(60) for p in procs]
+    e = np.random.default_rng(0).normal(size=1000)
+    for r in range(2):
+        np.testing.assert_allclose(res[r], orc.stats(e), rtol=1e-12, atol=1e-14)
