@@ -44,33 +44,32 @@ static int cuda_fail(cudaError_t e) {
 Geometry make_geometry(const Operator* op, int N, int M, int dtype) {
     Geometry g{};
     const bool cplx = dtype == NK_C64;
-    g.N = N; g.N_pad = round_up(N, 16);
+    g.N = N; g.n_words = (N + 31) / 32;
     g.M = M; g.M_pad = round_up(M, MPAD_ALIGN);
     g.planes = cplx ? 2 : 1;
     g.M_eff = g.planes * g.M_pad;
     g.n_rows = op ? (op->kind == NK_HEISENBERG ? op->n_bonds : op->n_sites) : 0;
     g.ok = g.M_pad / MPAD_ALIGN <= (cplx ? MAX_V_CPLX : MAX_V_REAL) && N <= 65535 && g.n_rows <= 65535;
     g.ctas_per_sm = fused_ctas_per_sm(g.M_pad, cplx);
-    // shared-memory plan of the fused kernel: [stages x tile][sigma rows][2 x stages mbarriers]
-    const size_t budget = (size_t)(227 * 1024) / g.ctas_per_sm - 1024;
-    const size_t sig = (size_t)fused_consumer_warps() * g.N_pad;
+    // shared-memory plan of the fused kernel: [stages x tile][bit-packed spins][2 x stages mbarriers];
+    // 4 stages, as many rows per stage as fit (<= 32: one ballot bit per row)
+    const size_t budget = (size_t)(227 * 1024) / g.ctas_per_sm - (g.ctas_per_sm > 1 ? 1024 : 0);
+    const size_t sig = ((size_t)fused_consumer_warps() * g.n_words * 4 + 15) & ~size_t(15);
     const size_t row_bytes = (size_t)g.M_eff * 4;
-    if (sig + 2 * row_bytes + 64 > budget) { g.ok = false; g.tile_rows = 1; g.stages = 2; }
+    const size_t fixed = sig + (8 + 4) * 4 + 128;         // spins + barriers + counters + alignment slack
+    if (fixed + 2 * row_bytes > budget) { g.ok = false; g.tile_rows = 1; g.stages = 2; }
     else {
-        size_t target = (budget - sig - 64) / 3;
-        if (target > 64 * 1024) target = 64 * 1024;
-        int tr = (int)(target / row_bytes);
-        if (tr < 1) tr = 1;
+        g.stages = 4;
+        int tr = (int)((budget - fixed) / (g.stages * row_bytes));
+        if (tr < 1) { g.stages = 2; tr = (int)((budget - fixed) / (g.stages * row_bytes)); }
         if (tr > 32) tr = 32;
         g.tile_rows = tr;
-        int stages = (int)((budget - sig - 64) / (tr * row_bytes));
-        if (stages > 4) stages = 4;
-        g.stages = stages;       // >= 2 by the check above (tr = 1) or >= 3 by construction
     }
     g.n_tiles = (g.n_rows + g.tile_rows - 1) / g.tile_rows;
     g.n_rows_pad = g.n_tiles * g.tile_rows;
     if (g.n_rows_pad == 0) g.n_rows_pad = g.tile_rows;   // keep the tables non-empty
-    g.smem_bytes = (size_t)g.stages * g.tile_rows * row_bytes + sig + 2 * 8 * (size_t)g.stages;
+    g.smem_bytes = (size_t)g.stages * g.tile_rows * row_bytes + sig + (8 + 4) * (size_t)g.stages + 16;
+    (void)fixed;
     return g;
 }
 

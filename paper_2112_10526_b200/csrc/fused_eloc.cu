@@ -3,9 +3,13 @@
 // bond-difference table, and accumulate  E_loc(s) = H_ss + sum_s' H_ss' psi(s')/psi(s)   (Eq. (12)).
 //
 // Mapping: one warp owns one sample; lane l holds hidden units {128 v + 4 l + c : v < V, c < 4} of theta in
-// registers.  A CTA = FW consumer warps + 1 producer warp.  The producer streams tiles of the table Dtab through a
-// shared-memory ring with 1-D bulk async copies (TMA engine) and mbarriers; every consumer warp walks the same
-// tiles, tests its own sample's bonds (ballot), and for each active row does, per hidden unit,
+// registers.  A CTA = FW = 16 warps (4 per SM sub-partition, so the four MUFU pipes carry equal load; 16 x 32 x
+// 128 registers = the whole register file).  Each CTA owns a contiguous range of samples and works through it in
+// rounds of 16 (the last round may be partial).  Tiles of the table Dtab flow through a shared-memory ring filled
+// by 1-D bulk async copies (TMA engine) that complete on mbarriers; there is no producer warp: the LAST warp to
+// finish a stage (a shared-memory arrival counter) re-arms that stage's barrier and issues the next copy.  Every
+// warp walks the same tiles, tests its own sample's bonds (spins bit-packed in shared memory, one ballot per
+// tile), and for each active row does, per hidden unit,
 //      theta_s' = theta_s + s D                      (theta_s = 2 log2(e) theta, s = -sigma_i)
 //      e'  = 2^(-|theta_s'|) = exp(-2|theta'|)       (1 MUFU)
 //      P  *= (1 + e')                                (FMA)
@@ -22,13 +26,13 @@
 
 namespace nk {
 
-constexpr int FW = 15;                       // consumer warps (samples in flight) per CTA; +1 producer = 512 threads
-constexpr int FTHREADS = (FW + 1) * 32;
+constexpr int FW = 16;                       // warps (samples in flight) per CTA
+constexpr int FTHREADS = FW * 32;
 
 struct FusedParams {
     const int8_t* sigma;
     int64_t B;
-    int N, N_pad;
+    int N, n_words;                          // n_words = ceil(N / 32): bit-packed spins per sample
     const float* theta;
     int M_pad, M_eff;
     const float* Dtab;
@@ -39,6 +43,7 @@ struct FusedParams {
     const float* Jf;
     int n_bonds, kind;
     float* eloc;
+    int64_t per_cta;                         // samples per CTA (contiguous range)
 };
 
 __device__ __forceinline__ float warp_sum_f(float v) {
@@ -168,58 +173,67 @@ struct CplxState {
 };
 
 // ---- kernel ----------------------------------------------------------------------------------------------
-template <int V, bool CPLX, int MINB>
-__global__ void __launch_bounds__(FTHREADS, MINB) fused_eloc_kernel(const FusedParams p) {
+template <int V, bool CPLX>
+constexpr int min_blocks() { return ((CPLX ? 8 : 4) * V <= 16) ? 2 : 1; }
+
+__device__ __forceinline__ void issue_tile(const FusedParams& p, uint32_t ring_u32, uint32_t full0, int stage,
+                                           int tile, uint32_t stage_bytes) {
+    mbar_arrive_expect_tx(full0 + 8 * stage, stage_bytes);
+    bulk_g2s(ring_u32 + stage * stage_bytes, p.Dtab + (size_t)tile * p.tile_rows * p.M_eff, stage_bytes,
+             full0 + 8 * stage);
+}
+
+template <int V, bool CPLX>
+__global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_kernel(const FusedParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t stage_bytes = (uint32_t)p.tile_rows * p.M_eff * 4u;
     float* ring = reinterpret_cast<float*>(smem);
-    int8_t* sig_all = reinterpret_cast<int8_t*>(smem + (size_t)p.stages * stage_bytes);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(sig_all + (size_t)FW * p.N_pad);   // full[stages], empty[stages]
-    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + p.stages);
+    uint32_t* bits_all = reinterpret_cast<uint32_t*>(smem + (size_t)p.stages * stage_bytes);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(bits_all + (size_t)FW * p.n_words);   // full[stages]
+    int* done_cnt = reinterpret_cast<int*>(bars + p.stages);                           // arrivals per stage
+    const uint32_t full0 = smem_u32(bars), ring_u32 = smem_u32(ring);
+
+    // this CTA's contiguous sample range, processed in rounds of FW samples
+    const int64_t first = (int64_t)blockIdx.x * p.per_cta;
+    const int64_t last = (first + p.per_cta < p.B) ? first + p.per_cta : p.B;
+    const int64_t n_rounds = (last > first) ? (last - first + FW - 1) / FW : 0;
+    const int64_t total_tiles = n_rounds * p.n_tiles;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < p.stages; ++s) {
             mbar_init(full0 + 8 * s, 1);
-            mbar_init(empty0 + 8 * s, FW);
+            done_cnt[s] = 0;
         }
         mbar_fence_init();
+        for (int s = 0; s < p.stages && s < total_tiles; ++s)          // prime the ring
+            issue_tile(p, ring_u32, full0, s, s % p.n_tiles, stage_bytes);
     }
     __syncthreads();
 
-    const int64_t n_groups = (p.B + FW - 1) / FW;
-    const int64_t my_groups = (n_groups > blockIdx.x) ? (n_groups - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
-    const int64_t total_tiles = my_groups * p.n_tiles;
-
-    if (warp == FW) {
-        // ===== producer: one lane streams Dtab tiles round-robin, tile index = g mod n_tiles =====
-        if (lane == 0) {
-            int stage = 0, tile = 0;
-            uint32_t parity = 1;                      // first pass over the ring: slots are free
-            for (int64_t g = 0; g < total_tiles; ++g) {
-                mbar_wait(empty0 + 8 * stage, parity);
-                mbar_arrive_expect_tx(full0 + 8 * stage, stage_bytes);
-                bulk_g2s(smem_u32(ring) + stage * stage_bytes, p.Dtab + (size_t)tile * p.tile_rows * p.M_eff,
-                         stage_bytes, full0 + 8 * stage);
-                if (++stage == p.stages) { stage = 0; parity ^= 1; }
-                if (++tile == p.n_tiles) tile = 0;
-            }
-        }
-        return;
-    }
-
     // ===== consumers =====
-    int8_t* sg = sig_all + warp * p.N_pad;
+    uint32_t* bits = bits_all + warp * p.n_words;     // bit i set <=> sigma_i = -1
+    auto spin_bit = [&](int i) -> int { return (int)((bits[i >> 5] >> (i & 31)) & 1u); };
     int stage = 0;
     uint32_t parity = 0;
+    int64_t g = 0;                                    // running tile counter of this CTA
     typename std::conditional<CPLX, CplxState<V>, RealState<V>>::type st;
 
-    for (int64_t grp = blockIdx.x; grp < n_groups; grp += gridDim.x) {
-        const int64_t sample = grp * FW + warp;
-        const bool valid = sample < p.B;
-        const int64_t srow = valid ? sample : 0;      // tail warps shadow sample 0 (results discarded)
+    for (int64_t rnd = 0; rnd < n_rounds; ++rnd) {
+        const int64_t sample = first + rnd * FW + warp;
+        const bool valid = sample < last;
+        const int64_t srow = valid ? sample : first;  // idle warps of a partial round shadow a valid row
         __syncwarp();
-        for (int i = lane; i < p.N; i += 32) sg[i] = p.sigma[srow * p.N + i];
+        {
+            const int8_t* sp = p.sigma + srow * p.N;
+            for (int wi = lane; wi < p.n_words; wi += 32) {
+                uint32_t w = 0;
+                const int base = wi * 32;
+                const int cnt = (p.N - base < 32) ? (p.N - base) : 32;
+                for (int t = 0; t < cnt; ++t) w |= (uint32_t)(sp[base + t] < 0) << t;
+                bits[wi] = w;
+            }
+        }
         st.load(p.theta + srow * p.M_eff, lane, p.M_pad);
         __syncwarp();
 
@@ -227,7 +241,8 @@ __global__ void __launch_bounds__(FTHREADS, MINB) fused_eloc_kernel(const FusedP
         if (p.kind == NK_ISING) {
             for (int b = lane; b < p.n_bonds; b += 32) {
                 const int i = p.bonds[2 * b], j = p.bonds[2 * b + 1];
-                diag += p.Jf[p.colors[b]] * (float)(sg[i] * sg[j]);
+                const float J = p.Jf[p.colors[b]];
+                diag += (spin_bit(i) != spin_bit(j)) ? -J : J;
             }
         }
         for (int t = 0; t < p.n_tiles; ++t) {
@@ -237,11 +252,12 @@ __global__ void __launch_bounds__(FTHREADS, MINB) fused_eloc_kernel(const FusedP
             if (lane < p.tile_rows) {
                 const RowInfo ri = p.rows[t * p.tile_rows + lane];
                 if (ri.i >= 0) {
-                    const int si = sg[ri.i];
-                    const int sj = (ri.j >= 0) ? (int)sg[ri.j] : -si;
-                    active = valid && (si != sj);
-                    diag += ri.jdiag * (float)(si * sj);
-                    sgn = (float)(-si); coef = ri.coef; a2re = ri.a2_re; a2im = ri.a2_im;
+                    const int bi = spin_bit(ri.i);
+                    const int bj = (ri.j >= 0) ? spin_bit(ri.j) : (bi ^ 1);
+                    active = valid && (bi != bj);
+                    diag += (bi != bj) ? -ri.jdiag : ri.jdiag;
+                    sgn = bi ? 1.f : -1.f;            // s = -sigma_i
+                    coef = ri.coef; a2re = ri.a2_re; a2im = ri.a2_im;
                 }
             }
             unsigned mask = __ballot_sync(0xffffffffu, active);
@@ -264,7 +280,19 @@ __global__ void __launch_bounds__(FTHREADS, MINB) fused_eloc_kernel(const FusedP
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+            if (lane == 0) {
+                // release the stage; the last of the FW warps refills it with tile g + stages
+                __threadfence_block();
+                if (atomicAdd(&done_cnt[stage], 1) == FW - 1) {
+                    done_cnt[stage] = 0;
+                    const int64_t g2 = g + p.stages;
+                    if (g2 < total_tiles) {
+                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                        issue_tile(p, ring_u32, full0, stage, (int)(g2 % p.n_tiles), stage_bytes);
+                    }
+                }
+            }
+            ++g;
             if (++stage == p.stages) { stage = 0; parity ^= 1; }
         }
         diag = warp_sum_f(diag);
@@ -278,18 +306,15 @@ __global__ void __launch_bounds__(FTHREADS, MINB) fused_eloc_kernel(const FusedP
 // ---- dispatch ----------------------------------------------------------------------------------------------
 using KernelFn = void (*)(const FusedParams);
 
-template <int V, bool CPLX>
-constexpr int min_blocks() { return ((CPLX ? 8 : 4) * V <= 16) ? 2 : 1; }
-
 template <int V>
 static KernelFn pick_real(int v) {
-    if (v == V) return fused_eloc_kernel<V, false, min_blocks<V, false>()>;
+    if (v == V) return fused_eloc_kernel<V, false>;
     if constexpr (V < MAX_V_REAL) return pick_real<V + 1>(v);
     return nullptr;
 }
 template <int V>
 static KernelFn pick_cplx(int v) {
-    if (v == V) return fused_eloc_kernel<V, true, min_blocks<V, true>()>;
+    if (v == V) return fused_eloc_kernel<V, true>;
     if constexpr (V < MAX_V_CPLX) return pick_cplx<V + 1>(v);
     return nullptr;
 }
@@ -333,16 +358,19 @@ cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, 
     KernelFn fn = cplx ? pick_cplx<1>(V) : pick_real<1>(V);
     if (fn == nullptr) return cudaErrorInvalidValue;
     FusedParams p;
-    p.sigma = sigma; p.B = B; p.N = g.N; p.N_pad = g.N_pad;
+    p.sigma = sigma; p.B = B; p.N = g.N; p.n_words = g.n_words;
     p.theta = theta; p.M_pad = g.M_pad; p.M_eff = g.M_eff;
     p.Dtab = Dtab; p.rows = rows; p.n_rows = g.n_rows; p.tile_rows = g.tile_rows; p.n_tiles = g.n_tiles;
     p.stages = g.stages;
     p.bonds = op->d_bonds; p.colors = op->d_colors; p.Jf = op->d_Jf; p.n_bonds = op->n_bonds; p.kind = op->kind;
     p.eloc = (float*)eloc_out;
-    const int64_t n_groups = (B + FW - 1) / FW;
+    // one CTA per SM slot, each with an equal contiguous share of the samples (rounds of FW inside the CTA);
+    // small batches use fewer CTAs so that every round is full
     const int64_t max_ctas = (int64_t)g_num_sms * g.ctas_per_sm;
-    const unsigned grid = (unsigned)(n_groups < max_ctas ? n_groups : max_ctas);
-    fn<<<grid, FTHREADS, g.smem_bytes, st>>>(p);
+    const int64_t n_groups = (B + FW - 1) / FW;
+    const int64_t grid = n_groups < max_ctas ? n_groups : max_ctas;
+    p.per_cta = (B + grid - 1) / grid;
+    fn<<<(unsigned)grid, FTHREADS, g.smem_bytes, st>>>(p);
     count_launch();
     return cudaGetLastError();
 }

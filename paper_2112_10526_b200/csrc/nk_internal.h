@@ -43,7 +43,7 @@ inline size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
 
 // Geometry derived from (op, N, M, dtype).
 struct Geometry {
-    int N, N_pad, M, M_pad, M_eff, planes;   // M_eff = planes * M_pad; N_pad = N rounded up to 16
+    int N, n_words, M, M_pad, M_eff, planes; // M_eff = planes * M_pad; n_words = ceil(N / 32)
     int n_rows, tile_rows, n_tiles, n_rows_pad;
     int stages, ctas_per_sm;                 // shared-memory ring plan of the fused kernel
     size_t smem_bytes;
