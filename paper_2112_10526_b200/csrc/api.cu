@@ -1,5 +1,6 @@
 // C ABI of libnkb200.so (include/nkb200.h): argument validation, workspace carving, the chunked driver
 // (Sec. 3.3.1: chunk_size bounds the configurations evaluated at once).
+#include <cstdlib>
 #include <new>
 #include <vector>
 
@@ -44,7 +45,7 @@ static int cuda_fail(cudaError_t e) {
 Geometry make_geometry(const Operator* op, int N, int M, int dtype) {
     Geometry g{};
     const bool cplx = dtype == NK_C64;
-    g.N = N; g.n_words = (N + 31) / 32;
+    g.N = N; g.n_words = (N + 31) / 32; g.K_pad = round_up(N, 64);
     g.M = M; g.M_pad = round_up(M, MPAD_ALIGN);
     g.planes = cplx ? 2 : 1;
     g.M_eff = g.planes * g.M_pad;
@@ -88,6 +89,8 @@ struct Carver {
 
 struct LogpsiWs {
     float *Wg, *bg, *theta;
+    uint16_t *Ws, *A;          // bf16 operands of the tensor-core contraction
+    unsigned* absmax;
     size_t bytes;
 };
 static LogpsiWs carve_logpsi(void* ws, const Geometry& g, int64_t rows) {
@@ -96,11 +99,16 @@ static LogpsiWs carve_logpsi(void* ws, const Geometry& g, int64_t rows) {
     w.Wg = c.take<float>((size_t)g.M_eff * g.N);
     w.bg = c.take<float>(g.M_eff);
     w.theta = c.take<float>((size_t)rows * g.M_eff);
+    w.Ws = c.take<uint16_t>((size_t)3 * g.M_eff * g.K_pad);
+    w.A = c.take<uint16_t>((size_t)rows * g.K_pad);
+    w.absmax = c.take<unsigned>(1);
     w.bytes = c.off;
     return w;
 }
 struct ElocWs {
     float *Wg, *bg, *Wt, *Dtab, *theta;
+    uint16_t *Ws, *A;
+    unsigned* absmax;
     RowInfo* rows;
     size_t bytes;
 };
@@ -113,8 +121,22 @@ static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk) {
     w.Dtab = c.take<float>((size_t)g.n_rows_pad * g.M_eff);
     w.rows = c.take<RowInfo>(g.n_rows_pad);
     w.theta = c.take<float>((size_t)chunk * g.M_eff);
+    w.Ws = c.take<uint16_t>((size_t)3 * g.M_eff * g.K_pad);
+    w.A = c.take<uint16_t>((size_t)chunk * g.K_pad);
+    w.absmax = c.take<unsigned>(1);
     w.bytes = c.off;
     return w;
+}
+
+// NK_THETA_SIMT=1 selects the FP32 SIMT contraction (debugging aid); default is the tcgen05 path.
+static bool use_simt_theta() {
+    static const bool v = [] { const char* e = std::getenv("NK_THETA_SIMT"); return e && e[0] == '1'; }();
+    return v;
+}
+static cudaError_t run_theta(const Geometry& g, const int8_t* sg, int64_t nb, const float* Wg, const float* bg,
+                             const uint16_t* Ws, uint16_t* A, float* theta, cudaStream_t st) {
+    if (use_simt_theta()) return launch_theta_gemm(sg, nb, g.N, g.M_eff, Wg, bg, theta, st);
+    return launch_theta_tc(sg, nb, g.N, g.M_eff, g.K_pad, Ws, A, bg, theta, st);
 }
 
 static bool bad_dims(int64_t B, int N, int M, int dtype) {
@@ -238,7 +260,8 @@ int nk_rbm_logpsi(const int8_t* sigma, int64_t B, int N, int M, int dtype, const
     cudaStream_t st = (cudaStream_t)stream;
     const LogpsiWs w = carve_logpsi(workspace, g, B);
     NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.Wg, w.bg, st));
-    NK_CUDA(launch_theta_gemm(sigma, B, N, g.M_eff, w.Wg, w.bg, w.theta, st));
+    if (!use_simt_theta()) NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
+    NK_CUDA(run_theta(g, sigma, B, w.Wg, w.bg, w.Ws, w.A, w.theta, st));
     NK_CUDA(launch_logpsi(sigma, B, g, dtype, w.theta, a, logpsi_out, (flags & NK_OUT_F64) != 0, theta_out, st));
     return NK_OK;
 }
@@ -282,6 +305,7 @@ int nk_local_energy(nk_operator_t h, const int8_t* sigma, int64_t B, int N, int 
     {
         Scope sc(PH_PACK, st);
         NK_CUDA(launch_pack(op, g, dtype, W, a, b, w.Wg, w.bg, w.Wt, w.Dtab, w.rows, st));
+        if (!use_simt_theta()) NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
     }
     const size_t esz = dtype == NK_C64 ? 8 : 4;
     for (int64_t s0 = 0; s0 < B; s0 += chunk) {
@@ -289,7 +313,7 @@ int nk_local_energy(nk_operator_t h, const int8_t* sigma, int64_t B, int N, int 
         const int8_t* sg = sigma + s0 * N;
         {
             Scope sc(PH_GEMM, st);
-            NK_CUDA(launch_theta_gemm(sg, nb, N, g.M_eff, w.Wg, w.bg, w.theta, st));
+            NK_CUDA(run_theta(g, sg, nb, w.Wg, w.bg, w.Ws, w.A, w.theta, st));
         }
         if (logpsi_out) {
             Scope sc(PH_LOGPSI, st);

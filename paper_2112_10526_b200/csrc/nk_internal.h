@@ -44,6 +44,7 @@ inline size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
 // Geometry derived from (op, N, M, dtype).
 struct Geometry {
     int N, n_words, M, M_pad, M_eff, planes; // M_eff = planes * M_pad; n_words = ceil(N / 32)
+    int K_pad;                               // N rounded up to 64: k extent of the bf16 tensor-core operands
     int n_rows, tile_rows, n_tiles, n_rows_pad;
     int stages, ctas_per_sm;                 // shared-memory ring plan of the fused kernel
     size_t smem_bytes;
@@ -62,6 +63,12 @@ cudaError_t launch_pack_gemm_only(const Geometry& g, int dtype, const void* W, c
 // theta_gemm.cu : theta[s][m] = bg[m] + sum_k sigma[s][k] Wg[m][k]
 cudaError_t launch_theta_gemm(const int8_t* sigma, int64_t B, int N, int M_eff, const float* Wg, const float* bg,
                               float* theta, cudaStream_t st);
+// theta_tc.cu : the same contraction on tcgen05 tensor cores (bf16 x3 split of W, two TMEM accumulators)
+cudaError_t theta_tc_init();
+cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* Ws_bf16, unsigned* absmax_scratch,
+                           cudaStream_t st);
+cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, int K_pad, const void* Ws_bf16,
+                            void* A_bf16, const float* bg, float* theta, cudaStream_t st);
 // logpsi.cu
 cudaError_t launch_logpsi(const int8_t* sigma, int64_t B, const Geometry& g, int dtype, const float* theta,
                           const void* a, void* logpsi_out, bool out_f64, void* theta_out, cudaStream_t st);

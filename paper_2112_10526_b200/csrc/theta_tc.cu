@@ -1,0 +1,299 @@
+// Base activations theta = sigma W^T + b on the 5th-generation tensor cores (BASELINE.json
+// north_star (2): "the one place tensor cores are justified").
+//
+// Exactness: sigma = +-1 is exact in bf16.  W (fp32) is split on three FIXED-POINT grids tied to max|W|:
+//   W ~ W_hi + W_mid + W_lo,  W_hi = m1 2^e1, W_mid = m2 2^(e1-8), W_lo = m3 2^(e1-16),  |m| <= 256 integers,
+//   2^(e1+8) > max|W|,  residual <= 2^(e1-17) < 2^-25 max|W|  (below one fp32 ulp of any |w| > max|W| / 4).
+// Every piece is exact in bf16, every product is exact, and each piece has its OWN TMEM accumulator, in which all
+// partial sums are integers < 2^24 times the piece's quantum: the tensor-core accumulation is exact whatever
+// rounding the adder uses (measured: with per-element bf16 splitting the adder's truncation of sub-ulp bits
+// biased theta toward zero by ~0.25 ulp, which adds up coherently over the M terms of ln psi).  Only the epilogue
+// rounds: theta = (D_hi + (D_mid + D_lo)) + b in fp32, round-to-nearest.
+//
+// Kernel: one CTA per 128 (samples) x 128 (hidden) tile.  Warp 0 = TMA producer (cp.async.bulk.tensor, 128B
+// swizzle, 3-stage ring: per stage the sigma tile and the three W-piece tiles for a 64-wide k block); warp 1 =
+// TMEM allocator and single-thread tcgen05.mma issuer (kind::f16, M=128, N=128, K=16; 12 MMAs per k block, three
+// 128-column fp32 accumulators);
+// warps 2-5 = epilogue (tcgen05.ld 32x32b, bias add, fp32 stores).
+#include <cuda.h>
+#include <cuda_bf16.h>
+
+#include "nk_internal.h"
+#include "ptx_helpers.cuh"
+
+namespace nk {
+
+namespace tc {
+constexpr int BM = 128, BN = 128, BK = 64, STAGES = 3, UMMA_K = 16;
+constexpr int TILE_BYTES = BM * BK * 2;                   // 16 KB: one 128-row x 64-col bf16 tile (A or one W piece)
+constexpr int STAGE_BYTES = 4 * TILE_BYTES;               // sigma + hi + mid + lo
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment*/ + 256 /*barriers*/;
+constexpr int THREADS = 192;
+constexpr uint32_t TMEM_COLS = 512;                       // D_hi [0,128), D_mid [128,256), D_lo [256,384); power of 2
+// instruction descriptor (cute::UMMA::InstrDescriptor bit layout): D=F32, A=B=BF16, K-major both, N=128, M=128
+constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+}  // namespace tc
+
+// ---- operand preparation ---------------------------------------------------------------------------------
+// max |Wg| as float bits (non-negative floats order like unsigned ints); *out must be zeroed first
+__global__ void absmax_kernel(const float* __restrict__ Wg, size_t n, unsigned* __restrict__ out) {
+    unsigned m = 0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        m = max(m, __float_as_uint(fabsf(Wg[i])));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
+}
+
+// Ws[piece][me][k] (bf16, K_pad columns, zero padded) from Wg[me][k] (fp32): fixed-point split on the grids
+// 2^e1, 2^(e1-8), 2^(e1-16) with 2^(e1+8) > max|W|
+__global__ void split_w_kernel(const float* __restrict__ Wg, int M_eff, int N, int K_pad,
+                               const unsigned* __restrict__ absmax_bits, __nv_bfloat16* __restrict__ Ws) {
+    const float wmax = __uint_as_float(*absmax_bits);
+    int ex = 0;
+    if (wmax > 0.f) frexpf(wmax, &ex);                    // wmax = f 2^ex, f in [0.5, 1)
+    else ex = -100;
+    const float q1 = ldexpf(1.f, ex - 8), q2 = ldexpf(1.f, ex - 16), q3 = ldexpf(1.f, ex - 24);
+    const float s1 = ldexpf(1.f, 8 - ex), s2 = ldexpf(1.f, 16 - ex), s3 = ldexpf(1.f, 24 - ex);
+    const int me = blockIdx.y;
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < K_pad; k += gridDim.x * blockDim.x) {
+        float w = (k < N) ? Wg[(size_t)me * N + k] : 0.f;
+        const float hi = rintf(w * s1) * q1;
+        w -= hi;                                          // exact
+        const float mid = rintf(w * s2) * q2;
+        w -= mid;                                         // exact
+        const float lo = rintf(w * s3) * q3;
+        const size_t o = (size_t)me * K_pad + k, plane = (size_t)M_eff * K_pad;
+        Ws[o] = __float2bfloat16_rn(hi);                  // |m| <= 256: exact in bf16
+        Ws[plane + o] = __float2bfloat16_rn(mid);
+        Ws[2 * plane + o] = __float2bfloat16_rn(lo);
+    }
+}
+
+// A[s][k] = (bf16) sigma[s][k], zero padded to K_pad
+__global__ void sigma_bf16_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int K_pad,
+                                  __nv_bfloat16* __restrict__ A) {
+    const int64_t total = B * K_pad;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t s = idx / K_pad;
+        const int k = (int)(idx - s * K_pad);
+        A[idx] = __float2bfloat16_rn(k < N ? (float)sigma[s * N + k] : 0.f);
+    }
+}
+
+// ---- tcgen05 / TMA wrappers --------------------------------------------------------------------------------
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+        ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ uint64_t make_sdesc(uint32_t smem_addr) {
+    // K-major, 128B swizzle: start address >> 4, LBO (unused for swizzled K-major) = 1, SBO = 1024 B (8 rows x
+    // 128 B) >> 4, descriptor version 1 (sm_100), layout type 2 = SWIZZLE_128B
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3FFFF) >> 4);
+    d |= (uint64_t)1 << 16;
+    d |= (uint64_t)(1024 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)2 << 61;
+    return d;
+}
+__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                          uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}\n" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
+    uint32_t* r = reinterpret_cast<uint32_t*>(v);
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+          "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+          "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+}
+
+// ---- the GEMM ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(tc::THREADS, 1)
+theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w, int64_t B,
+                int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta) {
+    using namespace tc;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;            // SWIZZLE_128B needs 1024 B
+    const uint32_t bars = smem_base + STAGES * STAGE_BYTES;                      // full[3], empty[3], tmem_full
+    const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, tfull = bars + 16 * STAGES;
+    const uint32_t tmem_slot = bars + 16 * STAGES + 8;
+    uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n0 = blockIdx.x * BN;                       // hidden-unit tile
+    const int64_t m0 = (int64_t)blockIdx.y * BM;          // sample tile
+    const int n_kb = K_pad / BK;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, 1); }
+        mbar_init(tfull, 1);
+        mbar_fence_init();
+    }
+    if (warp == 1) {   // TMEM allocation by one full warp; the base address lands in shared memory
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            int stage = 0; uint32_t parity = 1;
+            for (int kb = 0; kb < n_kb; ++kb) {
+                mbar_wait(empty0 + 8 * stage, parity);
+                mbar_arrive_expect_tx(full0 + 8 * stage, STAGE_BYTES);
+                const uint32_t dst = smem_base + stage * STAGE_BYTES;
+                tma_load_2d(dst, &map_a, kb * BK, (int)m0, full0 + 8 * stage);
+#pragma unroll
+                for (int pc = 0; pc < 3; ++pc)
+                    tma_load_2d(dst + (1 + pc) * TILE_BYTES, &map_w, kb * BK, pc * M_eff + n0, full0 + 8 * stage);
+                if (++stage == STAGES) { stage = 0; parity ^= 1; }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one thread) =====
+        if (lane == 0) {
+            int stage = 0; uint32_t parity = 0;
+            for (int kb = 0; kb < n_kb; ++kb) {
+                mbar_wait(full0 + 8 * stage, parity);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t a_addr = smem_base + stage * STAGE_BYTES;
+#pragma unroll
+                for (int k = 0; k < BK / UMMA_K; ++k) {
+                    const uint32_t koff = k * UMMA_K * 2;                       // bytes inside the 128 B swizzle row
+                    const uint64_t ad = make_sdesc(a_addr + koff);
+                    const uint32_t first = (kb | k) ? 1u : 0u;
+                    umma_bf16(tmem_base + 0, ad, make_sdesc(a_addr + 1 * TILE_BYTES + koff), IDESC, first);
+                    umma_bf16(tmem_base + BN, ad, make_sdesc(a_addr + 2 * TILE_BYTES + koff), IDESC, first);
+                    umma_bf16(tmem_base + 2 * BN, ad, make_sdesc(a_addr + 3 * TILE_BYTES + koff), IDESC, first);
+                }
+                umma_commit(empty0 + 8 * stage);          // frees the smem stage when these MMAs have read it
+                if (++stage == STAGES) { stage = 0; parity ^= 1; }
+            }
+            umma_commit(tfull);                           // accumulators complete
+        }
+    } else {
+        // ===== epilogue: warps 2..5, TMEM lane quarter = warp % 4 =====
+        const int q = warp & 3;
+        mbar_wait(tfull, 0);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const int64_t row = m0 + q * 32 + lane;
+        float* out = theta + row * M_eff + n0;
+#pragma unroll 1
+        for (int c0 = 0; c0 < BN; c0 += 32) {
+            float hi[32], mid[32], lo[32];
+            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + c0;
+            tmem_ld32(taddr, hi);
+            tmem_ld32(taddr + BN, mid);
+            tmem_ld32(taddr + 2 * BN, lo);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (row < B) {
+#pragma unroll
+                for (int j = 0; j < 32; j += 4) {
+                    const float4 bb = *reinterpret_cast<const float4*>(bg + n0 + c0 + j);
+                    float4 o;
+                    o.x = (hi[j] + (mid[j] + lo[j])) + bb.x;
+                    o.y = (hi[j + 1] + (mid[j + 1] + lo[j + 1])) + bb.y;
+                    o.z = (hi[j + 2] + (mid[j + 2] + lo[j + 2])) + bb.z;
+                    o.w = (hi[j + 3] + (mid[j + 3] + lo[j + 3])) + bb.w;
+                    *reinterpret_cast<float4*>(out + c0 + j) = o;
+                }
+            }
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 1) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+    }
+}
+
+// ---- host side ---------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn g_encode = nullptr;
+static bool g_tc_ready = false;
+
+cudaError_t theta_tc_init() {
+    if (g_tc_ready) return cudaSuccess;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess) return e;
+    if (qres != cudaDriverEntryPointSuccess || fn == nullptr) return cudaErrorNotSupported;
+    g_encode = (EncodeTiledFn)fn;
+    e = cudaFuncSetAttribute((const void*)theta_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    g_tc_ready = true;
+    return cudaSuccess;
+}
+
+static bool encode_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols) {
+    const cuuint64_t dims[2] = {cols, rows};
+    const cuuint64_t strides[1] = {cols * 2};
+    const cuuint32_t box[2] = {(cuuint32_t)tc::BK, (cuuint32_t)tc::BM};
+    const cuuint32_t estr[2] = {1, 1};
+    return g_encode(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* Ws, unsigned* absmax_scratch,
+                           cudaStream_t st) {
+    cudaError_t e = cudaMemsetAsync(absmax_scratch, 0, sizeof(unsigned), st);
+    if (e != cudaSuccess) return e;
+    const size_t n = (size_t)M_eff * N;
+    unsigned blocks = (unsigned)((n + 1023) / 1024);
+    if (blocks > 1184) blocks = 1184;
+    absmax_kernel<<<blocks, 256, 0, st>>>(Wg, n, absmax_scratch);
+    dim3 grid((K_pad + 255) / 256, M_eff);
+    split_w_kernel<<<grid, 256, 0, st>>>(Wg, M_eff, N, K_pad, absmax_scratch, (__nv_bfloat16*)Ws);
+    count_launch(2);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, int K_pad, const void* Ws, void* A,
+                            const float* bg, float* theta, cudaStream_t st) {
+    if (B <= 0) return cudaSuccess;
+    cudaError_t e = theta_tc_init();
+    if (e != cudaSuccess) return e;
+    const int64_t total = B * K_pad;
+    int64_t blocks = (total + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    sigma_bf16_kernel<<<(unsigned)blocks, 256, 0, st>>>(sigma, B, N, K_pad, (__nv_bfloat16*)A);
+    CUtensorMap map_a, map_w;
+    if (!encode_2d(&map_a, A, (uint64_t)B, (uint64_t)K_pad)) return cudaErrorInvalidValue;
+    if (!encode_2d(&map_w, Ws, (uint64_t)3 * M_eff, (uint64_t)K_pad)) return cudaErrorInvalidValue;
+    dim3 grid(M_eff / tc::BN, (unsigned)((B + tc::BM - 1) / tc::BM));
+    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_w, B, M_eff, K_pad, bg, theta);
+    count_launch(2);
+    return cudaGetLastError();
+}
+
+}  // namespace nk
