@@ -77,8 +77,9 @@ struct RealState {
         }
         qinv = 1.f / ((p0 * p1) * (p2 * p3));
     }
-    // returns psi'/psi without the visible-bias factor, identical on all lanes
-    __device__ __forceinline__ float ratio(const float* __restrict__ drow, int lane, float s, float a2) const {
+    // this lane's share of psi'/psi for one row: r = prod_{j in lane} (1+e'_j)/(1+e_j), acc = sum_j (|x'_j| - |x_j|)
+    __device__ __forceinline__ void partial(const float* __restrict__ drow, int lane, float s, float& r,
+                                            float& acc) const {
         float p0 = 1.f, p1 = 1.f, p2 = 1.f, p3 = 1.f, acc0 = 0.f, acc1 = 0.f;
 #pragma unroll
         for (int v = 0; v < V; ++v) {
@@ -95,13 +96,36 @@ struct RealState {
             acc0 += fabsf(x2) - fabsf(t.z);
             acc1 += fabsf(x3) - fabsf(t.w);
         }
-        float r = ((p0 * p1) * (p2 * p3)) * qinv;
-        float acc = acc0 + acc1;
-        r = warp_prod_f(r);
-        acc = warp_sum_f(acc);
-        return r * ex2_approx(fmaf(0.5f, acc, s * a2));
+        r = ((p0 * p1) * (p2 * p3)) * qinv;
+        acc = acc0 + acc1;
     }
 };
+
+// One pending row of a sample: lane partials plus the row's scalars.  Rows are reduced across the warp two at a
+// time: after the first exchange (lane ^ 16) the lower half-warp owns row A and the upper half row B, so the
+// five butterfly levels cost 10 shuffles per PAIR of rows instead of 10 per row, and the two rows' serial
+// reduction latencies overlap.
+struct RowPartR {
+    float r, acc, ex, coef;     // ex = s * a2 (visible-bias exponent, log2 units)
+};
+__device__ __forceinline__ float finish_pair(const RowPartR& A, const RowPartR& B, int lane) {
+    const bool up = (lane & 16) != 0;
+    float rk = up ? B.r : A.r, ak = up ? B.acc : A.acc;
+    const float rs = up ? A.r : B.r, as = up ? A.acc : B.acc;
+    rk *= __shfl_xor_sync(0xffffffffu, rs, 16);
+    ak += __shfl_xor_sync(0xffffffffu, as, 16);
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) {
+        rk *= __shfl_xor_sync(0xffffffffu, rk, o);
+        ak += __shfl_xor_sync(0xffffffffu, ak, o);
+    }
+    const float ex = up ? B.ex : A.ex, c = up ? B.coef : A.coef;
+    return c * (rk * ex2_approx(fmaf(0.5f, ak, ex)));   // lower half: row A's term, upper half: row B's
+}
+__device__ __forceinline__ float finish_single(const RowPartR& A) {
+    const float r = warp_prod_f(A.r), acc = warp_sum_f(A.acc);
+    return A.coef * (r * ex2_approx(fmaf(0.5f, acc, A.ex)));
+}
 
 template <int V>
 struct CplxState {
@@ -138,9 +162,11 @@ struct CplxState {
         const float inv = 1.f / fmaf(ar, ar, ai * ai);
         qr = ar * inv; qi = -ai * inv;
     }
-    __device__ __forceinline__ void ratio(const float* __restrict__ drow, int lane, int M_pad, float s, float a2re,
-                                          float a2im, float& out_re, float& out_im) const {
-        float ar = 1.f, ai = 0.f, br = 1.f, bi = 0.f, acc = 0.f;
+    // this lane's share: (ar + i ai) = prod_{j in lane} f'_j / f_j, acc = sum_j (|x'_j| - |x_j|)
+    __device__ __forceinline__ void partial(const float* __restrict__ drow, int lane, int M_pad, float s, float& ar,
+                                            float& ai, float& acc) const {
+        float br = 1.f, bi = 0.f;
+        ar = 1.f; ai = 0.f; acc = 0.f;
 #pragma unroll
         for (int v = 0; v < V; ++v) {
             const float4 dx = *reinterpret_cast<const float4*>(drow + (v * 32 + lane) * 4);
@@ -158,19 +184,50 @@ struct CplxState {
         }
         cmul(ar, ai, br, bi);
         cmul(ar, ai, qr, qi);
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const float orr = __shfl_xor_sync(0xffffffffu, ar, o), oi = __shfl_xor_sync(0xffffffffu, ai, o);
-            cmul(ar, ai, orr, oi);
-            acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        }
-        const float mag = ex2_approx(fmaf(0.5f, acc, s * a2re));
-        float sn, cs;
-        __sincosf(s * a2im, &sn, &cs);
-        cmul(ar, ai, mag * cs, mag * sn);
-        out_re = ar; out_im = ai;
     }
+    static __device__ __forceinline__ void cmul_pub(float& ar, float& ai, float br, float bi) { cmul(ar, ai, br, bi); }
 };
+
+struct RowPartC {
+    float ar, ai, acc, ex_re, ex_im, coef;   // ex_re = s a2_re (log2 units), ex_im = s a2_im (radians)
+};
+__device__ __forceinline__ void cmul_f(float& ar, float& ai, float br, float bi) {
+    const float r = fmaf(ar, br, -ai * bi), i = fmaf(ar, bi, ai * br);
+    ar = r; ai = i;
+}
+__device__ __forceinline__ void finish_c(float ar, float ai, float acc, float ex_re, float ex_im, float c,
+                                         float& out_re, float& out_im) {
+    const float mag = c * ex2_approx(fmaf(0.5f, acc, ex_re));
+    float sn, cs;
+    __sincosf(ex_im, &sn, &cs);
+    cmul_f(ar, ai, mag * cs, mag * sn);
+    out_re = ar; out_im = ai;
+}
+__device__ __forceinline__ void finish_pair_c(const RowPartC& A, const RowPartC& B, int lane, float& out_re,
+                                              float& out_im) {
+    const bool up = (lane & 16) != 0;
+    float kr = up ? B.ar : A.ar, ki = up ? B.ai : A.ai, ka = up ? B.acc : A.acc;
+    const float sr = up ? A.ar : B.ar, si = up ? A.ai : B.ai, sa = up ? A.acc : B.acc;
+    cmul_f(kr, ki, __shfl_xor_sync(0xffffffffu, sr, 16), __shfl_xor_sync(0xffffffffu, si, 16));
+    ka += __shfl_xor_sync(0xffffffffu, sa, 16);
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) {
+        const float orr = __shfl_xor_sync(0xffffffffu, kr, o), oi = __shfl_xor_sync(0xffffffffu, ki, o);
+        cmul_f(kr, ki, orr, oi);
+        ka += __shfl_xor_sync(0xffffffffu, ka, o);
+    }
+    finish_c(kr, ki, ka, up ? B.ex_re : A.ex_re, up ? B.ex_im : A.ex_im, up ? B.coef : A.coef, out_re, out_im);
+}
+__device__ __forceinline__ void finish_single_c(const RowPartC& A, float& out_re, float& out_im) {
+    float ar = A.ar, ai = A.ai, acc = A.acc;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const float orr = __shfl_xor_sync(0xffffffffu, ar, o), oi = __shfl_xor_sync(0xffffffffu, ai, o);
+        cmul_f(ar, ai, orr, oi);
+        acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    }
+    finish_c(ar, ai, acc, A.ex_re, A.ex_im, A.coef, out_re, out_im);
+}
 
 // ---- kernel ----------------------------------------------------------------------------------------------
 template <int V, bool CPLX>
@@ -237,7 +294,10 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
         st.load(p.theta + srow * p.M_eff, lane, p.M_pad);
         __syncwarp();
 
-        float diag = 0.f, e_re = 0.f, e_im = 0.f;
+        // e_u*: terms identical on all lanes (single rows); e_h*: half-warp-specific terms (paired rows)
+        float diag = 0.f, e_ure = 0.f, e_uim = 0.f, e_hre = 0.f, e_him = 0.f;
+        bool pending = false;                         // warp-uniform: one row waits for a partner
+        typename std::conditional<CPLX, RowPartC, RowPartR>::type pend;
         if (p.kind == NK_ISING) {
             for (int b = lane; b < p.n_bonds; b += 32) {
                 const int i = p.bonds[2 * b], j = p.bonds[2 * b + 1];
@@ -269,14 +329,23 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
                 const float s = __shfl_sync(0xffffffffu, sgn, r);
                 const float c = __shfl_sync(0xffffffffu, coef, r);
                 const float ar = __shfl_sync(0xffffffffu, a2re, r);
+                const float* drow = tile + (size_t)r * p.M_eff;
                 if constexpr (!CPLX) {
-                    e_re = fmaf(c, st.ratio(tile + (size_t)r * p.M_eff, lane, s, ar), e_re);
+                    RowPartR cur;
+                    st.partial(drow, lane, s, cur.r, cur.acc);
+                    cur.ex = s * ar; cur.coef = c;
+                    if (pending) { e_hre += finish_pair(pend, cur, lane); pending = false; }
+                    else { pend = cur; pending = true; }
                 } else {
                     const float ai = __shfl_sync(0xffffffffu, a2im, r);
-                    float rr, rim;
-                    st.ratio(tile + (size_t)r * p.M_eff, lane, p.M_pad, s, ar, ai, rr, rim);
-                    e_re = fmaf(c, rr, e_re);
-                    e_im = fmaf(c, rim, e_im);
+                    RowPartC cur;
+                    st.partial(drow, lane, p.M_pad, s, cur.ar, cur.ai, cur.acc);
+                    cur.ex_re = s * ar; cur.ex_im = s * ai; cur.coef = c;
+                    if (pending) {
+                        float rr, rim;
+                        finish_pair_c(pend, cur, lane, rr, rim);
+                        e_hre += rr; e_him += rim; pending = false;
+                    } else { pend = cur; pending = true; }
                 }
             }
             __syncwarp();
@@ -295,10 +364,16 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
             ++g;
             if (++stage == p.stages) { stage = 0; parity ^= 1; }
         }
+        if (pending) {
+            if constexpr (!CPLX) e_ure = finish_single(pend);
+            else finish_single_c(pend, e_ure, e_uim);
+        }
+        e_hre += __shfl_xor_sync(0xffffffffu, e_hre, 16);          // row-A half + row-B half
+        if constexpr (CPLX) e_him += __shfl_xor_sync(0xffffffffu, e_him, 16);
         diag = warp_sum_f(diag);
         if (valid && lane == 0) {
-            if constexpr (!CPLX) p.eloc[sample] = diag + e_re;
-            else { p.eloc[2 * sample] = diag + e_re; p.eloc[2 * sample + 1] = e_im; }
+            if constexpr (!CPLX) p.eloc[sample] = diag + (e_ure + e_hre);
+            else { p.eloc[2 * sample] = diag + (e_ure + e_hre); p.eloc[2 * sample + 1] = e_uim + e_him; }
         }
     }
 }
