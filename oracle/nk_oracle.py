@@ -15,6 +15,11 @@ What it computes, in the paper's order and notation (citations are PAPER.md line
   * `local_energy`           A~(s) = sum_s' psi(s')/psi(s) <s|A|s'>  (Eq. (12)) — every ln psi(s') FROM SCRATCH
   * `stats`                  E[A~] ~ (1/N_s) sum A~(s_i)            (Eq. (17)) and the population variance (Q10)
 
+  * `rbm_log_derivatives`, `force`, `energy_gradient[_batched]`   O_i = d ln psi/d theta_i (Eq. (13)),
+        f~ = Cov[O, H~] (Eq. (14)/(26)), gradient 2 Re f~ | f~ (Eq. (15)/(16), (27)/(28)) — SURVEY.md §8(f) rank 1;
+        pins in tests/test_oracle_gradient.py (finite differences of ln psi; finite differences of the exact
+        <H> from the dense Kronecker Hamiltonian over the full Born distribution; covariance properties)
+
 Pins (tests/test_oracle_pins.py, `-m "not gpu"`): dense Kronecker-product Hamiltonians built independently in
 tests/dense_ref.py (Born identity Eq. (11) L646 over the full space; row-by-row equality of the connected list),
 Eq. (2), closed forms (W = 0; M = 1 with np.cosh; uniform psi), known ring spectra, symmetries.
@@ -161,3 +166,61 @@ def count_amplitudes(kind, sigma, bonds, colors, J, h=0.0):
     colors = np.zeros(len(bonds), dtype=np.int64) if colors is None else np.asarray(colors)
     anti = sigma[:, bonds[:, 0]] != sigma[:, bonds[:, 1]]
     return int(anti[:, J[colors] != 0.0].sum())
+
+
+# ---------------------------------------------------------------------------------------------------------
+# NEXT-1: force vector / energy gradient for the RBM
+# ---------------------------------------------------------------------------------------------------------
+def rbm_log_derivatives(sigma, W, b=None):
+    """Log-derivatives O_i(s) = d ln psi(s) / d theta_i (Eq. (13)) of the RBM, written out from
+    ln psi = a.s + sum_j ln cosh(W s + b)_j:   O_{a_k} = s_k,  O_{b_j} = tanh theta_j,  O_{W_jk} = tanh theta_j s_k.
+    (Pinned by central finite differences of `rbm_logpsi` in tests/test_oracle_gradient.py.)
+    Returns (O_a [B][N], O_b [B][M], O_W [B][M][N])."""
+    sigma = np.atleast_2d(np.asarray(sigma))
+    theta = rbm_theta(sigma, W, b)
+    T = np.tanh(theta)
+    s = sigma.astype(T.dtype)
+    return s, T, T[:, :, None] * s[:, None, :]
+
+
+def force(O, eloc, weights=None):
+    """Force vector f~_i = Cov[O_i, H~] = E[O_i^* (H~ - E[H~])] (Eq. (14), Eq. (26)).
+    E[.] is the sample mean (Eq. (17)); `weights` (normalised probabilities) replaces it by a weighted mean —
+    used only by the exact-distribution pin."""
+    O = np.asarray(O)
+    e = np.asarray(eloc).astype(np.complex128 if np.iscomplexobj(eloc) or np.iscomplexobj(O) else np.float64)
+    if weights is None:
+        weights = np.full(e.shape[0], 1.0 / e.shape[0])
+    w = np.asarray(weights, dtype=np.float64)
+    de = e - np.sum(w * e)
+    return np.tensordot(w * de, np.conj(O), axes=(0, 0))
+
+
+def energy_gradient(sigma, W, b, eloc, weights=None):
+    """Gradient of <H> from samples: real parameters f = 2 Re f~ (Eq. (15) L664 / Eq. (27)); complex
+    parameters of a holomorphic ansatz (the complex RBM is one) f = f~ (Eq. (16) L668 / Eq. (28)).
+    Returns (g_a [N], g_b [M], g_W [M][N])."""
+    cplx = np.iscomplexobj(W)
+    O_a, O_b, O_W = rbm_log_derivatives(sigma, W, b)
+    out = []
+    for O in (O_a, O_b, O_W):
+        f = force(O, eloc, weights)
+        out.append(f if cplx else 2.0 * np.real(f))
+    return tuple(out)
+
+
+def energy_gradient_batched(sigma, W, b, eloc):
+    """Same numbers as `energy_gradient` without the [B][M][N] tensor of O_W (needed at full batch size):
+    g_W = sum_s conj(tanh theta_s) (dE_s / B) s_s^T as one library matmul."""
+    cplx = np.iscomplexobj(W)
+    sigma = np.atleast_2d(np.asarray(sigma))
+    T = np.tanh(rbm_theta(sigma, W, b))
+    e = np.asarray(eloc).astype(np.complex128 if cplx else np.float64)
+    de = (e - e.mean()) / e.shape[0]
+    s = sigma.astype(T.dtype)
+    g_a = de @ s
+    g_b = de @ np.conj(T)
+    g_W = (np.conj(T) * de[:, None]).T @ s
+    if not cplx:
+        return 2.0 * g_a.real, 2.0 * g_b.real, 2.0 * g_W.real
+    return g_a, g_b, g_W
