@@ -120,6 +120,21 @@ int nk_local_energy_host(nk_operator_t op, const int8_t* sigma_host, int64_t B, 
                          void* eloc_host, void* logpsi_host, double* stats_host, void* scratch,
                          size_t scratch_bytes, nk_stream_t stream);
 
+/* ---- energy gradient / force vector of the RBM -------------------------------------
+ * PAPER.md Eq. (13) L656 (log-derivatives O_i), Eq. (14) L660 / (26) L910 (force f~_i = E[O_i^* (H~ - E[H~])]),
+ * Eq. (15)/(16) L664-668 and (27)/(28) L918-922: the gradient of <H> is 2 Re f~ for real parameters (NK_F32) and
+ * f~ for the complex, holomorphic RBM (NK_C64).  O_a = s, O_b = tanh(theta), O_W = tanh(theta) s^T; E[.] is the
+ * mean over the B samples.
+ *   eloc   dev [B] float | (re,im) float, and stats dev double[4] (mean in [0],[1]) — as written by nk_local_energy
+ *   grad_a_out dev [N] or NULL, grad_b_out dev [M] or NULL, grad_W_out dev [M][N]; parameter dtype
+ * Samples are processed chunk_size at a time (0 = whole batch); the workspace scales with min(B, chunk_size).
+ * The contraction over samples runs on the tensor cores with exact products; results are bit-reproducible. */
+size_t nk_energy_gradient_workspace_bytes(int64_t B, int N, int M, int dtype, int64_t chunk_size);
+int nk_energy_gradient(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* b,
+                       const void* eloc, const double* stats, int64_t chunk_size, void* grad_a_out,
+                       void* grad_b_out, void* grad_W_out, void* workspace, size_t workspace_bytes,
+                       nk_stream_t stream);
+
 /* Per-phase device timing (bench accounting).  With nk_profile_enable(1), nk_local_energy brackets each phase
  * of each chunk with CUDA events on the call's stream (a few microseconds of timeline each).  nk_profile_read
  * synchronises on those events, adds up the elapsed milliseconds per phase since the last read and writes

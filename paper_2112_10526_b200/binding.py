@@ -10,7 +10,7 @@ import os
 
 import numpy as np
 
-__all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host",
+__all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host", "energy_gradient",
            "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
            "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "EXPORTS"]
 
@@ -35,6 +35,8 @@ EXPORTS = {
     "nk_local_energy": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_local_energy_host_scratch_bytes": (_sz, [_vp, _i64, _int, _int, _int, _i64]),
     "nk_local_energy_host": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "nk_energy_gradient_workspace_bytes": (_sz, [_i64, _int, _int, _int, _i64]),
+    "nk_energy_gradient": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_launch_count": (_i64, [_int]),
     "nk_profile_enable": (_int, [_int]),
     "nk_profile_read": (_int, [_vp]),
@@ -247,6 +249,31 @@ def local_energy_host(op: Operator, sigma, W, a=None, b=None, *, chunk_size: int
                                   p(logpsi), p(stats), _ptr(plan.scratch), plan.bytes, _stream())
     _check(rc, "nk_local_energy_host")
     return eloc, logpsi, stats
+
+
+def energy_gradient(sigma, W, b, eloc, stats, *, chunk_size: int = 0, ws=None):
+    """nk_energy_gradient on device tensors -> (grad_a [N], grad_b [M], grad_W [M][N]) in the parameter dtype.
+    `eloc`, `stats` are the outputs of local_energy on the same sigma."""
+    torch = _torch()
+    lib = load()
+    _check_params(sigma, W, None, b)
+    B, N = sigma.shape
+    M = W.shape[0]
+    dt = _dtype_code(W)
+    if eloc.dtype != W.dtype or eloc.shape != (B,) or stats.dtype != torch.float64 or stats.numel() != 4:
+        raise NkError("eloc must be [B] of W's dtype and stats double[4] (outputs of local_energy)")
+    ga = torch.empty(N, dtype=W.dtype, device=sigma.device)
+    gb = torch.empty(M, dtype=W.dtype, device=sigma.device)
+    gW = torch.empty((M, N), dtype=W.dtype, device=sigma.device)
+    nbytes = lib.nk_energy_gradient_workspace_bytes(B, N, M, dt, int(chunk_size))
+    if nbytes == 0:
+        raise NkError("nk_energy_gradient_workspace_bytes rejected the arguments")
+    if ws is None or ws.numel() < nbytes:
+        ws = torch.empty(nbytes, dtype=torch.uint8, device=sigma.device)
+    rc = lib.nk_energy_gradient(_ptr(sigma), B, N, M, dt, _ptr(W), _ptr(b), _ptr(eloc), _ptr(stats), int(chunk_size),
+                                _ptr(ga), _ptr(gb), _ptr(gW), _ptr(ws), ws.numel(), _stream())
+    _check(rc, "nk_energy_gradient")
+    return ga, gb, gW
 
 
 def launch_count(reset: bool = False) -> int:

@@ -128,6 +128,25 @@ static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk) {
     return w;
 }
 
+static GradWs carve_grad(void* ws, const Geometry& g, int64_t chunk, size_t* bytes) {
+    Carver c(ws);
+    GradWs w;
+    w.ld = (int)((chunk + 63) / 64 * 64);
+    w.Wg = c.take<float>((size_t)g.M_eff * g.N);
+    w.bg = c.take<float>(g.M_eff);
+    w.theta = c.take<float>((size_t)chunk * g.M_eff);
+    w.Gacc = c.take<float>((size_t)g.N * g.M_eff);
+    w.Ws = c.take<uint16_t>((size_t)3 * g.M_eff * g.K_pad);
+    w.A = c.take<uint16_t>((size_t)chunk * g.K_pad);
+    w.TwT = c.take<uint16_t>((size_t)3 * g.M_eff * w.ld);
+    w.sigT = c.take<uint16_t>((size_t)g.N * w.ld);
+    w.gb_acc = c.take<double>(g.M_eff);
+    w.ga_acc = c.take<double>((size_t)2 * g.N);
+    w.absmax = c.take<unsigned>(1);
+    *bytes = c.off;
+    return w;
+}
+
 // NK_THETA_SIMT=1 selects the FP32 SIMT contraction (debugging aid); default is the tcgen05 path.
 static bool use_simt_theta() {
     static const bool v = [] { const char* e = std::getenv("NK_THETA_SIMT"); return e && e[0] == '1'; }();
@@ -272,6 +291,45 @@ int nk_connected(nk_operator_t h, const int8_t* sigma, int64_t B, int32_t* flips
     const Operator* op = (const Operator*)h;
     if (op->n_sites > 48 * 1024) return NK_ERR_UNSUPPORTED;
     NK_CUDA(launch_connected(op, sigma, B, flips_out, mels_out, n_conn_out, sigma_prime_out, (cudaStream_t)stream));
+    return NK_OK;
+}
+
+static int64_t eff_chunk(int64_t B, int64_t chunk_size);
+
+size_t nk_energy_gradient_workspace_bytes(int64_t B, int N, int M, int dtype, int64_t chunk_size) {
+    if (bad_dims(B, N, M, dtype) || chunk_size < 0) return 0;
+    const Geometry g = make_geometry(nullptr, N, M, dtype);
+    size_t bytes = 0;
+    carve_grad(nullptr, g, eff_chunk(B, chunk_size), &bytes);
+    return bytes;
+}
+
+int nk_energy_gradient(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* b,
+                       const void* eloc, const double* stats, int64_t chunk_size, void* grad_a_out,
+                       void* grad_b_out, void* grad_W_out, void* workspace, size_t workspace_bytes,
+                       nk_stream_t stream) {
+    if (bad_dims(B, N, M, dtype) || B == 0 || chunk_size < 0 || !sigma || !W || !eloc || !stats || !grad_W_out)
+        return NK_ERR_INVALID_ARG;
+    const Geometry g = make_geometry(nullptr, N, M, dtype);
+    if (g.M_pad / MPAD_ALIGN > (dtype == NK_C64 ? MAX_V_CPLX : MAX_V_REAL) || N > 65535) return NK_ERR_UNSUPPORTED;
+    const int64_t chunk = eff_chunk(B, chunk_size);
+    size_t need = 0;
+    carve_grad(nullptr, g, chunk, &need);
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < need) return NK_ERR_WORKSPACE;
+    const GradWs w = carve_grad(workspace, g, chunk, &need);
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t esz = dtype == NK_C64 ? 8 : 4;
+    NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.Wg, w.bg, st));
+    NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
+    int first = 1;
+    for (int64_t s0 = 0; s0 < B; s0 += chunk) {
+        const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
+        const int8_t* sg = sigma + s0 * N;
+        NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.Ws, w.A, w.bg, w.theta, st));
+        NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B, (const uint8_t*)eloc + s0 * esz, stats, w, first, st));
+        first = 0;
+    }
+    NK_CUDA(launch_gradient_finalize(g, dtype, w, grad_a_out, grad_b_out, grad_W_out, st));
     return NK_OK;
 }
 

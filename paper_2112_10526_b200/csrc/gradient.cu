@@ -1,0 +1,222 @@
+// Force vector / energy gradient of the RBM.
+//   O_i(s) = d ln psi(s) / d theta_i                      PAPER.md Eq. (13)
+//   f~_i   = E[O_i^* (H~ - E[H~])]                        Eq. (14), Eq. (26)
+//   grad   = 2 Re f~ (real parameters) | f~ (complex, holomorphic)   Eq. (15)/(16) L664-668, Eq. (27)/(28) L918-922
+// RBM closed form: O_a = s, O_b = tanh(theta), O_W = tanh(theta) s^T, so with w_s = (E_loc(s) - mean) / B
+//   g_a[k] = sum_s s_k w_s,  g_b[j] = sum_s conj(T_sj) w_s,  g_W[j][k] = sum_s conj(T_sj) w_s s_k   (x2, real part, for real parameters).
+// g_W is a dense contraction over the samples -- tensor-core work: per chunk the values v_sj = conj(T_sj) w_s are split
+// on three fixed-point bf16 grids (as W is in theta_tc.cu; sigma = +-1 is exact), written k-contiguous (k = sample),
+// and contracted with sigma^T by the same tcgen05 kernel, accumulating [N][M_eff] in fp32 across chunks.
+// g_a and g_b are fp64 column sums with a fixed order (bit-reproducible).
+#include <cuda_bf16.h>
+
+#include "nk_internal.h"
+
+namespace nk {
+
+// w_s = (E_loc(s) - mean) / B in fp64 -> fp32 (complex: both parts)
+__device__ __forceinline__ void sample_weight(const float* __restrict__ eloc, const double* __restrict__ stats,
+                                              int64_t s, double inv_B, bool cplx, float& wr, float& wi) {
+    if (cplx) {
+        wr = (float)(((double)eloc[2 * s] - stats[0]) * inv_B);
+        wi = (float)(((double)eloc[2 * s + 1] - stats[1]) * inv_B);
+    } else {
+        wr = (float)(((double)eloc[s] - stats[0]) * inv_B);
+        wi = 0.f;
+    }
+}
+
+// theta[s][.] -> v[s][.] in place (complex: plane 0 = Re v, plane 1 = Im v), and max |v| as float bits
+template <bool CPLX>
+__global__ void grad_tv_kernel(float* __restrict__ theta, int64_t nb, int M, int M_pad, int M_eff,
+                               const float* __restrict__ eloc, const double* __restrict__ stats, double inv_B,
+                               unsigned* __restrict__ absmax) {
+    unsigned m = 0;
+    for (int64_t s = blockIdx.y; s < nb; s += gridDim.y) {
+    float wr, wi;
+    sample_weight(eloc, stats, s, inv_B, CPLX, wr, wi);
+    float* row = theta + s * M_eff;
+    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < M_pad; j += gridDim.x * blockDim.x) {
+        if (!CPLX) {
+            const float v = (j < M) ? 2.f * tanhf(row[j]) * wr : 0.f;
+            row[j] = v;
+            m = max(m, __float_as_uint(fabsf(v)));
+        } else {
+            float vr = 0.f, vi = 0.f;
+            if (j < M) {
+                // tanh(x + i y) = [sign(x)(1 - e^2) + i 2 e sin 2y] / (1 + e^2 + 2 e cos 2y),  e = exp(-2|x|)
+                const float x = row[j], y = row[M_pad + j];
+                const float e = expf(-2.f * fabsf(x));
+                float sn, cs;
+                sincosf(2.f * y, &sn, &cs);
+                const float den = 1.f / (1.f + e * e + 2.f * e * cs);
+                const float tr = copysignf((1.f - e) * (1.f + e), x) * den, ti = 2.f * e * sn * den;
+                vr = tr * wr + ti * wi;                   // conj(T) * w
+                vi = tr * wi - ti * wr;
+            }
+            row[j] = vr; row[M_pad + j] = vi;
+            m = max(m, max(__float_as_uint(fabsf(vr)), __float_as_uint(fabsf(vi))));
+        }
+    }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(absmax, m);
+}
+
+// gb_acc[me] (+)= sum_s v[s][me]   (one thread per column, samples in order: deterministic)
+__global__ void grad_colsum_kernel(const float* __restrict__ v, int64_t nb, int M_eff, double* __restrict__ gb_acc,
+                                   int first) {
+    const int me = blockIdx.x * blockDim.x + threadIdx.x;
+    if (me >= M_eff) return;
+    double acc = first ? 0.0 : gb_acc[me];
+    for (int64_t s = 0; s < nb; ++s) acc += (double)v[s * M_eff + me];
+    gb_acc[me] = acc;
+}
+
+// ga_acc[plane][k] (+)= sum_s sigma[s][k] w_s[plane]   (x2 for real parameters)
+__global__ void grad_a_kernel(const int8_t* __restrict__ sigma, int64_t nb, int N, const float* __restrict__ eloc,
+                              const double* __restrict__ stats, double inv_B, int cplx, double* __restrict__ ga_acc,
+                              int first) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    double ar = first ? 0.0 : ga_acc[k], ai = first ? 0.0 : ga_acc[N + k];
+    const double f = cplx ? 1.0 : 2.0;
+    for (int64_t s = 0; s < nb; ++s) {
+        float wr, wi;
+        sample_weight(eloc, stats, s, inv_B, cplx != 0, wr, wi);
+        const double sg = (double)sigma[s * N + k];
+        ar += f * sg * (double)wr;
+        ai += sg * (double)wi;
+    }
+    ga_acc[k] = ar; ga_acc[N + k] = ai;
+}
+
+// TwT[piece][me][s] (bf16, k-contiguous, leading dimension ld) from v[s][me]: fixed-point split on the grids
+// 2^e1, 2^(e1-8), 2^(e1-16), 2^(e1+8) > max|v|; rows s in [nb, k_len) are zero
+__global__ void grad_split_T_kernel(const float* __restrict__ v, int64_t nb, int k_len, int M_eff, int ld,
+                                    const unsigned* __restrict__ absmax_bits, __nv_bfloat16* __restrict__ TwT) {
+    __shared__ float tile[32][33];
+    const float vmax = __uint_as_float(*absmax_bits);
+    int ex = -100;
+    if (vmax > 0.f) frexpf(vmax, &ex);
+    const float q1 = ldexpf(1.f, ex - 8), q2 = ldexpf(1.f, ex - 16), q3 = ldexpf(1.f, ex - 24);
+    const float s1 = ldexpf(1.f, 8 - ex), s2 = ldexpf(1.f, 16 - ex), s3 = ldexpf(1.f, 24 - ex);
+    const int s0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int64_t s = s0 + r;
+        tile[r][threadIdx.x] = (s < nb) ? v[s * M_eff + m0 + threadIdx.x] : 0.f;
+    }
+    __syncthreads();
+    const size_t plane = (size_t)M_eff * ld;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int me = m0 + r, s = s0 + threadIdx.x;
+        if (s >= k_len) continue;
+        float w = tile[threadIdx.x][r];
+        const float hi = rintf(w * s1) * q1;
+        w -= hi;
+        const float mid = rintf(w * s2) * q2;
+        w -= mid;
+        const float lo = rintf(w * s3) * q3;
+        const size_t o = (size_t)me * ld + s;
+        TwT[o] = __float2bfloat16_rn(hi);
+        TwT[plane + o] = __float2bfloat16_rn(mid);
+        TwT[2 * plane + o] = __float2bfloat16_rn(lo);
+    }
+}
+
+// sigT[k][s] = (bf16) sigma[s][k], zero for s in [nb, k_len)
+__global__ void grad_sigma_T_kernel(const int8_t* __restrict__ sigma, int64_t nb, int k_len, int N, int ld,
+                                    __nv_bfloat16* __restrict__ sigT) {
+    __shared__ int8_t tile[32][33];
+    const int s0 = blockIdx.x * 32, k0 = blockIdx.y * 32;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int64_t s = s0 + r;
+        const int k = k0 + threadIdx.x;
+        tile[r][threadIdx.x] = (s < nb && k < N) ? sigma[s * N + k] : (int8_t)0;
+    }
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int k = k0 + r, s = s0 + threadIdx.x;
+        if (k < N && s < k_len) sigT[(size_t)k * ld + s] = __float2bfloat16_rn((float)tile[threadIdx.x][r]);
+    }
+}
+
+// g_W[j][k] = Gacc[k][j] (complex: (Gacc[k][j], Gacc[k][M_pad + j]) interleaved); 32x32 tiles through shared memory
+__global__ void grad_finalize_W_kernel(const float* __restrict__ Gacc, int N, int M, int M_pad, int M_eff, int cplx,
+                                       float* __restrict__ gW) {
+    __shared__ float tr[32][33], ti[32][33];
+    const int j0 = blockIdx.x * 32, k0 = blockIdx.y * 32;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int k = k0 + r, j = j0 + threadIdx.x;
+        const bool ok = k < N && j < M;
+        tr[r][threadIdx.x] = ok ? Gacc[(size_t)k * M_eff + j] : 0.f;
+        ti[r][threadIdx.x] = (ok && cplx) ? Gacc[(size_t)k * M_eff + M_pad + j] : 0.f;
+    }
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int j = j0 + r, k = k0 + threadIdx.x;
+        if (j < M && k < N) {
+            if (cplx) {
+                gW[((size_t)j * N + k) * 2] = tr[threadIdx.x][r];
+                gW[((size_t)j * N + k) * 2 + 1] = ti[threadIdx.x][r];
+            } else gW[(size_t)j * N + k] = tr[threadIdx.x][r];
+        }
+    }
+}
+
+__global__ void grad_finalize_ab_kernel(const double* __restrict__ ga_acc, const double* __restrict__ gb_acc, int N,
+                                        int M, int M_pad, int cplx, float* __restrict__ ga, float* __restrict__ gb) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ga != nullptr && i < N) {
+        if (cplx) { ga[2 * i] = (float)ga_acc[i]; ga[2 * i + 1] = (float)ga_acc[N + i]; }
+        else ga[i] = (float)ga_acc[i];
+    }
+    if (gb != nullptr && i < M) {
+        if (cplx) { gb[2 * i] = (float)gb_acc[i]; gb[2 * i + 1] = (float)gb_acc[M_pad + i]; }
+        else gb[i] = (float)gb_acc[i];
+    }
+}
+
+cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, int64_t B_total,
+                                  const void* eloc, const double* stats, const GradWs& w, int first_chunk,
+                                  cudaStream_t st) {
+    if (nb <= 0) return cudaSuccess;
+    const bool cplx = dtype == NK_C64;
+    const double inv_B = 1.0 / (double)B_total;
+    const int k_len = (int)((nb + 63) / 64 * 64);
+    cudaError_t e = cudaMemsetAsync(w.absmax, 0, sizeof(unsigned), st);
+    if (e != cudaSuccess) return e;
+    dim3 gtv((g.M_pad + 255) / 256, (unsigned)(nb < 32768 ? nb : 32768));
+    if (cplx)
+        grad_tv_kernel<true><<<gtv, 256, 0, st>>>(w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
+                                                  w.absmax);
+    else
+        grad_tv_kernel<false><<<gtv, 256, 0, st>>>(w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
+                                                   w.absmax);
+    grad_colsum_kernel<<<(g.M_eff + 63) / 64, 64, 0, st>>>(w.theta, nb, g.M_eff, w.gb_acc, first_chunk);
+    grad_a_kernel<<<(g.N + 63) / 64, 64, 0, st>>>(sigma, nb, g.N, (const float*)eloc, stats, inv_B, cplx, w.ga_acc,
+                                                  first_chunk);
+    grad_split_T_kernel<<<dim3(k_len / 32, g.M_eff / 32), dim3(32, 8), 0, st>>>(
+        w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (__nv_bfloat16*)w.TwT);
+    grad_sigma_T_kernel<<<dim3(k_len / 32, (g.N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, g.N, w.ld,
+                                                                                 (__nv_bfloat16*)w.sigT);
+    count_launch(5);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    return launch_tc_gemm_pieces(w.sigT, g.N, w.TwT, g.M_eff, w.ld, k_len, w.Gacc, first_chunk ? 0 : 1, st);
+}
+
+cudaError_t launch_gradient_finalize(const Geometry& g, int dtype, const GradWs& w, void* grad_a, void* grad_b,
+                                     void* grad_W, cudaStream_t st) {
+    const int cplx = dtype == NK_C64;
+    grad_finalize_W_kernel<<<dim3((g.M + 31) / 32, (g.N + 31) / 32), dim3(32, 8), 0, st>>>(
+        w.Gacc, g.N, g.M, g.M_pad, g.M_eff, cplx, (float*)grad_W);
+    const int n = g.N > g.M ? g.N : g.M;
+    grad_finalize_ab_kernel<<<(n + 127) / 128, 128, 0, st>>>(w.ga_acc, w.gb_acc, g.N, g.M, g.M_pad, cplx,
+                                                            (float*)grad_a, (float*)grad_b);
+    count_launch(2);
+    return cudaGetLastError();
+}
+
+}  // namespace nk

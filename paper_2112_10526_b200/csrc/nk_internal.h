@@ -69,6 +69,21 @@ cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* W
                            cudaStream_t st);
 cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, int K_pad, const void* Ws_bf16,
                             void* A_bf16, const float* bg, float* theta, cudaStream_t st);
+cudaError_t launch_tc_gemm_pieces(const void* A_bf16, int64_t rows, const void* P_bf16, int cols, int ld, int k_len,
+                                  float* out, int accumulate, cudaStream_t st);
+// gradient.cu : force vector / energy gradient of the RBM
+struct GradWs {
+    float *Wg, *bg, *theta, *Gacc;
+    uint16_t *Ws, *A, *TwT, *sigT;
+    double *gb_acc, *ga_acc;
+    unsigned* absmax;
+    int ld;                     // k extent (samples per chunk, rounded up to 64) of TwT / sigT
+};
+cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, int64_t B_total,
+                                  const void* eloc, const double* stats, const GradWs& w, int first_chunk,
+                                  cudaStream_t st);
+cudaError_t launch_gradient_finalize(const Geometry& g, int dtype, const GradWs& w, void* grad_a, void* grad_b,
+                                     void* grad_W, cudaStream_t st);
 // logpsi.cu
 cudaError_t launch_logpsi(const int8_t* sigma, int64_t B, const Geometry& g, int dtype, const float* theta,
                           const void* a, void* logpsi_out, bool out_f64, void* theta_out, cudaStream_t st);

@@ -130,7 +130,7 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
 // ---- the GEMM ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(tc::THREADS, 1)
 theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w, int64_t B,
-                int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta) {
+                int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta, int accumulate) {
     using namespace tc;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;            // SWIZZLE_128B needs 1024 B
@@ -214,7 +214,12 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
             if (row < B) {
 #pragma unroll
                 for (int j = 0; j < 32; j += 4) {
-                    const float4 bb = *reinterpret_cast<const float4*>(bg + n0 + c0 + j);
+                    float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (bg != nullptr) bb = *reinterpret_cast<const float4*>(bg + n0 + c0 + j);
+                    if (accumulate) {                      // out += D (the gradient contraction runs over chunks)
+                        const float4 old = *reinterpret_cast<const float4*>(out + c0 + j);
+                        bb.x += old.x; bb.y += old.y; bb.z += old.z; bb.w += old.w;
+                    }
                     float4 o;
                     o.x = (hi[j] + (mid[j] + lo[j])) + bb.x;
                     o.y = (hi[j + 1] + (mid[j + 1] + lo[j + 1])) + bb.y;
@@ -291,8 +296,24 @@ cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, in
     if (!encode_2d(&map_a, A, (uint64_t)B, (uint64_t)K_pad)) return cudaErrorInvalidValue;
     if (!encode_2d(&map_w, Ws, (uint64_t)3 * M_eff, (uint64_t)K_pad)) return cudaErrorInvalidValue;
     dim3 grid(M_eff / tc::BN, (unsigned)((B + tc::BM - 1) / tc::BM));
-    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_w, B, M_eff, K_pad, bg, theta);
+    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_w, B, M_eff, K_pad, bg, theta, 0);
     count_launch(2);
+    return cudaGetLastError();
+}
+
+// Generic entry used by the gradient: out[r][c] (+)= sum_k A[r][k] * (P0 + P1 + P2)[c][k], A bf16 [rows][ld] and
+// P bf16 [3][cols][ld] both k-contiguous, k < k_len (a multiple of 64), cols a multiple of 128.
+cudaError_t launch_tc_gemm_pieces(const void* A, int64_t rows, const void* P, int cols, int ld, int k_len, float* out,
+                                  int accumulate, cudaStream_t st) {
+    if (rows <= 0) return cudaSuccess;
+    cudaError_t e = theta_tc_init();
+    if (e != cudaSuccess) return e;
+    CUtensorMap map_a, map_p;
+    if (!encode_2d(&map_a, A, (uint64_t)rows, (uint64_t)ld)) return cudaErrorInvalidValue;
+    if (!encode_2d(&map_p, P, (uint64_t)3 * cols, (uint64_t)ld)) return cudaErrorInvalidValue;
+    dim3 grid(cols / tc::BN, (unsigned)((rows + tc::BM - 1) / tc::BM));
+    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_p, rows, cols, k_len, nullptr, out, accumulate);
+    count_launch();
     return cudaGetLastError();
 }
 
