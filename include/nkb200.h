@@ -50,6 +50,7 @@ enum nk_status {
 };
 enum nk_kind { NK_HEISENBERG = 0, NK_ISING = 1 };
 enum nk_dtype { NK_F32 = 0, NK_C64 = 1 };
+enum nk_rule { NK_RULE_LOCAL = 0, NK_RULE_EXCHANGE = 1 };
 enum nk_flags {
     NK_FLAG_MARSHALL = 1u,     /* nk_operator_create: off-diagonal Heisenberg element -2J (default +2J, Eq. (50)) */
     NK_OUT_F64 = 2u            /* nk_rbm_logpsi: logpsi_out is double / (re,im) double instead of float */
@@ -134,6 +135,28 @@ int nk_energy_gradient(const int8_t* sigma, int64_t B, int N, int M, int dtype, 
                        const void* eloc, const double* stats, int64_t chunk_size, void* grad_a_out,
                        void* grad_b_out, void* grad_W_out, void* workspace, size_t workspace_bytes,
                        nk_stream_t stream);
+
+/* ---- Metropolis-Hastings sampler for the RBM ------------------------------------------
+ * PAPER.md Sec. 3.4: a proposal s -> s' is accepted with probability min(1, |psi(s')|^2 / |psi(s)|^2) (Eq. (20)
+ * L709; both rules are symmetric kernels, L711).  Every row of sigma is one chain (n_chains = n_samples, L1583);
+ * the call advances each chain by n_steps transitions IN PLACE (one sweep = N transitions, footnote 20 L1590).
+ *   NK_RULE_LOCAL     negate one uniformly drawn spin (MetropolisLocal, L713); clusters_host = NULL, n_clusters = 0
+ *   NK_RULE_EXCHANGE  swap the spins of one uniformly drawn pair of clusters_host [n_clusters][2] (HOST pointer,
+ *                     0 <= i != j < N; e.g. the lattice bonds: MetropolisExchange with graph=lattice, L1600); a
+ *                     pair of equal spins proposes s' = s, which is accepted and counted
+ * Random numbers are a pure function of (seed, chain index, transition index): Philox4x32-10 with counter
+ * (chain lo, hi, transition lo, hi) and key (seed lo, hi) gives (r0, r1, ..); proposal = (r0 * n) >> 32,
+ * u = ((r1 >> 9) + 1/2) 2^-23, accept iff u < |psi'/psi|^2 evaluated in fp32.  Row r of sigma is chain
+ * chain_offset + r; its t-th transition of this call has index step_offset + t, so consecutive calls continue a
+ * stream and a sharded batch reproduces the unsharded one.  Results do not depend on chunk_size (chains are
+ * processed chunk_size at a time, 0 = all at once; the workspace scales with min(B, chunk_size)).
+ *   sigma         dev [B][N] int8, in/out        accepted_out  NULL or dev int32 [B]: accepted transitions of this call
+ * theta is contracted once per call from sigma and then updated incrementally in registers (fp32). */
+size_t nk_metropolis_workspace_bytes(int rule, int n_clusters, int64_t B, int N, int M, int dtype, int64_t chunk_size);
+int nk_metropolis_sample(int rule, const int32_t* clusters_host, int n_clusters, int8_t* sigma, int64_t B, int N,
+                         int M, int dtype, const void* W, const void* a, const void* b, int64_t n_steps,
+                         uint64_t seed, uint64_t step_offset, uint64_t chain_offset, int64_t chunk_size,
+                         int32_t* accepted_out, void* workspace, size_t workspace_bytes, nk_stream_t stream);
 
 /* Per-phase device timing (bench accounting).  With nk_profile_enable(1), nk_local_energy brackets each phase
  * of each chunk with CUDA events on the call's stream (a few microseconds of timeline each).  nk_profile_read

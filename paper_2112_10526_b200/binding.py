@@ -11,15 +11,17 @@ import os
 import numpy as np
 
 __all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host", "energy_gradient",
-           "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
+           "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
            "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "EXPORTS"]
 
 NK_HEISENBERG, NK_ISING = 0, 1
 NK_F32, NK_C64 = 0, 1
 NK_FLAG_MARSHALL, NK_OUT_F64 = 1, 2
+NK_RULE_LOCAL, NK_RULE_EXCHANGE = 0, 1
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libnkb200.so")
 
 _vp, _i64, _int, _sz, _u32, _dbl = C.c_void_p, C.c_int64, C.c_int, C.c_size_t, C.c_uint, C.c_double
+_u64 = C.c_uint64
 # name -> (restype, argtypes): every symbol include/nkb200.h declares
 EXPORTS = {
     "nk_status_string": (C.c_char_p, [_int]),
@@ -37,6 +39,9 @@ EXPORTS = {
     "nk_local_energy_host": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_energy_gradient_workspace_bytes": (_sz, [_i64, _int, _int, _int, _i64]),
     "nk_energy_gradient": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "nk_metropolis_workspace_bytes": (_sz, [_int, _int, _i64, _int, _int, _int, _i64]),
+    "nk_metropolis_sample": (_int, [_int, _vp, _int, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _u64, _u64, _u64,
+                                    _i64, _vp, _vp, _sz, _vp]),
     "nk_launch_count": (_i64, [_int]),
     "nk_profile_enable": (_int, [_int]),
     "nk_profile_read": (_int, [_vp]),
@@ -274,6 +279,36 @@ def energy_gradient(sigma, W, b, eloc, stats, *, chunk_size: int = 0, ws=None):
                                 _ptr(ga), _ptr(gb), _ptr(gW), _ptr(ws), ws.numel(), _stream())
     _check(rc, "nk_energy_gradient")
     return ga, gb, gW
+
+
+def metropolis_sample(sigma, W, a=None, b=None, *, rule: int = NK_RULE_LOCAL, clusters=None, n_steps: int | None = None,
+                      seed: int = 0, step_offset: int = 0, chain_offset: int = 0, chunk_size: int = 0, ws=None):
+    """nk_metropolis_sample: advances every row of `sigma` (device int8 [B][N], modified IN PLACE) by n_steps
+    Metropolis-Hastings transitions (default: one sweep = N).  `clusters`: host int32 [n][2] pairs for
+    NK_RULE_EXCHANGE (e.g. the lattice bonds).  Returns the accepted-transition counts, device int32 [B]."""
+    torch = _torch()
+    lib = load()
+    _check_params(sigma, W, a, b)
+    B, N = sigma.shape
+    M = W.shape[0]
+    dt = _dtype_code(W)
+    if n_steps is None:
+        n_steps = N
+    cl, n_cl = None, 0
+    if clusters is not None:
+        cl = np.ascontiguousarray(np.asarray(clusters), dtype=np.int32).reshape(-1, 2)
+        n_cl = int(cl.shape[0])
+    nbytes = lib.nk_metropolis_workspace_bytes(int(rule), n_cl, B, N, M, dt, int(chunk_size))
+    if nbytes == 0:
+        raise NkError("nk_metropolis_workspace_bytes rejected the arguments")
+    if ws is None or ws.numel() < nbytes:
+        ws = torch.empty(nbytes, dtype=torch.uint8, device=sigma.device)
+    accepted = torch.empty(B, dtype=torch.int32, device=sigma.device)
+    rc = lib.nk_metropolis_sample(int(rule), None if cl is None else cl.ctypes.data, n_cl, _ptr(sigma), B, N, M, dt,
+                                  _ptr(W), _ptr(a), _ptr(b), int(n_steps), int(seed), int(step_offset),
+                                  int(chain_offset), int(chunk_size), _ptr(accepted), _ptr(ws), ws.numel(), _stream())
+    _check(rc, "nk_metropolis_sample")
+    return accepted
 
 
 def launch_count(reset: bool = False) -> int:

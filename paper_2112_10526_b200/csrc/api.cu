@@ -147,6 +147,29 @@ static GradWs carve_grad(void* ws, const Geometry& g, int64_t chunk, size_t* byt
     return w;
 }
 
+struct SamplerWs {
+    float *Wg, *bg, *Wt, *Dtab, *theta;
+    uint16_t *Ws, *A;
+    unsigned* absmax;
+    int32_t* pairs;
+    size_t bytes;
+};
+static SamplerWs carve_sampler(void* ws, const Geometry& g, int n_rows, int64_t chunk) {
+    Carver c(ws);
+    SamplerWs w;
+    w.Wg = c.take<float>((size_t)g.M_eff * g.N);
+    w.bg = c.take<float>(g.M_eff);
+    w.Wt = c.take<float>((size_t)g.N * g.M_eff);
+    w.Dtab = c.take<float>((size_t)n_rows * g.M_eff);
+    w.theta = c.take<float>((size_t)chunk * g.M_eff);
+    w.Ws = c.take<uint16_t>((size_t)3 * g.M_eff * g.K_pad);
+    w.A = c.take<uint16_t>((size_t)chunk * g.K_pad);
+    w.absmax = c.take<unsigned>(1);
+    w.pairs = c.take<int32_t>((size_t)2 * n_rows);
+    w.bytes = c.off;
+    return w;
+}
+
 // NK_THETA_SIMT=1 selects the FP32 SIMT contraction (debugging aid); default is the tcgen05 path.
 static bool use_simt_theta() {
     static const bool v = [] { const char* e = std::getenv("NK_THETA_SIMT"); return e && e[0] == '1'; }();
@@ -336,6 +359,57 @@ int nk_energy_gradient(const int8_t* sigma, int64_t B, int N, int M, int dtype, 
 static int64_t eff_chunk(int64_t B, int64_t chunk_size) {
     if (chunk_size <= 0 || chunk_size > B) return B > 0 ? B : 1;
     return chunk_size;
+}
+
+static bool bad_rule(int rule, int n_clusters) {
+    return (rule != NK_RULE_LOCAL && rule != NK_RULE_EXCHANGE) || n_clusters < 0 ||
+           (rule == NK_RULE_EXCHANGE && n_clusters == 0);
+}
+
+size_t nk_metropolis_workspace_bytes(int rule, int n_clusters, int64_t B, int N, int M, int dtype, int64_t chunk_size) {
+    if (bad_dims(B, N, M, dtype) || chunk_size < 0 || bad_rule(rule, n_clusters)) return 0;
+    const Geometry g = make_geometry(nullptr, N, M, dtype);
+    return carve_sampler(nullptr, g, rule == NK_RULE_LOCAL ? N : n_clusters, eff_chunk(B, chunk_size)).bytes;
+}
+
+int nk_metropolis_sample(int rule, const int32_t* clusters_host, int n_clusters, int8_t* sigma, int64_t B, int N,
+                         int M, int dtype, const void* W, const void* a, const void* b, int64_t n_steps,
+                         uint64_t seed, uint64_t step_offset, uint64_t chain_offset, int64_t chunk_size,
+                         int32_t* accepted_out, void* workspace, size_t workspace_bytes, nk_stream_t stream) {
+    if (bad_dims(B, N, M, dtype) || chunk_size < 0 || n_steps < 0 || bad_rule(rule, n_clusters) || !W ||
+        (B > 0 && !sigma) || (rule == NK_RULE_EXCHANGE && !clusters_host))
+        return NK_ERR_INVALID_ARG;
+    if (rule == NK_RULE_EXCHANGE)
+        for (int c = 0; c < n_clusters; ++c) {
+            const int i = clusters_host[2 * c], j = clusters_host[2 * c + 1];
+            if (i < 0 || j < 0 || i >= N || j >= N || i == j) return NK_ERR_INVALID_ARG;
+        }
+    const Geometry g = make_geometry(nullptr, N, M, dtype);
+    if (g.M_pad / MPAD_ALIGN > (dtype == NK_C64 ? MAX_V_CPLX : MAX_V_REAL) || N > 65535) return NK_ERR_UNSUPPORTED;
+    if (B == 0) return NK_OK;
+    const int n_rows = rule == NK_RULE_LOCAL ? N : n_clusters;
+    const int64_t chunk = eff_chunk(B, chunk_size);
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_sampler(nullptr, g, n_rows, chunk).bytes)
+        return NK_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const SamplerWs w = carve_sampler(workspace, g, n_rows, chunk);
+    if (rule == NK_RULE_EXCHANGE)
+        NK_CUDA(cudaMemcpyAsync(w.pairs, clusters_host, (size_t)2 * n_clusters * sizeof(int32_t),
+                                cudaMemcpyHostToDevice, st));
+    NK_CUDA(launch_pack_table(g, dtype, W, b, rule == NK_RULE_EXCHANGE ? w.pairs : nullptr, n_rows, w.Wg, w.bg, w.Wt,
+                              w.Dtab, st));
+    NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
+    SamplerArgs sa;
+    sa.rule = rule; sa.n_idx = n_rows; sa.pairs = rule == NK_RULE_EXCHANGE ? w.pairs : nullptr; sa.a = a;
+    sa.n_steps = n_steps; sa.seed = seed; sa.step_offset = step_offset;
+    for (int64_t s0 = 0; s0 < B; s0 += chunk) {
+        const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
+        int8_t* sg = sigma + s0 * N;
+        sa.chain0 = chain_offset + (uint64_t)s0;
+        NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.Ws, w.A, w.bg, w.theta, st));
+        NK_CUDA(launch_metropolis(g, dtype, sg, nb, w.theta, w.Dtab, sa, accepted_out ? accepted_out + s0 : nullptr, st));
+    }
+    return NK_OK;
 }
 
 size_t nk_local_energy_workspace_bytes(nk_operator_t h, int64_t B, int N, int M, int dtype, int64_t chunk_size) {

@@ -23,6 +23,7 @@
 
 #include "nk_internal.h"
 #include "ptx_helpers.cuh"
+#include "rbm_lane_state.cuh"
 
 namespace nk {
 
@@ -45,189 +46,6 @@ struct FusedParams {
     float* eloc;
     int64_t per_cta;                         // samples per CTA (contiguous range)
 };
-
-__device__ __forceinline__ float warp_sum_f(float v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-__device__ __forceinline__ float warp_prod_f(float v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v *= __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// ---- per-row inner loops ---------------------------------------------------------------------------------
-template <int V>
-struct RealState {
-    float4 th[V];      // theta_s
-    float qinv;        // 1 / prod_{j in lane} (1 + e_j)
-
-    __device__ __forceinline__ void load(const float* __restrict__ row, int lane, int /*M_pad*/) {
-        float p0 = 1.f, p1 = 1.f, p2 = 1.f, p3 = 1.f;
-#pragma unroll
-        for (int v = 0; v < V; ++v) {
-            float4 t = *reinterpret_cast<const float4*>(row + (v * 32 + lane) * 4);
-            t.x *= KAPPA; t.y *= KAPPA; t.z *= KAPPA; t.w *= KAPPA;
-            th[v] = t;
-            p0 = fmaf(p0, ex2_approx(-fabsf(t.x)), p0);
-            p1 = fmaf(p1, ex2_approx(-fabsf(t.y)), p1);
-            p2 = fmaf(p2, ex2_approx(-fabsf(t.z)), p2);
-            p3 = fmaf(p3, ex2_approx(-fabsf(t.w)), p3);
-        }
-        qinv = 1.f / ((p0 * p1) * (p2 * p3));
-    }
-    // this lane's share of psi'/psi for one row: r = prod_{j in lane} (1+e'_j)/(1+e_j), acc = sum_j (|x'_j| - |x_j|)
-    __device__ __forceinline__ void partial(const float* __restrict__ drow, int lane, float s, float& r,
-                                            float& acc) const {
-        float p0 = 1.f, p1 = 1.f, p2 = 1.f, p3 = 1.f, acc0 = 0.f, acc1 = 0.f;
-#pragma unroll
-        for (int v = 0; v < V; ++v) {
-            const float4 d = *reinterpret_cast<const float4*>(drow + (v * 32 + lane) * 4);
-            const float4 t = th[v];
-            const float x0 = fmaf(s, d.x, t.x), x1 = fmaf(s, d.y, t.y);
-            const float x2 = fmaf(s, d.z, t.z), x3 = fmaf(s, d.w, t.w);
-            p0 = fmaf(p0, ex2_approx(-fabsf(x0)), p0);
-            p1 = fmaf(p1, ex2_approx(-fabsf(x1)), p1);
-            p2 = fmaf(p2, ex2_approx(-fabsf(x2)), p2);
-            p3 = fmaf(p3, ex2_approx(-fabsf(x3)), p3);
-            acc0 += fabsf(x0) - fabsf(t.x);
-            acc1 += fabsf(x1) - fabsf(t.y);
-            acc0 += fabsf(x2) - fabsf(t.z);
-            acc1 += fabsf(x3) - fabsf(t.w);
-        }
-        r = ((p0 * p1) * (p2 * p3)) * qinv;
-        acc = acc0 + acc1;
-    }
-};
-
-// One pending row of a sample: lane partials plus the row's scalars.  Rows are reduced across the warp two at a
-// time: after the first exchange (lane ^ 16) the lower half-warp owns row A and the upper half row B, so the
-// five butterfly levels cost 10 shuffles per PAIR of rows instead of 10 per row, and the two rows' serial
-// reduction latencies overlap.
-struct RowPartR {
-    float r, acc, ex, coef;     // ex = s * a2 (visible-bias exponent, log2 units)
-};
-__device__ __forceinline__ float finish_pair(const RowPartR& A, const RowPartR& B, int lane) {
-    const bool up = (lane & 16) != 0;
-    float rk = up ? B.r : A.r, ak = up ? B.acc : A.acc;
-    const float rs = up ? A.r : B.r, as = up ? A.acc : B.acc;
-    rk *= __shfl_xor_sync(0xffffffffu, rs, 16);
-    ak += __shfl_xor_sync(0xffffffffu, as, 16);
-#pragma unroll
-    for (int o = 8; o > 0; o >>= 1) {
-        rk *= __shfl_xor_sync(0xffffffffu, rk, o);
-        ak += __shfl_xor_sync(0xffffffffu, ak, o);
-    }
-    const float ex = up ? B.ex : A.ex, c = up ? B.coef : A.coef;
-    return c * (rk * ex2_approx(fmaf(0.5f, ak, ex)));   // lower half: row A's term, upper half: row B's
-}
-__device__ __forceinline__ float finish_single(const RowPartR& A) {
-    const float r = warp_prod_f(A.r), acc = warp_sum_f(A.acc);
-    return A.coef * (r * ex2_approx(fmaf(0.5f, acc, A.ex)));
-}
-
-template <int V>
-struct CplxState {
-    float4 tx[V], ty[V];   // Re theta_s (scaled), Im theta (radians)
-    float qr, qi;          // 1 / prod_{j in lane} f_j
-
-    static __device__ __forceinline__ void factor(float x, float y, float& p, float& q) {
-        const float e = ex2_approx(-fabsf(x));
-        float sn, cs;
-        __sincosf(y, &sn, &cs);
-        p = fmaf(e, cs, cs);                      // (1+e) cos y
-        q = fmaf(-e, sn, sn);                     // (1-e) sin y
-        q = __int_as_float(__float_as_int(q) ^ (__float_as_int(x) & 0x80000000));   // times sign(x)
-    }
-    static __device__ __forceinline__ void cmul(float& ar, float& ai, float br, float bi) {
-        const float r = fmaf(ar, br, -ai * bi), i = fmaf(ar, bi, ai * br);
-        ar = r; ai = i;
-    }
-    __device__ __forceinline__ void load(const float* __restrict__ row, int lane, int M_pad) {
-        float ar = 1.f, ai = 0.f, br = 1.f, bi = 0.f;
-#pragma unroll
-        for (int v = 0; v < V; ++v) {
-            float4 x = *reinterpret_cast<const float4*>(row + (v * 32 + lane) * 4);
-            const float4 y = *reinterpret_cast<const float4*>(row + M_pad + (v * 32 + lane) * 4);
-            x.x *= KAPPA; x.y *= KAPPA; x.z *= KAPPA; x.w *= KAPPA;
-            tx[v] = x; ty[v] = y;
-            float p, q;
-            factor(x.x, y.x, p, q); cmul(ar, ai, p, q);
-            factor(x.y, y.y, p, q); cmul(br, bi, p, q);
-            factor(x.z, y.z, p, q); cmul(ar, ai, p, q);
-            factor(x.w, y.w, p, q); cmul(br, bi, p, q);
-        }
-        cmul(ar, ai, br, bi);
-        const float inv = 1.f / fmaf(ar, ar, ai * ai);
-        qr = ar * inv; qi = -ai * inv;
-    }
-    // this lane's share: (ar + i ai) = prod_{j in lane} f'_j / f_j, acc = sum_j (|x'_j| - |x_j|)
-    __device__ __forceinline__ void partial(const float* __restrict__ drow, int lane, int M_pad, float s, float& ar,
-                                            float& ai, float& acc) const {
-        float br = 1.f, bi = 0.f;
-        ar = 1.f; ai = 0.f; acc = 0.f;
-#pragma unroll
-        for (int v = 0; v < V; ++v) {
-            const float4 dx = *reinterpret_cast<const float4*>(drow + (v * 32 + lane) * 4);
-            const float4 dy = *reinterpret_cast<const float4*>(drow + M_pad + (v * 32 + lane) * 4);
-            const float4 x = tx[v], y = ty[v];
-            float p, q;
-            const float x0 = fmaf(s, dx.x, x.x), x1 = fmaf(s, dx.y, x.y);
-            const float x2 = fmaf(s, dx.z, x.z), x3 = fmaf(s, dx.w, x.w);
-            factor(x0, fmaf(s, dy.x, y.x), p, q); cmul(ar, ai, p, q);
-            factor(x1, fmaf(s, dy.y, y.y), p, q); cmul(br, bi, p, q);
-            factor(x2, fmaf(s, dy.z, y.z), p, q); cmul(ar, ai, p, q);
-            factor(x3, fmaf(s, dy.w, y.w), p, q); cmul(br, bi, p, q);
-            acc += (fabsf(x0) - fabsf(x.x)) + (fabsf(x1) - fabsf(x.y));
-            acc += (fabsf(x2) - fabsf(x.z)) + (fabsf(x3) - fabsf(x.w));
-        }
-        cmul(ar, ai, br, bi);
-        cmul(ar, ai, qr, qi);
-    }
-    static __device__ __forceinline__ void cmul_pub(float& ar, float& ai, float br, float bi) { cmul(ar, ai, br, bi); }
-};
-
-struct RowPartC {
-    float ar, ai, acc, ex_re, ex_im, coef;   // ex_re = s a2_re (log2 units), ex_im = s a2_im (radians)
-};
-__device__ __forceinline__ void cmul_f(float& ar, float& ai, float br, float bi) {
-    const float r = fmaf(ar, br, -ai * bi), i = fmaf(ar, bi, ai * br);
-    ar = r; ai = i;
-}
-__device__ __forceinline__ void finish_c(float ar, float ai, float acc, float ex_re, float ex_im, float c,
-                                         float& out_re, float& out_im) {
-    const float mag = c * ex2_approx(fmaf(0.5f, acc, ex_re));
-    float sn, cs;
-    __sincosf(ex_im, &sn, &cs);
-    cmul_f(ar, ai, mag * cs, mag * sn);
-    out_re = ar; out_im = ai;
-}
-__device__ __forceinline__ void finish_pair_c(const RowPartC& A, const RowPartC& B, int lane, float& out_re,
-                                              float& out_im) {
-    const bool up = (lane & 16) != 0;
-    float kr = up ? B.ar : A.ar, ki = up ? B.ai : A.ai, ka = up ? B.acc : A.acc;
-    const float sr = up ? A.ar : B.ar, si = up ? A.ai : B.ai, sa = up ? A.acc : B.acc;
-    cmul_f(kr, ki, __shfl_xor_sync(0xffffffffu, sr, 16), __shfl_xor_sync(0xffffffffu, si, 16));
-    ka += __shfl_xor_sync(0xffffffffu, sa, 16);
-#pragma unroll
-    for (int o = 8; o > 0; o >>= 1) {
-        const float orr = __shfl_xor_sync(0xffffffffu, kr, o), oi = __shfl_xor_sync(0xffffffffu, ki, o);
-        cmul_f(kr, ki, orr, oi);
-        ka += __shfl_xor_sync(0xffffffffu, ka, o);
-    }
-    finish_c(kr, ki, ka, up ? B.ex_re : A.ex_re, up ? B.ex_im : A.ex_im, up ? B.coef : A.coef, out_re, out_im);
-}
-__device__ __forceinline__ void finish_single_c(const RowPartC& A, float& out_re, float& out_im) {
-    float ar = A.ar, ai = A.ai, acc = A.acc;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        const float orr = __shfl_xor_sync(0xffffffffu, ar, o), oi = __shfl_xor_sync(0xffffffffu, ai, o);
-        cmul_f(ar, ai, orr, oi);
-        acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    }
-    finish_c(ar, ai, acc, A.ex_re, A.ex_im, A.coef, out_re, out_im);
-}
 
 // ---- kernel ----------------------------------------------------------------------------------------------
 template <int V, bool CPLX>

@@ -60,6 +60,18 @@ cudaError_t launch_pack(const Operator* op, const Geometry& g, int dtype, const 
                         float* Wg, float* bg, float* Wt, float* Dtab, RowInfo* rows, cudaStream_t st);
 cudaError_t launch_pack_gemm_only(const Geometry& g, int dtype, const void* W, const void* b, float* Wg, float* bg,
                                   cudaStream_t st);
+cudaError_t launch_pack_table(const Geometry& g, int dtype, const void* W, const void* b, const int32_t* pairs_dev,
+                              int n_rows, float* Wg, float* bg, float* Wt, float* Dtab, cudaStream_t st);
+// sampler.cu : Metropolis-Hastings transitions with in-register incremental theta
+struct SamplerArgs {
+    int rule, n_idx;                 // NK_RULE_*; number of proposals (N sites or n_clusters pairs)
+    const int32_t* pairs;            // dev [n_idx][2] (exchange) or nullptr (local)
+    const void* a;                   // dev visible bias in the parameter dtype, or nullptr
+    int64_t n_steps;
+    uint64_t seed, step_offset, chain0;
+};
+cudaError_t launch_metropolis(const Geometry& g, int dtype, int8_t* sigma, int64_t nb, const float* theta,
+                              const float* Dtab, const SamplerArgs& sa, int32_t* accepted, cudaStream_t st);
 // theta_gemm.cu : theta[s][m] = bg[m] + sum_k sigma[s][k] Wg[m][k]
 cudaError_t launch_theta_gemm(const int8_t* sigma, int64_t B, int N, int M_eff, const float* Wg, const float* bg,
                               float* theta, cudaStream_t st);

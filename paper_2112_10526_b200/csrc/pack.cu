@@ -120,3 +120,21 @@ cudaError_t launch_pack(const Operator* op, const Geometry& g, int dtype, const 
 }
 
 }  // namespace nk
+
+namespace nk {
+
+// Table for the Metropolis sampler (sampler.cu): Wg, bg, Wt as above and one row of Dtab per proposal —
+// pairs_dev == nullptr: row k = 2 KAPPA W[:,k] (single flip of site k); else row c = 2 KAPPA (W[:,i_c] - W[:,j_c])
+// for the exchange pair c = (i_c, j_c).  No row padding.
+cudaError_t launch_pack_table(const Geometry& g, int dtype, const void* W, const void* b, const int32_t* pairs_dev,
+                              int n_rows, float* Wg, float* bg, float* Wt, float* Dtab, cudaStream_t st) {
+    cudaError_t e = launch_pack_gemm_only(g, dtype, W, b, Wg, bg, st);
+    if (e != cudaSuccess) return e;
+    transpose_kernel<<<dim3((g.N + 31) / 32, (g.M_eff + 31) / 32), dim3(32, 8), 0, st>>>(Wg, g.M_eff, g.N, Wt);
+    dim3 gd((g.M_eff + 255) / 256, n_rows);
+    dtab_kernel<<<gd, 256, 0, st>>>(Wt, pairs_dev, pairs_dev ? NK_HEISENBERG : NK_ISING, n_rows, g.M_pad, g.M_eff, Dtab);
+    count_launch(2);
+    return cudaGetLastError();
+}
+
+}  // namespace nk

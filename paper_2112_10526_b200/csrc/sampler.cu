@@ -1,0 +1,186 @@
+// Metropolis-Hastings sampler for the RBM (Sec. 3.4):
+//   P_acc(s -> s') = min(1, |psi(s')|^2 / |psi(s)|^2)       Eq. (20) L709 (local flips / exchanges: symmetric kernels)
+//   MetropolisLocal: negate one spin; MetropolisExchange: swap the spins of one pair of a cluster list     L713
+// One warp owns one chain for the whole call (n_chains = n_samples, L1583): theta_s = KAPPA theta lives in registers
+// exactly as in the fused local-energy kernel (rbm_lane_state.cuh), a proposal costs one row of the table Dtab
+// (theta' = theta - 2 s_k W[:,k], or - 2 s_i (W[:,i] - W[:,j])), read straight from L2 — every chain needs a
+// different row at every transition, so there is nothing to stage in shared memory — and an accepted move
+// overwrites theta in place.  ln psi is never formed: the ratio psi'/psi comes out of the same 1-MUFU-per-pair
+// product form as in fused_eloc.cu.
+//
+// Random numbers (S1-S3): Philox4x32-10, counter = (chain lo, hi, transition lo, hi), key = (seed lo, hi)
+//   proposal index = umulhi(r0, n);  u = ((r1 >> 9) + 1/2) 2^-23;  accept iff u < |psi'/psi|^2 (fp32).
+// Lane l draws for transition t0 + l, so one Philox evaluation per lane serves 32 transitions of the chain.
+#include <type_traits>
+
+#include "nk_internal.h"
+#include "ptx_helpers.cuh"
+#include "rbm_lane_state.cuh"
+
+namespace nk {
+
+constexpr int SW = 16;                       // warps (chains) per CTA
+
+struct SamplerParams {
+    int8_t* sigma;
+    int64_t nb;
+    int N, n_words;
+    const float* theta;
+    int M_pad, M_eff;
+    const float* Dtab;
+    const int32_t* pairs;
+    const float* a;
+    int rule, n_idx;
+    int64_t n_steps;
+    uint32_t key0, key1;
+    uint64_t step_offset, chain0;
+    int32_t* accepted;
+};
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t& r0, uint32_t& r1) {
+    constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
+        const uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+        c0 = hi1 ^ c1 ^ k0; c1 = lo1;
+        c2 = hi0 ^ c3 ^ k1; c3 = lo0;
+        k0 += W0; k1 += W1;
+    }
+    r0 = c0; r1 = c1;
+}
+
+template <int V, bool CPLX>
+constexpr int sampler_min_blocks() { return ((CPLX ? 8 : 4) * V <= 16) ? 2 : 1; }
+
+template <int V, bool CPLX>
+__global__ void __launch_bounds__(SW * 32, (sampler_min_blocks<V, CPLX>())) metropolis_kernel(const SamplerParams p) {
+    extern __shared__ __align__(16) uint32_t sbits[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t c_loc = (int64_t)blockIdx.x * SW + warp;
+    if (c_loc >= p.nb) return;                         // no CTA-wide synchronisation below
+    uint32_t* bits = sbits + (size_t)warp * p.n_words; // bit i set <=> sigma_i = -1
+    int8_t* sp = p.sigma + c_loc * p.N;
+    for (int wi = lane; wi < p.n_words; wi += 32) {
+        uint32_t w = 0;
+        const int base = wi * 32;
+        const int cnt = (p.N - base < 32) ? (p.N - base) : 32;
+        for (int t = 0; t < cnt; ++t) w |= (uint32_t)(sp[base + t] < 0) << t;
+        bits[wi] = w;
+    }
+    typename std::conditional<CPLX, CplxState<V>, RealState<V>>::type st;
+    st.load(p.theta + c_loc * p.M_eff, lane, p.M_pad);
+    __syncwarp();
+
+    const uint64_t chain = p.chain0 + (uint64_t)c_loc;
+    const uint32_t ch_lo = (uint32_t)chain, ch_hi = (uint32_t)(chain >> 32);
+    int n_acc = 0;
+    for (int64_t t0 = 0; t0 < p.n_steps; t0 += 32) {
+        // ---- this lane's draw for transition t0 + lane ----
+        const uint64_t step = p.step_offset + (uint64_t)(t0 + lane);
+        uint32_t r0, r1;
+        philox4x32_10(ch_lo, ch_hi, (uint32_t)step, (uint32_t)(step >> 32), p.key0, p.key1, r0, r1);
+        const int idx_l = (int)__umulhi(r0, (uint32_t)p.n_idx);
+        const float u_l = ((float)(r1 >> 9) + 0.5f) * 1.1920928955078125e-07f;   // 2^-23
+        int i_l = idx_l, j_l = -1;
+        if (p.rule == NK_RULE_EXCHANGE) { i_l = p.pairs[2 * idx_l]; j_l = p.pairs[2 * idx_l + 1]; }
+        float a2_l = 0.f;                             // 2 log2(e) Re(a_i - a_j): visible-bias exponent
+        if (p.a != nullptr) {
+            const int stride = CPLX ? 2 : 1;
+            a2_l = p.a[stride * i_l];
+            if (j_l >= 0) a2_l -= p.a[stride * j_l];
+            a2_l *= 2.f * LOG2E;
+        }
+        const int cnt = (p.n_steps - t0 < 32) ? (int)(p.n_steps - t0) : 32;
+        for (int tt = 0; tt < cnt; ++tt) {
+            const int idx = __shfl_sync(0xffffffffu, idx_l, tt);
+            const int i = __shfl_sync(0xffffffffu, i_l, tt);
+            const int j = __shfl_sync(0xffffffffu, j_l, tt);
+            const float u = __shfl_sync(0xffffffffu, u_l, tt);
+            const float a2 = __shfl_sync(0xffffffffu, a2_l, tt);
+            const uint32_t bi = (bits[i >> 5] >> (i & 31)) & 1u;
+            const uint32_t bj = (j >= 0) ? ((bits[j >> 5] >> (j & 31)) & 1u) : (bi ^ 1u);
+            if (bi == bj) { ++n_acc; continue; }      // exchange of equal spins: s' = s, ratio 1
+            const float s = bi ? 1.f : -1.f;          // s = -sigma_i
+            const float* drow = p.Dtab + (size_t)idx * p.M_eff;
+            bool accept;
+            if constexpr (!CPLX) {
+                float praw, acc;
+                st.partial_raw(drow, lane, s, praw, acc);
+                float r = praw * st.qinv;
+                r = warp_prod_f(r);
+                acc = warp_sum_f(acc);
+                const float ratio = r * ex2_approx(fmaf(0.5f, acc, s * a2));
+                accept = __shfl_sync(0xffffffffu, (int)(u < ratio * ratio), 0) != 0;
+                if (accept) st.commit(drow, lane, s, praw);
+            } else {
+                float pr, pi, acc;
+                st.partial_raw(drow, lane, p.M_pad, s, pr, pi, acc);
+                float cr = pr, ci = pi;
+                cmul_f(cr, ci, st.qr, st.qi);
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    const float orr = __shfl_xor_sync(0xffffffffu, cr, o), oi = __shfl_xor_sync(0xffffffffu, ci, o);
+                    cmul_f(cr, ci, orr, oi);
+                    acc += __shfl_xor_sync(0xffffffffu, acc, o);
+                }
+                const float mag2 = fmaf(cr, cr, ci * ci) * ex2_approx(fmaf(2.f * s, a2, acc));
+                accept = __shfl_sync(0xffffffffu, (int)(u < mag2), 0) != 0;
+                if (accept) st.commit(drow, lane, p.M_pad, s, pr, pi);
+            }
+            if (accept) {
+                ++n_acc;
+                __syncwarp();
+                if (lane == 0) {
+                    bits[i >> 5] ^= 1u << (i & 31);
+                    if (j >= 0) bits[j >> 5] ^= 1u << (j & 31);
+                }
+                __syncwarp();
+            }
+        }
+    }
+    __syncwarp();
+    for (int k = lane; k < p.N; k += 32) sp[k] = ((bits[k >> 5] >> (k & 31)) & 1u) ? (int8_t)-1 : (int8_t)1;
+    if (lane == 0 && p.accepted != nullptr) p.accepted[c_loc] = n_acc;
+}
+
+using SamplerFn = void (*)(const SamplerParams);
+template <int V>
+static SamplerFn pick_sreal(int v) {
+    if (v == V) return metropolis_kernel<V, false>;
+    if constexpr (V < MAX_V_REAL) return pick_sreal<V + 1>(v);
+    return nullptr;
+}
+template <int V>
+static SamplerFn pick_scplx(int v) {
+    if (v == V) return metropolis_kernel<V, true>;
+    if constexpr (V < MAX_V_CPLX) return pick_scplx<V + 1>(v);
+    return nullptr;
+}
+
+cudaError_t launch_metropolis(const Geometry& g, int dtype, int8_t* sigma, int64_t nb, const float* theta,
+                              const float* Dtab, const SamplerArgs& sa, int32_t* accepted, cudaStream_t st) {
+    if (nb <= 0) return cudaSuccess;
+    const bool cplx = dtype == NK_C64;
+    const int V = g.M_pad / MPAD_ALIGN;
+    SamplerFn fn = cplx ? pick_scplx<1>(V) : pick_sreal<1>(V);
+    if (fn == nullptr) return cudaErrorInvalidValue;
+    const size_t smem = (size_t)SW * g.n_words * 4;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    SamplerParams p;
+    p.sigma = sigma; p.nb = nb; p.N = g.N; p.n_words = g.n_words;
+    p.theta = theta; p.M_pad = g.M_pad; p.M_eff = g.M_eff; p.Dtab = Dtab;
+    p.pairs = sa.pairs; p.a = (const float*)sa.a; p.rule = sa.rule; p.n_idx = sa.n_idx; p.n_steps = sa.n_steps;
+    p.key0 = (uint32_t)sa.seed; p.key1 = (uint32_t)(sa.seed >> 32);
+    p.step_offset = sa.step_offset; p.chain0 = sa.chain0; p.accepted = accepted;
+    const int64_t grid = (nb + SW - 1) / SW;
+    fn<<<(unsigned)grid, SW * 32, smem, st>>>(p);
+    count_launch();
+    return cudaGetLastError();
+}
+
+}  // namespace nk
