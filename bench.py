@@ -126,6 +126,65 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def _time_ms(torch, fn, reps):
+    fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
+    """One Metropolis sweep (N transitions per chain, n_chains = n_samples; exchange rule on the lattice bonds for
+    the Heisenberg configs, local rule for TFIM) and one energy-gradient call on the bench batch."""
+    from paper_2112_10526_b200 import inputs as inp
+    B, N, M = p.n_samples, p.n_sites, p.n_hidden
+    lib = nk.load()
+    exch = p.kind == inp.KIND_HEISENBERG
+    rule = nk.NK_RULE_EXCHANGE if exch else nk.NK_RULE_LOCAL
+    clusters = p.bonds if exch else None
+    chains = sigma.clone()
+    ws = torch.empty(lib.nk_metropolis_workspace_bytes(rule, len(p.bonds) if exch else 0, B, N, M, dt_code, 0),
+                     dtype=torch.uint8, device=sigma.device)
+    acc = [None]
+    sweep = [0]
+
+    def one_sweep():
+        acc[0] = nk.metropolis_sample(chains, W, a, b, rule=rule, clusters=clusters, n_steps=N, seed=1,
+                                      step_offset=sweep[0] * N, ws=ws)
+        sweep[0] += 1
+
+    ms_sweep = _time_ms(torch, one_sweep, 3)
+    acceptance = float(acc[0].double().mean().item()) / N
+    # a transition that proposes s' = s (exchange of equal spins) evaluates nothing; count the evaluated ones
+    if exch:
+        anti = (chains[:, torch.from_numpy(p.bonds[:, 0]).to(chains.device).long()] !=
+                chains[:, torch.from_numpy(p.bonds[:, 1]).to(chains.device).long()]).double().mean().item()
+    else:
+        anti = 1.0
+    pairs = B * N * anti * M
+    eloc, _, stats = plan.run(chains, W, a, b)
+    gws = torch.empty(lib.nk_energy_gradient_workspace_bytes(B, N, M, dt_code, p.chunk_size), dtype=torch.uint8,
+                      device=sigma.device)
+    ms_grad = _time_ms(torch, lambda: nk.energy_gradient(chains, W, b, eloc, stats, chunk_size=p.chunk_size, ws=gws), 3)
+    ms_eloc = _time_ms(torch, lambda: plan.run(chains, W, a, b), 3)
+    planes = 2 if p.complex_params else 1
+    return {
+        "sampler": {"rule": "exchange" if exch else "local", "chains": B, "transitions_per_chain": N,
+                    "ms_per_sweep": ms_sweep, "transitions_per_sec": B * N / (ms_sweep * 1e-3), "acceptance": acceptance,
+                    "evaluated_fraction_estimate": anti,
+                    "roofline": {"bound": "alu", "kernel": "metropolis_kernel", "unit": "Gpair/s",
+                                 "achieved": pairs / (ms_sweep * 1e-3) / 1e9}},
+        "gradient": {"ms": ms_grad, "algorithmic_tflops": 2.0 * planes * B * M * N / (ms_grad * 1e-3) / 1e12},
+        "vmc_iteration": {"ms": ms_sweep + ms_eloc + ms_grad, "ms_local_energy_on_sampled_chains": ms_eloc,
+                          "what": "one sweep + local energies + energy gradient, same batch, device-resident"},
+    }
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -220,6 +279,11 @@ def run_ours(args):
     h2d = B * N + (M * N + N + M) * esz
     d2h = 2 * B * esz + 32
 
+    # ---- the neighbouring steps of a VMC iteration, timed apart from the step above ----
+    extras = None
+    if rank == 0 and not args.no_extras:
+        extras = time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan)
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -276,6 +340,12 @@ def run_ours(args):
                                       "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms},
             "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
             "step_ms": [round(x, 4) for x in step_ms], "inputs_sha256": p.sha256()}
+    if extras is not None:
+        for k in ("sampler",):
+            r = extras[k]["roofline"]
+            r["peak"] = peak_pairs
+            r["frac"] = r["achieved"] / peak_pairs if peak_pairs else None
+        line["extras"] = extras
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -288,6 +358,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-extras", action="store_true", help="skip the sampler / gradient timings")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -142,6 +142,8 @@ static GradWs carve_grad(void* ws, const Geometry& g, int64_t chunk, size_t* byt
     w.sigT = c.take<uint16_t>((size_t)g.N * w.ld);
     w.gb_acc = c.take<double>(g.M_eff);
     w.ga_acc = c.take<double>((size_t)2 * g.N);
+    w.part = c.take<double>((size_t)((chunk + grad_slab() - 1) / grad_slab()) *
+                            (size_t)(g.M_eff > 2 * g.N ? g.M_eff : 2 * g.N));
     w.absmax = c.take<unsigned>(1);
     *bytes = c.off;
     return w;

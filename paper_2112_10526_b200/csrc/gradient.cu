@@ -64,32 +64,51 @@ __global__ void grad_tv_kernel(float* __restrict__ theta, int64_t nb, int M, int
     if ((threadIdx.x & 31) == 0 && m) atomicMax(absmax, m);
 }
 
-// gb_acc[me] (+)= sum_s v[s][me]   (one thread per column, samples in order: deterministic)
-__global__ void grad_colsum_kernel(const float* __restrict__ v, int64_t nb, int M_eff, double* __restrict__ gb_acc,
-                                   int first) {
+// Column sums in fp64 with a fixed order (bit-reproducible): slabs of GRAD_SLAB samples are summed in parallel into
+// part[slab][col], then one thread per column adds the slabs in order onto the running accumulator.
+constexpr int GRAD_SLAB = 128;
+
+// part[slab][me] = sum_{s in slab} v[s][me]
+__global__ void grad_colsum_partial_kernel(const float* __restrict__ v, int64_t nb, int M_eff,
+                                           double* __restrict__ part) {
     const int me = blockIdx.x * blockDim.x + threadIdx.x;
     if (me >= M_eff) return;
-    double acc = first ? 0.0 : gb_acc[me];
-    for (int64_t s = 0; s < nb; ++s) acc += (double)v[s * M_eff + me];
-    gb_acc[me] = acc;
+    const int64_t s0 = (int64_t)blockIdx.y * GRAD_SLAB;
+    const int64_t s1 = (s0 + GRAD_SLAB < nb) ? s0 + GRAD_SLAB : nb;
+    double acc = 0.0;
+    for (int64_t s = s0; s < s1; ++s) acc += (double)v[s * M_eff + me];
+    part[(size_t)blockIdx.y * M_eff + me] = acc;
 }
 
-// ga_acc[plane][k] (+)= sum_s sigma[s][k] w_s[plane]   (x2 for real parameters)
-__global__ void grad_a_kernel(const int8_t* __restrict__ sigma, int64_t nb, int N, const float* __restrict__ eloc,
-                              const double* __restrict__ stats, double inv_B, int cplx, double* __restrict__ ga_acc,
-                              int first) {
+// part[slab][plane * N + k] = sum_{s in slab} sigma[s][k] w_s[plane]   (x2 for real parameters)
+__global__ void grad_a_partial_kernel(const int8_t* __restrict__ sigma, int64_t nb, int N,
+                                      const float* __restrict__ eloc, const double* __restrict__ stats, double inv_B,
+                                      int cplx, double* __restrict__ part) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
-    double ar = first ? 0.0 : ga_acc[k], ai = first ? 0.0 : ga_acc[N + k];
+    const int64_t s0 = (int64_t)blockIdx.y * GRAD_SLAB;
+    const int64_t s1 = (s0 + GRAD_SLAB < nb) ? s0 + GRAD_SLAB : nb;
     const double f = cplx ? 1.0 : 2.0;
-    for (int64_t s = 0; s < nb; ++s) {
+    double ar = 0.0, ai = 0.0;
+    for (int64_t s = s0; s < s1; ++s) {
         float wr, wi;
         sample_weight(eloc, stats, s, inv_B, cplx != 0, wr, wi);
         const double sg = (double)sigma[s * N + k];
         ar += f * sg * (double)wr;
         ai += sg * (double)wi;
     }
-    ga_acc[k] = ar; ga_acc[N + k] = ai;
+    part[(size_t)blockIdx.y * 2 * N + k] = ar;
+    part[(size_t)blockIdx.y * 2 * N + N + k] = ai;
+}
+
+// acc[c] (+)= sum_slab part[slab][c], slabs in order
+__global__ void grad_slab_reduce_kernel(const double* __restrict__ part, int n_slabs, int n_cols,
+                                        double* __restrict__ acc, int first) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n_cols) return;
+    double a = first ? 0.0 : acc[c];
+    for (int sl = 0; sl < n_slabs; ++sl) a += part[(size_t)sl * n_cols + c];
+    acc[c] = a;
 }
 
 // TwT[piece][me][s] (bf16, k-contiguous, leading dimension ld) from v[s][me]: fixed-point split on the grids
@@ -178,6 +197,8 @@ __global__ void grad_finalize_ab_kernel(const double* __restrict__ ga_acc, const
     }
 }
 
+int grad_slab() { return GRAD_SLAB; }
+
 cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, int64_t B_total,
                                   const void* eloc, const double* stats, const GradWs& w, int first_chunk,
                                   cudaStream_t st) {
@@ -194,14 +215,17 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
     else
         grad_tv_kernel<false><<<gtv, 256, 0, st>>>(w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
                                                    w.absmax);
-    grad_colsum_kernel<<<(g.M_eff + 63) / 64, 64, 0, st>>>(w.theta, nb, g.M_eff, w.gb_acc, first_chunk);
-    grad_a_kernel<<<(g.N + 63) / 64, 64, 0, st>>>(sigma, nb, g.N, (const float*)eloc, stats, inv_B, cplx, w.ga_acc,
-                                                  first_chunk);
+    const int n_slabs = (int)((nb + GRAD_SLAB - 1) / GRAD_SLAB);
+    grad_colsum_partial_kernel<<<dim3((g.M_eff + 127) / 128, n_slabs), 128, 0, st>>>(w.theta, nb, g.M_eff, w.part);
+    grad_slab_reduce_kernel<<<(g.M_eff + 127) / 128, 128, 0, st>>>(w.part, n_slabs, g.M_eff, w.gb_acc, first_chunk);
+    grad_a_partial_kernel<<<dim3((g.N + 127) / 128, n_slabs), 128, 0, st>>>(sigma, nb, g.N, (const float*)eloc, stats,
+                                                                            inv_B, cplx, w.part);
+    grad_slab_reduce_kernel<<<(2 * g.N + 127) / 128, 128, 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk);
     grad_split_T_kernel<<<dim3(k_len / 32, g.M_eff / 32), dim3(32, 8), 0, st>>>(
         w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (__nv_bfloat16*)w.TwT);
     grad_sigma_T_kernel<<<dim3(k_len / 32, (g.N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, g.N, w.ld,
                                                                                  (__nv_bfloat16*)w.sigT);
-    count_launch(5);
+    count_launch(7);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     return launch_tc_gemm_pieces(w.sigT, g.N, w.TwT, g.M_eff, w.ld, k_len, w.Gacc, first_chunk ? 0 : 1, st);

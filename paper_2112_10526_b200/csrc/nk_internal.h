@@ -88,9 +88,11 @@ struct GradWs {
     float *Wg, *bg, *theta, *Gacc;
     uint16_t *Ws, *A, *TwT, *sigT;
     double *gb_acc, *ga_acc;
+    double* part;               // [ceil(chunk / grad_slab())][max(M_eff, 2 N)] per-slab partial column sums
     unsigned* absmax;
     int ld;                     // k extent (samples per chunk, rounded up to 64) of TwT / sigT
 };
+int grad_slab();
 cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, int64_t B_total,
                                   const void* eloc, const double* stats, const GradWs& w, int first_chunk,
                                   cudaStream_t st);
