@@ -53,7 +53,8 @@ enum nk_dtype { NK_F32 = 0, NK_C64 = 1 };
 enum nk_rule { NK_RULE_LOCAL = 0, NK_RULE_EXCHANGE = 1 };
 enum nk_flags {
     NK_FLAG_MARSHALL = 1u,     /* nk_operator_create: off-diagonal Heisenberg element -2J (default +2J, Eq. (50)) */
-    NK_OUT_F64 = 2u            /* nk_rbm_logpsi: logpsi_out is double / (re,im) double instead of float */
+    NK_OUT_F64 = 2u,           /* nk_rbm_logpsi: logpsi_out is double / (re,im) double instead of float */
+    NK_FORM_PRODUCT = 4u       /* nk_local_energy_ex: product-form amplitude ratios (see there) */
 };
 
 /* Static, never-NULL description of a status code. */
@@ -109,6 +110,20 @@ size_t nk_local_energy_workspace_bytes(nk_operator_t op, int64_t B, int N, int M
 int nk_local_energy(nk_operator_t op, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
                     const void* a, const void* b, int64_t chunk_size, void* eloc_out, void* logpsi_out,
                     double* stats_out, void* workspace, size_t workspace_bytes, nk_stream_t stream);
+
+/* nk_local_energy with flags.  flags = 0: identical to nk_local_energy (every ratio as
+ * exp(ln psi' - ln psi) from stable ln cosh terms, BASELINE.json north_star (3)).  NK_FORM_PRODUCT: the same Eq. (12)
+ * with each ratio written as a product,
+ *   cosh(theta_j + s d_j) / cosh(theta_j) = cosh(d_j) (1 + s tanh(theta_j) tanh(d_j)),   s = +-1,
+ *   psi'/psi = e^{s da} prod_j cosh(d_j) prod_j (1 + s tanh(theta_j) tanh(d_j)),
+ * d the change of theta under the flip / exchange; tanh(d) and prod_j cosh(d_j) depend on the parameters only and are
+ * tabulated per call, tanh(theta) once per sample, so an (amplitude, hidden unit) pair costs two FP32 operations and
+ * no transcendental.  Same outputs and tolerances; for complex parameters tanh(theta) is unbounded next to the zeros
+ * of cosh (Q18), where the log-cosh form is the better conditioned one. */
+int nk_local_energy_ex(nk_operator_t op, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
+                       const void* a, const void* b, int64_t chunk_size, unsigned flags, void* eloc_out,
+                       void* logpsi_out, double* stats_out, void* workspace, size_t workspace_bytes,
+                       nk_stream_t stream);
 
 /* Same computation with HOST inputs and outputs (the end-to-end call): copies sigma/W/a/b host->device into
  * `scratch`, runs nk_local_energy, copies eloc / logpsi / stats back and SYNCHRONISES `stream` before returning.

@@ -12,11 +12,11 @@ import numpy as np
 
 __all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host", "energy_gradient",
            "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
-           "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "EXPORTS"]
+           "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "NK_FORM_PRODUCT", "EXPORTS"]
 
 NK_HEISENBERG, NK_ISING = 0, 1
 NK_F32, NK_C64 = 0, 1
-NK_FLAG_MARSHALL, NK_OUT_F64 = 1, 2
+NK_FLAG_MARSHALL, NK_OUT_F64, NK_FORM_PRODUCT = 1, 2, 4
 NK_RULE_LOCAL, NK_RULE_EXCHANGE = 0, 1
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libnkb200.so")
 
@@ -35,6 +35,8 @@ EXPORTS = {
     "nk_connected": (_int, [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp]),
     "nk_local_energy_workspace_bytes": (_sz, [_vp, _i64, _int, _int, _int, _i64]),
     "nk_local_energy": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "nk_local_energy_ex": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _u32, _vp, _vp, _vp, _vp, _sz,
+                                  _vp]),
     "nk_local_energy_host_scratch_bytes": (_sz, [_vp, _i64, _int, _int, _int, _i64]),
     "nk_local_energy_host": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_energy_gradient_workspace_bytes": (_sz, [_i64, _int, _int, _int, _i64]),
@@ -189,10 +191,11 @@ class LocalEnergyPlan:
     that the timed region contains nothing but the C call)."""
 
     def __init__(self, op: Operator, B: int, N: int, M: int, dtype_code: int, chunk_size: int = 0, device="cuda",
-                 want_logpsi: bool = True):
+                 want_logpsi: bool = True, flags: int = 0):
         torch = _torch()
         lib = load()
         self.op, self.B, self.N, self.M, self.dt, self.chunk = op, int(B), int(N), int(M), dtype_code, int(chunk_size)
+        self.flags = int(flags)
         cdt = torch.complex64 if dtype_code == NK_C64 else torch.float32
         self.eloc = torch.empty(B, dtype=cdt, device=device)
         self.logpsi = torch.empty(B, dtype=cdt, device=device) if want_logpsi else None
@@ -203,18 +206,19 @@ class LocalEnergyPlan:
         self.ws = torch.empty(self.ws_bytes, dtype=torch.uint8, device=device)
 
     def run(self, sigma, W, a, b):
-        rc = load().nk_local_energy(self.op.handle, _ptr(sigma), self.B, self.N, self.M, self.dt, _ptr(W), _ptr(a),
-                                    _ptr(b), self.chunk, _ptr(self.eloc), _ptr(self.logpsi), _ptr(self.stats),
-                                    _ptr(self.ws), self.ws_bytes, _stream())
-        _check(rc, "nk_local_energy")
+        rc = load().nk_local_energy_ex(self.op.handle, _ptr(sigma), self.B, self.N, self.M, self.dt, _ptr(W), _ptr(a),
+                                       _ptr(b), self.chunk, self.flags, _ptr(self.eloc), _ptr(self.logpsi),
+                                       _ptr(self.stats), _ptr(self.ws), self.ws_bytes, _stream())
+        _check(rc, "nk_local_energy_ex")
         return self.eloc, self.logpsi, self.stats
 
 
-def local_energy(op: Operator, sigma, W, a=None, b=None, *, chunk_size: int = 0, want_logpsi: bool = True):
+def local_energy(op: Operator, sigma, W, a=None, b=None, *, chunk_size: int = 0, want_logpsi: bool = True,
+                 flags: int = 0):
     """nk_local_energy on device tensors -> (eloc [B], logpsi [B] | None, stats double[4])."""
     _check_params(sigma, W, a, b)
     plan = LocalEnergyPlan(op, sigma.shape[0], sigma.shape[1], W.shape[0], _dtype_code(W), chunk_size,
-                           device=sigma.device, want_logpsi=want_logpsi)
+                           device=sigma.device, want_logpsi=want_logpsi, flags=flags)
     return plan.run(sigma, W, a, b)
 
 

@@ -424,8 +424,18 @@ size_t nk_local_energy_workspace_bytes(nk_operator_t h, int64_t B, int N, int M,
 int nk_local_energy(nk_operator_t h, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
                     const void* a, const void* b, int64_t chunk_size, void* eloc_out, void* logpsi_out,
                     double* stats_out, void* workspace, size_t workspace_bytes, nk_stream_t stream) {
-    if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0 || !W || (B > 0 && (!sigma || !eloc_out)))
+    return nk_local_energy_ex(h, sigma, B, N, M, dtype, W, a, b, chunk_size, 0u, eloc_out, logpsi_out, stats_out,
+                              workspace, workspace_bytes, stream);
+}
+
+int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
+                       const void* a, const void* b, int64_t chunk_size, unsigned flags, void* eloc_out,
+                       void* logpsi_out, double* stats_out, void* workspace, size_t workspace_bytes,
+                       nk_stream_t stream) {
+    if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0 || !W || (B > 0 && (!sigma || !eloc_out)) ||
+        (flags & ~NK_FORM_PRODUCT))
         return NK_ERR_INVALID_ARG;
+    const bool product = (flags & NK_FORM_PRODUCT) != 0;
     const Operator* op = (const Operator*)h;
     if (N != op->n_sites) return NK_ERR_INVALID_ARG;
     const Geometry g = make_geometry(op, N, M, dtype);
@@ -439,6 +449,7 @@ int nk_local_energy(nk_operator_t h, const int8_t* sigma, int64_t B, int N, int 
     {
         Scope sc(PH_PACK, st);
         NK_CUDA(launch_pack(op, g, dtype, W, a, b, w.Wg, w.bg, w.Wt, w.Dtab, w.rows, st));
+        if (product) NK_CUDA(launch_pack_product(op, g, dtype, w.Wt, w.Dtab, w.rows, st));
         if (!use_simt_theta()) NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
     }
     const size_t esz = dtype == NK_C64 ? 8 : 4;
@@ -455,7 +466,8 @@ int nk_local_energy(nk_operator_t h, const int8_t* sigma, int64_t B, int N, int 
         }
         {
             Scope sc(PH_FUSED, st);
-            NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Dtab, w.rows, (uint8_t*)eloc_out + s0 * esz, st));
+            NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Dtab, w.rows, (uint8_t*)eloc_out + s0 * esz,
+                                      product, st));
         }
     }
     if (stats_out) {

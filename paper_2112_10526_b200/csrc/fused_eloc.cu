@@ -51,6 +51,12 @@ struct FusedParams {
 template <int V, bool CPLX>
 constexpr int min_blocks() { return ((CPLX ? 8 : 4) * V <= 16) ? 2 : 1; }
 
+// per-lane state of the sample: log-cosh form (theta_s, 1 MUFU per pair) or product form (tanh theta, no MUFU)
+template <int V, bool CPLX, bool PROD>
+using LaneState = typename std::conditional<
+    PROD, typename std::conditional<CPLX, ProdCplxState<V>, ProdRealState<V>>::type,
+    typename std::conditional<CPLX, CplxState<V>, RealState<V>>::type>::type;
+
 __device__ __forceinline__ void issue_tile(const FusedParams& p, uint32_t ring_u32, uint32_t full0, int stage,
                                            int tile, uint32_t stage_bytes) {
     mbar_arrive_expect_tx(full0 + 8 * stage, stage_bytes);
@@ -58,7 +64,7 @@ __device__ __forceinline__ void issue_tile(const FusedParams& p, uint32_t ring_u
              full0 + 8 * stage);
 }
 
-template <int V, bool CPLX>
+template <int V, bool CPLX, bool PROD>
 __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_kernel(const FusedParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -92,7 +98,7 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
     int stage = 0;
     uint32_t parity = 0;
     int64_t g = 0;                                    // running tile counter of this CTA
-    typename std::conditional<CPLX, CplxState<V>, RealState<V>>::type st;
+    LaneState<V, CPLX, PROD> st;
 
     for (int64_t rnd = 0; rnd < n_rounds; ++rnd) {
         const int64_t sample = first + rnd * FW + warp;
@@ -126,7 +132,7 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
         for (int t = 0; t < p.n_tiles; ++t) {
             // enumerate this tile's rows for this sample: lane r <-> row t*tile_rows + r
             bool active = false;
-            float sgn = 0.f, coef = 0.f, a2re = 0.f, a2im = 0.f;
+            float sgn = 0.f, coef = 0.f, a2re = 0.f, a2im = 0.f, c2re = 0.f, c2im = 0.f;
             if (lane < p.tile_rows) {
                 const RowInfo ri = p.rows[t * p.tile_rows + lane];
                 if (ri.i >= 0) {
@@ -136,6 +142,7 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
                     diag += (bi != bj) ? -ri.jdiag : ri.jdiag;
                     sgn = bi ? 1.f : -1.f;            // s = -sigma_i
                     coef = ri.coef; a2re = ri.a2_re; a2im = ri.a2_im;
+                    if constexpr (PROD) { c2re = ri.c2_re; c2im = ri.c2_im; }
                 }
             }
             unsigned mask = __ballot_sync(0xffffffffu, active);
@@ -148,20 +155,27 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
                 const float c = __shfl_sync(0xffffffffu, coef, r);
                 const float ar = __shfl_sync(0xffffffffu, a2re, r);
                 const float* drow = tile + (size_t)r * p.M_eff;
+                float cre = 0.f;                      // product form: log2 of prod_j |cosh d_j| of this row
+                if constexpr (PROD) cre = __shfl_sync(0xffffffffu, c2re, r);
                 if constexpr (!CPLX) {
                     RowPartR cur;
                     st.partial(drow, lane, s, cur.r, cur.acc);
-                    cur.ex = s * ar; cur.coef = c;
-                    if (pending) { e_hre += finish_pair(pend, cur, lane); pending = false; }
-                    else { pend = cur; pending = true; }
+                    cur.ex = fmaf(s, ar, cre); cur.coef = c;
+                    if (pending) {
+                        e_hre += PROD ? finish_pair_prod(pend, cur, lane) : finish_pair(pend, cur, lane);
+                        pending = false;
+                    } else { pend = cur; pending = true; }
                 } else {
                     const float ai = __shfl_sync(0xffffffffu, a2im, r);
+                    float cim = 0.f;
+                    if constexpr (PROD) cim = __shfl_sync(0xffffffffu, c2im, r);
                     RowPartC cur;
                     st.partial(drow, lane, p.M_pad, s, cur.ar, cur.ai, cur.acc);
-                    cur.ex_re = s * ar; cur.ex_im = s * ai; cur.coef = c;
+                    cur.ex_re = fmaf(s, ar, cre); cur.ex_im = fmaf(s, ai, cim); cur.coef = c;
                     if (pending) {
                         float rr, rim;
-                        finish_pair_c(pend, cur, lane, rr, rim);
+                        if constexpr (PROD) finish_pair_prod_c(pend, cur, lane, rr, rim);
+                        else finish_pair_c(pend, cur, lane, rr, rim);
                         e_hre += rr; e_him += rim; pending = false;
                     } else { pend = cur; pending = true; }
                 }
@@ -183,7 +197,8 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
             if (++stage == p.stages) { stage = 0; parity ^= 1; }
         }
         if (pending) {
-            if constexpr (!CPLX) e_ure = finish_single(pend);
+            if constexpr (!CPLX) e_ure = PROD ? finish_single_prod(pend) : finish_single(pend);
+            else if constexpr (PROD) finish_single_prod_c(pend, e_ure, e_uim);
             else finish_single_c(pend, e_ure, e_uim);
         }
         e_hre += __shfl_xor_sync(0xffffffffu, e_hre, 16);          // row-A half + row-B half
@@ -199,16 +214,16 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
 // ---- dispatch ----------------------------------------------------------------------------------------------
 using KernelFn = void (*)(const FusedParams);
 
-template <int V>
+template <int V, bool PROD = false>
 static KernelFn pick_real(int v) {
-    if (v == V) return fused_eloc_kernel<V, false>;
-    if constexpr (V < MAX_V_REAL) return pick_real<V + 1>(v);
+    if (v == V) return fused_eloc_kernel<V, false, PROD>;
+    if constexpr (V < MAX_V_REAL) return pick_real<V + 1, PROD>(v);
     return nullptr;
 }
-template <int V>
+template <int V, bool PROD = false>
 static KernelFn pick_cplx(int v) {
-    if (v == V) return fused_eloc_kernel<V, true>;
-    if constexpr (V < MAX_V_CPLX) return pick_cplx<V + 1>(v);
+    if (v == V) return fused_eloc_kernel<V, true, PROD>;
+    if constexpr (V < MAX_V_CPLX) return pick_cplx<V + 1, PROD>(v);
     return nullptr;
 }
 
@@ -222,14 +237,16 @@ cudaError_t fused_eloc_init() {
     if (e != cudaSuccess) return e;
     e = cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return e;
-    for (int v = 1; v <= MAX_V_REAL; ++v) {
-        e = cudaFuncSetAttribute((const void*)pick_real<1>(v), cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
-    }
-    for (int v = 1; v <= MAX_V_CPLX; ++v) {
-        e = cudaFuncSetAttribute((const void*)pick_cplx<1>(v), cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
-    }
+    for (int v = 1; v <= MAX_V_REAL; ++v)
+        for (const void* fn : {(const void*)pick_real<1>(v), (const void*)pick_real<1, true>(v)}) {
+            e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+            if (e != cudaSuccess) return e;
+        }
+    for (int v = 1; v <= MAX_V_CPLX; ++v)
+        for (const void* fn : {(const void*)pick_cplx<1>(v), (const void*)pick_cplx<1, true>(v)}) {
+            e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+            if (e != cudaSuccess) return e;
+        }
     g_attr_done = true;
     return cudaSuccess;
 }
@@ -242,13 +259,14 @@ int fused_consumer_warps() { return FW; }
 
 cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
                               const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,
-                              cudaStream_t st) {
+                              bool product_form, cudaStream_t st) {
     if (B <= 0) return cudaSuccess;
     cudaError_t e = fused_eloc_init();
     if (e != cudaSuccess) return e;
     const bool cplx = dtype == NK_C64;
     const int V = g.M_pad / MPAD_ALIGN;
-    KernelFn fn = cplx ? pick_cplx<1>(V) : pick_real<1>(V);
+    KernelFn fn = product_form ? (cplx ? pick_cplx<1, true>(V) : pick_real<1, true>(V))
+                               : (cplx ? pick_cplx<1>(V) : pick_real<1>(V));
     if (fn == nullptr) return cudaErrorInvalidValue;
     FusedParams p;
     p.sigma = sigma; p.B = B; p.N = g.N; p.n_words = g.n_words;

@@ -59,9 +59,16 @@ __global__ void grad_tv_kernel(float* __restrict__ theta, int64_t nb, int M, int
         }
     }
     }
+    // one atomic per block (all blocks hit the same address)
+    __shared__ unsigned wmax[8];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
-    if ((threadIdx.x & 31) == 0 && m) atomicMax(absmax, m);
+    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) m = max(m, wmax[w]);
+        if (m) atomicMax(absmax, m);
+    }
 }
 
 // Column sums in fp64 with a fixed order (bit-reproducible): slabs of GRAD_SLAB samples are summed in parallel into
@@ -208,7 +215,7 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
     const int k_len = (int)((nb + 63) / 64 * 64);
     cudaError_t e = cudaMemsetAsync(w.absmax, 0, sizeof(unsigned), st);
     if (e != cudaSuccess) return e;
-    dim3 gtv((g.M_pad + 255) / 256, (unsigned)(nb < 32768 ? nb : 32768));
+    dim3 gtv((g.M_pad + 255) / 256, (unsigned)(nb < 1184 ? nb : 1184));
     if (cplx)
         grad_tv_kernel<true><<<gtv, 256, 0, st>>>(w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
                                                   w.absmax);

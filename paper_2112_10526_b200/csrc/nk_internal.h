@@ -25,7 +25,8 @@ struct __align__(32) RowInfo {
     float jdiag;      // Heisenberg: J_c of the bond (diagonal term J s_i s_j); Ising: 0
     float a2_re;      // log2(e) * 2 (a_i - a_j)   [or 2 a_i]: exponent contribution of the visible bias
     float a2_im;      // complex: 2 Im(a_i - a_j) in radians; real: 0
-    int32_t pad0, pad1;
+    float c2_re;      // product form: sum_j ln|cosh d_j| in log2 units (filled by rowc_kernel, else 0)
+    float c2_im;      // product form, complex: sum_j arg cosh d_j in radians
 };
 
 struct Operator {
@@ -60,6 +61,8 @@ cudaError_t launch_pack(const Operator* op, const Geometry& g, int dtype, const 
                         float* Wg, float* bg, float* Wt, float* Dtab, RowInfo* rows, cudaStream_t st);
 cudaError_t launch_pack_gemm_only(const Geometry& g, int dtype, const void* W, const void* b, float* Wg, float* bg,
                                   cudaStream_t st);
+cudaError_t launch_pack_product(const Operator* op, const Geometry& g, int dtype, const float* Wt, float* tab,
+                                RowInfo* rows, cudaStream_t st);
 cudaError_t launch_pack_table(const Geometry& g, int dtype, const void* W, const void* b, const int32_t* pairs_dev,
                               int n_rows, float* Wg, float* bg, float* Wt, float* Dtab, cudaStream_t st);
 // sampler.cu : Metropolis-Hastings transitions with in-register incremental theta
@@ -107,7 +110,7 @@ cudaError_t launch_connected(const Operator* op, const int8_t* sigma, int64_t B,
 // fused_eloc.cu
 cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
                               const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,
-                              cudaStream_t st);
+                              bool product_form, cudaStream_t st);
 cudaError_t fused_eloc_init();   // one-time cudaFuncSetAttribute calls
 // stats.cu
 cudaError_t launch_stats(const void* eloc, int64_t B, int dtype, double* stats_out, cudaStream_t st);

@@ -69,7 +69,7 @@ __global__ void rowinfo_kernel(const int32_t* __restrict__ bonds, const int32_t*
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n_rows_pad) return;
     RowInfo ri;
-    ri.i = -1; ri.j = -1; ri.coef = 0.f; ri.jdiag = 0.f; ri.a2_re = 0.f; ri.a2_im = 0.f; ri.pad0 = 0; ri.pad1 = 0;
+    ri.i = -1; ri.j = -1; ri.coef = 0.f; ri.jdiag = 0.f; ri.a2_re = 0.f; ri.a2_im = 0.f; ri.c2_re = 0.f; ri.c2_im = 0.f;
     if (r < n_rows) {
         float are = 0.f, aim = 0.f;
         if (kind == NK_HEISENBERG) {
@@ -133,6 +133,95 @@ cudaError_t launch_pack_table(const Geometry& g, int dtype, const void* W, const
     transpose_kernel<<<dim3((g.N + 31) / 32, (g.M_eff + 31) / 32), dim3(32, 8), 0, st>>>(Wg, g.M_eff, g.N, Wt);
     dim3 gd((g.M_eff + 255) / 256, n_rows);
     dtab_kernel<<<gd, 256, 0, st>>>(Wt, pairs_dev, pairs_dev ? NK_HEISENBERG : NK_ISING, n_rows, g.M_pad, g.M_eff, Dtab);
+    count_launch(2);
+    return cudaGetLastError();
+}
+
+}  // namespace nk
+
+namespace nk {
+
+// ---- product-form tables -------------------------------------------------------------
+// cosh(theta + s d) / cosh(theta) = cosh(d) (1 + s tanh(theta) tanh(d)),  s = +-1,  so with tau = tanh(d)
+//   psi'/psi = e^{s da} * prod_j cosh(d_j) * prod_j (1 + s t_j tau_j),   t = tanh(theta).
+// Ttab [n_rows_pad][M_eff]: tau for row r and hidden unit j (complex: plane 0 = Re tau, plane 1 = Im tau),
+// d = 2 (W[:,i] - W[:,j]) (exchange) or 2 W[:,k] (flip) — the same rows as Dtab, in natural units.
+__global__ void ttab_kernel(const float* __restrict__ Wt, const int32_t* __restrict__ bonds, int kind, int n_rows,
+                            int M_pad, int M_eff, int cplx, float* __restrict__ Ttab) {
+    const int r = blockIdx.y;
+    int i = -1, j = -1;
+    if (r < n_rows) {
+        if (kind == NK_HEISENBERG) { i = bonds[2 * r]; j = bonds[2 * r + 1]; }
+        else i = r;
+    }
+    for (int m = blockIdx.x * blockDim.x + threadIdx.x; m < M_pad; m += gridDim.x * blockDim.x) {
+        float tr = 0.f, ti = 0.f;
+        if (i >= 0) {
+            float x = Wt[(size_t)i * M_eff + m], y = cplx ? Wt[(size_t)i * M_eff + M_pad + m] : 0.f;
+            if (j >= 0) { x -= Wt[(size_t)j * M_eff + m]; if (cplx) y -= Wt[(size_t)j * M_eff + M_pad + m]; }
+            x *= 2.f; y *= 2.f;
+            if (!cplx) tr = tanhf(x);
+            else {
+                // tanh(x + i y) = [sign(x)(1 - e^2) + i 2 e sin 2y] / (1 + e^2 + 2 e cos 2y),  e = exp(-2|x|)
+                const float e = expf(-2.f * fabsf(x));
+                float sn, cs;
+                sincosf(2.f * y, &sn, &cs);
+                const float den = 1.f / (1.f + e * e + 2.f * e * cs);
+                tr = copysignf((1.f - e) * (1.f + e), x) * den;
+                ti = 2.f * e * sn * den;
+            }
+        }
+        Ttab[(size_t)r * M_eff + m] = tr;
+        if (cplx) Ttab[(size_t)r * M_eff + M_pad + m] = ti;
+    }
+}
+
+// rows[r].c2_re / c2_im = sum_j ln cosh(d_j) (log2 units / radians), fp64 sum in a fixed order: one warp per row,
+// lane-strided partial sums, butterfly.  ln cosh(x+iy) = |x| - ln 2 + (1/2) ln(1 + e^2 + 2 e cos 2y)
+//                                                       + i atan2(sign(x)(1-e) sin y, (1+e) cos y),  e = exp(-2|x|).
+__global__ void rowc_kernel(const float* __restrict__ Wt, int n_rows, int M_pad, int M_eff, int cplx,
+                            RowInfo* __restrict__ rows) {
+    const int r = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (r >= n_rows) return;
+    const int i = rows[r].i, j = rows[r].j;
+    double sre = 0.0, sim = 0.0;
+    if (i >= 0) {
+        for (int m = lane; m < M_pad; m += 32) {
+            double x = (double)Wt[(size_t)i * M_eff + m], y = cplx ? (double)Wt[(size_t)i * M_eff + M_pad + m] : 0.0;
+            if (j >= 0) {
+                x -= (double)Wt[(size_t)j * M_eff + m];
+                if (cplx) y -= (double)Wt[(size_t)j * M_eff + M_pad + m];
+            }
+            x *= 2.0; y *= 2.0;
+            const double e = exp(-2.0 * fabs(x));
+            if (!cplx) sre += fabs(x) + log1p(e) - 0.6931471805599453;
+            else {
+                double sn, cs;
+                sincos(y, &sn, &cs);
+                sre += fabs(x) - 0.6931471805599453 + 0.5 * log1p(e * e + 2.0 * e * (2.0 * cs * cs - 1.0));
+                sim += atan2(copysign((1.0 - e) * sn, x * sn), (1.0 + e) * cs);
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        sre += __shfl_xor_sync(0xffffffffu, sre, o);
+        sim += __shfl_xor_sync(0xffffffffu, sim, o);
+    }
+    if (lane == 0) {
+        rows[r].c2_re = (float)(sre * 1.4426950408889634);
+        rows[r].c2_im = (float)remainder(sim, 6.283185307179586);
+    }
+}
+
+// Overwrites `tab` (the Dtab buffer) with Ttab and fills rows[].c2_*; call after launch_pack.
+cudaError_t launch_pack_product(const Operator* op, const Geometry& g, int dtype, const float* Wt, float* tab,
+                                RowInfo* rows, cudaStream_t st) {
+    const int cplx = dtype == NK_C64;
+    dim3 gd((g.M_pad + 255) / 256, g.n_rows_pad);
+    ttab_kernel<<<gd, 256, 0, st>>>(Wt, op->d_bonds, op->kind, g.n_rows, g.M_pad, g.M_eff, cplx, tab);
+    rowc_kernel<<<(g.n_rows_pad + 7) / 8, 256, 0, st>>>(Wt, g.n_rows, g.M_pad, g.M_eff, cplx, rows);
     count_launch(2);
     return cudaGetLastError();
 }

@@ -228,4 +228,132 @@ __device__ __forceinline__ void finish_single_c(const RowPartC& A, float& out_re
     finish_c(ar, ai, acc, A.ex_re, A.ex_im, A.coef, out_re, out_im);
 }
 
+
+// ---- product form: psi'/psi = C_row * prod_j (1 + s t_j tau_j), t = tanh(theta) in registers,
+// tau = tanh(d) streamed from the table Ttab (pack.cu), C_row = prod_j cosh d_j folded into the row's exponent.
+// No MUFU in the pair loop: one FFMA and one FMUL per pair.  s is warp-uniform, so its sign selects one of two loops
+// (a negated source operand is free, a multiplication by s would not be).
+template <int V>
+struct ProdRealState {
+    float4 t[V];
+
+    __device__ __forceinline__ void load(const float* __restrict__ row, int lane, int /*M_pad*/) {
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            const float4 x = *reinterpret_cast<const float4*>(row + (v * 32 + lane) * 4);
+            t[v] = make_float4(tanhf(x.x), tanhf(x.y), tanhf(x.z), tanhf(x.w));
+        }
+    }
+    template <bool NEG>
+    __device__ __forceinline__ float partial_s(const float* __restrict__ trow, int lane) const {
+        float p0 = 1.f, p1 = 1.f, p2 = 1.f, p3 = 1.f;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            const float4 d = *reinterpret_cast<const float4*>(trow + (v * 32 + lane) * 4);
+            const float4 a = t[v];
+            p0 *= fmaf(NEG ? -a.x : a.x, d.x, 1.f);
+            p1 *= fmaf(NEG ? -a.y : a.y, d.y, 1.f);
+            p2 *= fmaf(NEG ? -a.z : a.z, d.z, 1.f);
+            p3 *= fmaf(NEG ? -a.w : a.w, d.w, 1.f);
+        }
+        return (p0 * p1) * (p2 * p3);
+    }
+    __device__ __forceinline__ void partial(const float* __restrict__ trow, int lane, float s, float& r,
+                                            float& acc) const {
+        r = (s > 0.f) ? partial_s<false>(trow, lane) : partial_s<true>(trow, lane);
+        acc = 0.f;
+    }
+};
+
+template <int V>
+struct ProdCplxState {
+    float4 tr[V], ti[V];
+
+    static __device__ __forceinline__ void ctanh(float x, float y, float& re, float& im) {
+        // tanh(x + i y) = [sign(x)(1 - e^2) + i 2 e sin 2y] / (1 + e^2 + 2 e cos 2y),  e = exp(-2|x|)
+        const float e = expf(-2.f * fabsf(x));
+        float sn, cs;
+        sincosf(2.f * y, &sn, &cs);
+        const float den = 1.f / (1.f + e * e + 2.f * e * cs);
+        re = copysignf((1.f - e) * (1.f + e), x) * den;
+        im = 2.f * e * sn * den;
+    }
+    __device__ __forceinline__ void load(const float* __restrict__ row, int lane, int M_pad) {
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            const float4 x = *reinterpret_cast<const float4*>(row + (v * 32 + lane) * 4);
+            const float4 y = *reinterpret_cast<const float4*>(row + M_pad + (v * 32 + lane) * 4);
+            ctanh(x.x, y.x, tr[v].x, ti[v].x); ctanh(x.y, y.y, tr[v].y, ti[v].y);
+            ctanh(x.z, y.z, tr[v].z, ti[v].z); ctanh(x.w, y.w, tr[v].w, ti[v].w);
+        }
+    }
+    // (pr + i pi) *= 1 + s (a_r + i a_i)(d_r + i d_i)
+    template <bool NEG>
+    static __device__ __forceinline__ void step(float& pr, float& pi, float a_r, float a_i, float d_r, float d_i) {
+        const float xr = fmaf(NEG ? a_i : -a_i, d_i, fmaf(NEG ? -a_r : a_r, d_r, 1.f));
+        const float xi = fmaf(NEG ? -a_i : a_i, d_r, (NEG ? -a_r : a_r) * d_i);
+        const float nr = fmaf(pr, xr, -pi * xi), ni = fmaf(pr, xi, pi * xr);
+        pr = nr; pi = ni;
+    }
+    template <bool NEG>
+    __device__ __forceinline__ void partial_s(const float* __restrict__ trow, int lane, int M_pad, float& ar,
+                                              float& ai) const {
+        float br = 1.f, bi = 0.f;
+        ar = 1.f; ai = 0.f;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            const float4 dr = *reinterpret_cast<const float4*>(trow + (v * 32 + lane) * 4);
+            const float4 di = *reinterpret_cast<const float4*>(trow + M_pad + (v * 32 + lane) * 4);
+            step<NEG>(ar, ai, tr[v].x, ti[v].x, dr.x, di.x);
+            step<NEG>(br, bi, tr[v].y, ti[v].y, dr.y, di.y);
+            step<NEG>(ar, ai, tr[v].z, ti[v].z, dr.z, di.z);
+            step<NEG>(br, bi, tr[v].w, ti[v].w, dr.w, di.w);
+        }
+        const float r = fmaf(ar, br, -ai * bi), i = fmaf(ar, bi, ai * br);
+        ar = r; ai = i;
+    }
+    __device__ __forceinline__ void partial(const float* __restrict__ trow, int lane, int M_pad, float s, float& ar,
+                                            float& ai, float& acc) const {
+        if (s > 0.f) partial_s<false>(trow, lane, M_pad, ar, ai);
+        else partial_s<true>(trow, lane, M_pad, ar, ai);
+        acc = 0.f;
+    }
+};
+
+// product-form row reductions: as finish_pair / finish_pair_c without the acc butterflies (acc = 0)
+__device__ __forceinline__ float finish_pair_prod(const RowPartR& A, const RowPartR& B, int lane) {
+    const bool up = (lane & 16) != 0;
+    float rk = up ? B.r : A.r;
+    const float rs = up ? A.r : B.r;
+    rk *= __shfl_xor_sync(0xffffffffu, rs, 16);
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) rk *= __shfl_xor_sync(0xffffffffu, rk, o);
+    return (up ? B.coef : A.coef) * (rk * ex2_approx(up ? B.ex : A.ex));
+}
+__device__ __forceinline__ float finish_single_prod(const RowPartR& A) {
+    return A.coef * (warp_prod_f(A.r) * ex2_approx(A.ex));
+}
+__device__ __forceinline__ void finish_pair_prod_c(const RowPartC& A, const RowPartC& B, int lane, float& out_re,
+                                                   float& out_im) {
+    const bool up = (lane & 16) != 0;
+    float kr = up ? B.ar : A.ar, ki = up ? B.ai : A.ai;
+    const float sr = up ? A.ar : B.ar, si = up ? A.ai : B.ai;
+    cmul_f(kr, ki, __shfl_xor_sync(0xffffffffu, sr, 16), __shfl_xor_sync(0xffffffffu, si, 16));
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) {
+        const float orr = __shfl_xor_sync(0xffffffffu, kr, o), oi = __shfl_xor_sync(0xffffffffu, ki, o);
+        cmul_f(kr, ki, orr, oi);
+    }
+    finish_c(kr, ki, 0.f, up ? B.ex_re : A.ex_re, up ? B.ex_im : A.ex_im, up ? B.coef : A.coef, out_re, out_im);
+}
+__device__ __forceinline__ void finish_single_prod_c(const RowPartC& A, float& out_re, float& out_im) {
+    float ar = A.ar, ai = A.ai;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const float orr = __shfl_xor_sync(0xffffffffu, ar, o), oi = __shfl_xor_sync(0xffffffffu, ai, o);
+        cmul_f(ar, ai, orr, oi);
+    }
+    finish_c(ar, ai, 0.f, A.ex_re, A.ex_im, A.coef, out_re, out_im);
+}
+
 }  // namespace nk

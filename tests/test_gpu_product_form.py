@@ -1,0 +1,105 @@
+"""GPU parity of the product-form local energy (nk_local_energy_ex with NK_FORM_PRODUCT)
+against the same float64 from-scratch oracle and tolerances as the log-cosh form (tests/test_gpu_parity.py):
+|dE| <= 1e-4 |E| + 1e-6 per sample.  The oracle knows nothing of either form: it evaluates Eq. (12) L652 with every
+ln psi(s') from scratch."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import nk_oracle as orc
+from paper_2112_10526_b200 import inputs as inp
+from test_gpu_parity import assert_eloc, assert_logpsi, dev, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def run_prod(nk, p, chunk=None, flags=0, a=True, b=True, form=None):
+    op = nk.Operator.from_problem(p, flags)
+    e, lp, st = nk.local_energy(op, dev(p.sigma), dev(p.W), dev(p.a) if a else None, dev(p.b) if b else None,
+                                chunk_size=p.chunk_size if chunk is None else chunk,
+                                flags=nk.NK_FORM_PRODUCT if form is None else form)
+    torch.cuda.synchronize()
+    out = e.cpu().numpy(), lp.cpu().numpy(), st.cpu().numpy()
+    op.close()
+    return out
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (2, 512), (3, 96), (4, 160), (5, 47)])
+def test_product_form_parity(nk, cfg, n):
+    p = inp.make_config(cfg, n_samples=n)
+    e, lp, st = run_prod(nk, p, chunk=0)
+    e_ref, lp_ref = run_oracle(p)
+    worst = assert_eloc(e, e_ref)
+    assert_logpsi(lp, lp_ref)
+    m = orc.stats(e_ref)
+    assert abs(st[0] - m[0]) <= 1e-4 * abs(m[0]) + 1e-6 and st[3] == n
+    print(f"cfg{cfg} product form: max rel err E_loc {worst:.2e}")
+
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_product_form_full_size_sampled(nk, cfg):
+    p = inp.make_config(cfg)
+    e, lp, st = run_prod(nk, p)
+    B = p.n_samples
+    chunk = p.chunk_size or B
+    rows = sorted({c * chunk + o for c in range(0, B // chunk, max(1, B // chunk // 4)) for o in (0, chunk - 1)}
+                  | {B - 1, B // 2 + 1})
+    if cfg != 5:
+        rows = sorted(set(rows) | set(range(17, B, B // 24)))
+    e_ref, _ = run_oracle(p, rows)
+    assert_eloc(e[rows], e_ref)
+    assert np.all(np.isfinite(e.view(np.float32))) and st[3] == B
+    # both forms agree over the whole batch far inside the tolerance
+    e_log, _, _ = run_prod(nk, p, form=0)
+    rel = np.abs(e.astype(np.complex128) - e_log.astype(np.complex128)) / (np.abs(e_log) + 1e-6)
+    assert rel.max() < 5e-5, rel.max()
+
+
+def test_product_form_closed_forms_and_flags(nk):
+    # uniform psi: E_loc = sum_c J_c n_{b,c}; W = 0 with a != 0: independent-spin closed form through the oracle
+    q = inp.make_config(2, n_samples=300)
+    q.W = np.zeros_like(q.W); q.a = np.zeros_like(q.a)
+    e0, _, _ = run_prod(nk, q)
+    np.testing.assert_allclose(e0, 200.0, rtol=2e-6)
+    q = inp.make_config(4, n_samples=64)
+    q.W = np.zeros_like(q.W)
+    e1, _, _ = run_prod(nk, q)
+    assert_eloc(e1, run_oracle(q)[0])
+    # Marshall sign, NULL biases, ragged sizes (N = 7, M = 5; M = 130 -> two 128-blocks)
+    p = inp.make_config(2, n_samples=97)
+    e2, _, _ = run_prod(nk, p, flags=nk.NK_FLAG_MARSHALL, a=False, b=False)
+    assert_eloc(e2, run_oracle(p, flags=orc.FLAG_MARSHALL, a=False, b=False)[0])
+    for kw in (dict(kind=inp.KIND_HEISENBERG, lattice="chain", L=7, n_hidden=5, n_samples=3, seed=3, sz0=False),
+               dict(kind=inp.KIND_ISING, lattice="square", L=3, n_hidden=130, n_samples=33, seed=4, h=0.7),
+               dict(kind=inp.KIND_HEISENBERG, lattice="square", L=4, n_hidden=130, n_samples=33, seed=5,
+                    complex_params=True, order=2, J=(1.0, 0.5), scale=0.05)):
+        kind, lattice, L, M, n = (kw.pop(k) for k in ("kind", "lattice", "L", "n_hidden", "n_samples"))
+        p = inp.make_problem(kind, lattice, L, M, n, **kw)
+        e3, _, _ = run_prod(nk, p)
+        assert_eloc(e3, run_oracle(p)[0])
+
+
+def test_product_form_larger_parameters(nk):
+    """x5 parameters (|theta| of a trained state, |tanh theta| near 1, ratios over several decades) stay inside the
+    1e-4 bound.  At x10 (|d| up to 4, tanh d = 0.9993) the factors 1 - |tanh theta tanh d| cancel to ~1e-3 and the
+    fp32 rounding of the two tanh values shows: the product form is then only good to ~1e-3 (checked here), which is
+    why the log-cosh form stays the default."""
+    p = inp.make_config(2, n_samples=256)
+    W0, a0, b0 = p.W, p.a, p.b
+    p.W, p.a, p.b = (x * np.float32(5.0) for x in (W0, a0, b0))
+    e, _, _ = run_prod(nk, p)
+    assert_eloc(e, run_oracle(p)[0])
+    p.W, p.a, p.b = (x * np.float32(10.0) for x in (W0, a0, b0))
+    e, _, _ = run_prod(nk, p)
+    e_ref = run_oracle(p)[0]
+    assert np.max(np.abs(e - e_ref) / np.abs(e_ref)) < 5e-3
+
+
+def test_product_form_chunking_and_bad_flags(nk):
+    p = inp.make_config(2, n_samples=700)
+    ref, _, st0 = run_prod(nk, p, chunk=0)
+    for chunk in (256, 100):
+        e, _, st = run_prod(nk, p, chunk=chunk)
+        assert np.array_equal(e, ref) and np.array_equal(st, st0)
+    with pytest.raises(nk.NkError):
+        run_prod(nk, p, form=64)
