@@ -173,7 +173,21 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
     ms_grad = _time_ms(torch, lambda: nk.energy_gradient(chains, W, b, eloc, stats, chunk_size=p.chunk_size, ws=gws), 3)
     ms_eloc = _time_ms(torch, lambda: plan.run(chains, W, a, b), 3)
     planes = 2 if p.complex_params else 1
+    # product-form variant of the same step (nk_local_energy_ex, NK_FORM_PRODUCT), fused kernel timed by the library
+    pplan = nk.LocalEnergyPlan(op, B, N, M, dt_code, p.chunk_size, device=sigma.device, flags=nk.NK_FORM_PRODUCT)
+    pplan.run(sigma, W, a, b)
+    torch.cuda.synchronize()
+    nk.profile_enable(True)
+    nk.profile_read()
+    ms_prod = _time_ms(torch, lambda: pplan.run(sigma, W, a, b), 3)
+    ph = nk.profile_read()
+    nk.profile_enable(False)
+    fused_prod_ms = ph["fused"][0] / 4                      # _time_ms runs the call 1 + 3 times
     return {
+        "product_form": {"ms_per_step": ms_prod, "local_energies_per_sec": B / (ms_prod * 1e-3),
+                         "fused_ms_per_step": fused_prod_ms,
+                         "roofline": {"bound": "smem", "kernel": "fused_eloc_kernel<V, CPLX, PROD=true>",
+                                      "unit": "Gpair/s", "fused_ms": fused_prod_ms}},
         "sampler": {"rule": "exchange" if exch else "local", "chains": B, "transitions_per_chain": N,
                     "ms_per_sweep": ms_sweep, "transitions_per_sec": B * N / (ms_sweep * 1e-3), "acceptance": acceptance,
                     "evaluated_fraction_estimate": anti,
@@ -345,6 +359,11 @@ def run_ours(args):
             r = extras[k]["roofline"]
             r["peak"] = peak_pairs
             r["frac"] = r["achieved"] / peak_pairs if peak_pairs else None
+        # product form: shared-memory bandwidth binds (128 B/clk/SM; 4 B per real pair, 8 B per complex pair)
+        r = extras["product_form"]["roofline"]
+        r["peak"] = N_SMS * (128 / (8 if p.complex_params else 4)) * sm_max * 1e6 / 1e9
+        r["achieved"] = pairs / (r.pop("fused_ms") * 1e-3) / 1e9
+        r["frac"] = r["achieved"] / r["peak"]
         line["extras"] = extras
     print(json.dumps(line), flush=True)
     if world > 1:
