@@ -20,6 +20,11 @@ What it computes, in the paper's order and notation (citations are PAPER.md line
         pins in tests/test_oracle_gradient.py (finite differences of ln psi; finite differences of the exact
         <H> from the dense Kronecker Hamiltonian over the full Born distribution; covariance properties)
 
+  * `rbm_jacobian`, `qgt_dense`, `qgt_matvec`, `sr_solve`   quantum geometric tensor G = Cov[O, O] (Eq. (23)), its product
+        with a vector in the three steps of Eq. (75) (QGTOnTheFly), the SR system Eq. (25)/(30)/(31) — SURVEY.md §8(f)
+        rank 4; pins in tests/test_oracle_qgt.py (Fubini-Study distance from exact overlaps over the full space,
+        np.cov, dense solve residuals)
+
 Pins (tests/test_oracle_pins.py, `-m "not gpu"`): dense Kronecker-product Hamiltonians built independently in
 tests/dense_ref.py (Born identity Eq. (11) L646 over the full space; row-by-row equality of the connected list),
 Eq. (2), closed forms (W = 0; M = 1 with np.cosh; uniform psi), known ring spectra, symmetries.
@@ -224,3 +229,59 @@ def energy_gradient_batched(sigma, W, b, eloc):
     if not cplx:
         return 2.0 * g_a.real, 2.0 * g_b.real, 2.0 * g_W.real
     return g_a, g_b, g_W
+
+
+# ---------------------------------------------------------------------------------------------------------
+# NEXT-4: quantum geometric tensor times a vector, stochastic reconfiguration
+# ---------------------------------------------------------------------------------------------------------
+def rbm_jacobian(sigma, W, b=None):
+    """J [B][P]: row s holds the log-derivatives O_i(s) (Eq. (13)) in the order a (N), b (M), W (M*N row-major),
+    P = N + M + M N.  ("the full Jacobian matrix J_kl", App. B.2)"""
+    O_a, O_b, O_W = rbm_log_derivatives(sigma, W, b)
+    return np.concatenate([O_a, O_b, O_W.reshape(O_W.shape[0], -1)], axis=1)
+
+
+def qgt_dense(sigma, W, b=None, weights=None):
+    """G_ij = E[O_i^* O_j] - E[O_i^*] E[O_j]  (Eq. (23)) as a dense P x P matrix; E[.] the sample mean, or
+    the weighted mean with normalised `weights` (exact-distribution pin only).  Real parameters: G is real."""
+    J = rbm_jacobian(sigma, W, b)
+    B = J.shape[0]
+    w = np.full(B, 1.0 / B) if weights is None else np.asarray(weights, dtype=np.float64)
+    mean = w @ J
+    return (np.conj(J) * w[:, None]).T @ J - np.outer(np.conj(mean), mean)
+
+
+def pack_params(v_a, v_b, v_W):
+    return np.concatenate([np.ravel(v_a), np.ravel(v_b), np.ravel(v_W)])
+
+
+def unpack_params(v, N, M):
+    return v[:N], v[N:N + M], v[N + M:].reshape(M, N)
+
+
+def qgt_matvec(sigma, W, b, v_a, v_b, v_W, diag_shift=0.0):
+    """(G + eps) v without forming G, in the three steps of Eq. (75) L2219 (QGTOnTheFly):
+        w = (1/N_s) J v;   dw = w - <w>;   v~ = J^dagger dw;     then  + eps v  (Eq. (25)).
+    Returns (v~_a [N], v~_b [M], v~_W [M][N]).  Real parameters: Re[G] v (Eq. (30)) — G is real there."""
+    sigma = np.atleast_2d(np.asarray(sigma))
+    N, M = sigma.shape[1], np.shape(W)[0]
+    J = rbm_jacobian(sigma, W, b)
+    v = pack_params(v_a, v_b, v_W).astype(J.dtype)
+    w = (J @ v) / J.shape[0]
+    dw = w - w.mean()
+    out = np.conj(J).T @ dw + diag_shift * v
+    if not np.iscomplexobj(W):
+        out = out.real
+    return unpack_params(out, N, M)
+
+
+def sr_solve(sigma, W, b, f_a, f_b, f_W, diag_shift):
+    """Stochastic reconfiguration: the solution delta of sum_j (G_ij + eps delta_ij) delta_j = f_i
+    (Eq. (25) L886 with Eq. (30)/(31) L961-967), by a dense direct solve of the definition."""
+    sigma = np.atleast_2d(np.asarray(sigma))
+    N, M = sigma.shape[1], np.shape(W)[0]
+    G = qgt_dense(sigma, W, b)
+    if not np.iscomplexobj(W):
+        G = G.real
+    f = pack_params(f_a, f_b, f_W).astype(G.dtype)
+    return unpack_params(np.linalg.solve(G + diag_shift * np.eye(G.shape[0]), f), N, M)
