@@ -151,6 +151,21 @@ int nk_energy_gradient(const int8_t* sigma, int64_t B, int N, int M, int dtype, 
                        void* grad_b_out, void* grad_W_out, void* workspace, size_t workspace_bytes,
                        nk_stream_t stream);
 
+/* ---- quantum geometric tensor times a vector, on the fly -----------------------------
+ * PAPER.md Eq. (23): G_ij = E[O_i^* O_j] - E[O_i^*] E[O_j] with the log-derivatives O of Eq. (13); its
+ * product with a vector without forming G, Eq. (75) L2219 (QGTOnTheFly):
+ *     w = (1/N_s) J v;   dw = w - <w>;   v~ = J^dagger dw;          out = v~ + diag_shift * v   (Eq. (25))
+ * E[.] is the mean over the B rows of sigma.  Parameter vectors are given block-wise in the parameter dtype:
+ * (v_a [N], v_b [M], v_W [M][N]) -> (out_a, out_b, out_W).  v_a / v_b may be NULL (= zeros), out_a / out_b may be
+ * NULL (not wanted).  NK_F32: G is real (the Re[G] of Eq. (30)); NK_C64: the full Hermitian G of the holomorphic
+ * RBM (Eq. (31)).  Samples are processed chunk_size at a time; the three contractions (theta, V_W sigma, J^dagger dw)
+ * run on the tensor cores with exact products, as in nk_rbm_logpsi / nk_energy_gradient. */
+size_t nk_qgt_matvec_workspace_bytes(int64_t B, int N, int M, int dtype, int64_t chunk_size);
+int nk_qgt_matvec(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* b,
+                  const void* v_a, const void* v_b, const void* v_W, double diag_shift, int64_t chunk_size,
+                  void* out_a, void* out_b, void* out_W, void* workspace, size_t workspace_bytes,
+                  nk_stream_t stream);
+
 /* ---- Metropolis-Hastings sampler for the RBM ------------------------------------------
  * PAPER.md Sec. 3.4: a proposal s -> s' is accepted with probability min(1, |psi(s')|^2 / |psi(s)|^2) (Eq. (20)
  * L709; both rules are symmetric kernels, L711).  Every row of sigma is one chain (n_chains = n_samples, L1583);

@@ -11,7 +11,7 @@ import os
 import numpy as np
 
 __all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host", "energy_gradient",
-           "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
+           "qgt_matvec", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
            "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "NK_FORM_PRODUCT", "EXPORTS"]
 
 NK_HEISENBERG, NK_ISING = 0, 1
@@ -41,6 +41,9 @@ EXPORTS = {
     "nk_local_energy_host": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_energy_gradient_workspace_bytes": (_sz, [_i64, _int, _int, _int, _i64]),
     "nk_energy_gradient": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "nk_qgt_matvec_workspace_bytes": (_sz, [_i64, _int, _int, _int, _i64]),
+    "nk_qgt_matvec": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _vp, _dbl, _i64, _vp, _vp, _vp, _vp, _sz,
+                             _vp]),
     "nk_metropolis_workspace_bytes": (_sz, [_int, _int, _i64, _int, _int, _int, _i64]),
     "nk_metropolis_sample": (_int, [_int, _vp, _int, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _u64, _u64, _u64,
                                     _i64, _vp, _vp, _sz, _vp]),
@@ -283,6 +286,35 @@ def energy_gradient(sigma, W, b, eloc, stats, *, chunk_size: int = 0, ws=None):
                                 _ptr(ga), _ptr(gb), _ptr(gW), _ptr(ws), ws.numel(), _stream())
     _check(rc, "nk_energy_gradient")
     return ga, gb, gW
+
+
+def qgt_matvec(sigma, W, b, v_a, v_b, v_W, *, diag_shift: float = 0.0, chunk_size: int = 0, ws=None, out=None):
+    """nk_qgt_matvec on device tensors: (G + diag_shift) v for v = (v_a [N], v_b [M], v_W [M][N]) in the parameter
+    dtype -> (out_a, out_b, out_W).  `out`: optional preallocated triple."""
+    torch = _torch()
+    lib = load()
+    _check_params(sigma, W, None, b)
+    B, N = sigma.shape
+    M = W.shape[0]
+    dt = _dtype_code(W)
+    for name, t, shape in (("v_a", v_a, (N,)), ("v_b", v_b, (M,)), ("v_W", v_W, (M, N))):
+        if t is not None and (t.dtype != W.dtype or tuple(t.shape) != shape or not t.is_contiguous() or not t.is_cuda):
+            raise NkError(f"{name} must be a contiguous CUDA tensor of W's dtype and shape {shape}")
+    if v_W is None:
+        raise NkError("v_W is required")
+    if out is None:
+        out = (torch.empty(N, dtype=W.dtype, device=sigma.device), torch.empty(M, dtype=W.dtype, device=sigma.device),
+               torch.empty((M, N), dtype=W.dtype, device=sigma.device))
+    nbytes = lib.nk_qgt_matvec_workspace_bytes(B, N, M, dt, int(chunk_size))
+    if nbytes == 0:
+        raise NkError("nk_qgt_matvec_workspace_bytes rejected the arguments")
+    if ws is None or ws.numel() < nbytes:
+        ws = torch.empty(nbytes, dtype=torch.uint8, device=sigma.device)
+    rc = lib.nk_qgt_matvec(_ptr(sigma), B, N, M, dt, _ptr(W), _ptr(b), _ptr(v_a), _ptr(v_b), _ptr(v_W),
+                           float(diag_shift), int(chunk_size), _ptr(out[0]), _ptr(out[1]), _ptr(out[2]), _ptr(ws),
+                           ws.numel(), _stream())
+    _check(rc, "nk_qgt_matvec")
+    return out
 
 
 def metropolis_sample(sigma, W, a=None, b=None, *, rule: int = NK_RULE_LOCAL, clusters=None, n_steps: int | None = None,

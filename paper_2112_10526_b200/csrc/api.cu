@@ -172,6 +172,30 @@ static SamplerWs carve_sampler(void* ws, const Geometry& g, int n_rows, int64_t 
     return w;
 }
 
+struct QgtWs {
+    GradWs g;
+    float *Vg, *vbg, *Y;
+    uint16_t* Vs;
+    float* wbuf;
+    double* wstats;
+    size_t bytes;
+};
+static QgtWs carve_qgt(void* ws, const Geometry& g, int64_t B, int64_t chunk, int dtype) {
+    size_t gbytes = 0;
+    QgtWs w;
+    w.g = carve_grad(ws, g, chunk, &gbytes);
+    Carver c(ws);
+    c.off = gbytes;
+    w.Vg = c.take<float>((size_t)g.M_eff * g.N);
+    w.vbg = c.take<float>(g.M_eff);
+    w.Y = c.take<float>((size_t)chunk * g.M_eff);
+    w.Vs = c.take<uint16_t>((size_t)3 * g.M_eff * g.K_pad);
+    w.wbuf = c.take<float>((size_t)B * (dtype == NK_C64 ? 2 : 1));
+    w.wstats = c.take<double>(4);
+    w.bytes = c.off;
+    return w;
+}
+
 // NK_THETA_SIMT=1 selects the FP32 SIMT contraction (debugging aid); default is the tcgen05 path.
 static bool use_simt_theta() {
     static const bool v = [] { const char* e = std::getenv("NK_THETA_SIMT"); return e && e[0] == '1'; }();
@@ -351,7 +375,7 @@ int nk_energy_gradient(const int8_t* sigma, int64_t B, int N, int M, int dtype, 
         const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
         const int8_t* sg = sigma + s0 * N;
         NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.Ws, w.A, w.bg, w.theta, st));
-        NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B, (const uint8_t*)eloc + s0 * esz, stats, w, first, st));
+        NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B, (const uint8_t*)eloc + s0 * esz, stats, w, first, 2.f, st));
         first = 0;
     }
     NK_CUDA(launch_gradient_finalize(g, dtype, w, grad_a_out, grad_b_out, grad_W_out, st));
@@ -361,6 +385,61 @@ int nk_energy_gradient(const int8_t* sigma, int64_t B, int N, int M, int dtype, 
 static int64_t eff_chunk(int64_t B, int64_t chunk_size) {
     if (chunk_size <= 0 || chunk_size > B) return B > 0 ? B : 1;
     return chunk_size;
+}
+
+size_t nk_qgt_matvec_workspace_bytes(int64_t B, int N, int M, int dtype, int64_t chunk_size) {
+    if (bad_dims(B, N, M, dtype) || chunk_size < 0) return 0;
+    const Geometry g = make_geometry(nullptr, N, M, dtype);
+    return carve_qgt(nullptr, g, B, eff_chunk(B, chunk_size), dtype).bytes;
+}
+
+int nk_qgt_matvec(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* b,
+                  const void* v_a, const void* v_b, const void* v_W, double diag_shift, int64_t chunk_size,
+                  void* out_a, void* out_b, void* out_W, void* workspace, size_t workspace_bytes,
+                  nk_stream_t stream) {
+    if (bad_dims(B, N, M, dtype) || B == 0 || chunk_size < 0 || !sigma || !W || !v_W || !out_W ||
+        (diag_shift < 0.0))
+        return NK_ERR_INVALID_ARG;
+    const Geometry g = make_geometry(nullptr, N, M, dtype);
+    if (g.M_pad / MPAD_ALIGN > (dtype == NK_C64 ? MAX_V_CPLX : MAX_V_REAL) || N > 65535) return NK_ERR_UNSUPPORTED;
+    const int64_t chunk = eff_chunk(B, chunk_size);
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_qgt(nullptr, g, B, chunk, dtype).bytes)
+        return NK_ERR_WORKSPACE;
+    const QgtWs w = carve_qgt(workspace, g, B, chunk, dtype);
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t esz = dtype == NK_C64 ? 8 : 4;
+    // operands of the two contractions: (W, b) -> theta and (V_W, v_b) -> Y
+    NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.g.Wg, w.g.bg, st));
+    NK_CUDA(launch_split_w(w.g.Wg, g.M_eff, N, g.K_pad, w.g.Ws, w.g.absmax, st));
+    NK_CUDA(launch_pack_gemm_only(g, dtype, v_W, v_b, w.Vg, w.vbg, st));
+    NK_CUDA(launch_split_w(w.Vg, g.M_eff, N, g.K_pad, w.Vs, w.g.absmax, st));
+    // step 1 of Eq. (75): w_s = (J v)_s for every sample
+    for (int64_t s0 = 0; s0 < B; s0 += chunk) {
+        const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
+        const int8_t* sg = sigma + s0 * N;
+        NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.g.Ws, w.g.A, w.g.bg, w.g.theta, st));
+        NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.Vs, w.g.A, w.vbg, w.Y, st));
+        NK_CUDA(launch_qgt_w(g, dtype, sg, nb, w.g.theta, w.Y, v_a, (uint8_t*)w.wbuf + s0 * esz, st));
+    }
+    // step 2: <w> (the 1/N_s and the subtraction happen inside the force contraction, as for E_loc)
+    NK_CUDA(launch_stats(w.wbuf, B, dtype, w.wstats, st));
+    // step 3: v~ = J^dagger (w - <w>) / N_s  — the force-vector contraction with w in the place of E_loc
+    int first = 1;
+    for (int64_t s0 = 0; s0 < B; s0 += chunk) {
+        const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
+        const int8_t* sg = sigma + s0 * N;
+        NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.g.Ws, w.g.A, w.g.bg, w.g.theta, st));
+        NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B, (const uint8_t*)w.wbuf + s0 * esz, w.wstats, w.g, first, 1.f,
+                                      st));
+        first = 0;
+    }
+    NK_CUDA(launch_gradient_finalize(g, dtype, w.g, out_a, out_b, out_W, st));
+    // Eq. (25): + eps v
+    const int64_t e = dtype == NK_C64 ? 2 : 1;
+    NK_CUDA(launch_qgt_shift(out_a, v_a, diag_shift, (int64_t)N * e, st));
+    NK_CUDA(launch_qgt_shift(out_b, v_b, diag_shift, (int64_t)M * e, st));
+    NK_CUDA(launch_qgt_shift(out_W, v_W, diag_shift, (int64_t)M * N * e, st));
+    return NK_OK;
 }
 
 static bool bad_rule(int rule, int n_clusters) {

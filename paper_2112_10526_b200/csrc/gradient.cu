@@ -30,7 +30,7 @@ __device__ __forceinline__ void sample_weight(const float* __restrict__ eloc, co
 template <bool CPLX>
 __global__ void grad_tv_kernel(float* __restrict__ theta, int64_t nb, int M, int M_pad, int M_eff,
                                const float* __restrict__ eloc, const double* __restrict__ stats, double inv_B,
-                               unsigned* __restrict__ absmax) {
+                               float real_scale, unsigned* __restrict__ absmax) {
     unsigned m = 0;
     for (int64_t s = blockIdx.y; s < nb; s += gridDim.y) {
     float wr, wi;
@@ -38,7 +38,7 @@ __global__ void grad_tv_kernel(float* __restrict__ theta, int64_t nb, int M, int
     float* row = theta + s * M_eff;
     for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < M_pad; j += gridDim.x * blockDim.x) {
         if (!CPLX) {
-            const float v = (j < M) ? 2.f * tanhf(row[j]) * wr : 0.f;
+            const float v = (j < M) ? real_scale * tanhf(row[j]) * wr : 0.f;
             row[j] = v;
             m = max(m, __float_as_uint(fabsf(v)));
         } else {
@@ -90,12 +90,12 @@ __global__ void grad_colsum_partial_kernel(const float* __restrict__ v, int64_t 
 // part[slab][plane * N + k] = sum_{s in slab} sigma[s][k] w_s[plane]   (x2 for real parameters)
 __global__ void grad_a_partial_kernel(const int8_t* __restrict__ sigma, int64_t nb, int N,
                                       const float* __restrict__ eloc, const double* __restrict__ stats, double inv_B,
-                                      int cplx, double* __restrict__ part) {
+                                      int cplx, double real_scale, double* __restrict__ part) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
     const int64_t s0 = (int64_t)blockIdx.y * GRAD_SLAB;
     const int64_t s1 = (s0 + GRAD_SLAB < nb) ? s0 + GRAD_SLAB : nb;
-    const double f = cplx ? 1.0 : 2.0;
+    const double f = cplx ? 1.0 : real_scale;
     double ar = 0.0, ai = 0.0;
     for (int64_t s = s0; s < s1; ++s) {
         float wr, wi;
@@ -208,7 +208,7 @@ int grad_slab() { return GRAD_SLAB; }
 
 cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, int64_t B_total,
                                   const void* eloc, const double* stats, const GradWs& w, int first_chunk,
-                                  cudaStream_t st) {
+                                  float real_scale, cudaStream_t st) {
     if (nb <= 0) return cudaSuccess;
     const bool cplx = dtype == NK_C64;
     const double inv_B = 1.0 / (double)B_total;
@@ -218,15 +218,15 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
     dim3 gtv((g.M_pad + 255) / 256, (unsigned)(nb < 1184 ? nb : 1184));
     if (cplx)
         grad_tv_kernel<true><<<gtv, 256, 0, st>>>(w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
-                                                  w.absmax);
+                                                  real_scale, w.absmax);
     else
         grad_tv_kernel<false><<<gtv, 256, 0, st>>>(w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
-                                                   w.absmax);
+                                                   real_scale, w.absmax);
     const int n_slabs = (int)((nb + GRAD_SLAB - 1) / GRAD_SLAB);
     grad_colsum_partial_kernel<<<dim3((g.M_eff + 127) / 128, n_slabs), 128, 0, st>>>(w.theta, nb, g.M_eff, w.part);
     grad_slab_reduce_kernel<<<(g.M_eff + 127) / 128, 128, 0, st>>>(w.part, n_slabs, g.M_eff, w.gb_acc, first_chunk);
     grad_a_partial_kernel<<<dim3((g.N + 127) / 128, n_slabs), 128, 0, st>>>(sigma, nb, g.N, (const float*)eloc, stats,
-                                                                            inv_B, cplx, w.part);
+                                                                            inv_B, cplx, (double)real_scale, w.part);
     grad_slab_reduce_kernel<<<(2 * g.N + 127) / 128, 128, 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk);
     grad_split_T_kernel<<<dim3(k_len / 32, g.M_eff / 32), dim3(32, 8), 0, st>>>(
         w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (__nv_bfloat16*)w.TwT);

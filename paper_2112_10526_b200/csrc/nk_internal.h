@@ -98,9 +98,13 @@ struct GradWs {
 int grad_slab();
 cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, int64_t B_total,
                                   const void* eloc, const double* stats, const GradWs& w, int first_chunk,
-                                  cudaStream_t st);
+                                  float real_scale, cudaStream_t st);   // real_scale: 2 (gradient 2 Re f~) | 1 (QGT)
 cudaError_t launch_gradient_finalize(const Geometry& g, int dtype, const GradWs& w, void* grad_a, void* grad_b,
                                      void* grad_W, cudaStream_t st);
+// qgt.cu : pieces of the QGT-vector product
+cudaError_t launch_qgt_w(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, const float* theta,
+                         const float* Y, const void* v_a, void* w_out, cudaStream_t st);
+cudaError_t launch_qgt_shift(void* out, const void* v, double shift, int64_t n_floats, cudaStream_t st);
 // logpsi.cu
 cudaError_t launch_logpsi(const int8_t* sigma, int64_t B, const Geometry& g, int dtype, const float* theta,
                           const void* a, void* logpsi_out, bool out_f64, void* theta_out, cudaStream_t st);

@@ -1,0 +1,89 @@
+"""GPU parity of nk_qgt_matvec against the float64 oracle's three-step product (Eq. (75)).
+
+Tolerance: every output entry is a sum over B samples of terms conj(O_s) (w_s - <w>) / B with |O| <= ~1; the kernel
+evaluates tanh(theta), w and the terms in fp32 (relative error ~1e-7 each) and contracts them exactly, so
+|out_gpu - out_ref| <= 1e-6 * max_s |w_s - <w>|  (+ 2e-7 of the output scale), the bound of tests/test_gpu_gradient.py.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import nk_oracle as orc
+from paper_2112_10526_b200 import inputs as inp
+
+pytestmark = pytest.mark.gpu
+
+
+def dev(x):
+    return None if x is None else torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def draw_v(p, seed):
+    rng = np.random.default_rng(seed)
+    def d(*sh):
+        x = rng.standard_normal(sh)
+        if p.complex_params:
+            return (x + 1j * rng.standard_normal(sh)).astype(np.complex64)
+        return x.astype(np.float32)
+    return d(p.n_sites), d(p.n_hidden), d(p.n_hidden, p.n_sites)
+
+
+def check(nk, p, v, shift, chunk, use_a=True, use_b=True):
+    va, vb, vW = v
+    out = nk.qgt_matvec(dev(p.sigma), dev(p.W), dev(p.b), dev(va) if use_a else None, dev(vb) if use_b else None,
+                        dev(vW), diag_shift=shift, chunk_size=chunk)
+    torch.cuda.synchronize()
+    za, zb = np.zeros_like(va), np.zeros_like(vb)
+    ref = orc.qgt_matvec(p.sigma, p.W, p.b, va if use_a else za, vb if use_b else zb, vW, shift)
+    J = orc.rbm_jacobian(p.sigma, p.W, p.b)
+    w = J @ orc.pack_params(va if use_a else za, vb if use_b else zb, vW).astype(J.dtype)
+    bound = 1e-6 * np.abs(w - w.mean()).max()
+    worst = 0.0
+    for name, g, r, vv, used in (("a", out[0], ref[0], va, use_a), ("b", out[1], ref[1], vb, use_b),
+                                 ("W", out[2], ref[2], vW, True)):
+        g = g.cpu().numpy().astype(r.dtype)
+        if not used:
+            r = r - 0.0                                  # shift * 0
+        scale = np.abs(r).max()
+        err = np.abs(g - r).max()
+        assert err <= bound + 2e-7 * scale + 1e-7 * shift * np.abs(vv).max(), f"out_{name}: err {err}, bound {bound}"
+        worst = max(worst, err / scale)
+    return worst
+
+
+@pytest.mark.parametrize("cfg,n,chunk", [(1, 1024, 0), (2, 500, 128), (3, 64, 0), (4, 160, 64), (5, 12, 0)])
+def test_qgt_matvec_parity_configs(nk, cfg, n, chunk):
+    p = inp.make_config(cfg, n_samples=n)
+    worst = check(nk, p, draw_v(p, 40 + cfg), 0.01, chunk)
+    print(f"cfg{cfg}: max QGT-vector error / max|out| = {worst:.2e}")
+
+
+def test_qgt_matvec_properties(nk):
+    p = inp.make_config(2, n_samples=256)
+    v, u = draw_v(p, 1), draw_v(p, 2)
+    sig, W, b = dev(p.sigma), dev(p.W), dev(p.b)
+    Gv = [t.cpu().numpy().astype(np.float64) for t in nk.qgt_matvec(sig, W, b, *map(dev, v))]
+    Gu = [t.cpu().numpy().astype(np.float64) for t in nk.qgt_matvec(sig, W, b, *map(dev, u))]
+    dot = lambda x, y: sum(float(np.vdot(a_, b_)) for a_, b_ in zip(x, y))
+    assert abs(dot(u, Gv) - dot(Gu, v)) < 1e-4 * abs(dot(u, Gv))          # symmetric
+    assert dot(v, Gv) > 0                                                 # positive semi-definite
+    # NULL blocks, missing outputs, zero shift; chunking is bit-reproducible per chunk size
+    check(nk, p, v, 0.0, 100, use_a=False, use_b=False)
+    o1 = nk.qgt_matvec(sig, W, b, *map(dev, v), diag_shift=0.1, chunk_size=64)
+    o2 = nk.qgt_matvec(sig, W, b, *map(dev, v), diag_shift=0.1, chunk_size=64)
+    assert all(torch.equal(x, y) for x, y in zip(o1, o2))
+    # a direction with constant O over the batch is annihilated: all samples identical
+    same = dev(np.tile(p.sigma[:1], (64, 1)))
+    z = nk.qgt_matvec(same, W, b, *map(dev, v))
+    assert max(float(t.abs().max()) for t in z) < 1e-5
+
+
+def test_qgt_matvec_complex_tiny_and_errors(nk):
+    p = inp.make_problem(inp.KIND_HEISENBERG, "chain", 7, 5, 33, seed=3, sz0=False, complex_params=True)
+    check(nk, p, draw_v(p, 9), 0.05, 0)
+    check(nk, p, draw_v(p, 9), 0.05, 10)
+    s, W = dev(p.sigma), dev(p.W)
+    with pytest.raises(nk.NkError):
+        nk.qgt_matvec(s, W, None, None, None, None)
+    with pytest.raises(nk.NkError):
+        nk.qgt_matvec(s, W, None, None, None, dev(draw_v(p, 1)[2]), diag_shift=-1.0)
