@@ -166,6 +166,18 @@ int nk_qgt_matvec(const int8_t* sigma, int64_t B, int N, int M, int dtype, const
                   void* out_a, void* out_b, void* out_W, void* workspace, size_t workspace_bytes,
                   nk_stream_t stream);
 
+/* Stochastic reconfiguration: solves  sum_j (G_ij + diag_shift delta_ij) delta_j = f_i  (Eq. (25) L886 with
+ * Eq. (30) L961 for real parameters — G = Re[G], f = 2 Re f~ — and Eq. (31) for the holomorphic complex RBM) by
+ * conjugate gradients (the paper's default solver, L969) started from zero; every iteration is one nk_qgt_matvec.
+ * f and delta are block-wise in the parameter dtype, all six pointers required (device).  Stops when
+ * |r| <= tol |f| or after max_iter iterations.  SYNCHRONISES `stream` (the residual is read back every few
+ * iterations).  info_host (host double[2], or NULL): iterations performed, final |r| / |f| of the CG recurrence. */
+size_t nk_sr_solve_workspace_bytes(int64_t B, int N, int M, int dtype, int64_t chunk_size);
+int nk_sr_solve(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* b,
+                const void* f_a, const void* f_b, const void* f_W, double diag_shift, double tol, int max_iter,
+                int64_t chunk_size, void* delta_a, void* delta_b, void* delta_W, double* info_host, void* workspace,
+                size_t workspace_bytes, nk_stream_t stream);
+
 /* ---- Metropolis-Hastings sampler for the RBM ------------------------------------------
  * PAPER.md Sec. 3.4: a proposal s -> s' is accepted with probability min(1, |psi(s')|^2 / |psi(s)|^2) (Eq. (20)
  * L709; both rules are symmetric kernels, L711).  Every row of sigma is one chain (n_chains = n_samples, L1583);

@@ -11,7 +11,7 @@ import os
 import numpy as np
 
 __all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host", "energy_gradient",
-           "qgt_matvec", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
+           "qgt_matvec", "sr_solve", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
            "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "NK_FORM_PRODUCT", "EXPORTS"]
 
 NK_HEISENBERG, NK_ISING = 0, 1
@@ -44,6 +44,9 @@ EXPORTS = {
     "nk_qgt_matvec_workspace_bytes": (_sz, [_i64, _int, _int, _int, _i64]),
     "nk_qgt_matvec": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _vp, _dbl, _i64, _vp, _vp, _vp, _vp, _sz,
                              _vp]),
+    "nk_sr_solve_workspace_bytes": (_sz, [_i64, _int, _int, _int, _i64]),
+    "nk_sr_solve": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _int, _i64, _vp, _vp, _vp,
+                           _vp, _vp, _sz, _vp]),
     "nk_metropolis_workspace_bytes": (_sz, [_int, _int, _i64, _int, _int, _int, _i64]),
     "nk_metropolis_sample": (_int, [_int, _vp, _int, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _u64, _u64, _u64,
                                     _i64, _vp, _vp, _sz, _vp]),
@@ -315,6 +318,34 @@ def qgt_matvec(sigma, W, b, v_a, v_b, v_W, *, diag_shift: float = 0.0, chunk_siz
                            ws.numel(), _stream())
     _check(rc, "nk_qgt_matvec")
     return out
+
+
+def sr_solve(sigma, W, b, f_a, f_b, f_W, *, diag_shift: float = 0.01, tol: float = 1e-5, max_iter: int = 200,
+             chunk_size: int = 0, ws=None):
+    """nk_sr_solve: delta = (G + diag_shift)^-1 f by conjugate gradients on the device.
+    Returns ((delta_a, delta_b, delta_W), iterations, relative residual)."""
+    torch = _torch()
+    lib = load()
+    _check_params(sigma, W, None, b)
+    B, N = sigma.shape
+    M = W.shape[0]
+    dt = _dtype_code(W)
+    for name, t, shape in (("f_a", f_a, (N,)), ("f_b", f_b, (M,)), ("f_W", f_W, (M, N))):
+        if t is None or t.dtype != W.dtype or tuple(t.shape) != shape or not t.is_contiguous() or not t.is_cuda:
+            raise NkError(f"{name} must be a contiguous CUDA tensor of W's dtype and shape {shape}")
+    out = (torch.empty(N, dtype=W.dtype, device=sigma.device), torch.empty(M, dtype=W.dtype, device=sigma.device),
+           torch.empty((M, N), dtype=W.dtype, device=sigma.device))
+    nbytes = lib.nk_sr_solve_workspace_bytes(B, N, M, dt, int(chunk_size))
+    if nbytes == 0:
+        raise NkError("nk_sr_solve_workspace_bytes rejected the arguments")
+    if ws is None or ws.numel() < nbytes:
+        ws = torch.empty(nbytes, dtype=torch.uint8, device=sigma.device)
+    info = np.zeros(2, dtype=np.float64)
+    rc = lib.nk_sr_solve(_ptr(sigma), B, N, M, dt, _ptr(W), _ptr(b), _ptr(f_a), _ptr(f_b), _ptr(f_W),
+                         float(diag_shift), float(tol), int(max_iter), int(chunk_size), _ptr(out[0]), _ptr(out[1]),
+                         _ptr(out[2]), info.ctypes.data, _ptr(ws), ws.numel(), _stream())
+    _check(rc, "nk_sr_solve")
+    return out, int(info[0]), float(info[1])
 
 
 def metropolis_sample(sigma, W, a=None, b=None, *, rule: int = NK_RULE_LOCAL, clusters=None, n_steps: int | None = None,

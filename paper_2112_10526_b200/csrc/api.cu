@@ -1,5 +1,6 @@
 // C ABI of libnkb200.so (include/nkb200.h): argument validation, workspace carving, the chunked driver
 // (Sec. 3.3.1: chunk_size bounds the configurations evaluated at once).
+#include <cmath>
 #include <cstdlib>
 #include <new>
 #include <vector>
@@ -439,6 +440,100 @@ int nk_qgt_matvec(const int8_t* sigma, int64_t B, int N, int M, int dtype, const
     NK_CUDA(launch_qgt_shift(out_a, v_a, diag_shift, (int64_t)N * e, st));
     NK_CUDA(launch_qgt_shift(out_b, v_b, diag_shift, (int64_t)M * e, st));
     NK_CUDA(launch_qgt_shift(out_W, v_W, diag_shift, (int64_t)M * N * e, st));
+    return NK_OK;
+}
+
+// ---- stochastic reconfiguration: (G + eps) delta = f by conjugate gradients -----------------------------------
+namespace {
+struct SrWs {
+    float *x, *r, *p, *Ap;       // packed [a | b | W] vectors, n floats each
+    double *part, *scal;         // reduction partials; scal[0..1] = rr (ping-pong), [2] = pAp, [3] = |f|^2
+    void* qgt;
+    size_t qgt_bytes, bytes;
+    int64_t n;
+};
+SrWs carve_sr(void* ws, int64_t B, int N, int M, int dtype, int64_t chunk_size) {
+    const int64_t e = dtype == NK_C64 ? 2 : 1;
+    Carver c(ws);
+    SrWs w;
+    w.n = ((int64_t)N + M + (int64_t)M * N) * e;
+    w.x = c.take<float>(w.n); w.r = c.take<float>(w.n); w.p = c.take<float>(w.n); w.Ap = c.take<float>(w.n);
+    w.part = c.take<double>(cg_partials());
+    w.scal = c.take<double>(8);
+    w.qgt_bytes = nk_qgt_matvec_workspace_bytes(B, N, M, dtype, chunk_size);
+    w.qgt = c.take<uint8_t>(w.qgt_bytes);
+    w.bytes = c.off;
+    return w;
+}
+}  // namespace
+
+size_t nk_sr_solve_workspace_bytes(int64_t B, int N, int M, int dtype, int64_t chunk_size) {
+    if (bad_dims(B, N, M, dtype) || chunk_size < 0) return 0;
+    return carve_sr(nullptr, B, N, M, dtype, chunk_size).bytes;
+}
+
+int nk_sr_solve(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* b,
+                const void* f_a, const void* f_b, const void* f_W, double diag_shift, double tol, int max_iter,
+                int64_t chunk_size, void* delta_a, void* delta_b, void* delta_W, double* info_host, void* workspace,
+                size_t workspace_bytes, nk_stream_t stream) {
+    if (bad_dims(B, N, M, dtype) || B == 0 || chunk_size < 0 || !sigma || !W || !f_a || !f_b || !f_W || !delta_a ||
+        !delta_b || !delta_W || diag_shift < 0.0 || !(tol >= 0.0) || max_iter < 0)
+        return NK_ERR_INVALID_ARG;
+    const Geometry g = make_geometry(nullptr, N, M, dtype);
+    if (g.M_pad / MPAD_ALIGN > (dtype == NK_C64 ? MAX_V_CPLX : MAX_V_REAL) || N > 65535) return NK_ERR_UNSUPPORTED;
+    if (!workspace || ((uintptr_t)workspace & 255) ||
+        workspace_bytes < carve_sr(nullptr, B, N, M, dtype, chunk_size).bytes)
+        return NK_ERR_WORKSPACE;
+    const SrWs w = carve_sr(workspace, B, N, M, dtype, chunk_size);
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t fsz = sizeof(float) * (dtype == NK_C64 ? 2 : 1);
+    const size_t na = (size_t)N * fsz, nb_ = (size_t)M * fsz, nW = (size_t)M * N * fsz;
+    auto blk = [&](float* v, int which) -> void* {
+        uint8_t* q = (uint8_t*)v;
+        return which == 0 ? (void*)q : which == 1 ? (void*)(q + na) : (void*)(q + na + nb_);
+    };
+    // x0 = 0, r0 = p0 = f
+    NK_CUDA(cudaMemsetAsync(w.x, 0, (size_t)w.n * sizeof(float), st));
+    const void* fsrc[3] = {f_a, f_b, f_W};
+    const size_t fbytes[3] = {na, nb_, nW};
+    for (int k = 0; k < 3; ++k) {
+        NK_CUDA(cudaMemcpyAsync(blk(w.r, k), fsrc[k], fbytes[k], cudaMemcpyDeviceToDevice, st));
+        NK_CUDA(cudaMemcpyAsync(blk(w.p, k), fsrc[k], fbytes[k], cudaMemcpyDeviceToDevice, st));
+    }
+    NK_CUDA(launch_cg_dot(w.r, w.r, w.n, w.part, w.scal + 0, st));
+    NK_CUDA(cudaMemcpyAsync(w.scal + 3, w.scal + 0, sizeof(double), cudaMemcpyDeviceToDevice, st));
+    double h[4] = {0, 0, 0, 0};
+    NK_CUDA(cudaMemcpyAsync(h, w.scal, sizeof(h), cudaMemcpyDeviceToHost, st));
+    NK_CUDA(cudaStreamSynchronize(st));
+    const double ff = h[0];
+    double rr = ff;
+    int it = 0;
+    const int check_every = 4;           // the residual is read back (one synchronisation) every few iterations
+    while (it < max_iter && ff > 0.0 && rr > tol * tol * ff) {
+        const int cur = it & 1, nxt = cur ^ 1;
+        const int rc = nk_qgt_matvec(sigma, B, N, M, dtype, W, b, blk(w.p, 0), blk(w.p, 1), blk(w.p, 2), diag_shift,
+                                     chunk_size, blk(w.Ap, 0), blk(w.Ap, 1), blk(w.Ap, 2), w.qgt, w.qgt_bytes, stream);
+        if (rc != NK_OK) return rc;
+        NK_CUDA(launch_cg_dot(w.p, w.Ap, w.n, w.part, w.scal + 2, st));
+        NK_CUDA(launch_cg_step(w.x, w.r, w.p, w.Ap, w.n, w.scal + cur, w.scal + 2, st));
+        NK_CUDA(launch_cg_dot(w.r, w.r, w.n, w.part, w.scal + nxt, st));
+        NK_CUDA(launch_cg_dir(w.p, w.r, w.n, w.scal + nxt, w.scal + cur, st));
+        ++it;
+        if (it % check_every == 0 || it == max_iter) {
+            NK_CUDA(cudaMemcpyAsync(h, w.scal, sizeof(h), cudaMemcpyDeviceToHost, st));
+            NK_CUDA(cudaStreamSynchronize(st));
+            rr = h[nxt];
+            if (!(h[2] > 0.0)) break;    // p^dagger A p <= 0 or NaN: breakdown, stop with what we have
+        }
+    }
+    void* dst[3] = {delta_a, delta_b, delta_W};
+    for (int k = 0; k < 3; ++k)
+        NK_CUDA(cudaMemcpyAsync(dst[k], blk(w.x, k), fbytes[k], cudaMemcpyDeviceToDevice, st));
+    NK_CUDA(cudaStreamSynchronize(st));
+    if (info_host) {
+        info_host[0] = (double)it;
+        info_host[1] = ff > 0.0 ? sqrt(rr / ff) : 0.0;
+    }
     return NK_OK;
 }
 

@@ -105,6 +105,13 @@ cudaError_t launch_gradient_finalize(const Geometry& g, int dtype, const GradWs&
 cudaError_t launch_qgt_w(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, const float* theta,
                          const float* Y, const void* v_a, void* w_out, cudaStream_t st);
 cudaError_t launch_qgt_shift(void* out, const void* v, double shift, int64_t n_floats, cudaStream_t st);
+// cg.cu : conjugate-gradient pieces of the SR solve
+int cg_partials();
+cudaError_t launch_cg_dot(const float* x, const float* y, int64_t n, double* part, double* out, cudaStream_t st);
+cudaError_t launch_cg_step(float* x, float* r, const float* p, const float* Ap, int64_t n, const double* rr,
+                           const double* pAp, cudaStream_t st);
+cudaError_t launch_cg_dir(float* p, const float* r, int64_t n, const double* rr_new, const double* rr_old,
+                          cudaStream_t st);
 // logpsi.cu
 cudaError_t launch_logpsi(const int8_t* sigma, int64_t B, const Geometry& g, int dtype, const float* theta,
                           const void* a, void* logpsi_out, bool out_f64, void* theta_out, cudaStream_t st);

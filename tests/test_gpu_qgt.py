@@ -87,3 +87,67 @@ def test_qgt_matvec_complex_tiny_and_errors(nk):
         nk.qgt_matvec(s, W, None, None, None, None)
     with pytest.raises(nk.NkError):
         nk.qgt_matvec(s, W, None, None, None, dev(draw_v(p, 1)[2]), diag_shift=-1.0)
+
+
+# ------------------------------------------------------------------ nk_sr_solve: CG against the dense direct solve
+def _sr_case(nk, p, shift, tol, chunk=0):
+    cplx = p.complex_params
+    f = draw_v(p, 77)
+    (da, db, dW), iters, res = nk.sr_solve(dev(p.sigma), dev(p.W), dev(p.b), *map(dev, f), diag_shift=shift, tol=tol,
+                                           max_iter=400, chunk_size=chunk)
+    delta = orc.pack_params(*(t.cpu().numpy() for t in (da, db, dW))).astype(np.complex128 if cplx else np.float64)
+    G = orc.qgt_dense(p.sigma, p.W, p.b)
+    if not cplx:
+        G = G.real
+    A = G + shift * np.eye(G.shape[0])
+    fv = orc.pack_params(*f).astype(A.dtype)
+    ref = orc.pack_params(*orc.sr_solve(p.sigma, p.W, p.b, *f, shift))
+    true_res = np.linalg.norm(A @ delta - fv) / np.linalg.norm(fv)
+    cond = np.linalg.cond(A)
+    err = np.linalg.norm(delta - ref) / np.linalg.norm(ref)
+    return iters, res, true_res, err, cond
+
+
+@pytest.mark.parametrize("case", [
+    dict(cfg=1, n=2048, shift=0.05),
+    dict(kind=0, lattice="square", L=4, M=16, n=1500, shift=0.02),
+    dict(kind=1, lattice="chain", L=9, M=20, n=1000, shift=0.05, h=1.0, complex_params=True),
+])
+def test_sr_solve_matches_dense_solve(nk, case):
+    case = dict(case)
+    shift, n = case.pop("shift"), case.pop("n")
+    if "cfg" in case:
+        p = inp.make_config(case["cfg"], n_samples=n)
+    else:
+        p = inp.make_problem(case.pop("kind"), case.pop("lattice"), case.pop("L"), case.pop("M"), n, seed=8,
+                             scale=0.2, **case)
+    tol = 1e-5
+    iters, res, true_res, err, cond = _sr_case(nk, p, shift, tol)
+    print(f"{p.name}: P = {p.n_sites + p.n_hidden * (1 + p.n_sites)}, cond {cond:.1f}, {iters} CG iterations, "
+          f"recurrence residual {res:.1e}, true residual {true_res:.1e}, |delta - dense| / |dense| = {err:.1e}")
+    assert 0 < iters < 400 and res <= tol
+    assert true_res <= 5 * tol + 2e-6            # the fp32 recurrence residual tracks the fp64 true residual
+    assert err <= cond * (5 * tol + 2e-6)        # |dx| / |x| <= cond * |r| / |f|
+
+
+def test_sr_solve_limits_and_errors(nk):
+    p = inp.make_config(1, n_samples=512)
+    f = draw_v(p, 5)
+    sig, W, b = dev(p.sigma), dev(p.W), dev(p.b)
+    # max_iter = 0 returns zero; a huge shift makes delta = f / shift after one iteration
+    (da, db, dW), iters, res = nk.sr_solve(sig, W, b, *map(dev, f), max_iter=0)
+    assert iters == 0 and float(dW.abs().max()) == 0.0 and res == 1.0
+    (da, db, dW), iters, res = nk.sr_solve(sig, W, b, *map(dev, f), diag_shift=1e6, tol=1e-4)
+    np.testing.assert_allclose(dW.cpu().numpy() * 1e6, f[2], rtol=1e-3, atol=1e-3)
+    assert iters <= 4
+    # f = 0 -> delta = 0 without iterating; chunked run reproduces the unchunked solution to CG accuracy
+    z = tuple(np.zeros_like(x) for x in f)
+    (da, db, dW), iters, _ = nk.sr_solve(sig, W, b, *map(dev, z))
+    assert iters == 0 and float(da.abs().max()) == 0.0
+    x0, _, _ = nk.sr_solve(sig, W, b, *map(dev, f), diag_shift=0.05, tol=1e-6)
+    x1, _, _ = nk.sr_solve(sig, W, b, *map(dev, f), diag_shift=0.05, tol=1e-6, chunk_size=100)
+    assert float((x0[2] - x1[2]).abs().max()) <= 1e-4 * float(x0[2].abs().max())
+    with pytest.raises(nk.NkError):
+        nk.sr_solve(sig, W, b, dev(f[0]), dev(f[1]), None)
+    with pytest.raises(nk.NkError):
+        nk.sr_solve(sig, W, b, *map(dev, f), tol=-1.0)
