@@ -172,6 +172,13 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
                       device=sigma.device)
     ms_grad = _time_ms(torch, lambda: nk.energy_gradient(chains, W, b, eloc, stats, chunk_size=p.chunk_size, ws=gws), 3)
     ms_eloc = _time_ms(torch, lambda: plan.run(chains, W, a, b), 3)
+    # QGT-vector product (one CG iteration of stochastic reconfiguration is this plus 4 vector kernels)
+    ga, gb, gW = nk.energy_gradient(chains, W, b, eloc, stats, chunk_size=p.chunk_size, ws=gws)
+    qws = torch.empty(lib.nk_qgt_matvec_workspace_bytes(B, N, M, dt_code, p.chunk_size), dtype=torch.uint8,
+                      device=sigma.device)
+    qout = (torch.empty_like(ga), torch.empty_like(gb), torch.empty_like(gW))
+    ms_qgt = _time_ms(torch, lambda: nk.qgt_matvec(chains, W, b, ga, gb, gW, diag_shift=0.01,
+                                                   chunk_size=p.chunk_size, ws=qws, out=qout), 3)
     planes = 2 if p.complex_params else 1
     # product-form variant of the same step (nk_local_energy_ex, NK_FORM_PRODUCT), fused kernel timed by the library
     pplan = nk.LocalEnergyPlan(op, B, N, M, dt_code, p.chunk_size, device=sigma.device, flags=nk.NK_FORM_PRODUCT)
@@ -194,6 +201,9 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
                     "roofline": {"bound": "alu", "kernel": "metropolis_kernel", "unit": "Gpair/s",
                                  "achieved": pairs / (ms_sweep * 1e-3) / 1e9}},
         "gradient": {"ms": ms_grad, "algorithmic_tflops": 2.0 * planes * B * M * N / (ms_grad * 1e-3) / 1e12},
+        "qgt_matvec": {"ms": ms_qgt, "n_parameters": N + M + M * N,
+                       "algorithmic_tflops": 3 * 2.0 * planes * B * M * N / (ms_qgt * 1e-3) / 1e12,
+                       "what": "(G + 0.01) v on the fly, Eq. (75): theta, V_W sigma and J^dagger dw contractions"},
         "vmc_iteration": {"ms": ms_sweep + ms_eloc + ms_grad, "ms_local_energy_on_sampled_chains": ms_eloc,
                           "what": "one sweep + local energies + energy gradient, same batch, device-resident"},
     }
