@@ -3,9 +3,12 @@
 //   MetropolisLocal: negate one spin; MetropolisExchange: swap the spins of one pair of a cluster list     L713
 // One warp owns one chain for the whole call (n_chains = n_samples, L1583): theta_s = KAPPA theta lives in registers
 // exactly as in the fused local-energy kernel (rbm_lane_state.cuh), a proposal costs one row of the table Dtab
-// (theta' = theta - 2 s_k W[:,k], or - 2 s_i (W[:,i] - W[:,j])), read straight from L2 — every chain needs a
-// different row at every transition, so there is nothing to stage in shared memory — and an accepted move
-// overwrites theta in place.  ln psi is never formed: the ratio psi'/psi comes out of the same 1-MUFU-per-pair
+// (theta' = theta - 2 s_k W[:,k], or - 2 s_i (W[:,i] - W[:,j])).  Every chain needs a different row at every
+// transition, so rows are not shared between warps; instead each warp owns two row buffers in shared memory and,
+// while it evaluates one proposal, a bulk async copy (TMA engine, completing on the warp's own mbarrier) already
+// brings the row of its next non-trivial proposal from L2 — proposal indices do not depend on the state, and whether
+// a coming exchange is trivial is judged on the current spins (a rare misjudgement costs one wasted or one late
+// copy, never a wrong result).  An accepted move re-reads the row from shared memory and overwrites theta in place.  ln psi is never formed: the ratio psi'/psi comes out of the same 1-MUFU-per-pair
 // product form as in fused_eloc.cu.
 //
 // Random numbers (S1-S3): Philox4x32-10, counter = (chain lo, hi, transition lo, hi), key = (seed lo, hi)
@@ -19,7 +22,7 @@
 
 namespace nk {
 
-constexpr int SW = 16;                       // warps (chains) per CTA
+constexpr int SW = 16;                       // most warps (chains) per CTA; fewer when two rows per warp do not fit
 
 struct SamplerParams {
     int8_t* sigma;
@@ -30,7 +33,7 @@ struct SamplerParams {
     const float* Dtab;
     const int32_t* pairs;
     const float* a;
-    int rule, n_idx;
+    int rule, n_idx, sw;                     // sw = warps per CTA of this launch
     int64_t n_steps;
     uint32_t key0, key1;
     uint64_t step_offset, chain0;
@@ -53,14 +56,46 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 
 template <int V, bool CPLX>
 constexpr int sampler_min_blocks() { return ((CPLX ? 8 : 4) * V <= 16) ? 2 : 1; }
+// warps per CTA: two row buffers of V * 512 B (x2 complex) per warp must fit; 12 warps leave 168 registers per thread
+// Rows are staged through shared memory (STAGED) only where that was measured to win: rows of 8 KB (config 5:
+// 40.3 -> 35.6 ms per sweep, with 12 warps); for rows of <= 4 KB the direct L2 reads of 16 warps were faster
+// (configs 3, 4: 1.51 vs 1.68 ms, 0.66 vs 0.71 ms).
+template <int V, bool CPLX>
+__host__ __device__ constexpr int sampler_warps() { return (16 * 2 * V * 512 * (CPLX ? 2 : 1) <= 216 * 1024) ? 16 : 12; }
 
 template <int V, bool CPLX>
-__global__ void __launch_bounds__(SW * 32, (sampler_min_blocks<V, CPLX>())) metropolis_kernel(const SamplerParams p) {
-    extern __shared__ __align__(16) uint32_t sbits[];
+__global__ void __launch_bounds__(sampler_warps<V, CPLX>() * 32, (sampler_min_blocks<V, CPLX>())) metropolis_kernel(const SamplerParams p) {
+    extern __shared__ __align__(128) uint8_t smem_s[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t c_loc = (int64_t)blockIdx.x * SW + warp;
+    const int64_t c_loc = (int64_t)blockIdx.x * p.sw + warp;
     if (c_loc >= p.nb) return;                         // no CTA-wide synchronisation below
-    uint32_t* bits = sbits + (size_t)warp * p.n_words; // bit i set <=> sigma_i = -1
+    // shared memory: [sw warps][2 row buffers][M_eff floats] | [sw][n_words] spin bits | [sw][2] mbarriers
+    const uint32_t row_bytes = (uint32_t)p.M_eff * 4u;
+    const size_t rows_bytes = (sampler_warps<V, CPLX>() < 16) ? (size_t)p.sw * 2 * row_bytes : 0;
+    float* rowbuf = reinterpret_cast<float*>(smem_s) + (size_t)warp * 2 * p.M_eff;
+    uint32_t* bits = reinterpret_cast<uint32_t*>(smem_s + rows_bytes) + (size_t)warp * p.n_words;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_s + rows_bytes + (size_t)p.sw * p.n_words * 4) +
+                     warp * 2;                          // bit i of `bits` set <=> sigma_i = -1
+    const uint32_t bar0 = smem_u32(bars), row0 = smem_u32(rowbuf);
+    constexpr bool STAGED = sampler_warps<V, CPLX>() < 16;
+    if (STAGED && lane == 0) {
+        mbar_init(bar0, 1);
+        mbar_init(bar0 + 8, 1);
+        mbar_fence_init();
+    }
+    uint32_t phase = 0u;                               // bit `slot` = parity the next wait on that slot expects
+    auto issue_row = [&](int slot, int row) {          // all lanes are past their reads of this slot (warp converged)
+        __syncwarp();
+        if (lane == 0) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            mbar_arrive_expect_tx(bar0 + 8 * slot, row_bytes);
+            bulk_g2s(row0 + slot * row_bytes, p.Dtab + (size_t)row * p.M_eff, row_bytes, bar0 + 8 * slot);
+        }
+    };
+    auto wait_row = [&](int slot) {
+        mbar_wait(bar0 + 8 * slot, (phase >> slot) & 1u);
+        phase ^= 1u << slot;
+    };
     int8_t* sp = p.sigma + c_loc * p.N;
     for (int wi = lane; wi < p.n_words; wi += 32) {
         uint32_t w = 0;
@@ -93,6 +128,7 @@ __global__ void __launch_bounds__(SW * 32, (sampler_min_blocks<V, CPLX>())) metr
             a2_l *= 2.f * LOG2E;
         }
         const int cnt = (p.n_steps - t0 < 32) ? (int)(p.n_steps - t0) : 32;
+        int pend_tt = -1, pend_slot = 0;              // a row copy in flight for transition pend_tt of this batch
         for (int tt = 0; tt < cnt; ++tt) {
             const int idx = __shfl_sync(0xffffffffu, idx_l, tt);
             const int i = __shfl_sync(0xffffffffu, i_l, tt);
@@ -101,9 +137,31 @@ __global__ void __launch_bounds__(SW * 32, (sampler_min_blocks<V, CPLX>())) metr
             const float a2 = __shfl_sync(0xffffffffu, a2_l, tt);
             const uint32_t bi = (bits[i >> 5] >> (i & 31)) & 1u;
             const uint32_t bj = (j >= 0) ? ((bits[j >> 5] >> (j & 31)) & 1u) : (bi ^ 1u);
-            if (bi == bj) { ++n_acc; continue; }      // exchange of equal spins: s' = s, ratio 1
+            int slot = 0;
+            if constexpr (!STAGED) {
+                if (bi == bj) { ++n_acc; continue; }  // exchange of equal spins: s' = s, ratio 1
+            } else if (pend_tt == tt) {                      // the prefetched row is this transition's
+                pend_tt = -1;
+                if (bi == bj) { wait_row(pend_slot); ++n_acc; continue; }   // turned trivial meanwhile: drop it
+                slot = pend_slot;
+            } else {
+                if (bi == bj) { ++n_acc; continue; }  // exchange of equal spins: s' = s, ratio 1
+                if (pend_tt >= 0) { wait_row(pend_slot); pend_tt = -1; }    // misjudged: drop the later row
+                issue_row(0, idx);                    // first of a batch, or misjudged as trivial: fetch now
+            }
+            if constexpr (STAGED) {   // start the copy of the next proposal that is non-trivial on the current spins
+                const uint32_t bi_l = (bits[i_l >> 5] >> (i_l & 31)) & 1u;
+                const uint32_t bj_l = (j_l >= 0) ? ((bits[j_l >> 5] >> (j_l & 31)) & 1u) : (bi_l ^ 1u);
+                const unsigned cand = __ballot_sync(0xffffffffu, lane > tt && lane < cnt && bi_l != bj_l);
+                if (cand) {
+                    pend_tt = __ffs(cand) - 1;
+                    pend_slot = slot ^ 1;
+                    issue_row(pend_slot, __shfl_sync(0xffffffffu, idx_l, pend_tt));
+                }
+            }
+            if constexpr (STAGED) wait_row(slot);
             const float s = bi ? 1.f : -1.f;          // s = -sigma_i
-            const float* drow = p.Dtab + (size_t)idx * p.M_eff;
+            const float* drow = STAGED ? rowbuf + (size_t)slot * p.M_eff : p.Dtab + (size_t)idx * p.M_eff;
             bool accept;
             if constexpr (!CPLX) {
                 float praw, acc;
@@ -166,7 +224,13 @@ cudaError_t launch_metropolis(const Geometry& g, int dtype, int8_t* sigma, int64
     const int V = g.M_pad / MPAD_ALIGN;
     SamplerFn fn = cplx ? pick_scplx<1>(V) : pick_sreal<1>(V);
     if (fn == nullptr) return cudaErrorInvalidValue;
-    const size_t smem = (size_t)SW * g.n_words * 4;
+    // as many warps per CTA (a multiple of 4, one chain each) as fit with two row buffers per warp
+    int sw = (16 * 2 * (size_t)g.M_eff * 4 <= (size_t)216 * 1024) ? 16 : 12;      // = sampler_warps<V, CPLX>()
+    const bool staged = sw < 16;
+    const size_t per_warp = (staged ? (size_t)2 * g.M_eff * 4 : 0) + (size_t)g.n_words * 4 + 16;
+    while (sw > 4 && sw * per_warp + 128 > (size_t)220 * 1024) sw -= 4;
+    const size_t smem = sw * per_warp + 128;
+    if (smem > (size_t)227 * 1024) return cudaErrorInvalidValue;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -174,11 +238,11 @@ cudaError_t launch_metropolis(const Geometry& g, int dtype, int8_t* sigma, int64
     SamplerParams p;
     p.sigma = sigma; p.nb = nb; p.N = g.N; p.n_words = g.n_words;
     p.theta = theta; p.M_pad = g.M_pad; p.M_eff = g.M_eff; p.Dtab = Dtab;
-    p.pairs = sa.pairs; p.a = (const float*)sa.a; p.rule = sa.rule; p.n_idx = sa.n_idx; p.n_steps = sa.n_steps;
+    p.pairs = sa.pairs; p.a = (const float*)sa.a; p.rule = sa.rule; p.n_idx = sa.n_idx; p.sw = sw; p.n_steps = sa.n_steps;
     p.key0 = (uint32_t)sa.seed; p.key1 = (uint32_t)(sa.seed >> 32);
     p.step_offset = sa.step_offset; p.chain0 = sa.chain0; p.accepted = accepted;
-    const int64_t grid = (nb + SW - 1) / SW;
-    fn<<<(unsigned)grid, SW * 32, smem, st>>>(p);
+    const int64_t grid = (nb + sw - 1) / sw;
+    fn<<<(unsigned)grid, sw * 32, smem, st>>>(p);
     count_launch();
     return cudaGetLastError();
 }
