@@ -285,3 +285,51 @@ def sr_solve(sigma, W, b, f_a, f_b, f_W, diag_shift):
         G = G.real
     f = pack_params(f_a, f_b, f_W).astype(G.dtype)
     return unpack_params(np.linalg.solve(G + diag_shift * np.eye(G.shape[0]), f), N, M)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# NEXT-4, second workload: the fully symmetric RBM (RBMSymm)
+# ---------------------------------------------------------------------------------------------------------
+def rbmsymm_features(sigma, W_sym, b_sym, perms):
+    """f_g^(i)(s) = sum_r W^(i)_r s_{g r} + b^(i)   (the embedding layer, Eq. (56), with a bias per feature).
+    sigma [B][N]; W_sym [F][N]; b_sym [F] or None; perms int [G][N] with perms[g][r] = the site g r.  Returns [B][F][G]."""
+    sigma = np.atleast_2d(np.asarray(sigma))
+    cplx = np.iscomplexobj(W_sym)
+    W = _up(W_sym, cplx)
+    s = sigma.astype(W.dtype)
+    perms = np.asarray(perms)
+    f = np.einsum("ir,sgr->sig", W, s[:, perms])         # s[:, perms][s][g][r] = s_{g r}
+    if b_sym is not None:
+        f = f + _up(b_sym, cplx)[None, :, None]
+    return f
+
+
+def rbmsymm_logpsi(sigma, W_sym, b_sym, perms):
+    """ln psi = sum_{i, g in G} ln cosh f_g^(i)   (Eq. (41))."""
+    f = rbmsymm_features(sigma, W_sym, b_sym, perms)
+    return log_cosh(f).reshape(f.shape[0], -1).sum(axis=1)
+
+
+def rbmsymm_local_energy(kind, sigma, bonds, colors, J, h, W_sym, b_sym, perms, flags=0):
+    """Eq. (12) L652 for the symmetric RBM, every ln psi(s') from scratch through `rbmsymm_logpsi`."""
+    sigma = np.atleast_2d(np.asarray(sigma))
+    lp = rbmsymm_logpsi(sigma, W_sym, b_sym, perms)
+    out = np.zeros(sigma.shape[0], dtype=np.complex128 if np.iscomplexobj(W_sym) else np.float64)
+    for n in range(sigma.shape[0]):
+        eta, mels, _, _ = connected(kind, sigma[n], bonds, colors, J, h, flags)
+        out[n] = np.sum(mels * np.exp(rbmsymm_logpsi(eta, W_sym, b_sym, perms) - lp[n]))
+    return out, lp
+
+
+def rbmsymm_energy_gradient(sigma, W_sym, b_sym, perms, eloc):
+    """Gradient of <H> with respect to the tied parameters: O_{b^(i)} = sum_g tanh f_g^(i),
+    O_{W^(i)_r} = sum_g tanh f_g^(i) s_{g r} (Eq. (13) applied to Eq. (41)/(56)); f~ = E[O^* (H~ - E[H~])], gradient
+    2 Re f~ (real) or f~ (complex), Eq. (14)-(16).  Returns (g_b [F], g_W [F][N])."""
+    sigma = np.atleast_2d(np.asarray(sigma))
+    cplx = np.iscomplexobj(W_sym)
+    T = np.tanh(rbmsymm_features(sigma, W_sym, b_sym, perms))       # [B][F][G]
+    s = sigma.astype(T.dtype)[:, np.asarray(perms)]                   # [B][G][N]: s_{g r}
+    O_b = T.sum(axis=2)
+    O_W = np.einsum("sig,sgr->sir", T, s)
+    gb, gW = force(O_b, eloc), force(O_W, eloc)
+    return (gb, gW) if cplx else (2.0 * gb.real, 2.0 * gW.real)

@@ -148,3 +148,13 @@ def make_problem(kind: int, lattice: str, L: int, n_hidden: int, n_samples: int,
     sigma = draw_samples(np.random.default_rng(2000 + seed), n_samples, N, sz0)
     return Problem(f"{lattice}{L}_k{kind}_M{n_hidden}_s{seed}", kind, N, n_hidden, bonds, colors, J, float(h),
                    complex_params, W, a, b, sigma, chunk_size)
+
+
+def translation_perms(lattice: str, L: int) -> np.ndarray:
+    """Translation group of the periodic chain (|G| = L) or L x L square lattice (|G| = L^2) as site permutations:
+    perms[g][r] = the site g r, with site = x * L + y as in `square_bonds`; g = 0 is the identity."""
+    if lattice == "chain":
+        r = np.arange(L)
+        return np.stack([(r + t) % L for t in range(L)]).astype(np.int32)
+    x, y = np.divmod(np.arange(L * L), L)
+    return np.stack([(((x + tx) % L) * L + (y + ty) % L) for tx in range(L) for ty in range(L)]).astype(np.int32)
