@@ -178,6 +178,21 @@ int nk_sr_solve(const int8_t* sigma, int64_t B, int N, int M, int dtype, const v
                 int64_t chunk_size, void* delta_a, void* delta_b, void* delta_W, double* info_host, void* workspace,
                 size_t workspace_bytes, nk_stream_t stream);
 
+/* ---- fully symmetric RBM (RBMSymm, second workload) ----------------------------------
+ * PAPER.md Eq. (41): ln psi = sum_{i, g in G} ln cosh f_g^(i), with the embedding of Eq. (56),
+ * f_g^(i) = sum_r W^(i)_r s_{g r} + b^(i).  This is an RBM with M = n_features * n_group tied hidden units; hidden
+ * unit (i, g) is row i * n_group + g:   W[(i,g)][g r] = W_sym[i][r],  b[(i,g)] = b_sym[i].
+ *   perms  dev int32 [n_group][N], perms[g][r] = the site g r; every row must be a permutation of 0..N-1 (caller's
+ *          responsibility: an out-of-range entry is an out-of-bounds write)
+ * nk_rbmsymm_expand writes the expanded (W [M][N], b [M] or NULL) to pass to any other call of this library (no
+ * visible bias: a = NULL); nk_rbmsymm_reduce_gradient maps a gradient / force / QGT-vector block of the expanded
+ * parameters to the tied ones by summing over orbits (the tying is linear):
+ *   grad_W_sym[i][r] = sum_g grad_W[(i,g)][g r],   grad_b_sym[i] = sum_g grad_b[(i,g)]   (fp64 sums, fixed order). */
+int nk_rbmsymm_expand(int n_features, int n_group, int N, int dtype, const void* W_sym, const void* b_sym,
+                      const int32_t* perms, void* W_out, void* b_out, nk_stream_t stream);
+int nk_rbmsymm_reduce_gradient(int n_features, int n_group, int N, int dtype, const void* grad_W, const void* grad_b,
+                               const int32_t* perms, void* grad_W_sym, void* grad_b_sym, nk_stream_t stream);
+
 /* ---- Metropolis-Hastings sampler for the RBM ------------------------------------------
  * PAPER.md Sec. 3.4: a proposal s -> s' is accepted with probability min(1, |psi(s')|^2 / |psi(s)|^2) (Eq. (20)
  * L709; both rules are symmetric kernels, L711).  Every row of sigma is one chain (n_chains = n_samples, L1583);

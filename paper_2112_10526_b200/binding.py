@@ -11,7 +11,7 @@ import os
 import numpy as np
 
 __all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host", "energy_gradient",
-           "qgt_matvec", "sr_solve", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
+           "qgt_matvec", "sr_solve", "rbmsymm_expand", "rbmsymm_reduce_gradient", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
            "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "NK_FORM_PRODUCT", "EXPORTS"]
 
 NK_HEISENBERG, NK_ISING = 0, 1
@@ -47,6 +47,8 @@ EXPORTS = {
     "nk_sr_solve_workspace_bytes": (_sz, [_i64, _int, _int, _int, _i64]),
     "nk_sr_solve": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _int, _i64, _vp, _vp, _vp,
                            _vp, _vp, _sz, _vp]),
+    "nk_rbmsymm_expand": (_int, [_int, _int, _int, _int, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "nk_rbmsymm_reduce_gradient": (_int, [_int, _int, _int, _int, _vp, _vp, _vp, _vp, _vp, _vp]),
     "nk_metropolis_workspace_bytes": (_sz, [_int, _int, _i64, _int, _int, _int, _i64]),
     "nk_metropolis_sample": (_int, [_int, _vp, _int, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _u64, _u64, _u64,
                                     _i64, _vp, _vp, _sz, _vp]),
@@ -346,6 +348,42 @@ def sr_solve(sigma, W, b, f_a, f_b, f_W, *, diag_shift: float = 0.01, tol: float
                          _ptr(out[2]), info.ctypes.data, _ptr(ws), ws.numel(), _stream())
     _check(rc, "nk_sr_solve")
     return out, int(info[0]), float(info[1])
+
+
+def _check_perms(perms, N):
+    torch = _torch()
+    if perms.dtype != torch.int32 or perms.dim() != 2 or perms.shape[1] != N or not perms.is_contiguous() or not perms.is_cuda:
+        raise NkError("perms must be a contiguous CUDA int32 tensor [G][N]")
+
+
+def rbmsymm_expand(W_sym, b_sym, perms):
+    """nk_rbmsymm_expand: tied (W_sym [F][N], b_sym [F] or None) + group permutations [G][N] -> (W [F*G][N], b [F*G])."""
+    torch = _torch()
+    F, N = W_sym.shape
+    _check_perms(perms, N)
+    G = perms.shape[0]
+    W = torch.zeros((F * G, N), dtype=W_sym.dtype, device=W_sym.device)
+    b = torch.zeros(F * G, dtype=W_sym.dtype, device=W_sym.device)
+    rc = load().nk_rbmsymm_expand(F, G, N, _dtype_code(W_sym), _ptr(W_sym), _ptr(b_sym), _ptr(perms), _ptr(W), _ptr(b),
+                                  _stream())
+    _check(rc, "nk_rbmsymm_expand")
+    return W, b
+
+
+def rbmsymm_reduce_gradient(grad_W, grad_b, perms, n_features: int):
+    """nk_rbmsymm_reduce_gradient: expanded (grad_W [F*G][N], grad_b [F*G]) -> tied (grad_W_sym [F][N], grad_b_sym [F])."""
+    torch = _torch()
+    M, N = grad_W.shape
+    _check_perms(perms, N)
+    G = perms.shape[0]
+    if n_features * G != M:
+        raise NkError("grad_W must have n_features * n_group rows")
+    gW = torch.empty((n_features, N), dtype=grad_W.dtype, device=grad_W.device)
+    gb = torch.empty(n_features, dtype=grad_W.dtype, device=grad_W.device)
+    rc = load().nk_rbmsymm_reduce_gradient(n_features, G, N, _dtype_code(grad_W), _ptr(grad_W), _ptr(grad_b),
+                                           _ptr(perms), _ptr(gW), _ptr(gb), _stream())
+    _check(rc, "nk_rbmsymm_reduce_gradient")
+    return gW, gb
 
 
 def metropolis_sample(sigma, W, a=None, b=None, *, rule: int = NK_RULE_LOCAL, clusters=None, n_steps: int | None = None,

@@ -537,6 +537,27 @@ int nk_sr_solve(const int8_t* sigma, int64_t B, int N, int M, int dtype, const v
     return NK_OK;
 }
 
+// ---- fully symmetric RBM: tied weights <-> expanded RBM -------------------------------------------------------
+static bool bad_symm(int F, int G, int N, int dtype) {
+    return F <= 0 || G <= 0 || N <= 0 || (dtype != NK_F32 && dtype != NK_C64) || (int64_t)F * G > (1 << 24);
+}
+
+int nk_rbmsymm_expand(int n_features, int n_group, int N, int dtype, const void* W_sym, const void* b_sym,
+                      const int32_t* perms, void* W_out, void* b_out, nk_stream_t stream) {
+    if (bad_symm(n_features, n_group, N, dtype) || !W_sym || !perms || !W_out) return NK_ERR_INVALID_ARG;
+    NK_CUDA(launch_rbmsymm_expand(n_features, n_group, N, dtype, W_sym, b_sym, perms, W_out, b_out,
+                                  (cudaStream_t)stream));
+    return NK_OK;
+}
+
+int nk_rbmsymm_reduce_gradient(int n_features, int n_group, int N, int dtype, const void* grad_W, const void* grad_b,
+                               const int32_t* perms, void* grad_W_sym, void* grad_b_sym, nk_stream_t stream) {
+    if (bad_symm(n_features, n_group, N, dtype) || !grad_W || !perms || !grad_W_sym) return NK_ERR_INVALID_ARG;
+    NK_CUDA(launch_rbmsymm_reduce(n_features, n_group, N, dtype, grad_W, grad_b, perms, grad_W_sym, grad_b_sym,
+                                  (cudaStream_t)stream));
+    return NK_OK;
+}
+
 static bool bad_rule(int rule, int n_clusters) {
     return (rule != NK_RULE_LOCAL && rule != NK_RULE_EXCHANGE) || n_clusters < 0 ||
            (rule == NK_RULE_EXCHANGE && n_clusters == 0);

@@ -112,6 +112,11 @@ cudaError_t launch_cg_step(float* x, float* r, const float* p, const float* Ap, 
                            const double* pAp, cudaStream_t st);
 cudaError_t launch_cg_dir(float* p, const float* r, int64_t n, const double* rr_new, const double* rr_old,
                           cudaStream_t st);
+// rbmsymm.cu : weight tying of the fully symmetric RBM
+cudaError_t launch_rbmsymm_expand(int F, int G, int N, int dtype, const void* Wsym, const void* bsym,
+                                  const int32_t* perms, void* W, void* b, cudaStream_t st);
+cudaError_t launch_rbmsymm_reduce(int F, int G, int N, int dtype, const void* gW, const void* gb,
+                                  const int32_t* perms, void* gWsym, void* gbsym, cudaStream_t st);
 // logpsi.cu
 cudaError_t launch_logpsi(const int8_t* sigma, int64_t B, const Geometry& g, int dtype, const float* theta,
                           const void* a, void* logpsi_out, bool out_f64, void* theta_out, cudaStream_t st);
