@@ -129,7 +129,9 @@ int nk_local_energy_ex(nk_operator_t op, const int8_t* sigma, int64_t B, int N, 
  * `scratch`, runs nk_local_energy, copies eloc / logpsi / stats back and SYNCHRONISES `stream` before returning.
  * Host buffers should be pinned for the copies to be asynchronous.  scratch: dev, 256-B aligned, at least
  * nk_local_energy_host_scratch_bytes(...) bytes (inputs + outputs + workspace).  eloc_host [B], logpsi_host [B]
- * or NULL, stats_host double[4] or NULL. */
+ * or NULL, stats_host double[4] or NULL.  The host->device copies run on one internal non-blocking stream per calling
+ * thread (created on first use, with a few events) so that sigma of chunk k + 1 is copied while chunk k is computed;
+ * everything the caller observes is still ordered on `stream`. */
 size_t nk_local_energy_host_scratch_bytes(nk_operator_t op, int64_t B, int N, int M, int dtype, int64_t chunk_size);
 int nk_local_energy_host(nk_operator_t op, const int8_t* sigma_host, int64_t B, int N, int M, int dtype,
                          const void* W_host, const void* a_host, const void* b_host, int64_t chunk_size,

@@ -33,6 +33,12 @@ struct Scope {
     }
 };
 
+// nk_local_energy_host overlaps its host->device copies with the chunk loop: when this is set, chunk k of
+// nk_local_energy_ex first makes the call's stream wait on event k (sigma of that chunk has arrived).
+static thread_local const std::vector<cudaEvent_t>* tl_chunk_ready = nullptr;
+static thread_local cudaStream_t tl_copy_stream = nullptr;
+static thread_local std::vector<cudaEvent_t> tl_copy_events;
+
 static int cuda_fail(cudaError_t e) {
     tl_last_cuda = (int)e;
     return NK_ERR_CUDA;
@@ -651,6 +657,7 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
     for (int64_t s0 = 0; s0 < B; s0 += chunk) {
         const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
         const int8_t* sg = sigma + s0 * N;
+        if (tl_chunk_ready != nullptr) NK_CUDA(cudaStreamWaitEvent(st, (*tl_chunk_ready)[(size_t)(s0 / chunk)], 0));
         {
             Scope sc(PH_GEMM, st);
             NK_CUDA(run_theta(g, sg, nb, w.Wg, w.bg, w.Ws, w.A, w.theta, st));
@@ -714,13 +721,35 @@ int nk_local_energy_host(nk_operator_t h, const int8_t* sigma_host, int64_t B, i
     if (scratch_bytes < s.bytes) return NK_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t esz = dtype == NK_C64 ? 8 : 4;
-    if (B > 0) NK_CUDA(cudaMemcpyAsync(s.sigma, sigma_host, (size_t)B * N, cudaMemcpyHostToDevice, st));
-    NK_CUDA(cudaMemcpyAsync(s.W, W_host, (size_t)M * N * esz, cudaMemcpyHostToDevice, st));
-    if (a_host) NK_CUDA(cudaMemcpyAsync(s.a, a_host, (size_t)N * esz, cudaMemcpyHostToDevice, st));
-    if (b_host) NK_CUDA(cudaMemcpyAsync(s.b, b_host, (size_t)M * esz, cudaMemcpyHostToDevice, st));
+    // Copies run on an internal stream so that sigma of chunk k + 1 travels while chunk k is computed: parameters
+    // first (the packing kernels need them), then sigma chunk by chunk, one event each.
+    if (tl_copy_stream == nullptr) NK_CUDA(cudaStreamCreateWithFlags(&tl_copy_stream, cudaStreamNonBlocking));
+    const int64_t chunk = (chunk_size <= 0 || chunk_size > B) ? (B > 0 ? B : 1) : chunk_size;
+    const size_t n_chunks = B > 0 ? (size_t)((B + chunk - 1) / chunk) : 0;
+    while (tl_copy_events.size() < n_chunks + 2) {
+        cudaEvent_t ev;
+        NK_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        tl_copy_events.push_back(ev);
+    }
+    cudaStream_t cs = tl_copy_stream;
+    const cudaEvent_t ev_start = tl_copy_events[n_chunks], ev_params = tl_copy_events[n_chunks + 1];
+    NK_CUDA(cudaEventRecord(ev_start, st));                 // earlier work on the caller's stream may still use scratch
+    NK_CUDA(cudaStreamWaitEvent(cs, ev_start, 0));
+    NK_CUDA(cudaMemcpyAsync(s.W, W_host, (size_t)M * N * esz, cudaMemcpyHostToDevice, cs));
+    if (a_host) NK_CUDA(cudaMemcpyAsync(s.a, a_host, (size_t)N * esz, cudaMemcpyHostToDevice, cs));
+    if (b_host) NK_CUDA(cudaMemcpyAsync(s.b, b_host, (size_t)M * esz, cudaMemcpyHostToDevice, cs));
+    NK_CUDA(cudaEventRecord(ev_params, cs));
+    for (size_t k = 0; k < n_chunks; ++k) {
+        const int64_t s0 = (int64_t)k * chunk, nb = (B - s0 < chunk) ? (B - s0) : chunk;
+        NK_CUDA(cudaMemcpyAsync(s.sigma + s0 * N, sigma_host + s0 * N, (size_t)nb * N, cudaMemcpyHostToDevice, cs));
+        NK_CUDA(cudaEventRecord(tl_copy_events[k], cs));
+    }
+    NK_CUDA(cudaStreamWaitEvent(st, ev_params, 0));
+    tl_chunk_ready = &tl_copy_events;
     const int rc = nk_local_energy(h, s.sigma, B, N, M, dtype, s.W, a_host ? s.a : nullptr, b_host ? s.b : nullptr,
                                    chunk_size, s.eloc, logpsi_host ? s.logpsi : nullptr, stats_host ? s.stats : nullptr,
                                    s.ws, s.ws_bytes, stream);
+    tl_chunk_ready = nullptr;
     if (rc != NK_OK) return rc;
     if (B > 0) NK_CUDA(cudaMemcpyAsync(eloc_host, s.eloc, (size_t)B * esz, cudaMemcpyDeviceToHost, st));
     if (B > 0 && logpsi_host) NK_CUDA(cudaMemcpyAsync(logpsi_host, s.logpsi, (size_t)B * esz, cudaMemcpyDeviceToHost, st));
