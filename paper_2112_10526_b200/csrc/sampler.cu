@@ -128,63 +128,71 @@ __global__ void __launch_bounds__(sampler_warps<V, CPLX>() * 32, (sampler_min_bl
             a2_l *= 2.f * LOG2E;
         }
         const int cnt = (p.n_steps - t0 < 32) ? (int)(p.n_steps - t0) : 32;
+        // Transitions of the batch are visited through a ballot of the proposals that are non-trivial on the CURRENT
+        // spins (lane l tests its own transition): runs of trivial exchanges (s' = s, ratio 1, accepted) are counted
+        // and skipped in one step, and the same mask names the next row to prefetch.
         int pend_tt = -1, pend_slot = 0;              // a row copy in flight for transition pend_tt of this batch
-        for (int tt = 0; tt < cnt; ++tt) {
+        int pos = 0;
+        while (true) {
+            const uint32_t bi_l = (bits[i_l >> 5] >> (i_l & 31)) & 1u;
+            const uint32_t bj_l = (j_l >= 0) ? ((bits[j_l >> 5] >> (j_l & 31)) & 1u) : (bi_l ^ 1u);
+            const unsigned cand = __ballot_sync(0xffffffffu, lane >= pos && lane < cnt && bi_l != bj_l);
+            if (cand == 0u) {
+                n_acc += cnt - pos;
+                if (STAGED && pend_tt >= 0) wait_row(pend_slot);          // misjudged: drop the row
+                break;
+            }
+            const int tt = __ffs(cand) - 1;
+            n_acc += tt - pos;                        // the trivial exchanges in between
+            pos = tt + 1;
             const int idx = __shfl_sync(0xffffffffu, idx_l, tt);
             const int i = __shfl_sync(0xffffffffu, i_l, tt);
             const int j = __shfl_sync(0xffffffffu, j_l, tt);
             const float u = __shfl_sync(0xffffffffu, u_l, tt);
             const float a2 = __shfl_sync(0xffffffffu, a2_l, tt);
-            const uint32_t bi = (bits[i >> 5] >> (i & 31)) & 1u;
-            const uint32_t bj = (j >= 0) ? ((bits[j >> 5] >> (j & 31)) & 1u) : (bi ^ 1u);
+            const uint32_t bi = __shfl_sync(0xffffffffu, bi_l, tt);
             int slot = 0;
-            if constexpr (!STAGED) {
-                if (bi == bj) { ++n_acc; continue; }  // exchange of equal spins: s' = s, ratio 1
-            } else if (pend_tt == tt) {                      // the prefetched row is this transition's
+            if constexpr (STAGED) {
+                if (pend_tt == tt) slot = pend_slot;  // the prefetched row is this transition's
+                else {
+                    if (pend_tt >= 0) wait_row(pend_slot);                // misjudged: drop the row
+                    issue_row(0, idx);                // first of a batch, or misjudged: fetch now
+                }
                 pend_tt = -1;
-                if (bi == bj) { wait_row(pend_slot); ++n_acc; continue; }   // turned trivial meanwhile: drop it
-                slot = pend_slot;
-            } else {
-                if (bi == bj) { ++n_acc; continue; }  // exchange of equal spins: s' = s, ratio 1
-                if (pend_tt >= 0) { wait_row(pend_slot); pend_tt = -1; }    // misjudged: drop the later row
-                issue_row(0, idx);                    // first of a batch, or misjudged as trivial: fetch now
-            }
-            if constexpr (STAGED) {   // start the copy of the next proposal that is non-trivial on the current spins
-                const uint32_t bi_l = (bits[i_l >> 5] >> (i_l & 31)) & 1u;
-                const uint32_t bj_l = (j_l >= 0) ? ((bits[j_l >> 5] >> (j_l & 31)) & 1u) : (bi_l ^ 1u);
-                const unsigned cand = __ballot_sync(0xffffffffu, lane > tt && lane < cnt && bi_l != bj_l);
-                if (cand) {
-                    pend_tt = __ffs(cand) - 1;
+                const unsigned next = cand & (cand - 1u);                 // next non-trivial proposal on the current spins
+                if (next) {
+                    pend_tt = __ffs(next) - 1;
                     pend_slot = slot ^ 1;
                     issue_row(pend_slot, __shfl_sync(0xffffffffu, idx_l, pend_tt));
                 }
+                wait_row(slot);
             }
-            if constexpr (STAGED) wait_row(slot);
             const float s = bi ? 1.f : -1.f;          // s = -sigma_i
             const float* drow = STAGED ? rowbuf + (size_t)slot * p.M_eff : p.Dtab + (size_t)idx * p.M_eff;
             bool accept;
             if constexpr (!CPLX) {
                 float praw, acc;
                 st.partial_raw(drow, lane, s, praw, acc);
-                float r = praw * st.qinv;
-                r = warp_prod_f(r);
-                acc = warp_sum_f(acc);
-                const float ratio = r * ex2_approx(fmaf(0.5f, acc, s * a2));
-                accept = __shfl_sync(0xffffffffu, (int)(u < ratio * ratio), 0) != 0;
+                // this lane's share with its exponent folded in: one butterfly instead of two; every lane ends with
+                // the same bits (each level multiplies the same two operands in both lanes of a pair)
+                const float z = warp_prod_f((praw * st.qinv) * ex2_approx(0.5f * acc));
+                const float ratio = z * ex2_approx(s * a2);
+                accept = u < ratio * ratio;
                 if (accept) st.commit(drow, lane, s, praw);
             } else {
                 float pr, pi, acc;
                 st.partial_raw(drow, lane, p.M_pad, s, pr, pi, acc);
                 float cr = pr, ci = pi;
                 cmul_f(cr, ci, st.qr, st.qi);
+                const float m = ex2_approx(0.5f * acc);   // exponent folded into the lane's factor
+                cr *= m; ci *= m;
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) {
                     const float orr = __shfl_xor_sync(0xffffffffu, cr, o), oi = __shfl_xor_sync(0xffffffffu, ci, o);
                     cmul_f(cr, ci, orr, oi);
-                    acc += __shfl_xor_sync(0xffffffffu, acc, o);
                 }
-                const float mag2 = fmaf(cr, cr, ci * ci) * ex2_approx(fmaf(2.f * s, a2, acc));
-                accept = __shfl_sync(0xffffffffu, (int)(u < mag2), 0) != 0;
+                const float mag2 = fmaf(cr, cr, ci * ci) * ex2_approx(2.f * s * a2);
+                accept = __shfl_sync(0xffffffffu, (int)(u < mag2), 0) != 0;   // complex products differ in rounding per lane
                 if (accept) st.commit(drow, lane, p.M_pad, s, pr, pi);
             }
             if (accept) {
