@@ -254,3 +254,25 @@ def test_errors_are_loud(nk):
     rc = lib.nk_local_energy(op.handle, dev(p.sigma).data_ptr(), 4, 6, 4, 0, dev(p.W).data_ptr(), None, None, 0,
                              out.data_ptr(), None, None, ws.data_ptr() + 1, 1023, None)
     assert rc == -3                                                      # misaligned / short workspace
+
+
+@pytest.mark.parametrize("case", [
+    dict(kind=0, lattice="chain", L=3000, M=128, B=6),                       # N = 3000: 94 spin words, 3000 table rows
+    dict(kind=1, lattice="chain", L=2100, M=100, B=5, h=0.9),                # long Ising chain, N + 1 = 2101 slots
+    dict(kind=0, lattice="chain", L=16, M=2048, B=40),                       # widest real RBM (V = 16) on a tiny lattice
+    dict(kind=0, lattice="square", L=4, M=1024, B=40, complex_params=True),  # widest complex RBM (V = 8)
+])
+def test_maximum_sizes(nk, case):
+    """The limits of this version (include/nkb200.h): M = 2048 real, M = 1024 complex, and N well beyond the 1024 of
+    config 5 (several shared-memory words of spins per lane, thousands of table rows), both forms of the kernel."""
+    case = dict(case)
+    p = inp.make_problem(case.pop("kind"), case.pop("lattice"), case.pop("L"), case.pop("M"), case.pop("B"),
+                         seed=44, scale=0.02, **case)
+    e_ref, lp_ref = run_oracle(p)
+    e, lp, _ = run_gpu(nk, p)
+    assert_eloc(e, e_ref)
+    assert_logpsi(lp, lp_ref)
+    op = nk.Operator.from_problem(p)
+    e2, _, _ = nk.local_energy(op, dev(p.sigma), dev(p.W), dev(p.a), dev(p.b), flags=nk.NK_FORM_PRODUCT)
+    assert_eloc(e2.cpu().numpy(), e_ref)
+    op.close()

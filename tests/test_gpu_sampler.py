@@ -147,3 +147,16 @@ def test_sampled_energy_matches_exact_expectation(nk):
     mean = stats[0].item()
     assert abs(mean - exact) < 5 * np.sqrt(var / p.n_samples), (mean, exact)
     op.close()
+
+
+def test_sampler_long_chain_and_widest_rbm(nk):
+    """N = 3000 (94 words of spin bits per chain in shared memory) with both rules; M = 2048 on a small lattice (8 KB
+    rows: the staged-row path) with an odd number of transitions."""
+    p = inp.make_problem(inp.KIND_HEISENBERG, "chain", 3000, 128, 20, seed=6, scale=0.02)
+    for r in (nk.NK_RULE_LOCAL, nk.NK_RULE_EXCHANGE):
+        got, gacc, ref, racc, margin = run_both(nk, p, r, 70)
+        assert_chains(p, r, got, gacc, ref, racc, margin, min_clear=0.7)
+    p = inp.make_problem(inp.KIND_HEISENBERG, "chain", 16, 2048, 30, seed=7, scale=0.01)
+    for r in (nk.NK_RULE_LOCAL, nk.NK_RULE_EXCHANGE):
+        got, gacc, ref, racc, margin = run_both(nk, p, r, 77)
+        assert_chains(p, r, got, gacc, ref, racc, margin, min_clear=0.7)
