@@ -179,6 +179,12 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
     qout = (torch.empty_like(ga), torch.empty_like(gb), torch.empty_like(gW))
     ms_qgt = _time_ms(torch, lambda: nk.qgt_matvec(chains, W, b, ga, gb, gW, diag_shift=0.01,
                                                    chunk_size=p.chunk_size, ws=qws, out=qout), 3)
+    # one conjugate-gradient iteration of the SR solve (theta and the spin conversions are cached across iterations)
+    sws = torch.empty(lib.nk_sr_solve_workspace_bytes(B, N, M, dt_code, p.chunk_size), dtype=torch.uint8,
+                      device=sigma.device)
+    n_cg = 8
+    ms_sr = _time_ms(torch, lambda: nk.sr_solve(chains, W, b, ga, gb, gW, diag_shift=0.01, tol=0.0, max_iter=n_cg,
+                                                chunk_size=p.chunk_size, ws=sws), 2)
     planes = 2 if p.complex_params else 1
     # product-form variant of the same step (nk_local_energy_ex, NK_FORM_PRODUCT), fused kernel timed by the library
     pplan = nk.LocalEnergyPlan(op, B, N, M, dt_code, p.chunk_size, device=sigma.device, flags=nk.NK_FORM_PRODUCT)
@@ -204,6 +210,8 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
         "qgt_matvec": {"ms": ms_qgt, "n_parameters": N + M + M * N,
                        "algorithmic_tflops": 3 * 2.0 * planes * B * M * N / (ms_qgt * 1e-3) / 1e12,
                        "what": "(G + 0.01) v on the fly, Eq. (75): theta, V_W sigma and J^dagger dw contractions"},
+        "sr_solve": {"cg_iterations": n_cg, "ms": ms_sr, "ms_per_cg_iteration": ms_sr / n_cg,
+                     "what": "nk_sr_solve with tol = 0: setup (theta of the batch, spin conversions) + 8 CG iterations"},
         "vmc_iteration": {"ms": ms_sweep + ms_eloc + ms_grad, "ms_local_energy_on_sampled_chains": ms_eloc,
                           "what": "one sweep + local energies + energy gradient, same batch, device-resident"},
     }

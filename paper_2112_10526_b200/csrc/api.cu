@@ -400,10 +400,21 @@ size_t nk_qgt_matvec_workspace_bytes(int64_t B, int N, int M, int dtype, int64_t
     return carve_qgt(nullptr, g, B, eff_chunk(B, chunk_size), dtype).bytes;
 }
 
-int nk_qgt_matvec(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* b,
-                  const void* v_a, const void* v_b, const void* v_W, double diag_shift, int64_t chunk_size,
-                  void* out_a, void* out_b, void* out_W, void* workspace, size_t workspace_bytes,
-                  nk_stream_t stream) {
+// theta, the bf16 spins and their transposes for the WHOLE batch, kept across the matvecs of one nk_sr_solve (the
+// parameters do not change during the solve): a matvec then costs one contraction less per pass and no conversions
+namespace {
+struct QgtCache {
+    float* theta_all;        // [B][M_eff]
+    uint16_t* A_all;         // [B][K_pad] bf16
+    uint16_t* sigT_all;      // [n_chunks][N][ld] bf16
+    size_t sigT_stride;      // N * ld
+};
+}  // namespace
+
+static int qgt_matvec_impl(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* b,
+                           const void* v_a, const void* v_b, const void* v_W, double diag_shift, int64_t chunk_size,
+                           void* out_a, void* out_b, void* out_W, void* workspace, size_t workspace_bytes,
+                           nk_stream_t stream, const QgtCache* cache) {
     if (bad_dims(B, N, M, dtype) || B == 0 || chunk_size < 0 || !sigma || !W || !v_W || !out_W ||
         (diag_shift < 0.0))
         return NK_ERR_INVALID_ARG;
@@ -415,18 +426,26 @@ int nk_qgt_matvec(const int8_t* sigma, int64_t B, int N, int M, int dtype, const
     const QgtWs w = carve_qgt(workspace, g, B, chunk, dtype);
     cudaStream_t st = (cudaStream_t)stream;
     const size_t esz = dtype == NK_C64 ? 8 : 4;
-    // operands of the two contractions: (W, b) -> theta and (V_W, v_b) -> Y
-    NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.g.Wg, w.g.bg, st));
-    NK_CUDA(launch_split_w(w.g.Wg, g.M_eff, N, g.K_pad, w.g.Ws, w.g.absmax, st));
+    // operands of the two contractions: (W, b) -> theta (not needed when theta is cached) and (V_W, v_b) -> Y
+    if (cache == nullptr) {
+        NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.g.Wg, w.g.bg, st));
+        NK_CUDA(launch_split_w(w.g.Wg, g.M_eff, N, g.K_pad, w.g.Ws, w.g.absmax, st));
+    }
     NK_CUDA(launch_pack_gemm_only(g, dtype, v_W, v_b, w.Vg, w.vbg, st));
     NK_CUDA(launch_split_w(w.Vg, g.M_eff, N, g.K_pad, w.Vs, w.g.absmax, st));
     // step 1 of Eq. (75): w_s = (J v)_s for every sample
     for (int64_t s0 = 0; s0 < B; s0 += chunk) {
         const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
         const int8_t* sg = sigma + s0 * N;
-        NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.g.Ws, w.g.A, w.g.bg, w.g.theta, st));
-        NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.Vs, w.g.A, w.vbg, w.Y, st));
-        NK_CUDA(launch_qgt_w(g, dtype, sg, nb, w.g.theta, w.Y, v_a, (uint8_t*)w.wbuf + s0 * esz, st));
+        const float* th = w.g.theta;
+        if (cache == nullptr) {
+            NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.g.Ws, w.g.A, w.g.bg, w.g.theta, st));
+            NK_CUDA(launch_theta_tc_pre(w.g.A, nb, g.M_eff, g.K_pad, w.Vs, w.vbg, w.Y, st));
+        } else {
+            th = cache->theta_all + (size_t)s0 * g.M_eff;
+            NK_CUDA(launch_theta_tc_pre(cache->A_all + (size_t)s0 * g.K_pad, nb, g.M_eff, g.K_pad, w.Vs, w.vbg, w.Y, st));
+        }
+        NK_CUDA(launch_qgt_w(g, dtype, sg, nb, th, w.Y, v_a, (uint8_t*)w.wbuf + s0 * esz, st));
     }
     // step 2: <w> (the 1/N_s and the subtraction happen inside the force contraction, as for E_loc)
     NK_CUDA(launch_stats(w.wbuf, B, dtype, w.wstats, st));
@@ -435,9 +454,15 @@ int nk_qgt_matvec(const int8_t* sigma, int64_t B, int N, int M, int dtype, const
     for (int64_t s0 = 0; s0 < B; s0 += chunk) {
         const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
         const int8_t* sg = sigma + s0 * N;
-        NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.g.Ws, w.g.A, w.g.bg, w.g.theta, st));
-        NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B, (const uint8_t*)w.wbuf + s0 * esz, w.wstats, w.g, first, 1.f,
-                                      st));
+        if (cache == nullptr) {
+            NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.g.Ws, w.g.A, w.g.bg, w.g.theta, st));
+            NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B, (const uint8_t*)w.wbuf + s0 * esz, w.wstats, w.g, first,
+                                          1.f, st));
+        } else {
+            NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B, (const uint8_t*)w.wbuf + s0 * esz, w.wstats, w.g, first,
+                                          1.f, st, cache->theta_all + (size_t)s0 * g.M_eff,
+                                          cache->sigT_all + (size_t)(s0 / chunk) * cache->sigT_stride));
+        }
         first = 0;
     }
     NK_CUDA(launch_gradient_finalize(g, dtype, w.g, out_a, out_b, out_W, st));
@@ -449,6 +474,14 @@ int nk_qgt_matvec(const int8_t* sigma, int64_t B, int N, int M, int dtype, const
     return NK_OK;
 }
 
+int nk_qgt_matvec(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* b,
+                  const void* v_a, const void* v_b, const void* v_W, double diag_shift, int64_t chunk_size,
+                  void* out_a, void* out_b, void* out_W, void* workspace, size_t workspace_bytes,
+                  nk_stream_t stream) {
+    return qgt_matvec_impl(sigma, B, N, M, dtype, W, b, v_a, v_b, v_W, diag_shift, chunk_size, out_a, out_b, out_W,
+                           workspace, workspace_bytes, stream, nullptr);
+}
+
 // ---- stochastic reconfiguration: (G + eps) delta = f by conjugate gradients -----------------------------------
 namespace {
 struct SrWs {
@@ -457,6 +490,7 @@ struct SrWs {
     void* qgt;
     size_t qgt_bytes, bytes;
     int64_t n;
+    QgtCache cache;
 };
 SrWs carve_sr(void* ws, int64_t B, int N, int M, int dtype, int64_t chunk_size) {
     const int64_t e = dtype == NK_C64 ? 2 : 1;
@@ -468,6 +502,14 @@ SrWs carve_sr(void* ws, int64_t B, int N, int M, int dtype, int64_t chunk_size) 
     w.scal = c.take<double>(8);
     w.qgt_bytes = nk_qgt_matvec_workspace_bytes(B, N, M, dtype, chunk_size);
     w.qgt = c.take<uint8_t>(w.qgt_bytes);
+    const Geometry g = make_geometry(nullptr, N, M, dtype);
+    const int64_t chunk = (chunk_size <= 0 || chunk_size > B) ? (B > 0 ? B : 1) : chunk_size;
+    const int64_t n_chunks = B > 0 ? (B + chunk - 1) / chunk : 1;
+    const size_t ld = (size_t)((chunk + 63) / 64 * 64);
+    w.cache.theta_all = c.take<float>((size_t)B * g.M_eff);
+    w.cache.A_all = c.take<uint16_t>((size_t)B * g.K_pad);
+    w.cache.sigT_stride = (size_t)N * ld;
+    w.cache.sigT_all = c.take<uint16_t>((size_t)n_chunks * w.cache.sigT_stride);
     w.bytes = c.off;
     return w;
 }
@@ -506,6 +548,20 @@ int nk_sr_solve(const int8_t* sigma, int64_t B, int N, int M, int dtype, const v
         NK_CUDA(cudaMemcpyAsync(blk(w.r, k), fsrc[k], fbytes[k], cudaMemcpyDeviceToDevice, st));
         NK_CUDA(cudaMemcpyAsync(blk(w.p, k), fsrc[k], fbytes[k], cudaMemcpyDeviceToDevice, st));
     }
+    {   // theta, bf16 spins and their transposes of the whole batch, once per solve
+        const QgtWs q = carve_qgt(w.qgt, g, B, eff_chunk(B, chunk_size), dtype);
+        const int64_t chunk = eff_chunk(B, chunk_size);
+        NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, q.g.Wg, q.g.bg, st));
+        NK_CUDA(launch_split_w(q.g.Wg, g.M_eff, N, g.K_pad, q.g.Ws, q.g.absmax, st));
+        NK_CUDA(launch_sigma_bf16(sigma, B, N, g.K_pad, w.cache.A_all, st));
+        for (int64_t s0 = 0; s0 < B; s0 += chunk) {
+            const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
+            NK_CUDA(launch_theta_tc_pre(w.cache.A_all + (size_t)s0 * g.K_pad, nb, g.M_eff, g.K_pad, q.g.Ws, q.g.bg,
+                                        w.cache.theta_all + (size_t)s0 * g.M_eff, st));
+            NK_CUDA(launch_sigma_T(sigma + s0 * N, nb, N, q.g.ld,
+                                   w.cache.sigT_all + (size_t)(s0 / chunk) * w.cache.sigT_stride, st));
+        }
+    }
     NK_CUDA(launch_cg_dot(w.r, w.r, w.n, w.part, w.scal + 0, st));
     NK_CUDA(cudaMemcpyAsync(w.scal + 3, w.scal + 0, sizeof(double), cudaMemcpyDeviceToDevice, st));
     double h[4] = {0, 0, 0, 0};
@@ -517,8 +573,9 @@ int nk_sr_solve(const int8_t* sigma, int64_t B, int N, int M, int dtype, const v
     const int check_every = 4;           // the residual is read back (one synchronisation) every few iterations
     while (it < max_iter && ff > 0.0 && rr > tol * tol * ff) {
         const int cur = it & 1, nxt = cur ^ 1;
-        const int rc = nk_qgt_matvec(sigma, B, N, M, dtype, W, b, blk(w.p, 0), blk(w.p, 1), blk(w.p, 2), diag_shift,
-                                     chunk_size, blk(w.Ap, 0), blk(w.Ap, 1), blk(w.Ap, 2), w.qgt, w.qgt_bytes, stream);
+        const int rc = qgt_matvec_impl(sigma, B, N, M, dtype, W, b, blk(w.p, 0), blk(w.p, 1), blk(w.p, 2), diag_shift,
+                                       chunk_size, blk(w.Ap, 0), blk(w.Ap, 1), blk(w.Ap, 2), w.qgt, w.qgt_bytes, stream,
+                                       &w.cache);
         if (rc != NK_OK) return rc;
         NK_CUDA(launch_cg_dot(w.p, w.Ap, w.n, w.part, w.scal + 2, st));
         NK_CUDA(launch_cg_step(w.x, w.r, w.p, w.Ap, w.n, w.scal + cur, w.scal + 2, st));

@@ -28,7 +28,7 @@ __device__ __forceinline__ void sample_weight(const float* __restrict__ eloc, co
 
 // theta[s][.] -> v[s][.] in place (complex: plane 0 = Re v, plane 1 = Im v), and max |v| as float bits
 template <bool CPLX>
-__global__ void grad_tv_kernel(float* __restrict__ theta, int64_t nb, int M, int M_pad, int M_eff,
+__global__ void grad_tv_kernel(const float* theta_in, float* theta, int64_t nb, int M, int M_pad, int M_eff,
                                const float* __restrict__ eloc, const double* __restrict__ stats, double inv_B,
                                float real_scale, unsigned* __restrict__ absmax) {
     unsigned m = 0;
@@ -36,16 +36,17 @@ __global__ void grad_tv_kernel(float* __restrict__ theta, int64_t nb, int M, int
     float wr, wi;
     sample_weight(eloc, stats, s, inv_B, CPLX, wr, wi);
     float* row = theta + s * M_eff;
+    const float* rin = theta_in + s * M_eff;          // may alias row (in place) or be a cached theta
     for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < M_pad; j += gridDim.x * blockDim.x) {
         if (!CPLX) {
-            const float v = (j < M) ? real_scale * tanhf(row[j]) * wr : 0.f;
+            const float v = (j < M) ? real_scale * tanhf(rin[j]) * wr : 0.f;
             row[j] = v;
             m = max(m, __float_as_uint(fabsf(v)));
         } else {
             float vr = 0.f, vi = 0.f;
             if (j < M) {
                 // tanh(x + i y) = [sign(x)(1 - e^2) + i 2 e sin 2y] / (1 + e^2 + 2 e cos 2y),  e = exp(-2|x|)
-                const float x = row[j], y = row[M_pad + j];
+                const float x = rin[j], y = rin[M_pad + j];
                 const float e = expf(-2.f * fabsf(x));
                 float sn, cs;
                 sincosf(2.f * y, &sn, &cs);
@@ -208,7 +209,7 @@ int grad_slab() { return GRAD_SLAB; }
 
 cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, int64_t B_total,
                                   const void* eloc, const double* stats, const GradWs& w, int first_chunk,
-                                  float real_scale, cudaStream_t st) {
+                                  float real_scale, cudaStream_t st, const float* theta_in, const void* sigT_ready) {
     if (nb <= 0) return cudaSuccess;
     const bool cplx = dtype == NK_C64;
     const double inv_B = 1.0 / (double)B_total;
@@ -217,10 +218,10 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
     if (e != cudaSuccess) return e;
     dim3 gtv((g.M_pad + 255) / 256, (unsigned)(nb < 1184 ? nb : 1184));
     if (cplx)
-        grad_tv_kernel<true><<<gtv, 256, 0, st>>>(w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
+        grad_tv_kernel<true><<<gtv, 256, 0, st>>>(theta_in ? theta_in : w.theta, w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
                                                   real_scale, w.absmax);
     else
-        grad_tv_kernel<false><<<gtv, 256, 0, st>>>(w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
+        grad_tv_kernel<false><<<gtv, 256, 0, st>>>(theta_in ? theta_in : w.theta, w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
                                                    real_scale, w.absmax);
     const int n_slabs = (int)((nb + GRAD_SLAB - 1) / GRAD_SLAB);
     grad_colsum_partial_kernel<<<dim3((g.M_eff + 127) / 128, n_slabs), 128, 0, st>>>(w.theta, nb, g.M_eff, w.part);
@@ -230,12 +231,23 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
     grad_slab_reduce_kernel<<<(2 * g.N + 127) / 128, 128, 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk);
     grad_split_T_kernel<<<dim3(k_len / 32, g.M_eff / 32), dim3(32, 8), 0, st>>>(
         w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (__nv_bfloat16*)w.TwT);
-    grad_sigma_T_kernel<<<dim3(k_len / 32, (g.N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, g.N, w.ld,
-                                                                                 (__nv_bfloat16*)w.sigT);
-    count_launch(7);
+    if (sigT_ready == nullptr)
+        grad_sigma_T_kernel<<<dim3(k_len / 32, (g.N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, g.N, w.ld,
+                                                                                     (__nv_bfloat16*)w.sigT);
+    count_launch(sigT_ready ? 6 : 7);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    return launch_tc_gemm_pieces(w.sigT, g.N, w.TwT, g.M_eff, w.ld, k_len, w.Gacc, first_chunk ? 0 : 1, st);
+    return launch_tc_gemm_pieces(sigT_ready ? sigT_ready : (const void*)w.sigT, g.N, w.TwT, g.M_eff, w.ld, k_len, w.Gacc,
+                                 first_chunk ? 0 : 1, st);
+}
+
+// sigT[k][s] = (bf16) sigma[s][k] for one chunk (what launch_gradient_chunk builds itself unless given sigT_ready)
+cudaError_t launch_sigma_T(const int8_t* sigma, int64_t nb, int N, int ld, void* sigT, cudaStream_t st) {
+    const int k_len = (int)((nb + 63) / 64 * 64);
+    grad_sigma_T_kernel<<<dim3(k_len / 32, (N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, N, ld,
+                                                                               (__nv_bfloat16*)sigT);
+    count_launch();
+    return cudaGetLastError();
 }
 
 cudaError_t launch_gradient_finalize(const Geometry& g, int dtype, const GradWs& w, void* grad_a, void* grad_b,

@@ -84,6 +84,9 @@ cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* W
                            cudaStream_t st);
 cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, int K_pad, const void* Ws_bf16,
                             void* A_bf16, const float* bg, float* theta, cudaStream_t st);
+cudaError_t launch_sigma_bf16(const int8_t* sigma, int64_t B, int N, int K_pad, void* A_bf16, cudaStream_t st);
+cudaError_t launch_theta_tc_pre(const void* A_bf16, int64_t B, int M_eff, int K_pad, const void* Ws_bf16,
+                                const float* bg, float* theta, cudaStream_t st);   // launch_theta_tc without the spin conversion
 cudaError_t launch_tc_gemm_pieces(const void* A_bf16, int64_t rows, const void* P_bf16, int cols, int ld, int k_len,
                                   float* out, int accumulate, cudaStream_t st);
 // gradient.cu : force vector / energy gradient of the RBM
@@ -98,7 +101,11 @@ struct GradWs {
 int grad_slab();
 cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, int64_t B_total,
                                   const void* eloc, const double* stats, const GradWs& w, int first_chunk,
-                                  float real_scale, cudaStream_t st);   // real_scale: 2 (gradient 2 Re f~) | 1 (QGT)
+                                  float real_scale, cudaStream_t st, const float* theta_in = nullptr,
+                                  const void* sigT_ready = nullptr);
+// real_scale: 2 (gradient 2 Re f~) | 1 (QGT).  theta_in: read theta from there (w.theta receives v) instead of in
+// place; sigT_ready: the chunk's transposed bf16 spins prepared earlier by launch_sigma_T (w.sigT is not touched).
+cudaError_t launch_sigma_T(const int8_t* sigma, int64_t nb, int N, int ld, void* sigT, cudaStream_t st);
 cudaError_t launch_gradient_finalize(const Geometry& g, int dtype, const GradWs& w, void* grad_a, void* grad_b,
                                      void* grad_W, cudaStream_t st);
 // qgt.cu : pieces of the QGT-vector product

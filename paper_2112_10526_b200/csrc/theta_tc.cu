@@ -301,6 +301,30 @@ cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, in
     return cudaGetLastError();
 }
 
+cudaError_t launch_sigma_bf16(const int8_t* sigma, int64_t B, int N, int K_pad, void* A, cudaStream_t st) {
+    if (B <= 0) return cudaSuccess;
+    const int64_t total = B * K_pad;
+    int64_t blocks = (total + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    sigma_bf16_kernel<<<(unsigned)blocks, 256, 0, st>>>(sigma, B, N, K_pad, (__nv_bfloat16*)A);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_theta_tc_pre(const void* A, int64_t B, int M_eff, int K_pad, const void* Ws, const float* bg,
+                                float* theta, cudaStream_t st) {
+    if (B <= 0) return cudaSuccess;
+    cudaError_t e = theta_tc_init();
+    if (e != cudaSuccess) return e;
+    CUtensorMap map_a, map_w;
+    if (!encode_2d(&map_a, A, (uint64_t)B, (uint64_t)K_pad)) return cudaErrorInvalidValue;
+    if (!encode_2d(&map_w, Ws, (uint64_t)3 * M_eff, (uint64_t)K_pad)) return cudaErrorInvalidValue;
+    dim3 grid(M_eff / tc::BN, (unsigned)((B + tc::BM - 1) / tc::BM));
+    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_w, B, M_eff, K_pad, bg, theta, 0);
+    count_launch();
+    return cudaGetLastError();
+}
+
 // Generic entry used by the gradient: out[r][c] (+)= sum_k A[r][k] * (P0 + P1 + P2)[c][k], A bf16 [rows][ld] and
 // P bf16 [3][cols][ld] both k-contiguous, k < k_len (a multiple of 64), cols a multiple of 128.
 cudaError_t launch_tc_gemm_pieces(const void* A, int64_t rows, const void* P, int cols, int ld, int k_len, float* out,
