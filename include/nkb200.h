@@ -185,7 +185,8 @@ int nk_sr_solve(const int8_t* sigma, int64_t B, int N, int M, int dtype, const v
  * f_g^(i) = sum_r W^(i)_r s_{g r} + b^(i).  This is an RBM with M = n_features * n_group tied hidden units; hidden
  * unit (i, g) is row i * n_group + g:   W[(i,g)][g r] = W_sym[i][r],  b[(i,g)] = b_sym[i].
  *   perms  dev int32 [n_group][N], perms[g][r] = the site g r; every row must be a permutation of 0..N-1 (caller's
- *          responsibility: an out-of-range entry is an out-of-bounds write)
+ *          responsibility; the table lives on the device, so the calls cannot check it without synchronising:
+ *          out-of-range entries are skipped, a repeated image leaves a column of the expansion unwritten)
  * nk_rbmsymm_expand writes the expanded (W [M][N], b [M] or NULL) to pass to any other call of this library (no
  * visible bias: a = NULL); nk_rbmsymm_reduce_gradient maps a gradient / force / QGT-vector block of the expanded
  * parameters to the tied ones by summing over orbits (the tying is linear):

@@ -17,6 +17,7 @@ __global__ void rbmsymm_expand_kernel(const float* __restrict__ Wsym, const floa
     const int row = blockIdx.x, i = row / G, g = row - i * G;
     for (int r = threadIdx.x; r < N; r += blockDim.x) {
         const int k = perms[(size_t)g * N + r];
+        if (k < 0 || k >= N) continue;                 // malformed table: stay inside the buffers
 #pragma unroll
         for (int e = 0; e < E; ++e) W[((size_t)row * N + k) * E + e] = Wsym[((size_t)i * N + r) * E + e];
     }
@@ -35,6 +36,7 @@ __global__ void rbmsymm_reduce_kernel(const float* __restrict__ gW, const float*
         for (int e = 0; e < E; ++e) acc[e] = 0.0;
         for (int g = 0; g < G; ++g) {
             const int k = perms[(size_t)g * N + r];
+            if (k < 0 || k >= N) continue;             // malformed table: stay inside the buffers
 #pragma unroll
             for (int e = 0; e < E; ++e) acc[e] += (double)gW[(((size_t)i * G + g) * N + k) * E + e];
         }
