@@ -43,7 +43,7 @@ typedef void* nk_stream_t;                      /* a cudaStream_t */
 enum nk_status {
     NK_OK = 0,
     NK_ERR_INVALID_ARG = -1,   /* NULL / out-of-range / inconsistent argument */
-    NK_ERR_BAD_SPIN = -2,      /* reserved: sigma value not in {+1,-1} (validation is opt-in, not yet wired) */
+    NK_ERR_BAD_SPIN = -2,      /* a sigma value is not +1 / -1; only reported under NK_CHECK_SPINS (nk_local_energy_ex) */
     NK_ERR_WORKSPACE = -3,     /* workspace NULL, misaligned (256 B) or smaller than the *_workspace_bytes query */
     NK_ERR_UNSUPPORTED = -4,   /* sizes beyond the limits above */
     NK_ERR_CUDA = -5           /* a CUDA runtime call failed; see nk_last_cuda_error() */
@@ -54,7 +54,9 @@ enum nk_rule { NK_RULE_LOCAL = 0, NK_RULE_EXCHANGE = 1 };
 enum nk_flags {
     NK_FLAG_MARSHALL = 1u,     /* nk_operator_create: off-diagonal Heisenberg element -2J (default +2J, Eq. (50)) */
     NK_OUT_F64 = 2u,           /* nk_rbm_logpsi: logpsi_out is double / (re,im) double instead of float */
-    NK_FORM_PRODUCT = 4u       /* nk_local_energy_ex: product-form amplitude ratios (see there) */
+    NK_FORM_PRODUCT = 4u,      /* nk_local_energy_ex: product-form amplitude ratios (see there) */
+    NK_CHECK_SPINS = 8u        /* nk_local_energy_ex: validate sigma in {+1,-1} first (one extra pass over sigma and one
+                                  stream synchronisation); NK_ERR_BAD_SPIN before any other launch if it is not */
 };
 
 /* Static, never-NULL description of a status code. */

@@ -691,7 +691,7 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
                        void* logpsi_out, double* stats_out, void* workspace, size_t workspace_bytes,
                        nk_stream_t stream) {
     if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0 || !W || (B > 0 && (!sigma || !eloc_out)) ||
-        (flags & ~NK_FORM_PRODUCT))
+        (flags & ~(NK_FORM_PRODUCT | NK_CHECK_SPINS)))
         return NK_ERR_INVALID_ARG;
     const bool product = (flags & NK_FORM_PRODUCT) != 0;
     const Operator* op = (const Operator*)h;
@@ -703,6 +703,13 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
         return NK_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     const ElocWs w = carve_eloc(workspace, g, chunk);
+    if ((flags & NK_CHECK_SPINS) && B > 0) {           // opt-in validation: one pass over sigma and one synchronisation
+        int bad = 0;
+        NK_CUDA(launch_check_spins(sigma, B * N, (int*)w.absmax, st));
+        NK_CUDA(cudaMemcpyAsync(&bad, w.absmax, sizeof(int), cudaMemcpyDeviceToHost, st));
+        NK_CUDA(cudaStreamSynchronize(st));
+        if (bad) return NK_ERR_BAD_SPIN;
+    }
     NK_CUDA(fused_eloc_init());
     {
         Scope sc(PH_PACK, st);

@@ -136,6 +136,7 @@ cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, 
                               bool product_form, cudaStream_t st);
 cudaError_t fused_eloc_init();   // one-time cudaFuncSetAttribute calls
 // stats.cu
+cudaError_t launch_check_spins(const int8_t* sigma, int64_t n, int* flag, cudaStream_t st);
 cudaError_t launch_stats(const void* eloc, int64_t B, int dtype, double* stats_out, cudaStream_t st);
 
 void count_launch(int n = 1);

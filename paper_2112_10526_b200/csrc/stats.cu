@@ -51,4 +51,24 @@ cudaError_t launch_stats(const void* eloc, int64_t B, int dtype, double* stats_o
     return cudaGetLastError();
 }
 
+// NK_CHECK_SPINS: *flag |= 1 if any entry of sigma is not +1 or -1 (the spin encoding of PAPER.md L178)
+__global__ void check_spins_kernel(const int8_t* __restrict__ sigma, int64_t n, int* __restrict__ flag) {
+    int bad = 0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int v = sigma[i];
+        bad |= (v != 1 && v != -1);
+    }
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(flag, 1);
+}
+
+cudaError_t launch_check_spins(const int8_t* sigma, int64_t n, int* flag, cudaStream_t st) {
+    cudaError_t e = cudaMemsetAsync(flag, 0, sizeof(int), st);
+    if (e != cudaSuccess || n <= 0) return e;
+    int64_t blocks = (n + 255) / 256;
+    if (blocks > 2368) blocks = 2368;
+    check_spins_kernel<<<(unsigned)blocks, 256, 0, st>>>(sigma, n, flag);
+    count_launch();
+    return cudaGetLastError();
+}
+
 }  // namespace nk

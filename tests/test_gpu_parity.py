@@ -254,6 +254,12 @@ def test_errors_are_loud(nk):
     rc = lib.nk_local_energy(op.handle, dev(p.sigma).data_ptr(), 4, 6, 4, 0, dev(p.W).data_ptr(), None, None, 0,
                              out.data_ptr(), None, None, ws.data_ptr() + 1, 1023, None)
     assert rc == -3                                                      # misaligned / short workspace
+    bad = p.sigma.copy(); bad[2, 3] = 0                                  # opt-in spin validation
+    with pytest.raises(nk.NkError, match="BAD_SPIN"):
+        nk.local_energy(op, dev(bad), dev(p.W), dev(p.a), dev(p.b), flags=nk.NK_CHECK_SPINS)
+    e_ok, _, _ = nk.local_energy(op, dev(p.sigma), dev(p.W), dev(p.a), dev(p.b), flags=nk.NK_CHECK_SPINS)
+    e_ref, _ = run_oracle(p)
+    assert_eloc(e_ok.cpu().numpy(), e_ref)
 
 
 @pytest.mark.parametrize("case", [
