@@ -53,6 +53,28 @@ def test_argument_errors_are_reported_before_any_launch(lib):
     assert lib.nk_rbm_logpsi_workspace_bytes(16, 10, 10, 0) > 0
     assert lib.nk_rbm_logpsi(None, 4, 10, 10, 0, None, None, None, None, None, 0, None, 0, None) == -1
     assert lib.nk_local_energy(None, None, 4, 10, 10, 0, None, None, None, 0, None, None, None, None, 0, None) == -1
+    # the calls around the hot path validate on the host too (a fake non-NULL pointer is never dereferenced there)
+    P = ctypes.c_void_p(256)
+    assert lib.nk_local_energy_ex(None, P, 4, 10, 10, 0, P, None, None, 0, 64, P, None, None, P, 1 << 20, None) == -1
+    assert lib.nk_energy_gradient_workspace_bytes(16, 10, 10, 0, 0) > 0
+    assert lib.nk_energy_gradient(P, 4, 10, 10, 0, P, None, None, P, 0, None, None, P, P, 1 << 20, None) == -1  # eloc NULL
+    assert lib.nk_qgt_matvec_workspace_bytes(16, 10, 10, 1, 4) > 0
+    assert lib.nk_qgt_matvec(P, 4, 10, 10, 0, P, None, None, None, None, 0.0, 0, None, None, P, P, 1 << 20, None) == -1
+    assert lib.nk_qgt_matvec(P, 4, 10, 10, 0, P, None, None, None, P, -1.0, 0, None, None, P, P, 1 << 20, None) == -1
+    assert lib.nk_qgt_matvec(P, 4, 10, 10, 0, P, None, None, None, P, 0.0, 0, None, None, P, None, 0, None) == -3
+    assert lib.nk_sr_solve_workspace_bytes(16, 10, 10, 0, 0) > lib.nk_qgt_matvec_workspace_bytes(16, 10, 10, 0, 0)
+    assert lib.nk_sr_solve(P, 4, 10, 10, 0, P, None, P, P, None, 0.01, 1e-5, 10, 0, P, P, P, None, P, 1 << 20, None) == -1
+    assert lib.nk_sr_solve(P, 4, 10, 10, 0, P, None, P, P, P, 0.01, -1.0, 10, 0, P, P, P, None, P, 1 << 20, None) == -1
+    assert lib.nk_metropolis_workspace_bytes(1, 0, 16, 10, 10, 0, 0) == 0          # exchange rule without pairs
+    assert lib.nk_metropolis_workspace_bytes(0, 0, 16, 10, 10, 0, 0) > 0
+    pairs = np.array([[0, 1], [3, 10]], dtype=np.int32)                             # site 10 out of range
+    assert lib.nk_metropolis_sample(1, pairs.ctypes.data, 2, P, 4, 10, 10, 0, P, None, None, 5, 0, 0, 0, 0, None, P,
+                                    1 << 20, None) == -1
+    assert lib.nk_metropolis_sample(7, None, 0, P, 4, 10, 10, 0, P, None, None, 5, 0, 0, 0, 0, None, P, 1 << 20, None) == -1
+    assert lib.nk_metropolis_sample(0, None, 0, P, 4, 10, 10, 0, P, None, None, -1, 0, 0, 0, 0, None, P, 1 << 20, None) == -1
+    assert lib.nk_rbmsymm_expand(0, 4, 10, 0, P, None, P, P, None, None) == -1
+    assert lib.nk_rbmsymm_reduce_gradient(2, 4, 10, 3, P, None, P, P, None, None) == -1
+    assert lib.nk_rbm_logpsi(P, 4, 10, 4096, 0, P, None, None, P, None, 0, P, 1 << 30, None) == -4               # M too large
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
