@@ -59,18 +59,30 @@ Geometry make_geometry(const Operator* op, int N, int M, int dtype) {
     g.n_rows = op ? (op->kind == NK_HEISENBERG ? op->n_bonds : op->n_sites) : 0;
     g.ok = g.M_pad / MPAD_ALIGN <= (cplx ? MAX_V_CPLX : MAX_V_REAL) && N <= 65535 && g.n_rows <= 65535;
     g.ctas_per_sm = fused_ctas_per_sm(g.M_pad, cplx);
-    // shared-memory plan of the fused kernel: [stages x tile][bit-packed spins][2 x stages mbarriers];
-    // 4 stages, as many rows per stage as fit (<= 32: one ballot bit per row)
+    // shared-memory plan of the fused kernel: [stages x tile][bit-packed spins][stages mbarriers + counters];
+    // as many rows per stage as fit (<= 32: one ballot bit per row)
     const size_t budget = (size_t)(227 * 1024) / g.ctas_per_sm - (g.ctas_per_sm > 1 ? 1024 : 0);
     const size_t sig = ((size_t)fused_consumer_warps() * g.n_words * 4 + 15) & ~size_t(15);
     const size_t row_bytes = (size_t)g.M_eff * 4;
-    const size_t fixed = sig + (8 + 4) * 4 + 128;         // spins + barriers + counters + alignment slack
+    const size_t fixed = sig + (8 + 4) * 8 + 128;         // spins + barriers + counters + alignment slack
     if (fixed + 2 * row_bytes > budget) { g.ok = false; g.tile_rows = 1; g.stages = 2; }
     else {
-        g.stages = 4;
+        // Few, large stages: every tile costs each warp a ballot, an mbarrier wait and a release, so the measured
+        // optimum at config 5 (8 KB rows) is 2 stages x 14 rows (fused 36.5 ms) over 3 x 9 (36.9) and 4 x 7 (37.5);
+        // more than 2 stages only once a stage already holds the 32 rows one ballot can name.
+        g.stages = 2;
         int tr = (int)((budget - fixed) / (g.stages * row_bytes));
-        if (tr < 1) { g.stages = 2; tr = (int)((budget - fixed) / (g.stages * row_bytes)); }
-        if (tr > 32) tr = 32;
+        if (tr > 32) {
+            tr = 32;
+            g.stages = (int)((budget - fixed) / ((size_t)tr * row_bytes));
+            if (g.stages > 4) g.stages = 4;
+        }
+        if (const char* e = std::getenv("NK_STAGES")) {                     // experiment knob
+            g.stages = atoi(e) < 2 ? 2 : atoi(e);
+            tr = (int)((budget - fixed) / (g.stages * row_bytes));
+            if (tr > 32) tr = 32;
+            if (tr < 1) { g.stages = 2; tr = (int)((budget - fixed) / (g.stages * row_bytes)); }
+        }
         g.tile_rows = tr;
     }
     g.n_tiles = (g.n_rows + g.tile_rows - 1) / g.tile_rows;
