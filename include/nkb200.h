@@ -120,8 +120,11 @@ int nk_local_energy(nk_operator_t op, const int8_t* sigma, int64_t B, int N, int
  *   psi'/psi = e^{s da} prod_j cosh(d_j) prod_j (1 + s tanh(theta_j) tanh(d_j)),
  * d the change of theta under the flip / exchange; tanh(d) and prod_j cosh(d_j) depend on the parameters only and are
  * tabulated per call, tanh(theta) once per sample, so an (amplitude, hidden unit) pair costs two FP32 operations and
- * no transcendental.  Same outputs and tolerances; for complex parameters tanh(theta) is unbounded next to the zeros
- * of cosh (Q18), where the log-cosh form is the better conditioned one. */
+ * no transcendental.  Same outputs and tolerances for |d| up to ~2 (parameters of the five configs x5); beyond, the
+ * factors 1 - |tanh(theta) tanh(d)| cancel and the fp32 rounding of the two tanh shows (~5e-4 at x10).  For complex
+ * parameters tanh(theta) is unbounded next to the zeros of cosh (Q18).  The log-cosh form is the better
+ * conditioned one in both regimes, hence the default.
+ * NK_CHECK_SPINS: validate sigma first (see enum nk_flags); the two flags may be combined. */
 int nk_local_energy_ex(nk_operator_t op, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
                        const void* a, const void* b, int64_t chunk_size, unsigned flags, void* eloc_out,
                        void* logpsi_out, double* stats_out, void* workspace, size_t workspace_bytes,
