@@ -11,7 +11,7 @@ import os
 import numpy as np
 
 __all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host", "energy_gradient",
-           "qgt_matvec", "sr_solve", "rbmsymm_expand", "rbmsymm_reduce_gradient", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "LIB_PATH",
+           "qgt_matvec", "sr_solve", "rbmsymm_expand", "rbmsymm_reduce_gradient", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "allreduce_gradient", "LIB_PATH",
            "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "NK_FORM_PRODUCT", "NK_CHECK_SPINS", "EXPORTS"]
 
 NK_HEISENBERG, NK_ISING = 0, 1
@@ -462,3 +462,25 @@ def allreduce_stats(stats):
     gathered = [torch.empty_like(t) for _ in range(dist.get_world_size())]
     dist.all_gather(gathered, t.contiguous())
     return combine_stats([g.cpu().numpy() for g in gathered])
+
+
+def allreduce_gradient(grads, n_local: int):
+    """Combine per-rank gradient / force / QGT-vector blocks into those of the union of the shards (in place).
+    Each rank calls nk_energy_gradient (or nk_qgt_matvec) on its own samples with the GLOBAL mean in `stats`
+    (allreduce_stats), which gives g_r = (1/B_r) sum_{s in r} O_s^* (E_s - mean); the union's g is
+    sum_r (B_r / B) g_r: one weighted all-reduce per block (NCCL on GPUs, gloo on CPU).  Returns `grads`."""
+    torch = _torch()
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return grads
+    n = torch.tensor([float(n_local)], dtype=torch.float64, device=grads[0].device)
+    dist.all_reduce(n)
+    w = float(n_local) / float(n.item())
+    for g in grads:
+        if g is not None:
+            g.mul_(w)
+            if g.is_complex():
+                dist.all_reduce(torch.view_as_real(g))
+            else:
+                dist.all_reduce(g)
+    return grads

@@ -128,7 +128,13 @@ def _rank_main(rank, world, port, q):
     e = rng.normal(size=1000)
     shard = e[rank::world]                                             # each rank owns a slice of the samples
     out = nk.allreduce_stats(torch.tensor(orc.stats(shard), dtype=torch.float64))
-    q.put((rank, out.tolist()))
+    # gradient blocks: each rank's force with the GLOBAL mean, shards of unequal size, weighted all-reduce
+    O = rng.normal(size=(1000, 7)) + 1j * rng.normal(size=(1000, 7))
+    ec = e + 1j * rng.normal(size=1000)
+    mine = np.arange(1000) % 3 == 0 if rank == 0 else np.arange(1000) % 3 != 0
+    g_r = (np.conj(O[mine]) * (ec[mine] - ec.mean())[:, None]).mean(axis=0)
+    g = nk.allreduce_gradient([torch.from_numpy(g_r.copy()), torch.from_numpy(g_r.real.copy())], int(mine.sum()))
+    q.put((rank, out.tolist(), g[0].numpy().tolist(), g[1].numpy().tolist()))
     dist.destroy_process_group()
 
 
@@ -139,8 +145,15 @@ def test_allreduce_stats_gloo_world_size_2():
     port = _free_port()
     procs = [ctx.Process(target=_rank_main, args=(r, 2, port, q)) for r in range(2)]
     [p.start() for p in procs]
-    res = dict(q.get(timeout=120) for _ in procs)
+    got = [q.get(timeout=120) for _ in procs]
+    res = {g[0]: g[1:] for g in got}
     [p.join(60) for p in procs]
-    e = np.random.default_rng(0).normal(size=1000)
+    rng = np.random.default_rng(0)
+    e = rng.normal(size=1000)
+    O = rng.normal(size=(1000, 7)) + 1j * rng.normal(size=(1000, 7))
+    ec = e + 1j * rng.normal(size=1000)
+    want = orc.force(O, ec)                                            # the unsharded force vector (Eq. (14))
     for r in range(2):
-        np.testing.assert_allclose(res[r], orc.stats(e), rtol=1e-12, atol=1e-14)
+        np.testing.assert_allclose(res[r][0], orc.stats(e), rtol=1e-12, atol=1e-14)
+        np.testing.assert_allclose(np.array(res[r][1]), want, atol=1e-13)
+        np.testing.assert_allclose(np.array(res[r][2]), want.real, atol=1e-13)
