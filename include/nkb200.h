@@ -80,7 +80,8 @@ int nk_operator_max_conn(nk_operator_t op, int* C_out);
 /* ---- ln psi ---------------------------------------------------------------------------------------------
  * logpsi_out dev [B]: float | (re,im) float, or double | (re,im) double with NK_OUT_F64.  The imaginary part
  * is returned modulo 2 pi (a sum of principal logs).  theta_out: NULL, or dev [B][M] (float | (re,im) float)
- * receiving theta = W s + b.  theta is contracted with exact +-1 products and fp32 accumulation; the ln cosh
+ * receiving theta = W s + b.  theta is contracted on the tensor cores from an exact fixed-point split of W (|W - W_fixed|
+ * <= 2^-23 max|W|) with exact +-1 products and exact integer accumulation; the ln cosh
  * terms and their sum are evaluated in fp64 (Q12).  workspace: dev, 256-B aligned, at least
  * nk_rbm_logpsi_workspace_bytes(B, N, M, dtype) bytes. */
 size_t nk_rbm_logpsi_workspace_bytes(int64_t B, int N, int M, int dtype);

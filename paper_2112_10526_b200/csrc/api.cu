@@ -52,7 +52,7 @@ static int cuda_fail(cudaError_t e) {
 Geometry make_geometry(const Operator* op, int N, int M, int dtype) {
     Geometry g{};
     const bool cplx = dtype == NK_C64;
-    g.N = N; g.n_words = (N + 31) / 32; g.K_pad = round_up(N, 64);
+    g.N = N; g.n_words = (N + 31) / 32; g.K_pad = round_up(N, 128);
     g.M = M; g.M_pad = round_up(M, MPAD_ALIGN);
     g.planes = cplx ? 2 : 1;
     g.M_eff = g.planes * g.M_pad;
@@ -108,7 +108,7 @@ struct Carver {
 
 struct LogpsiWs {
     float *Wg, *bg, *theta;
-    uint16_t *Ws, *A;          // bf16 operands of the tensor-core contraction
+    uint16_t *Ws, *A;          // operands of the tensor-core contraction (int8 planes + scale; padded int8 spins)
     unsigned* absmax;
     size_t bytes;
 };
@@ -412,12 +412,12 @@ size_t nk_qgt_matvec_workspace_bytes(int64_t B, int N, int M, int dtype, int64_t
     return carve_qgt(nullptr, g, B, eff_chunk(B, chunk_size), dtype).bytes;
 }
 
-// theta, the bf16 spins and their transposes for the WHOLE batch, kept across the matvecs of one nk_sr_solve (the
+// theta, the padded int8 spins and their bf16 transposes for the WHOLE batch, kept across the matvecs of one nk_sr_solve (the
 // parameters do not change during the solve): a matvec then costs one contraction less per pass and no conversions
 namespace {
 struct QgtCache {
     float* theta_all;        // [B][M_eff]
-    uint16_t* A_all;         // [B][K_pad] bf16
+    uint16_t* A_all;         // [B][K_pad] int8 (allocated as 2 B per entry)
     uint16_t* sigT_all;      // [n_chunks][N][ld] bf16
     size_t sigT_stride;      // N * ld
 };
@@ -452,10 +452,10 @@ static int qgt_matvec_impl(const int8_t* sigma, int64_t B, int N, int M, int dty
         const float* th = w.g.theta;
         if (cache == nullptr) {
             NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.g.Ws, w.g.A, w.g.bg, w.g.theta, st));
-            NK_CUDA(launch_theta_tc_pre(w.g.A, nb, g.M_eff, g.K_pad, w.Vs, w.vbg, w.Y, st));
+            NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.Vs, w.g.A, w.vbg, w.Y, st));
         } else {
             th = cache->theta_all + (size_t)s0 * g.M_eff;
-            NK_CUDA(launch_theta_tc_pre(cache->A_all + (size_t)s0 * g.K_pad, nb, g.M_eff, g.K_pad, w.Vs, w.vbg, w.Y, st));
+            NK_CUDA(launch_theta_tc_pre((const uint8_t*)cache->A_all + (size_t)s0 * g.K_pad, nb, g.M_eff, g.K_pad, w.Vs, w.vbg, w.Y, st));
         }
         NK_CUDA(launch_qgt_w(g, dtype, sg, nb, th, w.Y, v_a, (uint8_t*)w.wbuf + s0 * esz, st));
     }
@@ -560,15 +560,15 @@ int nk_sr_solve(const int8_t* sigma, int64_t B, int N, int M, int dtype, const v
         NK_CUDA(cudaMemcpyAsync(blk(w.r, k), fsrc[k], fbytes[k], cudaMemcpyDeviceToDevice, st));
         NK_CUDA(cudaMemcpyAsync(blk(w.p, k), fsrc[k], fbytes[k], cudaMemcpyDeviceToDevice, st));
     }
-    {   // theta, bf16 spins and their transposes of the whole batch, once per solve
+    {   // theta, padded spins and their transposes of the whole batch, once per solve
         const QgtWs q = carve_qgt(w.qgt, g, B, eff_chunk(B, chunk_size), dtype);
         const int64_t chunk = eff_chunk(B, chunk_size);
         NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, q.g.Wg, q.g.bg, st));
         NK_CUDA(launch_split_w(q.g.Wg, g.M_eff, N, g.K_pad, q.g.Ws, q.g.absmax, st));
-        NK_CUDA(launch_sigma_bf16(sigma, B, N, g.K_pad, w.cache.A_all, st));
+        NK_CUDA(launch_sigma_operand(sigma, B, N, g.K_pad, w.cache.A_all, st));
         for (int64_t s0 = 0; s0 < B; s0 += chunk) {
             const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
-            NK_CUDA(launch_theta_tc_pre(w.cache.A_all + (size_t)s0 * g.K_pad, nb, g.M_eff, g.K_pad, q.g.Ws, q.g.bg,
+            NK_CUDA(launch_theta_tc_pre((const uint8_t*)w.cache.A_all + (size_t)s0 * g.K_pad, nb, g.M_eff, g.K_pad, q.g.Ws, q.g.bg,
                                         w.cache.theta_all + (size_t)s0 * g.M_eff, st));
             NK_CUDA(launch_sigma_T(sigma + s0 * N, nb, N, q.g.ld,
                                    w.cache.sigT_all + (size_t)(s0 / chunk) * w.cache.sigT_stride, st));

@@ -45,7 +45,7 @@ inline size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
 // Geometry derived from (op, N, M, dtype).
 struct Geometry {
     int N, n_words, M, M_pad, M_eff, planes; // M_eff = planes * M_pad; n_words = ceil(N / 32)
-    int K_pad;                               // N rounded up to 64: k extent of the bf16 tensor-core operands
+    int K_pad;                               // N rounded up to 128: k extent (bytes per row) of the int8 tensor-core operands
     int n_rows, tile_rows, n_tiles, n_rows_pad;
     int stages, ctas_per_sm;                 // shared-memory ring plan of the fused kernel
     size_t smem_bytes;
@@ -78,14 +78,15 @@ cudaError_t launch_metropolis(const Geometry& g, int dtype, int8_t* sigma, int64
 // theta_gemm.cu : theta[s][m] = bg[m] + sum_k sigma[s][k] Wg[m][k]
 cudaError_t launch_theta_gemm(const int8_t* sigma, int64_t B, int N, int M_eff, const float* Wg, const float* bg,
                               float* theta, cudaStream_t st);
-// theta_tc.cu : the same contraction on tcgen05 tensor cores (bf16 x3 split of W, two TMEM accumulators)
+// theta_tc.cu : the same contraction on tcgen05 tensor cores (kind::i8, three int8 digit planes of W, three int32
+// TMEM accumulators); Ws = the planes + scale, A = scratch for a padded int8 copy of the spins when N % 128 != 0
 cudaError_t theta_tc_init();
-cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* Ws_bf16, unsigned* absmax_scratch,
+cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* Ws, unsigned* absmax_scratch,
                            cudaStream_t st);
-cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, int K_pad, const void* Ws_bf16,
-                            void* A_bf16, const float* bg, float* theta, cudaStream_t st);
-cudaError_t launch_sigma_bf16(const int8_t* sigma, int64_t B, int N, int K_pad, void* A_bf16, cudaStream_t st);
-cudaError_t launch_theta_tc_pre(const void* A_bf16, int64_t B, int M_eff, int K_pad, const void* Ws_bf16,
+cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, int K_pad, const void* Ws,
+                            void* A, const float* bg, float* theta, cudaStream_t st);
+cudaError_t launch_sigma_operand(const int8_t* sigma, int64_t B, int N, int K_pad, void* A_i8, cudaStream_t st);
+cudaError_t launch_theta_tc_pre(const void* A_i8, int64_t B, int M_eff, int K_pad, const void* Ws,
                                 const float* bg, float* theta, cudaStream_t st);   // launch_theta_tc without the spin conversion
 cudaError_t launch_tc_gemm_pieces(const void* A_bf16, int64_t rows, const void* P_bf16, int cols, int ld, int k_len,
                                   float* out, int accumulate, cudaStream_t st);

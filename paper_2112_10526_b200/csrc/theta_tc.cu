@@ -1,20 +1,24 @@
 // Base activations theta = sigma W^T + b on the 5th-generation tensor cores (BASELINE.json
 // north_star (2): "the one place tensor cores are justified").
 //
-// Exactness: sigma = +-1 is exact in bf16.  W (fp32) is split on three FIXED-POINT grids tied to max|W|:
-//   W ~ W_hi + W_mid + W_lo,  W_hi = m1 2^e1, W_mid = m2 2^(e1-8), W_lo = m3 2^(e1-16),  |m| <= 256 integers,
-//   2^(e1+8) > max|W|,  residual <= 2^(e1-17) < 2^-25 max|W|  (below one fp32 ulp of any |w| > max|W| / 4).
-// Every piece is exact in bf16, every product is exact, and each piece has its OWN TMEM accumulator, in which all
-// partial sums are integers < 2^24 times the piece's quantum: the tensor-core accumulation is exact whatever
-// rounding the adder uses (measured: with per-element bf16 splitting the adder's truncation of sub-ulp bits
-// biased theta toward zero by ~0.25 ulp, which adds up coherently over the M terms of ln psi).  Only the epilogue
-// rounds: theta = (D_hi + (D_mid + D_lo)) + b in fp32, round-to-nearest.
+// Two instantiations of one kernel:
+//  * theta (I8 = true): int8 operands, tcgen05 kind::i8 (twice the bf16 MMA rate, half the operand bytes), int32
+//    accumulators.  sigma = +-1 IS the A operand (used in place when its rows are a multiple of 128 long).  W (fp32)
+//    becomes three int8 digit planes of a fixed-point number, rint(W / q) = d2 2^16 + d1 2^8 + d0, q a power of two
+//    tied to max|W| (split_w_i8_kernel); every product and every int32 partial sum is exact, each plane has its own
+//    TMEM accumulator, and only the epilogue rounds: theta = q (D2 2^16 + D1 2^8 + D0) + b in fp32.
+//  * the contraction over samples of the force vector / QGT (I8 = false, launch_tc_gemm_pieces): bf16 operands,
+//    kind::f16, fp32 accumulators; the left operand v = conj(tanh theta) w_s is split by the caller on three
+//    fixed-point bf16 grids (|m| <= 256 integers times 2^e1, 2^(e1-8), 2^(e1-16)), exact in bf16 with exact products
+//    and partial sums that are integers below 2^24 quanta — exact whatever rounding the adder uses (measured: with
+//    per-element bf16 splitting the adder's truncation biased the result by ~0.25 ulp, coherently over the terms).
+//    Epilogue: out = (D_hi + (D_mid + D_lo)) in fp32.
 //
-// Kernel: one CTA per 128 (samples) x 128 (hidden) tile.  Warp 0 = TMA producer (cp.async.bulk.tensor, 128B
-// swizzle, 3-stage ring: per stage the sigma tile and the three W-piece tiles for a 64-wide k block); warp 1 =
-// TMEM allocator and single-thread tcgen05.mma issuer (kind::f16, M=128, N=128, K=16; 12 MMAs per k block, three
-// 128-column fp32 accumulators);
-// warps 2-5 = epilogue (tcgen05.ld 32x32b, bias add, fp32 stores).
+// Kernel: one CTA per 128 (rows) x 128 (columns) tile.  Warp 0 = TMA producer (cp.async.bulk.tensor, 128B swizzle,
+// 3-stage ring: per stage the A tile and the three piece tiles of a k block of 128 bytes per row = 128 int8 or 64
+// bf16); warp 1 = TMEM allocator and single-thread tcgen05.mma issuer (M = 128, N = 128, K = 32 int8 / 16 bf16:
+// 12 MMAs per k block, three 128-column accumulators); warps 2-5 = epilogue (tcgen05.ld 32x32b, scale / bias, fp32
+// stores).
 #include <cuda.h>
 #include <cuda_bf16.h>
 
@@ -31,6 +35,8 @@ constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment*/ + 256 /*bar
 constexpr int THREADS = 192;
 constexpr uint32_t TMEM_COLS = 512;                       // D_hi [0,128), D_mid [128,256), D_lo [256,384); power of 2
 // instruction descriptor (cute::UMMA::InstrDescriptor bit layout): D=F32, A=B=BF16, K-major both, N=128, M=128
+// kind::i8: D = S32 (c_format 2), A = B = signed 8 bit (format 1), K-major, N and M as for bf16
+constexpr uint32_t IDESC_I8 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
 constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
 }  // namespace tc
 
@@ -82,6 +88,51 @@ __global__ void sigma_bf16_kernel(const int8_t* __restrict__ sigma, int64_t B, i
     }
 }
 
+// ---- int8 operands of the theta contraction (tcgen05 kind::i8: twice the bf16 MMA rate, half the operand bytes) ----
+// Wq[piece][me][k] (int8, K_pad columns, zero padded): rint(W / q) = I = d2 2^16 + d1 2^8 + d0 with balanced base-256
+// digits d in [-128, 127]; q is a POWER OF TWO, 2^(ex-23) with 2^ex > max|W| (one step coarser if max|W| / q would
+// pass 8355000: three digits hold |I| <= 8355711), so W / q and q I are exact scalings — a scale that is not a
+// power of two was measured to bias every theta by the same 1e-7 relative error, which adds up coherently in ln psi.
+// Pieces stored hi, mid, lo.  The products with sigma = +-1 and their int32 sums over k are exact; the residual
+// |W - q I| <= q / 2 <= 2^-23 max|W|.  The scale q is left as a float right behind the three planes (byte offset
+// 3 M_eff K_pad).
+__global__ void split_w_i8_kernel(const float* __restrict__ Wg, int M_eff, int N, int K_pad,
+                                  const unsigned* __restrict__ absmax_bits, int8_t* __restrict__ Wq) {
+    const float wmax = __uint_as_float(*absmax_bits);
+    int ex = -100;
+    if (wmax > 0.f) frexpf(wmax, &ex);                    // wmax = f 2^ex, f in [0.5, 1)
+    if (ldexpf(wmax, 23 - ex) > 8355000.f) ++ex;          // f > 0.996: the top digit would overflow
+    const float sc = ldexpf(1.f, 23 - ex);
+    const int me = blockIdx.y;
+    const size_t plane = (size_t)M_eff * K_pad;
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < K_pad; k += gridDim.x * blockDim.x) {
+        const float w = (k < N) ? Wg[(size_t)me * N + k] : 0.f;
+        const int I = (int)rintf(w * sc);
+        const int d0 = ((I + 128) & 255) - 128;
+        const int I1 = (I - d0) >> 8;
+        const int d1 = ((I1 + 128) & 255) - 128;
+        const int d2 = (I1 - d1) >> 8;                    // |I| <= 8355000 < 8355711: fits [-128, 127]
+        const size_t o = (size_t)me * K_pad + k;
+        Wq[o] = (int8_t)d2;
+        Wq[plane + o] = (int8_t)d1;
+        Wq[2 * plane + o] = (int8_t)d0;
+    }
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0)
+        *reinterpret_cast<float*>(Wq + 3 * plane) = ldexpf(1.f, ex - 23);
+}
+
+// A[s][k] = sigma[s][k] zero padded to K_pad (only needed when N is not a multiple of 128: TMA wants 16-B strides)
+__global__ void sigma_pad_i8_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int K_pad,
+                                    int8_t* __restrict__ A) {
+    const int64_t total = B * K_pad;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t s = idx / K_pad;
+        const int k = (int)(idx - s * K_pad);
+        A[idx] = k < N ? sigma[s * N + k] : (int8_t)0;
+    }
+}
+
 // ---- tcgen05 / TMA wrappers --------------------------------------------------------------------------------
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
     asm volatile(
@@ -110,6 +161,16 @@ __device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint6
         "}\n" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+__device__ __forceinline__ void umma_i8(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                        uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t"
+        "}\n" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
@@ -128,9 +189,14 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
 }
 
 // ---- the GEMM ---------------------------------------------------------------------------------------------
+// I8 = false: bf16 operands (BK = 64 elements per 128-B swizzle row), fp32 accumulators, out = hi + mid + lo.
+// I8 = true:  int8 operands (BK = 128 elements per row, so K_pad / 128 k blocks), int32 accumulators,
+//             out = q (hi 2^16 + mid 2^8 + lo) with the scale q read from `scale`.
+template <bool I8>
 __global__ void __launch_bounds__(tc::THREADS, 1)
 theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w, int64_t B,
-                int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta, int accumulate) {
+                int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta, int accumulate,
+                const float* __restrict__ scale) {
     using namespace tc;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;            // SWIZZLE_128B needs 1024 B
@@ -142,7 +208,8 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n0 = blockIdx.x * BN;                       // hidden-unit tile
     const int64_t m0 = (int64_t)blockIdx.y * BM;          // sample tile
-    const int n_kb = K_pad / BK;
+    constexpr int BKE = I8 ? 2 * BK : BK;                 // elements per k block (128 B per row either way)
+    const int n_kb = K_pad / BKE;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, 1); }
@@ -167,10 +234,10 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                 mbar_wait(empty0 + 8 * stage, parity);
                 mbar_arrive_expect_tx(full0 + 8 * stage, STAGE_BYTES);
                 const uint32_t dst = smem_base + stage * STAGE_BYTES;
-                tma_load_2d(dst, &map_a, kb * BK, (int)m0, full0 + 8 * stage);
+                tma_load_2d(dst, &map_a, kb * BKE, (int)m0, full0 + 8 * stage);
 #pragma unroll
                 for (int pc = 0; pc < 3; ++pc)
-                    tma_load_2d(dst + (1 + pc) * TILE_BYTES, &map_w, kb * BK, pc * M_eff + n0, full0 + 8 * stage);
+                    tma_load_2d(dst + (1 + pc) * TILE_BYTES, &map_w, kb * BKE, pc * M_eff + n0, full0 + 8 * stage);
                 if (++stage == STAGES) { stage = 0; parity ^= 1; }
             }
         }
@@ -187,9 +254,15 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                     const uint32_t koff = k * UMMA_K * 2;                       // bytes inside the 128 B swizzle row
                     const uint64_t ad = make_sdesc(a_addr + koff);
                     const uint32_t first = (kb | k) ? 1u : 0u;
-                    umma_bf16(tmem_base + 0, ad, make_sdesc(a_addr + 1 * TILE_BYTES + koff), IDESC, first);
-                    umma_bf16(tmem_base + BN, ad, make_sdesc(a_addr + 2 * TILE_BYTES + koff), IDESC, first);
-                    umma_bf16(tmem_base + 2 * BN, ad, make_sdesc(a_addr + 3 * TILE_BYTES + koff), IDESC, first);
+                    if constexpr (I8) {                                         // 32 B = 32 int8 = one K = 32 MMA
+                        umma_i8(tmem_base + 0, ad, make_sdesc(a_addr + 1 * TILE_BYTES + koff), IDESC_I8, first);
+                        umma_i8(tmem_base + BN, ad, make_sdesc(a_addr + 2 * TILE_BYTES + koff), IDESC_I8, first);
+                        umma_i8(tmem_base + 2 * BN, ad, make_sdesc(a_addr + 3 * TILE_BYTES + koff), IDESC_I8, first);
+                    } else {
+                        umma_bf16(tmem_base + 0, ad, make_sdesc(a_addr + 1 * TILE_BYTES + koff), IDESC, first);
+                        umma_bf16(tmem_base + BN, ad, make_sdesc(a_addr + 2 * TILE_BYTES + koff), IDESC, first);
+                        umma_bf16(tmem_base + 2 * BN, ad, make_sdesc(a_addr + 3 * TILE_BYTES + koff), IDESC, first);
+                    }
                 }
                 umma_commit(empty0 + 8 * stage);          // frees the smem stage when these MMAs have read it
                 if (++stage == STAGES) { stage = 0; parity ^= 1; }
@@ -203,6 +276,7 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const int64_t row = m0 + q * 32 + lane;
         float* out = theta + row * M_eff + n0;
+        const float qs = I8 ? *scale : 1.f;
 #pragma unroll 1
         for (int c0 = 0; c0 < BN; c0 += 32) {
             float hi[32], mid[32], lo[32];
@@ -221,10 +295,20 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                         bb.x += old.x; bb.y += old.y; bb.z += old.z; bb.w += old.w;
                     }
                     float4 o;
-                    o.x = (hi[j] + (mid[j] + lo[j])) + bb.x;
-                    o.y = (hi[j + 1] + (mid[j + 1] + lo[j + 1])) + bb.y;
-                    o.z = (hi[j + 2] + (mid[j + 2] + lo[j + 2])) + bb.z;
-                    o.w = (hi[j + 3] + (mid[j + 3] + lo[j + 3])) + bb.w;
+                    if constexpr (I8) {
+                        auto comb = [&](int jj) -> float {                      // exact ints below 2^24 each
+                            const float h = (float)__float_as_int(hi[jj]), m = (float)__float_as_int(mid[jj]),
+                                        l = (float)__float_as_int(lo[jj]);
+                            return fmaf(h, 65536.f, fmaf(m, 256.f, l));
+                        };
+                        o.x = fmaf(qs, comb(j), bb.x); o.y = fmaf(qs, comb(j + 1), bb.y);
+                        o.z = fmaf(qs, comb(j + 2), bb.z); o.w = fmaf(qs, comb(j + 3), bb.w);
+                    } else {
+                        o.x = (hi[j] + (mid[j] + lo[j])) + bb.x;
+                        o.y = (hi[j + 1] + (mid[j + 1] + lo[j + 1])) + bb.y;
+                        o.z = (hi[j + 2] + (mid[j + 2] + lo[j + 2])) + bb.z;
+                        o.w = (hi[j + 3] + (mid[j + 3] + lo[j + 3])) + bb.w;
+                    }
                     *reinterpret_cast<float4*>(out + c0 + j) = o;
                 }
             }
@@ -253,22 +337,29 @@ cudaError_t theta_tc_init() {
     if (e != cudaSuccess) return e;
     if (qres != cudaDriverEntryPointSuccess || fn == nullptr) return cudaErrorNotSupported;
     g_encode = (EncodeTiledFn)fn;
-    e = cudaFuncSetAttribute((const void*)theta_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::SMEM_BYTES);
+    e = cudaFuncSetAttribute((const void*)theta_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             tc::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute((const void*)theta_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             tc::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     g_tc_ready = true;
     return cudaSuccess;
 }
 
-static bool encode_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols) {
+// 2-D tensor map over a k-contiguous [rows][cols] operand, box = 128 rows x 128 B (64 bf16 or 128 int8), 128B swizzle
+static bool encode_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols, bool i8 = false) {
     const cuuint64_t dims[2] = {cols, rows};
-    const cuuint64_t strides[1] = {cols * 2};
-    const cuuint32_t box[2] = {(cuuint32_t)tc::BK, (cuuint32_t)tc::BM};
+    const cuuint64_t strides[1] = {cols * (i8 ? 1u : 2u)};
+    const cuuint32_t box[2] = {(cuuint32_t)(i8 ? 2 * tc::BK : tc::BK), (cuuint32_t)tc::BM};
     const cuuint32_t estr[2] = {1, 1};
-    return g_encode(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
-                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+    return g_encode(map, i8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
+                    const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// W -> three int8 planes + scale (K_pad a multiple of 128); the buffer must hold 3 M_eff K_pad + 4 bytes
 cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* Ws, unsigned* absmax_scratch,
                            cudaStream_t st) {
     cudaError_t e = cudaMemsetAsync(absmax_scratch, 0, sizeof(unsigned), st);
@@ -278,51 +369,47 @@ cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* W
     if (blocks > 1184) blocks = 1184;
     absmax_kernel<<<blocks, 256, 0, st>>>(Wg, n, absmax_scratch);
     dim3 grid((K_pad + 255) / 256, M_eff);
-    split_w_kernel<<<grid, 256, 0, st>>>(Wg, M_eff, N, K_pad, absmax_scratch, (__nv_bfloat16*)Ws);
+    split_w_i8_kernel<<<grid, 256, 0, st>>>(Wg, M_eff, N, K_pad, absmax_scratch, (int8_t*)Ws);
     count_launch(2);
     return cudaGetLastError();
 }
 
-cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, int K_pad, const void* Ws, void* A,
-                            const float* bg, float* theta, cudaStream_t st) {
-    if (B <= 0) return cudaSuccess;
-    cudaError_t e = theta_tc_init();
-    if (e != cudaSuccess) return e;
-    const int64_t total = B * K_pad;
-    int64_t blocks = (total + 255) / 256;
-    if (blocks > 148 * 16) blocks = 148 * 16;
-    sigma_bf16_kernel<<<(unsigned)blocks, 256, 0, st>>>(sigma, B, N, K_pad, (__nv_bfloat16*)A);
-    CUtensorMap map_a, map_w;
-    if (!encode_2d(&map_a, A, (uint64_t)B, (uint64_t)K_pad)) return cudaErrorInvalidValue;
-    if (!encode_2d(&map_w, Ws, (uint64_t)3 * M_eff, (uint64_t)K_pad)) return cudaErrorInvalidValue;
-    dim3 grid(M_eff / tc::BN, (unsigned)((B + tc::BM - 1) / tc::BM));
-    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_w, B, M_eff, K_pad, bg, theta, 0);
-    count_launch(2);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_sigma_bf16(const int8_t* sigma, int64_t B, int N, int K_pad, void* A, cudaStream_t st) {
+// the spins as the A operand: sigma itself when its rows are already K_pad long, else a zero-padded int8 copy in A
+cudaError_t launch_sigma_operand(const int8_t* sigma, int64_t B, int N, int K_pad, void* A, cudaStream_t st) {
     if (B <= 0) return cudaSuccess;
     const int64_t total = B * K_pad;
     int64_t blocks = (total + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;
-    sigma_bf16_kernel<<<(unsigned)blocks, 256, 0, st>>>(sigma, B, N, K_pad, (__nv_bfloat16*)A);
+    sigma_pad_i8_kernel<<<(unsigned)blocks, 256, 0, st>>>(sigma, B, N, K_pad, (int8_t*)A);
     count_launch();
     return cudaGetLastError();
 }
 
+// theta[s][m] = bg[m] + sum_k A[s][k] W[m][k] with A an int8 [B][K_pad] operand (see launch_sigma_operand) and Ws the
+// planes of launch_split_w
 cudaError_t launch_theta_tc_pre(const void* A, int64_t B, int M_eff, int K_pad, const void* Ws, const float* bg,
                                 float* theta, cudaStream_t st) {
     if (B <= 0) return cudaSuccess;
     cudaError_t e = theta_tc_init();
     if (e != cudaSuccess) return e;
     CUtensorMap map_a, map_w;
-    if (!encode_2d(&map_a, A, (uint64_t)B, (uint64_t)K_pad)) return cudaErrorInvalidValue;
-    if (!encode_2d(&map_w, Ws, (uint64_t)3 * M_eff, (uint64_t)K_pad)) return cudaErrorInvalidValue;
+    if (!encode_2d(&map_a, A, (uint64_t)B, (uint64_t)K_pad, true)) return cudaErrorInvalidValue;
+    if (!encode_2d(&map_w, Ws, (uint64_t)3 * M_eff, (uint64_t)K_pad, true)) return cudaErrorInvalidValue;
+    const float* scale = reinterpret_cast<const float*>((const int8_t*)Ws + (size_t)3 * M_eff * K_pad);
     dim3 grid(M_eff / tc::BN, (unsigned)((B + tc::BM - 1) / tc::BM));
-    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_w, B, M_eff, K_pad, bg, theta, 0);
+    theta_tc_kernel<true><<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_w, B, M_eff, K_pad, bg, theta, 0, scale);
     count_launch();
     return cudaGetLastError();
+}
+
+cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, int K_pad, const void* Ws, void* A,
+                            const float* bg, float* theta, cudaStream_t st) {
+    if (B <= 0) return cudaSuccess;
+    if (N == K_pad && ((uintptr_t)sigma & 15) == 0)                      // rows already padded and 16-B aligned
+        return launch_theta_tc_pre(sigma, B, M_eff, K_pad, Ws, bg, theta, st);
+    cudaError_t e = launch_sigma_operand(sigma, B, N, K_pad, A, st);
+    if (e != cudaSuccess) return e;
+    return launch_theta_tc_pre(A, B, M_eff, K_pad, Ws, bg, theta, st);
 }
 
 // Generic entry used by the gradient: out[r][c] (+)= sum_k A[r][k] * (P0 + P1 + P2)[c][k], A bf16 [rows][ld] and
@@ -336,7 +423,8 @@ cudaError_t launch_tc_gemm_pieces(const void* A, int64_t rows, const void* P, in
     if (!encode_2d(&map_a, A, (uint64_t)rows, (uint64_t)ld)) return cudaErrorInvalidValue;
     if (!encode_2d(&map_p, P, (uint64_t)3 * cols, (uint64_t)ld)) return cudaErrorInvalidValue;
     dim3 grid(cols / tc::BN, (unsigned)((rows + tc::BM - 1) / tc::BM));
-    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_p, rows, cols, k_len, nullptr, out, accumulate);
+    theta_tc_kernel<false><<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_p, rows, cols, k_len, nullptr, out,
+                                                                      accumulate, nullptr);
     count_launch();
     return cudaGetLastError();
 }

@@ -282,3 +282,18 @@ def test_maximum_sizes(nk, case):
     e2, _, _ = nk.local_energy(op, dev(p.sigma), dev(p.W), dev(p.a), dev(p.b), flags=nk.NK_FORM_PRODUCT)
     assert_eloc(e2.cpu().numpy(), e_ref)
     op.close()
+
+
+def test_theta_fixed_point_split_at_the_top_of_a_binade(nk):
+    """max|W| just below a power of two (mantissa 0.99999): the int8 split of the contraction must step its scale up
+    instead of overflowing the top digit, and theta must still carry fp32-level accuracy."""
+    p = inp.make_config(2, n_samples=64)
+    W = p.W.copy()
+    W[3, 5] = np.nextafter(np.float32(0.25), np.float32(0))             # 0.99999994 * 2^-2, the largest entry
+    W[7, 11] = -np.nextafter(np.float32(0.25), np.float32(0))
+    assert np.abs(W).max() == np.abs(W[3, 5])
+    lp, theta = nk.rbm_logpsi(dev(p.sigma), dev(W), dev(p.a), dev(p.b), out_f64=True, return_theta=True)
+    torch.cuda.synchronize()
+    th_ref = orc.rbm_theta(p.sigma, W, p.b)
+    assert np.abs(theta.cpu().numpy() - th_ref).max() < 2e-6           # an overflowed digit would be an error of order 1
+    assert_logpsi(lp.cpu().numpy(), orc.rbm_logpsi(p.sigma, W, p.a, p.b))
