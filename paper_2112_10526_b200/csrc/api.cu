@@ -150,7 +150,7 @@ static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk) {
 static GradWs carve_grad(void* ws, const Geometry& g, int64_t chunk, size_t* bytes) {
     Carver c(ws);
     GradWs w;
-    w.ld = (int)((chunk + 63) / 64 * 64);
+    w.ld = (int)((chunk + 127) / 128 * 128);
     w.Wg = c.take<float>((size_t)g.M_eff * g.N);
     w.bg = c.take<float>(g.M_eff);
     w.theta = c.take<float>((size_t)chunk * g.M_eff);
@@ -418,7 +418,7 @@ namespace {
 struct QgtCache {
     float* theta_all;        // [B][M_eff]
     uint16_t* A_all;         // [B][K_pad] int8 (allocated as 2 B per entry)
-    uint16_t* sigT_all;      // [n_chunks][N][ld] bf16
+    uint16_t* sigT_all;      // [n_chunks][N][ld] int8 (allocated as 2 B per entry)
     size_t sigT_stride;      // N * ld
 };
 }  // namespace
@@ -473,7 +473,7 @@ static int qgt_matvec_impl(const int8_t* sigma, int64_t B, int N, int M, int dty
         } else {
             NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B, (const uint8_t*)w.wbuf + s0 * esz, w.wstats, w.g, first,
                                           1.f, st, cache->theta_all + (size_t)s0 * g.M_eff,
-                                          cache->sigT_all + (size_t)(s0 / chunk) * cache->sigT_stride));
+                                          (const uint8_t*)cache->sigT_all + (size_t)(s0 / chunk) * cache->sigT_stride));
         }
         first = 0;
     }
@@ -517,7 +517,7 @@ SrWs carve_sr(void* ws, int64_t B, int N, int M, int dtype, int64_t chunk_size) 
     const Geometry g = make_geometry(nullptr, N, M, dtype);
     const int64_t chunk = (chunk_size <= 0 || chunk_size > B) ? (B > 0 ? B : 1) : chunk_size;
     const int64_t n_chunks = B > 0 ? (B + chunk - 1) / chunk : 1;
-    const size_t ld = (size_t)((chunk + 63) / 64 * 64);
+    const size_t ld = (size_t)((chunk + 127) / 128 * 128);
     w.cache.theta_all = c.take<float>((size_t)B * g.M_eff);
     w.cache.A_all = c.take<uint16_t>((size_t)B * g.K_pad);
     w.cache.sigT_stride = (size_t)N * ld;
@@ -571,7 +571,7 @@ int nk_sr_solve(const int8_t* sigma, int64_t B, int N, int M, int dtype, const v
             NK_CUDA(launch_theta_tc_pre((const uint8_t*)w.cache.A_all + (size_t)s0 * g.K_pad, nb, g.M_eff, g.K_pad, q.g.Ws, q.g.bg,
                                         w.cache.theta_all + (size_t)s0 * g.M_eff, st));
             NK_CUDA(launch_sigma_T(sigma + s0 * N, nb, N, q.g.ld,
-                                   w.cache.sigT_all + (size_t)(s0 / chunk) * w.cache.sigT_stride, st));
+                                   (uint8_t*)w.cache.sigT_all + (size_t)(s0 / chunk) * w.cache.sigT_stride, st));
         }
     }
     NK_CUDA(launch_cg_dot(w.r, w.r, w.n, w.part, w.scal + 0, st));

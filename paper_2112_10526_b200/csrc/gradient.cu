@@ -8,7 +8,6 @@
 // on three fixed-point bf16 grids (as W is in theta_tc.cu; sigma = +-1 is exact), written k-contiguous (k = sample),
 // and contracted with sigma^T by the same tcgen05 kernel, accumulating [N][M_eff] in fp32 across chunks.
 // g_a and g_b are fp64 column sums with a fixed order (bit-reproducible).
-#include <cuda_bf16.h>
 
 #include "nk_internal.h"
 
@@ -119,16 +118,19 @@ __global__ void grad_slab_reduce_kernel(const double* __restrict__ part, int n_s
     acc[c] = a;
 }
 
-// TwT[piece][me][s] (bf16, k-contiguous, leading dimension ld) from v[s][me]: fixed-point split on the grids
-// 2^e1, 2^(e1-8), 2^(e1-16), 2^(e1+8) > max|v|; rows s in [nb, k_len) are zero
+// TwT[digit][me][s] (int8, k-contiguous, leading dimension ld bytes) from v[s][me]: rint(v / q) = d2 2^16 + d1 2^8 + d0
+// with balanced base-256 digits and q a power of two tied to max|v| (the split of theta_tc.cu's split_w_i8_kernel);
+// rows s in [nb, k_len) are zero; the scale q goes behind the three planes (byte offset 3 M_eff ld)
 __global__ void grad_split_T_kernel(const float* __restrict__ v, int64_t nb, int k_len, int M_eff, int ld,
-                                    const unsigned* __restrict__ absmax_bits, __nv_bfloat16* __restrict__ TwT) {
+                                    const unsigned* __restrict__ absmax_bits, int8_t* __restrict__ TwT) {
     __shared__ float tile[32][33];
     const float vmax = __uint_as_float(*absmax_bits);
     int ex = -100;
-    if (vmax > 0.f) frexpf(vmax, &ex);
-    const float q1 = ldexpf(1.f, ex - 8), q2 = ldexpf(1.f, ex - 16), q3 = ldexpf(1.f, ex - 24);
-    const float s1 = ldexpf(1.f, 8 - ex), s2 = ldexpf(1.f, 16 - ex), s3 = ldexpf(1.f, 24 - ex);
+    if (vmax > 0.f) {
+        frexpf(vmax, &ex);
+        if (ldexpf(vmax, 23 - ex) > 8355000.f) ++ex;      // keep the top digit inside [-128, 127]
+    }
+    const float sc = ldexpf(1.f, 23 - ex);
     const int s0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
         const int64_t s = s0 + r;
@@ -139,22 +141,22 @@ __global__ void grad_split_T_kernel(const float* __restrict__ v, int64_t nb, int
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
         const int me = m0 + r, s = s0 + threadIdx.x;
         if (s >= k_len) continue;
-        float w = tile[threadIdx.x][r];
-        const float hi = rintf(w * s1) * q1;
-        w -= hi;
-        const float mid = rintf(w * s2) * q2;
-        w -= mid;
-        const float lo = rintf(w * s3) * q3;
+        const int I = (int)rintf(tile[threadIdx.x][r] * sc);
+        const int d0 = ((I + 128) & 255) - 128;
+        const int I1 = (I - d0) >> 8;
+        const int d1 = ((I1 + 128) & 255) - 128;
         const size_t o = (size_t)me * ld + s;
-        TwT[o] = __float2bfloat16_rn(hi);
-        TwT[plane + o] = __float2bfloat16_rn(mid);
-        TwT[2 * plane + o] = __float2bfloat16_rn(lo);
+        TwT[o] = (int8_t)((I1 - d1) >> 8);
+        TwT[plane + o] = (int8_t)d1;
+        TwT[2 * plane + o] = (int8_t)d0;
     }
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && threadIdx.y == 0)
+        *reinterpret_cast<float*>(TwT + 3 * plane) = ldexpf(1.f, ex - 23);
 }
 
-// sigT[k][s] = (bf16) sigma[s][k], zero for s in [nb, k_len)
+// sigT[k][s] = sigma[s][k] (int8), zero for s in [nb, k_len)
 __global__ void grad_sigma_T_kernel(const int8_t* __restrict__ sigma, int64_t nb, int k_len, int N, int ld,
-                                    __nv_bfloat16* __restrict__ sigT) {
+                                    int8_t* __restrict__ sigT) {
     __shared__ int8_t tile[32][33];
     const int s0 = blockIdx.x * 32, k0 = blockIdx.y * 32;
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
@@ -165,7 +167,7 @@ __global__ void grad_sigma_T_kernel(const int8_t* __restrict__ sigma, int64_t nb
     __syncthreads();
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
         const int k = k0 + r, s = s0 + threadIdx.x;
-        if (k < N && s < k_len) sigT[(size_t)k * ld + s] = __float2bfloat16_rn((float)tile[threadIdx.x][r]);
+        if (k < N && s < k_len) sigT[(size_t)k * ld + s] = tile[threadIdx.x][r];
     }
 }
 
@@ -213,7 +215,7 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
     if (nb <= 0) return cudaSuccess;
     const bool cplx = dtype == NK_C64;
     const double inv_B = 1.0 / (double)B_total;
-    const int k_len = (int)((nb + 63) / 64 * 64);
+    const int k_len = (int)((nb + 127) / 128 * 128);
     cudaError_t e = cudaMemsetAsync(w.absmax, 0, sizeof(unsigned), st);
     if (e != cudaSuccess) return e;
     dim3 gtv((g.M_pad + 255) / 256, (unsigned)(nb < 1184 ? nb : 1184));
@@ -230,10 +232,10 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
                                                                             inv_B, cplx, (double)real_scale, w.part);
     grad_slab_reduce_kernel<<<(2 * g.N + 127) / 128, 128, 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk);
     grad_split_T_kernel<<<dim3(k_len / 32, g.M_eff / 32), dim3(32, 8), 0, st>>>(
-        w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (__nv_bfloat16*)w.TwT);
+        w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (int8_t*)w.TwT);
     if (sigT_ready == nullptr)
         grad_sigma_T_kernel<<<dim3(k_len / 32, (g.N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, g.N, w.ld,
-                                                                                     (__nv_bfloat16*)w.sigT);
+                                                                                     (int8_t*)w.sigT);
     count_launch(sigT_ready ? 6 : 7);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -241,11 +243,10 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
                                  first_chunk ? 0 : 1, st);
 }
 
-// sigT[k][s] = (bf16) sigma[s][k] for one chunk (what launch_gradient_chunk builds itself unless given sigT_ready)
+// sigT[k][s] = sigma[s][k] (int8, zero padded to a multiple of 128 samples) for one chunk (what launch_gradient_chunk builds itself unless given sigT_ready)
 cudaError_t launch_sigma_T(const int8_t* sigma, int64_t nb, int N, int ld, void* sigT, cudaStream_t st) {
-    const int k_len = (int)((nb + 63) / 64 * 64);
-    grad_sigma_T_kernel<<<dim3(k_len / 32, (N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, N, ld,
-                                                                               (__nv_bfloat16*)sigT);
+    const int k_len = (int)((nb + 127) / 128 * 128);
+    grad_sigma_T_kernel<<<dim3(k_len / 32, (N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, N, ld, (int8_t*)sigT);
     count_launch();
     return cudaGetLastError();
 }

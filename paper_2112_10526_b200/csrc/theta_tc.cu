@@ -1,26 +1,23 @@
 // Base activations theta = sigma W^T + b on the 5th-generation tensor cores (BASELINE.json
 // north_star (2): "the one place tensor cores are justified").
 //
-// Two instantiations of one kernel:
-//  * theta (I8 = true): int8 operands, tcgen05 kind::i8 (twice the bf16 MMA rate, half the operand bytes), int32
-//    accumulators.  sigma = +-1 IS the A operand (used in place when its rows are a multiple of 128 long).  W (fp32)
-//    becomes three int8 digit planes of a fixed-point number, rint(W / q) = d2 2^16 + d1 2^8 + d0, q a power of two
-//    tied to max|W| (split_w_i8_kernel); every product and every int32 partial sum is exact, each plane has its own
-//    TMEM accumulator, and only the epilogue rounds: theta = q (D2 2^16 + D1 2^8 + D0) + b in fp32.
-//  * the contraction over samples of the force vector / QGT (I8 = false, launch_tc_gemm_pieces): bf16 operands,
-//    kind::f16, fp32 accumulators; the left operand v = conj(tanh theta) w_s is split by the caller on three
-//    fixed-point bf16 grids (|m| <= 256 integers times 2^e1, 2^(e1-8), 2^(e1-16)), exact in bf16 with exact products
-//    and partial sums that are integers below 2^24 quanta — exact whatever rounding the adder uses (measured: with
-//    per-element bf16 splitting the adder's truncation biased the result by ~0.25 ulp, coherently over the terms).
-//    Epilogue: out = (D_hi + (D_mid + D_lo)) in fp32.
+// One kernel, two uses, both with int8 operands on tcgen05 kind::i8 (twice the bf16 MMA rate, half the operand bytes)
+// and int32 accumulators:
+//  * theta: sigma = +-1 IS the A operand (used in place when its rows are a multiple of 128 long).  W (fp32) becomes
+//    three int8 digit planes of a fixed-point number, rint(W / q) = d2 2^16 + d1 2^8 + d0, q a power of two tied to
+//    max|W| (split_w_i8_kernel); every product and every int32 partial sum is exact, each plane has its own TMEM
+//    accumulator, and only the epilogue rounds: theta = q (D2 2^16 + D1 2^8 + D0) + b in fp32.
+//  * the contraction over samples of the force vector / QGT (launch_tc_gemm_pieces): A = the transposed spins, the
+//    digit planes are those of v = conj(tanh theta) w_s, split the same way per chunk by gradient.cu.
+//  History: a bf16 kind::f16 version with three 9-bit fixed-point pieces (27 bits) ran at half the rate with twice
+//  the operand bytes; per-ELEMENT bf16 splitting had been measured to bias the result by ~0.25 ulp through the adder's
+//  truncation — with integer accumulators there is no adder rounding at all.
 //
 // Kernel: one CTA per 128 (rows) x 128 (columns) tile.  Warp 0 = TMA producer (cp.async.bulk.tensor, 128B swizzle,
-// 3-stage ring: per stage the A tile and the three piece tiles of a k block of 128 bytes per row = 128 int8 or 64
-// bf16); warp 1 = TMEM allocator and single-thread tcgen05.mma issuer (M = 128, N = 128, K = 32 int8 / 16 bf16:
-// 12 MMAs per k block, three 128-column accumulators); warps 2-5 = epilogue (tcgen05.ld 32x32b, scale / bias, fp32
-// stores).
+// 3-stage ring: per stage the A tile and the three digit tiles of a k block of 128 int8 per row); warp 1 = TMEM
+// allocator and single-thread tcgen05.mma issuer (M = 128, N = 128, K = 32: 12 MMAs per k block, three 128-column
+// int32 accumulators); warps 2-5 = epilogue (tcgen05.ld 32x32b, scale / bias, fp32 stores).
 #include <cuda.h>
-#include <cuda_bf16.h>
 
 #include "nk_internal.h"
 #include "ptx_helpers.cuh"
@@ -29,15 +26,14 @@ namespace nk {
 
 namespace tc {
 constexpr int BM = 128, BN = 128, BK = 64, STAGES = 3, UMMA_K = 16;
-constexpr int TILE_BYTES = BM * BK * 2;                   // 16 KB: one 128-row x 64-col bf16 tile (A or one W piece)
+constexpr int TILE_BYTES = BM * BK * 2;                   // 16 KB: one tile of 128 rows x 128 B (A or one digit plane)
 constexpr int STAGE_BYTES = 4 * TILE_BYTES;               // sigma + hi + mid + lo
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment*/ + 256 /*barriers*/;
 constexpr int THREADS = 192;
 constexpr uint32_t TMEM_COLS = 512;                       // D_hi [0,128), D_mid [128,256), D_lo [256,384); power of 2
 // instruction descriptor (cute::UMMA::InstrDescriptor bit layout): D=F32, A=B=BF16, K-major both, N=128, M=128
-// kind::i8: D = S32 (c_format 2), A = B = signed 8 bit (format 1), K-major, N and M as for bf16
+// instruction descriptor of kind::i8: D = S32 (c_format 2), A = B = signed 8 bit (format 1), K-major, N >> 3, M >> 4
 constexpr uint32_t IDESC_I8 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
-constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
 }  // namespace tc
 
 // ---- operand preparation ---------------------------------------------------------------------------------
@@ -49,43 +45,6 @@ __global__ void absmax_kernel(const float* __restrict__ Wg, size_t n, unsigned* 
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
     if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
-}
-
-// Ws[piece][me][k] (bf16, K_pad columns, zero padded) from Wg[me][k] (fp32): fixed-point split on the grids
-// 2^e1, 2^(e1-8), 2^(e1-16) with 2^(e1+8) > max|W|
-__global__ void split_w_kernel(const float* __restrict__ Wg, int M_eff, int N, int K_pad,
-                               const unsigned* __restrict__ absmax_bits, __nv_bfloat16* __restrict__ Ws) {
-    const float wmax = __uint_as_float(*absmax_bits);
-    int ex = 0;
-    if (wmax > 0.f) frexpf(wmax, &ex);                    // wmax = f 2^ex, f in [0.5, 1)
-    else ex = -100;
-    const float q1 = ldexpf(1.f, ex - 8), q2 = ldexpf(1.f, ex - 16), q3 = ldexpf(1.f, ex - 24);
-    const float s1 = ldexpf(1.f, 8 - ex), s2 = ldexpf(1.f, 16 - ex), s3 = ldexpf(1.f, 24 - ex);
-    const int me = blockIdx.y;
-    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < K_pad; k += gridDim.x * blockDim.x) {
-        float w = (k < N) ? Wg[(size_t)me * N + k] : 0.f;
-        const float hi = rintf(w * s1) * q1;
-        w -= hi;                                          // exact
-        const float mid = rintf(w * s2) * q2;
-        w -= mid;                                         // exact
-        const float lo = rintf(w * s3) * q3;
-        const size_t o = (size_t)me * K_pad + k, plane = (size_t)M_eff * K_pad;
-        Ws[o] = __float2bfloat16_rn(hi);                  // |m| <= 256: exact in bf16
-        Ws[plane + o] = __float2bfloat16_rn(mid);
-        Ws[2 * plane + o] = __float2bfloat16_rn(lo);
-    }
-}
-
-// A[s][k] = (bf16) sigma[s][k], zero padded to K_pad
-__global__ void sigma_bf16_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int K_pad,
-                                  __nv_bfloat16* __restrict__ A) {
-    const int64_t total = B * K_pad;
-    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
-         idx += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t s = idx / K_pad;
-        const int k = (int)(idx - s * K_pad);
-        A[idx] = __float2bfloat16_rn(k < N ? (float)sigma[s * N + k] : 0.f);
-    }
 }
 
 // ---- int8 operands of the theta contraction (tcgen05 kind::i8: twice the bf16 MMA rate, half the operand bytes) ----
@@ -151,16 +110,6 @@ __device__ __forceinline__ uint64_t make_sdesc(uint32_t smem_addr) {
     d |= (uint64_t)2 << 61;
     return d;
 }
-__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
-                                          uint32_t accumulate) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
-        "}\n" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
 __device__ __forceinline__ void umma_i8(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
                                         uint32_t accumulate) {
     asm volatile(
@@ -189,10 +138,8 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
 }
 
 // ---- the GEMM ---------------------------------------------------------------------------------------------
-// I8 = false: bf16 operands (BK = 64 elements per 128-B swizzle row), fp32 accumulators, out = hi + mid + lo.
-// I8 = true:  int8 operands (BK = 128 elements per row, so K_pad / 128 k blocks), int32 accumulators,
-//             out = q (hi 2^16 + mid 2^8 + lo) with the scale q read from `scale`.
-template <bool I8>
+// int8 operands (128 elements per 128-B swizzle row, so K_pad / 128 k blocks), int32 accumulators,
+// out (+)= q (D2 2^16 + D1 2^8 + D0) + bias with the scale q read from `scale`.
 __global__ void __launch_bounds__(tc::THREADS, 1)
 theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w, int64_t B,
                 int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta, int accumulate,
@@ -208,7 +155,7 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n0 = blockIdx.x * BN;                       // hidden-unit tile
     const int64_t m0 = (int64_t)blockIdx.y * BM;          // sample tile
-    constexpr int BKE = I8 ? 2 * BK : BK;                 // elements per k block (128 B per row either way)
+    constexpr int BKE = 2 * BK;                           // int8 elements per k block (128 B per row)
     const int n_kb = K_pad / BKE;
 
     if (threadIdx.x == 0) {
@@ -254,15 +201,10 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                     const uint32_t koff = k * UMMA_K * 2;                       // bytes inside the 128 B swizzle row
                     const uint64_t ad = make_sdesc(a_addr + koff);
                     const uint32_t first = (kb | k) ? 1u : 0u;
-                    if constexpr (I8) {                                         // 32 B = 32 int8 = one K = 32 MMA
-                        umma_i8(tmem_base + 0, ad, make_sdesc(a_addr + 1 * TILE_BYTES + koff), IDESC_I8, first);
-                        umma_i8(tmem_base + BN, ad, make_sdesc(a_addr + 2 * TILE_BYTES + koff), IDESC_I8, first);
-                        umma_i8(tmem_base + 2 * BN, ad, make_sdesc(a_addr + 3 * TILE_BYTES + koff), IDESC_I8, first);
-                    } else {
-                        umma_bf16(tmem_base + 0, ad, make_sdesc(a_addr + 1 * TILE_BYTES + koff), IDESC, first);
-                        umma_bf16(tmem_base + BN, ad, make_sdesc(a_addr + 2 * TILE_BYTES + koff), IDESC, first);
-                        umma_bf16(tmem_base + 2 * BN, ad, make_sdesc(a_addr + 3 * TILE_BYTES + koff), IDESC, first);
-                    }
+                    // 32 B = 32 int8 = one K = 32 MMA per digit plane
+                    umma_i8(tmem_base + 0, ad, make_sdesc(a_addr + 1 * TILE_BYTES + koff), IDESC_I8, first);
+                    umma_i8(tmem_base + BN, ad, make_sdesc(a_addr + 2 * TILE_BYTES + koff), IDESC_I8, first);
+                    umma_i8(tmem_base + 2 * BN, ad, make_sdesc(a_addr + 3 * TILE_BYTES + koff), IDESC_I8, first);
                 }
                 umma_commit(empty0 + 8 * stage);          // frees the smem stage when these MMAs have read it
                 if (++stage == STAGES) { stage = 0; parity ^= 1; }
@@ -276,7 +218,7 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const int64_t row = m0 + q * 32 + lane;
         float* out = theta + row * M_eff + n0;
-        const float qs = I8 ? *scale : 1.f;
+        const float qs = *scale;
 #pragma unroll 1
         for (int c0 = 0; c0 < BN; c0 += 32) {
             float hi[32], mid[32], lo[32];
@@ -295,20 +237,13 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                         bb.x += old.x; bb.y += old.y; bb.z += old.z; bb.w += old.w;
                     }
                     float4 o;
-                    if constexpr (I8) {
-                        auto comb = [&](int jj) -> float {                      // exact ints below 2^24 each
-                            const float h = (float)__float_as_int(hi[jj]), m = (float)__float_as_int(mid[jj]),
-                                        l = (float)__float_as_int(lo[jj]);
-                            return fmaf(h, 65536.f, fmaf(m, 256.f, l));
-                        };
-                        o.x = fmaf(qs, comb(j), bb.x); o.y = fmaf(qs, comb(j + 1), bb.y);
-                        o.z = fmaf(qs, comb(j + 2), bb.z); o.w = fmaf(qs, comb(j + 3), bb.w);
-                    } else {
-                        o.x = (hi[j] + (mid[j] + lo[j])) + bb.x;
-                        o.y = (hi[j + 1] + (mid[j + 1] + lo[j + 1])) + bb.y;
-                        o.z = (hi[j + 2] + (mid[j + 2] + lo[j + 2])) + bb.z;
-                        o.w = (hi[j + 3] + (mid[j + 3] + lo[j + 3])) + bb.w;
-                    }
+                    auto comb = [&](int jj) -> float {                          // exact ints below 2^24 each
+                        const float h = (float)__float_as_int(hi[jj]), m = (float)__float_as_int(mid[jj]),
+                                    l = (float)__float_as_int(lo[jj]);
+                        return fmaf(h, 65536.f, fmaf(m, 256.f, l));
+                    };
+                    o.x = fmaf(qs, comb(j), bb.x); o.y = fmaf(qs, comb(j + 1), bb.y);
+                    o.z = fmaf(qs, comb(j + 2), bb.z); o.w = fmaf(qs, comb(j + 3), bb.w);
                     *reinterpret_cast<float4*>(out + c0 + j) = o;
                 }
             }
@@ -337,23 +272,20 @@ cudaError_t theta_tc_init() {
     if (e != cudaSuccess) return e;
     if (qres != cudaDriverEntryPointSuccess || fn == nullptr) return cudaErrorNotSupported;
     g_encode = (EncodeTiledFn)fn;
-    e = cudaFuncSetAttribute((const void*)theta_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             tc::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute((const void*)theta_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    e = cudaFuncSetAttribute((const void*)theta_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              tc::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     g_tc_ready = true;
     return cudaSuccess;
 }
 
-// 2-D tensor map over a k-contiguous [rows][cols] operand, box = 128 rows x 128 B (64 bf16 or 128 int8), 128B swizzle
-static bool encode_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols, bool i8 = false) {
+// 2-D tensor map over a k-contiguous int8 [rows][cols] operand, box = 128 rows x 128 B, 128B swizzle
+static bool encode_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols) {
     const cuuint64_t dims[2] = {cols, rows};
-    const cuuint64_t strides[1] = {cols * (i8 ? 1u : 2u)};
-    const cuuint32_t box[2] = {(cuuint32_t)(i8 ? 2 * tc::BK : tc::BK), (cuuint32_t)tc::BM};
+    const cuuint64_t strides[1] = {cols};
+    const cuuint32_t box[2] = {(cuuint32_t)(2 * tc::BK), (cuuint32_t)tc::BM};
     const cuuint32_t estr[2] = {1, 1};
-    return g_encode(map, i8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
+    return g_encode(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
                     const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                     CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
@@ -393,11 +325,11 @@ cudaError_t launch_theta_tc_pre(const void* A, int64_t B, int M_eff, int K_pad, 
     cudaError_t e = theta_tc_init();
     if (e != cudaSuccess) return e;
     CUtensorMap map_a, map_w;
-    if (!encode_2d(&map_a, A, (uint64_t)B, (uint64_t)K_pad, true)) return cudaErrorInvalidValue;
-    if (!encode_2d(&map_w, Ws, (uint64_t)3 * M_eff, (uint64_t)K_pad, true)) return cudaErrorInvalidValue;
+    if (!encode_2d(&map_a, A, (uint64_t)B, (uint64_t)K_pad)) return cudaErrorInvalidValue;
+    if (!encode_2d(&map_w, Ws, (uint64_t)3 * M_eff, (uint64_t)K_pad)) return cudaErrorInvalidValue;
     const float* scale = reinterpret_cast<const float*>((const int8_t*)Ws + (size_t)3 * M_eff * K_pad);
     dim3 grid(M_eff / tc::BN, (unsigned)((B + tc::BM - 1) / tc::BM));
-    theta_tc_kernel<true><<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_w, B, M_eff, K_pad, bg, theta, 0, scale);
+    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_w, B, M_eff, K_pad, bg, theta, 0, scale);
     count_launch();
     return cudaGetLastError();
 }
@@ -412,8 +344,9 @@ cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, in
     return launch_theta_tc_pre(A, B, M_eff, K_pad, Ws, bg, theta, st);
 }
 
-// Generic entry used by the gradient: out[r][c] (+)= sum_k A[r][k] * (P0 + P1 + P2)[c][k], A bf16 [rows][ld] and
-// P bf16 [3][cols][ld] both k-contiguous, k < k_len (a multiple of 64), cols a multiple of 128.
+// Generic entry used by the gradient / QGT contraction over samples: out[r][c] (+)= q sum_k A[r][k] I[c][k] with A an
+// int8 [rows][ld] operand (the transposed spins) and P the three int8 digit planes [3][cols][ld] + scale q of
+// I = rint(v / q) (grad_split_T_kernel); k < k_len (a multiple of 128), cols a multiple of 128.
 cudaError_t launch_tc_gemm_pieces(const void* A, int64_t rows, const void* P, int cols, int ld, int k_len, float* out,
                                   int accumulate, cudaStream_t st) {
     if (rows <= 0) return cudaSuccess;
@@ -422,9 +355,10 @@ cudaError_t launch_tc_gemm_pieces(const void* A, int64_t rows, const void* P, in
     CUtensorMap map_a, map_p;
     if (!encode_2d(&map_a, A, (uint64_t)rows, (uint64_t)ld)) return cudaErrorInvalidValue;
     if (!encode_2d(&map_p, P, (uint64_t)3 * cols, (uint64_t)ld)) return cudaErrorInvalidValue;
+    const float* scale = reinterpret_cast<const float*>((const int8_t*)P + (size_t)3 * cols * ld);
     dim3 grid(cols / tc::BN, (unsigned)((rows + tc::BM - 1) / tc::BM));
-    theta_tc_kernel<false><<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_p, rows, cols, k_len, nullptr, out,
-                                                                      accumulate, nullptr);
+    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_p, rows, cols, k_len, nullptr, out,
+                                                                     accumulate, scale);
     count_launch();
     return cudaGetLastError();
 }
