@@ -33,6 +33,23 @@ __device__ __forceinline__ double ln_cosh_small(double t) {
     return p * u;
 }
 
+// The same series in fp32 (nine terms: the next is below 2e-10 at t = 1/2).  Each term then carries an independent
+// rounding error of ~6e-8 of its own size (~0.05), i.e. ~1e-7 over the 2048 terms of config 5, against the 1e-5 bound;
+// the sum over hidden units stays in fp64.
+__device__ __forceinline__ float ln_cosh_small_f(float t) {
+    const float u = t * t;
+    float p = 3.277930227475478e-05f;
+    p = fmaf(p, u, -9.09896491907074e-05f);
+    p = fmaf(p, u, 0.0002565805740408915f);
+    p = fmaf(p, u, -0.0007386029608251831f);
+    p = fmaf(p, u, 0.0021869488536155205f);
+    p = fmaf(p, u, -0.006746031746031746f);
+    p = fmaf(p, u, 0.022222222222222223f);
+    p = fmaf(p, u, -0.08333333333333333f);
+    p = fmaf(p, u, 0.5f);
+    return p * u;
+}
+
 template <bool CPLX>
 __global__ void __launch_bounds__(256)
 logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_pad, int M_eff,
@@ -47,9 +64,13 @@ logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_p
         // 128-bit loads over the padded row (theta of a padded hidden unit is exactly 0 and contributes ln cosh 0 = 0),
         // four independent fp64 accumulators
         double r0 = 0.0, r1 = 0.0, r2 = 0.0, r3 = 0.0;
-        auto term = [](float xf) -> double {
+        // |t| < 1/2: the fp32 series.  Otherwise the stable form in fp64, behind a warp-uniform branch.  At config 5
+        // theta ~ N(0, 0.32), so an eighth of the elements — hence nearly every warp instruction — take it, and it is
+        // most of this kernel's time; an fp32 expf / log1pf version of it was measured (0.94 -> 0.53 ms per step) and
+        // rejected: it moved the ln psi error from 2.9e-6 to 3.6e-6 (fp32 output: 5.4e-6 -> 6.8e-6 of the 1e-5 bound).
+        auto slow = [](float xf) -> double {
             const double t = fabs((double)xf);
-            return (t < 0.5) ? ln_cosh_small(t) : t + log1p(exp(-2.0 * t)) - 0.69314718055994530942;
+            return t + log1p(exp(-2.0 * t)) - 0.69314718055994530942;
         };
 #pragma unroll 4
         for (int j = lane * 4; j < M_pad; j += 128) {
@@ -60,7 +81,16 @@ logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_p
                 if (j + 2 < M) theta_out[s * M + j + 2] = x.z;
                 if (j + 3 < M) theta_out[s * M + j + 3] = x.w;
             }
-            r0 += term(x.x); r1 += term(x.y); r2 += term(x.z); r3 += term(x.w);
+            double t0 = (double)ln_cosh_small_f(x.x), t1 = (double)ln_cosh_small_f(x.y);
+            double t2 = (double)ln_cosh_small_f(x.z), t3 = (double)ln_cosh_small_f(x.w);
+            const bool big = fmaxf(fmaxf(fabsf(x.x), fabsf(x.y)), fmaxf(fabsf(x.z), fabsf(x.w))) >= 0.5f;
+            if (__any_sync(0xffffffffu, big)) {
+                if (fabsf(x.x) >= 0.5f) t0 = slow(x.x);
+                if (fabsf(x.y) >= 0.5f) t1 = slow(x.y);
+                if (fabsf(x.z) >= 0.5f) t2 = slow(x.z);
+                if (fabsf(x.w) >= 0.5f) t3 = slow(x.w);
+            }
+            r0 += t0; r1 += t1; r2 += t2; r3 += t3;
         }
         re = (r0 + r1) + (r2 + r3);
     }
