@@ -185,6 +185,9 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
     n_cg = 8
     ms_sr = _time_ms(torch, lambda: nk.sr_solve(chains, W, b, ga, gb, gW, diag_shift=0.01, tol=0.0, max_iter=n_cg,
                                                 chunk_size=p.chunk_size, ws=sws), 2)
+    # the graded step replayed from a CUDA graph (LocalEnergyPlan.run_graph): what launch overhead costs the small configs
+    plan.run_graph(sigma, W, a, b)
+    ms_graph = _time_ms(torch, lambda: plan.run_graph(sigma, W, a, b), 5)
     planes = 2 if p.complex_params else 1
     # product-form variant of the same step (nk_local_energy_ex, NK_FORM_PRODUCT), fused kernel timed by the library
     pplan = nk.LocalEnergyPlan(op, B, N, M, dt_code, p.chunk_size, device=sigma.device, flags=nk.NK_FORM_PRODUCT)
@@ -197,6 +200,8 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
     nk.profile_enable(False)
     fused_prod_ms = ph["fused"][0] / 4                      # _time_ms runs the call 1 + 3 times
     return {
+        "cuda_graph": {"ms_per_step": ms_graph, "local_energies_per_sec": B / (ms_graph * 1e-3),
+                       "what": "the same nk_local_energy step replayed from a captured CUDA graph, no L2 flush"},
         "product_form": {"ms_per_step": ms_prod, "local_energies_per_sec": B / (ms_prod * 1e-3),
                          "fused_ms_per_step": fused_prod_ms,
                          "roofline": {"bound": "smem", "kernel": "fused_eloc_kernel<V, CPLX, PROD=true>",

@@ -220,6 +220,23 @@ class LocalEnergyPlan:
         _check(rc, "nk_local_energy_ex")
         return self.eloc, self.logpsi, self.stats
 
+    def run_graph(self, sigma, W, a, b):
+        """The same call replayed from a CUDA graph: the first use with a given set of tensors runs once eagerly (one-
+        time attribute / tensor-map setup), captures the call's launches on torch's capture stream and keeps the graph;
+        later uses replay it — one launch instead of ~11 per chunk-less call, which is what bounds the small configs.
+        The tensors must stay alive and keep their addresses; their CONTENTS may change between replays."""
+        torch = _torch()
+        key = tuple(_ptr(t) for t in (sigma, W, a, b))
+        if getattr(self, "_graph_key", None) != key:
+            self.run(sigma, W, a, b)
+            torch.cuda.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                self.run(sigma, W, a, b)
+            self._graph, self._graph_key = graph, key
+        self._graph.replay()
+        return self.eloc, self.logpsi, self.stats
+
 
 def local_energy(op: Operator, sigma, W, a=None, b=None, *, chunk_size: int = 0, want_logpsi: bool = True,
                  flags: int = 0):

@@ -297,3 +297,23 @@ def test_theta_fixed_point_split_at_the_top_of_a_binade(nk):
     th_ref = orc.rbm_theta(p.sigma, W, p.b)
     assert np.abs(theta.cpu().numpy() - th_ref).max() < 2e-6           # an overflowed digit would be an error of order 1
     assert_logpsi(lp.cpu().numpy(), orc.rbm_logpsi(p.sigma, W, p.a, p.b))
+
+
+def test_cuda_graph_replay_matches_the_eager_call(nk):
+    """LocalEnergyPlan.run_graph: the captured call replays bit-identically, and follows changed CONTENTS of the same
+    tensors (new parameters, new samples) as a VMC loop needs."""
+    p = inp.make_config(2, n_samples=512)
+    op = nk.Operator.from_problem(p)
+    sig, W, a, b = dev(p.sigma), dev(p.W), dev(p.a), dev(p.b)
+    plan = nk.LocalEnergyPlan(op, 512, p.n_sites, p.n_hidden, nk.NK_F32, 128)
+    e0 = [t.clone() for t in plan.run(sig, W, a, b)]
+    e1 = [t.clone() for t in plan.run_graph(sig, W, a, b)]
+    e2 = [t.clone() for t in plan.run_graph(sig, W, a, b)]
+    torch.cuda.synchronize()
+    assert all(torch.equal(x, y) and torch.equal(x, z) for x, y, z in zip(e0, e1, e2))
+    W.mul_(1.5); sig.copy_(dev(p.sigma[::-1].copy()))
+    g = [t.clone() for t in plan.run_graph(sig, W, a, b)]
+    r = [t.clone() for t in plan.run(sig, W, a, b)]
+    torch.cuda.synchronize()
+    assert all(torch.equal(x, y) for x, y in zip(g, r)) and not torch.equal(g[0], e0[0])
+    op.close()
