@@ -87,3 +87,26 @@ def test_random_shapes_sampler_gradient_qgt(nk, seed):
     dw = np.abs(w - w.mean()).max()
     for g, r in zip(out, ref):
         assert np.abs(g.cpu().numpy().astype(r.dtype) - r).max() <= 2e-6 * dw + 4e-7 * np.abs(r).max() + 1e-12
+
+
+@pytest.mark.parametrize("M,cplx", [(1700, False), (1800, False), (1500, False), (900, True), (800, True)])
+def test_wide_rbm_variants(nk, M, cplx):
+    """Widths whose kernels are separate template instances (V = 12 ... 16 real, 7 ... 8 complex): the staged-row sampler
+    (rows >= 7 KB), the direct one just below, and both local-energy forms."""
+    from oracle import nk_sampler_oracle as smp
+    from test_gpu_sampler import assert_chains
+    p = inp.make_problem(inp.KIND_HEISENBERG, "chain", 12, M, 20, seed=M, complex_params=cplx, scale=0.01)
+    e_ref, lp_ref = run_oracle(p)
+    op = nk.Operator.from_problem(p)
+    sig, W, a, b = dev(p.sigma), dev(p.W), dev(p.a), dev(p.b)
+    for flags in (0, nk.NK_FORM_PRODUCT):
+        e, lp, _ = nk.local_energy(op, sig, W, a, b, flags=flags)
+        assert_eloc(e.cpu().numpy(), e_ref)
+        assert_logpsi(lp.cpu().numpy(), lp_ref)
+    for rule, clusters in ((nk.NK_RULE_LOCAL, None), (nk.NK_RULE_EXCHANGE, p.bonds)):
+        s = sig.clone()
+        acc = nk.metropolis_sample(s, W, a, b, rule=rule, clusters=clusters, n_steps=45, seed=3)
+        torch.cuda.synchronize()
+        ref, racc, margin, _ = smp.metropolis(rule, p.sigma, p.W, p.a, p.b, 45, 3, clusters=clusters)
+        assert_chains(p, rule, s.cpu().numpy(), acc.cpu().numpy(), ref, racc, margin, min_clear=0.5)
+    op.close()
