@@ -50,6 +50,8 @@ __device__ __forceinline__ float ln_cosh_small_f(float t) {
     return p * u;
 }
 
+constexpr int LOGPSI_WARPS_REAL = 4;      // warps per block of the real kernel: 4 x 8 KB of compaction lists
+
 template <bool CPLX>
 __global__ void __launch_bounds__(256)
 logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_pad, int M_eff,
@@ -64,13 +66,24 @@ logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_p
         // 128-bit loads over the padded row (theta of a padded hidden unit is exactly 0 and contributes ln cosh 0 = 0),
         // four independent fp64 accumulators
         double r0 = 0.0, r1 = 0.0, r2 = 0.0, r3 = 0.0;
-        // |t| < 1/2: the fp32 series.  Otherwise the stable form in fp64, behind a warp-uniform branch.  At config 5
-        // theta ~ N(0, 0.32), so an eighth of the elements — hence nearly every warp instruction — take it, and it is
-        // most of this kernel's time; an fp32 expf / log1pf version of it was measured (0.94 -> 0.53 ms per step) and
-        // rejected: it moved the ln psi error from 2.9e-6 to 3.6e-6 (fp32 output: 5.4e-6 -> 6.8e-6 of the 1e-5 bound).
-        auto slow = [](float xf) -> double {
-            const double t = fabs((double)xf);
-            return t + log1p(exp(-2.0 * t)) - 0.69314718055994530942;
+        // |t| < 1/2: the fp32 series, in place.  Larger arguments need the stable form in fp64 (exp + log1p: ~30 DFMA
+        // each).  At config 5 theta ~ N(0, 0.32): an eighth of the elements, spread over every warp instruction, so a
+        // branch per element made every warp pay the slow path 64 times per sample.  Instead the large arguments are
+        // compacted into a per-warp list in shared memory (ballot + popc) and evaluated densely afterwards: ~8 slow
+        // evaluations per lane and sample instead of 64, same fp64 formula.  (An fp32 expf / log1pf slow path was also
+        // measured, 0.94 -> 0.53 ms per step, and rejected: ln psi error 2.9e-6 -> 3.6e-6.)
+        __shared__ float big_list[LOGPSI_WARPS_REAL][MAX_V_REAL * MPAD_ALIGN];
+        float* big = big_list[threadIdx.x >> 5];
+        int n_big = 0;
+        const unsigned lt = (1u << lane) - 1u;
+        auto take = [&](float x) -> double {
+            const bool is_big = fabsf(x) >= 0.5f;
+            const unsigned m = __ballot_sync(0xffffffffu, is_big);
+            if (m) {
+                if (is_big) big[n_big + __popc(m & lt)] = x;
+                n_big += __popc(m);
+            }
+            return is_big ? 0.0 : (double)ln_cosh_small_f(x);
         };
 #pragma unroll 4
         for (int j = lane * 4; j < M_pad; j += 128) {
@@ -81,16 +94,12 @@ logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_p
                 if (j + 2 < M) theta_out[s * M + j + 2] = x.z;
                 if (j + 3 < M) theta_out[s * M + j + 3] = x.w;
             }
-            double t0 = (double)ln_cosh_small_f(x.x), t1 = (double)ln_cosh_small_f(x.y);
-            double t2 = (double)ln_cosh_small_f(x.z), t3 = (double)ln_cosh_small_f(x.w);
-            const bool big = fmaxf(fmaxf(fabsf(x.x), fabsf(x.y)), fmaxf(fabsf(x.z), fabsf(x.w))) >= 0.5f;
-            if (__any_sync(0xffffffffu, big)) {
-                if (fabsf(x.x) >= 0.5f) t0 = slow(x.x);
-                if (fabsf(x.y) >= 0.5f) t1 = slow(x.y);
-                if (fabsf(x.z) >= 0.5f) t2 = slow(x.z);
-                if (fabsf(x.w) >= 0.5f) t3 = slow(x.w);
-            }
-            r0 += t0; r1 += t1; r2 += t2; r3 += t3;
+            r0 += take(x.x); r1 += take(x.y); r2 += take(x.z); r3 += take(x.w);
+        }
+        __syncwarp();
+        for (int k = lane; k < n_big; k += 32) {
+            const double t = fabs((double)big[k]);
+            r0 += t + log1p(exp(-2.0 * t)) - 0.69314718055994530942;
         }
         re = (r0 + r1) + (r2 + r3);
     }
@@ -137,7 +146,7 @@ logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_p
 cudaError_t launch_logpsi(const int8_t* sigma, int64_t B, const Geometry& g, int dtype, const float* theta,
                           const void* a, void* logpsi_out, bool out_f64, void* theta_out, cudaStream_t st) {
     if (B <= 0) return cudaSuccess;
-    const int wpb = 8;
+    const int wpb = dtype == NK_C64 ? 8 : LOGPSI_WARPS_REAL;
     const unsigned grid = (unsigned)((B + wpb - 1) / wpb);
     if (dtype == NK_C64)
         logpsi_kernel<true><<<grid, wpb * 32, 0, st>>>(sigma, B, g.N, g.M, g.M_pad, g.M_eff, theta, (const float*)a,
