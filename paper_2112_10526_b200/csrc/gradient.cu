@@ -87,22 +87,29 @@ __global__ void grad_colsum_partial_kernel(const float* __restrict__ v, int64_t 
     part[(size_t)blockIdx.y * M_eff + me] = acc;
 }
 
-// part[slab][plane * N + k] = sum_{s in slab} sigma[s][k] w_s[plane]   (x2 for real parameters)
+// part[slab][plane * N + k] = sum_{s in slab} sigma[s][k] w_s[plane]   (x2 for real parameters); blockDim.x == GRAD_SLAB:
+// thread t first forms the weight of sample s0 + t once for the whole block
 __global__ void grad_a_partial_kernel(const int8_t* __restrict__ sigma, int64_t nb, int N,
                                       const float* __restrict__ eloc, const double* __restrict__ stats, double inv_B,
                                       int cplx, double real_scale, double* __restrict__ part) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= N) return;
+    __shared__ double wr_s[GRAD_SLAB], wi_s[GRAD_SLAB];
     const int64_t s0 = (int64_t)blockIdx.y * GRAD_SLAB;
     const int64_t s1 = (s0 + GRAD_SLAB < nb) ? s0 + GRAD_SLAB : nb;
-    const double f = cplx ? 1.0 : real_scale;
+    {
+        float wr = 0.f, wi = 0.f;
+        if (s0 + threadIdx.x < s1) sample_weight(eloc, stats, s0 + threadIdx.x, inv_B, cplx != 0, wr, wi);
+        wr_s[threadIdx.x] = (cplx ? 1.0 : real_scale) * (double)wr;
+        wi_s[threadIdx.x] = (double)wi;
+    }
+    __syncthreads();
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
     double ar = 0.0, ai = 0.0;
-    for (int64_t s = s0; s < s1; ++s) {
-        float wr, wi;
-        sample_weight(eloc, stats, s, inv_B, cplx != 0, wr, wi);
-        const double sg = (double)sigma[s * N + k];
-        ar += f * sg * (double)wr;
-        ai += sg * (double)wi;
+    const int n = (int)(s1 - s0);
+    for (int t = 0; t < n; ++t) {
+        const double sg = (double)sigma[(s0 + t) * N + k];
+        ar += sg * wr_s[t];
+        ai += sg * wi_s[t];
     }
     part[(size_t)blockIdx.y * 2 * N + k] = ar;
     part[(size_t)blockIdx.y * 2 * N + N + k] = ai;
