@@ -91,7 +91,8 @@ __global__ void grad_colsum_partial_kernel(const float* __restrict__ v, int64_t 
 // thread t first forms the weight of sample s0 + t once for the whole block
 __global__ void grad_a_partial_kernel(const int8_t* __restrict__ sigma, int64_t nb, int N,
                                       const float* __restrict__ eloc, const double* __restrict__ stats, double inv_B,
-                                      int cplx, double real_scale, double* __restrict__ part) {
+                                      int cplx, double real_scale, double* __restrict__ part,
+                                      unsigned* __restrict__ wmax_bits) {
     __shared__ double wr_s[GRAD_SLAB], wi_s[GRAD_SLAB];
     const int64_t s0 = (int64_t)blockIdx.y * GRAD_SLAB;
     const int64_t s1 = (s0 + GRAD_SLAB < nb) ? s0 + GRAD_SLAB : nb;
@@ -100,6 +101,12 @@ __global__ void grad_a_partial_kernel(const int8_t* __restrict__ sigma, int64_t 
         if (s0 + threadIdx.x < s1) sample_weight(eloc, stats, s0 + threadIdx.x, inv_B, cplx != 0, wr, wi);
         wr_s[threadIdx.x] = (cplx ? 1.0 : real_scale) * (double)wr;
         wi_s[threadIdx.x] = (double)wi;
+        if (wmax_bits != nullptr && blockIdx.x == 0) {        // max_s |real_scale w_s| >= max |v_sj| since |tanh| <= 1
+            unsigned m = __float_as_uint(fabsf((float)real_scale * wr));
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+            if ((threadIdx.x & 31) == 0 && m) atomicMax(wmax_bits, m);
+        }
     }
     __syncthreads();
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -158,6 +165,69 @@ __global__ void grad_split_T_kernel(const float* __restrict__ v, int64_t nb, int
         TwT[2 * plane + o] = (int8_t)d0;
     }
     if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && threadIdx.y == 0)
+        *reinterpret_cast<float*>(TwT + 3 * plane) = ldexpf(1.f, ex - 23);
+}
+
+// Real parameters, one pass: theta[s][.] -> v = real_scale tanh(theta) w_s -> the three int8 digit planes of
+// grad_split_T_kernel (same layout, same digits) and the fp64 column sums of the slab, without storing v.  The scale
+// is tied to max_s |real_scale w_s| >= max |v| (|tanh| <= 1; left by grad_a_partial_kernel), not to max |v| itself.
+// Tile = GRAD_SLAB samples x 32 hidden units per block of 256 threads; blockIdx.x = slab, blockIdx.y = 32-column group.
+__global__ void __launch_bounds__(256)
+grad_tv_split_kernel(const float* __restrict__ theta, int64_t nb, int k_len, int M, int M_eff, int ld,
+                     const float* __restrict__ eloc, const double* __restrict__ stats, double inv_B, float real_scale,
+                     const unsigned* __restrict__ wmax_bits, int8_t* __restrict__ TwT, double* __restrict__ part) {
+    __shared__ float w_s[GRAD_SLAB];
+    __shared__ __align__(4) int8_t dq[3][32][GRAD_SLAB + 4];      // row stride 33 words: byte writes down a column
+    __shared__ double cs[8][32];                                  // hit 32 different banks
+    const float vmax = __uint_as_float(*wmax_bits);
+    int ex = -100;
+    if (vmax > 0.f) {
+        frexpf(vmax, &ex);
+        if (ldexpf(vmax, 23 - ex) > 8355000.f) ++ex;
+    }
+    const float sc = ldexpf(1.f, 23 - ex);
+    const int64_t s0 = (int64_t)blockIdx.x * GRAD_SLAB;
+    const int m0 = blockIdx.y * 32;
+    if (threadIdx.x < GRAD_SLAB) {
+        float wr = 0.f, wi;
+        if (s0 + threadIdx.x < nb) sample_weight(eloc, stats, s0 + threadIdx.x, inv_B, false, wr, wi);
+        w_s[threadIdx.x] = wr;
+    }
+    __syncthreads();
+    const int c = threadIdx.x & 31, r = threadIdx.x >> 5;
+    const bool col_ok = m0 + c < M;
+    double acc = 0.0;
+#pragma unroll 8
+    for (int p = 0; p < GRAD_SLAB / 8; ++p) {
+        const int sl = p * 8 + r;
+        float v = 0.f;
+        if (col_ok && s0 + sl < nb) v = real_scale * tanhf(theta[(s0 + sl) * M_eff + m0 + c]) * w_s[sl];
+        acc += (double)v;
+        const int I = (int)rintf(v * sc);
+        const int d0 = ((I + 128) & 255) - 128;
+        const int I1 = (I - d0) >> 8;
+        const int d1 = ((I1 + 128) & 255) - 128;
+        dq[0][c][sl] = (int8_t)((I1 - d1) >> 8);
+        dq[1][c][sl] = (int8_t)d1;
+        dq[2][c][sl] = (int8_t)d0;
+    }
+    cs[r][c] = acc;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double t = 0.0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) t += cs[q][threadIdx.x];
+        part[(size_t)blockIdx.x * M_eff + m0 + threadIdx.x] = t;
+    }
+    const size_t plane = (size_t)M_eff * ld;
+    const int n_words = (int)min((int64_t)GRAD_SLAB, (int64_t)k_len - s0) >> 2;
+    for (int row = r; row < 96; row += 8) {
+        const int d = row >> 5, j = row & 31;
+        if (c < n_words)
+            *reinterpret_cast<int*>(TwT + d * plane + (size_t)(m0 + j) * ld + s0 + 4 * c) =
+                *reinterpret_cast<const int*>(&dq[d][j][4 * c]);
+    }
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0)
         *reinterpret_cast<float*>(TwT + 3 * plane) = ldexpf(1.f, ex - 23);
 }
 
@@ -225,25 +295,30 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
     const int k_len = (int)((nb + 127) / 128 * 128);
     cudaError_t e = cudaMemsetAsync(w.absmax, 0, sizeof(unsigned), st);
     if (e != cudaSuccess) return e;
-    dim3 gtv((g.M_pad + 255) / 256, (unsigned)(nb < 1184 ? nb : 1184));
-    if (cplx)
-        grad_tv_kernel<true><<<gtv, 256, 0, st>>>(theta_in ? theta_in : w.theta, w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
-                                                  real_scale, w.absmax);
-    else
-        grad_tv_kernel<false><<<gtv, 256, 0, st>>>(theta_in ? theta_in : w.theta, w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats, inv_B,
-                                                   real_scale, w.absmax);
     const int n_slabs = (int)((nb + GRAD_SLAB - 1) / GRAD_SLAB);
-    grad_colsum_partial_kernel<<<dim3((g.M_eff + 127) / 128, n_slabs), 128, 0, st>>>(w.theta, nb, g.M_eff, w.part);
-    grad_slab_reduce_kernel<<<(g.M_eff + 127) / 128, 128, 0, st>>>(w.part, n_slabs, g.M_eff, w.gb_acc, first_chunk);
-    grad_a_partial_kernel<<<dim3((g.N + 127) / 128, n_slabs), 128, 0, st>>>(sigma, nb, g.N, (const float*)eloc, stats,
-                                                                            inv_B, cplx, (double)real_scale, w.part);
+    const float* th_in = theta_in ? theta_in : w.theta;
+    grad_a_partial_kernel<<<dim3((g.N + 127) / 128, n_slabs), 128, 0, st>>>(
+        sigma, nb, g.N, (const float*)eloc, stats, inv_B, cplx, (double)real_scale, w.part, cplx ? nullptr : w.absmax);
     grad_slab_reduce_kernel<<<(2 * g.N + 127) / 128, 128, 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk);
-    grad_split_T_kernel<<<dim3(k_len / 32, g.M_eff / 32), dim3(32, 8), 0, st>>>(
-        w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (int8_t*)w.TwT);
+    if (!cplx) {
+        // k_len / GRAD_SLAB == n_slabs (both round nb up to 128)
+        grad_tv_split_kernel<<<dim3(n_slabs, g.M_eff / 32), 256, 0, st>>>(
+            th_in, nb, k_len, g.M, g.M_eff, w.ld, (const float*)eloc, stats, inv_B, real_scale, w.absmax,
+            (int8_t*)w.TwT, w.part);
+        count_launch(sigT_ready ? 4 : 5);
+    } else {
+        dim3 gtv((g.M_pad + 255) / 256, (unsigned)(nb < 1184 ? nb : 1184));
+        grad_tv_kernel<true><<<gtv, 256, 0, st>>>(th_in, w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats,
+                                                  inv_B, real_scale, w.absmax);
+        grad_colsum_partial_kernel<<<dim3((g.M_eff + 127) / 128, n_slabs), 128, 0, st>>>(w.theta, nb, g.M_eff, w.part);
+        grad_split_T_kernel<<<dim3(k_len / 32, g.M_eff / 32), dim3(32, 8), 0, st>>>(
+            w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (int8_t*)w.TwT);
+        count_launch(sigT_ready ? 6 : 7);
+    }
+    grad_slab_reduce_kernel<<<(g.M_eff + 127) / 128, 128, 0, st>>>(w.part, n_slabs, g.M_eff, w.gb_acc, first_chunk);
     if (sigT_ready == nullptr)
         grad_sigma_T_kernel<<<dim3(k_len / 32, (g.N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, g.N, w.ld,
                                                                                      (int8_t*)w.sigT);
-    count_launch(sigT_ready ? 6 : 7);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     return launch_tc_gemm_pieces(sigT_ready ? sigT_ready : (const void*)w.sigT, g.N, w.TwT, g.M_eff, w.ld, k_len, w.Gacc,
