@@ -123,8 +123,20 @@ __global__ void grad_a_partial_kernel(const int8_t* __restrict__ sigma, int64_t 
 }
 
 // acc[c] (+)= sum_slab part[slab][c], slabs in order
+// scale_io (optional): [0] = max |v| bound as float bits (in) -> [2] = 2^(23 - ex), [3] = q = 2^(ex - 23) as floats (out)
 __global__ void grad_slab_reduce_kernel(const double* __restrict__ part, int n_slabs, int n_cols,
-                                        double* __restrict__ acc, int first) {
+                                        double* __restrict__ acc, int first, unsigned* scale_io) {
+    if (scale_io != nullptr && blockIdx.x == 0 && threadIdx.x == 0) {
+        const float vmax = __uint_as_float(scale_io[0]);
+        int ex = -100;
+        if (vmax > 0.f) {
+            frexpf(vmax, &ex);
+            if (ldexpf(vmax, 23 - ex) > 8355000.f) ++ex;      // keep the top digit inside [-128, 127]
+            if (ex < -100) ex = -100;                         // keep 2^(23 - ex) finite
+        }
+        scale_io[2] = __float_as_uint(ldexpf(1.f, 23 - ex));
+        scale_io[3] = __float_as_uint(ldexpf(1.f, ex - 23));
+    }
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= n_cols) return;
     double a = first ? 0.0 : acc[c];
@@ -168,67 +180,101 @@ __global__ void grad_split_T_kernel(const float* __restrict__ v, int64_t nb, int
         *reinterpret_cast<float*>(TwT + 3 * plane) = ldexpf(1.f, ex - 23);
 }
 
+// tanh in fp32 without branches: |x| < 1 by x + x^3 P(x^2) (P = degree-6 least-squares fit of (tanh x - x) / x^3 in x^2,
+// relative error < 1e-7 in fp32), else 1 - 2 / (e^{2x} + 1) with one MUFU.EX2 and one MUFU.RCP (< 2e-7 relative)
+__device__ __forceinline__ float tanh_f32(float x) {
+    const float x2 = x * x;
+    float p = -0.0003552270936779678f;
+    p = fmaf(p, x2, 0.002289985306560993f);
+    p = fmaf(p, x2, -0.007930326275527477f);
+    p = fmaf(p, x2, 0.021475814282894135f);
+    p = fmaf(p, x2, -0.05387599393725395f);
+    p = fmaf(p, x2, 0.1333228200674057f);
+    p = fmaf(p, x2, -0.33333292603492737f);
+    const float small = fmaf(x * x2, p, x);
+    float E, rc;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(E) : "f"(x * 2.8853900817779268f));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rc) : "f"(E + 1.f));
+    const float big = fmaf(-2.f, rc, 1.f);
+    return fabsf(x) < 1.f ? small : big;
+}
+
 // Real parameters, one pass: theta[s][.] -> v = real_scale tanh(theta) w_s -> the three int8 digit planes of
 // grad_split_T_kernel (same layout, same digits) and the fp64 column sums of the slab, without storing v.  The scale
 // is tied to max_s |real_scale w_s| >= max |v| (|tanh| <= 1; left by grad_a_partial_kernel), not to max |v| itself.
-// Tile = GRAD_SLAB samples x 32 hidden units per block of 256 threads; blockIdx.x = slab, blockIdx.y = 32-column group.
+// Tile = GRAD_SLAB samples x 32 hidden units per block of 256 threads; blockIdx.x = slab * (M_eff / 32) + column group:
+// blocks in flight together cover whole rows of theta (DRAM page locality).
 __global__ void __launch_bounds__(256)
 grad_tv_split_kernel(const float* __restrict__ theta, int64_t nb, int k_len, int M, int M_eff, int ld,
                      const float* __restrict__ eloc, const double* __restrict__ stats, double inv_B, float real_scale,
-                     const unsigned* __restrict__ wmax_bits, int8_t* __restrict__ TwT, double* __restrict__ part) {
-    __shared__ float w_s[GRAD_SLAB];
-    __shared__ __align__(4) int8_t dq[3][32][GRAD_SLAB + 4];      // row stride 33 words: byte writes down a column
-    __shared__ double cs[8][32];                                  // hit 32 different banks
-    const float vmax = __uint_as_float(*wmax_bits);
-    int ex = -100;
-    if (vmax > 0.f) {
-        frexpf(vmax, &ex);
-        if (ldexpf(vmax, 23 - ex) > 8355000.f) ++ex;
-    }
-    const float sc = ldexpf(1.f, 23 - ex);
-    const int64_t s0 = (int64_t)blockIdx.x * GRAD_SLAB;
-    const int m0 = blockIdx.y * 32;
+                     const unsigned* __restrict__ scale_io, int8_t* __restrict__ TwT, double* __restrict__ part) {
+    __shared__ float w_s[GRAD_SLAB];                              // real_scale w_s / q: v / q = tanh(theta) * this
+    __shared__ int dq[3][32][GRAD_SLAB / 4 + 1];                  // [digit][column][4 samples per word], stride 33 words
+    __shared__ int cs[8][32];
+    const float sc = __uint_as_float(scale_io[2]), q = __uint_as_float(scale_io[3]);
+    const int n_cg = M_eff >> 5;
+    const int slab = blockIdx.x / n_cg;
+    const int64_t s0 = (int64_t)slab * GRAD_SLAB;
+    const int m0 = (blockIdx.x - slab * n_cg) * 32;
+    const int n_rows = (int)min((int64_t)GRAD_SLAB, nb - s0);
     if (threadIdx.x < GRAD_SLAB) {
         float wr = 0.f, wi;
-        if (s0 + threadIdx.x < nb) sample_weight(eloc, stats, s0 + threadIdx.x, inv_B, false, wr, wi);
-        w_s[threadIdx.x] = wr;
+        if ((int)threadIdx.x < n_rows) sample_weight(eloc, stats, s0 + threadIdx.x, inv_B, false, wr, wi);
+        w_s[threadIdx.x] = real_scale * wr * sc;                  // two exact scalings (1 or 2, a power of two)
     }
     __syncthreads();
     const int c = threadIdx.x & 31, r = threadIdx.x >> 5;
-    const bool col_ok = m0 + c < M;
-    double acc = 0.0;
-#pragma unroll 8
-    for (int p = 0; p < GRAD_SLAB / 8; ++p) {
-        const int sl = p * 8 + r;
-        float v = 0.f;
-        if (col_ok && s0 + sl < nb) v = real_scale * tanhf(theta[(s0 + sl) * M_eff + m0 + c]) * w_s[sl];
-        acc += (double)v;
-        const int I = (int)rintf(v * sc);
-        const int d0 = ((I + 128) & 255) - 128;
-        const int I1 = (I - d0) >> 8;
-        const int d1 = ((I1 + 128) & 255) - 128;
-        dq[0][c][sl] = (int8_t)((I1 - d1) >> 8);
-        dq[1][c][sl] = (int8_t)d1;
-        dq[2][c][sl] = (int8_t)d0;
+    const float* col = theta + s0 * M_eff + m0 + c;
+    const int lim = (m0 + c < M) ? n_rows : 0;
+    const bool whole = n_rows == GRAD_SLAB && m0 + 32 <= M;       // block-uniform: no predicates on the loads
+    const float* ptr = col + (unsigned)(4 * r * M_eff);
+    int acc = 0;                                                  // sum of the slab's integers: |I| <= 2^23, 128 of them
+#pragma unroll
+    for (int p = 0; p < GRAD_SLAB / 32; ++p) {
+        const int sl = 4 * (r + 8 * p);                           // this thread: samples sl .. sl + 3 of column c
+        float th[4];
+        if (whole) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) th[i] = ptr[i * M_eff];
+        } else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) th[i] = (sl + i < lim) ? ptr[i * M_eff] : 0.f;
+        }
+        ptr += 32 * M_eff;
+        // rint(v / q) = d2 2^16 + d1 2^8 + d0 with balanced digits: the low bytes of I, (I + 128) >> 8 and of that again
+        unsigned w0 = 0, w1 = 0, w2 = 0;
+#define NK_DIGITS(i, sel)                                                         \
+        {                                                                         \
+            const int I = __float2int_rn(tanh_f32(th[i]) * w_s[sl + i]);          \
+            const int I1 = (I + 128) >> 8;                                        \
+            const int I2 = (I1 + 128) >> 8;                                       \
+            acc += I;                                                             \
+            w0 = __byte_perm(w0, (unsigned)I, sel);                               \
+            w1 = __byte_perm(w1, (unsigned)I1, sel);                              \
+            w2 = __byte_perm(w2, (unsigned)I2, sel);                              \
+        }
+        NK_DIGITS(0, 0x3214) NK_DIGITS(1, 0x3240) NK_DIGITS(2, 0x3410) NK_DIGITS(3, 0x4210)
+#undef NK_DIGITS
+        dq[0][c][r + 8 * p] = (int)w2;
+        dq[1][c][r + 8 * p] = (int)w1;
+        dq[2][c][r + 8 * p] = (int)w0;
     }
     cs[r][c] = acc;
     __syncthreads();
     if (threadIdx.x < 32) {
-        double t = 0.0;
+        int t = 0;
 #pragma unroll
-        for (int q = 0; q < 8; ++q) t += cs[q][threadIdx.x];
-        part[(size_t)blockIdx.x * M_eff + m0 + threadIdx.x] = t;
+        for (int k = 0; k < 8; ++k) t += cs[k][threadIdx.x];
+        part[(size_t)slab * M_eff + m0 + threadIdx.x] = (double)t * (double)q;
     }
     const size_t plane = (size_t)M_eff * ld;
-    const int n_words = (int)min((int64_t)GRAD_SLAB, (int64_t)k_len - s0) >> 2;
+    int8_t* out = TwT + (size_t)m0 * ld + s0 + 4 * c;             // k_len is a multiple of GRAD_SLAB: whole rows of the tile
+#pragma unroll
     for (int row = r; row < 96; row += 8) {
         const int d = row >> 5, j = row & 31;
-        if (c < n_words)
-            *reinterpret_cast<int*>(TwT + d * plane + (size_t)(m0 + j) * ld + s0 + 4 * c) =
-                *reinterpret_cast<const int*>(&dq[d][j][4 * c]);
+        *reinterpret_cast<int*>(out + d * plane + (size_t)j * ld) = dq[d][j][c];
     }
-    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0)
-        *reinterpret_cast<float*>(TwT + 3 * plane) = ldexpf(1.f, ex - 23);
+    if (blockIdx.x == 0 && threadIdx.x == 0) *reinterpret_cast<float*>(TwT + 3 * plane) = q;
 }
 
 // sigT[k][s] = sigma[s][k] (int8), zero for s in [nb, k_len)
@@ -299,10 +345,11 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
     const float* th_in = theta_in ? theta_in : w.theta;
     grad_a_partial_kernel<<<dim3((g.N + 127) / 128, n_slabs), 128, 0, st>>>(
         sigma, nb, g.N, (const float*)eloc, stats, inv_B, cplx, (double)real_scale, w.part, cplx ? nullptr : w.absmax);
-    grad_slab_reduce_kernel<<<(2 * g.N + 127) / 128, 128, 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk);
+    grad_slab_reduce_kernel<<<(2 * g.N + 127) / 128, 128, 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk,
+                                                                   cplx ? nullptr : w.absmax);
     if (!cplx) {
         // k_len / GRAD_SLAB == n_slabs (both round nb up to 128)
-        grad_tv_split_kernel<<<dim3(n_slabs, g.M_eff / 32), 256, 0, st>>>(
+        grad_tv_split_kernel<<<(unsigned)n_slabs * (unsigned)(g.M_eff / 32), 256, 0, st>>>(
             th_in, nb, k_len, g.M, g.M_eff, w.ld, (const float*)eloc, stats, inv_B, real_scale, w.absmax,
             (int8_t*)w.TwT, w.part);
         count_launch(sigT_ready ? 4 : 5);
@@ -315,7 +362,8 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
             w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (int8_t*)w.TwT);
         count_launch(sigT_ready ? 6 : 7);
     }
-    grad_slab_reduce_kernel<<<(g.M_eff + 127) / 128, 128, 0, st>>>(w.part, n_slabs, g.M_eff, w.gb_acc, first_chunk);
+    grad_slab_reduce_kernel<<<(g.M_eff + 127) / 128, 128, 0, st>>>(w.part, n_slabs, g.M_eff, w.gb_acc, first_chunk,
+                                                                   nullptr);
     if (sigT_ready == nullptr)
         grad_sigma_T_kernel<<<dim3(k_len / 32, (g.N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, g.N, w.ld,
                                                                                      (int8_t*)w.sigT);
