@@ -13,10 +13,19 @@
 //  the operand bytes; per-ELEMENT bf16 splitting had been measured to bias the result by ~0.25 ulp through the adder's
 //  truncation — with integer accumulators there is no adder rounding at all.
 //
-// Kernel: one CTA per 128 (rows) x 128 (columns) tile.  Warp 0 = TMA producer (cp.async.bulk.tensor, 128B swizzle,
-// 3-stage ring: per stage the A tile and the three digit tiles of a k block of 128 int8 per row); warp 1 = TMEM
-// allocator and single-thread tcgen05.mma issuer (M = 128, N = 128, K = 32: 12 MMAs per k block, three 128-column
-// int32 accumulators); warps 2-5 = epilogue (tcgen05.ld 32x32b, scale / bias, fp32 stores).
+// Kernel: persistent, one CTA per SM walking over 128 (rows) x 64 (columns) tiles (column tiles fastest: neighbouring
+// CTAs share their A rows in L2).  Warp 0 = TMA producer (cp.async.bulk.tensor, 128B swizzle, 4-stage ring: per stage
+// the A tile and the three digit tiles of a k block of 128 int8 per row, 40 KB); warp 1 = TMEM allocator and
+// single-thread tcgen05.mma issuer: the three digit tiles lie back to back in the stage, so ONE MMA with M = 128,
+// N = 192, K = 32 per k step contracts all three planes and reads the A tile from shared memory once (three N = 64
+// MMAs, one per plane, read it three times and were measured shared-memory-bandwidth-bound: 547 against 390 us);
+// the accumulator columns [0, 64), [64, 128), [128, 192) are D_hi, D_mid, D_lo.  Warps 2-5 = epilogue (tcgen05.ld
+// 32x32b, scale / bias, fp32 stores).  The accumulators are double-buffered in TMEM (2 x 192 of the 512 columns), so
+// the epilogue of tile i runs under the MMAs of tile i + 1 and the producer runs ahead across tile boundaries; one
+// TMEM allocation and one barrier set-up per CTA instead of per tile.  Thread-block clusters of CM x CN CTAs share
+// operand tiles by TMA multicast (default 2 x 1: the two CTAs of a tile column load half of every digit tile each).
+// (The first version, one CTA per 128 x 128 tile with three 128-column accumulators, the prologue, the MMAs and the
+// epilogue in series, took 437 us for the same product.)
 #include <cuda.h>
 
 #include "nk_internal.h"
@@ -25,15 +34,17 @@
 namespace nk {
 
 namespace tc {
-constexpr int BM = 128, BN = 128, BK = 64, STAGES = 3, UMMA_K = 16;
-constexpr int TILE_BYTES = BM * BK * 2;                   // 16 KB: one tile of 128 rows x 128 B (A or one digit plane)
-constexpr int STAGE_BYTES = 4 * TILE_BYTES;               // sigma + hi + mid + lo
+constexpr int BM = 128, BN = 64, BKB = 128, STAGES = 4, UMMA_KB = 32;   // BKB: bytes = int8 elements per k-block row
+constexpr int A_BYTES = BM * BKB;                         // 16 KB: 128 rows x 128 B
+constexpr int P_BYTES = BN * BKB;                         //  8 KB: one digit plane, 64 rows x 128 B
+constexpr int STAGE_BYTES = A_BYTES + 3 * P_BYTES;        // sigma + hi + mid + lo
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment*/ + 256 /*barriers*/;
 constexpr int THREADS = 192;
-constexpr uint32_t TMEM_COLS = 512;                       // D_hi [0,128), D_mid [128,256), D_lo [256,384); power of 2
-// instruction descriptor (cute::UMMA::InstrDescriptor bit layout): D=F32, A=B=BF16, K-major both, N=128, M=128
-// instruction descriptor of kind::i8: D = S32 (c_format 2), A = B = signed 8 bit (format 1), K-major, N >> 3, M >> 4
-constexpr uint32_t IDESC_I8 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+constexpr uint32_t TMEM_COLS = 512;                       // two accumulator sets: D_hi, D_mid, D_lo at +0, +64, +128
+constexpr uint32_t ACC_STRIDE = 256;                      // of column 0 and of column 256
+// instruction descriptor of kind::i8 (cute::UMMA::InstrDescriptor bit layout): D = S32 (c_format 2), A = B = signed
+// 8 bit (format 1), K-major both, N >> 3, M >> 4
+constexpr uint32_t IDESC_I8 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)((3 * BN) >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
 }  // namespace tc
 
 // ---- operand preparation ---------------------------------------------------------------------------------
@@ -99,6 +110,28 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
         ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar)
         : "memory");
 }
+__device__ __forceinline__ void tma_load_2d_mc(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar,
+                                               uint16_t cta_mask) {
+    // the box lands at the same shared-memory offset, and completes bytes on the same barrier offset, in every CTA
+    // of the cluster whose rank bit is set
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.multicast::cluster "
+        "[%0], [%1, {%2, %3}], [%4], %5;" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar), "h"(cta_mask)
+        : "memory");
+}
+__device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t cta_mask) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+                 "h"(cta_mask)
+                 : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 __device__ __forceinline__ uint64_t make_sdesc(uint32_t smem_addr) {
     // K-major, 128B swizzle: start address >> 4, LBO (unused for swizzled K-major) = 1, SBO = 1024 B (8 rows x
     // 128 B) >> 4, descriptor version 1 (sm_100), layout type 2 = SWIZZLE_128B
@@ -140,27 +173,39 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
 // ---- the GEMM ---------------------------------------------------------------------------------------------
 // int8 operands (128 elements per 128-B swizzle row, so K_pad / 128 k blocks), int32 accumulators,
 // out (+)= q (D2 2^16 + D1 2^8 + D0) + bias with the scale q read from `scale`.
+// A cluster of CM x CN CTAs (rank = rm CN + rn) works on CM x CN neighbouring tiles: the CN CTAs of a tile row share
+// their A tile (each loads 1 / CN of its rows and multicasts it), the CM CTAs of a tile column share the three digit
+// tiles (each loads 1 / CM of the rows of every plane).  A stage of a CTA is therefore written by CM + CN - 1 CTAs
+// (itself included), and the MMA commit that frees the stage arrives on the `empty` barrier of every one of them.
+template <int CM, int CN>
 __global__ void __launch_bounds__(tc::THREADS, 1)
 theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w, int64_t B,
                 int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta, int accumulate,
-                const float* __restrict__ scale) {
+                const float* __restrict__ scale, int n_sup_n, int n_sup) {
     using namespace tc;
+    constexpr int CS = CM * CN;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;            // SWIZZLE_128B needs 1024 B
-    const uint32_t bars = smem_base + STAGES * STAGE_BYTES;                      // full[3], empty[3], tmem_full
-    const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, tfull = bars + 16 * STAGES;
-    const uint32_t tmem_slot = bars + 16 * STAGES + 8;
+    const uint32_t bars = smem_base + STAGES * STAGE_BYTES;
+    const uint32_t full0 = bars, empty0 = bars + 8 * STAGES;                     // smem ring
+    const uint32_t tfull0 = bars + 16 * STAGES, tempty0 = tfull0 + 16;          // the two accumulator sets
+    const uint32_t tmem_slot = tempty0 + 16;
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n0 = blockIdx.x * BN;                       // hidden-unit tile
-    const int64_t m0 = (int64_t)blockIdx.y * BM;          // sample tile
-    constexpr int BKE = 2 * BK;                           // int8 elements per k block (128 B per row)
-    const int n_kb = K_pad / BKE;
+    const int n_kb = K_pad / BKB;
+    const int rank = CS > 1 ? (int)cluster_ctarank() : 0;
+    const int rm = rank / CN, rn = rank - rm * CN;
+    const int cluster_id = blockIdx.x / CS, n_clusters = gridDim.x / CS;
+    uint16_t mask_a = 0, mask_w = 0;
+#pragma unroll
+    for (int j = 0; j < CN; ++j) mask_a |= (uint16_t)(1u << (rm * CN + j));
+#pragma unroll
+    for (int i = 0; i < CM; ++i) mask_w |= (uint16_t)(1u << (i * CN + rn));
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, 1); }
-        mbar_init(tfull, 1);
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, CM + CN - 1); }
+        for (int a = 0; a < 2; ++a) { mbar_init(tfull0 + 8 * a, 1); mbar_init(tempty0 + 8 * a, 128); }
         mbar_fence_init();
     }
     if (warp == 1) {   // TMEM allocation by one full warp; the base address lands in shared memory
@@ -170,87 +215,121 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (CS > 1) cluster_sync_all();                       // every CTA's barriers exist before anything is multicast
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem_base = *tmem_slot_ptr;
 
     if (warp == 0) {
-        // ===== TMA producer =====
+        // ===== TMA producer: runs ahead of the MMAs across tile boundaries =====
         if (lane == 0) {
             int stage = 0; uint32_t parity = 1;
-            for (int kb = 0; kb < n_kb; ++kb) {
-                mbar_wait(empty0 + 8 * stage, parity);
-                mbar_arrive_expect_tx(full0 + 8 * stage, STAGE_BYTES);
-                const uint32_t dst = smem_base + stage * STAGE_BYTES;
-                tma_load_2d(dst, &map_a, kb * BKE, (int)m0, full0 + 8 * stage);
+            for (int sup = cluster_id; sup < n_sup; sup += n_clusters) {
+                const int sm = sup / n_sup_n;
+                const int m0 = (sm * CM + rm) * BM, n0 = ((sup - sm * n_sup_n) * CN + rn) * BN;
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(empty0 + 8 * stage, parity);
+                    mbar_arrive_expect_tx(full0 + 8 * stage, STAGE_BYTES);
+                    const uint32_t dst = smem_base + stage * STAGE_BYTES;
+                    if (CN > 1)
+                        tma_load_2d_mc(dst + rn * (A_BYTES / CN), &map_a, kb * BKB, m0 + rn * (BM / CN),
+                                       full0 + 8 * stage, mask_a);
+                    else
+                        tma_load_2d(dst, &map_a, kb * BKB, m0, full0 + 8 * stage);
 #pragma unroll
-                for (int pc = 0; pc < 3; ++pc)
-                    tma_load_2d(dst + (1 + pc) * TILE_BYTES, &map_w, kb * BKE, pc * M_eff + n0, full0 + 8 * stage);
-                if (++stage == STAGES) { stage = 0; parity ^= 1; }
+                    for (int pc = 0; pc < 3; ++pc) {
+                        if (CM > 1)
+                            tma_load_2d_mc(dst + A_BYTES + pc * P_BYTES + rm * (P_BYTES / CM), &map_w, kb * BKB,
+                                           pc * M_eff + n0 + rm * (BN / CM), full0 + 8 * stage, mask_w);
+                        else
+                            tma_load_2d(dst + A_BYTES + pc * P_BYTES, &map_w, kb * BKB, pc * M_eff + n0,
+                                        full0 + 8 * stage);
+                    }
+                    if (++stage == STAGES) { stage = 0; parity ^= 1; }
+                }
             }
         }
     } else if (warp == 1) {
         // ===== MMA issuer (one thread) =====
         if (lane == 0) {
             int stage = 0; uint32_t parity = 0;
-            for (int kb = 0; kb < n_kb; ++kb) {
-                mbar_wait(full0 + 8 * stage, parity);
+            int it = 0;
+            for (int sup = cluster_id; sup < n_sup; sup += n_clusters, ++it) {
+                const int set = it & 1;
+                mbar_wait(tempty0 + 8 * set, ((it >> 1) & 1) ^ 1);      // the epilogue has drained this set (free at first)
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t a_addr = smem_base + stage * STAGE_BYTES;
+                const uint32_t acc = tmem_base + set * ACC_STRIDE;
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(full0 + 8 * stage, parity);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const uint32_t a_addr = smem_base + stage * STAGE_BYTES;
 #pragma unroll
-                for (int k = 0; k < BK / UMMA_K; ++k) {
-                    const uint32_t koff = k * UMMA_K * 2;                       // bytes inside the 128 B swizzle row
-                    const uint64_t ad = make_sdesc(a_addr + koff);
-                    const uint32_t first = (kb | k) ? 1u : 0u;
-                    // 32 B = 32 int8 = one K = 32 MMA per digit plane
-                    umma_i8(tmem_base + 0, ad, make_sdesc(a_addr + 1 * TILE_BYTES + koff), IDESC_I8, first);
-                    umma_i8(tmem_base + BN, ad, make_sdesc(a_addr + 2 * TILE_BYTES + koff), IDESC_I8, first);
-                    umma_i8(tmem_base + 2 * BN, ad, make_sdesc(a_addr + 3 * TILE_BYTES + koff), IDESC_I8, first);
+                    for (int k = 0; k < BKB / UMMA_KB; ++k) {
+                        const uint32_t koff = k * UMMA_KB;                      // bytes inside the 128 B swizzle row
+                        const uint64_t ad = make_sdesc(a_addr + koff);
+                        const uint32_t first = (kb | k) ? 1u : 0u;
+                        // 32 B = 32 int8 = one K = 32 MMA; the three digit tiles lie back to back in the stage, so ONE
+                        // MMA with N = 3 BN takes them as a single B operand and reads the A tile once instead of thrice
+                        umma_i8(acc, ad, make_sdesc(a_addr + A_BYTES + koff), IDESC_I8, first);
+                    }
+                    // frees the stage, here and in the CTAs that multicast into it, once these MMAs have read it
+                    if (CS > 1) umma_commit_mc(empty0 + 8 * stage, (uint16_t)(mask_a | mask_w));
+                    else umma_commit(empty0 + 8 * stage);
+                    if (++stage == STAGES) { stage = 0; parity ^= 1; }
                 }
-                umma_commit(empty0 + 8 * stage);          // frees the smem stage when these MMAs have read it
-                if (++stage == STAGES) { stage = 0; parity ^= 1; }
+                umma_commit(tfull0 + 8 * set);            // this tile's accumulators are complete
             }
-            umma_commit(tfull);                           // accumulators complete
         }
     } else {
         // ===== epilogue: warps 2..5, TMEM lane quarter = warp % 4 =====
         const int q = warp & 3;
-        mbar_wait(tfull, 0);
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const int64_t row = m0 + q * 32 + lane;
-        float* out = theta + row * M_eff + n0;
         const float qs = *scale;
+        int it = 0;
+        for (int sup = cluster_id; sup < n_sup; sup += n_clusters, ++it) {
+            const int set = it & 1;
+            const int sm = sup / n_sup_n;
+            const int n0 = ((sup - sm * n_sup_n) * CN + rn) * BN;
+            const int64_t row = (int64_t)(sm * CM + rm) * BM + q * 32 + lane;
+            float* out = theta + row * M_eff + n0;
+            mbar_wait(tfull0 + 8 * set, (it >> 1) & 1);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
-        for (int c0 = 0; c0 < BN; c0 += 32) {
-            float hi[32], mid[32], lo[32];
-            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + c0;
-            tmem_ld32(taddr, hi);
-            tmem_ld32(taddr + BN, mid);
-            tmem_ld32(taddr + 2 * BN, lo);
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-            if (row < B) {
+            for (int c0 = 0; c0 < BN; c0 += 32) {
+                float hi[32], mid[32], lo[32];
+                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + set * ACC_STRIDE + c0;
+                tmem_ld32(taddr, hi);
+                tmem_ld32(taddr + BN, mid);
+                tmem_ld32(taddr + 2 * BN, lo);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                if (c0 + 32 == BN) {                       // everything is in registers: hand the set back to the MMAs
+                    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                    mbar_arrive(tempty0 + 8 * set);
+                }
+                if (row < B) {
 #pragma unroll
-                for (int j = 0; j < 32; j += 4) {
-                    float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (bg != nullptr) bb = *reinterpret_cast<const float4*>(bg + n0 + c0 + j);
-                    if (accumulate) {                      // out += D (the gradient contraction runs over chunks)
-                        const float4 old = *reinterpret_cast<const float4*>(out + c0 + j);
-                        bb.x += old.x; bb.y += old.y; bb.z += old.z; bb.w += old.w;
+                    for (int j = 0; j < 32; j += 4) {
+                        float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (bg != nullptr) bb = *reinterpret_cast<const float4*>(bg + n0 + c0 + j);
+                        if (accumulate) {                  // out += D (the gradient contraction runs over chunks)
+                            const float4 old = *reinterpret_cast<const float4*>(out + c0 + j);
+                            bb.x += old.x; bb.y += old.y; bb.z += old.z; bb.w += old.w;
+                        }
+                        float4 o;
+                        auto comb = [&](int jj) -> float {                      // exact ints below 2^24 each
+                            const float h = (float)__float_as_int(hi[jj]), m = (float)__float_as_int(mid[jj]),
+                                        l = (float)__float_as_int(lo[jj]);
+                            return fmaf(h, 65536.f, fmaf(m, 256.f, l));
+                        };
+                        o.x = fmaf(qs, comb(j), bb.x); o.y = fmaf(qs, comb(j + 1), bb.y);
+                        o.z = fmaf(qs, comb(j + 2), bb.z); o.w = fmaf(qs, comb(j + 3), bb.w);
+                        *reinterpret_cast<float4*>(out + c0 + j) = o;
                     }
-                    float4 o;
-                    auto comb = [&](int jj) -> float {                          // exact ints below 2^24 each
-                        const float h = (float)__float_as_int(hi[jj]), m = (float)__float_as_int(mid[jj]),
-                                    l = (float)__float_as_int(lo[jj]);
-                        return fmaf(h, 65536.f, fmaf(m, 256.f, l));
-                    };
-                    o.x = fmaf(qs, comb(j), bb.x); o.y = fmaf(qs, comb(j + 1), bb.y);
-                    o.z = fmaf(qs, comb(j + 2), bb.z); o.w = fmaf(qs, comb(j + 3), bb.w);
-                    *reinterpret_cast<float4*>(out + c0 + j) = o;
                 }
             }
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (CS > 1) cluster_sync_all();                       // no peer still multicasts into, or arrives on, this CTA
     if (warp == 1) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
@@ -263,6 +342,45 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 static EncodeTiledFn g_encode = nullptr;
 static bool g_tc_ready = false;
+static bool encode_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols, int box_rows);
+static int g_num_sms = 148;
+static int g_cm = 1, g_cn = 1, g_max_clusters = 148;      // the cluster shape in use and how many fit on the device
+
+template <int CM, int CN>
+static cudaError_t tc_prepare(int* max_clusters) {
+    const void* fn = (const void*)theta_tc_kernel<CM, CN>;
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(CM * CN, 1, 1);
+    cfg.blockDim = dim3(tc::THREADS, 1, 1);
+    cfg.dynamicSmemBytes = tc::SMEM_BYTES;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CM * CN; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaOccupancyMaxActiveClusters(max_clusters, fn, &cfg);
+}
+
+template <int CM, int CN>
+static cudaError_t tc_launch(const CUtensorMap& map_a, const CUtensorMap& map_w, int64_t rows, int cols, int k_len,
+                             const float* bg, float* out, int accumulate, const float* scale, cudaStream_t st) {
+    const int n_sup_n = cols / (tc::BN * CN);
+    const int64_t n_sup = (rows + (int64_t)tc::BM * CM - 1) / ((int64_t)tc::BM * CM) * n_sup_n;
+    if (n_sup > 0x7fffffff) return cudaErrorInvalidValue;
+    const int n_clusters = (int)(n_sup < g_max_clusters ? n_sup : g_max_clusters);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(n_clusters * CM * CN), 1, 1);
+    cfg.blockDim = dim3(tc::THREADS, 1, 1);
+    cfg.dynamicSmemBytes = tc::SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CM * CN; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, theta_tc_kernel<CM, CN>, map_a, map_w, rows, cols, k_len, bg, out, accumulate, scale,
+                              n_sup_n, (int)n_sup);
+}
 
 cudaError_t theta_tc_init() {
     if (g_tc_ready) return cudaSuccess;
@@ -272,18 +390,56 @@ cudaError_t theta_tc_init() {
     if (e != cudaSuccess) return e;
     if (qres != cudaDriverEntryPointSuccess || fn == nullptr) return cudaErrorNotSupported;
     g_encode = (EncodeTiledFn)fn;
-    e = cudaFuncSetAttribute((const void*)theta_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             tc::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+        sms > 0)
+        g_num_sms = sms;
+    // cluster shape: 2 x 1 (measured best at 65536 x 2048 x 1024: 374 us against 390 for 1 x 1, 394 for 2 x 2, 403 for
+    // 4 x 1 and 4 x 2) unless NK_TC_CLUSTER (an experiment knob: "1x1", "2x1", "2x2", "4x1", "4x2") says otherwise or the
+    // device cannot co-schedule such clusters
+    int want_m = 2, want_n = 1;
+    if (const char* v = getenv("NK_TC_CLUSTER")) {
+        if (v[0] >= '1' && v[0] <= '4' && v[1] == 'x' && v[2] >= '1' && v[2] <= '2') { want_m = v[0] - '0'; want_n = v[2] - '0'; }
+    }
+    int n = 0;
+    g_cm = g_cn = 1;
+    if (want_m == 4 && want_n == 2 && tc_prepare<4, 2>(&n) == cudaSuccess && n > 0) { g_cm = 4; g_cn = 2; }
+    else if (want_m == 4 && want_n == 1 && tc_prepare<4, 1>(&n) == cudaSuccess && n > 0) { g_cm = 4; g_cn = 1; }
+    else if (want_m == 2 && want_n == 2 && tc_prepare<2, 2>(&n) == cudaSuccess && n > 0) { g_cm = 2; g_cn = 2; }
+    else if (want_m == 2 && want_n == 1 && tc_prepare<2, 1>(&n) == cudaSuccess && n > 0) { g_cm = 2; g_cn = 1; }
+    (void)cudaGetLastError();                              // a refused cluster shape is not an error of the call
+    if (g_cm * g_cn == 1) {
+        e = tc_prepare<1, 1>(&n);
+        if (e != cudaSuccess) return e;
+        if (n <= 0) n = g_num_sms;
+    }
+    g_max_clusters = n;
     g_tc_ready = true;
     return cudaSuccess;
 }
 
-// 2-D tensor map over a k-contiguous int8 [rows][cols] operand, box = 128 rows x 128 B, 128B swizzle
-static bool encode_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols) {
+static cudaError_t tc_gemm(const void* A, int64_t rows, const void* P, int cols, int ld, int k_len, const float* bg,
+                           float* out, int accumulate, cudaStream_t st) {
+    cudaError_t e = theta_tc_init();
+    if (e != cudaSuccess) return e;
+    CUtensorMap map_a, map_p;
+    if (!encode_2d(&map_a, A, (uint64_t)rows, (uint64_t)ld, tc::BM / g_cn)) return cudaErrorInvalidValue;
+    if (!encode_2d(&map_p, P, (uint64_t)3 * cols, (uint64_t)ld, tc::BN / g_cm)) return cudaErrorInvalidValue;
+    const float* scale = reinterpret_cast<const float*>((const int8_t*)P + (size_t)3 * cols * ld);
+    if (g_cm == 4 && g_cn == 2) e = tc_launch<4, 2>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, st);
+    else if (g_cm == 4) e = tc_launch<4, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, st);
+    else if (g_cm == 2 && g_cn == 2) e = tc_launch<2, 2>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, st);
+    else if (g_cm == 2) e = tc_launch<2, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, st);
+    else e = tc_launch<1, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, st);
+    count_launch();
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+// 2-D tensor map over a k-contiguous int8 [rows][cols] operand, box = box_rows rows x 128 B, 128B swizzle
+static bool encode_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols, int box_rows) {
     const cuuint64_t dims[2] = {cols, rows};
     const cuuint64_t strides[1] = {cols};
-    const cuuint32_t box[2] = {(cuuint32_t)(2 * tc::BK), (cuuint32_t)tc::BM};
+    const cuuint32_t box[2] = {(cuuint32_t)tc::BKB, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1, 1};
     return g_encode(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
                     const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -322,16 +478,7 @@ cudaError_t launch_sigma_operand(const int8_t* sigma, int64_t B, int N, int K_pa
 cudaError_t launch_theta_tc_pre(const void* A, int64_t B, int M_eff, int K_pad, const void* Ws, const float* bg,
                                 float* theta, cudaStream_t st) {
     if (B <= 0) return cudaSuccess;
-    cudaError_t e = theta_tc_init();
-    if (e != cudaSuccess) return e;
-    CUtensorMap map_a, map_w;
-    if (!encode_2d(&map_a, A, (uint64_t)B, (uint64_t)K_pad)) return cudaErrorInvalidValue;
-    if (!encode_2d(&map_w, Ws, (uint64_t)3 * M_eff, (uint64_t)K_pad)) return cudaErrorInvalidValue;
-    const float* scale = reinterpret_cast<const float*>((const int8_t*)Ws + (size_t)3 * M_eff * K_pad);
-    dim3 grid(M_eff / tc::BN, (unsigned)((B + tc::BM - 1) / tc::BM));
-    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_w, B, M_eff, K_pad, bg, theta, 0, scale);
-    count_launch();
-    return cudaGetLastError();
+    return tc_gemm(A, B, Ws, M_eff, K_pad, K_pad, bg, theta, 0, st);
 }
 
 cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, int K_pad, const void* Ws, void* A,
@@ -350,17 +497,7 @@ cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, in
 cudaError_t launch_tc_gemm_pieces(const void* A, int64_t rows, const void* P, int cols, int ld, int k_len, float* out,
                                   int accumulate, cudaStream_t st) {
     if (rows <= 0) return cudaSuccess;
-    cudaError_t e = theta_tc_init();
-    if (e != cudaSuccess) return e;
-    CUtensorMap map_a, map_p;
-    if (!encode_2d(&map_a, A, (uint64_t)rows, (uint64_t)ld)) return cudaErrorInvalidValue;
-    if (!encode_2d(&map_p, P, (uint64_t)3 * cols, (uint64_t)ld)) return cudaErrorInvalidValue;
-    const float* scale = reinterpret_cast<const float*>((const int8_t*)P + (size_t)3 * cols * ld);
-    dim3 grid(cols / tc::BN, (unsigned)((rows + tc::BM - 1) / tc::BM));
-    theta_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(map_a, map_p, rows, cols, k_len, nullptr, out,
-                                                                     accumulate, scale);
-    count_launch();
-    return cudaGetLastError();
+    return tc_gemm(A, rows, P, cols, ld, k_len, nullptr, out, accumulate, st);
 }
 
 }  // namespace nk
