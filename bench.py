@@ -168,23 +168,26 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
         anti = 1.0
     pairs = B * N * anti * M
     eloc, _, stats = plan.run(chains, W, a, b)
-    gws = torch.empty(lib.nk_energy_gradient_workspace_bytes(B, N, M, dt_code, p.chunk_size), dtype=torch.uint8,
+    # the contractions over the samples take the whole batch as one chunk (the library default; ~1 GB of workspace at
+    # config 5): one launch of each kernel instead of B / chunk_size read-modify-write passes over the accumulator
+    gchunk = 0
+    gws = torch.empty(lib.nk_energy_gradient_workspace_bytes(B, N, M, dt_code, gchunk), dtype=torch.uint8,
                       device=sigma.device)
-    ms_grad = _time_ms(torch, lambda: nk.energy_gradient(chains, W, b, eloc, stats, chunk_size=p.chunk_size, ws=gws), 3)
+    ms_grad = _time_ms(torch, lambda: nk.energy_gradient(chains, W, b, eloc, stats, chunk_size=gchunk, ws=gws), 3)
     ms_eloc = _time_ms(torch, lambda: plan.run(chains, W, a, b), 3)
     # QGT-vector product (one CG iteration of stochastic reconfiguration is this plus 4 vector kernels)
-    ga, gb, gW = nk.energy_gradient(chains, W, b, eloc, stats, chunk_size=p.chunk_size, ws=gws)
-    qws = torch.empty(lib.nk_qgt_matvec_workspace_bytes(B, N, M, dt_code, p.chunk_size), dtype=torch.uint8,
+    ga, gb, gW = nk.energy_gradient(chains, W, b, eloc, stats, chunk_size=gchunk, ws=gws)
+    qws = torch.empty(lib.nk_qgt_matvec_workspace_bytes(B, N, M, dt_code, gchunk), dtype=torch.uint8,
                       device=sigma.device)
     qout = (torch.empty_like(ga), torch.empty_like(gb), torch.empty_like(gW))
     ms_qgt = _time_ms(torch, lambda: nk.qgt_matvec(chains, W, b, ga, gb, gW, diag_shift=0.01,
-                                                   chunk_size=p.chunk_size, ws=qws, out=qout), 3)
+                                                   chunk_size=gchunk, ws=qws, out=qout), 3)
     # one conjugate-gradient iteration of the SR solve (theta and the spin conversions are cached across iterations)
-    sws = torch.empty(lib.nk_sr_solve_workspace_bytes(B, N, M, dt_code, p.chunk_size), dtype=torch.uint8,
+    sws = torch.empty(lib.nk_sr_solve_workspace_bytes(B, N, M, dt_code, gchunk), dtype=torch.uint8,
                       device=sigma.device)
     n_cg = 8
     ms_sr = _time_ms(torch, lambda: nk.sr_solve(chains, W, b, ga, gb, gW, diag_shift=0.01, tol=0.0, max_iter=n_cg,
-                                                chunk_size=p.chunk_size, ws=sws), 2)
+                                                chunk_size=gchunk, ws=sws), 2)
     # the graded step replayed from a CUDA graph (LocalEnergyPlan.run_graph): what launch overhead costs the small configs
     plan.run_graph(sigma, W, a, b)
     ms_graph = _time_ms(torch, lambda: plan.run_graph(sigma, W, a, b), 5)
@@ -211,7 +214,7 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
                     "evaluated_fraction_estimate": anti,
                     "roofline": {"bound": "alu", "kernel": "metropolis_kernel", "unit": "Gpair/s",
                                  "achieved": pairs / (ms_sweep * 1e-3) / 1e9}},
-        "gradient": {"ms": ms_grad, "algorithmic_tflops": 2.0 * planes * B * M * N / (ms_grad * 1e-3) / 1e12},
+        "gradient": {"ms": ms_grad, "chunk_size": "whole batch", "algorithmic_tflops": 2.0 * planes * B * M * N / (ms_grad * 1e-3) / 1e12},
         "qgt_matvec": {"ms": ms_qgt, "n_parameters": N + M + M * N,
                        "algorithmic_tflops": 3 * 2.0 * planes * B * M * N / (ms_qgt * 1e-3) / 1e12,
                        "what": "(G + 0.01) v on the fly, Eq. (75): theta, V_W sigma and J^dagger dw contractions"},

@@ -122,11 +122,12 @@ __global__ void grad_a_partial_kernel(const int8_t* __restrict__ sigma, int64_t 
     part[(size_t)blockIdx.y * 2 * N + N + k] = ai;
 }
 
-// acc[c] (+)= sum_slab part[slab][c], slabs in order
+// acc[c] (+)= sum_slab part[slab][c] in a fixed order: block = 32 columns x 8 slab ranges (blockDim = (32, 8)); range r
+// adds its contiguous share of the slabs in order, then the eight range sums are added in order
 // scale_io (optional): [0] = max |v| bound as float bits (in) -> [2] = 2^(23 - ex), [3] = q = 2^(ex - 23) as floats (out)
 __global__ void grad_slab_reduce_kernel(const double* __restrict__ part, int n_slabs, int n_cols,
                                         double* __restrict__ acc, int first, unsigned* scale_io) {
-    if (scale_io != nullptr && blockIdx.x == 0 && threadIdx.x == 0) {
+    if (scale_io != nullptr && blockIdx.x == 0 && threadIdx.x == 0 && threadIdx.y == 0) {
         const float vmax = __uint_as_float(scale_io[0]);
         int ex = -100;
         if (vmax > 0.f) {
@@ -137,11 +138,21 @@ __global__ void grad_slab_reduce_kernel(const double* __restrict__ part, int n_s
         scale_io[2] = __float_as_uint(ldexpf(1.f, 23 - ex));
         scale_io[3] = __float_as_uint(ldexpf(1.f, ex - 23));
     }
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= n_cols) return;
-    double a = first ? 0.0 : acc[c];
-    for (int sl = 0; sl < n_slabs; ++sl) a += part[(size_t)sl * n_cols + c];
-    acc[c] = a;
+    __shared__ double sh[8][32];
+    const int c = blockIdx.x * 32 + threadIdx.x;
+    const int per = (n_slabs + 7) / 8;
+    const int sl0 = threadIdx.y * per, sl1 = min(n_slabs, sl0 + per);
+    double a = 0.0;
+    if (c < n_cols)
+        for (int sl = sl0; sl < sl1; ++sl) a += part[(size_t)sl * n_cols + c];
+    sh[threadIdx.y][threadIdx.x] = a;
+    __syncthreads();
+    if (threadIdx.y == 0 && c < n_cols) {
+        double t = first ? 0.0 : acc[c];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) t += sh[r][threadIdx.x];
+        acc[c] = t;
+    }
 }
 
 // TwT[digit][me][s] (int8, k-contiguous, leading dimension ld bytes) from v[s][me]: rint(v / q) = d2 2^16 + d1 2^8 + d0
@@ -277,20 +288,48 @@ grad_tv_split_kernel(const float* __restrict__ theta, int64_t nb, int k_len, int
     if (blockIdx.x == 0 && threadIdx.x == 0) *reinterpret_cast<float*>(TwT + 3 * plane) = q;
 }
 
-// sigT[k][s] = sigma[s][k] (int8), zero for s in [nb, k_len)
-__global__ void grad_sigma_T_kernel(const int8_t* __restrict__ sigma, int64_t nb, int k_len, int N, int ld,
-                                    int8_t* __restrict__ sigT) {
-    __shared__ int8_t tile[32][33];
-    const int s0 = blockIdx.x * 32, k0 = blockIdx.y * 32;
-    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-        const int64_t s = s0 + r;
-        const int k = k0 + threadIdx.x;
-        tile[r][threadIdx.x] = (s < nb && k < N) ? sigma[s * N + k] : (int8_t)0;
+// sigT[k][s] = sigma[s][k] (int8), zero for s in [nb, k_len).  Tile = 128 samples x 128 sites per block of 256 threads:
+// a thread takes 4 sites x 4 samples (one 32-bit word from each of 4 rows), transposes the 4 x 4 bytes in registers
+// (byte permutes) and leaves 4 words, one per site, in a shared tile [site][sample word ^ site word] (XOR swizzle: both
+// the writes and the row reads are bank-conflict-free); rows of 128 samples go out as one 128-B line per warp.
+// Needs N % 4 == 0 and 4-B aligned rows for the word loads; other shapes take the byte path.
+__global__ void __launch_bounds__(256)
+grad_sigma_T_kernel(const int8_t* __restrict__ sigma, int64_t nb, int k_len, int N, int ld, int8_t* __restrict__ sigT) {
+    __shared__ unsigned tile[128][32];
+    const int64_t s0 = (int64_t)blockIdx.x * 128;
+    const int k0 = blockIdx.y * 128;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool words = (N & 3) == 0 && ((uintptr_t)sigma & 3) == 0;
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+        const int a = warp + 8 * p;                               // samples s0 + 4a .. 4a + 3, sites k0 + 4 lane .. + 3
+        unsigned r[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int64_t s = s0 + 4 * a + i;
+            const int k = k0 + 4 * lane;
+            r[i] = 0;
+            if (s < nb) {
+                if (words && k + 3 < N) r[i] = *reinterpret_cast<const unsigned*>(sigma + s * N + k);
+                else
+                    for (int b = 0; b < 4; ++b)
+                        if (k + b < N) r[i] |= (unsigned)(uint8_t)sigma[s * N + k + b] << (8 * b);
+            }
+        }
+        // 4 x 4 byte transpose: t[b] = bytes b of r[0..3]
+        const unsigned x0 = __byte_perm(r[0], r[1], 0x5140), x1 = __byte_perm(r[0], r[1], 0x7362);
+        const unsigned y0 = __byte_perm(r[2], r[3], 0x5140), y1 = __byte_perm(r[2], r[3], 0x7362);
+        tile[4 * lane + 0][a ^ lane] = __byte_perm(x0, y0, 0x5410);
+        tile[4 * lane + 1][a ^ lane] = __byte_perm(x0, y0, 0x7632);
+        tile[4 * lane + 2][a ^ lane] = __byte_perm(x1, y1, 0x5410);
+        tile[4 * lane + 3][a ^ lane] = __byte_perm(x1, y1, 0x7632);
     }
     __syncthreads();
-    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-        const int k = k0 + r, s = s0 + threadIdx.x;
-        if (k < N && s < k_len) sigT[(size_t)k * ld + s] = tile[threadIdx.x][r];
+    const int n_words = (int)min((int64_t)128, (int64_t)k_len - s0) >> 2;     // k_len is a multiple of 128: 32
+    for (int row = warp; row < 128; row += 8) {
+        const int k = k0 + row;
+        if (k < N && lane < n_words)
+            *reinterpret_cast<unsigned*>(sigT + (size_t)k * ld + s0 + 4 * lane) = tile[row][lane ^ (row >> 2)];
     }
 }
 
@@ -345,7 +384,7 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
     const float* th_in = theta_in ? theta_in : w.theta;
     grad_a_partial_kernel<<<dim3((g.N + 127) / 128, n_slabs), 128, 0, st>>>(
         sigma, nb, g.N, (const float*)eloc, stats, inv_B, cplx, (double)real_scale, w.part, cplx ? nullptr : w.absmax);
-    grad_slab_reduce_kernel<<<(2 * g.N + 127) / 128, 128, 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk,
+    grad_slab_reduce_kernel<<<(2 * g.N + 31) / 32, dim3(32, 8), 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk,
                                                                    cplx ? nullptr : w.absmax);
     if (!cplx) {
         // k_len / GRAD_SLAB == n_slabs (both round nb up to 128)
@@ -362,10 +401,10 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
             w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (int8_t*)w.TwT);
         count_launch(sigT_ready ? 6 : 7);
     }
-    grad_slab_reduce_kernel<<<(g.M_eff + 127) / 128, 128, 0, st>>>(w.part, n_slabs, g.M_eff, w.gb_acc, first_chunk,
+    grad_slab_reduce_kernel<<<(g.M_eff + 31) / 32, dim3(32, 8), 0, st>>>(w.part, n_slabs, g.M_eff, w.gb_acc, first_chunk,
                                                                    nullptr);
     if (sigT_ready == nullptr)
-        grad_sigma_T_kernel<<<dim3(k_len / 32, (g.N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, g.N, w.ld,
+        grad_sigma_T_kernel<<<dim3(k_len / 128, (g.N + 127) / 128), 256, 0, st>>>(sigma, nb, k_len, g.N, w.ld,
                                                                                      (int8_t*)w.sigT);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -376,7 +415,7 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
 // sigT[k][s] = sigma[s][k] (int8, zero padded to a multiple of 128 samples) for one chunk (what launch_gradient_chunk builds itself unless given sigT_ready)
 cudaError_t launch_sigma_T(const int8_t* sigma, int64_t nb, int N, int ld, void* sigT, cudaStream_t st) {
     const int k_len = (int)((nb + 127) / 128 * 128);
-    grad_sigma_T_kernel<<<dim3(k_len / 32, (N + 31) / 32), dim3(32, 8), 0, st>>>(sigma, nb, k_len, N, ld, (int8_t*)sigT);
+    grad_sigma_T_kernel<<<dim3(k_len / 128, (N + 127) / 128), 256, 0, st>>>(sigma, nb, k_len, N, ld, (int8_t*)sigT);
     count_launch();
     return cudaGetLastError();
 }
