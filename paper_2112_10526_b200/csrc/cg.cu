@@ -28,12 +28,13 @@ __global__ void cg_dot_partial_kernel(const float* __restrict__ x, const float* 
         part[blockIdx.x] = t;
     }
 }
+// one warp: lane l adds the partials l, l + 32, ... in order, then a butterfly over the lanes (a fixed order)
 __global__ void cg_dot_final_kernel(const double* __restrict__ part, int n_part, double* __restrict__ out) {
-    if (threadIdx.x == 0 && blockIdx.x == 0) {
-        double t = 0.0;
-        for (int i = 0; i < n_part; ++i) t += part[i];
-        *out = t;
-    }
+    double t = 0.0;
+    for (int i = threadIdx.x; i < n_part; i += 32) t += part[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (threadIdx.x == 0) *out = t;
 }
 
 // alpha = rr / pAp;  x += alpha p;  r -= alpha Ap       (alpha = 0 when pAp <= 0: converged or breakdown)

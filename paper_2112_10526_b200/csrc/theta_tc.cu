@@ -321,7 +321,7 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                         };
                         o.x = fmaf(qs, comb(j), bb.x); o.y = fmaf(qs, comb(j + 1), bb.y);
                         o.z = fmaf(qs, comb(j + 2), bb.z); o.w = fmaf(qs, comb(j + 3), bb.w);
-                        *reinterpret_cast<float4*>(out + c0 + j) = o;
+                        __stcs(reinterpret_cast<float4*>(out + c0 + j), o);
                     }
                 }
             }
