@@ -202,7 +202,21 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
     ph = nk.profile_read()
     nk.profile_enable(False)
     fused_prod_ms = ph["fused"][0] / 4                      # _time_ms runs the call 1 + 3 times
+    # ... and the log-cosh form forced (NK_FORM_LOGCOSH): the form the automatic choice falls back to
+    lplan = nk.LocalEnergyPlan(op, B, N, M, dt_code, p.chunk_size, device=sigma.device, flags=nk.NK_FORM_LOGCOSH)
+    lplan.run(sigma, W, a, b)
+    torch.cuda.synchronize()
+    nk.profile_enable(True)
+    nk.profile_read()
+    ms_log = _time_ms(torch, lambda: lplan.run(sigma, W, a, b), 3)
+    ph = nk.profile_read()
+    nk.profile_enable(False)
+    fused_log_ms = ph["fused"][0] / 4
     return {
+        "logcosh_form": {"ms_per_step": ms_log, "local_energies_per_sec": B / (ms_log * 1e-3),
+                         "fused_ms_per_step": fused_log_ms,
+                         "roofline": {"bound": "alu", "kernel": "fused_eloc_kernel<V, CPLX, PROD=false>",
+                                      "unit": "Gpair/s", "fused_ms": fused_log_ms}},
         "cuda_graph": {"ms_per_step": ms_graph, "local_energies_per_sec": B / (ms_graph * 1e-3),
                        "what": "the same nk_local_energy step replayed from a captured CUDA graph, no L2 flush"},
         "product_form": {"ms_per_step": ms_prod, "local_energies_per_sec": B / (ms_prod * 1e-3),
@@ -343,19 +357,35 @@ def run_ours(args):
     mufu_per_pair = 3 if p.complex_params else 1
     peak_pairs = N_SMS * MUFU_LANES_PER_CLK_PER_SM * sm_max * 1e6 / mufu_per_pair / 1e9       # Gpair/s at max clock
     ach_pairs = pairs / (fused_ms_per_step * 1e-3) / 1e9 if fused_ms_per_step > 0 else 0.0
+    # which form of the amplitude ratios the automatic choice took (include/nkb200.h): decides the bound of the kernel
+    form, tau_max = plan.form()
+    product = form == nk.NK_FORM_PRODUCT
+    smem_peak_pairs = N_SMS * (128 / (8 if p.complex_params else 4)) * sm_max * 1e6 / 1e9
+    if product:
+        # product form: shared-memory bandwidth binds (128 B/clk/SM; 4 B of the table per real pair)
+        bound, peak_used = "smem", smem_peak_pairs
+        basis = (f"shared memory: {N_SMS} SMs x 128 B/clk x {sm_max:.0f} MHz / 4 B of the tanh(delta) table per "
+                 f"(amplitude, hidden unit) pair (DESIGN.md 13)")
+        tname = f"fused_prod_dram_bytes_cfg{args.config}.txt"
+    else:
+        bound, peak_used = "alu", peak_pairs
+        basis = (f"MUFU pipe: {N_SMS} SMs x {MUFU_LANES_PER_CLK_PER_SM} lanes/clk x {sm_max:.0f} MHz / "
+                 f"{mufu_per_pair} MUFU per (amplitude, hidden unit) pair (DESIGN.md)")
+        tname = f"fused_dram_bytes_cfg{args.config}.txt"
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", f"fused_dram_bytes_cfg{args.config}.txt")
+    tpath = os.path.join(ROOT, "profiles", tname)
     if os.path.exists(tpath):
         try:
             traffic = float(open(tpath).read().split()[0])
         except Exception:
             traffic = None
-    roofline = {"bound": "alu", "kernel": "fused_eloc_kernel", "achieved": ach_pairs, "peak": peak_pairs,
-                "unit": "Gpair/s", "frac": ach_pairs / peak_pairs if peak_pairs else None, "traffic": traffic,
-                "peak_basis": f"MUFU pipe: {N_SMS} SMs x {MUFU_LANES_PER_CLK_PER_SM} lanes/clk x {sm_max:.0f} MHz / "
-                              f"{mufu_per_pair} MUFU per (amplitude, hidden unit) pair (DESIGN.md)",
+    roofline = {"bound": bound, "kernel": "fused_eloc_kernel<V, CPLX, PROD=%s>" % ("true" if product else "false"),
+                "form": "product" if product else "logcosh", "tau_max": tau_max,
+                "achieved": ach_pairs, "peak": peak_used,
+                "unit": "Gpair/s", "frac": ach_pairs / peak_used if peak_used else None, "traffic": traffic,
+                "peak_basis": basis,
                 "ms_per_launch": fused_ms / fused_n if fused_n else None, "launches_per_step": fused_n / args.steps,
-                "frac_at_measured_clock": (ach_pairs / (peak_pairs * clocks["sm_mhz"] / sm_max)
+                "frac_at_measured_clock": (ach_pairs / (peak_used * clocks["sm_mhz"] / sm_max)
                                            if clocks.get("sm_mhz") else None),
                 "phase_ms_per_step": {k: v[0] / args.steps for k, v in phases.items()}}
 
@@ -392,7 +422,12 @@ def run_ours(args):
             r["frac"] = r["achieved"] / peak_pairs if peak_pairs else None
         # product form: shared-memory bandwidth binds (128 B/clk/SM; 4 B per real pair, 8 B per complex pair)
         r = extras["product_form"]["roofline"]
-        r["peak"] = N_SMS * (128 / (8 if p.complex_params else 4)) * sm_max * 1e6 / 1e9
+        r["peak"] = smem_peak_pairs
+        r["achieved"] = pairs / (r.pop("fused_ms") * 1e-3) / 1e9
+        r["frac"] = r["achieved"] / r["peak"]
+        # log-cosh form: the MUFU pipe binds (1 exponential per real pair, 3 per complex pair)
+        r = extras["logcosh_form"]["roofline"]
+        r["peak"] = peak_pairs
         r["achieved"] = pairs / (r.pop("fused_ms") * 1e-3) / 1e9
         r["frac"] = r["achieved"] / r["peak"]
         line["extras"] = extras

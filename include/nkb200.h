@@ -55,8 +55,9 @@ enum nk_flags {
     NK_FLAG_MARSHALL = 1u,     /* nk_operator_create: off-diagonal Heisenberg element -2J (default +2J, Eq. (50)) */
     NK_OUT_F64 = 2u,           /* nk_rbm_logpsi: logpsi_out is double / (re,im) double instead of float */
     NK_FORM_PRODUCT = 4u,      /* nk_local_energy_ex: product-form amplitude ratios (see there) */
-    NK_CHECK_SPINS = 8u        /* nk_local_energy_ex: validate sigma in {+1,-1} first (one extra pass over sigma and one
+    NK_CHECK_SPINS = 8u,       /* nk_local_energy_ex: validate sigma in {+1,-1} first (one extra pass over sigma and one
                                   stream synchronisation); NK_ERR_BAD_SPIN before any other launch if it is not */
+    NK_FORM_LOGCOSH = 16u      /* nk_local_energy_ex: log-cosh amplitude ratios (see there) */
 };
 
 /* Static, never-NULL description of a status code. */
@@ -114,22 +115,35 @@ int nk_local_energy(nk_operator_t op, const int8_t* sigma, int64_t B, int N, int
                     const void* a, const void* b, int64_t chunk_size, void* eloc_out, void* logpsi_out,
                     double* stats_out, void* workspace, size_t workspace_bytes, nk_stream_t stream);
 
-/* nk_local_energy with flags.  flags = 0: identical to nk_local_energy (every ratio as
- * exp(ln psi' - ln psi) from stable ln cosh terms, BASELINE.json north_star (3)).  NK_FORM_PRODUCT: the same Eq. (12)
- * with each ratio written as a product,
- *   cosh(theta_j + s d_j) / cosh(theta_j) = cosh(d_j) (1 + s tanh(theta_j) tanh(d_j)),   s = +-1,
- *   psi'/psi = e^{s da} prod_j cosh(d_j) prod_j (1 + s tanh(theta_j) tanh(d_j)),
- * d the change of theta under the flip / exchange; tanh(d) and prod_j cosh(d_j) depend on the parameters only and are
- * tabulated per call, tanh(theta) once per sample, so an (amplitude, hidden unit) pair costs two FP32 operations and
- * no transcendental.  Same outputs and tolerances for |d| up to ~2 (parameters of the five configs x5); beyond, the
- * factors 1 - |tanh(theta) tanh(d)| cancel and the fp32 rounding of the two tanh shows (~5e-4 at x10).  For complex
- * parameters tanh(theta) is unbounded next to the zeros of cosh (Q18).  The log-cosh form is the better
- * conditioned one in both regimes, hence the default.
- * NK_CHECK_SPINS: validate sigma first (see enum nk_flags); the two flags may be combined. */
+/* nk_local_energy with flags.  Two evaluations of the same Eq. (12) ratios:
+ *  - NK_FORM_LOGCOSH: every ratio as exp(ln psi' - ln psi) from stable ln cosh terms (BASELINE.json north_star (3));
+ *    one exponential per (amplitude, hidden unit) pair.
+ *  - NK_FORM_PRODUCT: each ratio written as a product,
+ *      cosh(theta_j + s d_j) / cosh(theta_j) = cosh(d_j) (1 + s tanh(theta_j) tanh(d_j)),   s = +-1,
+ *      psi'/psi = e^{s da} prod_j cosh(d_j) prod_j (1 + s tanh(theta_j) tanh(d_j)),
+ *    d the change of theta under the flip / exchange; tanh(d) and prod_j cosh(d_j) depend on the parameters only and
+ *    are tabulated per call, tanh(theta) once per sample, so a pair costs two FP32 operations and no transcendental.
+ *    Same outputs and tolerances for |d| up to ~2 (parameters of the five configs x5); beyond, the factors
+ *    1 - |tanh(theta) tanh(d)| cancel and the fp32 rounding of the two tanh shows (~5e-4 at x10).  For complex
+ *    parameters tanh(theta) is unbounded next to the zeros of cosh (Q18).
+ *  - neither flag (flags = 0, and nk_local_energy): automatic.  Real parameters: both tables are packed, the device
+ *    finds tau_max = max |tanh(d)| over the table and the product form runs iff tau_max <= 0.5 (every factor then
+ *    lies in [1/2, 3/2]; its rounding error is amplified at most (1 + tau_max) / (1 - tau_max) <= 3 times), else the
+ *    log-cosh form; no host synchronisation (both kernels are launched, one returns at once).  Complex parameters:
+ *    always the log-cosh form.  The choice depends on the parameters only, never on sigma, B or chunk_size.
+ *  The two NK_FORM_* flags are mutually exclusive (NK_ERR_INVALID_ARG).
+ * NK_CHECK_SPINS: validate sigma first (see enum nk_flags); may be combined with a form flag. */
 int nk_local_energy_ex(nk_operator_t op, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
                        const void* a, const void* b, int64_t chunk_size, unsigned flags, void* eloc_out,
                        void* logpsi_out, double* stats_out, void* workspace, size_t workspace_bytes,
                        nk_stream_t stream);
+
+/* Which form the most recent automatic nk_local_energy / nk_local_energy_ex call on `workspace` took (same op, B, N,
+ * M, dtype, chunk_size as that call): *form_host = NK_FORM_PRODUCT or NK_FORM_LOGCOSH, *tau_max_host (may be NULL) =
+ * max |tanh(d)| of the table.  Reads one word of the workspace and SYNCHRONISES `stream`.  Undefined after a call
+ * with a forced form (the word is only written by automatic calls). */
+int nk_local_energy_form(nk_operator_t op, int64_t B, int N, int M, int dtype, int64_t chunk_size, const void* workspace,
+                         size_t workspace_bytes, nk_stream_t stream, int* form_host, float* tau_max_host);
 
 /* Same computation with HOST inputs and outputs (the end-to-end call): copies sigma/W/a/b host->device into
  * `scratch`, runs nk_local_energy, copies eloc / logpsi / stats back and SYNCHRONISES `stream` before returning.

@@ -125,9 +125,9 @@ static LogpsiWs carve_logpsi(void* ws, const Geometry& g, int64_t rows) {
     return w;
 }
 struct ElocWs {
-    float *Wg, *bg, *Wt, *Dtab, *theta;
+    float *Wg, *bg, *Wt, *Dtab, *Ttab, *theta;        // Dtab: log-cosh form, Ttab: product form (both when automatic)
     uint16_t *Ws, *A;
-    unsigned* absmax;
+    unsigned *absmax, *taumax;                        // taumax: max |tanh delta| of Ttab as float bits (the form gate)
     RowInfo* rows;
     size_t bytes;
 };
@@ -143,6 +143,8 @@ static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk) {
     w.Ws = c.take<uint16_t>((size_t)3 * g.M_eff * g.K_pad);
     w.A = c.take<uint16_t>((size_t)chunk * g.K_pad);
     w.absmax = c.take<unsigned>(1);
+    w.taumax = c.take<unsigned>(1);
+    w.Ttab = c.take<float>((size_t)g.n_rows_pad * g.M_eff);
     w.bytes = c.off;
     return w;
 }
@@ -703,9 +705,13 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
                        void* logpsi_out, double* stats_out, void* workspace, size_t workspace_bytes,
                        nk_stream_t stream) {
     if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0 || !W || (B > 0 && (!sigma || !eloc_out)) ||
-        (flags & ~(NK_FORM_PRODUCT | NK_CHECK_SPINS)))
+        (flags & ~(NK_FORM_PRODUCT | NK_FORM_LOGCOSH | NK_CHECK_SPINS)) ||
+        ((flags & NK_FORM_PRODUCT) && (flags & NK_FORM_LOGCOSH)))
         return NK_ERR_INVALID_ARG;
-    const bool product = (flags & NK_FORM_PRODUCT) != 0;
+    // form of the amplitude ratios: forced by a flag, else chosen on the device from the parameters (real parameters;
+    // complex ones keep the log-cosh form: tanh theta is unbounded next to the zeros of cosh)
+    const bool force_product = (flags & NK_FORM_PRODUCT) != 0;
+    const bool automatic = !force_product && !(flags & NK_FORM_LOGCOSH) && dtype == NK_F32;
     const Operator* op = (const Operator*)h;
     if (N != op->n_sites) return NK_ERR_INVALID_ARG;
     const Geometry g = make_geometry(op, N, M, dtype);
@@ -726,7 +732,8 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
     {
         Scope sc(PH_PACK, st);
         NK_CUDA(launch_pack(op, g, dtype, W, a, b, w.Wg, w.bg, w.Wt, w.Dtab, w.rows, st));
-        if (product) NK_CUDA(launch_pack_product(op, g, dtype, w.Wt, w.Dtab, w.rows, st));
+        if (force_product || automatic)
+            NK_CUDA(launch_pack_product(op, g, dtype, w.Wt, w.Ttab, w.rows, st, automatic ? w.taumax : nullptr));
         if (!use_simt_theta()) NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
     }
     const size_t esz = dtype == NK_C64 ? 8 : 4;
@@ -744,14 +751,42 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
         }
         {
             Scope sc(PH_FUSED, st);
-            NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Dtab, w.rows, (uint8_t*)eloc_out + s0 * esz,
-                                      product, st));
+            void* out = (uint8_t*)eloc_out + s0 * esz;
+            if (automatic) {           // both launches; the one on the wrong side of the gate returns at once
+                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Ttab, w.rows, out, true, st, w.taumax, 1));
+                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Dtab, w.rows, out, false, st, w.taumax, 2));
+            } else {
+                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, force_product ? w.Ttab : w.Dtab, w.rows, out,
+                                          force_product, st));
+            }
         }
     }
     if (stats_out) {
         Scope sc(PH_STATS, st);
         NK_CUDA(launch_stats(eloc_out, B, dtype, stats_out, st));
     }
+    return NK_OK;
+}
+
+int nk_local_energy_form(nk_operator_t h, int64_t B, int N, int M, int dtype, int64_t chunk_size, const void* workspace,
+                         size_t workspace_bytes, nk_stream_t stream, int* form_host, float* tau_max_host) {
+    if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0 || !form_host) return NK_ERR_INVALID_ARG;
+    const Operator* op = (const Operator*)h;
+    if (N != op->n_sites) return NK_ERR_INVALID_ARG;
+    const Geometry g = make_geometry(op, N, M, dtype);
+    if (!g.ok) return NK_ERR_UNSUPPORTED;
+    const int64_t chunk = eff_chunk(B, chunk_size);
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_eloc(nullptr, g, chunk).bytes)
+        return NK_ERR_WORKSPACE;
+    const ElocWs w = carve_eloc(const_cast<void*>(workspace), g, chunk);
+    float tau = 0.f;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == NK_F32) {                              // complex parameters never pack the product table
+        NK_CUDA(cudaMemcpyAsync(&tau, w.taumax, sizeof(float), cudaMemcpyDeviceToHost, st));
+        NK_CUDA(cudaStreamSynchronize(st));
+    }
+    *form_host = (dtype == NK_F32 && tau <= NK_FORM_TAU_MAX) ? (int)NK_FORM_PRODUCT : (int)NK_FORM_LOGCOSH;
+    if (tau_max_host) *tau_max_host = tau;
     return NK_OK;
 }
 

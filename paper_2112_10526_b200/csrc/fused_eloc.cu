@@ -45,6 +45,11 @@ struct FusedParams {
     int n_bonds, kind;
     float* eloc;
     int64_t per_cta;                         // samples per CTA (contiguous range)
+    // automatic choice of the form (api.cu): both kernels are launched, each returns at once unless the table's
+    // max |tanh delta| (float bits at *gate) is on its side of NK_FORM_TAU_MAX.  gate_mode 0: always run,
+    // 1: run iff max <= NK_FORM_TAU_MAX (product form), 2: run iff max > NK_FORM_TAU_MAX (log-cosh form)
+    const unsigned* gate;
+    int gate_mode;
 };
 
 // ---- kernel ----------------------------------------------------------------------------------------------
@@ -67,6 +72,10 @@ __device__ __forceinline__ void issue_tile(const FusedParams& p, uint32_t ring_u
 template <int V, bool CPLX, bool PROD>
 __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_kernel(const FusedParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
+    if (p.gate_mode != 0) {                                  // grid-uniform: every thread takes the same branch
+        const bool product_ok = __uint_as_float(*p.gate) <= NK_FORM_TAU_MAX;
+        if ((p.gate_mode == 1) != product_ok) return;
+    }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t stage_bytes = (uint32_t)p.tile_rows * p.M_eff * 4u;
     float* ring = reinterpret_cast<float*>(smem);
@@ -259,7 +268,7 @@ int fused_consumer_warps() { return FW; }
 
 cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
                               const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,
-                              bool product_form, cudaStream_t st) {
+                              bool product_form, cudaStream_t st, const unsigned* gate, int gate_mode) {
     if (B <= 0) return cudaSuccess;
     cudaError_t e = fused_eloc_init();
     if (e != cudaSuccess) return e;
@@ -275,6 +284,7 @@ cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, 
     p.stages = g.stages;
     p.bonds = op->d_bonds; p.colors = op->d_colors; p.Jf = op->d_Jf; p.n_bonds = op->n_bonds; p.kind = op->kind;
     p.eloc = (float*)eloc_out;
+    p.gate = gate; p.gate_mode = gate_mode;
     // one CTA per SM slot, each with an equal contiguous share of the samples (rounds of FW inside the CTA);
     // small batches use fewer CTAs so that every round is full
     const int64_t max_ctas = (int64_t)g_num_sms * g.ctas_per_sm;

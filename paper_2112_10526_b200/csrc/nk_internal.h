@@ -8,6 +8,12 @@
 
 namespace nk {
 
+// automatic form of the amplitude ratios (nk_local_energy_ex without a NK_FORM_* flag, real parameters): the product
+// form runs iff max |tanh delta| over the table is at most this — every factor 1 +- t tau then lies in [1/2, 3/2] and its
+// relative rounding error is amplified by at most (1 + tau) / (1 - tau) <= 3
+#define NK_FORM_TAU_MAX 0.5f
+
+
 // theta is kept in the fused kernel as theta_s = KAPPA * theta, so that exp(-2|theta|) = 2^(-|theta_s|)
 // is a bare MUFU.EX2 (no multiply).  KAPPA = 2 log2(e).
 constexpr float KAPPA = 2.8853900817779268f;
@@ -62,7 +68,7 @@ cudaError_t launch_pack(const Operator* op, const Geometry& g, int dtype, const 
 cudaError_t launch_pack_gemm_only(const Geometry& g, int dtype, const void* W, const void* b, float* Wg, float* bg,
                                   cudaStream_t st);
 cudaError_t launch_pack_product(const Operator* op, const Geometry& g, int dtype, const float* Wt, float* tab,
-                                RowInfo* rows, cudaStream_t st);
+                                RowInfo* rows, cudaStream_t st, unsigned* taumax_bits = nullptr);
 cudaError_t launch_pack_table(const Geometry& g, int dtype, const void* W, const void* b, const int32_t* pairs_dev,
                               int n_rows, float* Wg, float* bg, float* Wt, float* Dtab, cudaStream_t st);
 // sampler.cu : Metropolis-Hastings transitions with in-register incremental theta
@@ -134,7 +140,7 @@ cudaError_t launch_connected(const Operator* op, const int8_t* sigma, int64_t B,
 // fused_eloc.cu
 cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
                               const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,
-                              bool product_form, cudaStream_t st);
+                              bool product_form, cudaStream_t st, const unsigned* gate = nullptr, int gate_mode = 0);
 cudaError_t fused_eloc_init();   // one-time cudaFuncSetAttribute calls
 // stats.cu
 cudaError_t launch_check_spins(const int8_t* sigma, int64_t n, int* flag, cudaStream_t st);

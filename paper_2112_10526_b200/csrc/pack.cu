@@ -147,8 +147,10 @@ namespace nk {
 // Ttab [n_rows_pad][M_eff]: tau for row r and hidden unit j (complex: plane 0 = Re tau, plane 1 = Im tau),
 // d = 2 (W[:,i] - W[:,j]) (exchange) or 2 W[:,k] (flip) — the same rows as Dtab, in natural units.
 __global__ void ttab_kernel(const float* __restrict__ Wt, const int32_t* __restrict__ bonds, int kind, int n_rows,
-                            int M_pad, int M_eff, int cplx, float* __restrict__ Ttab) {
+                            int M_pad, int M_eff, int cplx, float* __restrict__ Ttab,
+                            unsigned* __restrict__ taumax_bits) {
     const int r = blockIdx.y;
+    unsigned tmax = 0;
     int i = -1, j = -1;
     if (r < n_rows) {
         if (kind == NK_HEISENBERG) { i = bonds[2 * r]; j = bonds[2 * r + 1]; }
@@ -173,6 +175,12 @@ __global__ void ttab_kernel(const float* __restrict__ Wt, const int32_t* __restr
         }
         Ttab[(size_t)r * M_eff + m] = tr;
         if (cplx) Ttab[(size_t)r * M_eff + M_pad + m] = ti;
+        tmax = max(tmax, __float_as_uint(fabsf(tr)));
+    }
+    if (taumax_bits != nullptr) {                            // max |tau| of the table (real parameters), float bits
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) tmax = max(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
+        if ((threadIdx.x & 31) == 0 && tmax) atomicMax(taumax_bits, tmax);
     }
 }
 
@@ -215,12 +223,16 @@ __global__ void rowc_kernel(const float* __restrict__ Wt, int n_rows, int M_pad,
     }
 }
 
-// Overwrites `tab` (the Dtab buffer) with Ttab and fills rows[].c2_*; call after launch_pack.
+// Fills `tab` with Ttab and rows[].c2_*; call after launch_pack.  taumax_bits (optional): max |tau| as float bits.
 cudaError_t launch_pack_product(const Operator* op, const Geometry& g, int dtype, const float* Wt, float* tab,
-                                RowInfo* rows, cudaStream_t st) {
+                                RowInfo* rows, cudaStream_t st, unsigned* taumax_bits) {
     const int cplx = dtype == NK_C64;
+    if (taumax_bits != nullptr) {
+        cudaError_t e = cudaMemsetAsync(taumax_bits, 0, sizeof(unsigned), st);
+        if (e != cudaSuccess) return e;
+    }
     dim3 gd((g.M_pad + 255) / 256, g.n_rows_pad);
-    ttab_kernel<<<gd, 256, 0, st>>>(Wt, op->d_bonds, op->kind, g.n_rows, g.M_pad, g.M_eff, cplx, tab);
+    ttab_kernel<<<gd, 256, 0, st>>>(Wt, op->d_bonds, op->kind, g.n_rows, g.M_pad, g.M_eff, cplx, tab, taumax_bits);
     rowc_kernel<<<(g.n_rows_pad + 7) / 8, 256, 0, st>>>(Wt, g.n_rows, g.M_pad, g.M_eff, cplx, rows);
     count_launch(2);
     return cudaGetLastError();

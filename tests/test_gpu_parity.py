@@ -24,10 +24,23 @@ def dev(x):
     return None if x is None else torch.from_numpy(np.ascontiguousarray(x)).to(DEV)
 
 
+# Every test of this module that goes through run_gpu runs twice: with flags = 0 (the automatic choice of the form of
+# the amplitude ratios: the product form for these parameters when they are real, include/nkb200.h) and with the
+# log-cosh form forced; tests/test_gpu_product_form.py forces the product form and checks the choice itself.
+FORM = {"flags": 0}
+
+
+@pytest.fixture(params=["auto", "logcosh"], autouse=True)
+def _form(request, nk):
+    FORM["flags"] = 0 if request.param == "auto" else nk.NK_FORM_LOGCOSH
+    yield
+    FORM["flags"] = 0
+
+
 def run_gpu(nk, p, chunk=None, flags=0, a=True, b=True):
     op = nk.Operator.from_problem(p, flags)
     e, lp, st = nk.local_energy(op, dev(p.sigma), dev(p.W), dev(p.a) if a else None, dev(p.b) if b else None,
-                                chunk_size=p.chunk_size if chunk is None else chunk)
+                                chunk_size=p.chunk_size if chunk is None else chunk, flags=FORM["flags"])
     torch.cuda.synchronize()
     out = e.cpu().numpy(), lp.cpu().numpy(), st.cpu().numpy()
     op.close()

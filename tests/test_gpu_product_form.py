@@ -50,7 +50,7 @@ def test_product_form_full_size_sampled(nk, cfg):
     assert_eloc(e[rows], e_ref)
     assert np.all(np.isfinite(e.view(np.float32))) and st[3] == B
     # both forms agree over the whole batch far inside the tolerance
-    e_log, _, _ = run_prod(nk, p, form=0)
+    e_log, _, _ = run_prod(nk, p, form=nk.NK_FORM_LOGCOSH)
     rel = np.abs(e.astype(np.complex128) - e_log.astype(np.complex128)) / (np.abs(e_log) + 1e-6)
     assert rel.max() < 5e-5, rel.max()
 
@@ -103,3 +103,47 @@ def test_product_form_chunking_and_bad_flags(nk):
         assert np.array_equal(e, ref) and np.array_equal(st, st0)
     with pytest.raises(nk.NkError):
         run_prod(nk, p, form=64)
+
+
+def _plan_run(nk, p, flags, scale=1.0):
+    op = nk.Operator.from_problem(p)
+    plan = nk.LocalEnergyPlan(op, p.n_samples, p.n_sites, p.n_hidden, nk.NK_C64 if p.complex_params else nk.NK_F32,
+                              p.chunk_size, device="cuda", flags=flags)
+    W = dev((p.W * scale).astype(p.W.dtype))
+    e, lp, st = plan.run(dev(p.sigma), W, dev(p.a), dev(p.b))
+    torch.cuda.synchronize()
+    return plan, e.cpu().numpy().copy(), op
+
+
+def test_automatic_form_follows_the_parameters(nk):
+    """flags = 0: the device picks the product form iff max |tanh delta| <= 0.5 (include/nkb200.h) and the result is
+    bit-identical to the forced form it picked; the choice depends on the parameters only."""
+    p = inp.make_config(2, n_samples=300)
+    delta = 2.0 * (p.W[:, p.bonds[:, 0]] - p.W[:, p.bonds[:, 1]])
+    tau_ref = float(np.abs(np.tanh(delta.astype(np.float64))).max())
+    for scale, want in ((0.5, "product"), (4.0, "logcosh")):
+        tau_s = float(np.abs(np.tanh(scale * delta.astype(np.float64))).max())
+        assert (tau_s <= 0.5) == (want == "product")
+        plan, e_auto, op = _plan_run(nk, p, 0, scale)
+        form, tau = plan.form()
+        assert form == (nk.NK_FORM_PRODUCT if want == "product" else nk.NK_FORM_LOGCOSH)
+        assert abs(tau - tau_s) < 1e-5
+        _, e_forced, op2 = _plan_run(nk, p, form, scale)
+        assert np.array_equal(e_auto, e_forced)
+        _, e_other, op3 = _plan_run(nk, p, nk.NK_FORM_PRODUCT if want == "logcosh" else nk.NK_FORM_LOGCOSH, scale)
+        assert not np.array_equal(e_auto, e_other)             # the two kernels do differ in the last digits
+        e_ref, _ = orc.local_energy(p.kind, p.sigma, p.bonds, p.colors, p.J, p.h, (p.W * scale).astype(p.W.dtype), p.a, p.b)
+        assert_eloc(e_auto, e_ref)
+        for o in (op, op2, op3):
+            o.close()
+    assert 0.5 < tau_ref < 0.52                                  # config 2 itself sits just above the gate
+
+
+def test_automatic_form_is_logcosh_for_complex_parameters_and_flags_exclude_each_other(nk):
+    p = inp.make_config(4, n_samples=64)
+    plan, e_auto, op = _plan_run(nk, p, 0)
+    _, e_log, op2 = _plan_run(nk, p, nk.NK_FORM_LOGCOSH)
+    assert np.array_equal(e_auto, e_log)
+    with pytest.raises(nk.NkError, match="NK_ERR_INVALID_ARG"):
+        nk.local_energy(op, dev(p.sigma), dev(p.W), dev(p.a), dev(p.b), flags=nk.NK_FORM_PRODUCT | nk.NK_FORM_LOGCOSH)
+    op.close(); op2.close()
