@@ -389,6 +389,24 @@ def run_ours(args):
                                            if clocks.get("sm_mhz") else None),
                 "phase_ms_per_step": {k: v[0] / args.steps for k, v in phases.items()}}
 
+    # theta contraction: second roofline, tensor pipe.  Algorithmic work 2 B M N flop per step (x 2
+    # planes for complex W); the kernel executes three int8 digit-plane MMAs per product (the exact fixed-point
+    # split), so the tensor pipe sees 3 x that in int8 operations.  Peak: measured dense bf16 (burst: the kernel is
+    # 31 us between kernels that leave the tensor pipe idle) x the guide's nominal int8 : bf16 ratio of 2.
+    th_ms, th_n = phases["theta"]
+    bf16_peak = float(peaks.get("bf16_tflops") or 0.0)
+    alg_flop = 2.0 * B * M * N * (2 if p.complex_params else 1)
+    if th_ms > 0 and bf16_peak > 0:
+        th_s = th_ms / args.steps * 1e-3
+        roofline["theta"] = {
+            "bound": "tensor", "kernel": "theta_tc_kernel<I8> (tcgen05 kind::i8, 3 digit planes)",
+            "achieved": 3.0 * alg_flop / th_s / 1e12, "peak": 2.0 * bf16_peak, "unit": "TOP/s (int8, executed)",
+            "frac": 3.0 * alg_flop / th_s / 1e12 / (2.0 * bf16_peak),
+            "algorithmic_tflops": alg_flop / th_s / 1e12,
+            "frac_of_tf32_peak_algorithmic": alg_flop / th_s / 1e12 / (0.5 * bf16_peak),
+            "peak_basis": "MEASURED_PEAKS.json bf16_tflops (burst) x 2 (nominal int8 : bf16); tf32 = bf16 / 2",
+            "ms_per_launch": th_ms / th_n if th_n else None, "launches_per_step": th_n / args.steps}
+
     # CPU baseline: the oracle as it stands on a bounded sample worth ~12 s of host time (a short probe sizes it)
     n0 = min(ORACLE_ROWS_PER_STEP[args.config], B)
     rate0, t0 = oracle_rate(p, n0)

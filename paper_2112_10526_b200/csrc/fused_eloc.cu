@@ -130,6 +130,7 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
         // e_u*: terms identical on all lanes (single rows); e_h*: half-warp-specific terms (paired rows)
         float diag = 0.f, e_ure = 0.f, e_uim = 0.f, e_hre = 0.f, e_him = 0.f;
         bool pending = false;                         // warp-uniform: one row waits for a partner
+        int pend_lane = -1;                           // real product form: the waiting row's lane in the current tile
         typename std::conditional<CPLX, RowPartC, RowPartR>::type pend;
         if (p.kind == NK_ISING) {
             for (int b = lane; b < p.n_bonds; b += 32) {
@@ -155,11 +156,38 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
                 }
             }
             unsigned mask = __ballot_sync(0xffffffffu, active);
+            // real product form: lane r keeps its row's factor c_r 2^(s a2 + c2) and adds the row's term itself, so
+            // the row scalars are never broadcast; the sign of s travels in a ballot
+            unsigned negm = 0;
+            float ce = 0.f;
+            if constexpr (PROD && !CPLX) {
+                negm = __ballot_sync(0xffffffffu, sgn < 0.f);
+                ce = coef * ex2_approx(fmaf(sgn, a2re, c2re));
+            }
             mbar_wait(full0 + 8 * stage, parity);
             const float* tile = ring + (size_t)stage * (stage_bytes / 4);
             while (mask) {
                 const int r = __ffs(mask) - 1;
                 mask &= mask - 1;
+                if constexpr (PROD && !CPLX) {
+                    const float* trow = tile + (size_t)r * p.M_eff;
+                    const float pr = ((negm >> r) & 1u) ? st.template partial_s<true>(trow, lane)
+                                                        : st.template partial_s<false>(trow, lane);
+                    if (pending) {
+                        // lower half-warp reduces the waiting row, upper half this one
+                        const bool up = (lane & 16) != 0;
+                        float rk = up ? pr : pend.r;
+                        rk *= __shfl_xor_sync(0xffffffffu, up ? pend.r : pr, 16);
+#pragma unroll
+                        for (int o = 8; o > 0; o >>= 1) rk *= __shfl_xor_sync(0xffffffffu, rk, o);
+                        const float rA = __shfl_sync(0xffffffffu, rk, 0), rB = __shfl_sync(0xffffffffu, rk, 16);
+                        if (pend_lane >= 0) { if (lane == pend_lane) e_hre = fmaf(ce, rA, e_hre); }
+                        else if (lane == 0) e_hre = fmaf(pend.coef, rA, e_hre);
+                        if (lane == r) e_hre = fmaf(ce, rB, e_hre);
+                        pending = false;
+                    } else { pend.r = pr; pend_lane = r; pending = true; }
+                    continue;
+                }
                 const float s = __shfl_sync(0xffffffffu, sgn, r);
                 const float c = __shfl_sync(0xffffffffu, coef, r);
                 const float ar = __shfl_sync(0xffffffffu, a2re, r);
@@ -189,6 +217,10 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
                     } else { pend = cur; pending = true; }
                 }
             }
+            if constexpr (PROD && !CPLX) {
+                // a row waiting across the tile boundary takes its factor along (its lane's ce is about to change)
+                if (pending && pend_lane >= 0) { pend.coef = __shfl_sync(0xffffffffu, ce, pend_lane); pend_lane = -1; }
+            }
             __syncwarp();
             if (lane == 0) {
                 // release the stage; the last of the FW warps refills it with tile g + stages
@@ -206,11 +238,13 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
             if (++stage == p.stages) { stage = 0; parity ^= 1; }
         }
         if (pending) {
-            if constexpr (!CPLX) e_ure = PROD ? finish_single_prod(pend) : finish_single(pend);
+            if constexpr (PROD && !CPLX) e_ure = pend.coef * warp_prod_f(pend.r);   // pend_lane = -1 here
+            else if constexpr (!CPLX) e_ure = finish_single(pend);
             else if constexpr (PROD) finish_single_prod_c(pend, e_ure, e_uim);
             else finish_single_c(pend, e_ure, e_uim);
         }
-        e_hre += __shfl_xor_sync(0xffffffffu, e_hre, 16);          // row-A half + row-B half
+        if constexpr (PROD && !CPLX) e_hre = warp_sum_f(e_hre);    // one term per row, on the row's lane
+        else e_hre += __shfl_xor_sync(0xffffffffu, e_hre, 16);     // row-A half + row-B half
         if constexpr (CPLX) e_him += __shfl_xor_sync(0xffffffffu, e_him, 16);
         diag = warp_sum_f(diag);
         if (valid && lane == 0) {
