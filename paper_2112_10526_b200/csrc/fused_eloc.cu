@@ -130,7 +130,9 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
         // e_u*: terms identical on all lanes (single rows); e_h*: half-warp-specific terms (paired rows)
         float diag = 0.f, e_ure = 0.f, e_uim = 0.f, e_hre = 0.f, e_him = 0.f;
         bool pending = false;                         // warp-uniform: one row waits for a partner
-        int pend_lane = -1;                           // real product form: the waiting row's lane in the current tile
+        // real product form: the row pair whose reduction is deferred by one step (products per lane, factors uniform;
+        // the neutral start contributes 0)
+        float d_a = 1.f, d_b = 1.f, d_fa = 0.f, d_fb = 0.f;
         typename std::conditional<CPLX, RowPartC, RowPartR>::type pend;
         if (p.kind == NK_ISING) {
             for (int b = lane; b < p.n_bonds; b += 32) {
@@ -170,22 +172,35 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
                 const int r = __ffs(mask) - 1;
                 mask &= mask - 1;
                 if constexpr (PROD && !CPLX) {
+                    // rows are reduced in pairs, one step late: the butterfly of the pair completed before runs inside
+                    // the next row's loads (partial_s_retire).  f: the row's factor, broadcast from its lane now, while
+                    // the lanes still hold this tile's factors
                     const float* trow = tile + (size_t)r * p.M_eff;
-                    const float pr = ((negm >> r) & 1u) ? st.template partial_s<true>(trow, lane)
-                                                        : st.template partial_s<false>(trow, lane);
-                    if (pending) {
-                        // lower half-warp reduces the waiting row, upper half this one
-                        const bool up = (lane & 16) != 0;
-                        float rk = up ? pr : pend.r;
-                        rk *= __shfl_xor_sync(0xffffffffu, up ? pend.r : pr, 16);
-#pragma unroll
-                        for (int o = 8; o > 0; o >>= 1) rk *= __shfl_xor_sync(0xffffffffu, rk, o);
-                        const float rA = __shfl_sync(0xffffffffu, rk, 0), rB = __shfl_sync(0xffffffffu, rk, 16);
-                        if (pend_lane >= 0) { if (lane == pend_lane) e_hre = fmaf(ce, rA, e_hre); }
-                        else if (lane == 0) e_hre = fmaf(pend.coef, rA, e_hre);
-                        if (lane == r) e_hre = fmaf(ce, rB, e_hre);
-                        pending = false;
-                    } else { pend.r = pr; pend_lane = r; pending = true; }
+                    const bool neg = ((negm >> r) & 1u) != 0;
+                    const float f = __shfl_sync(0xffffffffu, ce, r);
+                    if (pending || mask != 0u) {
+                        float rk;
+                        const float pr = neg ? st.template partial_s_retire<true>(trow, lane, d_a, d_b, rk)
+                                             : st.template partial_s_retire<false>(trow, lane, d_a, d_b, rk);
+                        e_hre = fmaf((lane & 16) ? d_fb : d_fa, rk, e_hre);
+                        if (pending) { d_a = pend.r; d_fa = pend.coef; pending = false; }
+                        else {
+                            d_a = pr; d_fa = f;
+                            const int r2 = __ffs(mask) - 1;
+                            mask &= mask - 1;
+                            const float* trow2 = tile + (size_t)r2 * p.M_eff;
+                            const float f2 = __shfl_sync(0xffffffffu, ce, r2);
+                            const float pr2 = ((negm >> r2) & 1u) ? st.template partial_s<true>(trow2, lane)
+                                                                  : st.template partial_s<false>(trow2, lane);
+                            d_b = pr2; d_fb = f2;
+                            continue;
+                        }
+                        d_b = pr; d_fb = f;
+                    } else {                              // last row of the tile, no partner yet
+                        pend.r = neg ? st.template partial_s<true>(trow, lane) : st.template partial_s<false>(trow, lane);
+                        pend.coef = f;
+                        pending = true;
+                    }
                     continue;
                 }
                 const float s = __shfl_sync(0xffffffffu, sgn, r);
@@ -217,10 +232,6 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
                     } else { pend = cur; pending = true; }
                 }
             }
-            if constexpr (PROD && !CPLX) {
-                // a row waiting across the tile boundary takes its factor along (its lane's ce is about to change)
-                if (pending && pend_lane >= 0) { pend.coef = __shfl_sync(0xffffffffu, ce, pend_lane); pend_lane = -1; }
-            }
             __syncwarp();
             if (lane == 0) {
                 // release the stage; the last of the FW warps refills it with tile g + stages
@@ -238,13 +249,20 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
             if (++stage == p.stages) { stage = 0; parity ^= 1; }
         }
         if (pending) {
-            if constexpr (PROD && !CPLX) e_ure = pend.coef * warp_prod_f(pend.r);   // pend_lane = -1 here
+            if constexpr (PROD && !CPLX) e_ure = pend.coef * warp_prod_f(pend.r);
             else if constexpr (!CPLX) e_ure = finish_single(pend);
             else if constexpr (PROD) finish_single_prod_c(pend, e_ure, e_uim);
             else finish_single_c(pend, e_ure, e_uim);
         }
-        if constexpr (PROD && !CPLX) e_hre = warp_sum_f(e_hre);    // one term per row, on the row's lane
-        else e_hre += __shfl_xor_sync(0xffffffffu, e_hre, 16);     // row-A half + row-B half
+        if constexpr (PROD && !CPLX) {                             // the pair still deferred
+            const bool up = (lane & 16) != 0;
+            float k = up ? d_b : d_a;
+            k *= __shfl_xor_sync(0xffffffffu, up ? d_a : d_b, 16);
+#pragma unroll
+            for (int o = 8; o > 0; o >>= 1) k *= __shfl_xor_sync(0xffffffffu, k, o);
+            e_hre = fmaf(up ? d_fb : d_fa, k, e_hre);
+        }
+        e_hre += __shfl_xor_sync(0xffffffffu, e_hre, 16);          // row-A half + row-B half
         if constexpr (CPLX) e_him += __shfl_xor_sync(0xffffffffu, e_him, 16);
         diag = warp_sum_f(diag);
         if (valid && lane == 0) {

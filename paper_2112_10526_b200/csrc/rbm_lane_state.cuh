@@ -258,6 +258,33 @@ struct ProdRealState {
         }
         return (p0 * p1) * (p2 * p3);
     }
+    // partial_s of one row and, in the same basic block, the butterfly of the row pair (da, db) that was completed
+    // one step earlier: the shuffles of that reduction (a dependent chain of five) issue between this row's loads and
+    // the multiplications that wait for them, instead of leaving the warp without loads in flight.  rk: the product
+    // of row a on the lower half-warp, of row b on the upper.
+    template <bool NEG>
+    __device__ __forceinline__ float partial_s_retire(const float* __restrict__ trow, int lane, float da, float db,
+                                                      float& rk) const {
+        const bool up = (lane & 16) != 0;
+        float k = up ? db : da;
+        k *= __shfl_xor_sync(0xffffffffu, up ? da : db, 16);
+        float p0 = 1.f, p1 = 1.f, p2 = 1.f, p3 = 1.f;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            const float4 d = *reinterpret_cast<const float4*>(trow + (v * 32 + lane) * 4);
+            const float4 a = t[v];
+            p0 *= fmaf(NEG ? -a.x : a.x, d.x, 1.f);
+            p1 *= fmaf(NEG ? -a.y : a.y, d.y, 1.f);
+            p2 *= fmaf(NEG ? -a.z : a.z, d.z, 1.f);
+            p3 *= fmaf(NEG ? -a.w : a.w, d.w, 1.f);
+            if (v == V / 4) k *= __shfl_xor_sync(0xffffffffu, k, 8);
+            if (v == V / 2) k *= __shfl_xor_sync(0xffffffffu, k, 4);
+            if (v == (3 * V) / 4) k *= __shfl_xor_sync(0xffffffffu, k, 2);
+        }
+        k *= __shfl_xor_sync(0xffffffffu, k, 1);
+        rk = k;
+        return (p0 * p1) * (p2 * p3);
+    }
     __device__ __forceinline__ void partial(const float* __restrict__ trow, int lane, float s, float& r,
                                             float& acc) const {
         r = (s > 0.f) ? partial_s<false>(trow, lane) : partial_s<true>(trow, lane);
