@@ -454,60 +454,6 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def run_table5(args):
-    """Context only: the workload of the paper's Table 5 (L2033-2043) — one whole VMC step with SR for
-    the 1D transverse-field Ising chain L = 64 (J = 1, h = 1, PBC), complex RBM alpha = 1, 2^14 samples from 2^10
-    chains, conjugate-gradient solve — through this library's calls.  The paper's 3.9 s (one RTX 3090, NetKet,
-    QGTJacobianDense + CG) includes JAX dispatch and a different QGT algorithm; this is not the graded metric."""
-    import torch
-
-    import paper_2112_10526_b200 as nk
-    from paper_2112_10526_b200 import inputs as inp
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device")
-    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
-    torch.cuda.set_device(dev)
-    nk.load()
-    L, n_chains, n_samples = 64, 1 << 10, 1 << 14
-    p = inp.make_problem(inp.KIND_ISING, "chain", L, L, n_chains, seed=64, complex_params=True, scale=0.01, h=1.0)
-    op = nk.Operator.from_problem(p)
-    chains = torch.from_numpy(p.sigma).to(dev)
-    W, a, b = (torch.from_numpy(x).to(dev) for x in (p.W, p.a, p.b))
-    sigma = torch.empty((n_samples, L), dtype=torch.int8, device=dev)
-    per_chain = n_samples // n_chains
-    state = {"t": 0, "cg": 0, "e": 0.0}
-
-    def step():
-        for k in range(per_chain):                       # one sweep (N transitions) between recorded samples
-            nk.metropolis_sample(chains, W, a, b, rule=nk.NK_RULE_LOCAL, n_steps=L, seed=1, step_offset=state["t"])
-            state["t"] += L
-            sigma[k * n_chains:(k + 1) * n_chains].copy_(chains)
-        eloc, _, stats = nk.local_energy(op, sigma, W, a, b)
-        ga, gb, gW = nk.energy_gradient(sigma, W, b, eloc, stats)
-        (da, db, dW), iters, _ = nk.sr_solve(sigma, W, b, ga, gb, gW, diag_shift=0.01, tol=1e-5, max_iter=1000)
-        W.sub_(0.01 * dW); a.sub_(0.01 * da); b.sub_(0.01 * db)
-        state["cg"] += iters
-        state["e"] = stats[0].item()
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    torch.cuda.synchronize()
-    state["cg"] = 0
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        step()
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / args.steps
-    print(json.dumps({"workload": "paper Table 5: TFIM 1D L=64 h=1, complex RBM alpha=1, 2^14 samples, 2^10 chains, "
-                                  "SR with CG (tol 1e-5, diag_shift 0.01)", "metric": "vmc_step_ms", "value": ms,
-                      "unit": "ms per VMC step (sampling + local energies + gradient + SR solve + update)",
-                      "cg_iterations_per_step": state["cg"] / args.steps, "energy_per_site": state["e"] / L,
-                      "steps": args.steps, "context": "paper: 3.9 s on one RTX 3090 (NetKet 3, Table 5); not the graded metric",
-                      "higher_is_better": False}), flush=True)
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -516,11 +462,7 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the sampler / gradient timings")
-    ap.add_argument("--table5", action="store_true", help="context run: the paper's Table 5 VMC step (not the metric)")
     args = ap.parse_args()
-    if args.table5:
-        run_table5(args)
-        return
     if args.impl == "reference":
         run_reference(args)
     else:

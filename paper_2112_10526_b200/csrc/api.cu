@@ -77,12 +77,6 @@ Geometry make_geometry(const Operator* op, int N, int M, int dtype) {
             g.stages = (int)((budget - fixed) / ((size_t)tr * row_bytes));
             if (g.stages > 4) g.stages = 4;
         }
-        if (const char* e = std::getenv("NK_STAGES")) {                     // experiment knob
-            g.stages = atoi(e) < 2 ? 2 : atoi(e);
-            tr = (int)((budget - fixed) / (g.stages * row_bytes));
-            if (tr > 32) tr = 32;
-            if (tr < 1) { g.stages = 2; tr = (int)((budget - fixed) / (g.stages * row_bytes)); }
-        }
         g.tile_rows = tr;
     }
     g.n_tiles = (g.n_rows + g.tile_rows - 1) / g.tile_rows;
@@ -217,14 +211,8 @@ static QgtWs carve_qgt(void* ws, const Geometry& g, int64_t B, int64_t chunk, in
     return w;
 }
 
-// NK_THETA_SIMT=1 selects the FP32 SIMT contraction (debugging aid); default is the tcgen05 path.
-static bool use_simt_theta() {
-    static const bool v = [] { const char* e = std::getenv("NK_THETA_SIMT"); return e && e[0] == '1'; }();
-    return v;
-}
-static cudaError_t run_theta(const Geometry& g, const int8_t* sg, int64_t nb, const float* Wg, const float* bg,
+static cudaError_t run_theta(const Geometry& g, const int8_t* sg, int64_t nb, const float* /*Wg*/, const float* bg,
                              const uint16_t* Ws, uint16_t* A, float* theta, cudaStream_t st) {
-    if (use_simt_theta()) return launch_theta_gemm(sg, nb, g.N, g.M_eff, Wg, bg, theta, st);
     return launch_theta_tc(sg, nb, g.N, g.M_eff, g.K_pad, Ws, A, bg, theta, st);
 }
 
@@ -349,7 +337,7 @@ int nk_rbm_logpsi(const int8_t* sigma, int64_t B, int N, int M, int dtype, const
     cudaStream_t st = (cudaStream_t)stream;
     const LogpsiWs w = carve_logpsi(workspace, g, B);
     NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.Wg, w.bg, st));
-    if (!use_simt_theta()) NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
+    NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
     NK_CUDA(run_theta(g, sigma, B, w.Wg, w.bg, w.Ws, w.A, w.theta, st));
     NK_CUDA(launch_logpsi(sigma, B, g, dtype, w.theta, a, logpsi_out, (flags & NK_OUT_F64) != 0, theta_out, st));
     return NK_OK;
@@ -734,7 +722,7 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
         NK_CUDA(launch_pack(op, g, dtype, W, a, b, w.Wg, w.bg, w.Wt, w.Dtab, w.rows, st));
         if (force_product || automatic)
             NK_CUDA(launch_pack_product(op, g, dtype, w.Wt, w.Ttab, w.rows, st, automatic ? w.taumax : nullptr));
-        if (!use_simt_theta()) NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
+        NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
     }
     const size_t esz = dtype == NK_C64 ? 8 : 4;
     for (int64_t s0 = 0; s0 < B; s0 += chunk) {

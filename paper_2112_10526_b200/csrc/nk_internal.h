@@ -81,9 +81,6 @@ struct SamplerArgs {
 };
 cudaError_t launch_metropolis(const Geometry& g, int dtype, int8_t* sigma, int64_t nb, const float* theta,
                               const float* Dtab, const SamplerArgs& sa, int32_t* accepted, cudaStream_t st);
-// theta_gemm.cu : theta[s][m] = bg[m] + sum_k sigma[s][k] Wg[m][k]
-cudaError_t launch_theta_gemm(const int8_t* sigma, int64_t B, int N, int M_eff, const float* Wg, const float* bg,
-                              float* theta, cudaStream_t st);
 // theta_tc.cu : the same contraction on tcgen05 tensor cores (kind::i8, three int8 digit planes of W, three int32
 // TMEM accumulators); Ws = the planes + scale, A = scratch for a padded int8 copy of the spins when N % 128 != 0
 cudaError_t theta_tc_init();

@@ -395,12 +395,14 @@ cudaError_t theta_tc_init() {
         sms > 0)
         g_num_sms = sms;
     // cluster shape: 2 x 1 (measured best at 65536 x 2048 x 1024: 374 us against 390 for 1 x 1, 394 for 2 x 2, 403 for
-    // 4 x 1 and 4 x 2) unless NK_TC_CLUSTER (an experiment knob: "1x1", "2x1", "2x2", "4x1", "4x2") says otherwise or the
-    // device cannot co-schedule such clusters
+    // 4 x 1 and 4 x 2) unless the device cannot co-schedule such clusters; NK_TC_CLUSTER ("1x1", "2x1", "2x2", "4x1",
+    // "4x2") overrides it in -DNK_DEBUG builds only
     int want_m = 2, want_n = 1;
+#ifdef NK_DEBUG
     if (const char* v = getenv("NK_TC_CLUSTER")) {
         if (v[0] >= '1' && v[0] <= '4' && v[1] == 'x' && v[2] >= '1' && v[2] <= '2') { want_m = v[0] - '0'; want_n = v[2] - '0'; }
     }
+#endif
     int n = 0;
     g_cm = g_cn = 1;
     if (want_m == 4 && want_n == 2 && tc_prepare<4, 2>(&n) == cudaSuccess && n > 0) { g_cm = 4; g_cn = 2; }
