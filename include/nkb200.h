@@ -57,7 +57,9 @@ enum nk_flags {
     NK_FORM_PRODUCT = 4u,      /* nk_local_energy_ex: product-form amplitude ratios (see there) */
     NK_CHECK_SPINS = 8u,       /* nk_local_energy_ex: validate sigma in {+1,-1} first (one extra pass over sigma and one
                                   stream synchronisation); NK_ERR_BAD_SPIN before any other launch if it is not */
-    NK_FORM_LOGCOSH = 16u      /* nk_local_energy_ex: log-cosh amplitude ratios (see there) */
+    NK_FORM_LOGCOSH = 16u,     /* nk_local_energy_ex: log-cosh amplitude ratios (see there) */
+    NK_FORM_SERIES = 32u       /* nk_local_energy_ex: product form with the logarithm expanded into a short series of
+                                  tensor-core GEMMs (see there); real parameters only */
 };
 
 /* Static, never-NULL description of a status code. */
@@ -126,12 +128,22 @@ int nk_local_energy(nk_operator_t op, const int8_t* sigma, int64_t B, int N, int
  *    Same outputs and tolerances for |d| up to ~2 (parameters of the five configs x5); beyond, the factors
  *    1 - |tanh(theta) tanh(d)| cancel and the fp32 rounding of the two tanh shows (~5e-4 at x10).  For complex
  *    parameters tanh(theta) is unbounded next to the zeros of cosh (Q18).
- *  - neither flag (flags = 0, and nk_local_energy): automatic.  Real parameters: both tables are packed, the device
- *    finds tau_max = max |tanh(d)| over the table and the product form runs iff tau_max <= 0.5 (every factor then
- *    lies in [1/2, 3/2]; its rounding error is amplified at most (1 + tau_max) / (1 - tau_max) <= 3 times), else the
- *    log-cosh form; no host synchronisation (both kernels are launched, one returns at once).  Complex parameters:
- *    always the log-cosh form.  The choice depends on the parameters only, never on sigma, B or chunk_size.
- *  The two NK_FORM_* flags are mutually exclusive (NK_ERR_INVALID_ARG).
+ *  - NK_FORM_SERIES: the product form with its logarithm expanded,
+ *      ln prod_j (1 + s t_j tau_j) = sum_k ((-1)^(k+1) / k) s^k sum_j t_j^k tau_j^k,   t = tanh(theta), tau = tanh(d),
+ *    so that the log-ratios of a chunk against all table rows are a short series of GEMMs over the hidden units, run
+ *    on the tensor cores (tcgen05, fp16 hi/lo split of the k = 1 term, fp32 accumulation) with the exponential, the
+ *    matrix element, the spin masks and the sum over connected configurations fused into the epilogue.  The series is
+ *    cut after K <= 6 terms, K chosen on the device so that the remainder bound
+ *    max_rows sum_j |tau_j|^(K+1) / ((K+1)(1 - tau_max)) <= 1e-5 (a property of the parameters).  Real parameters,
+ *    M_pad >= 256 and >= 128 table rows only (else NK_ERR_UNSUPPORTED when forced); forced, it uses K = 6 when the
+ *    bound cannot be met.
+ *  - no form flag (flags = 0, and nk_local_energy): automatic.  Real parameters: the tables are packed, the device
+ *    finds tau_max = max |tanh(d)| over the table; the series form runs if the sizes allow it, tau_max <= 0.5 and its
+ *    bound can be met; else the product form iff tau_max <= 0.5 (every factor then lies in [1/2, 3/2]; its rounding
+ *    error is amplified at most (1 + tau_max) / (1 - tau_max) <= 3 times); else the log-cosh form.  No host
+ *    synchronisation (every kernel is launched, those on the wrong side of the gates return at once).  Complex
+ *    parameters: always the log-cosh form.  The choice depends on the parameters only, never on sigma, B or chunk_size.
+ *  The NK_FORM_* flags are mutually exclusive (NK_ERR_INVALID_ARG).
  * NK_CHECK_SPINS: validate sigma first (see enum nk_flags); may be combined with a form flag. */
 int nk_local_energy_ex(nk_operator_t op, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
                        const void* a, const void* b, int64_t chunk_size, unsigned flags, void* eloc_out,
@@ -139,11 +151,13 @@ int nk_local_energy_ex(nk_operator_t op, const int8_t* sigma, int64_t B, int N, 
                        nk_stream_t stream);
 
 /* Which form the most recent automatic nk_local_energy / nk_local_energy_ex call on `workspace` took (same op, B, N,
- * M, dtype, chunk_size as that call): *form_host = NK_FORM_PRODUCT or NK_FORM_LOGCOSH, *tau_max_host (may be NULL) =
- * max |tanh(d)| of the table.  Reads one word of the workspace and SYNCHRONISES `stream`.  Undefined after a call
- * with a forced form (the word is only written by automatic calls). */
+ * M, dtype, chunk_size as that call): *form_host = NK_FORM_SERIES, NK_FORM_PRODUCT or NK_FORM_LOGCOSH, *tau_max_host
+ * (may be NULL) = max |tanh(d)| of the table, *series_terms_host (may be NULL) = the K of the series form (0 if it did
+ * not run).  Reads two words of the workspace and SYNCHRONISES `stream`.  Undefined after a call with a forced
+ * product or log-cosh form (the words are only written by automatic and forced-series calls). */
 int nk_local_energy_form(nk_operator_t op, int64_t B, int N, int M, int dtype, int64_t chunk_size, const void* workspace,
-                         size_t workspace_bytes, nk_stream_t stream, int* form_host, float* tau_max_host);
+                         size_t workspace_bytes, nk_stream_t stream, int* form_host, float* tau_max_host,
+                         int* series_terms_host);
 
 /* Same computation with HOST inputs and outputs (the end-to-end call): copies sigma/W/a/b host->device into
  * `scratch`, runs nk_local_energy, copies eloc / logpsi / stats back and SYNCHRONISES `stream` before returning.

@@ -12,11 +12,11 @@ import numpy as np
 
 __all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host", "energy_gradient",
            "qgt_matvec", "sr_solve", "rbmsymm_expand", "rbmsymm_reduce_gradient", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "allreduce_gradient", "LIB_PATH",
-           "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "NK_FORM_PRODUCT", "NK_CHECK_SPINS", "NK_FORM_LOGCOSH", "EXPORTS"]
+           "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "NK_FORM_PRODUCT", "NK_CHECK_SPINS", "NK_FORM_LOGCOSH", "NK_FORM_SERIES", "EXPORTS"]
 
 NK_HEISENBERG, NK_ISING = 0, 1
 NK_F32, NK_C64 = 0, 1
-NK_FLAG_MARSHALL, NK_OUT_F64, NK_FORM_PRODUCT, NK_CHECK_SPINS, NK_FORM_LOGCOSH = 1, 2, 4, 8, 16
+NK_FLAG_MARSHALL, NK_OUT_F64, NK_FORM_PRODUCT, NK_CHECK_SPINS, NK_FORM_LOGCOSH, NK_FORM_SERIES = 1, 2, 4, 8, 16, 32
 NK_RULE_LOCAL, NK_RULE_EXCHANGE = 0, 1
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libnkb200.so")
 
@@ -37,7 +37,7 @@ EXPORTS = {
     "nk_local_energy": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_local_energy_ex": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _u32, _vp, _vp, _vp, _vp, _sz,
                                   _vp]),
-    "nk_local_energy_form": (_int, [_vp, _i64, _int, _int, _int, _i64, _vp, _sz, _vp, _vp, _vp]),
+    "nk_local_energy_form": (_int, [_vp, _i64, _int, _int, _int, _i64, _vp, _sz, _vp, _vp, _vp, _vp]),
     "nk_local_energy_host_scratch_bytes": (_sz, [_vp, _i64, _int, _int, _int, _i64]),
     "nk_local_energy_host": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_energy_gradient_workspace_bytes": (_sz, [_i64, _int, _int, _int, _i64]),
@@ -222,11 +222,13 @@ class LocalEnergyPlan:
         return self.eloc, self.logpsi, self.stats
 
     def form(self):
-        """nk_local_energy_form: (NK_FORM_PRODUCT | NK_FORM_LOGCOSH, tau_max) of the last automatic run (synchronises)."""
-        form, tau = C.c_int(0), C.c_float(0.0)
+        """nk_local_energy_form: (NK_FORM_SERIES | NK_FORM_PRODUCT | NK_FORM_LOGCOSH, tau_max) of the last automatic run
+        (synchronises); the number of series terms K is kept in `self.series_terms`."""
+        form, tau, terms = C.c_int(0), C.c_float(0.0), C.c_int(0)
         rc = load().nk_local_energy_form(self.op.handle, self.B, self.N, self.M, self.dt, self.chunk, _ptr(self.ws),
-                                         self.ws_bytes, _stream(), C.byref(form), C.byref(tau))
+                                         self.ws_bytes, _stream(), C.byref(form), C.byref(tau), C.byref(terms))
         _check(rc, "nk_local_energy_form")
+        self.series_terms = terms.value
         return form.value, tau.value
 
     def run_graph(self, sigma, W, a, b):

@@ -123,9 +123,11 @@ struct ElocWs {
     uint16_t *Ws, *A;
     unsigned *absmax, *taumax;                        // taumax: max |tanh delta| of Ttab as float bits (the form gate)
     RowInfo* rows;
+    bool has_series;                                  // the tensor-core series form is possible for these sizes
+    SeriesWs ser;
     size_t bytes;
 };
-static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk) {
+static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk, int dtype) {
     Carver c(ws);
     ElocWs w;
     w.Wg = c.take<float>((size_t)g.M_eff * g.N);
@@ -139,6 +141,8 @@ static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk) {
     w.absmax = c.take<unsigned>(1);
     w.taumax = c.take<unsigned>(1);
     w.Ttab = c.take<float>((size_t)g.n_rows_pad * g.M_eff);
+    w.has_series = series_possible(g, dtype);
+    if (w.has_series) w.ser = carve_series(c.base, &c.off, g, chunk);
     w.bytes = c.off;
     return w;
 }
@@ -678,7 +682,7 @@ size_t nk_local_energy_workspace_bytes(nk_operator_t h, int64_t B, int N, int M,
     if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0) return 0;
     const Operator* op = (const Operator*)h;
     const Geometry g = make_geometry(op, N, M, dtype);
-    return carve_eloc(nullptr, g, eff_chunk(B, chunk_size)).bytes;
+    return carve_eloc(nullptr, g, eff_chunk(B, chunk_size), dtype).bytes;
 }
 
 int nk_local_energy(nk_operator_t h, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
@@ -693,22 +697,28 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
                        void* logpsi_out, double* stats_out, void* workspace, size_t workspace_bytes,
                        nk_stream_t stream) {
     if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0 || !W || (B > 0 && (!sigma || !eloc_out)) ||
-        (flags & ~(NK_FORM_PRODUCT | NK_FORM_LOGCOSH | NK_CHECK_SPINS)) ||
-        ((flags & NK_FORM_PRODUCT) && (flags & NK_FORM_LOGCOSH)))
+        (flags & ~(NK_FORM_PRODUCT | NK_FORM_LOGCOSH | NK_FORM_SERIES | NK_CHECK_SPINS)))
         return NK_ERR_INVALID_ARG;
+    {
+        const unsigned forms = flags & (NK_FORM_PRODUCT | NK_FORM_LOGCOSH | NK_FORM_SERIES);
+        if (forms & (forms - 1)) return NK_ERR_INVALID_ARG;             // at most one form may be forced
+    }
     // form of the amplitude ratios: forced by a flag, else chosen on the device from the parameters (real parameters;
     // complex ones keep the log-cosh form: tanh theta is unbounded next to the zeros of cosh)
     const bool force_product = (flags & NK_FORM_PRODUCT) != 0;
-    const bool automatic = !force_product && !(flags & NK_FORM_LOGCOSH) && dtype == NK_F32;
+    const bool force_series = (flags & NK_FORM_SERIES) != 0;
+    const bool automatic = !force_product && !force_series && !(flags & NK_FORM_LOGCOSH) && dtype == NK_F32;
     const Operator* op = (const Operator*)h;
     if (N != op->n_sites) return NK_ERR_INVALID_ARG;
     const Geometry g = make_geometry(op, N, M, dtype);
     if (!g.ok) return NK_ERR_UNSUPPORTED;
     const int64_t chunk = eff_chunk(B, chunk_size);
-    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_eloc(nullptr, g, chunk).bytes)
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_eloc(nullptr, g, chunk, dtype).bytes)
         return NK_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
-    const ElocWs w = carve_eloc(workspace, g, chunk);
+    const ElocWs w = carve_eloc(workspace, g, chunk, dtype);
+    if (force_series && !w.has_series) return NK_ERR_UNSUPPORTED;       // complex parameters or a tiny problem
+    const bool series = w.has_series && (automatic || force_series);
     if ((flags & NK_CHECK_SPINS) && B > 0) {           // opt-in validation: one pass over sigma and one synchronisation
         int bad = 0;
         NK_CUDA(launch_check_spins(sigma, B * N, (int*)w.absmax, st));
@@ -720,8 +730,10 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
     {
         Scope sc(PH_PACK, st);
         NK_CUDA(launch_pack(op, g, dtype, W, a, b, w.Wg, w.bg, w.Wt, w.Dtab, w.rows, st));
-        if (force_product || automatic)
-            NK_CUDA(launch_pack_product(op, g, dtype, w.Wt, w.Ttab, w.rows, st, automatic ? w.taumax : nullptr));
+        if (force_product || automatic || force_series)
+            NK_CUDA(launch_pack_product(op, g, dtype, w.Wt, w.Ttab, w.rows, st,
+                                        (automatic || force_series) ? w.taumax : nullptr));
+        if (series) NK_CUDA(launch_series_pack(g, w.Ttab, w.taumax, w.ser, force_series, st));
         NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
     }
     const size_t esz = dtype == NK_C64 ? 8 : 4;
@@ -740,9 +752,12 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
         {
             Scope sc(PH_FUSED, st);
             void* out = (uint8_t*)eloc_out + s0 * esz;
-            if (automatic) {           // both launches; the one on the wrong side of the gate returns at once
-                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Ttab, w.rows, out, true, st, w.taumax, 1));
-                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Dtab, w.rows, out, false, st, w.taumax, 2));
+            if (series) NK_CUDA(launch_series_eloc(op, g, sg, nb, w.theta, w.rows, w.ser, (float*)out, st));
+            if (automatic) {           // every launch; those on the wrong side of the gates return at once
+                const unsigned* sctl = series ? w.ser.ctl : nullptr;
+                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Ttab, w.rows, out, true, st, w.taumax, 1, sctl));
+                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Dtab, w.rows, out, false, st, w.taumax, 2, sctl));
+            } else if (force_series) {
             } else {
                 NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, force_product ? w.Ttab : w.Dtab, w.rows, out,
                                           force_product, st));
@@ -757,24 +772,29 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
 }
 
 int nk_local_energy_form(nk_operator_t h, int64_t B, int N, int M, int dtype, int64_t chunk_size, const void* workspace,
-                         size_t workspace_bytes, nk_stream_t stream, int* form_host, float* tau_max_host) {
+                         size_t workspace_bytes, nk_stream_t stream, int* form_host, float* tau_max_host,
+                         int* series_terms_host) {
     if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0 || !form_host) return NK_ERR_INVALID_ARG;
     const Operator* op = (const Operator*)h;
     if (N != op->n_sites) return NK_ERR_INVALID_ARG;
     const Geometry g = make_geometry(op, N, M, dtype);
     if (!g.ok) return NK_ERR_UNSUPPORTED;
     const int64_t chunk = eff_chunk(B, chunk_size);
-    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_eloc(nullptr, g, chunk).bytes)
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_eloc(nullptr, g, chunk, dtype).bytes)
         return NK_ERR_WORKSPACE;
-    const ElocWs w = carve_eloc(const_cast<void*>(workspace), g, chunk);
+    const ElocWs w = carve_eloc(const_cast<void*>(workspace), g, chunk, dtype);
     float tau = 0.f;
+    unsigned K = 0;
     cudaStream_t st = (cudaStream_t)stream;
     if (dtype == NK_F32) {                              // complex parameters never pack the product table
         NK_CUDA(cudaMemcpyAsync(&tau, w.taumax, sizeof(float), cudaMemcpyDeviceToHost, st));
+        if (w.has_series) NK_CUDA(cudaMemcpyAsync(&K, w.ser.ctl, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
         NK_CUDA(cudaStreamSynchronize(st));
     }
-    *form_host = (dtype == NK_F32 && tau <= NK_FORM_TAU_MAX) ? (int)NK_FORM_PRODUCT : (int)NK_FORM_LOGCOSH;
+    *form_host = K > 0 ? (int)NK_FORM_SERIES
+                       : (dtype == NK_F32 && tau <= NK_FORM_TAU_MAX) ? (int)NK_FORM_PRODUCT : (int)NK_FORM_LOGCOSH;
     if (tau_max_host) *tau_max_host = tau;
+    if (series_terms_host) *series_terms_host = (int)K;
     return NK_OK;
 }
 

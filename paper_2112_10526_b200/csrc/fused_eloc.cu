@@ -19,6 +19,7 @@
 //      psi'/psi = 2^(acc/2 + s a2) * prod_j (1+e'_j) / prod_j (1+e_j).
 // Complex parameters: cosh(x+iy) = (e^{|x|}/2) [(1+e) cos u + i (1-e) sin u], u = sign(x) y, and the product runs
 // over complex factors.
+#include <mutex>
 #include <type_traits>
 
 #include "nk_internal.h"
@@ -50,6 +51,8 @@ struct FusedParams {
     // 1: run iff max <= NK_FORM_TAU_MAX (product form), 2: run iff max > NK_FORM_TAU_MAX (log-cosh form)
     const unsigned* gate;
     int gate_mode;
+    const unsigned* series_ctl;              // automatic choice: both SIMT kernels stand down when the tensor-core
+                                             // series form runs (series_tc.cu: *series_ctl = K > 0)
 };
 
 // ---- kernel ----------------------------------------------------------------------------------------------
@@ -75,6 +78,7 @@ __global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_
     if (p.gate_mode != 0) {                                  // grid-uniform: every thread takes the same branch
         const bool product_ok = __uint_as_float(*p.gate) <= NK_FORM_TAU_MAX;
         if ((p.gate_mode == 1) != product_ok) return;
+        if (p.series_ctl != nullptr && *p.series_ctl != 0u) return;
     }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t stage_bytes = (uint32_t)p.tile_rows * p.M_eff * 4u;
@@ -288,15 +292,19 @@ static KernelFn pick_cplx(int v) {
     return nullptr;
 }
 
-static int g_num_sms = 0;
-static bool g_attr_done = false;
+// per-device one-time set-up (the shared-memory attribute and the SM count belong to the current device)
+static std::mutex g_fused_mutex;
+static int g_sms_of[NK_MAX_DEVICES];
+static bool g_attr_done_of[NK_MAX_DEVICES];
+#define g_num_sms (g_sms_of[current_device()])
 
 cudaError_t fused_eloc_init() {
-    if (g_attr_done) return cudaSuccess;
+    std::lock_guard<std::mutex> lock(g_fused_mutex);
+    if (g_attr_done_of[current_device()]) return cudaSuccess;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    e = cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+    e = cudaDeviceGetAttribute(&g_sms_of[current_device()], cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return e;
     for (int v = 1; v <= MAX_V_REAL; ++v)
         for (const void* fn : {(const void*)pick_real<1>(v), (const void*)pick_real<1, true>(v)}) {
@@ -308,7 +316,7 @@ cudaError_t fused_eloc_init() {
             e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
             if (e != cudaSuccess) return e;
         }
-    g_attr_done = true;
+    g_attr_done_of[current_device()] = true;
     return cudaSuccess;
 }
 
@@ -320,7 +328,8 @@ int fused_consumer_warps() { return FW; }
 
 cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
                               const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,
-                              bool product_form, cudaStream_t st, const unsigned* gate, int gate_mode) {
+                              bool product_form, cudaStream_t st, const unsigned* gate, int gate_mode,
+                              const unsigned* series_ctl) {
     if (B <= 0) return cudaSuccess;
     cudaError_t e = fused_eloc_init();
     if (e != cudaSuccess) return e;
@@ -336,7 +345,7 @@ cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, 
     p.stages = g.stages;
     p.bonds = op->d_bonds; p.colors = op->d_colors; p.Jf = op->d_Jf; p.n_bonds = op->n_bonds; p.kind = op->kind;
     p.eloc = (float*)eloc_out;
-    p.gate = gate; p.gate_mode = gate_mode;
+    p.gate = gate; p.gate_mode = gate_mode; p.series_ctl = series_ctl;
     // one CTA per SM slot, each with an equal contiguous share of the samples (rounds of FW inside the CTA);
     // small batches use fewer CTAs so that every round is full
     const int64_t max_ctas = (int64_t)g_num_sms * g.ctas_per_sm;

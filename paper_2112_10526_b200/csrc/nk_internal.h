@@ -14,6 +14,16 @@ namespace nk {
 #define NK_FORM_TAU_MAX 0.5f
 
 
+// tensor-core series form (series_tc.cu): highest power of the series, 16-bit segments per operand row, the bound on the
+// truncation error of a log-ratio (natural-log units) the automatic choice accepts, and the smallest problem it is
+// used for.  Like NK_FORM_TAU_MAX these depend on the parameters / operator only, never on sigma, B or chunk_size.
+#define SERIES_K_MAX 6
+#define SERIES_SEGS (SERIES_K_MAX + 1)
+#define SERIES_TOL 1e-5f
+#define SERIES_TAU_MAX 0.5f
+#define SERIES_MIN_ROWS 128
+#define SERIES_MIN_MPAD 256
+
 // theta is kept in the fused kernel as theta_s = KAPPA * theta, so that exp(-2|theta|) = 2^(-|theta_s|)
 // is a bare MUFU.EX2 (no multiply).  KAPPA = 2 log2(e).
 constexpr float KAPPA = 2.8853900817779268f;
@@ -44,6 +54,14 @@ struct Operator {
     float* d_Jf;         // [n_colors]
     double* d_Jd;        // [n_colors]
 };
+
+// per-device one-time state (function attributes, SM counts) is kept in arrays indexed by the device ordinal
+constexpr int NK_MAX_DEVICES = 64;
+inline int current_device() {
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= NK_MAX_DEVICES) d = 0;
+    return d;
+}
 
 inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
 inline size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
@@ -134,10 +152,27 @@ cudaError_t launch_logpsi(const int8_t* sigma, int64_t B, const Geometry& g, int
 // connected.cu
 cudaError_t launch_connected(const Operator* op, const int8_t* sigma, int64_t B, int32_t* flips, float* mels,
                              int32_t* n_conn, int8_t* sigma_prime, cudaStream_t st);
+// series_tc.cu : amplitude ratios as a short series of tensor-core GEMMs (product form, logarithm expanded)
+struct SeriesWs {
+    unsigned* ctl;              // [16] control block written per call: ctl[0] = K (0 = path off), scales, row bounds
+    uint16_t *Bp, *Ap;          // [n_rows][SERIES_SEGS][M_pad], [chunk][SERIES_SEGS][M_pad] 16-bit operand rows
+    uint32_t* sigT;             // [N][w32] transposed bit-packed spins of the chunk
+    float* part;                // [n_nt][part_stride] partial local energies per column tile
+    int w32, n_nt;
+    int64_t part_stride;
+};
+bool series_possible(const Geometry& g, int dtype);
+SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk);
+cudaError_t launch_series_pack(const Geometry& g, const float* Ttab, const unsigned* taumax_bits, const SeriesWs& w,
+                               bool force, cudaStream_t st);
+cudaError_t launch_series_eloc(const Operator* op, const Geometry& g, const int8_t* sigma, int64_t nb,
+                               const float* theta, const RowInfo* rows, const SeriesWs& w, float* eloc_out,
+                               cudaStream_t st);
 // fused_eloc.cu
 cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
                               const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,
-                              bool product_form, cudaStream_t st, const unsigned* gate = nullptr, int gate_mode = 0);
+                              bool product_form, cudaStream_t st, const unsigned* gate = nullptr, int gate_mode = 0,
+                              const unsigned* series_ctl = nullptr);
 cudaError_t fused_eloc_init();   // one-time cudaFuncSetAttribute calls
 // stats.cu
 cudaError_t launch_check_spins(const int8_t* sigma, int64_t n, int* flag, cudaStream_t st);

@@ -1,0 +1,528 @@
+// Local energies with the amplitude ratios evaluated on the tensor cores (Eq. (12); the cost the paper
+// names at L691 / L1630: one model evaluation per connected configuration).
+//
+// Product form: psi'/psi = e^{s da} prod_j cosh(d_j) prod_j (1 + s t_j tau_j), t = tanh(theta) per
+// sample, tau = tanh(d) per table row, s = +-1.  Taking the logarithm of the last product and expanding,
+//     ln prod_j (1 + s t_sj tau_bj) = sum_{k>=1} ((-1)^{k+1} / k) s^k  sum_j t_sj^k tau_bj^k ,
+// turns the [samples] x [rows] block of log-ratios into a SHORT SERIES OF GEMMs over the hidden units, one per power k:
+//     odd [s][b] = sum_{k odd}  (1/k)  (T^k (tau^k)^T)[s][b]        (multiplied by s in the epilogue)
+//     even[s][b] = sum_{k even} (-1/k) (T^k (tau^k)^T)[s][b]
+//     ln(psi'/psi)[s][b] = c_b + s (da_b + odd) + even .
+// |t| <= 1, so the remainder after K terms is at most sum_j |tau_bj|^(K+1) / ((K+1)(1 - tau_max)) — a number that
+// depends on the parameters only.  series_select_kernel takes the smallest K <= K_MAX that brings it under
+// SERIES_TOL for every row (config 5: K = 5, bound 5.6e-6) or switches the path off (K = 0: the SIMT kernels of
+// fused_eloc.cu run instead); everything downstream reads K from device memory, so the call never synchronises.
+//
+// Precision plan (fp32 accumulation in tensor memory; measured against the float64 oracle in tests/test_gpu_series.py):
+//   k = 1   carries ~0.4 in the exponent and needs ~17 bits: both operands are split into fp16 hi + lo pieces and
+//           three MMA passes hi*hi + lo*hi + hi*lo run (the dropped lo*lo is 2^-24 relative);
+//   k = 2   one fp16 pass (11 bits: 1.3e-6 rms at config 5);   k >= 3: one bf16 pass each (range down to 1e-38).
+//   tau is scaled by a power of two so that tau_max lands in [1/2, 1) and by log2(e) (the epilogue works in log2 units);
+//   the scale is undone exactly in the epilogue.
+// So a sample row / table row is a vector of (K + 1) M_pad 16-bit numbers [hi | lo | k=2 | ... | k=K] and the whole
+// series is ONE GEMM with K + 2 passes per block of hidden units into two fp32 accumulators (odd, even).
+//
+// Kernel (series_gemm_kernel): persistent, one CTA per SM, 128 (samples) x 256 (table rows) tiles, tcgen05.mma
+// kind::f16 M = 128, N = 256, K = 16 issued by one thread; accumulators odd / even fill the 512 TMEM columns.  The two
+// operands flow through SEPARATE shared-memory rings (4 x 16 KB and 4 x 32 KB, 128B-swizzled TMA boxes of 64 hidden
+// units), each with its own producer warp, because a tile is used by more than one pass: t_hi by passes 2 and 3,
+// tau_hi by passes 1 and 2 — K + 1 tiles of each operand are loaded per block of hidden units for K + 2 passes, and a
+// ring slot is handed back by the tcgen05.commit of the last pass that reads it.  Four epilogue warps (one TMEM lane
+// quarter each) read both accumulators, form the exponent, take 2^x, multiply by the matrix element, mask by the
+// sample's spins (antiparallel bond / sign of s from bit-packed transposed spins) and sum over the tile's rows —
+// [samples] x [rows] never leaves the SM.  Partial sums per column tile go to `part`, summed in a fixed order by
+// series_finish_kernel (bit-reproducible, independent of chunk_size).
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include <mutex>
+
+#include "nk_internal.h"
+#include "ptx_helpers.cuh"
+#include "tc_helpers.cuh"
+
+namespace nk {
+
+namespace ser {
+constexpr int BM = 128, BN = 256, BK = 64;                // BK 16-bit elements = one 128-B swizzle row
+constexpr int A_TILE = BM * BK * 2, B_TILE = BN * BK * 2; // 16 KB, 32 KB
+constexpr int NA = 4, NB = 4;                             // ring depths
+constexpr int THREADS = 224;                              // warps: A producer, MMA, B producer, 4 x epilogue
+constexpr int TAB_BYTES = BN * 16, MSK_BYTES = BN * 8;    // per epilogue warp: (coef, jdiag, a2, c2) and (act, neg) per column
+constexpr int SMEM_BYTES = NA * A_TILE + NB * B_TILE + 4 * (TAB_BYTES + MSK_BYTES) + 256 /*barriers*/ + 1024 /*alignment*/;
+constexpr uint32_t TMEM_COLS = 512;                       // odd at column 0, even at column 256
+// instruction descriptors of kind::f16 (the cute::UMMA::InstrDescriptor bit layout): D = F32 (c_format 1 at bit 4),
+// A / B format at bits 7 / 10 (0 = F16, 1 = BF16), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
+constexpr uint32_t IDESC_F16 = (1u << 4) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+constexpr uint32_t IDESC_BF16 = IDESC_F16 | (1u << 7) | (1u << 10);
+}  // namespace ser
+
+// ---- control block (device): ctl[0] = K (0: path off), ctl[1] = 2^e as float bits (undoes the power-of-two scale of
+// tau), ctl[2] = log2(e) 2^-e as float bits (the scale applied to tau), ctl[4 + p] = max over rows of sum_j |tau|^p ----
+constexpr int SER_CTL_WORDS = 16;
+
+__global__ void __launch_bounds__(256)
+series_rowsum_kernel(const float* __restrict__ Ttab, int M_pad, int M_eff, unsigned* __restrict__ ctl) {
+    const float* row = Ttab + (size_t)blockIdx.x * M_eff;
+    float s[SERIES_K_MAX - 1];                            // powers 3 .. K_MAX + 1
+#pragma unroll
+    for (int i = 0; i < SERIES_K_MAX - 1; ++i) s[i] = 0.f;
+    for (int j = threadIdx.x; j < M_pad; j += blockDim.x) {
+        const float x = fabsf(row[j]);
+        float p = x * x;
+#pragma unroll
+        for (int i = 0; i < SERIES_K_MAX - 1; ++i) { p *= x; s[i] += p; }
+    }
+    __shared__ float red[8][SERIES_K_MAX - 1];
+#pragma unroll
+    for (int i = 0; i < SERIES_K_MAX - 1; ++i) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s[i] += __shfl_xor_sync(0xffffffffu, s[i], o);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5][i] = s[i];
+    }
+    __syncthreads();
+    if (threadIdx.x < SERIES_K_MAX - 1) {
+        float t = 0.f;
+        for (int w = 0; w < 8; ++w) t += red[w][threadIdx.x];
+        if (t != t) t = __int_as_float(0x7f800000);       // a NaN in the table must not look like a small bound
+        atomicMax(&ctl[4 + 3 + threadIdx.x], __float_as_uint(t));
+    }
+}
+
+// force: 0 = automatic (K = 0 when no K <= K_MAX meets SERIES_TOL or tau_max > SERIES_TAU_MAX); 1 = the caller forced
+// the path (NK_FORM_SERIES): K_MAX terms are used when the bound cannot be met
+__global__ void series_select_kernel(unsigned* __restrict__ ctl, const unsigned* __restrict__ taumax_bits, int force) {
+    const float tau = __uint_as_float(*taumax_bits);
+    int K = 0;
+    if (tau <= SERIES_TAU_MAX) {
+        for (int k = 2; k <= SERIES_K_MAX; ++k) {
+            const float bound = __uint_as_float(ctl[4 + k + 1]) / ((float)(k + 1) * (1.f - tau));
+            if (bound <= SERIES_TOL) { K = k; break; }
+        }
+    }
+    if (force && K == 0) K = SERIES_K_MAX;
+    int ex = 0;
+    if (tau > 0.f && tau < 1.f) frexpf(tau, &ex);         // tau = f 2^ex, f in [1/2, 1): tau 2^-ex lands in [1/2, 1)
+    ctl[0] = (unsigned)K;
+    ctl[1] = __float_as_uint(ldexpf(1.f, ex));
+    ctl[2] = __float_as_uint(LOG2E * ldexpf(1.f, -ex));
+}
+
+__device__ __forceinline__ uint16_t f2h(float x) { return __half_as_ushort(__float2half_rn(x)); }
+__device__ __forceinline__ float h2f(uint16_t h) { return __half2float(__ushort_as_half(h)); }
+__device__ __forceinline__ uint16_t f2b(float x) { return __bfloat16_as_ushort(__float2bfloat16_rn(x)); }
+
+// Bp[r][seg][j]: seg 0 / 1 = fp16 hi / lo of x = log2(e) 2^-e tau; seg k >= 2 = (-1)^(k+1) log2(e) 2^-e tau^k / k
+// (fp16 for k = 2, bf16 above).  One block per table row.
+__global__ void __launch_bounds__(256)
+series_bpow_kernel(const float* __restrict__ Ttab, int M_pad, int M_eff, const unsigned* __restrict__ ctl,
+                   uint16_t* __restrict__ Bp) {
+    const int K = (int)ctl[0];
+    if (K == 0) return;
+    const float sc = __uint_as_float(ctl[2]);
+    const float* row = Ttab + (size_t)blockIdx.x * M_eff;
+    uint16_t* out = Bp + (size_t)blockIdx.x * SERIES_SEGS * M_pad;
+    for (int j = threadIdx.x; j < M_pad; j += blockDim.x) {
+        const float tau = row[j];
+        const float x = sc * tau;
+        const uint16_t hi = f2h(x);
+        out[j] = hi;
+        out[M_pad + j] = f2h(x - h2f(hi));
+        float p = x;                                       // sc tau^k
+        for (int k = 2; k <= K; ++k) {
+            p *= tau;
+            const float v = ((k & 1) ? p : -p) / (float)k;
+            out[(size_t)k * M_pad + j] = k == 2 ? f2h(v) : f2b(v);
+        }
+    }
+}
+
+// Ap[s][seg][j]: seg 0 / 1 = fp16 hi / lo of t = tanh(theta); seg 2 = fp16 t^2; seg k >= 3 = bf16 t^k.
+// One thread per 8 consecutive hidden units (one 16-B store per segment).
+__global__ void __launch_bounds__(256)
+series_tpow_kernel(const float* __restrict__ theta, int64_t nb, int M_pad, int M_eff,
+                   const unsigned* __restrict__ ctl, uint16_t* __restrict__ Ap) {
+    const int K = (int)ctl[0];
+    if (K == 0) return;
+    const int per_row = M_pad / 8;
+    const int64_t total = nb * per_row;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t s = idx / per_row;
+        const int j0 = (int)(idx - s * per_row) * 8;
+        const float4 x0 = *reinterpret_cast<const float4*>(theta + s * M_eff + j0);
+        const float4 x1 = *reinterpret_cast<const float4*>(theta + s * M_eff + j0 + 4);
+        float t[8] = {tanhf(x0.x), tanhf(x0.y), tanhf(x0.z), tanhf(x0.w),
+                      tanhf(x1.x), tanhf(x1.y), tanhf(x1.z), tanhf(x1.w)};
+        uint16_t* out = Ap + (size_t)s * SERIES_SEGS * M_pad + j0;
+        uint16_t hi[8], v[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) hi[e] = f2h(t[e]);
+        *reinterpret_cast<uint4*>(out) = *reinterpret_cast<const uint4*>(hi);
+#pragma unroll
+        for (int e = 0; e < 8; ++e) v[e] = f2h(t[e] - h2f(hi[e]));
+        *reinterpret_cast<uint4*>(out + M_pad) = *reinterpret_cast<const uint4*>(v);
+        float p[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) p[e] = t[e];
+        for (int k = 2; k <= K; ++k) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) { p[e] *= t[e]; v[e] = k == 2 ? f2h(p[e]) : f2b(p[e]); }
+            *reinterpret_cast<uint4*>(out + (size_t)k * M_pad) = *reinterpret_cast<const uint4*>(v);
+        }
+    }
+}
+
+// sigT[i][w]: bit l of word w <=> sigma[32 w + l][i] = -1 (samples beyond nb: 0).  Block = 32 samples x 256 sites.
+__global__ void __launch_bounds__(256)
+series_bits_kernel(const int8_t* __restrict__ sigma, int64_t nb, int N, int w32, const unsigned* __restrict__ ctl,
+                   uint32_t* __restrict__ sigT) {
+    if (ctl[0] == 0) return;
+    __shared__ int8_t sm[32][256 + 4];
+    const int64_t s0 = (int64_t)blockIdx.x * 32;
+    const int i0 = blockIdx.y * 256;
+    for (int idx = threadIdx.x; idx < 32 * 256; idx += 256) {
+        const int l = idx >> 8, c = idx & 255;
+        sm[l][c] = (s0 + l < nb && i0 + c < N) ? sigma[(s0 + l) * N + i0 + c] : (int8_t)1;
+    }
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int c = warp; c < 256; c += 8) {
+        const unsigned w = __ballot_sync(0xffffffffu, sm[lane][c] < 0);
+        if (lane == 0 && i0 + c < N) sigT[(size_t)(i0 + c) * w32 + blockIdx.x] = w;
+    }
+}
+
+// ---- the GEMM with the fused local-energy epilogue ---------------------------------------------------------------
+struct SeriesParams {
+    const unsigned* ctl;
+    const RowInfo* rows;
+    const uint32_t* sigT;
+    int w32;                      // words per site of sigT
+    int64_t nb;                   // samples of this chunk
+    int n_rows, M_pad;
+    int n_mt, n_nt;               // tiles along samples / table rows
+    float* part;                  // [n_nt][part_stride]
+    int64_t part_stride;
+};
+
+__device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                         uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}\n" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+__global__ void __launch_bounds__(ser::THREADS, 1)
+series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b,
+                   const SeriesParams p) {
+    using namespace ser;
+    const int K = (int)p.ctl[0];
+    if (K == 0) return;                                    // grid-uniform: the path is off for these parameters
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t* smem_al = smem_raw + (smem_base - smem_u32(smem_raw));
+    const uint32_t a_ring = smem_base, b_ring = smem_base + NA * A_TILE;
+    const uint32_t epi_off = NA * A_TILE + NB * B_TILE;
+    const uint32_t bars = smem_base + epi_off + 4 * (TAB_BYTES + MSK_BYTES);
+    const uint32_t a_full = bars, a_empty = bars + 8 * NA, b_full = bars + 16 * NA, b_empty = b_full + 8 * NB;
+    const uint32_t t_full = b_empty + 8 * NB, t_empty = t_full + 8, tmem_slot = t_empty + 8;
+    uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_al + (tmem_slot - smem_base));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_jb = p.M_pad / BK;
+    const int n_tiles = p.n_mt * p.n_nt;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NA; ++s) { mbar_init(a_full + 8 * s, 1); mbar_init(a_empty + 8 * s, 1); }
+        for (int s = 0; s < NB; ++s) { mbar_init(b_full + 8 * s, 1); mbar_init(b_empty + 8 * s, 1); }
+        mbar_init(t_full, 1);
+        mbar_init(t_empty, 128);
+        mbar_fence_init();
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===== A producer: per block of hidden units the tiles t_lo, t_hi, t^2 .. t^K of this sample tile =====
+        if (lane == 0) {
+            uint32_t it = 0;
+            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+                const int m0 = (tile / p.n_nt) * BM;
+                for (int jb = 0; jb < n_jb; ++jb)
+                    for (int idx = 0; idx <= K; ++idx, ++it) {
+                        const int seg = idx == 0 ? 1 : (idx == 1 ? 0 : idx);
+                        const uint32_t slot = it % NA, par = ((it / NA) & 1u) ^ 1u;
+                        mbar_wait(a_empty + 8 * slot, par);
+                        mbar_arrive_expect_tx(a_full + 8 * slot, A_TILE);
+                        tma_load_2d(a_ring + slot * A_TILE, &map_a, seg * p.M_pad + jb * BK, m0, a_full + 8 * slot);
+                    }
+            }
+        }
+    } else if (warp == 2) {
+        // ===== B producer: tau_hi, tau_lo, tau^2 .. tau^K of this row tile =====
+        if (lane == 0) {
+            uint32_t it = 0;
+            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+                const int n0 = (tile % p.n_nt) * BN;
+                for (int jb = 0; jb < n_jb; ++jb)
+                    for (int seg = 0; seg <= K; ++seg, ++it) {
+                        const uint32_t slot = it % NB, par = ((it / NB) & 1u) ^ 1u;
+                        mbar_wait(b_empty + 8 * slot, par);
+                        mbar_arrive_expect_tx(b_full + 8 * slot, B_TILE);
+                        tma_load_2d(b_ring + slot * B_TILE, &map_b, seg * p.M_pad + jb * BK, n0, b_full + 8 * slot);
+                    }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one thread) =====
+        if (lane == 0) {
+            uint32_t ia = 0, ib = 0, n_done = 0;
+            const uint32_t acc_odd = tmem_base, acc_even = tmem_base + BN;
+            auto a_wait = [&](uint32_t i) { mbar_wait(a_full + 8 * (i % NA), (i / NA) & 1u); };
+            auto b_wait = [&](uint32_t i) { mbar_wait(b_full + 8 * (i % NB), (i / NB) & 1u); };
+            auto pass = [&](uint32_t sa, uint32_t sb, uint32_t acc, uint32_t idesc, bool fresh) {
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t a_addr = a_ring + (sa % NA) * A_TILE, b_addr = b_ring + (sb % NB) * B_TILE;
+#pragma unroll
+                for (int k = 0; k < BK / 16; ++k)          // 16 elements = 32 B inside the 128-B swizzle row
+                    umma_f16(acc, make_sdesc(a_addr + k * 32), make_sdesc(b_addr + k * 32), idesc,
+                             (fresh && k == 0) ? 0u : 1u);
+            };
+            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++n_done) {
+                mbar_wait(t_empty, (n_done & 1u) ^ 1u);    // the epilogue has drained the accumulators (free at first)
+                for (int jb = 0; jb < n_jb; ++jb) {
+                    const uint32_t a_lo = ia, a_hi = ia + 1, b_hi = ib, b_lo = ib + 1;
+                    a_wait(a_lo); b_wait(b_hi);
+                    pass(a_lo, b_hi, acc_odd, IDESC_F16, jb == 0);
+                    umma_commit(a_empty + 8 * (a_lo % NA));
+                    a_wait(a_hi);
+                    pass(a_hi, b_hi, acc_odd, IDESC_F16, false);
+                    umma_commit(b_empty + 8 * (b_hi % NB));
+                    b_wait(b_lo);
+                    pass(a_hi, b_lo, acc_odd, IDESC_F16, false);
+                    umma_commit(a_empty + 8 * (a_hi % NA));
+                    umma_commit(b_empty + 8 * (b_lo % NB));
+                    ia += 2; ib += 2;
+                    for (int k = 2; k <= K; ++k, ++ia, ++ib) {
+                        a_wait(ia); b_wait(ib);
+                        pass(ia, ib, (k & 1) ? acc_odd : acc_even, k == 2 ? IDESC_F16 : IDESC_BF16, jb == 0 && k == 2);
+                        umma_commit(a_empty + 8 * (ia % NA));
+                        umma_commit(b_empty + 8 * (ib % NB));
+                    }
+                }
+                umma_commit(t_full);
+            }
+        }
+    } else {
+        // ===== epilogue: warps 3..6, TMEM lane quarter q = warp % 4 =====
+        const int q = warp & 3;
+        float4* tab = reinterpret_cast<float4*>(smem_al + epi_off + q * (TAB_BYTES + MSK_BYTES));
+        uint2* msk = reinterpret_cast<uint2*>(smem_al + epi_off + q * (TAB_BYTES + MSK_BYTES) + TAB_BYTES);
+        const float inv = __uint_as_float(p.ctl[1]);
+        uint32_t n_done = 0;
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++n_done) {
+            const int mt = tile / p.n_nt, nt = tile - mt * p.n_nt;
+            const int n0 = nt * BN;
+            // this warp's 32 samples: matrix element, diagonal coupling, exponents and the two spin masks per column
+            __syncwarp();
+            for (int c = lane; c < BN; c += 32) {
+                float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+                uint2 m = make_uint2(0u, 0u);
+                if (n0 + c < p.n_rows) {
+                    const RowInfo ri = p.rows[n0 + c];
+                    if (ri.i >= 0) {
+                        const uint32_t wi = p.sigT[(size_t)ri.i * p.w32 + mt * 4 + q];
+                        const uint32_t wj = ri.j >= 0 ? p.sigT[(size_t)ri.j * p.w32 + mt * 4 + q] : ~wi;
+                        m = make_uint2(wi ^ wj, wi);       // antiparallel <=> active; sigma_i = -1 <=> s = +1
+                        t = make_float4(ri.coef, ri.jdiag, ri.a2_re, ri.c2_re);
+                    }
+                }
+                tab[c] = t;
+                msk[c] = m;
+            }
+            __syncwarp();
+            const int64_t row = (int64_t)mt * BM + q * 32 + lane;
+            float E = 0.f;
+            mbar_wait(t_full, n_done & 1u);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll 1
+            for (int c0 = 0; c0 < BN; c0 += 32) {
+                float od[32], ev[32];
+                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + c0;
+                tmem_ld32(taddr, od);
+                tmem_ld32(taddr + BN, ev);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                if (c0 + 32 == BN) {                       // both accumulators are in registers: hand them back
+                    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                    mbar_arrive(t_empty);
+                }
+#pragma unroll
+                for (int jj = 0; jj < 32; ++jj) {
+                    const float4 t = tab[c0 + jj];
+                    const uint2 m = msk[c0 + jj];
+                    const float u = fmaf(inv, od[jj], t.z);                 // da + odd        (log2 units)
+                    const float v = fmaf(inv, ev[jj], t.w);                 // c + even
+                    const float e2 = ((m.y >> lane) & 1u) ? v + u : v - u;  // c + s (da + odd) + even
+                    const float term = fmaf(t.x, ex2_approx(e2), -t.y);     // mel psi'/psi - J   (antiparallel bond)
+                    E += ((m.x >> lane) & 1u) ? term : t.y;                 // parallel bond: + J, no connected state
+                }
+            }
+            if (row < p.nb) p.part[(size_t)nt * p.part_stride + row] = E;
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 1) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+    }
+}
+
+// eloc[s] = sum over column tiles of part (fixed order) + the diagonal of the Ising bonds (the Heisenberg diagonal is
+// already inside part: every bond is a table row).  One warp per sample.
+__global__ void __launch_bounds__(256)
+series_finish_kernel(const float* __restrict__ part, int n_nt, int64_t part_stride, const int8_t* __restrict__ sigma,
+                     int64_t nb, int N, int kind, const int32_t* __restrict__ bonds, const int32_t* __restrict__ colors,
+                     const float* __restrict__ Jf, int n_bonds, const unsigned* __restrict__ ctl,
+                     float* __restrict__ eloc) {
+    if (ctl[0] == 0) return;
+    const int lane = threadIdx.x & 31;
+    const int64_t s = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (s >= nb) return;
+    float diag = 0.f;
+    if (kind == NK_ISING) {
+        const int8_t* sg = sigma + s * N;
+        for (int b = lane; b < n_bonds; b += 32) {
+            const float J = Jf[colors[b]];
+            diag += (sg[bonds[2 * b]] != sg[bonds[2 * b + 1]]) ? -J : J;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) diag += __shfl_xor_sync(0xffffffffu, diag, o);
+    }
+    if (lane == 0) {
+        float e = 0.f;
+        for (int t = 0; t < n_nt; ++t) e += part[(size_t)t * part_stride + s];
+        eloc[s] = diag + e;
+    }
+}
+
+// ---- host side ---------------------------------------------------------------------------------------------------
+static std::mutex g_ser_mutex;
+static bool g_ser_ready[NK_MAX_DEVICES];
+static int g_ser_sms[NK_MAX_DEVICES];
+
+static cudaError_t series_init() {
+    std::lock_guard<std::mutex> lock(g_ser_mutex);
+    const int d = current_device();
+    if (g_ser_ready[d]) return cudaSuccess;
+    if (tensor_map_encoder() == nullptr) return cudaErrorNotSupported;
+    cudaError_t e = cudaFuncSetAttribute((const void*)series_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         ser::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    int dev = 0, sms = 0;
+    e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    g_ser_sms[d] = sms > 0 ? sms : 148;
+    g_ser_ready[d] = true;
+    return cudaSuccess;
+}
+
+// 2-D tensor map over a [rows][cols] operand of 16-bit elements, box = box_rows x 64 elements (128 B), 128B swizzle;
+// rows beyond `rows` read as zeros
+static bool encode_u16(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols, int box_rows) {
+    const cuuint64_t dims[2] = {cols, rows};
+    const cuuint64_t strides[1] = {cols * 2};
+    const cuuint32_t box[2] = {(cuuint32_t)ser::BK, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    return tensor_map_encoder()(map, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, const_cast<void*>(base), dims, strides, box,
+                                estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+bool series_possible(const Geometry& g, int dtype) {
+    // real parameters; large enough that 128 x 256 tiles over >= 4 blocks of 64 hidden units make sense
+    return dtype == NK_F32 && g.n_rows >= SERIES_MIN_ROWS && g.M_pad >= SERIES_MIN_MPAD;
+}
+
+SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk) {
+    auto take = [&](size_t bytes) -> void* {
+        void* r = base ? base + *off : nullptr;
+        *off += align256(bytes);
+        return r;
+    };
+    SeriesWs w;
+    w.w32 = (int)((chunk + 127) / 128 * 4);
+    w.n_nt = (g.n_rows + ser::BN - 1) / ser::BN;
+    w.part_stride = (chunk + 127) / 128 * 128;
+    w.ctl = (unsigned*)take(SER_CTL_WORDS * sizeof(unsigned));
+    w.Bp = (uint16_t*)take((size_t)g.n_rows * SERIES_SEGS * g.M_pad * 2);
+    w.Ap = (uint16_t*)take((size_t)chunk * SERIES_SEGS * g.M_pad * 2);
+    w.sigT = (uint32_t*)take((size_t)g.N * w.w32 * 4);
+    w.part = (float*)take((size_t)w.n_nt * w.part_stride * 4);
+    return w;
+}
+
+// per call, after launch_pack_product (Ttab, tau_max): choose K and write the table-row operand
+cudaError_t launch_series_pack(const Geometry& g, const float* Ttab, const unsigned* taumax_bits, const SeriesWs& w,
+                               bool force, cudaStream_t st) {
+    cudaError_t e = series_init();
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(w.ctl, 0, SER_CTL_WORDS * sizeof(unsigned), st);
+    if (e != cudaSuccess) return e;
+    series_rowsum_kernel<<<g.n_rows, 256, 0, st>>>(Ttab, g.M_pad, g.M_eff, w.ctl);
+    series_select_kernel<<<1, 1, 0, st>>>(w.ctl, taumax_bits, force ? 1 : 0);
+    series_bpow_kernel<<<g.n_rows, 256, 0, st>>>(Ttab, g.M_pad, g.M_eff, w.ctl, w.Bp);
+    count_launch(3);
+    return cudaGetLastError();
+}
+
+// per chunk: E_loc of nb samples from theta (all four kernels return at once when ctl says the path is off)
+cudaError_t launch_series_eloc(const Operator* op, const Geometry& g, const int8_t* sigma, int64_t nb,
+                               const float* theta, const RowInfo* rows, const SeriesWs& w, float* eloc_out,
+                               cudaStream_t st) {
+    if (nb <= 0) return cudaSuccess;
+    cudaError_t e = series_init();
+    if (e != cudaSuccess) return e;
+    const int sms = g_ser_sms[current_device()];
+    {
+        const int64_t total = nb * (g.M_pad / 8);
+        int64_t blocks = (total + 255) / 256;
+        if (blocks > (int64_t)sms * 16) blocks = (int64_t)sms * 16;
+        series_tpow_kernel<<<(unsigned)blocks, 256, 0, st>>>(theta, nb, g.M_pad, g.M_eff, w.ctl, w.Ap);
+    }
+    const int n_mt = (int)((nb + ser::BM - 1) / ser::BM);
+    {
+        dim3 grid((unsigned)(n_mt * 4), (unsigned)((g.N + 255) / 256));
+        series_bits_kernel<<<grid, 256, 0, st>>>(sigma, nb, g.N, w.w32, w.ctl, w.sigT);
+    }
+    CUtensorMap map_a, map_b;
+    const uint64_t cols = (uint64_t)SERIES_SEGS * g.M_pad;
+    if (!encode_u16(&map_a, w.Ap, (uint64_t)nb, cols, ser::BM)) return cudaErrorInvalidValue;
+    if (!encode_u16(&map_b, w.Bp, (uint64_t)g.n_rows, cols, ser::BN)) return cudaErrorInvalidValue;
+    SeriesParams p;
+    p.ctl = w.ctl; p.rows = rows; p.sigT = w.sigT; p.w32 = w.w32; p.nb = nb; p.n_rows = g.n_rows; p.M_pad = g.M_pad;
+    p.n_mt = n_mt; p.n_nt = w.n_nt; p.part = w.part; p.part_stride = w.part_stride;
+    const int n_tiles = n_mt * w.n_nt;
+    series_gemm_kernel<<<n_tiles < sms ? n_tiles : sms, ser::THREADS, ser::SMEM_BYTES, st>>>(map_a, map_b, p);
+    series_finish_kernel<<<(unsigned)((nb + 7) / 8), 256, 0, st>>>(w.part, w.n_nt, w.part_stride, sigma, nb, g.N,
+                                                                  op->kind, op->d_bonds, op->d_colors, op->d_Jf,
+                                                                  op->n_bonds, w.ctl, eloc_out);
+    count_launch(4);
+    return cudaGetLastError();
+}
+
+}  // namespace nk

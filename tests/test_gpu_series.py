@@ -1,0 +1,127 @@
+"""GPU parity of the tensor-core series form of the local energy (nk_local_energy_ex with NK_FORM_SERIES, and the
+automatic choice when its gate opens; paper_2112_10526_b200/csrc/series_tc.cu) against the float64 oracles:
+the from-scratch one on sample subsets and the incremental one (oracle/nk_incremental.c, pinned to the from-scratch
+one in test_oracle_incremental.py) on whole batches.  Same tolerance as every other form: |dE| <= 1e-4 |E| + 1e-6
+(Eq. (12); BASELINE.json north_star)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import nk_incremental as inc
+from oracle import nk_oracle as orc
+from paper_2112_10526_b200 import inputs as inp
+from test_gpu_parity import assert_eloc, assert_logpsi, dev, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def run_form(nk, p, form, chunk=None, flags=0, a=True, b=True):
+    op = nk.Operator.from_problem(p, flags)
+    plan = nk.LocalEnergyPlan(op, p.sigma.shape[0], p.n_sites, p.n_hidden, nk.NK_F32,
+                              p.chunk_size if chunk is None else chunk, flags=form)
+    e, lp, st = plan.run(dev(p.sigma), dev(p.W), dev(p.a) if a else None, dev(p.b) if b else None)
+    torch.cuda.synchronize()
+    out = e.cpu().numpy(), lp.cpu().numpy(), st.cpu().numpy()
+    took = plan.form() if form in (0, nk.NK_FORM_SERIES) else (form, None)
+    terms = getattr(plan, "series_terms", 0)
+    op.close()
+    return out, took[0], terms
+
+
+@pytest.mark.parametrize("cfg,n", [(5, 47), (3, 96), (5, 300)])
+def test_series_form_parity_forced(nk, cfg, n):
+    p = inp.make_config(cfg, n_samples=n)
+    (e, lp, st), form, terms = run_form(nk, p, nk.NK_FORM_SERIES, chunk=0)
+    assert form == nk.NK_FORM_SERIES and 2 <= terms <= 6
+    e_ref, lp_ref = (run_oracle(p) if n <= 100 else
+                     inc.local_energy(p.kind, p.sigma, p.bonds, p.colors, p.J, p.h, p.W, p.a, p.b))
+    worst = assert_eloc(e, e_ref)
+    assert_logpsi(lp, lp_ref)
+    m = orc.stats(e_ref)
+    assert abs(st[0] - m[0]) <= 1e-4 * abs(m[0]) + 1e-6 and st[3] == n
+    print(f"cfg{cfg} series form (K = {terms}): max rel err E_loc {worst:.2e}")
+
+
+def test_series_gate_automatic_choice(nk):
+    """Config 5 and config 3 meet the remainder bound (the automatic call takes the series form, and its result is
+    bit-identical to the forced one); config 2 is below the size limits, and parameters x6 leave the bound unmet:
+    the automatic call then takes a SIMT form and NK_FORM_SERIES is refused / still runs with K = 6."""
+    for cfg, n, k_want in ((5, 64, 5), (3, 64, None)):
+        p = inp.make_config(cfg, n_samples=n)
+        (e_auto, _, _), form, terms = run_form(nk, p, 0)
+        assert form == nk.NK_FORM_SERIES and (k_want is None or terms == k_want), (cfg, form, terms)
+        (e_forced, _, _), _, terms2 = run_form(nk, p, nk.NK_FORM_SERIES)
+        assert terms2 == terms and np.array_equal(e_auto, e_forced)
+    p = inp.make_config(2, n_samples=64)
+    _, form, terms = run_form(nk, p, 0)
+    assert form != nk.NK_FORM_SERIES and terms == 0
+    with pytest.raises(nk.NkError):
+        run_form(nk, p, nk.NK_FORM_SERIES)
+    p = inp.make_config(5, n_samples=40)
+    p.W = (p.W * 6).astype(np.float32)
+    (e_auto, _, _), form, terms = run_form(nk, p, 0)
+    assert form != nk.NK_FORM_SERIES and terms == 0
+    assert_eloc(e_auto, run_oracle(p)[0])
+
+
+def test_series_ragged_sizes_chunks_and_flags(nk):
+    """N = 144 (not a multiple of 128), M = 300 (M_pad = 384), 288 + 288 bonds in two colours (two column tiles, the
+    second ragged), B = 333 in chunks of 100 (ragged sample tiles), Marshall sign, missing biases; TFIM 12 x 12."""
+    p = inp.make_problem(inp.KIND_HEISENBERG, "square", 12, 300, 333, seed=11, order=2, J=(1.0, 0.5), scale=0.02)
+    e_ref, lp_ref = inc.local_energy(p.kind, p.sigma, p.bonds, p.colors, p.J, p.h, p.W, p.a, p.b)
+    outs = []
+    for chunk in (0, 100, 128, 1):
+        (e, lp, st), form, terms = run_form(nk, p, nk.NK_FORM_SERIES, chunk=chunk)
+        assert form == nk.NK_FORM_SERIES
+        assert_eloc(e, e_ref)
+        assert_logpsi(lp, lp_ref)
+        outs.append(e)
+    for e in outs[1:]:
+        assert np.array_equal(outs[0], e), "per-sample results must not depend on chunk_size"
+    (e, _, _), _, _ = run_form(nk, p, nk.NK_FORM_SERIES, flags=nk.NK_FLAG_MARSHALL, a=False, b=False)
+    assert_eloc(e, inc.local_energy(p.kind, p.sigma, p.bonds, p.colors, p.J, p.h, p.W, None, None,
+                                    orc.FLAG_MARSHALL)[0])
+    q = inp.make_problem(inp.KIND_ISING, "square", 12, 288, 200, seed=12, scale=0.03, h=1.3)
+    (e, lp, _), form, _ = run_form(nk, q, nk.NK_FORM_SERIES, chunk=77)
+    e_ref, lp_ref = inc.local_energy(q.kind, q.sigma, q.bonds, q.colors, q.J, q.h, q.W, q.a, q.b)
+    assert form == nk.NK_FORM_SERIES
+    assert_eloc(e, e_ref)
+    assert_logpsi(lp, lp_ref)
+
+
+def test_series_closed_forms(nk):
+    """Uniform psi (W = 0, a = 0): E_loc = n_bonds J for every sample; W = 0, a != 0 through the oracle."""
+    p = inp.make_config(5, n_samples=130)
+    p.W = np.zeros_like(p.W); p.a = np.zeros_like(p.a)
+    (e, _, _), form, terms = run_form(nk, p, 0)
+    assert form == nk.NK_FORM_SERIES and terms == 2
+    np.testing.assert_allclose(e, 2048.0, rtol=2e-6)
+    p = inp.make_config(5, n_samples=40)
+    p.W = np.zeros_like(p.W)
+    (e, _, _), _, _ = run_form(nk, p, 0)
+    assert_eloc(e, run_oracle(p)[0])
+
+
+@pytest.fixture(scope="module")
+def cfg5_full():
+    """All 65536 samples of config 5 through the incremental float64 route (minutes of host time, once per module)."""
+    p = inp.make_config(5)
+    e_ref, lp_ref = inc.local_energy(p.kind, p.sigma, p.bonds, p.colors, p.J, p.h, p.W, p.a, p.b)
+    return p, e_ref, lp_ref
+
+
+@pytest.mark.parametrize("form_name", ["auto", "series", "product", "logcosh"])
+def test_config5_full_batch_every_sample(nk, cfg5_full, form_name):
+    """Every one of the 65536 local energies of config 5, in the chunked launch configuration bench.py times, against
+    the incremental float64 route; all forms."""
+    p, e_ref, lp_ref = cfg5_full
+    form = {"auto": 0, "series": nk.NK_FORM_SERIES, "product": nk.NK_FORM_PRODUCT, "logcosh": nk.NK_FORM_LOGCOSH}[form_name]
+    (e, lp, st), took, terms = run_form(nk, p, form)
+    if form_name == "auto":
+        assert took == nk.NK_FORM_SERIES and terms == 5
+    worst = assert_eloc(e, e_ref)
+    assert_logpsi(lp, lp_ref)
+    m = orc.stats(e_ref)
+    assert abs(st[0] - m[0]) <= 1e-4 * abs(m[0]) + 1e-6 and st[3] == p.n_samples
+    assert abs(st[2] - m[2]) <= 1e-3 * m[2]
+    print(f"config 5, all {p.n_samples} samples, {form_name}: max rel err E_loc {worst:.2e}")
