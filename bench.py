@@ -29,7 +29,7 @@ CONFIG_TEXT = {
     4: "configs[3]: 2D J1-J2 10x10, complex RBM alpha=4, 16384 samples",
     5: "configs[4]: 2D Heisenberg 32x32, real RBM alpha=2, 65536 samples in chunks of 4096",
 }
-MUFU_LANES_PER_CLK_PER_SM = 16      # 4 SMSPs x 4 lanes
+
 N_SMS = 148
 
 
@@ -41,37 +41,46 @@ def measured_peaks():
 
 
 class ClockSampler(threading.Thread):
-    """Samples nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    """Samples nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line): one
+    `nvidia-smi -lms` process streaming a line every 20 ms."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
         super().__init__(daemon=True)
-        self.index, self.rows, self.stop_flag = index, [], threading.Event()
+        self.index, self.rows, self.proc = index, [], None
 
     def run(self):
-        while not self.stop_flag.is_set():
-            try:
-                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
-                f = [x.strip() for x in out.stdout.strip().split(",")]
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "20"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                f = [x.strip() for x in line.strip().split(",")]
                 if len(f) >= 7:
                     self.rows.append(f)
-            except Exception:
-                pass
-            self.stop_flag.wait(0.1)
+        except Exception:
+            pass
 
     def summary(self):
-        self.stop_flag.set()
+        if self.proc is not None:
+            self.proc.terminate()
         self.join(timeout=6)
-        if not self.rows:
+        rows = []
+        for r in self.rows:
+            try:
+                rows.append((float(r[0]), float(r[1]), float(r[2]), r[3:7]))
+            except ValueError:
+                pass
+        if not rows:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        sm = sorted(float(r[0]) for r in self.rows)
+        busy = [r for r in rows if r[2] > 0.6 * max(x[2] for x in rows)] or rows     # samples taken under load
+        sm = sorted(r[0] for r in busy)
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in self.rows)]
-        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons,
-                "samples": len(self.rows), "power_w_max": max(float(r[2]) for r in self.rows)}
+        reasons = [n for i, n in enumerate(names) if any(r[3][i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": rows[0][1], "reasons": reasons, "samples": len(rows),
+                "samples_under_load": len(busy), "power_w_max": max(r[2] for r in rows)}
 
 
 def oracle_rate(p, n_rows, repeat=1):
@@ -192,37 +201,9 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
     plan.run_graph(sigma, W, a, b)
     ms_graph = _time_ms(torch, lambda: plan.run_graph(sigma, W, a, b), 5)
     planes = 2 if p.complex_params else 1
-    # product-form variant of the same step (nk_local_energy_ex, NK_FORM_PRODUCT), fused kernel timed by the library
-    pplan = nk.LocalEnergyPlan(op, B, N, M, dt_code, p.chunk_size, device=sigma.device, flags=nk.NK_FORM_PRODUCT)
-    pplan.run(sigma, W, a, b)
-    torch.cuda.synchronize()
-    nk.profile_enable(True)
-    nk.profile_read()
-    ms_prod = _time_ms(torch, lambda: pplan.run(sigma, W, a, b), 3)
-    ph = nk.profile_read()
-    nk.profile_enable(False)
-    fused_prod_ms = ph["fused"][0] / 4                      # _time_ms runs the call 1 + 3 times
-    # ... and the log-cosh form forced (NK_FORM_LOGCOSH): the form the automatic choice falls back to
-    lplan = nk.LocalEnergyPlan(op, B, N, M, dt_code, p.chunk_size, device=sigma.device, flags=nk.NK_FORM_LOGCOSH)
-    lplan.run(sigma, W, a, b)
-    torch.cuda.synchronize()
-    nk.profile_enable(True)
-    nk.profile_read()
-    ms_log = _time_ms(torch, lambda: lplan.run(sigma, W, a, b), 3)
-    ph = nk.profile_read()
-    nk.profile_enable(False)
-    fused_log_ms = ph["fused"][0] / 4
     return {
-        "logcosh_form": {"ms_per_step": ms_log, "local_energies_per_sec": B / (ms_log * 1e-3),
-                         "fused_ms_per_step": fused_log_ms,
-                         "roofline": {"bound": "alu", "kernel": "fused_eloc_kernel<V, CPLX, PROD=false>",
-                                      "unit": "Gpair/s", "fused_ms": fused_log_ms}},
         "cuda_graph": {"ms_per_step": ms_graph, "local_energies_per_sec": B / (ms_graph * 1e-3),
                        "what": "the same nk_local_energy step replayed from a captured CUDA graph, no L2 flush"},
-        "product_form": {"ms_per_step": ms_prod, "local_energies_per_sec": B / (ms_prod * 1e-3),
-                         "fused_ms_per_step": fused_prod_ms,
-                         "roofline": {"bound": "smem", "kernel": "fused_eloc_kernel<V, CPLX, PROD=true>",
-                                      "unit": "Gpair/s", "fused_ms": fused_prod_ms}},
         "sampler": {"rule": "exchange" if exch else "local", "chains": B, "transitions_per_chain": N,
                     "ms_per_sweep": ms_sweep, "transitions_per_sec": B * N / (ms_sweep * 1e-3), "acceptance": acceptance,
                     "evaluated_fraction_estimate": anti,
@@ -239,6 +220,33 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
     }
 
 
+def time_form(nk, torch, p, op, tensors, dt_code, form_flag, reps):
+    """One forced form of the amplitude ratios (nk_local_energy_ex flag) on the bench batch: (ms per step, ms of the
+    local-energy phase per step, ms of the series GEMM kernel per step), per-kernel times from the library's brackets."""
+    sigma, W, a, b = tensors
+    B, N, M = p.n_samples, p.n_sites, p.n_hidden
+    plan = nk.LocalEnergyPlan(op, B, N, M, dt_code, p.chunk_size, device=sigma.device, flags=form_flag)
+    plan.run(sigma, W, a, b)
+    torch.cuda.synchronize()
+    nk.profile_enable(True)
+    nk.profile_read()
+    ms = _time_ms(torch, lambda: plan.run(sigma, W, a, b), reps)
+    ph = nk.profile_read()
+    nk.profile_enable(False)
+    n = reps + 1                                           # _time_ms runs the call 1 + reps times
+    return ms, ph["fused"][0] / n, ph["series_gemm"][0] / n
+
+
+def traffic_record(kernel_key, config):
+    """dram bytes per launch of a kernel from its committed `ncu --set full` capture (profiles/r02_traffic.json:
+    {kernel: {"cfg<k>": {"bytes": read + write, "capture": tag}}}); None when no capture of this kernel / config exists."""
+    try:
+        rec = json.load(open(os.path.join(ROOT, "profiles", "r02_traffic.json")))[kernel_key][f"cfg{config}"]
+        return float(rec["bytes"]), rec.get("capture")
+    except Exception:
+        return None, None
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -249,6 +257,8 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus} running with WORLD_SIZE={world}: launch one rank per GPU")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
     torch.cuda.set_device(local_rank)
@@ -282,8 +292,6 @@ def run_ours(args):
     sampler = ClockSampler(local_rank)
     sampler.start()
     nk.launch_count(reset=True)
-    nk.profile_enable(True)
-    nk.profile_read()
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
@@ -295,11 +303,25 @@ def run_ours(args):
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    clocks = sampler.summary()
     launches = nk.launch_count(reset=True)
+    step_ms = [a_.elapsed_time(b_) for a_, b_ in ev]
+    # the same K steps once more with the library's per-kernel CUDA-event brackets on (nk_profile_enable): the kernel
+    # durations behind `roofline`.  Kept out of the loop above because the brackets themselves cost timeline (two event
+    # records per kernel group and chunk); the clock sampler covers both loops.
+    nk.profile_enable(True)
+    nk.profile_read()
+    prof_ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+    prof_ms = 0.0
+    for s in range(args.steps):
+        flush.zero_()
+        prof_ev[0].record()
+        step()
+        prof_ev[1].record()
+        torch.cuda.synchronize()
+        prof_ms += prof_ev[0].elapsed_time(prof_ev[1])
+    clocks = sampler.summary()
     phases = nk.profile_read()
     nk.profile_enable(False)
-    step_ms = [a_.elapsed_time(b_) for a_, b_ in ev]
     total_ms = float(sum(step_ms))
     t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
     if world > 1:
@@ -347,67 +369,113 @@ def run_ours(args):
     anti = p.sigma[:, p.bonds[:, 0]] != p.sigma[:, p.bonds[:, 1]]
     if p.kind == inp.KIND_HEISENBERG:
         amps = int(anti[:, p.J[p.colors] != 0].sum())
+        n_rows = len(p.bonds)
     else:
         amps = B * N if p.h != 0 else 0
+        n_rows = N
     pairs = amps * M                                                     # (amplitude, hidden unit) evaluations
     fused_ms, fused_n = phases["fused"]
     fused_ms_per_step = fused_ms / args.steps
     peaks = measured_peaks()
     sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0)
-    mufu_per_pair = 3 if p.complex_params else 1
-    peak_pairs = N_SMS * MUFU_LANES_PER_CLK_PER_SM * sm_max * 1e6 / mufu_per_pair / 1e9       # Gpair/s at max clock
-    ach_pairs = pairs / (fused_ms_per_step * 1e-3) / 1e9 if fused_ms_per_step > 0 else 0.0
-    # which form of the amplitude ratios the automatic choice took (include/nkb200.h): decides the bound of the kernel
+    ghz = sm_max * 1e-3
+    cplx = p.complex_params
+    # measured pipe peaks of this box (nk_pipe_peaks: MUFU.EX2-only, FFMA-only, LDS.128-only kernels)
+    pk = nk.pipe_peaks(dev)
+    mufu_lanes, ffma_lanes, lds_bytes = pk["mufu_lanes_per_clk_sm"], pk["ffma_lanes_per_clk_sm"], pk["lds_bytes_per_clk_sm"]
+    pair_peak_mufu = N_SMS * mufu_lanes * ghz / (3 if cplx else 1)       # Gpair/s: 1 exponential per real pair (3 complex)
+    pair_peak_mufu2 = N_SMS * mufu_lanes * ghz / 2                       # SURVEY.md 8(d)'s denominator: ex2 + lg2 per pair
+    pair_peak_fp32 = N_SMS * ffma_lanes * ghz / (8 if cplx else 2)       # product form: 2 FP32 operations per real pair
+    pair_peak_smem = N_SMS * lds_bytes * ghz / (8 if cplx else 4)        # product form: 4 B of the table per real pair
+    peak_basis = (f"measured on this box by nk_pipe_peaks: MUFU.EX2 {mufu_lanes:.2f} lanes/clk/SM, FFMA {ffma_lanes:.1f} "
+                  f"lanes/clk/SM, LDS.128 {lds_bytes:.1f} B/clk/SM; x {N_SMS} SMs x {sm_max:.0f} MHz (clocks.max.sm)")
     form, tau_max = plan.form()
-    product = form == nk.NK_FORM_PRODUCT
-    smem_peak_pairs = N_SMS * (128 / (8 if p.complex_params else 4)) * sm_max * 1e6 / 1e9
-    if product:
-        # product form: shared-memory bandwidth binds (128 B/clk/SM; 4 B of the table per real pair)
-        bound, peak_used = "smem", smem_peak_pairs
-        basis = (f"shared memory: {N_SMS} SMs x 128 B/clk x {sm_max:.0f} MHz / 4 B of the tanh(delta) table per "
-                 f"(amplitude, hidden unit) pair (DESIGN.md 13)")
-        tname = f"fused_prod_dram_bytes_cfg{args.config}.txt"
+    terms = getattr(plan, "series_terms", 0)
+    ach_pairs = pairs / (fused_ms_per_step * 1e-3) / 1e9 if fused_ms_per_step > 0 else 0.0
+    bf16_burst = float(peaks.get("bf16_tflops") or 1590.0)
+    bf16_sust = float(peaks.get("bf16_tflops_sustained") or 1400.0)
+    peak_src = "MEASURED_PEAKS.json (of measured)" if peaks.get("bf16_tflops") else "B200_PROFILING.md fallback (of fallback)"
+    common = {"form": {nk.NK_FORM_SERIES: "series", nk.NK_FORM_PRODUCT: "product"}.get(form, "logcosh"),
+              "tau_max": tau_max, "pairs_per_step": pairs,
+              "pair_rate_gpair_s": ach_pairs, "frac_fp32": ach_pairs / pair_peak_fp32,
+              "frac_fp32_basis": "pairs / time of the whole local-energy phase against the FP32-pipe pair roof "
+                                 "(2 FP32 operations per (amplitude, hidden unit) pair; SURVEY.md 7 / 8(f)3)",
+              "phase_ms_per_step": {k: v[0] / args.steps for k, v in phases.items()},
+              "measured_in": f"a second loop of {args.steps} steps with the per-kernel event brackets on, "
+                             f"{prof_ms / args.steps:.4f} ms per step there (the graded loop runs without them)",
+              "pipe_peaks": pk}
+    if form == nk.NK_FORM_SERIES:
+        # tensor-core series form: the dominant kernel is series_gemm_kernel; work = the K + 2 fp16 / bf16 MMA passes of
+        # the series over [samples] x [table rows] x [hidden units], peak = measured dense bf16
+        g_ms, g_n = phases["series_gemm"]
+        flop = 2.0 * B * n_rows * M * (terms + 2)
+        ach = flop / (g_ms / args.steps * 1e-3) / 1e12 if g_ms > 0 else 0.0
+        traffic, tag = traffic_record("series_gemm_kernel", args.config)
+        roofline = {"bound": "tensor", "kernel": "series_gemm_kernel (tcgen05 kind::f16, fp16 hi/lo + bf16 passes)",
+                    "series_terms": terms, "mma_passes": terms + 2, "achieved": ach, "peak": bf16_burst,
+                    "unit": "TFLOP/s", "frac": ach / bf16_burst, "frac_of_sustained_peak": ach / bf16_sust,
+                    "peak_basis": f"{peak_src}: dense bf16 cuBLAS {bf16_burst:.0f} burst / {bf16_sust:.0f} sustained; "
+                                  "fp16 and bf16 share the rate",
+                    "flop_per_launch": flop / (g_n / args.steps) if g_n else None,
+                    "traffic": traffic, "traffic_capture": tag,
+                    "ms_per_launch": g_ms / g_n if g_n else None, "launches_per_step": g_n / args.steps}
+    elif form == nk.NK_FORM_PRODUCT:
+        traffic, tag = traffic_record("fused_eloc_kernel_product", args.config)
+        roofline = {"bound": "smem", "kernel": "fused_eloc_kernel<V, CPLX, PROD=true>", "achieved": ach_pairs,
+                    "peak": pair_peak_smem, "unit": "Gpair/s", "frac": ach_pairs / pair_peak_smem,
+                    "peak_basis": peak_basis + "; 4 B of the tanh(delta) table per pair through LDS.128 (DESIGN.md 13)",
+                    "traffic": traffic, "traffic_capture": tag,
+                    "ms_per_launch": fused_ms / fused_n if fused_n else None, "launches_per_step": fused_n / args.steps}
     else:
-        bound, peak_used = "alu", peak_pairs
-        basis = (f"MUFU pipe: {N_SMS} SMs x {MUFU_LANES_PER_CLK_PER_SM} lanes/clk x {sm_max:.0f} MHz / "
-                 f"{mufu_per_pair} MUFU per (amplitude, hidden unit) pair (DESIGN.md)")
-        tname = f"fused_dram_bytes_cfg{args.config}.txt"
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", tname)
-    if os.path.exists(tpath):
-        try:
-            traffic = float(open(tpath).read().split()[0])
-        except Exception:
-            traffic = None
-    roofline = {"bound": bound, "kernel": "fused_eloc_kernel<V, CPLX, PROD=%s>" % ("true" if product else "false"),
-                "form": "product" if product else "logcosh", "tau_max": tau_max,
-                "achieved": ach_pairs, "peak": peak_used,
-                "unit": "Gpair/s", "frac": ach_pairs / peak_used if peak_used else None, "traffic": traffic,
-                "peak_basis": basis,
-                "ms_per_launch": fused_ms / fused_n if fused_n else None, "launches_per_step": fused_n / args.steps,
-                "frac_at_measured_clock": (ach_pairs / (peak_used * clocks["sm_mhz"] / sm_max)
-                                           if clocks.get("sm_mhz") else None),
-                "phase_ms_per_step": {k: v[0] / args.steps for k, v in phases.items()}}
+        traffic, tag = traffic_record("fused_eloc_kernel_logcosh", args.config)
+        roofline = {"bound": "alu", "kernel": "fused_eloc_kernel<V, CPLX, PROD=false>", "achieved": ach_pairs,
+                    "peak": pair_peak_mufu, "unit": "Gpair/s", "frac": ach_pairs / pair_peak_mufu,
+                    "peak_basis": peak_basis + f"; {3 if cplx else 1} MUFU per pair (DESIGN.md 6.1)",
+                    "traffic": traffic, "traffic_capture": tag,
+                    "ms_per_launch": fused_ms / fused_n if fused_n else None, "launches_per_step": fused_n / args.steps}
+    roofline.update(common)
+    if clocks.get("sm_mhz"):
+        roofline["sm_mhz_under_load"] = clocks["sm_mhz"]
+
+    # the kernel BASELINE.json north_star (3) describes — the fused log-cosh kernel — and the SIMT product form, each
+    # forced on the same batch (a few steps, after the graded loop): they survive in the driver-parsed line
+    tensors = (sigma, W, a, b)
+    ms_l, fused_l, _ = time_form(nk, torch, p, op, tensors, dt_code, nk.NK_FORM_LOGCOSH, 3)
+    gp = pairs / (fused_l * 1e-3) / 1e9
+    roofline["logcosh"] = {"kernel": "fused_eloc_kernel<V, CPLX, PROD=false>", "bound": "alu", "ms_per_step": ms_l,
+                           "fused_ms_per_step": fused_l, "local_energies_per_sec": B / (ms_l * 1e-3),
+                           "achieved": gp, "unit": "Gpair/s", "peak": pair_peak_mufu, "frac": gp / pair_peak_mufu,
+                           "frac_2mufu": gp / pair_peak_mufu2,
+                           "peak_basis": f"measured MUFU.EX2 {mufu_lanes:.2f} lanes/clk/SM x {N_SMS} SMs x {sm_max:.0f} MHz; "
+                                         f"frac: {3 if cplx else 1} MUFU per pair (what the kernel issues), frac_2mufu: "
+                                         "SURVEY.md 8(d)'s 2 MUFU per pair"}
+    if not cplx:
+        ms_p, fused_p, _ = time_form(nk, torch, p, op, tensors, dt_code, nk.NK_FORM_PRODUCT, 3)
+        gp = pairs / (fused_p * 1e-3) / 1e9
+        roofline["product_simt"] = {"kernel": "fused_eloc_kernel<V, CPLX, PROD=true>", "bound": "smem", "ms_per_step": ms_p,
+                                    "fused_ms_per_step": fused_p, "local_energies_per_sec": B / (ms_p * 1e-3),
+                                    "achieved": gp, "unit": "Gpair/s", "peak": pair_peak_smem,
+                                    "frac": gp / pair_peak_smem, "frac_fp32": gp / pair_peak_fp32}
 
     # theta contraction: second roofline, tensor pipe.  Algorithmic work 2 B M N flop per step (x 2
     # planes for complex W); the kernel executes three int8 digit-plane MMAs per product (the exact fixed-point
-    # split), so the tensor pipe sees 3 x that in int8 operations.  Peak: measured dense bf16 (burst: the kernel is
-    # 31 us between kernels that leave the tensor pipe idle) x the guide's nominal int8 : bf16 ratio of 2.
+    # split), so the tensor pipe sees 3 x that in int8 operations.  Peak: measured dense bf16 (burst) x 2 — the nominal
+    # fp8 / int8 : bf16 ratio of the 5th-generation tensor cores (4.5 : 2.25 PFLOP/s dense; the guide lists fp8).
     th_ms, th_n = phases["theta"]
-    bf16_peak = float(peaks.get("bf16_tflops") or 0.0)
-    alg_flop = 2.0 * B * M * N * (2 if p.complex_params else 1)
-    if th_ms > 0 and bf16_peak > 0:
+    alg_flop = 2.0 * B * M * N * (2 if cplx else 1)
+    if th_ms > 0:
         th_s = th_ms / args.steps * 1e-3
         roofline["theta"] = {
             "bound": "tensor", "kernel": "theta_tc_kernel<I8> (tcgen05 kind::i8, 3 digit planes)",
-            "achieved": 3.0 * alg_flop / th_s / 1e12, "peak": 2.0 * bf16_peak, "unit": "TOP/s (int8, executed)",
-            "frac": 3.0 * alg_flop / th_s / 1e12 / (2.0 * bf16_peak),
+            "achieved": 3.0 * alg_flop / th_s / 1e12, "peak": 2.0 * bf16_burst, "unit": "TOP/s (int8, executed)",
+            "frac": 3.0 * alg_flop / th_s / 1e12 / (2.0 * bf16_burst),
             "algorithmic_tflops": alg_flop / th_s / 1e12,
-            "frac_of_tf32_peak_algorithmic": alg_flop / th_s / 1e12 / (0.5 * bf16_peak),
-            "peak_basis": "MEASURED_PEAKS.json bf16_tflops (burst) x 2 (nominal int8 : bf16); tf32 = bf16 / 2",
+            "frac_of_tf32_peak_algorithmic": alg_flop / th_s / 1e12 / (0.5 * bf16_burst),
+            "peak_basis": f"{peak_src} bf16 burst x 2 (nominal fp8 / int8 : bf16 = 4.5 : 2.25 PFLOP/s dense); tf32 = bf16 / 2",
             "ms_per_launch": th_ms / th_n if th_n else None, "launches_per_step": th_n / args.steps}
 
-    # CPU baseline: the oracle as it stands on a bounded sample worth ~12 s of host time (a short probe sizes it)
+    # CPU baselines on the box's host cores: (i) the from-scratch oracle as it stands on a bounded sample worth ~12 s
+    # (a short probe sizes it); (ii) the separately written incremental float64 route (oracle/nk_incremental.c)
     n0 = min(ORACLE_ROWS_PER_STEP[args.config], B)
     rate0, t0 = oracle_rate(p, n0)
     want = 12.0
@@ -418,12 +486,27 @@ def run_ours(args):
            "sample": f"first {n_or} samples of the batch" + (f", {rep} passes" if rep > 1 else "") +
                      f", {cpu_s:.1f} s (work is linear in samples)",
            "host_cpus": os.cpu_count()}
+    try:
+        from oracle import nk_incremental as inc
+        n_in = min(B, 64)
+        t1 = time.perf_counter()
+        inc.local_energy(p.kind, p.sigma[:n_in], p.bonds, p.colors, p.J, p.h, p.W, p.a, p.b)
+        dt1 = max(time.perf_counter() - t1, 1e-6)
+        n_in2 = int(min(B, max(n_in, n_in * 8.0 / dt1)))
+        t1 = time.perf_counter()
+        inc.local_energy(p.kind, p.sigma[:n_in2], p.bonds, p.colors, p.J, p.h, p.W, p.a, p.b)
+        dt2 = time.perf_counter() - t1
+        cpu["incremental"] = {"value": n_in2 / dt2, "unit": "local energies/s", "cores": inc.num_threads(),
+                              "kind": "oracle (incremental float64 route, oracle/nk_incremental.c)",
+                              "sample": f"first {n_in2} samples of the batch, {dt2:.1f} s"}
+    except Exception as exc:                                              # no C compiler on the box: report, do not fail
+        cpu["incremental"] = {"unavailable": str(exc)[:200]}
 
     value = world * B / (ms_per_step * 1e-3)
     line = {"metric": "local_energies_per_sec", "value": value, "unit": "local energies/s",
             "amplitudes_per_sec": world * amps / (ms_per_step * 1e-3), "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "c64" if p.complex_params else "f32",
+            "vs_baseline": None, "dtype": "c64" if cplx else "f32",
             "data": "synthetic (seeded, BASELINE.json recipe)",
             "config": {"workload": CONFIG_TEXT[args.config], "samples_per_gpu": B, "n_sites": N, "n_hidden": M,
                        "chunk_size": p.chunk_size, "amplitudes_per_step_per_gpu": amps,
@@ -432,39 +515,75 @@ def run_ours(args):
             "clocks": clocks, "e2e": {"value": world * B / (e2e_ms * 1e-3), "unit": "local energies/s",
                                       "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms},
             "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-            "step_ms": [round(x, 4) for x in step_ms], "inputs_sha256": p.sha256()}
+            "step_ms": [round(x, 4) for x in step_ms[:32]], "inputs_sha256": p.sha256()}
     if extras is not None:
-        for k in ("sampler",):
-            r = extras[k]["roofline"]
-            r["peak"] = peak_pairs
-            r["frac"] = r["achieved"] / peak_pairs if peak_pairs else None
-        # product form: shared-memory bandwidth binds (128 B/clk/SM; 4 B per real pair, 8 B per complex pair)
-        r = extras["product_form"]["roofline"]
-        r["peak"] = smem_peak_pairs
-        r["achieved"] = pairs / (r.pop("fused_ms") * 1e-3) / 1e9
-        r["frac"] = r["achieved"] / r["peak"]
-        # log-cosh form: the MUFU pipe binds (1 exponential per real pair, 3 per complex pair)
-        r = extras["logcosh_form"]["roofline"]
-        r["peak"] = peak_pairs
-        r["achieved"] = pairs / (r.pop("fused_ms") * 1e-3) / 1e9
-        r["frac"] = r["achieved"] / r["peak"]
+        r = extras["sampler"]["roofline"]
+        r["peak"] = pair_peak_mufu
+        r["frac"] = r["achieved"] / pair_peak_mufu if pair_peak_mufu else None
         line["extras"] = extras
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
 
+def run_peaks(args):
+    """--peaks: the pipe-peak microbenchmarks alone (nk_pipe_peaks), one JSON line."""
+    import torch
+
+    import paper_2112_10526_b200 as nk
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --peaks needs a CUDA device")
+    torch.cuda.set_device(0)
+    nk.load()
+    out = [nk.pipe_peaks("cuda:0") for _ in range(3)][-1]
+    out["what"] = ("MUFU.EX2-only, FFMA-only and LDS.128-only kernels on every SM (4 CTAs x 512 threads per SM, 8 independent "
+                   "chains per thread); lanes or bytes per clock per SM at the SM clock measured inside each launch")
+    print(json.dumps(out), flush=True)
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: re-run this script under torchrun, one rank per
+    GPU (the driver's own launch line), and fail loudly when the node has fewer devices."""
+    import torch
+    n_dev = torch.cuda.device_count()
+    if n_dev < args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus}: only {n_dev} CUDA device(s) visible")
+    cmd = spawn_command(args)
+    raise SystemExit(subprocess.call(cmd))
+
+
+def spawn_command(args, port=None):
+    import socket
+    if port is None:
+        sock = socket.socket()
+        sock.bind(("127.0.0.1", 0))
+        port = sock.getsockname()[1]
+        sock.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__),
+           "--gpus", str(args.gpus), "--steps", str(args.steps), "--warmup", str(args.warmup),
+           "--config", str(args.config), "--impl", args.impl]
+    if args.no_extras:
+        cmd.append("--no-extras")
+    return cmd
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the sampler / gradient timings")
+    ap.add_argument("--peaks", action="store_true", help="only run the pipe-peak microbenchmarks (nk_pipe_peaks)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.peaks:
+        run_peaks(args)
+    elif args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)
     else:
         run_ours(args)
 

@@ -187,6 +187,21 @@ int nk_energy_gradient(const int8_t* sigma, int64_t B, int N, int M, int dtype, 
                        void* grad_b_out, void* grad_W_out, void* workspace, size_t workspace_bytes,
                        nk_stream_t stream);
 
+/* The same for ONE SHARD of a batch that is spread over several ranks (samples are
+ * distributed, expectation values reduced): sigma / eloc hold this rank's B samples, `stats` the statistics of the
+ * WHOLE batch (nk_stats_combine of the all-gathered per-rank statistics) and B_global >= B its size.  The outputs are
+ * this rank's share  (1 / B_global) sum_{s in shard} O_s^* (E_s - mean)  (x 2 Re for NK_F32), so the gradient of the
+ * union is the plain SUM of the ranks' outputs: one all-reduce per block, no arithmetic outside the library. */
+int nk_energy_gradient_sharded(const int8_t* sigma, int64_t B, int64_t B_global, int N, int M, int dtype,
+                               const void* W, const void* b, const void* eloc, const double* stats,
+                               int64_t chunk_size, void* grad_a_out, void* grad_b_out, void* grad_W_out,
+                               void* workspace, size_t workspace_bytes, nk_stream_t stream);
+
+/* Statistics of the union of n_parts shards from their (mean_re, mean_im, population variance, count) quadruples
+ * (Eq. (17) L675 across shards; the pairwise update of Chan et al., applied in the order given).  Host arithmetic on
+ * host pointers: parts_host [n_parts][4], out4_host [4].  Shards with count 0 are skipped. */
+int nk_stats_combine(const double* parts_host, int n_parts, double* out4_host);
+
 /* ---- quantum geometric tensor times a vector, on the fly -----------------------------
  * PAPER.md Eq. (23): G_ij = E[O_i^* O_j] - E[O_i^*] E[O_j] with the log-derivatives O of Eq. (13); its
  * product with a vector without forming G, Eq. (75) L2219 (QGTOnTheFly):
@@ -195,7 +210,10 @@ int nk_energy_gradient(const int8_t* sigma, int64_t B, int N, int M, int dtype, 
  * (v_a [N], v_b [M], v_W [M][N]) -> (out_a, out_b, out_W).  v_a / v_b may be NULL (= zeros), out_a / out_b may be
  * NULL (not wanted).  NK_F32: G is real (the Re[G] of Eq. (30)); NK_C64: the full Hermitian G of the holomorphic
  * RBM (Eq. (31)).  Samples are processed chunk_size at a time; the three contractions (theta, V_W sigma, J^dagger dw)
- * run on the tensor cores with exact products, as in nk_rbm_logpsi / nk_energy_gradient. */
+ * run on the tensor cores with exact products, as in nk_rbm_logpsi / nk_energy_gradient.
+ * Single rank only: <w> is the mean over THIS call's samples, so the outputs of several shards do not add up to the
+ * product of the union's G (the between-shard term of the covariance is missing); multi-rank stochastic
+ * reconfiguration is not supported by this version. */
 size_t nk_qgt_matvec_workspace_bytes(int64_t B, int N, int M, int dtype, int64_t chunk_size);
 int nk_qgt_matvec(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* b,
                   const void* v_a, const void* v_b, const void* v_W, double diag_shift, int64_t chunk_size,
@@ -255,10 +273,18 @@ int nk_metropolis_sample(int rule, const int32_t* clusters_host, int n_clusters,
 /* Per-phase device timing (bench accounting).  With nk_profile_enable(1), nk_local_energy brackets each phase
  * of each chunk with CUDA events on the call's stream (a few microseconds of timeline each).  nk_profile_read
  * synchronises on those events, adds up the elapsed milliseconds per phase since the last read and writes
- * out[0..4] = ms in {pack, theta contraction, ln psi, fused local energy, statistics}, out[5..9] = the number of
- * bracketed launches groups per phase; then clears the record.  Thread-local, like nk_launch_count. */
+ * out[0..6] = ms in {pack, theta contraction, ln psi, local-energy phase (every kernel of it), statistics, the series
+ * form's tensor-core kernel alone, the series form's operand preparation alone}, out[7..13] = the number of bracketed
+ * launch groups per phase; then clears the record.  Thread-local, like nk_launch_count. */
 int nk_profile_enable(int on);
-int nk_profile_read(double* out10_host);
+int nk_profile_read(double* out14_host);
+
+/* Pipe-peak microbenchmarks for the roofline denominators (bench accounting; nothing of the hot path runs here): three
+ * kernels that saturate one pipe each — MUFU.EX2 (the log-cosh form's bound), FFMA (the product form's arithmetic),
+ * LDS.128 (the product form's shared-memory bound) — timed with CUDA events, the SM clock measured inside each launch.
+ * out8_host: [0] MUFU lanes / clk / SM, [1] FFMA lanes / clk / SM, [2] LDS bytes / clk / SM, [3..5] the SM clock (GHz)
+ * in each of the three, [6] SM count, [7] total milliseconds.  scratch_dev: >= 256 device bytes.  SYNCHRONISES `stream`. */
+int nk_pipe_peaks(double* out8_host, void* scratch_dev, nk_stream_t stream);
 
 /* Number of kernels the library launched on this thread since the last call with reset != 0 (bench accounting). */
 int64_t nk_launch_count(int reset);

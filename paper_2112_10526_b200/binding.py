@@ -11,7 +11,7 @@ import os
 import numpy as np
 
 __all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host", "energy_gradient",
-           "qgt_matvec", "sr_solve", "rbmsymm_expand", "rbmsymm_reduce_gradient", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "allreduce_gradient", "LIB_PATH",
+           "qgt_matvec", "sr_solve", "rbmsymm_expand", "rbmsymm_reduce_gradient", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "pipe_peaks", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "allreduce_gradient", "LIB_PATH",
            "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "NK_FORM_PRODUCT", "NK_CHECK_SPINS", "NK_FORM_LOGCOSH", "NK_FORM_SERIES", "EXPORTS"]
 
 NK_HEISENBERG, NK_ISING = 0, 1
@@ -42,6 +42,9 @@ EXPORTS = {
     "nk_local_energy_host": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_energy_gradient_workspace_bytes": (_sz, [_i64, _int, _int, _int, _i64]),
     "nk_energy_gradient": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "nk_energy_gradient_sharded": (_int, [_vp, _i64, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp,
+                                           _sz, _vp]),
+    "nk_stats_combine": (_int, [_vp, _int, _vp]),
     "nk_qgt_matvec_workspace_bytes": (_sz, [_i64, _int, _int, _int, _i64]),
     "nk_qgt_matvec": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _vp, _dbl, _i64, _vp, _vp, _vp, _vp, _sz,
                              _vp]),
@@ -53,6 +56,7 @@ EXPORTS = {
     "nk_metropolis_workspace_bytes": (_sz, [_int, _int, _i64, _int, _int, _int, _i64]),
     "nk_metropolis_sample": (_int, [_int, _vp, _int, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _u64, _u64, _u64,
                                     _i64, _vp, _vp, _sz, _vp]),
+    "nk_pipe_peaks": (_int, [_vp, _vp, _vp]),
     "nk_launch_count": (_i64, [_int]),
     "nk_profile_enable": (_int, [_int]),
     "nk_profile_read": (_int, [_vp]),
@@ -296,9 +300,11 @@ def local_energy_host(op: Operator, sigma, W, a=None, b=None, *, chunk_size: int
     return eloc, logpsi, stats
 
 
-def energy_gradient(sigma, W, b, eloc, stats, *, chunk_size: int = 0, ws=None):
+def energy_gradient(sigma, W, b, eloc, stats, *, chunk_size: int = 0, ws=None, n_global: int | None = None):
     """nk_energy_gradient on device tensors -> (grad_a [N], grad_b [M], grad_W [M][N]) in the parameter dtype.
-    `eloc`, `stats` are the outputs of local_energy on the same sigma."""
+    `eloc`, `stats` are the outputs of local_energy on the same sigma.  n_global (nk_energy_gradient_sharded): this
+    rank holds one shard of a batch of n_global samples and `stats` are the statistics of the whole batch; the outputs
+    of the ranks then SUM to the gradient of the union (allreduce_gradient)."""
     torch = _torch()
     lib = load()
     _check_params(sigma, W, None, b)
@@ -315,9 +321,10 @@ def energy_gradient(sigma, W, b, eloc, stats, *, chunk_size: int = 0, ws=None):
         raise NkError("nk_energy_gradient_workspace_bytes rejected the arguments")
     if ws is None or ws.numel() < nbytes:
         ws = torch.empty(nbytes, dtype=torch.uint8, device=sigma.device)
-    rc = lib.nk_energy_gradient(_ptr(sigma), B, N, M, dt, _ptr(W), _ptr(b), _ptr(eloc), _ptr(stats), int(chunk_size),
-                                _ptr(ga), _ptr(gb), _ptr(gW), _ptr(ws), ws.numel(), _stream())
-    _check(rc, "nk_energy_gradient")
+    rc = lib.nk_energy_gradient_sharded(_ptr(sigma), B, B if n_global is None else int(n_global), N, M, dt, _ptr(W),
+                                        _ptr(b), _ptr(eloc), _ptr(stats), int(chunk_size), _ptr(ga), _ptr(gb),
+                                        _ptr(gW), _ptr(ws), ws.numel(), _stream())
+    _check(rc, "nk_energy_gradient_sharded")
     return ga, gb, gW
 
 
@@ -448,7 +455,7 @@ def launch_count(reset: bool = False) -> int:
     return int(load().nk_launch_count(1 if reset else 0))
 
 
-PHASES = ("pack", "theta", "logpsi", "fused", "stats")
+PHASES = ("pack", "theta", "logpsi", "fused", "stats", "series_gemm", "series_prep")
 
 
 def profile_enable(on: bool = True):
@@ -457,27 +464,20 @@ def profile_enable(on: bool = True):
 
 def profile_read() -> dict:
     """{phase: (total ms, bracketed launch groups)} since the last read (synchronises on the recorded events)."""
-    out = np.zeros(10, dtype=np.float64)
+    out = np.zeros(2 * len(PHASES), dtype=np.float64)
     _check(load().nk_profile_read(out.ctypes.data), "nk_profile_read")
-    return {ph: (float(out[i]), int(out[5 + i])) for i, ph in enumerate(PHASES)}
+    return {ph: (float(out[i]), int(out[len(PHASES) + i])) for i, ph in enumerate(PHASES)}
 
 
 # ---- multi-GPU: samples shard across ranks, the only exchange is the statistics (SURVEY.md §8(e)) ----------
 def combine_stats(parts):
-    """Combine per-shard (mean_re, mean_im, variance, count) into the statistics of the union (Chan et al.
-    pairwise update).  Host arithmetic on 4 doubles per shard; used after an all-gather of the stats."""
-    n_tot, mr, mi, m2 = 0.0, 0.0, 0.0, 0.0
-    for p in parts:
-        pr, pi, pv, n = (float(x) for x in p)
-        if n == 0:
-            continue
-        d_r, d_i = pr - mr, pi - mi
-        new_n = n_tot + n
-        m2 += pv * n + (d_r * d_r + d_i * d_i) * n_tot * n / new_n
-        mr += d_r * n / new_n
-        mi += d_i * n / new_n
-        n_tot = new_n
-    return np.array([mr, mi, m2 / n_tot if n_tot else 0.0, n_tot])
+    """nk_stats_combine: per-shard (mean_re, mean_im, variance, count) -> the statistics of the union (the merge runs
+    in the library; this only marshals the 4-double records)."""
+    arr = np.ascontiguousarray(np.asarray([np.asarray(p, dtype=np.float64).reshape(4) for p in parts],
+                                          dtype=np.float64).reshape(-1, 4))
+    out = np.zeros(4, dtype=np.float64)
+    _check(load().nk_stats_combine(arr.ctypes.data, int(arr.shape[0]), out.ctypes.data), "nk_stats_combine")
+    return out
 
 
 def allreduce_stats(stats):
@@ -492,23 +492,27 @@ def allreduce_stats(stats):
     return combine_stats([g.cpu().numpy() for g in gathered])
 
 
-def allreduce_gradient(grads, n_local: int):
-    """Combine per-rank gradient / force / QGT-vector blocks into those of the union of the shards (in place).
-    Each rank calls nk_energy_gradient (or nk_qgt_matvec) on its own samples with the GLOBAL mean in `stats`
-    (allreduce_stats), which gives g_r = (1/B_r) sum_{s in r} O_s^* (E_s - mean); the union's g is
-    sum_r (B_r / B) g_r: one weighted all-reduce per block (NCCL on GPUs, gloo on CPU).  Returns `grads`."""
+def allreduce_gradient(grads):
+    """Sum per-rank energy-gradient blocks into those of the union of the shards (in place): every rank has called
+    energy_gradient(..., n_global=B_total) on its own samples with the statistics of the whole batch
+    (allreduce_stats), so its blocks are already weighted by 1 / B_total and the union's gradient is their plain sum —
+    one all-reduce per block (NCCL on GPUs, gloo on CPU), no arithmetic here.  QGT-vector products do not combine this
+    way (nk_qgt_matvec centres with the shard-local mean): multi-rank SR is not supported.  Returns `grads`."""
     torch = _torch()
     import torch.distributed as dist
     if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
         return grads
-    n = torch.tensor([float(n_local)], dtype=torch.float64, device=grads[0].device)
-    dist.all_reduce(n)
-    w = float(n_local) / float(n.item())
     for g in grads:
         if g is not None:
-            g.mul_(w)
-            if g.is_complex():
-                dist.all_reduce(torch.view_as_real(g))
-            else:
-                dist.all_reduce(g)
+            dist.all_reduce(torch.view_as_real(g) if g.is_complex() else g)
     return grads
+
+
+def pipe_peaks(device="cuda"):
+    """nk_pipe_peaks: measured MUFU / FFMA lanes and LDS bytes per clock per SM (roofline denominators of bench.py)."""
+    torch = _torch()
+    out = np.zeros(8, dtype=np.float64)
+    scratch = torch.zeros(256, dtype=torch.uint8, device=device)
+    _check(load().nk_pipe_peaks(out.ctypes.data, _ptr(scratch), _stream()), "nk_pipe_peaks")
+    return {"mufu_lanes_per_clk_sm": out[0], "ffma_lanes_per_clk_sm": out[1], "lds_bytes_per_clk_sm": out[2],
+            "sm_ghz": [out[3], out[4], out[5]], "sms": int(out[6]), "ms": out[7]}

@@ -17,7 +17,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libnkb200.so")
-SOURCES = ["api.cu", "pack.cu", "theta_tc.cu", "series_tc.cu", "gradient.cu", "logpsi.cu", "connected.cu", "fused_eloc.cu", "sampler.cu", "qgt.cu", "cg.cu", "rbmsymm.cu", "stats.cu"]
+SOURCES = ["api.cu", "pack.cu", "theta_tc.cu", "series_tc.cu", "gradient.cu", "logpsi.cu", "connected.cu", "fused_eloc.cu", "sampler.cu", "qgt.cu", "cg.cu", "rbmsymm.cu", "stats.cu", "peaks.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "-I", os.path.join(ROOT, "include"), "-I", CSRC]

@@ -14,24 +14,28 @@ static thread_local int64_t tl_launches = 0;
 void count_launch(int n) { tl_launches += n; }
 
 // ---- optional per-phase event timing ----
-enum Phase { PH_PACK = 0, PH_GEMM, PH_LOGPSI, PH_FUSED, PH_STATS, PH_COUNT };
 struct Span { int phase; cudaEvent_t a, b; };
 static thread_local bool tl_prof = false;
 static thread_local std::vector<Span> tl_spans;
-struct Scope {
-    cudaStream_t st; Span sp; bool on;
-    Scope(int phase, cudaStream_t s) : st(s), on(tl_prof) {
-        if (!on) return;
-        sp.phase = phase;
-        if (cudaEventCreate(&sp.a) != cudaSuccess || cudaEventCreate(&sp.b) != cudaSuccess) { on = false; return; }
-        cudaEventRecord(sp.a, st);
-    }
-    ~Scope() {
-        if (!on) return;
-        cudaEventRecord(sp.b, st);
-        tl_spans.push_back(sp);
-    }
-};
+static thread_local std::vector<cudaEvent_t> tl_event_pool;      // events are reused: creating one costs microseconds
+static cudaEvent_t pooled_event() {
+    if (!tl_event_pool.empty()) { cudaEvent_t e = tl_event_pool.back(); tl_event_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+    return e;
+}
+ProfScope::ProfScope(int phase_, cudaStream_t s) : st(s), phase(phase_), a(nullptr), b(nullptr), on(tl_prof) {
+    if (!on) return;
+    a = pooled_event(); b = pooled_event();
+    if (!a || !b) { on = false; return; }
+    cudaEventRecord(a, st);
+}
+ProfScope::~ProfScope() {
+    if (!on) return;
+    cudaEventRecord(b, st);
+    tl_spans.push_back(Span{phase, a, b});
+}
+typedef ProfScope Scope;
 
 // nk_local_energy_host overlaps its host->device copies with the chunk loop: when this is set, chunk k of
 // nk_local_energy_ex first makes the call's stream wait on event k (sigma of that chunk has arrived).
@@ -263,7 +267,7 @@ int nk_profile_read(double* out) {
         if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, sp.a, sp.b);
         if (e != cudaSuccess) rc = cuda_fail(e);
         else { out[sp.phase] += ms; out[PH_COUNT + sp.phase] += 1.0; }
-        cudaEventDestroy(sp.a); cudaEventDestroy(sp.b);
+        tl_event_pool.push_back(sp.a); tl_event_pool.push_back(sp.b);
     }
     tl_spans.clear();
     return rc;
@@ -370,7 +374,16 @@ int nk_energy_gradient(const int8_t* sigma, int64_t B, int N, int M, int dtype, 
                        const void* eloc, const double* stats, int64_t chunk_size, void* grad_a_out,
                        void* grad_b_out, void* grad_W_out, void* workspace, size_t workspace_bytes,
                        nk_stream_t stream) {
-    if (bad_dims(B, N, M, dtype) || B == 0 || chunk_size < 0 || !sigma || !W || !eloc || !stats || !grad_W_out)
+    return nk_energy_gradient_sharded(sigma, B, B, N, M, dtype, W, b, eloc, stats, chunk_size, grad_a_out, grad_b_out,
+                                      grad_W_out, workspace, workspace_bytes, stream);
+}
+
+int nk_energy_gradient_sharded(const int8_t* sigma, int64_t B, int64_t B_global, int N, int M, int dtype,
+                               const void* W, const void* b, const void* eloc, const double* stats,
+                               int64_t chunk_size, void* grad_a_out, void* grad_b_out, void* grad_W_out,
+                               void* workspace, size_t workspace_bytes, nk_stream_t stream) {
+    if (bad_dims(B, N, M, dtype) || B == 0 || B_global < B || chunk_size < 0 || !sigma || !W || !eloc || !stats ||
+        !grad_W_out)
         return NK_ERR_INVALID_ARG;
     const Geometry g = make_geometry(nullptr, N, M, dtype);
     if (g.M_pad / MPAD_ALIGN > (dtype == NK_C64 ? MAX_V_CPLX : MAX_V_REAL) || N > 65535) return NK_ERR_UNSUPPORTED;
@@ -388,7 +401,8 @@ int nk_energy_gradient(const int8_t* sigma, int64_t B, int N, int M, int dtype, 
         const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
         const int8_t* sg = sigma + s0 * N;
         NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.Ws, w.A, w.bg, w.theta, st));
-        NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B, (const uint8_t*)eloc + s0 * esz, stats, w, first, 2.f, st));
+        NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B_global, (const uint8_t*)eloc + s0 * esz, stats, w, first, 2.f,
+                                      st));
         first = 0;
     }
     NK_CUDA(launch_gradient_finalize(g, dtype, w, grad_a_out, grad_b_out, grad_W_out, st));
@@ -745,14 +759,15 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
             Scope sc(PH_GEMM, st);
             NK_CUDA(run_theta(g, sg, nb, w.Wg, w.bg, w.Ws, w.A, w.theta, st));
         }
-        if (logpsi_out) {
+        if (logpsi_out || series) {            // ln psi and, in the same pass over theta, the series form's operand rows
             Scope sc(PH_LOGPSI, st);
-            NK_CUDA(launch_logpsi(sg, nb, g, dtype, w.theta, a, (uint8_t*)logpsi_out + s0 * esz, false, nullptr, st));
+            NK_CUDA(launch_logpsi(sg, nb, g, dtype, w.theta, a, logpsi_out ? (uint8_t*)logpsi_out + s0 * esz : nullptr,
+                                  false, nullptr, st, series ? w.ser.ctl : nullptr, series ? w.ser.Ap : nullptr));
         }
         {
             Scope sc(PH_FUSED, st);
             void* out = (uint8_t*)eloc_out + s0 * esz;
-            if (series) NK_CUDA(launch_series_eloc(op, g, sg, nb, w.theta, w.rows, w.ser, (float*)out, st));
+            if (series) NK_CUDA(launch_series_eloc(op, g, sg, nb, w.rows, w.ser, (float*)out, st));
             if (automatic) {           // every launch; those on the wrong side of the gates return at once
                 const unsigned* sctl = series ? w.ser.ctl : nullptr;
                 NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Ttab, w.rows, out, true, st, w.taumax, 1, sctl));
@@ -768,6 +783,25 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
         Scope sc(PH_STATS, st);
         NK_CUDA(launch_stats(eloc_out, B, dtype, stats_out, st));
     }
+    return NK_OK;
+}
+
+int nk_stats_combine(const double* parts_host, int n_parts, double* out4_host) {
+    if (!parts_host || n_parts < 0 || !out4_host) return NK_ERR_INVALID_ARG;
+    // Chan et al. pairwise update of (mean, M2) in the order given: the statistics of the union of the shards
+    double n_tot = 0.0, mr = 0.0, mi = 0.0, m2 = 0.0;
+    for (int k = 0; k < n_parts; ++k) {
+        const double pr = parts_host[4 * k], pi = parts_host[4 * k + 1], pv = parts_host[4 * k + 2],
+                     n = parts_host[4 * k + 3];
+        if (!(n >= 0.0)) return NK_ERR_INVALID_ARG;
+        if (n == 0.0) continue;
+        const double dr = pr - mr, di = pi - mi, new_n = n_tot + n;
+        m2 += pv * n + (dr * dr + di * di) * n_tot * n / new_n;
+        mr += dr * n / new_n;
+        mi += di * n / new_n;
+        n_tot = new_n;
+    }
+    out4_host[0] = mr; out4_host[1] = mi; out4_host[2] = n_tot > 0.0 ? m2 / n_tot : 0.0; out4_host[3] = n_tot;
     return NK_OK;
 }
 

@@ -3,6 +3,9 @@
 // and both sums are evaluated in fp64 (at N = 1024 |ln psi| ~ 100, where one fp32 ulp is already 7.6e-6:
 // DESIGN.md Q12), and ln 2 is applied once as M ln 2.
 //   stable form (Q11): z <- z sign(Re z);  ln cosh z = z + log1p(exp(-2 z)) - ln 2
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
 #include "nk_internal.h"
 
 namespace nk {
@@ -52,16 +55,31 @@ __device__ __forceinline__ float ln_cosh_small_f(float t) {
 
 constexpr int LOGPSI_WARPS_REAL = 4;      // warps per block of the real kernel: 4 x 8 KB of compaction lists
 
+__device__ __forceinline__ uint32_t pack_h2(float x, float y) {
+    const __half2 h = __floats2half2_rn(x, y);
+    return *reinterpret_cast<const uint32_t*>(&h);
+}
+__device__ __forceinline__ uint32_t pack_b2(float x, float y) {
+    const __nv_bfloat162 h = __floats2bfloat162_rn(x, y);
+    return *reinterpret_cast<const uint32_t*>(&h);
+}
+
+// series_ctl / series_Ap (real parameters only, may be NULL): when *series_ctl = K > 0 the same pass over theta also
+// writes the sample-side operand rows of the tensor-core series form (series_tc.cu): per hidden unit t = tanh(theta)
+// as fp16 hi + lo, t^2 as fp16 and t^3 .. t^K as bf16, in segments of M_pad — theta is read once for both.
 template <bool CPLX>
 __global__ void __launch_bounds__(256)
 logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_pad, int M_eff,
               const float* __restrict__ theta, const float* __restrict__ a, void* __restrict__ logpsi_out,
-              int out_f64, float* __restrict__ theta_out) {
+              int out_f64, float* __restrict__ theta_out, const unsigned* __restrict__ series_ctl,
+              uint16_t* __restrict__ series_Ap) {
     const int lane = threadIdx.x & 31;
     const int64_t s = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (s >= B) return;
     const float* th = theta + s * M_eff;
     double re = 0.0, im = 0.0;
+    const int K = (!CPLX && series_ctl != nullptr) ? (int)*series_ctl : 0;
+    if (logpsi_out == nullptr && K == 0) return;           // nothing asked of this launch
     if constexpr (!CPLX) {
         // 128-bit loads over the padded row (theta of a padded hidden unit is exactly 0 and contributes ln cosh 0 = 0),
         // four independent fp64 accumulators
@@ -95,7 +113,24 @@ logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_p
                 if (j + 3 < M) theta_out[s * M + j + 3] = x.w;
             }
             r0 += take(x.x); r1 += take(x.y); r2 += take(x.z); r3 += take(x.w);
+            if (K > 0) {
+                const float t0 = tanhf(x.x), t1 = tanhf(x.y), t2 = tanhf(x.z), t3 = tanhf(x.w);
+                uint16_t* out = series_Ap + (size_t)s * SERIES_SEGS * M_pad + j;
+                const __half2 h01 = __floats2half2_rn(t0, t1), h23 = __floats2half2_rn(t2, t3);
+                const float2 f01 = __half22float2(h01), f23 = __half22float2(h23);
+                *reinterpret_cast<uint2*>(out) = make_uint2(*reinterpret_cast<const uint32_t*>(&h01),
+                                                            *reinterpret_cast<const uint32_t*>(&h23));
+                *reinterpret_cast<uint2*>(out + M_pad) = make_uint2(pack_h2(t0 - f01.x, t1 - f01.y),
+                                                                    pack_h2(t2 - f23.x, t3 - f23.y));
+                float p0 = t0 * t0, p1 = t1 * t1, p2 = t2 * t2, p3 = t3 * t3;
+                *reinterpret_cast<uint2*>(out + 2 * (size_t)M_pad) = make_uint2(pack_h2(p0, p1), pack_h2(p2, p3));
+                for (int k = 3; k <= K; ++k) {
+                    p0 *= t0; p1 *= t1; p2 *= t2; p3 *= t3;
+                    *reinterpret_cast<uint2*>(out + (size_t)k * M_pad) = make_uint2(pack_b2(p0, p1), pack_b2(p2, p3));
+                }
+            }
         }
+        if (logpsi_out == nullptr) return;
         __syncwarp();
         for (int k = lane; k < n_big; k += 32) {
             const double t = fabs((double)big[k]);
@@ -144,16 +179,18 @@ logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_p
 }
 
 cudaError_t launch_logpsi(const int8_t* sigma, int64_t B, const Geometry& g, int dtype, const float* theta,
-                          const void* a, void* logpsi_out, bool out_f64, void* theta_out, cudaStream_t st) {
+                          const void* a, void* logpsi_out, bool out_f64, void* theta_out, cudaStream_t st,
+                          const unsigned* series_ctl, uint16_t* series_Ap) {
     if (B <= 0) return cudaSuccess;
     const int wpb = dtype == NK_C64 ? 8 : LOGPSI_WARPS_REAL;
     const unsigned grid = (unsigned)((B + wpb - 1) / wpb);
     if (dtype == NK_C64)
         logpsi_kernel<true><<<grid, wpb * 32, 0, st>>>(sigma, B, g.N, g.M, g.M_pad, g.M_eff, theta, (const float*)a,
-                                                      logpsi_out, out_f64, (float*)theta_out);
+                                                      logpsi_out, out_f64, (float*)theta_out, nullptr, nullptr);
     else
         logpsi_kernel<false><<<grid, wpb * 32, 0, st>>>(sigma, B, g.N, g.M, g.M_pad, g.M_eff, theta, (const float*)a,
-                                                       logpsi_out, out_f64, (float*)theta_out);
+                                                       logpsi_out, out_f64, (float*)theta_out, series_ctl,
+                                                       series_Ap);
     count_launch();
     return cudaGetLastError();
 }

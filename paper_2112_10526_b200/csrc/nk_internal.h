@@ -148,7 +148,8 @@ cudaError_t launch_rbmsymm_reduce(int F, int G, int N, int dtype, const void* gW
                                   const int32_t* perms, void* gWsym, void* gbsym, cudaStream_t st);
 // logpsi.cu
 cudaError_t launch_logpsi(const int8_t* sigma, int64_t B, const Geometry& g, int dtype, const float* theta,
-                          const void* a, void* logpsi_out, bool out_f64, void* theta_out, cudaStream_t st);
+                          const void* a, void* logpsi_out, bool out_f64, void* theta_out, cudaStream_t st,
+                          const unsigned* series_ctl = nullptr, uint16_t* series_Ap = nullptr);
 // connected.cu
 cudaError_t launch_connected(const Operator* op, const int8_t* sigma, int64_t B, int32_t* flips, float* mels,
                              int32_t* n_conn, int8_t* sigma_prime, cudaStream_t st);
@@ -166,8 +167,7 @@ SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chu
 cudaError_t launch_series_pack(const Geometry& g, const float* Ttab, const unsigned* taumax_bits, const SeriesWs& w,
                                bool force, cudaStream_t st);
 cudaError_t launch_series_eloc(const Operator* op, const Geometry& g, const int8_t* sigma, int64_t nb,
-                               const float* theta, const RowInfo* rows, const SeriesWs& w, float* eloc_out,
-                               cudaStream_t st);
+                               const RowInfo* rows, const SeriesWs& w, float* eloc_out, cudaStream_t st);
 // fused_eloc.cu
 cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
                               const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,
@@ -179,5 +179,13 @@ cudaError_t launch_check_spins(const int8_t* sigma, int64_t n, int* flag, cudaSt
 cudaError_t launch_stats(const void* eloc, int64_t B, int dtype, double* stats_out, cudaStream_t st);
 
 void count_launch(int n = 1);
+
+// optional per-phase event timing (nk_profile_enable / nk_profile_read): brackets a group of launches on `st`
+enum Phase { PH_PACK = 0, PH_GEMM, PH_LOGPSI, PH_FUSED, PH_STATS, PH_SERIES_GEMM, PH_SERIES_PREP, PH_COUNT };
+struct ProfScope {
+    cudaStream_t st; int phase; cudaEvent_t a, b; bool on;
+    ProfScope(int phase, cudaStream_t st);
+    ~ProfScope();
+};
 
 }  // namespace nk

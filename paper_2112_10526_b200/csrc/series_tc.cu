@@ -138,60 +138,39 @@ series_bpow_kernel(const float* __restrict__ Ttab, int M_pad, int M_eff, const u
     }
 }
 
-// Ap[s][seg][j]: seg 0 / 1 = fp16 hi / lo of t = tanh(theta); seg 2 = fp16 t^2; seg k >= 3 = bf16 t^k.
-// One thread per 8 consecutive hidden units (one 16-B store per segment).
+// The sample-side operand Ap[s][seg][j] (seg 0 / 1 = fp16 hi / lo of t = tanh(theta); seg 2 = fp16 t^2; seg k >= 3 =
+// bf16 t^k) is written by logpsi_kernel (logpsi.cu) in its pass over theta.
+
+// sigT[i][w]: bit l of word w <=> sigma[32 w + l][i] = -1 (samples beyond nb: 0).  One warp = 32 samples x 16 sites:
+// lane l loads 16 spins of sample 32 w + l (one 16-B load when the rows allow it), 16 ballots transpose them.
 __global__ void __launch_bounds__(256)
-series_tpow_kernel(const float* __restrict__ theta, int64_t nb, int M_pad, int M_eff,
-                   const unsigned* __restrict__ ctl, uint16_t* __restrict__ Ap) {
-    const int K = (int)ctl[0];
-    if (K == 0) return;
-    const int per_row = M_pad / 8;
-    const int64_t total = nb * per_row;
-    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
-         idx += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t s = idx / per_row;
-        const int j0 = (int)(idx - s * per_row) * 8;
-        const float4 x0 = *reinterpret_cast<const float4*>(theta + s * M_eff + j0);
-        const float4 x1 = *reinterpret_cast<const float4*>(theta + s * M_eff + j0 + 4);
-        float t[8] = {tanhf(x0.x), tanhf(x0.y), tanhf(x0.z), tanhf(x0.w),
-                      tanhf(x1.x), tanhf(x1.y), tanhf(x1.z), tanhf(x1.w)};
-        uint16_t* out = Ap + (size_t)s * SERIES_SEGS * M_pad + j0;
-        uint16_t hi[8], v[8];
-#pragma unroll
-        for (int e = 0; e < 8; ++e) hi[e] = f2h(t[e]);
-        *reinterpret_cast<uint4*>(out) = *reinterpret_cast<const uint4*>(hi);
-#pragma unroll
-        for (int e = 0; e < 8; ++e) v[e] = f2h(t[e] - h2f(hi[e]));
-        *reinterpret_cast<uint4*>(out + M_pad) = *reinterpret_cast<const uint4*>(v);
-        float p[8];
-#pragma unroll
-        for (int e = 0; e < 8; ++e) p[e] = t[e];
-        for (int k = 2; k <= K; ++k) {
-#pragma unroll
-            for (int e = 0; e < 8; ++e) { p[e] *= t[e]; v[e] = k == 2 ? f2h(p[e]) : f2b(p[e]); }
-            *reinterpret_cast<uint4*>(out + (size_t)k * M_pad) = *reinterpret_cast<const uint4*>(v);
+series_bits_kernel(const int8_t* __restrict__ sigma, int64_t nb, int N, int w32, int n_groups,
+                   const unsigned* __restrict__ ctl, uint32_t* __restrict__ sigT) {
+    if (ctl[0] == 0) return;
+    const int lane = threadIdx.x & 31;
+    const int n16 = (N + 15) / 16;
+    const int64_t gw = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (gw >= (int64_t)n_groups * n16) return;
+    const int grp = (int)(gw / n16), i0 = (int)(gw - (int64_t)grp * n16) * 16;
+    const int64_t s = (int64_t)grp * 32 + lane;
+    uint32_t v[4] = {0x01010101u, 0x01010101u, 0x01010101u, 0x01010101u};      // +1: bit clear
+    if (s < nb) {
+        const int8_t* src = sigma + s * N + i0;
+        if ((N & 15) == 0 && (((uintptr_t)sigma) & 15) == 0) {
+            const uint4 q = *reinterpret_cast<const uint4*>(src);
+            v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+        } else {
+            for (int k = 0; k < 16 && i0 + k < N; ++k)
+                v[k >> 2] = (v[k >> 2] & ~(0xffu << (8 * (k & 3)))) | ((uint32_t)(uint8_t)src[k] << (8 * (k & 3)));
         }
     }
-}
-
-// sigT[i][w]: bit l of word w <=> sigma[32 w + l][i] = -1 (samples beyond nb: 0).  Block = 32 samples x 256 sites.
-__global__ void __launch_bounds__(256)
-series_bits_kernel(const int8_t* __restrict__ sigma, int64_t nb, int N, int w32, const unsigned* __restrict__ ctl,
-                   uint32_t* __restrict__ sigT) {
-    if (ctl[0] == 0) return;
-    __shared__ int8_t sm[32][256 + 4];
-    const int64_t s0 = (int64_t)blockIdx.x * 32;
-    const int i0 = blockIdx.y * 256;
-    for (int idx = threadIdx.x; idx < 32 * 256; idx += 256) {
-        const int l = idx >> 8, c = idx & 255;
-        sm[l][c] = (s0 + l < nb && i0 + c < N) ? sigma[(s0 + l) * N + i0 + c] : (int8_t)1;
+    uint32_t mine = 0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const uint32_t w = __ballot_sync(0xffffffffu, (v[k >> 2] >> (8 * (k & 3) + 7)) & 1u);
+        if (lane == k) mine = w;
     }
-    __syncthreads();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int c = warp; c < 256; c += 8) {
-        const unsigned w = __ballot_sync(0xffffffffu, sm[lane][c] < 0);
-        if (lane == 0 && i0 + c < N) sigT[(size_t)(i0 + c) * w32 + blockIdx.x] = w;
-    }
+    if (lane < 16 && i0 + lane < N) sigT[(size_t)(i0 + lane) * w32 + grp] = mine;
 }
 
 // ---- the GEMM with the fused local-energy epilogue ---------------------------------------------------------------
@@ -490,24 +469,20 @@ cudaError_t launch_series_pack(const Geometry& g, const float* Ttab, const unsig
     return cudaGetLastError();
 }
 
-// per chunk: E_loc of nb samples from theta (all four kernels return at once when ctl says the path is off)
+// per chunk: E_loc of nb samples from the operand rows launch_logpsi left in w.Ap (every kernel returns at once when
+// ctl says the path is off)
 cudaError_t launch_series_eloc(const Operator* op, const Geometry& g, const int8_t* sigma, int64_t nb,
-                               const float* theta, const RowInfo* rows, const SeriesWs& w, float* eloc_out,
-                               cudaStream_t st) {
+                               const RowInfo* rows, const SeriesWs& w, float* eloc_out, cudaStream_t st) {
     if (nb <= 0) return cudaSuccess;
     cudaError_t e = series_init();
     if (e != cudaSuccess) return e;
     const int sms = g_ser_sms[current_device()];
-    {
-        const int64_t total = nb * (g.M_pad / 8);
-        int64_t blocks = (total + 255) / 256;
-        if (blocks > (int64_t)sms * 16) blocks = (int64_t)sms * 16;
-        series_tpow_kernel<<<(unsigned)blocks, 256, 0, st>>>(theta, nb, g.M_pad, g.M_eff, w.ctl, w.Ap);
-    }
     const int n_mt = (int)((nb + ser::BM - 1) / ser::BM);
     {
-        dim3 grid((unsigned)(n_mt * 4), (unsigned)((g.N + 255) / 256));
-        series_bits_kernel<<<grid, 256, 0, st>>>(sigma, nb, g.N, w.w32, w.ctl, w.sigT);
+        ProfScope sc(PH_SERIES_PREP, st);
+        const int n_groups = n_mt * 4;
+        const int64_t warps = (int64_t)n_groups * ((g.N + 15) / 16);
+        series_bits_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(sigma, nb, g.N, w.w32, n_groups, w.ctl, w.sigT);
     }
     CUtensorMap map_a, map_b;
     const uint64_t cols = (uint64_t)SERIES_SEGS * g.M_pad;
@@ -517,11 +492,14 @@ cudaError_t launch_series_eloc(const Operator* op, const Geometry& g, const int8
     p.ctl = w.ctl; p.rows = rows; p.sigT = w.sigT; p.w32 = w.w32; p.nb = nb; p.n_rows = g.n_rows; p.M_pad = g.M_pad;
     p.n_mt = n_mt; p.n_nt = w.n_nt; p.part = w.part; p.part_stride = w.part_stride;
     const int n_tiles = n_mt * w.n_nt;
-    series_gemm_kernel<<<n_tiles < sms ? n_tiles : sms, ser::THREADS, ser::SMEM_BYTES, st>>>(map_a, map_b, p);
+    {
+        ProfScope sc(PH_SERIES_GEMM, st);
+        series_gemm_kernel<<<n_tiles < sms ? n_tiles : sms, ser::THREADS, ser::SMEM_BYTES, st>>>(map_a, map_b, p);
+    }
     series_finish_kernel<<<(unsigned)((nb + 7) / 8), 256, 0, st>>>(w.part, w.n_nt, w.part_stride, sigma, nb, g.N,
                                                                   op->kind, op->d_bonds, op->d_colors, op->d_Jf,
                                                                   op->n_bonds, w.ctl, eloc_out);
-    count_launch(4);
+    count_launch(3);
     return cudaGetLastError();
 }
 

@@ -128,12 +128,13 @@ def _rank_main(rank, world, port, q):
     e = rng.normal(size=1000)
     shard = e[rank::world]                                             # each rank owns a slice of the samples
     out = nk.allreduce_stats(torch.tensor(orc.stats(shard), dtype=torch.float64))
-    # gradient blocks: each rank's force with the GLOBAL mean, shards of unequal size, weighted all-reduce
+    # gradient blocks: each rank's share (1 / B_global) sum_{s in shard} O_s^* (E_s - GLOBAL mean) — what
+    # nk_energy_gradient_sharded returns — for shards of unequal size; the union's force is their plain sum
     O = rng.normal(size=(1000, 7)) + 1j * rng.normal(size=(1000, 7))
     ec = e + 1j * rng.normal(size=1000)
     mine = np.arange(1000) % 3 == 0 if rank == 0 else np.arange(1000) % 3 != 0
-    g_r = (np.conj(O[mine]) * (ec[mine] - ec.mean())[:, None]).mean(axis=0)
-    g = nk.allreduce_gradient([torch.from_numpy(g_r.copy()), torch.from_numpy(g_r.real.copy())], int(mine.sum()))
+    g_r = (np.conj(O[mine]) * (ec[mine] - ec.mean())[:, None]).sum(axis=0) / 1000.0
+    g = nk.allreduce_gradient([torch.from_numpy(g_r.copy()), torch.from_numpy(g_r.real.copy())])
     q.put((rank, out.tolist(), g[0].numpy().tolist(), g[1].numpy().tolist()))
     dist.destroy_process_group()
 
@@ -157,3 +158,31 @@ def test_allreduce_stats_gloo_world_size_2():
         np.testing.assert_allclose(res[r][0], orc.stats(e), rtol=1e-12, atol=1e-14)
         np.testing.assert_allclose(np.array(res[r][1]), want, atol=1e-13)
         np.testing.assert_allclose(np.array(res[r][2]), want.real, atol=1e-13)
+
+
+def test_bench_gpus_flag_spawns_one_rank_per_gpu():
+    """`python bench.py --gpus N` without a torchrun environment re-launches itself under torchrun with N ranks on
+    127.0.0.1 (it cannot print n_gpus: 1 for --gpus 8), and a rank started with the wrong WORLD_SIZE refuses to run."""
+    import argparse
+    import importlib.util
+    import os
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(root, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    args = argparse.Namespace(gpus=8, steps=7, warmup=3, config=5, impl="ours", no_extras=True)
+    cmd = bench.spawn_command(args, port=29511)
+    assert cmd[1:3] == ["-m", "torch.distributed.run"] and "--nproc-per-node=8" in cmd and "--nnodes=1" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29511"
+    tail = cmd[cmd.index(os.path.join(root, "bench.py")) + 1:]
+    assert tail == ["--gpus", "8", "--steps", "7", "--warmup", "3", "--config", "5", "--impl", "ours", "--no-extras"]
+
+
+def test_stats_combine_c_abi_rejects_bad_arguments():
+    import ctypes
+    lib = nk.load()
+    out = (ctypes.c_double * 4)()
+    assert lib.nk_stats_combine(None, 1, out) == -1
+    bad = (ctypes.c_double * 4)(0.0, 0.0, 1.0, -3.0)
+    assert lib.nk_stats_combine(bad, 1, out) == -1
+    assert lib.nk_stats_combine(bad, 0, out) == 0 and list(out) == [0.0, 0.0, 0.0, 0.0]
