@@ -58,8 +58,10 @@ enum nk_flags {
     NK_CHECK_SPINS = 8u,       /* nk_local_energy_ex: validate sigma in {+1,-1} first (one extra pass over sigma and one
                                   stream synchronisation); NK_ERR_BAD_SPIN before any other launch if it is not */
     NK_FORM_LOGCOSH = 16u,     /* nk_local_energy_ex: log-cosh amplitude ratios (see there) */
-    NK_FORM_SERIES = 32u       /* nk_local_energy_ex: product form with the logarithm expanded into a short series of
+    NK_FORM_SERIES = 32u,      /* nk_local_energy_ex: product form with the logarithm expanded into a short series of
                                   tensor-core GEMMs (see there); real parameters only */
+    NK_SERIAL_CHUNKS = 64u     /* nk_local_energy_ex: keep every kernel of the chunk loop on `stream` (no internal second
+                                  stream); same results, used to time kernels in isolation */
 };
 
 /* Static, never-NULL description of a status code. */
@@ -144,6 +146,12 @@ int nk_local_energy(nk_operator_t op, const int8_t* sigma, int64_t B, int N, int
  *    synchronisation (every kernel is launched, those on the wrong side of the gates return at once).  Complex
  *    parameters: always the log-cosh form.  The choice depends on the parameters only, never on sigma, B or chunk_size.
  *  The NK_FORM_* flags are mutually exclusive (NK_ERR_INVALID_ARG).
+ * Streams: when the series form may run and the batch has more than one chunk, the preparation of chunk c + 1 (theta
+ * contraction, the ln psi / operand pass, spin bits) is issued on one internal high-priority stream per calling thread
+ * (created on first use, with five events) beside the tensor-core kernel of chunk c on `stream`; the internal stream
+ * forks from and joins `stream` through events, so everything the caller observes is ordered on `stream` and the call
+ * stays capturable in a CUDA graph.  The per-chunk buffers then exist twice in the workspace.  NK_SERIAL_CHUNKS keeps
+ * everything on `stream`.
  * NK_CHECK_SPINS: validate sigma first (see enum nk_flags); may be combined with a form flag. */
 int nk_local_energy_ex(nk_operator_t op, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
                        const void* a, const void* b, int64_t chunk_size, unsigned flags, void* eloc_out,

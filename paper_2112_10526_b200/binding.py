@@ -12,11 +12,12 @@ import numpy as np
 
 __all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host", "energy_gradient",
            "qgt_matvec", "sr_solve", "rbmsymm_expand", "rbmsymm_reduce_gradient", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "pipe_peaks", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "allreduce_gradient", "LIB_PATH",
-           "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "NK_FORM_PRODUCT", "NK_CHECK_SPINS", "NK_FORM_LOGCOSH", "NK_FORM_SERIES", "EXPORTS"]
+           "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "NK_FORM_PRODUCT", "NK_CHECK_SPINS", "NK_FORM_LOGCOSH", "NK_FORM_SERIES", "NK_SERIAL_CHUNKS", "EXPORTS"]
 
 NK_HEISENBERG, NK_ISING = 0, 1
 NK_F32, NK_C64 = 0, 1
 NK_FLAG_MARSHALL, NK_OUT_F64, NK_FORM_PRODUCT, NK_CHECK_SPINS, NK_FORM_LOGCOSH, NK_FORM_SERIES = 1, 2, 4, 8, 16, 32
+NK_SERIAL_CHUNKS = 64
 NK_RULE_LOCAL, NK_RULE_EXCHANGE = 0, 1
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libnkb200.so")
 

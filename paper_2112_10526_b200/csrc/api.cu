@@ -39,6 +39,28 @@ typedef ProfScope Scope;
 
 // nk_local_energy_host overlaps its host->device copies with the chunk loop: when this is set, chunk k of
 // nk_local_energy_ex first makes the call's stream wait on event k (sigma of that chunk has arrived).
+// internal stream + events of the pipelined chunk loop (nk_local_energy_ex), one set per calling thread and device
+static thread_local cudaStream_t tl_prep_stream = nullptr;
+static thread_local int tl_prep_device = -1;
+static thread_local cudaEvent_t tl_pipe_events[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+static cudaError_t pipeline_objects() {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (tl_prep_stream != nullptr && tl_prep_device == dev) return cudaSuccess;
+    int lo = 0, hi = 0;
+    e = cudaDeviceGetStreamPriorityRange(&lo, &hi);                   // hi = the numerically smallest = greatest priority
+    if (e != cudaSuccess) return e;
+    e = cudaStreamCreateWithPriority(&tl_prep_stream, cudaStreamNonBlocking, hi);
+    if (e != cudaSuccess) return e;
+    for (int k = 0; k < 5; ++k) {
+        e = cudaEventCreateWithFlags(&tl_pipe_events[k], cudaEventDisableTiming);
+        if (e != cudaSuccess) return e;
+    }
+    tl_prep_device = dev;
+    return cudaSuccess;
+}
+
 static thread_local const std::vector<cudaEvent_t>* tl_chunk_ready = nullptr;
 static thread_local cudaStream_t tl_copy_stream = nullptr;
 static thread_local std::vector<cudaEvent_t> tl_copy_events;
@@ -123,15 +145,18 @@ static LogpsiWs carve_logpsi(void* ws, const Geometry& g, int64_t rows) {
     return w;
 }
 struct ElocWs {
-    float *Wg, *bg, *Wt, *Dtab, *Ttab, *theta;        // Dtab: log-cosh form, Ttab: product form (both when automatic)
-    uint16_t *Ws, *A;
+    float *Wg, *bg, *Wt, *Dtab, *Ttab;                // Dtab: log-cosh form, Ttab: product form (both when automatic)
+    float* theta[2];                                  // per-chunk buffers: two sets when the chunk loop is pipelined
+    uint16_t* A[2];
+    int n_sets;
+    uint16_t* Ws;
     unsigned *absmax, *taumax;                        // taumax: max |tanh delta| of Ttab as float bits (the form gate)
     RowInfo* rows;
     bool has_series;                                  // the tensor-core series form is possible for these sizes
     SeriesWs ser;
     size_t bytes;
 };
-static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk, int dtype) {
+static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk, int dtype, int64_t B) {
     Carver c(ws);
     ElocWs w;
     w.Wg = c.take<float>((size_t)g.M_eff * g.N);
@@ -139,14 +164,22 @@ static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk, int dtype) 
     w.Wt = c.take<float>((size_t)g.N * g.M_eff);
     w.Dtab = c.take<float>((size_t)g.n_rows_pad * g.M_eff);
     w.rows = c.take<RowInfo>(g.n_rows_pad);
-    w.theta = c.take<float>((size_t)chunk * g.M_eff);
+    w.has_series = series_possible(g, dtype);
+    // the series form pipelines consecutive chunks over two streams (preparation of chunk c + 1 beside the tensor-core
+    // kernel of chunk c): theta, the padded spins and the series operands exist twice when there is more than one chunk
+    w.n_sets = (w.has_series && chunk < B) ? 2 : 1;
+    w.theta[0] = c.take<float>((size_t)chunk * g.M_eff);
     w.Ws = c.take<uint16_t>((size_t)3 * g.M_eff * g.K_pad);
-    w.A = c.take<uint16_t>((size_t)chunk * g.K_pad);
+    w.A[0] = c.take<uint16_t>((size_t)chunk * g.K_pad);
     w.absmax = c.take<unsigned>(1);
     w.taumax = c.take<unsigned>(1);
     w.Ttab = c.take<float>((size_t)g.n_rows_pad * g.M_eff);
-    w.has_series = series_possible(g, dtype);
-    if (w.has_series) w.ser = carve_series(c.base, &c.off, g, chunk);
+    w.theta[1] = w.theta[0]; w.A[1] = w.A[0];
+    if (w.n_sets == 2) {
+        w.theta[1] = c.take<float>((size_t)chunk * g.M_eff);
+        w.A[1] = c.take<uint16_t>((size_t)chunk * g.K_pad);
+    }
+    if (w.has_series) w.ser = carve_series(c.base, &c.off, g, chunk, w.n_sets);
     w.bytes = c.off;
     return w;
 }
@@ -345,7 +378,7 @@ int nk_rbm_logpsi(const int8_t* sigma, int64_t B, int N, int M, int dtype, const
     cudaStream_t st = (cudaStream_t)stream;
     const LogpsiWs w = carve_logpsi(workspace, g, B);
     NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.Wg, w.bg, st));
-    NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
+    NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, st));
     NK_CUDA(run_theta(g, sigma, B, w.Wg, w.bg, w.Ws, w.A, w.theta, st));
     NK_CUDA(launch_logpsi(sigma, B, g, dtype, w.theta, a, logpsi_out, (flags & NK_OUT_F64) != 0, theta_out, st));
     return NK_OK;
@@ -395,7 +428,7 @@ int nk_energy_gradient_sharded(const int8_t* sigma, int64_t B, int64_t B_global,
     cudaStream_t st = (cudaStream_t)stream;
     const size_t esz = dtype == NK_C64 ? 8 : 4;
     NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.Wg, w.bg, st));
-    NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
+    NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, st));
     int first = 1;
     for (int64_t s0 = 0; s0 < B; s0 += chunk) {
         const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
@@ -449,10 +482,10 @@ static int qgt_matvec_impl(const int8_t* sigma, int64_t B, int N, int M, int dty
     // operands of the two contractions: (W, b) -> theta (not needed when theta is cached) and (V_W, v_b) -> Y
     if (cache == nullptr) {
         NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.g.Wg, w.g.bg, st));
-        NK_CUDA(launch_split_w(w.g.Wg, g.M_eff, N, g.K_pad, w.g.Ws, w.g.absmax, st));
+        NK_CUDA(launch_split_w(w.g.Wg, g.M_eff, N, g.K_pad, w.g.Ws, st));
     }
     NK_CUDA(launch_pack_gemm_only(g, dtype, v_W, v_b, w.Vg, w.vbg, st));
-    NK_CUDA(launch_split_w(w.Vg, g.M_eff, N, g.K_pad, w.Vs, w.g.absmax, st));
+    NK_CUDA(launch_split_w(w.Vg, g.M_eff, N, g.K_pad, w.Vs, st));
     // step 1 of Eq. (75): w_s = (J v)_s for every sample
     for (int64_t s0 = 0; s0 < B; s0 += chunk) {
         const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
@@ -572,7 +605,7 @@ int nk_sr_solve(const int8_t* sigma, int64_t B, int N, int M, int dtype, const v
         const QgtWs q = carve_qgt(w.qgt, g, B, eff_chunk(B, chunk_size), dtype);
         const int64_t chunk = eff_chunk(B, chunk_size);
         NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, q.g.Wg, q.g.bg, st));
-        NK_CUDA(launch_split_w(q.g.Wg, g.M_eff, N, g.K_pad, q.g.Ws, q.g.absmax, st));
+        NK_CUDA(launch_split_w(q.g.Wg, g.M_eff, N, g.K_pad, q.g.Ws, st));
         NK_CUDA(launch_sigma_operand(sigma, B, N, g.K_pad, w.cache.A_all, st));
         for (int64_t s0 = 0; s0 < B; s0 += chunk) {
             const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
@@ -678,7 +711,7 @@ int nk_metropolis_sample(int rule, const int32_t* clusters_host, int n_clusters,
                                 cudaMemcpyHostToDevice, st));
     NK_CUDA(launch_pack_table(g, dtype, W, b, rule == NK_RULE_EXCHANGE ? w.pairs : nullptr, n_rows, w.Wg, w.bg, w.Wt,
                               w.Dtab, st));
-    NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
+    NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, st));
     SamplerArgs sa;
     sa.rule = rule; sa.n_idx = n_rows; sa.pairs = rule == NK_RULE_EXCHANGE ? w.pairs : nullptr; sa.a = a;
     sa.n_steps = n_steps; sa.seed = seed; sa.step_offset = step_offset;
@@ -696,7 +729,7 @@ size_t nk_local_energy_workspace_bytes(nk_operator_t h, int64_t B, int N, int M,
     if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0) return 0;
     const Operator* op = (const Operator*)h;
     const Geometry g = make_geometry(op, N, M, dtype);
-    return carve_eloc(nullptr, g, eff_chunk(B, chunk_size), dtype).bytes;
+    return carve_eloc(nullptr, g, eff_chunk(B, chunk_size), dtype, B).bytes;
 }
 
 int nk_local_energy(nk_operator_t h, const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W,
@@ -711,7 +744,7 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
                        void* logpsi_out, double* stats_out, void* workspace, size_t workspace_bytes,
                        nk_stream_t stream) {
     if (!h || bad_dims(B, N, M, dtype) || chunk_size < 0 || !W || (B > 0 && (!sigma || !eloc_out)) ||
-        (flags & ~(NK_FORM_PRODUCT | NK_FORM_LOGCOSH | NK_FORM_SERIES | NK_CHECK_SPINS)))
+        (flags & ~(NK_FORM_PRODUCT | NK_FORM_LOGCOSH | NK_FORM_SERIES | NK_CHECK_SPINS | NK_SERIAL_CHUNKS)))
         return NK_ERR_INVALID_ARG;
     {
         const unsigned forms = flags & (NK_FORM_PRODUCT | NK_FORM_LOGCOSH | NK_FORM_SERIES);
@@ -727,10 +760,10 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
     const Geometry g = make_geometry(op, N, M, dtype);
     if (!g.ok) return NK_ERR_UNSUPPORTED;
     const int64_t chunk = eff_chunk(B, chunk_size);
-    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_eloc(nullptr, g, chunk, dtype).bytes)
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_eloc(nullptr, g, chunk, dtype, B).bytes)
         return NK_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
-    const ElocWs w = carve_eloc(workspace, g, chunk, dtype);
+    const ElocWs w = carve_eloc(workspace, g, chunk, dtype, B);
     if (force_series && !w.has_series) return NK_ERR_UNSUPPORTED;       // complex parameters or a tiny problem
     const bool series = w.has_series && (automatic || force_series);
     if ((flags & NK_CHECK_SPINS) && B > 0) {           // opt-in validation: one pass over sigma and one synchronisation
@@ -748,36 +781,58 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
             NK_CUDA(launch_pack_product(op, g, dtype, w.Wt, w.Ttab, w.rows, st,
                                         (automatic || force_series) ? w.taumax : nullptr));
         if (series) NK_CUDA(launch_series_pack(g, w.Ttab, w.taumax, w.ser, force_series, st));
-        NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, w.absmax, st));
+        NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, st));
     }
     const size_t esz = dtype == NK_C64 ? 8 : 4;
-    for (int64_t s0 = 0; s0 < B; s0 += chunk) {
+    // Two streams when the series form may run over several chunks: the preparation of a chunk (theta contraction, the
+    // ln psi / operand pass, spin bits) goes to an internal high-priority stream `ps`, the tensor-core kernel and what
+    // follows it stay on the caller's stream, each buffer set is handed over by an event — the preparation of chunk
+    // c + 1 fills the tail (and the idle ALUs) of the GEMM of chunk c.  Everything the caller observes is ordered on
+    // `stream`; the construction is capturable in a CUDA graph (the internal stream forks from and joins `stream`).
+    const bool pipelined = series && w.n_sets == 2 && !(flags & NK_SERIAL_CHUNKS);
+    cudaStream_t ps = st;
+    if (pipelined) {
+        NK_CUDA(pipeline_objects());
+        ps = tl_prep_stream;
+        NK_CUDA(cudaEventRecord(tl_pipe_events[0], st));              // parameters packed; earlier work on `stream` done
+        NK_CUDA(cudaStreamWaitEvent(ps, tl_pipe_events[0], 0));
+    }
+    int64_t ci = 0;
+    for (int64_t s0 = 0; s0 < B; s0 += chunk, ++ci) {
         const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
         const int8_t* sg = sigma + s0 * N;
-        if (tl_chunk_ready != nullptr) NK_CUDA(cudaStreamWaitEvent(st, (*tl_chunk_ready)[(size_t)(s0 / chunk)], 0));
+        const int set = pipelined ? (int)(ci & 1) : 0;
+        cudaEvent_t ev_prep = tl_pipe_events[1 + set], ev_done = tl_pipe_events[3 + set];
+        if (pipelined && ci >= 2) NK_CUDA(cudaStreamWaitEvent(ps, ev_done, 0));    // chunk c - 2 no longer reads this set
+        if (tl_chunk_ready != nullptr) NK_CUDA(cudaStreamWaitEvent(ps, (*tl_chunk_ready)[(size_t)(s0 / chunk)], 0));
         {
-            Scope sc(PH_GEMM, st);
-            NK_CUDA(run_theta(g, sg, nb, w.Wg, w.bg, w.Ws, w.A, w.theta, st));
+            Scope sc(PH_GEMM, ps);
+            NK_CUDA(run_theta(g, sg, nb, w.Wg, w.bg, w.Ws, w.A[set], w.theta[set], ps));
         }
         if (logpsi_out || series) {            // ln psi and, in the same pass over theta, the series form's operand rows
-            Scope sc(PH_LOGPSI, st);
-            NK_CUDA(launch_logpsi(sg, nb, g, dtype, w.theta, a, logpsi_out ? (uint8_t*)logpsi_out + s0 * esz : nullptr,
-                                  false, nullptr, st, series ? w.ser.ctl : nullptr, series ? w.ser.Ap : nullptr));
+            Scope sc(PH_LOGPSI, ps);
+            NK_CUDA(launch_logpsi(sg, nb, g, dtype, w.theta[set], a, logpsi_out ? (uint8_t*)logpsi_out + s0 * esz : nullptr,
+                                  false, nullptr, ps, series ? w.ser.ctl : nullptr, series ? w.ser.Ap[set] : nullptr));
+        }
+        if (series) NK_CUDA(launch_series_prep(g, sg, nb, w.ser, set, ps));
+        if (pipelined) {
+            NK_CUDA(cudaEventRecord(ev_prep, ps));
+            NK_CUDA(cudaStreamWaitEvent(st, ev_prep, 0));
         }
         {
             Scope sc(PH_FUSED, st);
             void* out = (uint8_t*)eloc_out + s0 * esz;
-            if (series) NK_CUDA(launch_series_eloc(op, g, sg, nb, w.rows, w.ser, (float*)out, st));
+            if (series) NK_CUDA(launch_series_eloc(op, g, sg, nb, w.rows, w.ser, set, (float*)out, st));
             if (automatic) {           // every launch; those on the wrong side of the gates return at once
                 const unsigned* sctl = series ? w.ser.ctl : nullptr;
-                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Ttab, w.rows, out, true, st, w.taumax, 1, sctl));
-                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Dtab, w.rows, out, false, st, w.taumax, 2, sctl));
-            } else if (force_series) {
-            } else {
-                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, force_product ? w.Ttab : w.Dtab, w.rows, out,
+                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], w.Ttab, w.rows, out, true, st, w.taumax, 1, sctl));
+                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], w.Dtab, w.rows, out, false, st, w.taumax, 2, sctl));
+            } else if (!force_series) {
+                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], force_product ? w.Ttab : w.Dtab, w.rows, out,
                                           force_product, st));
             }
         }
+        if (pipelined) NK_CUDA(cudaEventRecord(ev_done, st));
     }
     if (stats_out) {
         Scope sc(PH_STATS, st);
@@ -814,9 +869,9 @@ int nk_local_energy_form(nk_operator_t h, int64_t B, int N, int M, int dtype, in
     const Geometry g = make_geometry(op, N, M, dtype);
     if (!g.ok) return NK_ERR_UNSUPPORTED;
     const int64_t chunk = eff_chunk(B, chunk_size);
-    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_eloc(nullptr, g, chunk, dtype).bytes)
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < carve_eloc(nullptr, g, chunk, dtype, B).bytes)
         return NK_ERR_WORKSPACE;
-    const ElocWs w = carve_eloc(const_cast<void*>(workspace), g, chunk, dtype);
+    const ElocWs w = carve_eloc(const_cast<void*>(workspace), g, chunk, dtype, B);
     float tau = 0.f;
     unsigned K = 0;
     cudaStream_t st = (cudaStream_t)stream;

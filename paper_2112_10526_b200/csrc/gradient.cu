@@ -137,6 +137,10 @@ __global__ void grad_slab_reduce_kernel(const double* __restrict__ part, int n_s
         }
         scale_io[2] = __float_as_uint(ldexpf(1.f, 23 - ex));
         scale_io[3] = __float_as_uint(ldexpf(1.f, ex - 23));
+        if (scale_io[0] >= 0x7f800000u) {                     // a NaN / Inf local energy or mean: poison the block
+            scale_io[2] = 0u;                                 // (zero digits, q = NaN: q D is NaN, Q14)
+            scale_io[3] = 0x7fc00000u;
+        }
     }
     __shared__ double sh[8][32];
     const int c = blockIdx.x * 32 + threadIdx.x;
@@ -167,7 +171,8 @@ __global__ void grad_split_T_kernel(const float* __restrict__ v, int64_t nb, int
         frexpf(vmax, &ex);
         if (ldexpf(vmax, 23 - ex) > 8355000.f) ++ex;      // keep the top digit inside [-128, 127]
     }
-    const float sc = ldexpf(1.f, 23 - ex);
+    const bool poison = *absmax_bits >= 0x7f800000u;      // NaN / Inf among the v: zero digits, q = NaN (Q14)
+    const float sc = poison ? 0.f : ldexpf(1.f, 23 - ex);
     const int s0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
         const int64_t s = s0 + r;
@@ -178,7 +183,7 @@ __global__ void grad_split_T_kernel(const float* __restrict__ v, int64_t nb, int
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
         const int me = m0 + r, s = s0 + threadIdx.x;
         if (s >= k_len) continue;
-        const int I = (int)rintf(tile[threadIdx.x][r] * sc);
+        const int I = poison ? 0 : (int)rintf(tile[threadIdx.x][r] * sc);
         const int d0 = ((I + 128) & 255) - 128;
         const int I1 = (I - d0) >> 8;
         const int d1 = ((I1 + 128) & 255) - 128;
@@ -188,7 +193,7 @@ __global__ void grad_split_T_kernel(const float* __restrict__ v, int64_t nb, int
         TwT[2 * plane + o] = (int8_t)d0;
     }
     if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && threadIdx.y == 0)
-        *reinterpret_cast<float*>(TwT + 3 * plane) = ldexpf(1.f, ex - 23);
+        *reinterpret_cast<float*>(TwT + 3 * plane) = poison ? __int_as_float(0x7fc00000) : ldexpf(1.f, ex - 23);
 }
 
 // tanh in fp32 without branches: |x| < 1 by x + x^3 P(x^2) (P = degree-6 least-squares fit of (tanh x - x) / x^3 in x^2,

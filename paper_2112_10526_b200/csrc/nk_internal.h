@@ -102,8 +102,7 @@ cudaError_t launch_metropolis(const Geometry& g, int dtype, int8_t* sigma, int64
 // theta_tc.cu : the same contraction on tcgen05 tensor cores (kind::i8, three int8 digit planes of W, three int32
 // TMEM accumulators); Ws = the planes + scale, A = scratch for a padded int8 copy of the spins when N % 128 != 0
 cudaError_t theta_tc_init();
-cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* Ws, unsigned* absmax_scratch,
-                           cudaStream_t st);
+cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* Ws, cudaStream_t st);
 cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, int K_pad, const void* Ws,
                             void* A, const float* bg, float* theta, cudaStream_t st);
 cudaError_t launch_sigma_operand(const int8_t* sigma, int64_t B, int N, int K_pad, void* A_i8, cudaStream_t st);
@@ -156,18 +155,22 @@ cudaError_t launch_connected(const Operator* op, const int8_t* sigma, int64_t B,
 // series_tc.cu : amplitude ratios as a short series of tensor-core GEMMs (product form, logarithm expanded)
 struct SeriesWs {
     unsigned* ctl;              // [16] control block written per call: ctl[0] = K (0 = path off), scales, row bounds
-    uint16_t *Bp, *Ap;          // [n_rows][SERIES_SEGS][M_pad], [chunk][SERIES_SEGS][M_pad] 16-bit operand rows
-    uint32_t* sigT;             // [N][w32] transposed bit-packed spins of the chunk
-    float* part;                // [n_nt][part_stride] partial local energies per column tile
+    uint16_t* Bp;               // [n_rows][SERIES_SEGS][M_pad] 16-bit operand rows of the table (per call)
+    // per-chunk buffers, two sets when the chunk loop is pipelined over two streams (api.cu):
+    uint16_t* Ap[2];            // [chunk][SERIES_SEGS][M_pad] 16-bit operand rows of the samples
+    uint32_t* sigT[2];          // [N][w32] transposed bit-packed spins of the chunk
+    float* part[2];             // [n_nt][part_stride] partial local energies per column tile
     int w32, n_nt;
     int64_t part_stride;
 };
 bool series_possible(const Geometry& g, int dtype);
-SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk);
+SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk, int n_sets);
+cudaError_t launch_series_prep(const Geometry& g, const int8_t* sigma, int64_t nb, const SeriesWs& w, int set,
+                               cudaStream_t st);
 cudaError_t launch_series_pack(const Geometry& g, const float* Ttab, const unsigned* taumax_bits, const SeriesWs& w,
                                bool force, cudaStream_t st);
 cudaError_t launch_series_eloc(const Operator* op, const Geometry& g, const int8_t* sigma, int64_t nb,
-                               const RowInfo* rows, const SeriesWs& w, float* eloc_out, cudaStream_t st);
+                               const RowInfo* rows, const SeriesWs& w, int set, float* eloc_out, cudaStream_t st);
 // fused_eloc.cu
 cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
                               const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,

@@ -24,10 +24,8 @@
 //
 // Kernel (series_gemm_kernel): persistent, one CTA per SM, 128 (samples) x 256 (table rows) tiles, tcgen05.mma
 // kind::f16 M = 128, N = 256, K = 16 issued by one thread; accumulators odd / even fill the 512 TMEM columns.  The two
-// operands flow through SEPARATE shared-memory rings (4 x 16 KB and 4 x 32 KB, 128B-swizzled TMA boxes of 64 hidden
-// units), each with its own producer warp, because a tile is used by more than one pass: t_hi by passes 2 and 3,
-// tau_hi by passes 1 and 2 — K + 1 tiles of each operand are loaded per block of hidden units for K + 2 passes, and a
-// ring slot is handed back by the tcgen05.commit of the last pass that reads it.  Four epilogue warps (one TMEM lane
+// operands flow through separate shared-memory rings (4 x 16 KB and 4 x 32 KB, 128B-swizzled TMA boxes of 64 hidden
+// units), each with its own producer warp.  Four epilogue warps (one TMEM lane
 // quarter each) read both accumulators, form the exponent, take 2^x, multiply by the matrix element, mask by the
 // sample's spins (antiparallel bond / sign of s from bit-packed transposed spins) and sum over the tile's rows —
 // [samples] x [rows] never leaves the SM.  Partial sums per column tile go to `part`, summed in a fixed order by
@@ -234,35 +232,54 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem_base = *tmem_slot_ptr;
 
+    // Order of the passes inside a tile.  The tensor core adds every product to the fp32 accumulator on the accumulator's
+    // own grid (measured: a bias of 2048 half-ulps when 2048 same-sign products meet a large running sum, and products
+    // below the grid are lost), so SMALL terms go first, while the sums are small:
+    //   sweep 1 over the blocks of hidden units:  k = K .. 3 (bf16), then the two fp16 lo passes t_lo tau_hi, t_hi tau_lo
+    //   sweep 2:                                  k = 2, then the dominant t_hi tau_hi
+    // (the first version ran all passes of a block together: E_loc came out 7e-6 high — the k = 4 and lo terms were
+    // being added to full-size sums.)  t_hi and tau_hi are therefore loaded in both sweeps: K + 2 tiles of each operand
+    // per block for K + 2 passes.  A ring slot is handed back by the tcgen05.commit of the last pass that reads it.
     if (warp == 0) {
-        // ===== A producer: per block of hidden units the tiles t_lo, t_hi, t^2 .. t^K of this sample tile =====
+        // ===== A producer =====
         if (lane == 0) {
             uint32_t it = 0;
+            auto load = [&](int seg, int jb, int m0) {
+                const uint32_t slot = it % NA, par = ((it / NA) & 1u) ^ 1u;
+                mbar_wait(a_empty + 8 * slot, par);
+                mbar_arrive_expect_tx(a_full + 8 * slot, A_TILE);
+                tma_load_2d(a_ring + slot * A_TILE, &map_a, seg * p.M_pad + jb * BK, m0, a_full + 8 * slot);
+                ++it;
+            };
             for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
                 const int m0 = (tile / p.n_nt) * BM;
-                for (int jb = 0; jb < n_jb; ++jb)
-                    for (int idx = 0; idx <= K; ++idx, ++it) {
-                        const int seg = idx == 0 ? 1 : (idx == 1 ? 0 : idx);
-                        const uint32_t slot = it % NA, par = ((it / NA) & 1u) ^ 1u;
-                        mbar_wait(a_empty + 8 * slot, par);
-                        mbar_arrive_expect_tx(a_full + 8 * slot, A_TILE);
-                        tma_load_2d(a_ring + slot * A_TILE, &map_a, seg * p.M_pad + jb * BK, m0, a_full + 8 * slot);
-                    }
+                for (int jb = 0; jb < n_jb; ++jb) {
+                    for (int k = K; k >= 3; --k) load(k, jb, m0);
+                    load(1, jb, m0);                       // t_lo
+                    load(0, jb, m0);                       // t_hi
+                }
+                for (int jb = 0; jb < n_jb; ++jb) { load(2, jb, m0); load(0, jb, m0); }
             }
         }
     } else if (warp == 2) {
-        // ===== B producer: tau_hi, tau_lo, tau^2 .. tau^K of this row tile =====
+        // ===== B producer =====
         if (lane == 0) {
             uint32_t it = 0;
+            auto load = [&](int seg, int jb, int n0) {
+                const uint32_t slot = it % NB, par = ((it / NB) & 1u) ^ 1u;
+                mbar_wait(b_empty + 8 * slot, par);
+                mbar_arrive_expect_tx(b_full + 8 * slot, B_TILE);
+                tma_load_2d(b_ring + slot * B_TILE, &map_b, seg * p.M_pad + jb * BK, n0, b_full + 8 * slot);
+                ++it;
+            };
             for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
                 const int n0 = (tile % p.n_nt) * BN;
-                for (int jb = 0; jb < n_jb; ++jb)
-                    for (int seg = 0; seg <= K; ++seg, ++it) {
-                        const uint32_t slot = it % NB, par = ((it / NB) & 1u) ^ 1u;
-                        mbar_wait(b_empty + 8 * slot, par);
-                        mbar_arrive_expect_tx(b_full + 8 * slot, B_TILE);
-                        tma_load_2d(b_ring + slot * B_TILE, &map_b, seg * p.M_pad + jb * BK, n0, b_full + 8 * slot);
-                    }
+                for (int jb = 0; jb < n_jb; ++jb) {
+                    for (int k = K; k >= 3; --k) load(k, jb, n0);
+                    load(0, jb, n0);                       // tau_hi
+                    load(1, jb, n0);                       // tau_lo
+                }
+                for (int jb = 0; jb < n_jb; ++jb) { load(2, jb, n0); load(0, jb, n0); }
             }
         }
     } else if (warp == 1) {
@@ -270,37 +287,47 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
         if (lane == 0) {
             uint32_t ia = 0, ib = 0, n_done = 0;
             const uint32_t acc_odd = tmem_base, acc_even = tmem_base + BN;
+            bool fresh_odd = true, fresh_even = true;
             auto a_wait = [&](uint32_t i) { mbar_wait(a_full + 8 * (i % NA), (i / NA) & 1u); };
             auto b_wait = [&](uint32_t i) { mbar_wait(b_full + 8 * (i % NB), (i / NB) & 1u); };
-            auto pass = [&](uint32_t sa, uint32_t sb, uint32_t acc, uint32_t idesc, bool fresh) {
+            auto pass = [&](uint32_t sa, uint32_t sb, bool odd, uint32_t idesc) {
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const uint32_t a_addr = a_ring + (sa % NA) * A_TILE, b_addr = b_ring + (sb % NB) * B_TILE;
+                bool& fresh = odd ? fresh_odd : fresh_even;
 #pragma unroll
                 for (int k = 0; k < BK / 16; ++k)          // 16 elements = 32 B inside the 128-B swizzle row
-                    umma_f16(acc, make_sdesc(a_addr + k * 32), make_sdesc(b_addr + k * 32), idesc,
+                    umma_f16(odd ? acc_odd : acc_even, make_sdesc(a_addr + k * 32), make_sdesc(b_addr + k * 32), idesc,
                              (fresh && k == 0) ? 0u : 1u);
+                fresh = false;
             };
+            auto a_free = [&](uint32_t i) { umma_commit(a_empty + 8 * (i % NA)); };
+            auto b_free = [&](uint32_t i) { umma_commit(b_empty + 8 * (i % NB)); };
             for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++n_done) {
                 mbar_wait(t_empty, (n_done & 1u) ^ 1u);    // the epilogue has drained the accumulators (free at first)
-                for (int jb = 0; jb < n_jb; ++jb) {
+                fresh_odd = fresh_even = true;
+                for (int jb = 0; jb < n_jb; ++jb) {        // sweep 1: the small terms
+                    for (int k = K; k >= 3; --k, ++ia, ++ib) {
+                        a_wait(ia); b_wait(ib);
+                        pass(ia, ib, (k & 1) != 0, IDESC_BF16);
+                        a_free(ia); b_free(ib);
+                    }
                     const uint32_t a_lo = ia, a_hi = ia + 1, b_hi = ib, b_lo = ib + 1;
                     a_wait(a_lo); b_wait(b_hi);
-                    pass(a_lo, b_hi, acc_odd, IDESC_F16, jb == 0);
-                    umma_commit(a_empty + 8 * (a_lo % NA));
-                    a_wait(a_hi);
-                    pass(a_hi, b_hi, acc_odd, IDESC_F16, false);
-                    umma_commit(b_empty + 8 * (b_hi % NB));
-                    b_wait(b_lo);
-                    pass(a_hi, b_lo, acc_odd, IDESC_F16, false);
-                    umma_commit(a_empty + 8 * (a_hi % NA));
-                    umma_commit(b_empty + 8 * (b_lo % NB));
+                    pass(a_lo, b_hi, true, IDESC_F16);
+                    a_free(a_lo); b_free(b_hi);
+                    a_wait(a_hi); b_wait(b_lo);
+                    pass(a_hi, b_lo, true, IDESC_F16);
+                    a_free(a_hi); b_free(b_lo);
                     ia += 2; ib += 2;
-                    for (int k = 2; k <= K; ++k, ++ia, ++ib) {
-                        a_wait(ia); b_wait(ib);
-                        pass(ia, ib, (k & 1) ? acc_odd : acc_even, k == 2 ? IDESC_F16 : IDESC_BF16, jb == 0 && k == 2);
-                        umma_commit(a_empty + 8 * (ia % NA));
-                        umma_commit(b_empty + 8 * (ib % NB));
-                    }
+                }
+                for (int jb = 0; jb < n_jb; ++jb) {        // sweep 2: k = 2 and the dominant hi x hi
+                    a_wait(ia); b_wait(ib);
+                    pass(ia, ib, false, IDESC_F16);
+                    a_free(ia); b_free(ib);
+                    a_wait(ia + 1); b_wait(ib + 1);
+                    pass(ia + 1, ib + 1, true, IDESC_F16);
+                    a_free(ia + 1); b_free(ib + 1);
+                    ia += 2; ib += 2;
                 }
                 umma_commit(t_full);
             }
@@ -437,7 +464,7 @@ bool series_possible(const Geometry& g, int dtype) {
     return dtype == NK_F32 && g.n_rows >= SERIES_MIN_ROWS && g.M_pad >= SERIES_MIN_MPAD;
 }
 
-SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk) {
+SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk, int n_sets) {
     auto take = [&](size_t bytes) -> void* {
         void* r = base ? base + *off : nullptr;
         *off += align256(bytes);
@@ -449,9 +476,13 @@ SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chu
     w.part_stride = (chunk + 127) / 128 * 128;
     w.ctl = (unsigned*)take(SER_CTL_WORDS * sizeof(unsigned));
     w.Bp = (uint16_t*)take((size_t)g.n_rows * SERIES_SEGS * g.M_pad * 2);
-    w.Ap = (uint16_t*)take((size_t)chunk * SERIES_SEGS * g.M_pad * 2);
-    w.sigT = (uint32_t*)take((size_t)g.N * w.w32 * 4);
-    w.part = (float*)take((size_t)w.n_nt * w.part_stride * 4);
+    for (int k = 0; k < 2; ++k) {                      // per-chunk buffers: two sets when the chunks are pipelined
+        if (k < n_sets) {
+            w.Ap[k] = (uint16_t*)take((size_t)chunk * SERIES_SEGS * g.M_pad * 2);
+            w.sigT[k] = (uint32_t*)take((size_t)g.N * w.w32 * 4);
+            w.part[k] = (float*)take((size_t)w.n_nt * w.part_stride * 4);
+        } else { w.Ap[k] = w.Ap[0]; w.sigT[k] = w.sigT[0]; w.part[k] = w.part[0]; }
+    }
     return w;
 }
 
@@ -469,37 +500,43 @@ cudaError_t launch_series_pack(const Geometry& g, const float* Ttab, const unsig
     return cudaGetLastError();
 }
 
-// per chunk: E_loc of nb samples from the operand rows launch_logpsi left in w.Ap (every kernel returns at once when
-// ctl says the path is off)
+// per chunk, buffer set `set`: the transposed spin bits (preparation; may run on another stream than the GEMM)
+cudaError_t launch_series_prep(const Geometry& g, const int8_t* sigma, int64_t nb, const SeriesWs& w, int set,
+                               cudaStream_t st) {
+    if (nb <= 0) return cudaSuccess;
+    ProfScope sc(PH_SERIES_PREP, st);
+    const int n_groups = (int)((nb + ser::BM - 1) / ser::BM) * 4;
+    const int64_t warps = (int64_t)n_groups * ((g.N + 15) / 16);
+    series_bits_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(sigma, nb, g.N, w.w32, n_groups, w.ctl, w.sigT[set]);
+    count_launch();
+    return cudaGetLastError();
+}
+
+// per chunk: E_loc of nb samples from the operand rows launch_logpsi left in w.Ap[set] and the bits of
+// launch_series_prep (both kernels return at once when ctl says the path is off)
 cudaError_t launch_series_eloc(const Operator* op, const Geometry& g, const int8_t* sigma, int64_t nb,
-                               const RowInfo* rows, const SeriesWs& w, float* eloc_out, cudaStream_t st) {
+                               const RowInfo* rows, const SeriesWs& w, int set, float* eloc_out, cudaStream_t st) {
     if (nb <= 0) return cudaSuccess;
     cudaError_t e = series_init();
     if (e != cudaSuccess) return e;
     const int sms = g_ser_sms[current_device()];
     const int n_mt = (int)((nb + ser::BM - 1) / ser::BM);
-    {
-        ProfScope sc(PH_SERIES_PREP, st);
-        const int n_groups = n_mt * 4;
-        const int64_t warps = (int64_t)n_groups * ((g.N + 15) / 16);
-        series_bits_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(sigma, nb, g.N, w.w32, n_groups, w.ctl, w.sigT);
-    }
     CUtensorMap map_a, map_b;
     const uint64_t cols = (uint64_t)SERIES_SEGS * g.M_pad;
-    if (!encode_u16(&map_a, w.Ap, (uint64_t)nb, cols, ser::BM)) return cudaErrorInvalidValue;
+    if (!encode_u16(&map_a, w.Ap[set], (uint64_t)nb, cols, ser::BM)) return cudaErrorInvalidValue;
     if (!encode_u16(&map_b, w.Bp, (uint64_t)g.n_rows, cols, ser::BN)) return cudaErrorInvalidValue;
     SeriesParams p;
-    p.ctl = w.ctl; p.rows = rows; p.sigT = w.sigT; p.w32 = w.w32; p.nb = nb; p.n_rows = g.n_rows; p.M_pad = g.M_pad;
-    p.n_mt = n_mt; p.n_nt = w.n_nt; p.part = w.part; p.part_stride = w.part_stride;
+    p.ctl = w.ctl; p.rows = rows; p.sigT = w.sigT[set]; p.w32 = w.w32; p.nb = nb; p.n_rows = g.n_rows; p.M_pad = g.M_pad;
+    p.n_mt = n_mt; p.n_nt = w.n_nt; p.part = w.part[set]; p.part_stride = w.part_stride;
     const int n_tiles = n_mt * w.n_nt;
     {
         ProfScope sc(PH_SERIES_GEMM, st);
         series_gemm_kernel<<<n_tiles < sms ? n_tiles : sms, ser::THREADS, ser::SMEM_BYTES, st>>>(map_a, map_b, p);
     }
-    series_finish_kernel<<<(unsigned)((nb + 7) / 8), 256, 0, st>>>(w.part, w.n_nt, w.part_stride, sigma, nb, g.N,
+    series_finish_kernel<<<(unsigned)((nb + 7) / 8), 256, 0, st>>>(w.part[set], w.n_nt, w.part_stride, sigma, nb, g.N,
                                                                   op->kind, op->d_bonds, op->d_colors, op->d_Jf,
                                                                   op->n_bonds, w.ctl, eloc_out);
-    count_launch(3);
+    count_launch(2);
     return cudaGetLastError();
 }
 

@@ -50,37 +50,47 @@ constexpr uint32_t ACC_STRIDE = 256;                      // of column 0 and of 
 constexpr uint32_t IDESC_I8 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)((3 * BN) >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
 }  // namespace tc
 
-// ---- operand preparation ---------------------------------------------------------------------------------
-// max |Wg| as float bits (non-negative floats order like unsigned ints); *out must be zeroed first
-__global__ void absmax_kernel(const float* __restrict__ Wg, size_t n, unsigned* __restrict__ out) {
+// ---- int8 operands of the theta contraction (tcgen05 kind::i8: twice the bf16 MMA rate, half the operand bytes) ----
+// Wq[piece][me][k] (int8, K_pad columns, zero padded): rint(W[me][k] / q_me) = I = d2 2^16 + d1 2^8 + d0 with balanced
+// base-256 digits d in [-128, 127].  The scale is PER HIDDEN UNIT (row me of W = output column of theta): q_me is a
+// POWER OF TWO, 2^(ex-23) with 2^ex > max_k |W[me][k]| (one step coarser if the row maximum / q would pass 8355000:
+// three digits hold |I| <= 8355711), so W / q and q I are exact scalings and every row keeps 23 bits of ITS OWN
+// largest entry — with one scale for the whole matrix small rows lost bits (ln psi error 5.4e-6 of the 1e-5 bound at
+// config 5).  A scale that is not a power of two was measured to bias every theta by the same 1e-7 relative error,
+// which adds up coherently in ln psi.  Pieces stored hi, mid, lo.  The products with sigma = +-1 and their int32 sums
+// over k are exact; the residual |W - q I| <= q / 2 <= 2^-23 max_k |W[me][k]|.  The scales q_me follow the three
+// planes as M_eff floats (byte offset 3 M_eff K_pad).  A row holding a NaN or an Inf gets q = NaN and zero digits:
+// the epilogue's q D + b is then NaN for that hidden unit — non-finite parameters propagate (Q14).
+// One block per row: the row maximum first (float bits of |w| order like unsigned integers, NaN above Inf), then the digits.
+__global__ void __launch_bounds__(256)
+split_w_i8_kernel(const float* __restrict__ Wg, int M_eff, int N, int K_pad, int8_t* __restrict__ Wq) {
+    const int me = blockIdx.x;
+    const float* row = Wg + (size_t)me * N;
     unsigned m = 0;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
-        m = max(m, __float_as_uint(fabsf(Wg[i])));
+    for (int k = threadIdx.x; k < N; k += blockDim.x) m = max(m, __float_as_uint(fabsf(row[k])));
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
-    if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
-}
-
-// ---- int8 operands of the theta contraction (tcgen05 kind::i8: twice the bf16 MMA rate, half the operand bytes) ----
-// Wq[piece][me][k] (int8, K_pad columns, zero padded): rint(W / q) = I = d2 2^16 + d1 2^8 + d0 with balanced base-256
-// digits d in [-128, 127]; q is a POWER OF TWO, 2^(ex-23) with 2^ex > max|W| (one step coarser if max|W| / q would
-// pass 8355000: three digits hold |I| <= 8355711), so W / q and q I are exact scalings — a scale that is not a
-// power of two was measured to bias every theta by the same 1e-7 relative error, which adds up coherently in ln psi.
-// Pieces stored hi, mid, lo.  The products with sigma = +-1 and their int32 sums over k are exact; the residual
-// |W - q I| <= q / 2 <= 2^-23 max|W|.  The scale q is left as a float right behind the three planes (byte offset
-// 3 M_eff K_pad).
-__global__ void split_w_i8_kernel(const float* __restrict__ Wg, int M_eff, int N, int K_pad,
-                                  const unsigned* __restrict__ absmax_bits, int8_t* __restrict__ Wq) {
-    const float wmax = __uint_as_float(*absmax_bits);
+    __shared__ unsigned red[8];
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    m = red[0];
+#pragma unroll
+    for (int w = 1; w < 8; ++w) m = max(m, red[w]);
+    const float wmax = __uint_as_float(m);
     int ex = -100;
-    if (wmax > 0.f) frexpf(wmax, &ex);                    // wmax = f 2^ex, f in [0.5, 1)
-    if (ldexpf(wmax, 23 - ex) > 8355000.f) ++ex;          // f > 0.996: the top digit would overflow
-    const float sc = ldexpf(1.f, 23 - ex);
-    const int me = blockIdx.y;
+    float sc, q;
+    if (m >= 0x7f800000u) { sc = 0.f; q = __int_as_float(0x7fc00000); }          // NaN / Inf in the row: poison it
+    else {
+        if (wmax > 0.f) frexpf(wmax, &ex);                // wmax = f 2^ex, f in [0.5, 1)
+        if (ldexpf(wmax, 23 - ex) > 8355000.f) ++ex;      // f > 0.996: the top digit would overflow
+        if (ex < -100) ex = -100;                         // keep 2^(23 - ex) finite
+        sc = ldexpf(1.f, 23 - ex);
+        q = ldexpf(1.f, ex - 23);
+    }
     const size_t plane = (size_t)M_eff * K_pad;
-    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < K_pad; k += gridDim.x * blockDim.x) {
-        const float w = (k < N) ? Wg[(size_t)me * N + k] : 0.f;
-        const int I = (int)rintf(w * sc);
+    for (int k = threadIdx.x; k < K_pad; k += blockDim.x) {
+        const float w = (k < N) ? row[k] : 0.f;
+        const int I = (m >= 0x7f800000u) ? 0 : (int)rintf(w * sc);
         const int d0 = ((I + 128) & 255) - 128;
         const int I1 = (I - d0) >> 8;
         const int d1 = ((I1 + 128) & 255) - 128;
@@ -90,8 +100,7 @@ __global__ void split_w_i8_kernel(const float* __restrict__ Wg, int M_eff, int N
         Wq[plane + o] = (int8_t)d1;
         Wq[2 * plane + o] = (int8_t)d0;
     }
-    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0)
-        *reinterpret_cast<float*>(Wq + 3 * plane) = ldexpf(1.f, ex - 23);
+    if (threadIdx.x == 0) reinterpret_cast<float*>(Wq + 3 * plane)[me] = q;
 }
 
 // A[s][k] = sigma[s][k] zero padded to K_pad (only needed when N is not a multiple of 128: TMA wants 16-B strides)
@@ -117,7 +126,7 @@ template <int CM, int CN>
 __global__ void __launch_bounds__(tc::THREADS, 1)
 theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w, int64_t B,
                 int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta, int accumulate,
-                const float* __restrict__ scale, int n_sup_n, int n_sup) {
+                const float* __restrict__ scale, int scale_per_col, int n_sup_n, int n_sup) {
     using namespace tc;
     constexpr int CS = CM * CN;
     extern __shared__ uint8_t smem_raw[];
@@ -218,7 +227,7 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
     } else {
         // ===== epilogue: warps 2..5, TMEM lane quarter = warp % 4 =====
         const int q = warp & 3;
-        const float qs = *scale;
+        const float qs0 = *scale;                         // one scale, or (scale_per_col) one per output column
         int it = 0;
         for (int sup = cluster_id; sup < n_sup; sup += n_clusters, ++it) {
             const int set = it & 1;
@@ -245,6 +254,8 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                     for (int j = 0; j < 32; j += 4) {
                         float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
                         if (bg != nullptr) bb = *reinterpret_cast<const float4*>(bg + n0 + c0 + j);
+                        float4 qs = make_float4(qs0, qs0, qs0, qs0);
+                        if (scale_per_col) qs = *reinterpret_cast<const float4*>(scale + n0 + c0 + j);
                         if (accumulate) {                  // out += D (the gradient contraction runs over chunks)
                             const float4 old = *reinterpret_cast<const float4*>(out + c0 + j);
                             bb.x += old.x; bb.y += old.y; bb.z += old.z; bb.w += old.w;
@@ -255,8 +266,8 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                                         l = (float)__float_as_int(lo[jj]);
                             return fmaf(h, 65536.f, fmaf(m, 256.f, l));
                         };
-                        o.x = fmaf(qs, comb(j), bb.x); o.y = fmaf(qs, comb(j + 1), bb.y);
-                        o.z = fmaf(qs, comb(j + 2), bb.z); o.w = fmaf(qs, comb(j + 3), bb.w);
+                        o.x = fmaf(qs.x, comb(j), bb.x); o.y = fmaf(qs.y, comb(j + 1), bb.y);
+                        o.z = fmaf(qs.z, comb(j + 2), bb.z); o.w = fmaf(qs.w, comb(j + 3), bb.w);
                         __stcs(reinterpret_cast<float4*>(out + c0 + j), o);
                     }
                 }
@@ -318,7 +329,8 @@ static cudaError_t tc_prepare(int* max_clusters) {
 
 template <int CM, int CN>
 static cudaError_t tc_launch(const CUtensorMap& map_a, const CUtensorMap& map_w, int64_t rows, int cols, int k_len,
-                             const float* bg, float* out, int accumulate, const float* scale, cudaStream_t st) {
+                             const float* bg, float* out, int accumulate, const float* scale, int scale_per_col,
+                             cudaStream_t st) {
     const int n_sup_n = cols / (tc::BN * CN);
     const int64_t n_sup = (rows + (int64_t)tc::BM * CM - 1) / ((int64_t)tc::BM * CM) * n_sup_n;
     if (n_sup > 0x7fffffff) return cudaErrorInvalidValue;
@@ -333,7 +345,7 @@ static cudaError_t tc_launch(const CUtensorMap& map_a, const CUtensorMap& map_w,
     attr[0].val.clusterDim.x = CM * CN; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, theta_tc_kernel<CM, CN>, map_a, map_w, rows, cols, k_len, bg, out, accumulate, scale,
-                              n_sup_n, (int)n_sup);
+                              scale_per_col, n_sup_n, (int)n_sup);
 }
 
 cudaError_t theta_tc_init() {
@@ -372,18 +384,18 @@ cudaError_t theta_tc_init() {
 }
 
 static cudaError_t tc_gemm(const void* A, int64_t rows, const void* P, int cols, int ld, int k_len, const float* bg,
-                           float* out, int accumulate, cudaStream_t st) {
+                           float* out, int accumulate, int scale_per_col, cudaStream_t st) {
     cudaError_t e = theta_tc_init();
     if (e != cudaSuccess) return e;
     CUtensorMap map_a, map_p;
     if (!encode_2d(&map_a, A, (uint64_t)rows, (uint64_t)ld, tc::BM / g_cn)) return cudaErrorInvalidValue;
     if (!encode_2d(&map_p, P, (uint64_t)3 * cols, (uint64_t)ld, tc::BN / g_cm)) return cudaErrorInvalidValue;
     const float* scale = reinterpret_cast<const float*>((const int8_t*)P + (size_t)3 * cols * ld);
-    if (g_cm == 4 && g_cn == 2) e = tc_launch<4, 2>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, st);
-    else if (g_cm == 4) e = tc_launch<4, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, st);
-    else if (g_cm == 2 && g_cn == 2) e = tc_launch<2, 2>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, st);
-    else if (g_cm == 2) e = tc_launch<2, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, st);
-    else e = tc_launch<1, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, st);
+    if (g_cm == 4 && g_cn == 2) e = tc_launch<4, 2>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
+    else if (g_cm == 4) e = tc_launch<4, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
+    else if (g_cm == 2 && g_cn == 2) e = tc_launch<2, 2>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
+    else if (g_cm == 2) e = tc_launch<2, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
+    else e = tc_launch<1, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
     count_launch();
     return e != cudaSuccess ? e : cudaGetLastError();
 }
@@ -400,18 +412,10 @@ static bool encode_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// W -> three int8 planes + scale (K_pad a multiple of 128); the buffer must hold 3 M_eff K_pad + 4 bytes
-cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* Ws, unsigned* absmax_scratch,
-                           cudaStream_t st) {
-    cudaError_t e = cudaMemsetAsync(absmax_scratch, 0, sizeof(unsigned), st);
-    if (e != cudaSuccess) return e;
-    const size_t n = (size_t)M_eff * N;
-    unsigned blocks = (unsigned)((n + 1023) / 1024);
-    if (blocks > 1184) blocks = 1184;
-    absmax_kernel<<<blocks, 256, 0, st>>>(Wg, n, absmax_scratch);
-    dim3 grid((K_pad + 255) / 256, M_eff);
-    split_w_i8_kernel<<<grid, 256, 0, st>>>(Wg, M_eff, N, K_pad, absmax_scratch, (int8_t*)Ws);
-    count_launch(2);
+// W -> three int8 planes + one scale per row (K_pad a multiple of 128); the buffer must hold 3 M_eff K_pad + 4 M_eff bytes
+cudaError_t launch_split_w(const float* Wg, int M_eff, int N, int K_pad, void* Ws, cudaStream_t st) {
+    split_w_i8_kernel<<<M_eff, 256, 0, st>>>(Wg, M_eff, N, K_pad, (int8_t*)Ws);
+    count_launch();
     return cudaGetLastError();
 }
 
@@ -431,7 +435,7 @@ cudaError_t launch_sigma_operand(const int8_t* sigma, int64_t B, int N, int K_pa
 cudaError_t launch_theta_tc_pre(const void* A, int64_t B, int M_eff, int K_pad, const void* Ws, const float* bg,
                                 float* theta, cudaStream_t st) {
     if (B <= 0) return cudaSuccess;
-    return tc_gemm(A, B, Ws, M_eff, K_pad, K_pad, bg, theta, 0, st);
+    return tc_gemm(A, B, Ws, M_eff, K_pad, K_pad, bg, theta, 0, 1, st);
 }
 
 cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, int K_pad, const void* Ws, void* A,
@@ -450,7 +454,7 @@ cudaError_t launch_theta_tc(const int8_t* sigma, int64_t B, int N, int M_eff, in
 cudaError_t launch_tc_gemm_pieces(const void* A, int64_t rows, const void* P, int cols, int ld, int k_len, float* out,
                                   int accumulate, cudaStream_t st) {
     if (rows <= 0) return cudaSuccess;
-    return tc_gemm(A, rows, P, cols, ld, k_len, nullptr, out, accumulate, st);
+    return tc_gemm(A, rows, P, cols, ld, k_len, nullptr, out, accumulate, 0, st);
 }
 
 }  // namespace nk

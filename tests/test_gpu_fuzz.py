@@ -43,8 +43,9 @@ def test_random_shapes(nk, seed):
         e, lp, st = nk.local_energy(op, *args, chunk_size=chunk, flags=flags)
         torch.cuda.synchronize()
         assert_eloc(e.cpu().numpy(), e_ref)
-        # sigma_param up to 0.2 puts |theta| ~ 1 at these sizes: outside the regime of the 1e-5 bound (Q13)
-        assert_logpsi(lp.cpu().numpy(), lp_ref, atol=3e-5)
+        # real parameters: the bound as it stands; complex ones keep the DESIGN.md Q18 carve-out (theta next to the
+        # zeros of cosh at sigma_param up to 0.2)
+        assert_logpsi(lp.cpu().numpy(), lp_ref, atol=3e-5 if p.complex_params else 1e-5)
         assert st[3].item() == B
     op.close()
 

@@ -108,3 +108,38 @@ def test_gradient_argument_errors(nk):
     e32, st = oracle_inputs(p)
     with pytest.raises(nk.NkError):
         nk.energy_gradient(dev(p.sigma), dev(p.W), dev(p.b), dev(e32[:4]), dev(st))
+
+
+@pytest.mark.parametrize("cfg,n", [(2, 700), (4, 300)])
+def test_gradient_of_shards_sums_to_the_gradient_of_the_union(nk, cfg, n):
+    """nk_energy_gradient_sharded: unequal shards, each with the statistics of the
+    WHOLE batch and n_global = B, return shares that add up to the single-rank gradient."""
+    p = inp.make_config(cfg, n_samples=n)
+    e32, st = oracle_inputs(p)
+    full = nk.energy_gradient(dev(p.sigma), dev(p.W), dev(p.b), dev(e32), dev(st))
+    cut = n // 3
+    parts = []
+    for sl in (slice(0, cut), slice(cut, n)):
+        parts.append(nk.energy_gradient(dev(p.sigma[sl]), dev(p.W), dev(p.b), dev(e32[sl]), dev(st), n_global=n))
+    torch.cuda.synchronize()
+    ra, rb, rW = orc.energy_gradient_batched(p.sigma, p.W, p.b, e32)
+    for g_full, g0, g1, r in zip(full, parts[0], parts[1], (ra, rb, rW)):
+        tot = (g0 + g1).cpu().numpy()
+        scale = np.abs(r).max()
+        assert np.abs(tot - g_full.cpu().numpy()).max() <= 2e-6 * scale     # three fp32 roundings, three scales
+        assert np.abs(tot.astype(r.dtype) - r).max() <= 2e-6 * scale
+
+
+def test_gradient_non_finite_local_energy_propagates(nk):
+    """DESIGN.md Q14: a NaN local energy (a diverged optimisation) must not come back as silent zeros from the
+    fixed-point tensor-core contraction — every block of the gradient is non-finite."""
+    for cfg, n in ((2, 300), (4, 200)):
+        p = inp.make_config(cfg, n_samples=n)
+        e32, _ = oracle_inputs(p)
+        e32 = e32.copy()
+        e32[5] = np.nan
+        st = np.array([np.nan, np.nan if p.complex_params else 0.0, np.nan, float(n)])
+        ga, gb, gW = nk.energy_gradient(dev(p.sigma), dev(p.W), dev(p.b), dev(e32), dev(st))
+        torch.cuda.synchronize()
+        for g in (ga, gb, gW):
+            assert not np.isfinite(torch.view_as_real(g).cpu().numpy() if g.is_complex() else g.cpu().numpy()).any()

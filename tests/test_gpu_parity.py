@@ -216,9 +216,10 @@ def test_edge_cases(nk, case):
     e, lp, _ = run_gpu(nk, p)
     e_ref, lp_ref = run_oracle(p)
     assert_eloc(e, e_ref)
-    # sigma_param = 0.2 gives |theta| ~ 1 and |ln psi| ~ 100 at tiny N: outside the regime of the 1e-5 bound
-    # (Q13/Q18); these cases exercise code paths, so the ln psi check is loosened to 3e-5
-    assert_logpsi(lp, lp_ref, atol=3e-5)
+    # real parameters: the north_star bound as it stands (the per-hidden-unit scales of the W split gave the margin
+    # back).  Complex parameters keep the DESIGN.md Q18 carve-out: sigma_param = 0.2 puts theta next to the zeros of
+    # cosh, where d ln cosh / d theta = tanh theta is unbounded and an fp32 theta error is amplified without limit
+    assert_logpsi(lp, lp_ref, atol=3e-5 if p.complex_params else LOGPSI_ATOL)
 
 
 def test_null_biases_marshall_flag_and_empty_batch(nk):
@@ -242,7 +243,10 @@ def test_larger_parameters_stress(nk):
     e, lp, _ = run_gpu(nk, p)
     e_ref, lp_ref = run_oracle(p)
     assert_eloc(e, e_ref)
-    assert_logpsi(lp, lp_ref, atol=2e-5)     # |ln psi| ~ 300, |theta| ~ 5 here: the fp32 theta error is 10x larger
+    # |theta| ~ 5 .. 8 here: theta is handed to the ln cosh pass as fp32, whose spacing there is 4.8e-7 (1e-7 at the five
+    # configs), so the sum over hidden units carries ~1e-5 by itself — a limit of the fp32 theta buffer, not of the W
+    # split; |ln psi| ~ 300 adds half an fp32 ulp of the output (assert_logpsi).  Measured 1.1e-5 + 1.5e-5.
+    assert_logpsi(lp, lp_ref, atol=2e-5)
 
 
 def test_host_entry_point_matches_device_entry_point(nk):
@@ -330,3 +334,23 @@ def test_cuda_graph_replay_matches_the_eager_call(nk):
     torch.cuda.synchronize()
     assert all(torch.equal(x, y) for x, y in zip(g, r)) and not torch.equal(g[0], e0[0])
     op.close()
+
+
+def test_non_finite_parameters_propagate(nk):
+    """DESIGN.md Q14: no clamping — a NaN or Inf in W reaches theta, ln psi and E_loc on the tensor-core path (the
+    fixed-point split poisons the row's scale instead of saturating its digits)."""
+    p = inp.make_config(2, n_samples=64)
+    for bad in (np.nan, np.inf):
+        W = p.W.copy()
+        W[3, 7] = bad
+        lp, theta = nk.rbm_logpsi(dev(p.sigma), dev(W), dev(p.a), dev(p.b), return_theta=True)
+        torch.cuda.synchronize()
+        th = theta.cpu().numpy()
+        assert not np.isfinite(th[:, 3]).any() and np.isfinite(np.delete(th, 3, axis=1)).all()
+        assert not np.isfinite(lp.cpu().numpy()).any()
+        op = nk.Operator.from_problem(p)
+        e, lp2, st = nk.local_energy(op, dev(p.sigma), dev(W), dev(p.a), dev(p.b))
+        torch.cuda.synchronize()
+        assert not np.isfinite(e.cpu().numpy()).any() and not np.isfinite(lp2.cpu().numpy()).any()
+        assert not np.isfinite(st.cpu().numpy()[0])
+        op.close()
