@@ -179,7 +179,7 @@ static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk, int dtype, 
         w.theta[1] = c.take<float>((size_t)chunk * g.M_eff);
         w.A[1] = c.take<uint16_t>((size_t)chunk * g.K_pad);
     }
-    if (w.has_series) w.ser = carve_series(c.base, &c.off, g, chunk, w.n_sets);
+    if (w.has_series) w.ser = carve_series(c.base, &c.off, g, chunk, w.n_sets, B);
     w.bytes = c.off;
     return w;
 }
@@ -815,24 +815,36 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
                                   false, nullptr, ps, series ? w.ser.ctl : nullptr, series ? w.ser.Ap[set] : nullptr));
         }
         if (series) NK_CUDA(launch_series_prep(g, sg, nb, w.ser, set, ps));
+        {
+            // the SIMT forms (the only ones when the series form is impossible; gated stand-ins when it may run: every
+            // launch is made, those on the wrong side of the gates return at once) stay on the preparation stream, off
+            // the critical path of the tensor-core kernels
+            Scope sc(PH_FUSED, ps);
+            void* out = (uint8_t*)eloc_out + s0 * esz;
+            if (automatic) {
+                const unsigned* sctl = series ? w.ser.ctl : nullptr;
+                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], w.Ttab, w.rows, out, true, ps, w.taumax, 1, sctl));
+                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], w.Dtab, w.rows, out, false, ps, w.taumax, 2, sctl));
+            } else if (!force_series) {
+                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], force_product ? w.Ttab : w.Dtab, w.rows, out,
+                                          force_product, ps));
+            }
+        }
         if (pipelined) {
             NK_CUDA(cudaEventRecord(ev_prep, ps));
             NK_CUDA(cudaStreamWaitEvent(st, ev_prep, 0));
         }
-        {
+        if (series) {
             Scope sc(PH_FUSED, st);
-            void* out = (uint8_t*)eloc_out + s0 * esz;
-            if (series) NK_CUDA(launch_series_eloc(op, g, sg, nb, w.rows, w.ser, set, (float*)out, st));
-            if (automatic) {           // every launch; those on the wrong side of the gates return at once
-                const unsigned* sctl = series ? w.ser.ctl : nullptr;
-                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], w.Ttab, w.rows, out, true, st, w.taumax, 1, sctl));
-                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], w.Dtab, w.rows, out, false, st, w.taumax, 2, sctl));
-            } else if (!force_series) {
-                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], force_product ? w.Ttab : w.Dtab, w.rows, out,
-                                          force_product, st));
-            }
+            NK_CUDA(launch_series_gemm(g, s0, nb, w.rows, w.ser, set, st));
         }
         if (pipelined) NK_CUDA(cudaEventRecord(ev_done, st));
+    }
+    // the series form's partial sums per column tile -> E_loc, one pass over the whole batch (gated like the rest; it
+    // runs after the SIMT stand-ins, which wrote nothing if the series form ran, and writes nothing if it did not)
+    if (series) {
+        Scope sc(PH_FUSED, st);
+        NK_CUDA(launch_series_finish(op, g, sigma, B, w.ser, (float*)eloc_out, st));
     }
     if (stats_out) {
         Scope sc(PH_STATS, st);

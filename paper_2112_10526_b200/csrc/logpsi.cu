@@ -53,7 +53,11 @@ __device__ __forceinline__ float ln_cosh_small_f(float t) {
     return p * u;
 }
 
-constexpr int LOGPSI_WARPS_REAL = 4;      // warps per block of the real kernel: 4 x 8 KB of compaction lists
+constexpr int LOGPSI_WARPS_REAL = 4;      // warps per block of the real kernel
+// entries of a warp's compaction list (2 KB; the list is evaluated and emptied whenever the next 128 elements might not
+// fit).  8 KB per block: small enough to run beside a CTA of the series form's tensor-core kernel (205 KB), which is
+// what lets this pass over chunk c + 1 hide under the GEMM of chunk c (api.cu, the pipelined chunk loop)
+constexpr int LOGPSI_LIST = 512;
 
 __device__ __forceinline__ uint32_t pack_h2(float x, float y) {
     const __half2 h = __floats2half2_rn(x, y);
@@ -90,7 +94,7 @@ logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_p
         // compacted into a per-warp list in shared memory (ballot + popc) and evaluated densely afterwards: ~8 slow
         // evaluations per lane and sample instead of 64, same fp64 formula.  (An fp32 expf / log1pf slow path was also
         // measured, 0.94 -> 0.53 ms per step, and rejected: ln psi error 2.9e-6 -> 3.6e-6.)
-        __shared__ float big_list[LOGPSI_WARPS_REAL][MAX_V_REAL * MPAD_ALIGN];
+        __shared__ float big_list[LOGPSI_WARPS_REAL][LOGPSI_LIST];
         float* big = big_list[threadIdx.x >> 5];
         int n_big = 0;
         const unsigned lt = (1u << lane) - 1u;
@@ -103,8 +107,18 @@ logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_p
             }
             return is_big ? 0.0 : (double)ln_cosh_small_f(x);
         };
-#pragma unroll 4
+        auto drain = [&]() {                                // the stable form, fp64, for the compacted large arguments
+            __syncwarp();
+            for (int k = lane; k < n_big; k += 32) {
+                const double t = fabs((double)big[k]);
+                r0 += t + log1p(exp(-2.0 * t)) - 0.69314718055994530942;
+            }
+            __syncwarp();
+            n_big = 0;
+        };
+#pragma unroll 2
         for (int j = lane * 4; j < M_pad; j += 128) {
+            if (n_big + 128 > LOGPSI_LIST) drain();         // warp-uniform
             const float4 x = *reinterpret_cast<const float4*>(th + j);
             if (theta_out) {
                 if (j < M) theta_out[s * M + j] = x.x;
@@ -131,11 +145,7 @@ logpsi_kernel(const int8_t* __restrict__ sigma, int64_t B, int N, int M, int M_p
             }
         }
         if (logpsi_out == nullptr) return;
-        __syncwarp();
-        for (int k = lane; k < n_big; k += 32) {
-            const double t = fabs((double)big[k]);
-            r0 += t + log1p(exp(-2.0 * t)) - 0.69314718055994530942;
-        }
+        drain();
         re = (r0 + r1) + (r2 + r3);
     }
     for (int j = lane; CPLX && j < M; j += 32) {

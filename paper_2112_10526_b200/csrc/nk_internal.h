@@ -159,18 +159,20 @@ struct SeriesWs {
     // per-chunk buffers, two sets when the chunk loop is pipelined over two streams (api.cu):
     uint16_t* Ap[2];            // [chunk][SERIES_SEGS][M_pad] 16-bit operand rows of the samples
     uint32_t* sigT[2];          // [N][w32] transposed bit-packed spins of the chunk
-    float* part[2];             // [n_nt][part_stride] partial local energies per column tile
+    float* part;                // [n_nt][part_stride] partial local energies per column tile, whole batch
     int w32, n_nt;
     int64_t part_stride;
 };
 bool series_possible(const Geometry& g, int dtype);
-SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk, int n_sets);
+SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk, int n_sets, int64_t B);
 cudaError_t launch_series_prep(const Geometry& g, const int8_t* sigma, int64_t nb, const SeriesWs& w, int set,
                                cudaStream_t st);
 cudaError_t launch_series_pack(const Geometry& g, const float* Ttab, const unsigned* taumax_bits, const SeriesWs& w,
                                bool force, cudaStream_t st);
-cudaError_t launch_series_eloc(const Operator* op, const Geometry& g, const int8_t* sigma, int64_t nb,
-                               const RowInfo* rows, const SeriesWs& w, int set, float* eloc_out, cudaStream_t st);
+cudaError_t launch_series_gemm(const Geometry& g, int64_t s0, int64_t nb, const RowInfo* rows, const SeriesWs& w, int set,
+                               cudaStream_t st);
+cudaError_t launch_series_finish(const Operator* op, const Geometry& g, const int8_t* sigma, int64_t B, const SeriesWs& w,
+                                 float* eloc_out, cudaStream_t st);
 // fused_eloc.cu
 cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
                               const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,

@@ -45,10 +45,11 @@ namespace nk {
 namespace ser {
 constexpr int BM = 128, BN = 256, BK = 64;                // BK 16-bit elements = one 128-B swizzle row
 constexpr int A_TILE = BM * BK * 2, B_TILE = BN * BK * 2; // 16 KB, 32 KB
-constexpr int NA = 4, NB = 4;                             // ring depths
+constexpr int NA = 4, NB = 4;                             // ring depths (3 + 3 measured: GEMM 181 -> 207 us per chunk)
 constexpr int THREADS = 224;                              // warps: A producer, MMA, B producer, 4 x epilogue
-constexpr int TAB_BYTES = BN * 16, MSK_BYTES = BN * 8;    // per epilogue warp: (coef, jdiag, a2, c2) and (act, neg) per column
-constexpr int SMEM_BYTES = NA * A_TILE + NB * B_TILE + 4 * (TAB_BYTES + MSK_BYTES) + 256 /*barriers*/ + 1024 /*alignment*/;
+constexpr int TAB_BYTES = BN * 16, MSK_BYTES = BN * 8;    // (coef, jdiag, a2, c2) per column, shared by the epilogue warps;
+                                                          // (act, neg) spin masks per column and epilogue warp
+constexpr int SMEM_BYTES = NA * A_TILE + NB * B_TILE + TAB_BYTES + 4 * MSK_BYTES + 256 /*barriers*/ + 1024 /*alignment*/;
 constexpr uint32_t TMEM_COLS = 512;                       // odd at column 0, even at column 256
 // instruction descriptors of kind::f16 (the cute::UMMA::InstrDescriptor bit layout): D = F32 (c_format 1 at bit 4),
 // A / B format at bits 7 / 10 (0 = F16, 1 = BF16), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
@@ -206,7 +207,7 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
     uint8_t* smem_al = smem_raw + (smem_base - smem_u32(smem_raw));
     const uint32_t a_ring = smem_base, b_ring = smem_base + NA * A_TILE;
     const uint32_t epi_off = NA * A_TILE + NB * B_TILE;
-    const uint32_t bars = smem_base + epi_off + 4 * (TAB_BYTES + MSK_BYTES);
+    const uint32_t bars = smem_base + epi_off + TAB_BYTES + 4 * MSK_BYTES;
     const uint32_t a_full = bars, a_empty = bars + 8 * NA, b_full = bars + 16 * NA, b_empty = b_full + 8 * NB;
     const uint32_t t_full = b_empty + 8 * NB, t_empty = t_full + 8, tmem_slot = t_empty + 8;
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_al + (tmem_slot - smem_base));
@@ -335,18 +336,20 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
     } else {
         // ===== epilogue: warps 3..6, TMEM lane quarter q = warp % 4 =====
         const int q = warp & 3;
-        float4* tab = reinterpret_cast<float4*>(smem_al + epi_off + q * (TAB_BYTES + MSK_BYTES));
-        uint2* msk = reinterpret_cast<uint2*>(smem_al + epi_off + q * (TAB_BYTES + MSK_BYTES) + TAB_BYTES);
+        float4* tab = reinterpret_cast<float4*>(smem_al + epi_off);
+        uint2* msk = reinterpret_cast<uint2*>(smem_al + epi_off + TAB_BYTES + q * MSK_BYTES);
+        const int wq = warp - 3;                           // 0..3: which quarter of the row records this warp stages
         const float inv = __uint_as_float(p.ctl[1]);
         uint32_t n_done = 0;
         for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++n_done) {
             const int mt = tile / p.n_nt, nt = tile - mt * p.n_nt;
             const int n0 = nt * BN;
-            // this warp's 32 samples: matrix element, diagonal coupling, exponents and the two spin masks per column
-            __syncwarp();
+            // per column: matrix element, diagonal coupling and exponents (staged once for the four warps) and this warp's
+            // 32 samples' two spin masks
+            asm volatile("bar.sync 1, 128;" ::: "memory");  // every epilogue warp is done with the previous tile's records
             for (int c = lane; c < BN; c += 32) {
-                float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
                 uint2 m = make_uint2(0u, 0u);
+                float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (n0 + c < p.n_rows) {
                     const RowInfo ri = p.rows[n0 + c];
                     if (ri.i >= 0) {
@@ -356,10 +359,10 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
                         t = make_float4(ri.coef, ri.jdiag, ri.a2_re, ri.c2_re);
                     }
                 }
-                tab[c] = t;
+                if ((c >> 6) == wq) tab[c] = t;
                 msk[c] = m;
             }
-            __syncwarp();
+            asm volatile("bar.sync 1, 128;" ::: "memory");
             const int64_t row = (int64_t)mt * BM + q * 32 + lane;
             float E = 0.f;
             mbar_wait(t_full, n_done & 1u);
@@ -464,7 +467,7 @@ bool series_possible(const Geometry& g, int dtype) {
     return dtype == NK_F32 && g.n_rows >= SERIES_MIN_ROWS && g.M_pad >= SERIES_MIN_MPAD;
 }
 
-SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk, int n_sets) {
+SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk, int n_sets, int64_t B) {
     auto take = [&](size_t bytes) -> void* {
         void* r = base ? base + *off : nullptr;
         *off += align256(bytes);
@@ -473,16 +476,16 @@ SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chu
     SeriesWs w;
     w.w32 = (int)((chunk + 127) / 128 * 4);
     w.n_nt = (g.n_rows + ser::BN - 1) / ser::BN;
-    w.part_stride = (chunk + 127) / 128 * 128;
+    w.part_stride = (B + 127) / 128 * 128 + 128;       // whole batch (32 B per sample at config 5): one finishing pass
     w.ctl = (unsigned*)take(SER_CTL_WORDS * sizeof(unsigned));
     w.Bp = (uint16_t*)take((size_t)g.n_rows * SERIES_SEGS * g.M_pad * 2);
     for (int k = 0; k < 2; ++k) {                      // per-chunk buffers: two sets when the chunks are pipelined
         if (k < n_sets) {
             w.Ap[k] = (uint16_t*)take((size_t)chunk * SERIES_SEGS * g.M_pad * 2);
             w.sigT[k] = (uint32_t*)take((size_t)g.N * w.w32 * 4);
-            w.part[k] = (float*)take((size_t)w.n_nt * w.part_stride * 4);
-        } else { w.Ap[k] = w.Ap[0]; w.sigT[k] = w.sigT[0]; w.part[k] = w.part[0]; }
+        } else { w.Ap[k] = w.Ap[0]; w.sigT[k] = w.sigT[0]; }
     }
+    w.part = (float*)take((size_t)w.n_nt * w.part_stride * 4);
     return w;
 }
 
@@ -512,10 +515,10 @@ cudaError_t launch_series_prep(const Geometry& g, const int8_t* sigma, int64_t n
     return cudaGetLastError();
 }
 
-// per chunk: E_loc of nb samples from the operand rows launch_logpsi left in w.Ap[set] and the bits of
-// launch_series_prep (both kernels return at once when ctl says the path is off)
-cudaError_t launch_series_eloc(const Operator* op, const Geometry& g, const int8_t* sigma, int64_t nb,
-                               const RowInfo* rows, const SeriesWs& w, int set, float* eloc_out, cudaStream_t st) {
+// per chunk (samples s0 .. s0 + nb of the batch): partial local energies per column tile into w.part, from the operand
+// rows launch_logpsi left in w.Ap[set] and the bits of launch_series_prep (returns at once when ctl says the path is off)
+cudaError_t launch_series_gemm(const Geometry& g, int64_t s0, int64_t nb, const RowInfo* rows, const SeriesWs& w, int set,
+                               cudaStream_t st) {
     if (nb <= 0) return cudaSuccess;
     cudaError_t e = series_init();
     if (e != cudaSuccess) return e;
@@ -527,16 +530,22 @@ cudaError_t launch_series_eloc(const Operator* op, const Geometry& g, const int8
     if (!encode_u16(&map_b, w.Bp, (uint64_t)g.n_rows, cols, ser::BN)) return cudaErrorInvalidValue;
     SeriesParams p;
     p.ctl = w.ctl; p.rows = rows; p.sigT = w.sigT[set]; p.w32 = w.w32; p.nb = nb; p.n_rows = g.n_rows; p.M_pad = g.M_pad;
-    p.n_mt = n_mt; p.n_nt = w.n_nt; p.part = w.part[set]; p.part_stride = w.part_stride;
+    p.n_mt = n_mt; p.n_nt = w.n_nt; p.part = w.part + s0; p.part_stride = w.part_stride;
     const int n_tiles = n_mt * w.n_nt;
-    {
-        ProfScope sc(PH_SERIES_GEMM, st);
-        series_gemm_kernel<<<n_tiles < sms ? n_tiles : sms, ser::THREADS, ser::SMEM_BYTES, st>>>(map_a, map_b, p);
-    }
-    series_finish_kernel<<<(unsigned)((nb + 7) / 8), 256, 0, st>>>(w.part[set], w.n_nt, w.part_stride, sigma, nb, g.N,
-                                                                  op->kind, op->d_bonds, op->d_colors, op->d_Jf,
-                                                                  op->n_bonds, w.ctl, eloc_out);
-    count_launch(2);
+    ProfScope sc(PH_SERIES_GEMM, st);
+    series_gemm_kernel<<<n_tiles < sms ? n_tiles : sms, ser::THREADS, ser::SMEM_BYTES, st>>>(map_a, map_b, p);
+    count_launch();
+    return cudaGetLastError();
+}
+
+// once per call, after the last chunk: E_loc of the whole batch from the partial sums
+cudaError_t launch_series_finish(const Operator* op, const Geometry& g, const int8_t* sigma, int64_t B, const SeriesWs& w,
+                                 float* eloc_out, cudaStream_t st) {
+    if (B <= 0) return cudaSuccess;
+    series_finish_kernel<<<(unsigned)((B + 7) / 8), 256, 0, st>>>(w.part, w.n_nt, w.part_stride, sigma, B, g.N, op->kind,
+                                                                 op->d_bonds, op->d_colors, op->d_Jf, op->n_bonds,
+                                                                 w.ctl, eloc_out);
+    count_launch();
     return cudaGetLastError();
 }
 

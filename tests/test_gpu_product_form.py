@@ -102,7 +102,7 @@ def test_product_form_chunking_and_bad_flags(nk):
         e, _, st = run_prod(nk, p, chunk=chunk)
         assert np.array_equal(e, ref) and np.array_equal(st, st0)
     with pytest.raises(nk.NkError):
-        run_prod(nk, p, form=64)
+        run_prod(nk, p, form=1024)                         # an undefined flag bit
 
 
 def _plan_run(nk, p, flags, scale=1.0):
