@@ -146,10 +146,8 @@ static LogpsiWs carve_logpsi(void* ws, const Geometry& g, int64_t rows) {
 }
 struct ElocWs {
     float *Wg, *bg, *Wt, *Dtab, *Ttab;                // Dtab: log-cosh form, Ttab: product form (both when automatic)
-    float* theta[2];                                  // per-chunk buffers: two sets when the chunk loop is pipelined
-    uint16_t* A[2];
-    int n_sets;
-    uint16_t* Ws;
+    float* theta;                                     // per-chunk buffers
+    uint16_t *A, *Ws;
     unsigned *absmax, *taumax;                        // taumax: max |tanh delta| of Ttab as float bits (the form gate)
     RowInfo* rows;
     bool has_series;                                  // the tensor-core series form is possible for these sizes
@@ -165,21 +163,13 @@ static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk, int dtype, 
     w.Dtab = c.take<float>((size_t)g.n_rows_pad * g.M_eff);
     w.rows = c.take<RowInfo>(g.n_rows_pad);
     w.has_series = series_possible(g, dtype);
-    // the series form pipelines consecutive chunks over two streams (preparation of chunk c + 1 beside the tensor-core
-    // kernel of chunk c): theta, the padded spins and the series operands exist twice when there is more than one chunk
-    w.n_sets = (w.has_series && chunk < B) ? 2 : 1;
-    w.theta[0] = c.take<float>((size_t)chunk * g.M_eff);
+    w.theta = c.take<float>((size_t)chunk * g.M_eff);
     w.Ws = c.take<uint16_t>((size_t)3 * g.M_eff * g.K_pad);
-    w.A[0] = c.take<uint16_t>((size_t)chunk * g.K_pad);
+    w.A = c.take<uint16_t>((size_t)chunk * g.K_pad);
     w.absmax = c.take<unsigned>(1);
     w.taumax = c.take<unsigned>(1);
     w.Ttab = c.take<float>((size_t)g.n_rows_pad * g.M_eff);
-    w.theta[1] = w.theta[0]; w.A[1] = w.A[0];
-    if (w.n_sets == 2) {
-        w.theta[1] = c.take<float>((size_t)chunk * g.M_eff);
-        w.A[1] = c.take<uint16_t>((size_t)chunk * g.K_pad);
-    }
-    if (w.has_series) w.ser = carve_series(c.base, &c.off, g, chunk, w.n_sets, B);
+    if (w.has_series) w.ser = carve_series(c.base, &c.off, g, chunk, B);
     w.bytes = c.off;
     return w;
 }
@@ -784,12 +774,14 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
         NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, st));
     }
     const size_t esz = dtype == NK_C64 ? 8 : 4;
-    // Two streams when the series form may run over several chunks: the preparation of a chunk (theta contraction, the
-    // ln psi / operand pass, spin bits) goes to an internal high-priority stream `ps`, the tensor-core kernel and what
-    // follows it stay on the caller's stream, each buffer set is handed over by an event — the preparation of chunk
-    // c + 1 fills the tail (and the idle ALUs) of the GEMM of chunk c.  Everything the caller observes is ordered on
-    // `stream`; the construction is capturable in a CUDA graph (the internal stream forks from and joins `stream`).
-    const bool pipelined = series && w.n_sets == 2 && !(flags & NK_SERIAL_CHUNKS);
+    // The series form contracts GROUPS of chunks (series_tc.cu: as many as make the tensor-core launch a whole number
+    // of waves).  With more than one group the work is split over two streams: the preparation of a group's chunks
+    // (theta contraction, the ln psi / operand pass, the gated SIMT stand-ins, spin bits) goes to an internal
+    // high-priority stream `ps`, the tensor-core launches stay on the caller's stream, and each of the two operand
+    // buffers is handed over by a pair of events — the preparation of group G + 1 runs beside the launch of group G.
+    // Everything the caller observes is ordered on `stream`; the construction is capturable in a CUDA graph (the
+    // internal stream forks from and joins `stream`).
+    const bool pipelined = series && w.ser.n_sets == 2 && !(flags & NK_SERIAL_CHUNKS);
     cudaStream_t ps = st;
     if (pipelined) {
         NK_CUDA(pipeline_objects());
@@ -797,46 +789,52 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
         NK_CUDA(cudaEventRecord(tl_pipe_events[0], st));              // parameters packed; earlier work on `stream` done
         NK_CUDA(cudaStreamWaitEvent(ps, tl_pipe_events[0], 0));
     }
-    int64_t ci = 0;
-    for (int64_t s0 = 0; s0 < B; s0 += chunk, ++ci) {
-        const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
-        const int8_t* sg = sigma + s0 * N;
-        const int set = pipelined ? (int)(ci & 1) : 0;
+    const int64_t group_rows = series ? w.ser.group_rows : chunk;
+    int64_t gi = 0;
+    for (int64_t g0 = 0; g0 < B; g0 += group_rows, ++gi) {
+        const int64_t gn = (B - g0 < group_rows) ? (B - g0) : group_rows;
+        const int set = (series && w.ser.n_sets == 2) ? (int)(gi & 1) : 0;
         cudaEvent_t ev_prep = tl_pipe_events[1 + set], ev_done = tl_pipe_events[3 + set];
-        if (pipelined && ci >= 2) NK_CUDA(cudaStreamWaitEvent(ps, ev_done, 0));    // chunk c - 2 no longer reads this set
-        if (tl_chunk_ready != nullptr) NK_CUDA(cudaStreamWaitEvent(ps, (*tl_chunk_ready)[(size_t)(s0 / chunk)], 0));
-        {
-            Scope sc(PH_GEMM, ps);
-            NK_CUDA(run_theta(g, sg, nb, w.Wg, w.bg, w.Ws, w.A[set], w.theta[set], ps));
-        }
-        if (logpsi_out || series) {            // ln psi and, in the same pass over theta, the series form's operand rows
-            Scope sc(PH_LOGPSI, ps);
-            NK_CUDA(launch_logpsi(sg, nb, g, dtype, w.theta[set], a, logpsi_out ? (uint8_t*)logpsi_out + s0 * esz : nullptr,
-                                  false, nullptr, ps, series ? w.ser.ctl : nullptr, series ? w.ser.Ap[set] : nullptr));
-        }
-        if (series) NK_CUDA(launch_series_prep(g, sg, nb, w.ser, set, ps));
-        {
-            // the SIMT forms (the only ones when the series form is impossible; gated stand-ins when it may run: every
-            // launch is made, those on the wrong side of the gates return at once) stay on the preparation stream, off
-            // the critical path of the tensor-core kernels
-            Scope sc(PH_FUSED, ps);
-            void* out = (uint8_t*)eloc_out + s0 * esz;
-            if (automatic) {
-                const unsigned* sctl = series ? w.ser.ctl : nullptr;
-                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], w.Ttab, w.rows, out, true, ps, w.taumax, 1, sctl));
-                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], w.Dtab, w.rows, out, false, ps, w.taumax, 2, sctl));
-            } else if (!force_series) {
-                NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta[set], force_product ? w.Ttab : w.Dtab, w.rows, out,
-                                          force_product, ps));
+        if (pipelined && gi >= 2) NK_CUDA(cudaStreamWaitEvent(ps, ev_done, 0));    // group G - 2 no longer reads this set
+        for (int64_t s0 = g0; s0 < g0 + gn; s0 += chunk) {
+            const int64_t nb = (g0 + gn - s0 < chunk) ? (g0 + gn - s0) : chunk;
+            const int8_t* sg = sigma + s0 * N;
+            if (tl_chunk_ready != nullptr) NK_CUDA(cudaStreamWaitEvent(ps, (*tl_chunk_ready)[(size_t)(s0 / chunk)], 0));
+            {
+                Scope sc(PH_GEMM, ps);
+                NK_CUDA(run_theta(g, sg, nb, w.Wg, w.bg, w.Ws, w.A, w.theta, ps));
+            }
+            if (logpsi_out || series) {        // ln psi and, in the same pass over theta, the series form's operand rows
+                Scope sc(PH_LOGPSI, ps);
+                uint16_t* ap = series ? w.ser.Ap[set] + (size_t)(s0 - g0) * SERIES_SEGS * g.M_pad : nullptr;
+                NK_CUDA(launch_logpsi(sg, nb, g, dtype, w.theta, a, logpsi_out ? (uint8_t*)logpsi_out + s0 * esz : nullptr,
+                                      false, nullptr, ps, series ? w.ser.ctl : nullptr, ap));
+            }
+            {
+                // the SIMT forms (the only ones when the series form is impossible; gated stand-ins when it may run:
+                // every launch is made, those on the wrong side of the gates return at once) stay on the preparation
+                // stream, off the critical path of the tensor-core launches
+                Scope sc(PH_FUSED, ps);
+                void* out = (uint8_t*)eloc_out + s0 * esz;
+                if (automatic) {
+                    const unsigned* sctl = series ? w.ser.ctl : nullptr;
+                    NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Ttab, w.rows, out, true, ps, w.taumax, 1, sctl));
+                    NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Dtab, w.rows, out, false, ps, w.taumax, 2, sctl));
+                } else if (!force_series) {
+                    NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, force_product ? w.Ttab : w.Dtab, w.rows, out,
+                                              force_product, ps));
+                }
             }
         }
+        if (!series) continue;
+        NK_CUDA(launch_series_prep(g, sigma + g0 * N, gn, w.ser, set, ps));
         if (pipelined) {
             NK_CUDA(cudaEventRecord(ev_prep, ps));
             NK_CUDA(cudaStreamWaitEvent(st, ev_prep, 0));
         }
-        if (series) {
+        {
             Scope sc(PH_FUSED, st);
-            NK_CUDA(launch_series_gemm(g, s0, nb, w.rows, w.ser, set, st));
+            NK_CUDA(launch_series_gemm(g, g0, gn, w.rows, w.ser, set, st));
         }
         if (pipelined) NK_CUDA(cudaEventRecord(ev_done, st));
     }

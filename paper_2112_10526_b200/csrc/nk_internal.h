@@ -156,15 +156,17 @@ cudaError_t launch_connected(const Operator* op, const int8_t* sigma, int64_t B,
 struct SeriesWs {
     unsigned* ctl;              // [16] control block written per call: ctl[0] = K (0 = path off), scales, row bounds
     uint16_t* Bp;               // [n_rows][SERIES_SEGS][M_pad] 16-bit operand rows of the table (per call)
-    // per-chunk buffers, two sets when the chunk loop is pipelined over two streams (api.cu):
-    uint16_t* Ap[2];            // [chunk][SERIES_SEGS][M_pad] 16-bit operand rows of the samples
-    uint32_t* sigT[2];          // [N][w32] transposed bit-packed spins of the chunk
+    // per-group buffers (a group = `group` consecutive chunks contracted by one launch), two sets when there is more
+    // than one group (api.cu pipelines them over two streams):
+    uint16_t* Ap[2];            // [group_rows][SERIES_SEGS][M_pad] 16-bit operand rows of the samples
+    uint32_t* sigT[2];          // [N][w32] transposed bit-packed spins of the group
     float* part;                // [n_nt][part_stride] partial local energies per column tile, whole batch
-    int w32, n_nt;
+    int w32, n_nt, group, n_sets;
+    int64_t group_rows;
     int64_t part_stride;
 };
 bool series_possible(const Geometry& g, int dtype);
-SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk, int n_sets, int64_t B);
+SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk, int64_t B);
 cudaError_t launch_series_prep(const Geometry& g, const int8_t* sigma, int64_t nb, const SeriesWs& w, int set,
                                cudaStream_t st);
 cudaError_t launch_series_pack(const Geometry& g, const float* Ttab, const unsigned* taumax_bits, const SeriesWs& w,

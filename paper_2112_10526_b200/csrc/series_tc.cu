@@ -44,17 +44,26 @@ namespace nk {
 
 namespace ser {
 constexpr int BM = 128, BN = 256, BK = 64;                // BK 16-bit elements = one 128-B swizzle row
-constexpr int A_TILE = BM * BK * 2, B_TILE = BN * BK * 2; // 16 KB, 32 KB
-constexpr int NA = 4, NB = 4;                             // ring depths (3 + 3 measured: GEMM 181 -> 207 us per chunk)
+constexpr int A_TILE = BM * BK * 2;                       // 16 KB
+constexpr int NA = 4;                                     // ring depths (3 + 3 measured: GEMM 181 -> 207 us per chunk)
 constexpr int THREADS = 224;                              // warps: A producer, MMA, B producer, 4 x epilogue
 constexpr int TAB_BYTES = BN * 16, MSK_BYTES = BN * 8;    // (coef, jdiag, a2, c2) per column, shared by the epilogue warps;
                                                           // (act, neg) spin masks per column and epilogue warp
-constexpr int SMEM_BYTES = NA * A_TILE + NB * B_TILE + TAB_BYTES + 4 * MSK_BYTES + 256 /*barriers*/ + 1024 /*alignment*/;
+// CG = CTAs per tile: 1 (a CTA owns a 128 x 256 tile) or 2 (a CTA PAIR owns 256 x 256 through tcgen05 cta_group::2: each
+// CTA holds its 128 samples' A tiles and HALF of every B tile, so the table-row operand crosses L2 -> shared memory and
+// shared memory -> tensor core once per 256 samples instead of once per 128)
+template <int CG> struct Cfg {
+    static constexpr int B_TILE = (BN / CG) * BK * 2;     // 32 KB, or 16 KB per CTA of a pair
+    static constexpr int NB = CG == 2 ? 6 : 4;
+    static constexpr int SMEM_BYTES = NA * A_TILE + NB * B_TILE + TAB_BYTES + 4 * MSK_BYTES + 256 /*barriers*/ + 1024 /*alignment*/;
+};
 constexpr uint32_t TMEM_COLS = 512;                       // odd at column 0, even at column 256
 // instruction descriptors of kind::f16 (the cute::UMMA::InstrDescriptor bit layout): D = F32 (c_format 1 at bit 4),
 // A / B format at bits 7 / 10 (0 = F16, 1 = BF16), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
-constexpr uint32_t IDESC_F16 = (1u << 4) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
-constexpr uint32_t IDESC_BF16 = IDESC_F16 | (1u << 7) | (1u << 10);
+template <int CG> struct Idesc {
+    static constexpr uint32_t F16 = (1u << 4) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)((BM * CG) >> 4) << 24);
+    static constexpr uint32_t BF16 = F16 | (1u << 7) | (1u << 10);
+};
 }  // namespace ser
 
 // ---- control block (device): ctl[0] = K (0: path off), ctl[1] = 2^e as float bits (undoes the power-of-two scale of
@@ -196,10 +205,48 @@ __device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t adesc, uint64
         : "memory");
 }
 
+// ---- cta_group::2 forms (the CTA pair of one TPC; rank 0 = the leader, which alone issues the MMAs) -----------------
+__device__ __forceinline__ void umma_f16_cg2(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                             uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}\n" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// arrives (once) on the barrier at this shared-memory offset in BOTH CTAs of the pair when the MMAs issued so far are done
+__device__ __forceinline__ void umma_commit_cg2(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+                 "h"((uint16_t)3)
+                 : "memory");
+}
+// the shared::cluster address of `addr` (an address in this CTA's shared window) in the CTA of rank `rank`
+__device__ __forceinline__ uint32_t map_to_rank(uint32_t addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+// TMA load of a CTA of the pair: the box lands in THIS CTA's shared memory, the bytes are counted on the leader's barrier
+__device__ __forceinline__ void tma_load_2d_cg2(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t leader_bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+        ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(leader_bar)
+        : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+
+template <int CG>
 __global__ void __launch_bounds__(ser::THREADS, 1)
 series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b,
                    const SeriesParams p) {
     using namespace ser;
+    constexpr int NB = Cfg<CG>::NB, B_TILE = Cfg<CG>::B_TILE;
+    constexpr uint32_t IDESC_F16 = Idesc<CG>::F16, IDESC_BF16 = Idesc<CG>::BF16;
+    const uint32_t rank = CG == 2 ? cluster_ctarank() : 0u;            // rank 0 leads the pair
     const int K = (int)p.ctl[0];
     if (K == 0) return;                                    // grid-uniform: the path is off for these parameters
     extern __shared__ uint8_t smem_raw[];
@@ -214,22 +261,36 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_jb = p.M_pad / BK;
-    const int n_tiles = p.n_mt * p.n_nt;
+    const int n_tiles = ((p.n_mt + CG - 1) / CG) * p.n_nt;              // tiles of CG x 128 samples x 256 table rows
+    const int unit = blockIdx.x / CG, n_units = gridDim.x / CG;         // the CTA (pair) as a tile worker
+    // `full` barriers count the bytes of BOTH CTAs of a pair and live in the leader; `empty` / accumulator-ready barriers
+    // are local, signalled in both CTAs by the leader's multicast commits; the accumulators of both CTAs are handed back
+    // on the leader's t_empty
+    const uint32_t a_full_l = CG == 2 ? map_to_rank(a_full, 0) : a_full;
+    const uint32_t b_full_l = CG == 2 ? map_to_rank(b_full, 0) : b_full;
+    const uint32_t t_empty_l = CG == 2 ? map_to_rank(t_empty, 0) : t_empty;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < NA; ++s) { mbar_init(a_full + 8 * s, 1); mbar_init(a_empty + 8 * s, 1); }
         for (int s = 0; s < NB; ++s) { mbar_init(b_full + 8 * s, 1); mbar_init(b_empty + 8 * s, 1); }
         mbar_init(t_full, 1);
-        mbar_init(t_empty, 128);
+        mbar_init(t_empty, 128 * CG);
         mbar_fence_init();
     }
-    if (warp == 1) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS)
-                     : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if (warp == 1) {                                       // the same warp in both CTAs of a pair
+        if (CG == 2) {
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS)
+                         : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+        } else {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS)
+                         : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (CG == 2) cluster_sync_all();                       // the peer's barriers exist before anything signals them
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem_base = *tmem_slot_ptr;
 
@@ -248,12 +309,13 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
             auto load = [&](int seg, int jb, int m0) {
                 const uint32_t slot = it % NA, par = ((it / NA) & 1u) ^ 1u;
                 mbar_wait(a_empty + 8 * slot, par);
-                mbar_arrive_expect_tx(a_full + 8 * slot, A_TILE);
-                tma_load_2d(a_ring + slot * A_TILE, &map_a, seg * p.M_pad + jb * BK, m0, a_full + 8 * slot);
+                if (rank == 0) mbar_arrive_expect_tx(a_full + 8 * slot, CG * A_TILE);
+                if (CG == 2) tma_load_2d_cg2(a_ring + slot * A_TILE, &map_a, seg * p.M_pad + jb * BK, m0, a_full_l + 8 * slot);
+                else tma_load_2d(a_ring + slot * A_TILE, &map_a, seg * p.M_pad + jb * BK, m0, a_full + 8 * slot);
                 ++it;
             };
-            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-                const int m0 = (tile / p.n_nt) * BM;
+            for (int tile = unit; tile < n_tiles; tile += n_units) {
+                const int m0 = ((tile / p.n_nt) * CG + (int)rank) * BM;
                 for (int jb = 0; jb < n_jb; ++jb) {
                     for (int k = K; k >= 3; --k) load(k, jb, m0);
                     load(1, jb, m0);                       // t_lo
@@ -269,12 +331,13 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
             auto load = [&](int seg, int jb, int n0) {
                 const uint32_t slot = it % NB, par = ((it / NB) & 1u) ^ 1u;
                 mbar_wait(b_empty + 8 * slot, par);
-                mbar_arrive_expect_tx(b_full + 8 * slot, B_TILE);
-                tma_load_2d(b_ring + slot * B_TILE, &map_b, seg * p.M_pad + jb * BK, n0, b_full + 8 * slot);
+                if (rank == 0) mbar_arrive_expect_tx(b_full + 8 * slot, CG * B_TILE);
+                if (CG == 2) tma_load_2d_cg2(b_ring + slot * B_TILE, &map_b, seg * p.M_pad + jb * BK, n0, b_full_l + 8 * slot);
+                else tma_load_2d(b_ring + slot * B_TILE, &map_b, seg * p.M_pad + jb * BK, n0, b_full + 8 * slot);
                 ++it;
             };
-            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-                const int n0 = (tile % p.n_nt) * BN;
+            for (int tile = unit; tile < n_tiles; tile += n_units) {
+                const int n0 = (tile % p.n_nt) * BN + (int)rank * (BN / CG);      // this CTA's half of the table rows
                 for (int jb = 0; jb < n_jb; ++jb) {
                     for (int k = K; k >= 3; --k) load(k, jb, n0);
                     load(0, jb, n0);                       // tau_hi
@@ -284,8 +347,8 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer (one thread) =====
-        if (lane == 0) {
+        // ===== MMA issuer (one thread of the leader CTA) =====
+        if (lane == 0 && rank == 0) {
             uint32_t ia = 0, ib = 0, n_done = 0;
             const uint32_t acc_odd = tmem_base, acc_even = tmem_base + BN;
             bool fresh_odd = true, fresh_even = true;
@@ -296,14 +359,20 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
                 const uint32_t a_addr = a_ring + (sa % NA) * A_TILE, b_addr = b_ring + (sb % NB) * B_TILE;
                 bool& fresh = odd ? fresh_odd : fresh_even;
 #pragma unroll
-                for (int k = 0; k < BK / 16; ++k)          // 16 elements = 32 B inside the 128-B swizzle row
-                    umma_f16(odd ? acc_odd : acc_even, make_sdesc(a_addr + k * 32), make_sdesc(b_addr + k * 32), idesc,
-                             (fresh && k == 0) ? 0u : 1u);
+                for (int k = 0; k < BK / 16; ++k) {        // 16 elements = 32 B inside the 128-B swizzle row
+                    if (CG == 2)
+                        umma_f16_cg2(odd ? acc_odd : acc_even, make_sdesc(a_addr + k * 32), make_sdesc(b_addr + k * 32),
+                                     idesc, (fresh && k == 0) ? 0u : 1u);
+                    else
+                        umma_f16(odd ? acc_odd : acc_even, make_sdesc(a_addr + k * 32), make_sdesc(b_addr + k * 32), idesc,
+                                 (fresh && k == 0) ? 0u : 1u);
+                }
                 fresh = false;
             };
-            auto a_free = [&](uint32_t i) { umma_commit(a_empty + 8 * (i % NA)); };
-            auto b_free = [&](uint32_t i) { umma_commit(b_empty + 8 * (i % NB)); };
-            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++n_done) {
+            auto commit = [&](uint32_t bar) { if (CG == 2) umma_commit_cg2(bar); else umma_commit(bar); };
+            auto a_free = [&](uint32_t i) { commit(a_empty + 8 * (i % NA)); };
+            auto b_free = [&](uint32_t i) { commit(b_empty + 8 * (i % NB)); };
+            for (int tile = unit; tile < n_tiles; tile += n_units, ++n_done) {
                 mbar_wait(t_empty, (n_done & 1u) ^ 1u);    // the epilogue has drained the accumulators (free at first)
                 fresh_odd = fresh_even = true;
                 for (int jb = 0; jb < n_jb; ++jb) {        // sweep 1: the small terms
@@ -330,7 +399,7 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
                     a_free(ia + 1); b_free(ib + 1);
                     ia += 2; ib += 2;
                 }
-                umma_commit(t_full);
+                commit(t_full);
             }
         }
     } else {
@@ -341,8 +410,8 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
         const int wq = warp - 3;                           // 0..3: which quarter of the row records this warp stages
         const float inv = __uint_as_float(p.ctl[1]);
         uint32_t n_done = 0;
-        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++n_done) {
-            const int mt = tile / p.n_nt, nt = tile - mt * p.n_nt;
+        for (int tile = unit; tile < n_tiles; tile += n_units, ++n_done) {
+            const int nt = tile % p.n_nt, mt = (tile / p.n_nt) * CG + (int)rank;     // this CTA's 128 samples
             const int n0 = nt * BN;
             // per column: matrix element, diagonal coupling and exponents (staged once for the four warps) and this warp's
             // 32 samples' two spin masks
@@ -376,7 +445,7 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
                 if (c0 + 32 == BN) {                       // both accumulators are in registers: hand them back
                     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                    mbar_arrive(t_empty);
+                    if (CG == 2) mbar_arrive_cluster(t_empty_l); else mbar_arrive(t_empty);
                 }
 #pragma unroll
                 for (int jj = 0; jj < 32; ++jj) {
@@ -394,9 +463,13 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (CG == 2) cluster_sync_all();                       // no peer still signals this CTA's barriers or reads its operands
     if (warp == 1) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+        if (CG == 2)
+            asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+        else
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
     }
 }
 
@@ -432,20 +505,36 @@ series_finish_kernel(const float* __restrict__ part, int n_nt, int64_t part_stri
 static std::mutex g_ser_mutex;
 static bool g_ser_ready[NK_MAX_DEVICES];
 static int g_ser_sms[NK_MAX_DEVICES];
+static int g_ser_pairs[NK_MAX_DEVICES];                    // co-resident CTA pairs (0: the device refuses 2-CTA clusters)
 
 static cudaError_t series_init() {
     std::lock_guard<std::mutex> lock(g_ser_mutex);
     const int d = current_device();
     if (g_ser_ready[d]) return cudaSuccess;
     if (tensor_map_encoder() == nullptr) return cudaErrorNotSupported;
-    cudaError_t e = cudaFuncSetAttribute((const void*)series_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         ser::SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute((const void*)series_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         ser::Cfg<1>::SMEM_BYTES);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute((const void*)series_gemm_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 ser::Cfg<2>::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     int dev = 0, sms = 0;
     e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return e;
     g_ser_sms[d] = sms > 0 ? sms : 148;
+    {   // how many CTA pairs the device co-schedules
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(2, 1, 1); cfg.blockDim = dim3(ser::THREADS, 1, 1); cfg.dynamicSmemBytes = ser::Cfg<2>::SMEM_BYTES;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, (const void*)series_gemm_kernel<2>, &cfg) != cudaSuccess) n = 0;
+        (void)cudaGetLastError();
+        g_ser_pairs[d] = n;
+    }
     g_ser_ready[d] = true;
     return cudaSuccess;
 }
@@ -467,21 +556,55 @@ bool series_possible(const Geometry& g, int dtype) {
     return dtype == NK_F32 && g.n_rows >= SERIES_MIN_ROWS && g.M_pad >= SERIES_MIN_MPAD;
 }
 
-SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk, int n_sets, int64_t B) {
+// How many chunks one tensor-core launch covers.  A launch runs ceil(tiles / units) waves of tiles over `units` CTA pairs
+// (or CTAs), so a chunk whose tile count is not a multiple of `units` leaves the last wave partly idle (config 5: 128
+// pair tiles on 74 pairs = 1.73 waves, 13 % idle).  The sample-side operand rows of `group` consecutive chunks are
+// therefore kept (two such buffers when there is more than one group: the preparation of group G + 1 runs beside the
+// launch of group G) and contracted together: the smallest group <= 8 within 3 % of the best wave efficiency, capped at
+// 1 GiB of operand rows per buffer.  Depends on sizes only, never on the parameters or the samples.
+static int series_group(const Geometry& g, int64_t chunk, int64_t B, int n_nt) {
+    if (chunk >= B) return 1;
+    int units = 74, cg = 2;
+    if (series_init() == cudaSuccess) {
+        const int d = current_device();
+        if (g_ser_pairs[d] > 0) units = g_ser_pairs[d];
+        else { units = g_ser_sms[d]; cg = 1; }
+    }
+    const size_t row_bytes = (size_t)SERIES_SEGS * g.M_pad * 2;
+    double best = 0.0, eff[9];
+    int gmax = 1;
+    for (int k = 1; k <= 8; ++k) {
+        if ((int64_t)k * chunk > B && k > 1 && (int64_t)(k - 1) * chunk >= B) break;
+        if ((size_t)k * chunk * row_bytes > ((size_t)1 << 30) && k > 1) break;
+        const int64_t rows = (int64_t)k * chunk < B ? (int64_t)k * chunk : B;
+        const int64_t tiles = (rows + 128 * cg - 1) / (128 * cg) * n_nt;
+        eff[k] = (double)tiles / (double)((tiles + units - 1) / units * units);
+        if (eff[k] > best) best = eff[k];
+        gmax = k;
+    }
+    for (int k = 1; k <= gmax; ++k)
+        if (eff[k] >= 0.97 * best) return k;
+    return 1;
+}
+
+SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk, int64_t B) {
     auto take = [&](size_t bytes) -> void* {
         void* r = base ? base + *off : nullptr;
         *off += align256(bytes);
         return r;
     };
     SeriesWs w;
-    w.w32 = (int)((chunk + 127) / 128 * 4);
     w.n_nt = (g.n_rows + ser::BN - 1) / ser::BN;
+    w.group = series_group(g, chunk, B, w.n_nt);
+    w.group_rows = (int64_t)w.group * chunk < B ? (int64_t)w.group * chunk : B;
+    w.n_sets = w.group_rows < B ? 2 : 1;
+    w.w32 = (int)((w.group_rows + 127) / 128 * 4);
     w.part_stride = (B + 127) / 128 * 128 + 128;       // whole batch (32 B per sample at config 5): one finishing pass
     w.ctl = (unsigned*)take(SER_CTL_WORDS * sizeof(unsigned));
     w.Bp = (uint16_t*)take((size_t)g.n_rows * SERIES_SEGS * g.M_pad * 2);
-    for (int k = 0; k < 2; ++k) {                      // per-chunk buffers: two sets when the chunks are pipelined
-        if (k < n_sets) {
-            w.Ap[k] = (uint16_t*)take((size_t)chunk * SERIES_SEGS * g.M_pad * 2);
+    for (int k = 0; k < 2; ++k) {                      // per-group buffers
+        if (k < w.n_sets) {
+            w.Ap[k] = (uint16_t*)take((size_t)w.group_rows * SERIES_SEGS * g.M_pad * 2);
             w.sigT[k] = (uint32_t*)take((size_t)g.N * w.w32 * 4);
         } else { w.Ap[k] = w.Ap[0]; w.sigT[k] = w.sigT[0]; }
     }
@@ -503,7 +626,8 @@ cudaError_t launch_series_pack(const Geometry& g, const float* Ttab, const unsig
     return cudaGetLastError();
 }
 
-// per chunk, buffer set `set`: the transposed spin bits (preparation; may run on another stream than the GEMM)
+// per group of chunks (nb samples), buffer set `set`: the transposed spin bits (preparation; may run on another stream
+// than the GEMM)
 cudaError_t launch_series_prep(const Geometry& g, const int8_t* sigma, int64_t nb, const SeriesWs& w, int set,
                                cudaStream_t st) {
     if (nb <= 0) return cudaSuccess;
@@ -515,25 +639,42 @@ cudaError_t launch_series_prep(const Geometry& g, const int8_t* sigma, int64_t n
     return cudaGetLastError();
 }
 
-// per chunk (samples s0 .. s0 + nb of the batch): partial local energies per column tile into w.part, from the operand
+// per group of chunks (samples s0 .. s0 + nb of the batch): partial local energies per column tile into w.part, from the operand
 // rows launch_logpsi left in w.Ap[set] and the bits of launch_series_prep (returns at once when ctl says the path is off)
 cudaError_t launch_series_gemm(const Geometry& g, int64_t s0, int64_t nb, const RowInfo* rows, const SeriesWs& w, int set,
                                cudaStream_t st) {
     if (nb <= 0) return cudaSuccess;
     cudaError_t e = series_init();
     if (e != cudaSuccess) return e;
-    const int sms = g_ser_sms[current_device()];
+    const int sms = g_ser_sms[current_device()], pairs = g_ser_pairs[current_device()];
     const int n_mt = (int)((nb + ser::BM - 1) / ser::BM);
+    const bool pair = pairs > 0 && n_mt >= 2;              // CTA pairs (cta_group::2) whenever there are two sample tiles
     CUtensorMap map_a, map_b;
     const uint64_t cols = (uint64_t)SERIES_SEGS * g.M_pad;
     if (!encode_u16(&map_a, w.Ap[set], (uint64_t)nb, cols, ser::BM)) return cudaErrorInvalidValue;
-    if (!encode_u16(&map_b, w.Bp, (uint64_t)g.n_rows, cols, ser::BN)) return cudaErrorInvalidValue;
+    if (!encode_u16(&map_b, w.Bp, (uint64_t)g.n_rows, cols, pair ? ser::BN / 2 : ser::BN)) return cudaErrorInvalidValue;
     SeriesParams p;
     p.ctl = w.ctl; p.rows = rows; p.sigT = w.sigT[set]; p.w32 = w.w32; p.nb = nb; p.n_rows = g.n_rows; p.M_pad = g.M_pad;
     p.n_mt = n_mt; p.n_nt = w.n_nt; p.part = w.part + s0; p.part_stride = w.part_stride;
-    const int n_tiles = n_mt * w.n_nt;
     ProfScope sc(PH_SERIES_GEMM, st);
-    series_gemm_kernel<<<n_tiles < sms ? n_tiles : sms, ser::THREADS, ser::SMEM_BYTES, st>>>(map_a, map_b, p);
+    if (pair) {
+        const int n_tiles = ((n_mt + 1) / 2) * w.n_nt;
+        const int units = n_tiles < pairs ? n_tiles : pairs;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(2 * units), 1, 1);
+        cfg.blockDim = dim3(ser::THREADS, 1, 1);
+        cfg.dynamicSmemBytes = ser::Cfg<2>::SMEM_BYTES;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, series_gemm_kernel<2>, map_a, map_b, p);
+        if (e != cudaSuccess) return e;
+    } else {
+        const int n_tiles = n_mt * w.n_nt;
+        series_gemm_kernel<1><<<n_tiles < sms ? n_tiles : sms, ser::THREADS, ser::Cfg<1>::SMEM_BYTES, st>>>(map_a, map_b, p);
+    }
     count_launch();
     return cudaGetLastError();
 }
