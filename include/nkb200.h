@@ -52,7 +52,10 @@ enum nk_kind { NK_HEISENBERG = 0, NK_ISING = 1 };
 enum nk_dtype { NK_F32 = 0, NK_C64 = 1 };
 enum nk_rule { NK_RULE_LOCAL = 0, NK_RULE_EXCHANGE = 1 };
 enum nk_flags {
-    NK_FLAG_MARSHALL = 1u,     /* nk_operator_create: off-diagonal Heisenberg element -2J (default +2J, Eq. (50)) */
+    NK_FLAG_MARSHALL = 1u,     /* nk_operator_create: off-diagonal Heisenberg element -2J on EVERY bond (default +2J, Eq. (50)).
+                                  This is the sublattice rotation U H U, U = prod_{i in A} sz_i, only if every bond joins
+                                  the two sublattices; with same-sublattice bonds in the list (e.g. next-nearest neighbours)
+                                  it defines a different Hamiltonian — give such bonds a colour with the sign folded into J */
     NK_OUT_F64 = 2u,           /* nk_rbm_logpsi: logpsi_out is double / (re,im) double instead of float */
     NK_FORM_PRODUCT = 4u,      /* nk_local_energy_ex: product-form amplitude ratios (see there) */
     NK_CHECK_SPINS = 8u,       /* nk_local_energy_ex: validate sigma in {+1,-1} first (one extra pass over sigma and one

@@ -106,6 +106,19 @@ __device__ __forceinline__ float finish_single(const RowPartR& A) {
     return A.coef * (r * ex2_approx(fmaf(0.5f, acc, A.ex)));
 }
 
+// y - 2 pi rint(y / 2 pi): the fast __sincosf keeps its 2^-21.4 bound only on [-pi, pi] (beyond, its error grows like
+// |y| 2^-24), and a trained complex RBM has |Im theta| of order 10 .. 100.  Im theta is wrapped once per sample at load
+// and at every accepted move (the per-pair argument is then the wrapped value plus one table entry, |D| <~ 1), the
+// exponent's imaginary part once per amplitude.  Two-constant reduction: 2 pi = 6.28125 + 1.9353072e-3 (the first exact
+// in 8 bits, so k * 6.28125 is exact for |k| < 2^16).
+__device__ __forceinline__ float wrap_pi(float y) {
+    const float k = rintf(y * 0.15915494309189535f);
+    return fmaf(k, -1.9353071795864769e-3f, fmaf(k, -6.28125f, y));
+}
+__device__ __forceinline__ float4 wrap_pi4(float4 y) {
+    return make_float4(wrap_pi(y.x), wrap_pi(y.y), wrap_pi(y.z), wrap_pi(y.w));
+}
+
 template <int V>
 struct CplxState {
     float4 tx[V], ty[V];   // Re theta_s (scaled), Im theta (radians)
@@ -128,7 +141,7 @@ struct CplxState {
 #pragma unroll
         for (int v = 0; v < V; ++v) {
             float4 x = *reinterpret_cast<const float4*>(row + (v * 32 + lane) * 4);
-            const float4 y = *reinterpret_cast<const float4*>(row + M_pad + (v * 32 + lane) * 4);
+            const float4 y = wrap_pi4(*reinterpret_cast<const float4*>(row + M_pad + (v * 32 + lane) * 4));
             x.x *= KAPPA; x.y *= KAPPA; x.z *= KAPPA; x.w *= KAPPA;
             tx[v] = x; ty[v] = y;
             float p, q;
@@ -180,6 +193,7 @@ struct CplxState {
             tx[v].z = fmaf(s, dx.z, tx[v].z); tx[v].w = fmaf(s, dx.w, tx[v].w);
             ty[v].x = fmaf(s, dy.x, ty[v].x); ty[v].y = fmaf(s, dy.y, ty[v].y);
             ty[v].z = fmaf(s, dy.z, ty[v].z); ty[v].w = fmaf(s, dy.w, ty[v].w);
+            ty[v] = wrap_pi4(ty[v]);
         }
         const float inv = 1.f / fmaf(pr, pr, pi * pi);
         qr = pr * inv; qi = -pi * inv;
@@ -198,7 +212,7 @@ __device__ __forceinline__ void finish_c(float ar, float ai, float acc, float ex
                                          float& out_re, float& out_im) {
     const float mag = c * ex2_approx(fmaf(0.5f, acc, ex_re));
     float sn, cs;
-    __sincosf(ex_im, &sn, &cs);
+    __sincosf(wrap_pi(ex_im), &sn, &cs);
     cmul_f(ar, ai, mag * cs, mag * sn);
     out_re = ar; out_im = ai;
 }

@@ -354,3 +354,17 @@ def test_non_finite_parameters_propagate(nk):
         assert not np.isfinite(e.cpu().numpy()).any() and not np.isfinite(lp2.cpu().numpy()).any()
         assert not np.isfinite(st.cpu().numpy()[0])
         op.close()
+
+
+def test_complex_large_imaginary_theta(nk):
+    """Im b shifted by whole multiples of 2 pi (|Im theta| up to ~13, as in trained sign structures): the fused kernel's
+    fast sincos sees range-reduced arguments (rbm_lane_state.cuh wrap_pi), so E_loc keeps its bound; ln psi mod 2 pi
+    likewise.  cosh is 2 pi i-periodic, so the conditioning of the problem is that of config 4 itself."""
+    p = inp.make_config(4, n_samples=96)
+    rng = np.random.default_rng(5)
+    shift = (2 * np.pi * rng.integers(-2, 3, size=p.b.shape)).astype(np.float32)
+    p.b = (p.b + 1j * shift).astype(np.complex64)
+    e, lp, _ = run_gpu(nk, p)
+    e_ref, lp_ref = run_oracle(p)
+    assert_eloc(e, e_ref)
+    assert_logpsi(lp, lp_ref, atol=3e-5)
