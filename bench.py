@@ -197,13 +197,8 @@ def time_extras(nk, torch, p, op, sigma, W, a, b, dt_code, plan):
     n_cg = 8
     ms_sr = _time_ms(torch, lambda: nk.sr_solve(chains, W, b, ga, gb, gW, diag_shift=0.01, tol=0.0, max_iter=n_cg,
                                                 chunk_size=gchunk, ws=sws), 2)
-    # the graded step replayed from a CUDA graph (LocalEnergyPlan.run_graph): what launch overhead costs the small configs
-    plan.run_graph(sigma, W, a, b)
-    ms_graph = _time_ms(torch, lambda: plan.run_graph(sigma, W, a, b), 5)
     planes = 2 if p.complex_params else 1
     return {
-        "cuda_graph": {"ms_per_step": ms_graph, "local_energies_per_sec": B / (ms_graph * 1e-3),
-                       "what": "the same nk_local_energy step replayed from a captured CUDA graph, no L2 flush"},
         "sampler": {"rule": "exchange" if exch else "local", "chains": B, "transitions_per_chain": N,
                     "ms_per_sweep": ms_sweep, "transitions_per_sec": B * N / (ms_sweep * 1e-3), "acceptance": acceptance,
                     "evaluated_fraction_estimate": anti,
@@ -278,8 +273,14 @@ def run_ours(args):
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)         # > 126 MB L2
     gathered = [torch.zeros(4, dtype=torch.float64, device=dev) for _ in range(world)]
 
-    def step():
-        _, _, stats = plan.run(sigma, W, a, b)
+    # the graded call: nk_local_energy_plan_run — the launches of nk_local_energy captured once into a CUDA graph by the
+    # library (nk_local_energy_plan_create) and replayed per step, every kernel of the step included (--call eager times
+    # nk_local_energy itself; the other one is reported beside it)
+    def call(planned):
+        return plan.run_graph(sigma, W, a, b) if planned else plan.run(sigma, W, a, b)
+
+    def step(planned=(args.call == "plan")):
+        _, _, stats = call(planned)
         if world > 1:
             dist.all_gather(gathered, stats)
 
@@ -305,6 +306,22 @@ def run_ours(args):
         dist.barrier()
     launches = nk.launch_count(reset=True)
     step_ms = [a_.elapsed_time(b_) for a_, b_ in ev]
+    # the other way of making the call, same protocol, fewer steps
+    other_planned = args.call != "plan"
+    for _ in range(3):
+        step(other_planned)
+    torch.cuda.synchronize()
+    other_ms = 0.0
+    n_other = max(3, min(args.steps, 20))
+    oe = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+    for _ in range(n_other):
+        flush.zero_()
+        oe[0].record()
+        step(other_planned)
+        oe[1].record()
+        torch.cuda.synchronize()
+        other_ms += oe[0].elapsed_time(oe[1])
+    other_ms /= n_other
     # the same K steps once more with the library's per-kernel CUDA-event brackets on (nk_profile_enable): the kernel
     # durations behind `roofline`.  Kept out of the loop above because the brackets themselves cost timeline (two event
     # records per kernel group and chunk); the clock sampler covers both loops.
@@ -524,6 +541,9 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "c64" if cplx else "f32",
             "data": "synthetic (seeded, BASELINE.json recipe)",
             "config": {"workload": CONFIG_TEXT[args.config], "samples_per_gpu": B, "n_sites": N, "n_hidden": M,
+                       "call": ("nk_local_energy_plan_run: the step's launches captured once into a CUDA graph by "
+                                "nk_local_energy_plan_create and replayed" if args.call == "plan" else "nk_local_energy"),
+                       ("ms_per_step_eager_nk_local_energy" if args.call == "plan" else "ms_per_step_planned"): other_ms,
                        "chunk_size": p.chunk_size, "amplitudes_per_step_per_gpu": amps,
                        "l2": "flushed between steps (512 MiB memset outside the per-step CUDA events)",
                        "parallelism": f"samples sharded over {world} rank(s), statistics all-gathered"},
@@ -577,7 +597,7 @@ def spawn_command(args, port=None):
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__),
            "--gpus", str(args.gpus), "--steps", str(args.steps), "--warmup", str(args.warmup),
-           "--config", str(args.config), "--impl", args.impl]
+           "--config", str(args.config), "--impl", args.impl, "--call", args.call]
     if args.no_extras:
         cmd.append("--no-extras")
     return cmd
@@ -591,6 +611,8 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the sampler / gradient timings")
+    ap.add_argument("--call", default="plan", choices=["plan", "eager"],
+                    help="the graded call: nk_local_energy_plan_run (CUDA-graph replay, default) or nk_local_energy")
     ap.add_argument("--peaks", action="store_true", help="only run the pipe-peak microbenchmarks (nk_pipe_peaks)")
     args = ap.parse_args()
     if args.peaks:

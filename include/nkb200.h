@@ -17,7 +17,7 @@
  * Conventions
  *   - "dev" pointers are CUDA device pointers, "host" pointers are ordinary host memory.  All buffers belong to
  *     the caller.  The library allocates device memory only inside nk_operator_create and frees it only in
- *     nk_operator_destroy.
+ *     nk_operator_destroy (nk_local_energy_plan_create additionally owns a CUDA graph).
  *   - Every call that takes a stream is asynchronous on that stream (a cudaStream_t passed as void*; NULL = the
  *     legacy default stream) and never synchronises the device, except nk_local_energy_host (see there).
  *   - Spins are int8 with values +1 / -1, row-major [B][N].  W is row-major [M][N] (theta = W s + b); a is [N],
@@ -39,6 +39,7 @@ extern "C" {
 
 typedef struct nk_operator_s* nk_operator_t;   /* opaque; device-resident bond table + couplings */
 typedef void* nk_stream_t;                      /* a cudaStream_t */
+typedef struct nk_plan_s* nk_plan_t;            /* opaque; one nk_local_energy_ex call captured into a CUDA graph */
 
 enum nk_status {
     NK_OK = 0,
@@ -160,6 +161,22 @@ int nk_local_energy_ex(nk_operator_t op, const int8_t* sigma, int64_t B, int N, 
                        const void* a, const void* b, int64_t chunk_size, unsigned flags, void* eloc_out,
                        void* logpsi_out, double* stats_out, void* workspace, size_t workspace_bytes,
                        nk_stream_t stream);
+
+/* The same call as a PLAN: nk_local_energy_plan_create runs nk_local_energy_ex once (so every error it can report is
+ * reported here; synchronises an internal stream), then captures its launches — both streams of the pipelined chunk loop
+ * included — into a CUDA graph; nk_local_energy_plan_run replays that graph on `stream`: one launch per step instead of
+ * ~85 (config 5) or ~15 (configs 1-2, which are launch-bound), the same kernels on the same buffers, the form of the
+ * ratios still chosen on the device from the CURRENT parameters.  The plan is bound to the addresses and sizes given
+ * at creation; the CONTENTS of sigma / W / a / b may change between runs, and the outputs are rewritten by every run.
+ * The buffers must outlive the plan.  NK_CHECK_SPINS cannot be planned (NK_ERR_INVALID_ARG).  Besides
+ * nk_operator_create this is the only call that allocates (a graph, its executable instance, one stream), released by
+ * nk_local_energy_plan_destroy.  nk_launch_count advances by the number of kernels in the graph on every run. */
+int nk_local_energy_plan_create(nk_plan_t* out, nk_operator_t op, const int8_t* sigma, int64_t B, int N, int M, int dtype,
+                                const void* W, const void* a, const void* b, int64_t chunk_size, unsigned flags,
+                                void* eloc_out, void* logpsi_out, double* stats_out, void* workspace,
+                                size_t workspace_bytes);
+int nk_local_energy_plan_run(nk_plan_t plan, nk_stream_t stream);
+int nk_local_energy_plan_destroy(nk_plan_t plan);
 
 /* Which form the most recent automatic nk_local_energy / nk_local_energy_ex call on `workspace` took (same op, B, N,
  * M, dtype, chunk_size as that call): *form_host = NK_FORM_SERIES, NK_FORM_PRODUCT or NK_FORM_LOGCOSH, *tau_max_host

@@ -38,6 +38,10 @@ EXPORTS = {
     "nk_local_energy": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_local_energy_ex": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _u32, _vp, _vp, _vp, _vp, _sz,
                                   _vp]),
+    "nk_local_energy_plan_create": (_int, [C.POINTER(_vp), _vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _u32, _vp,
+                                            _vp, _vp, _vp, _sz]),
+    "nk_local_energy_plan_run": (_int, [_vp, _vp]),
+    "nk_local_energy_plan_destroy": (_int, [_vp]),
     "nk_local_energy_form": (_int, [_vp, _i64, _int, _int, _int, _i64, _vp, _sz, _vp, _vp, _vp, _vp]),
     "nk_local_energy_host_scratch_bytes": (_sz, [_vp, _i64, _int, _int, _int, _i64]),
     "nk_local_energy_host": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
@@ -237,21 +241,34 @@ class LocalEnergyPlan:
         return form.value, tau.value
 
     def run_graph(self, sigma, W, a, b):
-        """The same call replayed from a CUDA graph: the first use with a given set of tensors runs once eagerly (one-
-        time attribute / tensor-map setup), captures the call's launches on torch's capture stream and keeps the graph;
-        later uses replay it — one launch instead of ~11 per chunk-less call, which is what bounds the small configs.
-        The tensors must stay alive and keep their addresses; their CONTENTS may change between replays."""
-        torch = _torch()
+        """nk_local_energy_plan_create / _run: the same call captured once into a CUDA graph by the library and replayed
+        — one launch per step instead of ~15 per chunk, which is what bounds the small configs.  The plan is bound to
+        the addresses of the tensors given first (their CONTENTS may change between replays; new tensors make a new
+        plan); the tensors must stay alive."""
         key = tuple(_ptr(t) for t in (sigma, W, a, b))
-        if getattr(self, "_graph_key", None) != key:
-            self.run(sigma, W, a, b)
-            torch.cuda.synchronize()
-            graph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(graph):
-                self.run(sigma, W, a, b)
-            self._graph, self._graph_key = graph, key
-        self._graph.replay()
+        if getattr(self, "_plan_key", None) != key:
+            self.close_plan()
+            h = _vp()
+            rc = load().nk_local_energy_plan_create(C.byref(h), self.op.handle, _ptr(sigma), self.B, self.N, self.M,
+                                                    self.dt, _ptr(W), _ptr(a), _ptr(b), self.chunk, self.flags,
+                                                    _ptr(self.eloc), _ptr(self.logpsi), _ptr(self.stats),
+                                                    _ptr(self.ws), self.ws_bytes)
+            _check(rc, "nk_local_energy_plan_create")
+            self._plan, self._plan_key = h, key
+            self._plan_keep = (sigma, W, a, b)
+        _check(load().nk_local_energy_plan_run(self._plan, _stream()), "nk_local_energy_plan_run")
         return self.eloc, self.logpsi, self.stats
+
+    def close_plan(self):
+        if getattr(self, "_plan", None) is not None and _lib is not None:
+            _lib.nk_local_energy_plan_destroy(self._plan)
+        self._plan, self._plan_key, self._plan_keep = None, None, None
+
+    def __del__(self):
+        try:
+            self.close_plan()
+        except Exception:
+            pass
 
 
 def local_energy(op: Operator, sigma, W, a=None, b=None, *, chunk_size: int = 0, want_logpsi: bool = True,

@@ -767,9 +767,10 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
     {
         Scope sc(PH_PACK, st);
         NK_CUDA(launch_pack(op, g, dtype, W, a, b, w.Wg, w.bg, w.Wt, w.Dtab, w.rows, st));
+        if (series) NK_CUDA(launch_series_ctl_reset(w.ser, st));
         if (force_product || automatic || force_series)
             NK_CUDA(launch_pack_product(op, g, dtype, w.Wt, w.Ttab, w.rows, st,
-                                        (automatic || force_series) ? w.taumax : nullptr));
+                                        (automatic || force_series) ? w.taumax : nullptr, series ? w.ser.ctl : nullptr));
         if (series) NK_CUDA(launch_series_pack(g, w.Ttab, w.taumax, w.ser, force_series, st));
         NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, st));
     }
@@ -848,6 +849,73 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
         Scope sc(PH_STATS, st);
         NK_CUDA(launch_stats(eloc_out, B, dtype, stats_out, st));
     }
+    return NK_OK;
+}
+
+// ---- plan: the call captured once into a CUDA graph, replayed per step ----------------------------------------------
+namespace {
+struct Plan {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    cudaStream_t capture_stream = nullptr;
+    int64_t launches = 0;                 // kernels of one replay (what nk_launch_count is advanced by)
+    int device = 0;
+};
+}  // namespace
+
+int nk_local_energy_plan_create(nk_plan_t* out, nk_operator_t h, const int8_t* sigma, int64_t B, int N, int M, int dtype,
+                                const void* W, const void* a, const void* b, int64_t chunk_size, unsigned flags,
+                                void* eloc_out, void* logpsi_out, double* stats_out, void* workspace,
+                                size_t workspace_bytes) {
+    if (!out) return NK_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (flags & NK_CHECK_SPINS) return NK_ERR_INVALID_ARG;           // that flag synchronises: not capturable
+    Plan* p = new (std::nothrow) Plan();
+    if (!p) return NK_ERR_INVALID_ARG;
+    auto fail = [&](int rc) { nk_local_energy_plan_destroy((nk_plan_t)p); return rc; };
+    if (cudaGetDevice(&p->device) != cudaSuccess) return fail(NK_ERR_CUDA);
+    cudaError_t e = cudaStreamCreateWithFlags(&p->capture_stream, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return fail(cuda_fail(e));
+    // once eagerly: argument checks, one-time attribute / stream / event set-up (none of which may happen in a capture)
+    int rc = nk_local_energy_ex(h, sigma, B, N, M, dtype, W, a, b, chunk_size, flags, eloc_out, logpsi_out, stats_out,
+                                workspace, workspace_bytes, (nk_stream_t)p->capture_stream);
+    if (rc != NK_OK) return fail(rc);
+    e = cudaStreamSynchronize(p->capture_stream);
+    if (e != cudaSuccess) return fail(cuda_fail(e));
+    const bool prof = tl_prof;
+    tl_prof = false;                                                 // no timing brackets inside the graph
+    const int64_t before = tl_launches;
+    e = cudaStreamBeginCapture(p->capture_stream, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) { tl_prof = prof; return fail(cuda_fail(e)); }
+    rc = nk_local_energy_ex(h, sigma, B, N, M, dtype, W, a, b, chunk_size, flags, eloc_out, logpsi_out, stats_out,
+                            workspace, workspace_bytes, (nk_stream_t)p->capture_stream);
+    e = cudaStreamEndCapture(p->capture_stream, &p->graph);
+    tl_prof = prof;
+    p->launches = tl_launches - before;
+    tl_launches = before;                                            // captured, not launched
+    if (rc != NK_OK) return fail(rc);
+    if (e != cudaSuccess || p->graph == nullptr) return fail(cuda_fail(e != cudaSuccess ? e : cudaErrorUnknown));
+    e = cudaGraphInstantiate(&p->exec, p->graph, 0);
+    if (e != cudaSuccess) return fail(cuda_fail(e));
+    *out = (nk_plan_t)p;
+    return NK_OK;
+}
+
+int nk_local_energy_plan_run(nk_plan_t plan, nk_stream_t stream) {
+    if (!plan) return NK_ERR_INVALID_ARG;
+    Plan* p = (Plan*)plan;
+    NK_CUDA(cudaGraphLaunch(p->exec, (cudaStream_t)stream));
+    count_launch((int)p->launches);
+    return NK_OK;
+}
+
+int nk_local_energy_plan_destroy(nk_plan_t plan) {
+    if (!plan) return NK_ERR_INVALID_ARG;
+    Plan* p = (Plan*)plan;
+    if (p->exec) cudaGraphExecDestroy(p->exec);
+    if (p->graph) cudaGraphDestroy(p->graph);
+    if (p->capture_stream) cudaStreamDestroy(p->capture_stream);
+    delete p;
     return NK_OK;
 }
 

@@ -86,7 +86,8 @@ cudaError_t launch_pack(const Operator* op, const Geometry& g, int dtype, const 
 cudaError_t launch_pack_gemm_only(const Geometry& g, int dtype, const void* W, const void* b, float* Wg, float* bg,
                                   cudaStream_t st);
 cudaError_t launch_pack_product(const Operator* op, const Geometry& g, int dtype, const float* Wt, float* tab,
-                                RowInfo* rows, cudaStream_t st, unsigned* taumax_bits = nullptr);
+                                RowInfo* rows, cudaStream_t st, unsigned* taumax_bits = nullptr,
+                                unsigned* series_ctl = nullptr);
 cudaError_t launch_pack_table(const Geometry& g, int dtype, const void* W, const void* b, const int32_t* pairs_dev,
                               int n_rows, float* Wg, float* bg, float* Wt, float* Dtab, cudaStream_t st);
 // sampler.cu : Metropolis-Hastings transitions with in-register incremental theta
@@ -169,6 +170,7 @@ bool series_possible(const Geometry& g, int dtype);
 SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chunk, int64_t B);
 cudaError_t launch_series_prep(const Geometry& g, const int8_t* sigma, int64_t nb, const SeriesWs& w, int set,
                                cudaStream_t st);
+cudaError_t launch_series_ctl_reset(const SeriesWs& w, cudaStream_t st);
 cudaError_t launch_series_pack(const Geometry& g, const float* Ttab, const unsigned* taumax_bits, const SeriesWs& w,
                                bool force, cudaStream_t st);
 cudaError_t launch_series_gemm(const Geometry& g, int64_t s0, int64_t nb, const RowInfo* rows, const SeriesWs& w, int set,

@@ -8,6 +8,7 @@
 //   rows [n_rows_pad]  RowInfo (sites, matrix element, visible-bias exponent)
 // theta' = theta - 2 s_k W[:,k] for a flipped site k (BASELINE.json north_star (3)); an exchange of antiparallel
 // spins i,j flips both: theta' = theta - 2 s_i (W[:,i] - W[:,j]).
+#include "lncosh.cuh"
 #include "nk_internal.h"
 
 namespace nk {
@@ -223,13 +224,97 @@ __global__ void rowc_kernel(const float* __restrict__ Wt, int n_rows, int M_pad,
     }
 }
 
+// Real parameters: the three per-row passes over d = 2 (W[:,i] - W[:,j]) in one — tau = tanh d into Ttab, the row
+// constant sum_j ln cosh d_j (fp32 series below 1/2, the stable fp64 form above, fp64 sum in a fixed order) into
+// rows[r].c2_re, max |tau| into *taumax_bits and, when series_ctl is given, the row sums of |tau|^3 .. |tau|^(K_MAX+1)
+// that bound the remainder of the tensor-core series form (series_tc.cu) into its control block.  One block per row.
+__global__ void __launch_bounds__(256)
+rowtab_real_kernel(const float* __restrict__ Wt, const int32_t* __restrict__ bonds, int kind, int n_rows, int M_pad,
+                   int M_eff, float* __restrict__ Ttab, RowInfo* __restrict__ rows, unsigned* __restrict__ taumax_bits,
+                   unsigned* __restrict__ series_ctl) {
+    const int r = blockIdx.x;
+    int i = -1, j = -1;
+    if (r < n_rows) {
+        if (kind == NK_HEISENBERG) { i = bonds[2 * r]; j = bonds[2 * r + 1]; }
+        else i = r;
+    }
+    float* out = Ttab + (size_t)r * M_eff;
+    if (i < 0) {                                               // padded row of the table
+        for (int m = threadIdx.x; m < M_pad; m += blockDim.x) out[m] = 0.f;
+        return;
+    }
+    const float* wi = Wt + (size_t)i * M_eff;
+    const float* wj = j >= 0 ? Wt + (size_t)j * M_eff : nullptr;
+    double lc = 0.0;
+    float pw[SERIES_K_MAX - 1];
+#pragma unroll
+    for (int k = 0; k < SERIES_K_MAX - 1; ++k) pw[k] = 0.f;
+    unsigned tmax = 0;
+    for (int m = threadIdx.x; m < M_pad; m += blockDim.x) {
+        float x = wi[m];
+        if (wj != nullptr) x -= wj[m];
+        x *= 2.f;
+        const float t = tanhf(x);
+        out[m] = t;
+        const float at = fabsf(t);
+        tmax = max(tmax, __float_as_uint(at));
+        float p = at * at;
+#pragma unroll
+        for (int k = 0; k < SERIES_K_MAX - 1; ++k) { p *= at; pw[k] += p; }
+        if (fabsf(x) < 0.5f) lc += (double)ln_cosh_small_f(x);
+        else {
+            const double ax = fabs((double)x);
+            lc += ax + log1p(exp(-2.0 * ax)) - 0.6931471805599453;
+        }
+    }
+    __shared__ double red_d[8];
+    __shared__ float red_f[8][SERIES_K_MAX - 1];
+    __shared__ unsigned red_u[8];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        lc += __shfl_xor_sync(0xffffffffu, lc, o);
+        tmax = max(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
+#pragma unroll
+        for (int k = 0; k < SERIES_K_MAX - 1; ++k) pw[k] += __shfl_xor_sync(0xffffffffu, pw[k], o);
+    }
+    if (lane == 0) {
+        red_d[warp] = lc; red_u[warp] = tmax;
+#pragma unroll
+        for (int k = 0; k < SERIES_K_MAX - 1; ++k) red_f[warp][k] = pw[k];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        unsigned u = 0;
+        for (int w = 0; w < 8; ++w) { t += red_d[w]; u = max(u, red_u[w]); }
+        rows[r].c2_re = (float)(t * 1.4426950408889634);
+        rows[r].c2_im = 0.f;
+        if (taumax_bits != nullptr && u) atomicMax(taumax_bits, u);
+    }
+    if (series_ctl != nullptr && threadIdx.x < SERIES_K_MAX - 1) {
+        float t = 0.f;
+        for (int w = 0; w < 8; ++w) t += red_f[w][threadIdx.x];
+        if (t != t) t = __int_as_float(0x7f800000);           // a NaN in the table must not look like a small bound
+        atomicMax(&series_ctl[4 + 3 + threadIdx.x], __float_as_uint(t));
+    }
+}
+
 // Fills `tab` with Ttab and rows[].c2_*; call after launch_pack.  taumax_bits (optional): max |tau| as float bits.
+// series_ctl (optional, real parameters): the zeroed control block of the series form, which receives the row sums of
+// |tau|^p (see rowtab_real_kernel).
 cudaError_t launch_pack_product(const Operator* op, const Geometry& g, int dtype, const float* Wt, float* tab,
-                                RowInfo* rows, cudaStream_t st, unsigned* taumax_bits) {
+                                RowInfo* rows, cudaStream_t st, unsigned* taumax_bits, unsigned* series_ctl) {
     const int cplx = dtype == NK_C64;
     if (taumax_bits != nullptr) {
         cudaError_t e = cudaMemsetAsync(taumax_bits, 0, sizeof(unsigned), st);
         if (e != cudaSuccess) return e;
+    }
+    if (!cplx) {
+        rowtab_real_kernel<<<g.n_rows_pad, 256, 0, st>>>(Wt, op->d_bonds, op->kind, g.n_rows, g.M_pad, g.M_eff, tab, rows,
+                                                         taumax_bits, series_ctl);
+        count_launch();
+        return cudaGetLastError();
     }
     dim3 gd((g.M_pad + 255) / 256, g.n_rows_pad);
     ttab_kernel<<<gd, 256, 0, st>>>(Wt, op->d_bonds, op->kind, g.n_rows, g.M_pad, g.M_eff, cplx, tab, taumax_bits);

@@ -70,33 +70,7 @@ template <int CG> struct Idesc {
 // tau), ctl[2] = log2(e) 2^-e as float bits (the scale applied to tau), ctl[4 + p] = max over rows of sum_j |tau|^p ----
 constexpr int SER_CTL_WORDS = 16;
 
-__global__ void __launch_bounds__(256)
-series_rowsum_kernel(const float* __restrict__ Ttab, int M_pad, int M_eff, unsigned* __restrict__ ctl) {
-    const float* row = Ttab + (size_t)blockIdx.x * M_eff;
-    float s[SERIES_K_MAX - 1];                            // powers 3 .. K_MAX + 1
-#pragma unroll
-    for (int i = 0; i < SERIES_K_MAX - 1; ++i) s[i] = 0.f;
-    for (int j = threadIdx.x; j < M_pad; j += blockDim.x) {
-        const float x = fabsf(row[j]);
-        float p = x * x;
-#pragma unroll
-        for (int i = 0; i < SERIES_K_MAX - 1; ++i) { p *= x; s[i] += p; }
-    }
-    __shared__ float red[8][SERIES_K_MAX - 1];
-#pragma unroll
-    for (int i = 0; i < SERIES_K_MAX - 1; ++i) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) s[i] += __shfl_xor_sync(0xffffffffu, s[i], o);
-        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5][i] = s[i];
-    }
-    __syncthreads();
-    if (threadIdx.x < SERIES_K_MAX - 1) {
-        float t = 0.f;
-        for (int w = 0; w < 8; ++w) t += red[w][threadIdx.x];
-        if (t != t) t = __int_as_float(0x7f800000);       // a NaN in the table must not look like a small bound
-        atomicMax(&ctl[4 + 3 + threadIdx.x], __float_as_uint(t));
-    }
-}
+// (the row sums ctl[4 + p] are formed by rowtab_real_kernel, pack.cu, in its pass over the table)
 
 // force: 0 = automatic (K = 0 when no K <= K_MAX meets SERIES_TOL or tau_max > SERIES_TAU_MAX); 1 = the caller forced
 // the path (NK_FORM_SERIES): K_MAX terms are used when the bound cannot be met
@@ -216,29 +190,6 @@ __device__ __forceinline__ void umma_f16_cg2(uint32_t d_tmem, uint64_t adesc, ui
         "}\n" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
-// arrives (once) on the barrier at this shared-memory offset in BOTH CTAs of the pair when the MMAs issued so far are done
-__device__ __forceinline__ void umma_commit_cg2(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
-                 "h"((uint16_t)3)
-                 : "memory");
-}
-// the shared::cluster address of `addr` (an address in this CTA's shared window) in the CTA of rank `rank`
-__device__ __forceinline__ uint32_t map_to_rank(uint32_t addr, uint32_t rank) {
-    uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
-    return r;
-}
-// TMA load of a CTA of the pair: the box lands in THIS CTA's shared memory, the bytes are counted on the leader's barrier
-__device__ __forceinline__ void tma_load_2d_cg2(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t leader_bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-        ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(leader_bar)
-        : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
-}
-
 template <int CG>
 __global__ void __launch_bounds__(ser::THREADS, 1)
 series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b,
@@ -613,16 +564,18 @@ SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chu
 }
 
 // per call, after launch_pack_product (Ttab, tau_max): choose K and write the table-row operand
+// before launch_pack_product: zero the control block that its row pass fills
+cudaError_t launch_series_ctl_reset(const SeriesWs& w, cudaStream_t st) {
+    return cudaMemsetAsync(w.ctl, 0, SER_CTL_WORDS * sizeof(unsigned), st);
+}
+
 cudaError_t launch_series_pack(const Geometry& g, const float* Ttab, const unsigned* taumax_bits, const SeriesWs& w,
                                bool force, cudaStream_t st) {
     cudaError_t e = series_init();
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(w.ctl, 0, SER_CTL_WORDS * sizeof(unsigned), st);
-    if (e != cudaSuccess) return e;
-    series_rowsum_kernel<<<g.n_rows, 256, 0, st>>>(Ttab, g.M_pad, g.M_eff, w.ctl);
     series_select_kernel<<<1, 1, 0, st>>>(w.ctl, taumax_bits, force ? 1 : 0);
     series_bpow_kernel<<<g.n_rows, 256, 0, st>>>(Ttab, g.M_pad, g.M_eff, w.ctl, w.Bp);
-    count_launch(3);
+    count_launch(2);
     return cudaGetLastError();
 }
 

@@ -283,12 +283,182 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
     }
 }
 
+// ---- the same contraction by CTA PAIRS (tcgen05 cta_group::2) ------------------------------------------------------
+// A pair of CTAs of one TPC owns 256 rows x 64 output columns: each CTA holds its 128 rows' A tile and HALF of the B
+// operand — rows [96 r, 96 r + 96) of the 192 digit rows (hi | mid | lo) x 64 columns, three TMA boxes of 32 rows — so
+// a stage is 28 KB instead of 40 and the digit planes cross L2 -> shared memory -> tensor core once per 256 rows.  What
+// bounded the single-CTA kernel was shared-memory bandwidth (40 KB of MMA reads + 40 KB of TMA writes = 625 cycles per k
+// block against 384 MMA cycles); here it is 28 + 28 KB.  The leader (rank 0) issues M = 256, N = 192,
+// K = 32 MMAs; both CTAs' loads count on the leader's `full` barrier, multicast commits free the stage and publish the
+// accumulators in both, and both CTAs' epilogue warps hand the accumulator set back on the leader's `tempty`.
+namespace tc2 {
+constexpr int STAGES = 6;
+constexpr int B_HALF = 96 * tc::BKB;                       // 12 KB
+constexpr int STAGE_BYTES = tc::A_BYTES + B_HALF;          // 28 KB
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256;
+constexpr uint32_t IDESC_I8 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)((3 * tc::BN) >> 3) << 17) | ((uint32_t)((2 * tc::BM) >> 4) << 24);
+}  // namespace tc2
+
+__device__ __forceinline__ void umma_i8_cg2(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                            uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::i8 [%0], %1, %2, %3, p;\n\t"
+        "}\n" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+__global__ void __launch_bounds__(tc::THREADS, 1)
+theta_tc2_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w, int64_t B,
+                 int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta, int accumulate,
+                 const float* __restrict__ scale, int scale_per_col, int n_tn, int n_tiles) {
+    using namespace tc;
+    constexpr int STAGES2 = tc2::STAGES, STAGE2 = tc2::STAGE_BYTES;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bars = smem_base + STAGES2 * STAGE2;
+    const uint32_t full0 = bars, empty0 = bars + 8 * STAGES2;
+    const uint32_t tfull0 = bars + 16 * STAGES2, tempty0 = tfull0 + 16;
+    const uint32_t tmem_slot = tempty0 + 16;
+    uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_kb = K_pad / BKB;
+    const uint32_t rank = cluster_ctarank();
+    const int unit = blockIdx.x / 2, n_units = gridDim.x / 2;
+    const uint32_t full_l = map_to_rank(full0, 0), tempty_l = map_to_rank(tempty0, 0);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES2; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, 1); }
+        for (int a = 0; a < 2; ++a) { mbar_init(tfull0 + 8 * a, 1); mbar_init(tempty0 + 8 * a, 256); }
+        mbar_fence_init();
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    cluster_sync_all();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===== TMA producer (each CTA: its A rows and its half of the digit rows) =====
+        if (lane == 0) {
+            int stage = 0; uint32_t parity = 1;
+            for (int t = unit; t < n_tiles; t += n_units) {
+                const int tm = t / n_tn;
+                const int m0 = (tm * 2 + (int)rank) * BM, n0 = (t - tm * n_tn) * BN;
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(empty0 + 8 * stage, parity);
+                    if (rank == 0) mbar_arrive_expect_tx(full0 + 8 * stage, 2 * STAGE2);
+                    const uint32_t dst = smem_base + stage * STAGE2;
+                    tma_load_2d_cg2(dst, &map_a, kb * BKB, m0, full_l + 8 * stage);
+#pragma unroll
+                    for (int bx = 0; bx < 3; ++bx) {       // digit row v = 96 rank + 32 bx .. + 31 of (hi | mid | lo) x 64
+                        const int v = 96 * (int)rank + 32 * bx;
+                        tma_load_2d_cg2(dst + A_BYTES + bx * 32 * BKB, &map_w, kb * BKB, (v >> 6) * M_eff + n0 + (v & 63),
+                                        full_l + 8 * stage);
+                    }
+                    if (++stage == STAGES2) { stage = 0; parity ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one thread of the leader) =====
+        if (lane == 0 && rank == 0) {
+            int stage = 0; uint32_t parity = 0;
+            int it = 0;
+            for (int t = unit; t < n_tiles; t += n_units, ++it) {
+                const int set = it & 1;
+                mbar_wait(tempty0 + 8 * set, ((it >> 1) & 1) ^ 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t acc = tmem_base + set * ACC_STRIDE;
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(full0 + 8 * stage, parity);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const uint32_t a_addr = smem_base + stage * STAGE2;
+#pragma unroll
+                    for (int k = 0; k < BKB / UMMA_KB; ++k) {
+                        const uint32_t koff = k * UMMA_KB;
+                        umma_i8_cg2(acc, make_sdesc(a_addr + koff), make_sdesc(a_addr + A_BYTES + koff), tc2::IDESC_I8,
+                                    (kb | k) ? 1u : 0u);
+                    }
+                    umma_commit_cg2(empty0 + 8 * stage);
+                    if (++stage == STAGES2) { stage = 0; parity ^= 1; }
+                }
+                umma_commit_cg2(tfull0 + 8 * set);
+            }
+        }
+    } else {
+        // ===== epilogue: warps 2..5 of each CTA, its own 128 rows =====
+        const int q = warp & 3;
+        const float qs0 = *scale;
+        int it = 0;
+        for (int t = unit; t < n_tiles; t += n_units, ++it) {
+            const int set = it & 1;
+            const int tm = t / n_tn;
+            const int n0 = (t - tm * n_tn) * BN;
+            const int64_t row = (int64_t)(tm * 2 + (int)rank) * BM + q * 32 + lane;
+            float* out = theta + row * M_eff + n0;
+            mbar_wait(tfull0 + 8 * set, (it >> 1) & 1);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll 1
+            for (int c0 = 0; c0 < BN; c0 += 32) {
+                float hi[32], mid[32], lo[32];
+                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + set * ACC_STRIDE + c0;
+                tmem_ld32(taddr, hi);
+                tmem_ld32(taddr + BN, mid);
+                tmem_ld32(taddr + 2 * BN, lo);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                if (c0 + 32 == BN) {
+                    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                    mbar_arrive_cluster(tempty_l + 8 * set);
+                }
+                if (row < B) {
+#pragma unroll
+                    for (int j = 0; j < 32; j += 4) {
+                        float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (bg != nullptr) bb = *reinterpret_cast<const float4*>(bg + n0 + c0 + j);
+                        float4 qs = make_float4(qs0, qs0, qs0, qs0);
+                        if (scale_per_col) qs = *reinterpret_cast<const float4*>(scale + n0 + c0 + j);
+                        if (accumulate) {
+                            const float4 old = *reinterpret_cast<const float4*>(out + c0 + j);
+                            bb.x += old.x; bb.y += old.y; bb.z += old.z; bb.w += old.w;
+                        }
+                        float4 o;
+                        auto comb = [&](int jj) -> float {
+                            const float h = (float)__float_as_int(hi[jj]), m = (float)__float_as_int(mid[jj]),
+                                        l = (float)__float_as_int(lo[jj]);
+                            return fmaf(h, 65536.f, fmaf(m, 256.f, l));
+                        };
+                        o.x = fmaf(qs.x, comb(j), bb.x); o.y = fmaf(qs.y, comb(j + 1), bb.y);
+                        o.z = fmaf(qs.z, comb(j + 2), bb.z); o.w = fmaf(qs.w, comb(j + 3), bb.w);
+                        __stcs(reinterpret_cast<float4*>(out + c0 + j), o);
+                    }
+                }
+            }
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == 1) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+    }
+}
+
 // ---- host side ---------------------------------------------------------------------------------------------
 static bool encode_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols, int box_rows);
 // One-time set-up is per DEVICE (function attributes, SM and cluster counts belong to the current device) and guarded
 // by a mutex: a process may drive several GPUs, and first calls may come from several host threads.
 namespace {
-struct TcDevice { bool ready = false; int num_sms = 148, cm = 1, cn = 1, max_clusters = 148; };
+struct TcDevice { bool ready = false; int num_sms = 148, cm = 1, cn = 1, max_clusters = 148, pairs = 0; };
 std::mutex g_tc_mutex;
 TcDevice g_tc_dev[NK_MAX_DEVICES];
 EncodeTiledFn g_encode = nullptr;
@@ -379,6 +549,21 @@ cudaError_t theta_tc_init() {
         if (n <= 0) n = g_num_sms;
     }
     g_max_clusters = n;
+    {   // CTA pairs for the cta_group::2 kernel
+        int np = 0;
+        if (cudaFuncSetAttribute((const void*)theta_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 tc2::SMEM_BYTES) == cudaSuccess) {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(2, 1, 1); cfg.blockDim = dim3(tc::THREADS, 1, 1); cfg.dynamicSmemBytes = tc2::SMEM_BYTES;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+            cfg.attrs = attr; cfg.numAttrs = 1;
+            if (cudaOccupancyMaxActiveClusters(&np, (const void*)theta_tc2_kernel, &cfg) != cudaSuccess) np = 0;
+        }
+        (void)cudaGetLastError();
+        tc_dev().pairs = np;
+    }
     tc_dev().ready = true;
     return cudaSuccess;
 }
@@ -388,6 +573,28 @@ static cudaError_t tc_gemm(const void* A, int64_t rows, const void* P, int cols,
     cudaError_t e = theta_tc_init();
     if (e != cudaSuccess) return e;
     CUtensorMap map_a, map_p;
+    if (tc_dev().pairs > 0 && rows > tc::BM) {            // CTA pairs whenever there are two row tiles
+        if (!encode_2d(&map_a, A, (uint64_t)rows, (uint64_t)ld, tc::BM)) return cudaErrorInvalidValue;
+        if (!encode_2d(&map_p, P, (uint64_t)3 * cols, (uint64_t)ld, 32)) return cudaErrorInvalidValue;
+        const float* scale2 = reinterpret_cast<const float*>((const int8_t*)P + (size_t)3 * cols * ld);
+        const int n_tn = cols / tc::BN;
+        const int64_t n_tiles = (rows + 2 * tc::BM - 1) / (2 * tc::BM) * n_tn;
+        if (n_tiles > 0x7fffffff) return cudaErrorInvalidValue;
+        const int units = (int)(n_tiles < tc_dev().pairs ? n_tiles : tc_dev().pairs);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(2 * units), 1, 1);
+        cfg.blockDim = dim3(tc::THREADS, 1, 1);
+        cfg.dynamicSmemBytes = tc2::SMEM_BYTES;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, theta_tc2_kernel, map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale2,
+                               scale_per_col, n_tn, (int)n_tiles);
+        count_launch();
+        return e != cudaSuccess ? e : cudaGetLastError();
+    }
     if (!encode_2d(&map_a, A, (uint64_t)rows, (uint64_t)ld, tc::BM / g_cn)) return cudaErrorInvalidValue;
     if (!encode_2d(&map_p, P, (uint64_t)3 * cols, (uint64_t)ld, tc::BN / g_cm)) return cudaErrorInvalidValue;
     const float* scale = reinterpret_cast<const float*>((const int8_t*)P + (size_t)3 * cols * ld);

@@ -125,3 +125,32 @@ def test_config5_full_batch_every_sample(nk, cfg5_full, form_name):
     assert abs(st[0] - m[0]) <= 1e-4 * abs(m[0]) + 1e-6 and st[3] == p.n_samples
     assert abs(st[2] - m[2]) <= 1e-3 * m[2]
     print(f"config 5, all {p.n_samples} samples, {form_name}: max rel err E_loc {worst:.2e}")
+
+
+@pytest.mark.parametrize("cfg,n,chunk", [(5, 700, 256), (2, 300, 128), (4, 200, 0)])
+def test_plan_replay_equals_the_eager_call(nk, cfg, n, chunk):
+    """nk_local_energy_plan_*: the captured graph replays the same kernels — bit-identical outputs, new CONTENTS of the
+    bound buffers are picked up (the form is still chosen on the device), and the flag that synchronises is refused."""
+    p = inp.make_config(cfg, n_samples=n)
+    dt = nk.NK_C64 if p.complex_params else nk.NK_F32
+    op = nk.Operator.from_problem(p)
+    sig, W, a, b = dev(p.sigma), dev(p.W), dev(p.a), dev(p.b)
+    plan = nk.LocalEnergyPlan(op, n, p.n_sites, p.n_hidden, dt, chunk)
+    e0, lp0, st0 = (t.clone() for t in plan.run(sig, W, a, b))
+    e1, lp1, st1 = (t.clone() for t in plan.run_graph(sig, W, a, b))
+    torch.cuda.synchronize()
+    assert torch.equal(e0, e1) and torch.equal(lp0, lp1) and torch.equal(st0, st1)
+    scale = 6.0 if cfg == 5 else 1.5                   # same addresses, new parameters (config 5: the gate now closes)
+    W.mul_(scale)
+    e2, _, _ = (t.clone() for t in plan.run_graph(sig, W, a, b))
+    e3, _, _ = (t.clone() for t in plan.run(sig, W, a, b))
+    torch.cuda.synchronize()
+    assert torch.equal(e2, e3) and not torch.equal(e2, e1)
+    p.W = (p.W * scale).astype(p.W.dtype)
+    rows = list(range(0, n, max(1, n // 24)))
+    assert_eloc(e2.cpu().numpy()[rows], run_oracle(p, rows=rows)[0])
+    bad = nk.LocalEnergyPlan(op, n, p.n_sites, p.n_hidden, dt, chunk, flags=nk.NK_CHECK_SPINS)
+    with pytest.raises(nk.NkError):
+        bad.run_graph(sig, W, a, b)
+    plan.close_plan()
+    op.close()

@@ -170,12 +170,13 @@ def test_bench_gpus_flag_spawns_one_rank_per_gpu():
     spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(root, "bench.py"))
     bench = importlib.util.module_from_spec(spec)
     spec.loader.exec_module(bench)
-    args = argparse.Namespace(gpus=8, steps=7, warmup=3, config=5, impl="ours", no_extras=True)
+    args = argparse.Namespace(gpus=8, steps=7, warmup=3, config=5, impl="ours", no_extras=True, call="plan")
     cmd = bench.spawn_command(args, port=29511)
     assert cmd[1:3] == ["-m", "torch.distributed.run"] and "--nproc-per-node=8" in cmd and "--nnodes=1" in cmd
     assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29511"
     tail = cmd[cmd.index(os.path.join(root, "bench.py")) + 1:]
-    assert tail == ["--gpus", "8", "--steps", "7", "--warmup", "3", "--config", "5", "--impl", "ours", "--no-extras"]
+    assert tail == ["--gpus", "8", "--steps", "7", "--warmup", "3", "--config", "5", "--impl", "ours", "--call", "plan",
+                    "--no-extras"]
 
 
 def test_stats_combine_c_abi_rejects_bad_arguments():
