@@ -150,6 +150,7 @@ struct ElocWs {
     uint16_t *A, *Ws;
     unsigned *absmax, *taumax;                        // taumax: max |tanh delta| of Ttab as float bits (the form gate)
     RowInfo* rows;
+    int64_t unit_rows;                                // rows of theta / A: one chunk, or one group of chunks (series form)
     bool has_series;                                  // the tensor-core series form is possible for these sizes
     SeriesWs ser;
     size_t bytes;
@@ -163,13 +164,15 @@ static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk, int dtype, 
     w.Dtab = c.take<float>((size_t)g.n_rows_pad * g.M_eff);
     w.rows = c.take<RowInfo>(g.n_rows_pad);
     w.has_series = series_possible(g, dtype);
-    w.theta = c.take<float>((size_t)chunk * g.M_eff);
     w.Ws = c.take<uint16_t>((size_t)3 * g.M_eff * g.K_pad);
-    w.A = c.take<uint16_t>((size_t)chunk * g.K_pad);
     w.absmax = c.take<unsigned>(1);
     w.taumax = c.take<unsigned>(1);
     w.Ttab = c.take<float>((size_t)g.n_rows_pad * g.M_eff);
     if (w.has_series) w.ser = carve_series(c.base, &c.off, g, chunk, B);
+    // the unit the chunk loop works in: a chunk, or (series form possible) the group of chunks one tensor-core launch covers
+    w.unit_rows = w.has_series ? w.ser.group_rows : chunk;
+    w.theta = c.take<float>((size_t)w.unit_rows * g.M_eff);
+    w.A = c.take<uint16_t>((size_t)w.unit_rows * g.K_pad);
     w.bytes = c.off;
     return w;
 }
@@ -790,24 +793,29 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
         NK_CUDA(cudaEventRecord(tl_pipe_events[0], st));              // parameters packed; earlier work on `stream` done
         NK_CUDA(cudaStreamWaitEvent(ps, tl_pipe_events[0], 0));
     }
-    const int64_t group_rows = series ? w.ser.group_rows : chunk;
+    // Where the series form is possible the whole group is the unit of work for every kernel (theta, ln psi, stand-ins):
+    // four launches of each per step at config 5 instead of sixteen (also when a SIMT form is forced there).
+    const int64_t group_rows = w.unit_rows;
+    const int64_t copy_chunk = chunk;                                 // granularity of the host path's arrival events
     int64_t gi = 0;
     for (int64_t g0 = 0; g0 < B; g0 += group_rows, ++gi) {
         const int64_t gn = (B - g0 < group_rows) ? (B - g0) : group_rows;
         const int set = (series && w.ser.n_sets == 2) ? (int)(gi & 1) : 0;
         cudaEvent_t ev_prep = tl_pipe_events[1 + set], ev_done = tl_pipe_events[3 + set];
         if (pipelined && gi >= 2) NK_CUDA(cudaStreamWaitEvent(ps, ev_done, 0));    // group G - 2 no longer reads this set
-        for (int64_t s0 = g0; s0 < g0 + gn; s0 += chunk) {
-            const int64_t nb = (g0 + gn - s0 < chunk) ? (g0 + gn - s0) : chunk;
+        {
+            const int64_t s0 = g0, nb = gn;
             const int8_t* sg = sigma + s0 * N;
-            if (tl_chunk_ready != nullptr) NK_CUDA(cudaStreamWaitEvent(ps, (*tl_chunk_ready)[(size_t)(s0 / chunk)], 0));
+            if (tl_chunk_ready != nullptr)                            // every chunk of the group has arrived
+                for (int64_t c0 = s0; c0 < s0 + nb; c0 += copy_chunk)
+                    NK_CUDA(cudaStreamWaitEvent(ps, (*tl_chunk_ready)[(size_t)(c0 / copy_chunk)], 0));
             {
                 Scope sc(PH_GEMM, ps);
                 NK_CUDA(run_theta(g, sg, nb, w.Wg, w.bg, w.Ws, w.A, w.theta, ps));
             }
             if (logpsi_out || series) {        // ln psi and, in the same pass over theta, the series form's operand rows
                 Scope sc(PH_LOGPSI, ps);
-                uint16_t* ap = series ? w.ser.Ap[set] + (size_t)(s0 - g0) * SERIES_SEGS * g.M_pad : nullptr;
+                uint16_t* ap = series ? w.ser.Ap[set] : nullptr;
                 NK_CUDA(launch_logpsi(sg, nb, g, dtype, w.theta, a, logpsi_out ? (uint8_t*)logpsi_out + s0 * esz : nullptr,
                                       false, nullptr, ps, series ? w.ser.ctl : nullptr, ap));
             }

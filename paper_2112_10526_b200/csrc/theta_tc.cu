@@ -41,7 +41,7 @@ constexpr int BM = 128, BN = 64, BKB = 128, STAGES = 4, UMMA_KB = 32;   // BKB: 
 constexpr int A_BYTES = BM * BKB;                         // 16 KB: 128 rows x 128 B
 constexpr int P_BYTES = BN * BKB;                         //  8 KB: one digit plane, 64 rows x 128 B
 constexpr int STAGE_BYTES = A_BYTES + 3 * P_BYTES;        // sigma + hi + mid + lo
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment*/ + 256 /*barriers*/;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * 128 * 128 /*output staging*/ + 1024 /*alignment*/ + 256 /*barriers*/;
 constexpr int THREADS = 192;
 constexpr uint32_t TMEM_COLS = 512;                       // two accumulator sets: D_hi, D_mid, D_lo at +0, +64, +128
 constexpr uint32_t ACC_STRIDE = 256;                      // of column 0 and of column 256
@@ -115,6 +115,80 @@ __global__ void sigma_pad_i8_kernel(const int8_t* __restrict__ sigma, int64_t B,
     }
 }
 
+// ---- epilogue of one 128 x 64 output tile (shared by the three kernels below) -----------------------------------------
+// out (+)= q (D2 2^16 + D1 2^8 + D0) + bias.  The four epilogue warps (TMEM lane quarter q each) read the three int32
+// accumulators, combine them in fp32, write the tile into a 128B-swizzled staging buffer (two boxes of 128 rows x 32
+// floats: a thread owns a row, so its eight 16-B chunks per box go to chunk ^ (row & 7) — conflict-free quarter-warps)
+// and ONE thread hands it to the TMA engine: a bulk tensor store, or a bulk tensor reduce-add when the product
+// accumulates over chunks.  (Until round 2 every thread stored its own row with 16-B STG 8 KB apart: the epilogue, not
+// the MMAs, bounded theta-shaped products — 9 k cycles per tile against 3 k of MMAs.)  Rows beyond the operand are
+// clipped by the tensor map.  `arrive` hands the accumulator set back to the MMA issuer.
+constexpr int TC_STAGE_OUT = 2 * 128 * 128;                // 32 KB staging tile
+template <typename Arrive>
+__device__ __forceinline__ void tc_epilogue_tile(uint32_t tmem_acc, int q, int lane, bool elected, uint32_t stage_u32,
+                                                 uint8_t* stage_ptr, const CUtensorMap* map_out, int row0, int n0,
+                                                 const float* __restrict__ bg, const float* __restrict__ scale,
+                                                 int scale_per_col, float qs0, int accumulate, Arrive arrive) {
+    using namespace tc;
+    const int r = q * 32 + lane;
+#pragma unroll 1
+    for (int c0 = 0; c0 < BN; c0 += 32) {
+        // bias and scale of these 32 columns first: their latency runs under the TMEM loads
+        float4 bb[8], qs[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            bb[j] = bg != nullptr ? __ldg(reinterpret_cast<const float4*>(bg + n0 + c0) + j) : make_float4(0.f, 0.f, 0.f, 0.f);
+            qs[j] = scale_per_col ? __ldg(reinterpret_cast<const float4*>(scale + n0 + c0) + j)
+                                  : make_float4(qs0, qs0, qs0, qs0);
+        }
+        float hi[32], mid[32], lo[32];
+        const uint32_t taddr = tmem_acc + ((uint32_t)(q * 32) << 16) + c0;
+        tmem_ld32(taddr, hi);
+        tmem_ld32(taddr + BN, mid);
+        tmem_ld32(taddr + 2 * BN, lo);
+        // the two halves of the staging tile alternate: the store of this half issued for the previous tile has finished
+        // READING it (at most one newer store — the other half's — may still be in flight)
+        if (elected) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        if (c0 + 32 == BN) {                               // everything is in registers: hand the set back to the MMAs
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            arrive();
+        }
+        const int bx = c0 >> 5;
+        uint8_t* box = stage_ptr + bx * (128 * 128) + r * 128;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            float4 o;
+            auto comb = [&](int jj) -> float {             // exact ints below 2^24 each
+                const float h = (float)__float_as_int(hi[jj]), m = (float)__float_as_int(mid[jj]),
+                            l = (float)__float_as_int(lo[jj]);
+                return fmaf(h, 65536.f, fmaf(m, 256.f, l));
+            };
+            o.x = fmaf(qs[j].x, comb(4 * j), bb[j].x); o.y = fmaf(qs[j].y, comb(4 * j + 1), bb[j].y);
+            o.z = fmaf(qs[j].z, comb(4 * j + 2), bb[j].z); o.w = fmaf(qs[j].w, comb(4 * j + 3), bb[j].w);
+            *reinterpret_cast<float4*>(box + ((j ^ (r & 7)) << 4)) = o;
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy writes -> visible to the TMA engine
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (elected) {
+            if (accumulate)
+                asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group [%0, {%1, %2}], [%3];"
+                             ::"l"(map_out), "r"(n0 + c0), "r"(row0), "r"(stage_u32 + bx * (128 * 128))
+                             : "memory");
+            else
+                asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%1, %2}], [%3];"
+                             ::"l"(map_out), "r"(n0 + c0), "r"(row0), "r"(stage_u32 + bx * (128 * 128))
+                             : "memory");
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+    }
+}
+// before the CTA exits: the last store has read the staging buffer
+__device__ __forceinline__ void tc_epilogue_drain(bool elected) {
+    if (elected) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+
 // ---- the GEMM ---------------------------------------------------------------------------------------------
 // int8 operands (128 elements per 128-B swizzle row, so K_pad / 128 k blocks), int32 accumulators,
 // out (+)= q (D2 2^16 + D1 2^8 + D0) + bias with the scale q read from `scale`.
@@ -124,14 +198,15 @@ __global__ void sigma_pad_i8_kernel(const int8_t* __restrict__ sigma, int64_t B,
 // (itself included), and the MMA commit that frees the stage arrives on the `empty` barrier of every one of them.
 template <int CM, int CN>
 __global__ void __launch_bounds__(tc::THREADS, 1)
-theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w, int64_t B,
+theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w,
+                const __grid_constant__ CUtensorMap map_out, int64_t B,
                 int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta, int accumulate,
                 const float* __restrict__ scale, int scale_per_col, int n_sup_n, int n_sup) {
     using namespace tc;
     constexpr int CS = CM * CN;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;            // SWIZZLE_128B needs 1024 B
-    const uint32_t bars = smem_base + STAGES * STAGE_BYTES;
+    const uint32_t bars = smem_base + STAGES * STAGE_BYTES + TC_STAGE_OUT;       // ring | output staging tile | barriers
     const uint32_t full0 = bars, empty0 = bars + 8 * STAGES;                     // smem ring
     const uint32_t tfull0 = bars + 16 * STAGES, tempty0 = tfull0 + 16;          // the two accumulator sets
     const uint32_t tmem_slot = tempty0 + 16;
@@ -228,51 +303,21 @@ theta_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
         // ===== epilogue: warps 2..5, TMEM lane quarter = warp % 4 =====
         const int q = warp & 3;
         const float qs0 = *scale;                         // one scale, or (scale_per_col) one per output column
+        const bool elected = warp == 2 && lane == 0;
+        const uint32_t stage_u32 = smem_base + STAGES * STAGE_BYTES;
+        uint8_t* stage_ptr = smem_raw + (stage_u32 - smem_u32(smem_raw));
         int it = 0;
         for (int sup = cluster_id; sup < n_sup; sup += n_clusters, ++it) {
             const int set = it & 1;
             const int sm = sup / n_sup_n;
             const int n0 = ((sup - sm * n_sup_n) * CN + rn) * BN;
-            const int64_t row = (int64_t)(sm * CM + rm) * BM + q * 32 + lane;
-            float* out = theta + row * M_eff + n0;
             mbar_wait(tfull0 + 8 * set, (it >> 1) & 1);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-#pragma unroll 1
-            for (int c0 = 0; c0 < BN; c0 += 32) {
-                float hi[32], mid[32], lo[32];
-                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + set * ACC_STRIDE + c0;
-                tmem_ld32(taddr, hi);
-                tmem_ld32(taddr + BN, mid);
-                tmem_ld32(taddr + 2 * BN, lo);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                if (c0 + 32 == BN) {                       // everything is in registers: hand the set back to the MMAs
-                    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                    mbar_arrive(tempty0 + 8 * set);
-                }
-                if (row < B) {
-#pragma unroll
-                    for (int j = 0; j < 32; j += 4) {
-                        float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (bg != nullptr) bb = *reinterpret_cast<const float4*>(bg + n0 + c0 + j);
-                        float4 qs = make_float4(qs0, qs0, qs0, qs0);
-                        if (scale_per_col) qs = *reinterpret_cast<const float4*>(scale + n0 + c0 + j);
-                        if (accumulate) {                  // out += D (the gradient contraction runs over chunks)
-                            const float4 old = *reinterpret_cast<const float4*>(out + c0 + j);
-                            bb.x += old.x; bb.y += old.y; bb.z += old.z; bb.w += old.w;
-                        }
-                        float4 o;
-                        auto comb = [&](int jj) -> float {                      // exact ints below 2^24 each
-                            const float h = (float)__float_as_int(hi[jj]), m = (float)__float_as_int(mid[jj]),
-                                        l = (float)__float_as_int(lo[jj]);
-                            return fmaf(h, 65536.f, fmaf(m, 256.f, l));
-                        };
-                        o.x = fmaf(qs.x, comb(j), bb.x); o.y = fmaf(qs.y, comb(j + 1), bb.y);
-                        o.z = fmaf(qs.z, comb(j + 2), bb.z); o.w = fmaf(qs.w, comb(j + 3), bb.w);
-                        __stcs(reinterpret_cast<float4*>(out + c0 + j), o);
-                    }
-                }
-            }
+            tc_epilogue_tile(tmem_base + set * ACC_STRIDE, q, lane, elected, stage_u32, stage_ptr, &map_out,
+                             (sm * CM + rm) * BM, n0, bg, scale, scale_per_col, qs0, accumulate,
+                             [&]() { mbar_arrive(tempty0 + 8 * set); });
         }
+        tc_epilogue_drain(elected);
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
@@ -295,7 +340,7 @@ namespace tc2 {
 constexpr int STAGES = 6;
 constexpr int B_HALF = 96 * tc::BKB;                       // 12 KB
 constexpr int STAGE_BYTES = tc::A_BYTES + B_HALF;          // 28 KB
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * 128 * 128 + 1024 + 256;
 constexpr uint32_t IDESC_I8 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)((3 * tc::BN) >> 3) << 17) | ((uint32_t)((2 * tc::BM) >> 4) << 24);
 }  // namespace tc2
 
@@ -311,14 +356,15 @@ __device__ __forceinline__ void umma_i8_cg2(uint32_t d_tmem, uint64_t adesc, uin
 }
 
 __global__ void __launch_bounds__(tc::THREADS, 1)
-theta_tc2_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w, int64_t B,
+theta_tc2_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w,
+                 const __grid_constant__ CUtensorMap map_out, int64_t B,
                  int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta, int accumulate,
                  const float* __restrict__ scale, int scale_per_col, int n_tn, int n_tiles) {
     using namespace tc;
     constexpr int STAGES2 = tc2::STAGES, STAGE2 = tc2::STAGE_BYTES;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bars = smem_base + STAGES2 * STAGE2;
+    const uint32_t bars = smem_base + STAGES2 * STAGE2 + TC_STAGE_OUT;
     const uint32_t full0 = bars, empty0 = bars + 8 * STAGES2;
     const uint32_t tfull0 = bars + 16 * STAGES2, tempty0 = tfull0 + 16;
     const uint32_t tmem_slot = tempty0 + 16;
@@ -398,51 +444,171 @@ theta_tc2_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constan
         // ===== epilogue: warps 2..5 of each CTA, its own 128 rows =====
         const int q = warp & 3;
         const float qs0 = *scale;
+        const bool elected = warp == 2 && lane == 0;
+        const uint32_t stage_u32 = smem_base + STAGES2 * STAGE2;
+        uint8_t* stage_ptr = smem_raw + (stage_u32 - smem_u32(smem_raw));
         int it = 0;
         for (int t = unit; t < n_tiles; t += n_units, ++it) {
             const int set = it & 1;
             const int tm = t / n_tn;
             const int n0 = (t - tm * n_tn) * BN;
-            const int64_t row = (int64_t)(tm * 2 + (int)rank) * BM + q * 32 + lane;
-            float* out = theta + row * M_eff + n0;
             mbar_wait(tfull0 + 8 * set, (it >> 1) & 1);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-#pragma unroll 1
-            for (int c0 = 0; c0 < BN; c0 += 32) {
-                float hi[32], mid[32], lo[32];
-                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + set * ACC_STRIDE + c0;
-                tmem_ld32(taddr, hi);
-                tmem_ld32(taddr + BN, mid);
-                tmem_ld32(taddr + 2 * BN, lo);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                if (c0 + 32 == BN) {
-                    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                    mbar_arrive_cluster(tempty_l + 8 * set);
+            tc_epilogue_tile(tmem_base + set * ACC_STRIDE, q, lane, elected, stage_u32, stage_ptr, &map_out,
+                             (tm * 2 + (int)rank) * BM, n0, bg, scale, scale_per_col, qs0, accumulate,
+                             [&]() { mbar_arrive_cluster(tempty_l + 8 * set); });
+        }
+        tc_epilogue_drain(elected);
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == 1) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+    }
+}
+
+// ---- theta-shaped products (k extent <= 1024 bytes): CTA pairs with the A operand RESIDENT in shared memory ----------
+// theta = sigma W^T has a short k extent (N <= 1024 spins = 8 k blocks) and many output columns, so the streaming kernels
+// above read every spin tile once per 64-column tile — 32 times at M = 2048 — and are bound by L2 -> shared-memory
+// traffic (ncu: L2 63 %, tensor pipe 46 % on the 65536 x 2048 x 1024 launch).  Here a CTA pair loads the spins of its
+// 256 rows ONCE (n_kb x 16 KB per CTA, kept for all the column tiles of its work range) and streams only its half of the
+// digit rows (12 KB per k block): per k block a CTA writes 12 KB and the MMAs read 28 KB = 312 shared-memory cycles
+// against 384 MMA cycles, and the pair pulls 24 KB instead of 56 KB through L2.  Work = (row-pair tile, column tile)
+// items, column tiles fastest; pair u takes a contiguous range of them (the spins are reloaded when the row tile changes).
+namespace tc3 {
+constexpr int MAX_KB = 8;                                  // resident k blocks: K_pad <= 1024
+constexpr int STAGES = 4;
+constexpr int B_HALF = 96 * tc::BKB;                       // 12 KB
+constexpr int SMEM_BYTES = MAX_KB * tc::A_BYTES + STAGES * B_HALF + 2 * 128 * 128 + 1024 + 256;
+}  // namespace tc3
+
+__global__ void __launch_bounds__(tc::THREADS, 1)
+theta_tc3_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_w,
+                 const __grid_constant__ CUtensorMap map_out, int64_t B,
+                 int M_eff, int K_pad, const float* __restrict__ bg, float* __restrict__ theta, int accumulate,
+                 const float* __restrict__ scale, int scale_per_col, int n_tn, int n_items, int per_unit) {
+    using namespace tc;
+    constexpr int STG = tc3::STAGES, BH = tc3::B_HALF;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t b_ring = smem_base + tc3::MAX_KB * A_BYTES;
+    const uint32_t bars = b_ring + STG * BH + TC_STAGE_OUT;
+    const uint32_t full0 = bars, empty0 = bars + 8 * STG;
+    const uint32_t tfull0 = bars + 16 * STG, tempty0 = tfull0 + 16;
+    const uint32_t afull = tempty0 + 16, aempty = afull + 8;
+    const uint32_t tmem_slot = aempty + 8;
+    uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_kb = K_pad / BKB;
+    const uint32_t rank = cluster_ctarank();
+    const int unit = blockIdx.x / 2;
+    const int item_lo = unit * per_unit, item_hi = min(n_items, item_lo + per_unit);
+    const uint32_t full_l = map_to_rank(full0, 0), tempty_l = map_to_rank(tempty0, 0), afull_l = map_to_rank(afull, 0);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STG; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, 1); }
+        for (int a = 0; a < 2; ++a) { mbar_init(tfull0 + 8 * a, 1); mbar_init(tempty0 + 8 * a, 256); }
+        mbar_init(afull, 1);
+        mbar_init(aempty, 1);
+        mbar_fence_init();
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    cluster_sync_all();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            int stage = 0; uint32_t parity = 1, a_parity = 1;
+            int cur_tm = -1;
+            for (int it = item_lo; it < item_hi; ++it) {
+                const int tm = it / n_tn;
+                const int n0 = (it - tm * n_tn) * BN;
+                if (tm != cur_tm) {                        // the spins of this pair's 256 rows, once per row tile
+                    cur_tm = tm;
+                    mbar_wait(aempty, a_parity);
+                    a_parity ^= 1;
+                    if (rank == 0) mbar_arrive_expect_tx(afull, 2 * n_kb * A_BYTES);
+                    const int m0 = (tm * 2 + (int)rank) * BM;
+                    for (int kb = 0; kb < n_kb; ++kb)
+                        tma_load_2d_cg2(smem_base + kb * A_BYTES, &map_a, kb * BKB, m0, afull_l);
                 }
-                if (row < B) {
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(empty0 + 8 * stage, parity);
+                    if (rank == 0) mbar_arrive_expect_tx(full0 + 8 * stage, 2 * BH);
+                    const uint32_t dst = b_ring + stage * BH;
 #pragma unroll
-                    for (int j = 0; j < 32; j += 4) {
-                        float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (bg != nullptr) bb = *reinterpret_cast<const float4*>(bg + n0 + c0 + j);
-                        float4 qs = make_float4(qs0, qs0, qs0, qs0);
-                        if (scale_per_col) qs = *reinterpret_cast<const float4*>(scale + n0 + c0 + j);
-                        if (accumulate) {
-                            const float4 old = *reinterpret_cast<const float4*>(out + c0 + j);
-                            bb.x += old.x; bb.y += old.y; bb.z += old.z; bb.w += old.w;
-                        }
-                        float4 o;
-                        auto comb = [&](int jj) -> float {
-                            const float h = (float)__float_as_int(hi[jj]), m = (float)__float_as_int(mid[jj]),
-                                        l = (float)__float_as_int(lo[jj]);
-                            return fmaf(h, 65536.f, fmaf(m, 256.f, l));
-                        };
-                        o.x = fmaf(qs.x, comb(j), bb.x); o.y = fmaf(qs.y, comb(j + 1), bb.y);
-                        o.z = fmaf(qs.z, comb(j + 2), bb.z); o.w = fmaf(qs.w, comb(j + 3), bb.w);
-                        __stcs(reinterpret_cast<float4*>(out + c0 + j), o);
+                    for (int bx = 0; bx < 3; ++bx) {       // digit row v = 96 rank + 32 bx .. + 31 of (hi | mid | lo) x 64
+                        const int v = 96 * (int)rank + 32 * bx;
+                        tma_load_2d_cg2(dst + bx * 32 * BKB, &map_w, kb * BKB, (v >> 6) * M_eff + n0 + (v & 63),
+                                        full_l + 8 * stage);
                     }
+                    if (++stage == STG) { stage = 0; parity ^= 1; }
                 }
             }
         }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one thread of the leader) =====
+        if (lane == 0 && rank == 0) {
+            int stage = 0; uint32_t parity = 0, a_parity = 0;
+            int cur_tm = -1, n = 0;
+            for (int it = item_lo; it < item_hi; ++it, ++n) {
+                const int tm = it / n_tn;
+                if (tm != cur_tm) {
+                    cur_tm = tm;
+                    mbar_wait(afull, a_parity);
+                    a_parity ^= 1;
+                }
+                const int set = n & 1;
+                mbar_wait(tempty0 + 8 * set, ((n >> 1) & 1) ^ 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t acc = tmem_base + set * ACC_STRIDE;
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(full0 + 8 * stage, parity);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const uint32_t a_addr = smem_base + kb * A_BYTES, b_addr = b_ring + stage * BH;
+#pragma unroll
+                    for (int k = 0; k < BKB / UMMA_KB; ++k) {
+                        const uint32_t koff = k * UMMA_KB;
+                        umma_i8_cg2(acc, make_sdesc(a_addr + koff), make_sdesc(b_addr + koff), tc2::IDESC_I8,
+                                    (kb | k) ? 1u : 0u);
+                    }
+                    umma_commit_cg2(empty0 + 8 * stage);
+                    if (++stage == STG) { stage = 0; parity ^= 1; }
+                }
+                umma_commit_cg2(tfull0 + 8 * set);
+                if (it + 1 == item_hi || (it + 1) / n_tn != tm) umma_commit_cg2(aempty);   // the spins may be replaced
+            }
+        }
+    } else {
+        // ===== epilogue: warps 2..5 of each CTA, its own 128 rows =====
+        const int q = warp & 3;
+        const float qs0 = *scale;
+        const bool elected = warp == 2 && lane == 0;
+        const uint32_t stage_u32 = b_ring + STG * BH;
+        uint8_t* stage_ptr = smem_raw + (stage_u32 - smem_u32(smem_raw));
+        int n = 0;
+        for (int it = item_lo; it < item_hi; ++it, ++n) {
+            const int set = n & 1;
+            const int tm = it / n_tn;
+            const int n0 = (it - tm * n_tn) * BN;
+            mbar_wait(tfull0 + 8 * set, (n >> 1) & 1);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            tc_epilogue_tile(tmem_base + set * ACC_STRIDE, q, lane, elected, stage_u32, stage_ptr, &map_out,
+                             (tm * 2 + (int)rank) * BM, n0, bg, scale, scale_per_col, qs0, accumulate,
+                             [&]() { mbar_arrive_cluster(tempty_l + 8 * set); });
+        }
+        tc_epilogue_drain(elected);
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
@@ -498,7 +664,8 @@ static cudaError_t tc_prepare(int* max_clusters) {
 }
 
 template <int CM, int CN>
-static cudaError_t tc_launch(const CUtensorMap& map_a, const CUtensorMap& map_w, int64_t rows, int cols, int k_len,
+static cudaError_t tc_launch(const CUtensorMap& map_a, const CUtensorMap& map_w, const CUtensorMap& map_out,
+                             int64_t rows, int cols, int k_len,
                              const float* bg, float* out, int accumulate, const float* scale, int scale_per_col,
                              cudaStream_t st) {
     const int n_sup_n = cols / (tc::BN * CN);
@@ -514,7 +681,7 @@ static cudaError_t tc_launch(const CUtensorMap& map_a, const CUtensorMap& map_w,
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CM * CN; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, theta_tc_kernel<CM, CN>, map_a, map_w, rows, cols, k_len, bg, out, accumulate, scale,
+    return cudaLaunchKernelEx(&cfg, theta_tc_kernel<CM, CN>, map_a, map_w, map_out, rows, cols, k_len, bg, out, accumulate, scale,
                               scale_per_col, n_sup_n, (int)n_sup);
 }
 
@@ -552,7 +719,9 @@ cudaError_t theta_tc_init() {
     {   // CTA pairs for the cta_group::2 kernel
         int np = 0;
         if (cudaFuncSetAttribute((const void*)theta_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 tc2::SMEM_BYTES) == cudaSuccess) {
+                                 tc2::SMEM_BYTES) == cudaSuccess &&
+            cudaFuncSetAttribute((const void*)theta_tc3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 tc3::SMEM_BYTES) == cudaSuccess) {
             cudaLaunchConfig_t cfg = {};
             cfg.gridDim = dim3(2, 1, 1); cfg.blockDim = dim3(tc::THREADS, 1, 1); cfg.dynamicSmemBytes = tc2::SMEM_BYTES;
             cudaLaunchAttribute attr[1];
@@ -572,8 +741,21 @@ static cudaError_t tc_gemm(const void* A, int64_t rows, const void* P, int cols,
                            float* out, int accumulate, int scale_per_col, cudaStream_t st) {
     cudaError_t e = theta_tc_init();
     if (e != cudaSuccess) return e;
-    CUtensorMap map_a, map_p;
-    if (tc_dev().pairs > 0 && rows > tc::BM) {            // CTA pairs whenever there are two row tiles
+    CUtensorMap map_a, map_p, map_out;
+    {   // fp32 output [rows][cols], box = 128 rows x 32 floats (128 B), 128B swizzle: the epilogue's staging layout
+        const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+        const cuuint64_t strides[1] = {(cuuint64_t)cols * 4};
+        const cuuint32_t box[2] = {32, 128};
+        const cuuint32_t estr[2] = {1, 1};
+        if (g_encode(&map_out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, out, dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return cudaErrorInvalidValue;
+    }
+    // CTA pairs (cta_group::2) whenever there are two row tiles: the resident-A kernel for short k extents (theta-shaped
+    // products), the streaming one for long ones (the contractions over samples); the single-CTA cluster kernel otherwise
+    const bool resident = k_len <= tc3::MAX_KB * tc::BKB;
+    if (tc_dev().pairs > 0 && rows > tc::BM && (resident || k_len >= 4096)) {
         if (!encode_2d(&map_a, A, (uint64_t)rows, (uint64_t)ld, tc::BM)) return cudaErrorInvalidValue;
         if (!encode_2d(&map_p, P, (uint64_t)3 * cols, (uint64_t)ld, 32)) return cudaErrorInvalidValue;
         const float* scale2 = reinterpret_cast<const float*>((const int8_t*)P + (size_t)3 * cols * ld);
@@ -584,25 +766,31 @@ static cudaError_t tc_gemm(const void* A, int64_t rows, const void* P, int cols,
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3((unsigned)(2 * units), 1, 1);
         cfg.blockDim = dim3(tc::THREADS, 1, 1);
-        cfg.dynamicSmemBytes = tc2::SMEM_BYTES;
+        cfg.dynamicSmemBytes = resident ? tc3::SMEM_BYTES : tc2::SMEM_BYTES;
         cfg.stream = st;
         cudaLaunchAttribute attr[1];
         attr[0].id = cudaLaunchAttributeClusterDimension;
         attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr; cfg.numAttrs = 1;
-        e = cudaLaunchKernelEx(&cfg, theta_tc2_kernel, map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale2,
-                               scale_per_col, n_tn, (int)n_tiles);
+        if (resident) {
+            const int per_unit = (int)((n_tiles + units - 1) / units);
+            e = cudaLaunchKernelEx(&cfg, theta_tc3_kernel, map_a, map_p, map_out, rows, cols, k_len, bg, out, accumulate, scale2,
+                                   scale_per_col, n_tn, (int)n_tiles, per_unit);
+        } else {
+            e = cudaLaunchKernelEx(&cfg, theta_tc2_kernel, map_a, map_p, map_out, rows, cols, k_len, bg, out, accumulate, scale2,
+                                   scale_per_col, n_tn, (int)n_tiles);
+        }
         count_launch();
         return e != cudaSuccess ? e : cudaGetLastError();
     }
     if (!encode_2d(&map_a, A, (uint64_t)rows, (uint64_t)ld, tc::BM / g_cn)) return cudaErrorInvalidValue;
     if (!encode_2d(&map_p, P, (uint64_t)3 * cols, (uint64_t)ld, tc::BN / g_cm)) return cudaErrorInvalidValue;
     const float* scale = reinterpret_cast<const float*>((const int8_t*)P + (size_t)3 * cols * ld);
-    if (g_cm == 4 && g_cn == 2) e = tc_launch<4, 2>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
-    else if (g_cm == 4) e = tc_launch<4, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
-    else if (g_cm == 2 && g_cn == 2) e = tc_launch<2, 2>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
-    else if (g_cm == 2) e = tc_launch<2, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
-    else e = tc_launch<1, 1>(map_a, map_p, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
+    if (g_cm == 4 && g_cn == 2) e = tc_launch<4, 2>(map_a, map_p, map_out, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
+    else if (g_cm == 4) e = tc_launch<4, 1>(map_a, map_p, map_out, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
+    else if (g_cm == 2 && g_cn == 2) e = tc_launch<2, 2>(map_a, map_p, map_out, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
+    else if (g_cm == 2) e = tc_launch<2, 1>(map_a, map_p, map_out, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
+    else e = tc_launch<1, 1>(map_a, map_p, map_out, rows, cols, k_len, bg, out, accumulate, scale, scale_per_col, st);
     count_launch();
     return e != cudaSuccess ? e : cudaGetLastError();
 }
