@@ -25,7 +25,7 @@
  *   - Return value: NK_OK (0) or a negative nk_status.  Argument errors are detected on the host before any
  *     launch.  No exceptions, no exit(), no CPU fallback: without a CUDA device every compute call returns
  *     NK_ERR_CUDA.
- *   - Limits of this version: M <= 2048 (NK_F32) or M <= 1024 (NK_C64); N <= 65535; larger -> NK_ERR_UNSUPPORTED.
+ *   - Limits of this version: M <= 4096 (NK_F32) or M <= 2048 (NK_C64); N <= 65535; larger -> NK_ERR_UNSUPPORTED.
  */
 #ifndef NKB200_H
 #define NKB200_H

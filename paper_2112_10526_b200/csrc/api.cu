@@ -88,7 +88,7 @@ Geometry make_geometry(const Operator* op, int N, int M, int dtype) {
     // shared-memory plan of the fused kernel: [stages x tile][bit-packed spins][stages mbarriers + counters];
     // as many rows per stage as fit (<= 32: one ballot bit per row)
     const size_t budget = (size_t)(227 * 1024) / g.ctas_per_sm - (g.ctas_per_sm > 1 ? 1024 : 0);
-    const size_t sig = ((size_t)fused_consumer_warps() * g.n_words * 4 + 15) & ~size_t(15);
+    const size_t sig = ((size_t)fused_consumer_warps(g.M_pad, cplx) * g.n_words * 4 + 15) & ~size_t(15);
     const size_t row_bytes = (size_t)g.M_eff * 4;
     const size_t fixed = sig + (8 + 4) * 8 + 128;         // spins + barriers + counters + alignment slack
     if (fixed + 2 * row_bytes > budget) { g.ok = false; g.tile_rows = 1; g.stages = 2; }

@@ -28,8 +28,8 @@
 
 namespace nk {
 
-constexpr int FW = 16;                       // warps (samples in flight) per CTA
-constexpr int FTHREADS = FW * 32;
+// warps (samples in flight) per CTA: lane_state_warps(V, CPLX) — 16, or 8 for the wide variants (M_pad > 2048 real,
+// > 1024 complex: theta alone takes up to 128 registers per lane)
 
 struct FusedParams {
     const int8_t* sigma;
@@ -73,7 +73,8 @@ __device__ __forceinline__ void issue_tile(const FusedParams& p, uint32_t ring_u
 }
 
 template <int V, bool CPLX, bool PROD>
-__global__ void __launch_bounds__(FTHREADS, (min_blocks<V, CPLX>())) fused_eloc_kernel(const FusedParams p) {
+__global__ void __launch_bounds__(lane_state_warps(V, CPLX) * 32, (min_blocks<V, CPLX>())) fused_eloc_kernel(const FusedParams p) {
+    constexpr int FW = lane_state_warps(V, CPLX);
     extern __shared__ __align__(128) uint8_t smem[];
     if (p.gate_mode != 0) {                                  // grid-uniform: every thread takes the same branch
         const bool product_ok = __uint_as_float(*p.gate) <= NK_FORM_TAU_MAX;
@@ -324,7 +325,7 @@ int fused_ctas_per_sm(int M_pad, bool cplx) {
     const int V = M_pad / MPAD_ALIGN;
     return ((cplx ? 8 : 4) * V <= 16) ? 2 : 1;
 }
-int fused_consumer_warps() { return FW; }
+int fused_consumer_warps(int M_pad, bool cplx) { return lane_state_warps(M_pad / MPAD_ALIGN, cplx); }
 
 cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, const int8_t* sigma, int64_t B,
                               const float* theta, const float* Dtab, const RowInfo* rows, void* eloc_out,
@@ -348,11 +349,12 @@ cudaError_t launch_fused_eloc(const Operator* op, const Geometry& g, int dtype, 
     p.gate = gate; p.gate_mode = gate_mode; p.series_ctl = series_ctl;
     // one CTA per SM slot, each with an equal contiguous share of the samples (rounds of FW inside the CTA);
     // small batches use fewer CTAs so that every round is full
+    const int FW = lane_state_warps(V, cplx);
     const int64_t max_ctas = (int64_t)g_num_sms * g.ctas_per_sm;
     const int64_t n_groups = (B + FW - 1) / FW;
     const int64_t grid = n_groups < max_ctas ? n_groups : max_ctas;
     p.per_cta = (B + grid - 1) / grid;
-    fn<<<(unsigned)grid, FTHREADS, g.smem_bytes, st>>>(p);
+    fn<<<(unsigned)grid, FW * 32, g.smem_bytes, st>>>(p);
     count_launch();
     return cudaGetLastError();
 }

@@ -30,8 +30,12 @@ constexpr float KAPPA = 2.8853900817779268f;
 constexpr float LOG2E = 1.4426950408889634f;
 
 constexpr int MPAD_ALIGN = 128;      // hidden units padded to a multiple of 128: one float4 per lane per 128
-constexpr int MAX_V_REAL = 16;       // M_pad <= 2048 (real)
-constexpr int MAX_V_CPLX = 8;        // M_pad <= 1024 (complex, two planes)
+constexpr int MAX_V_REAL = 32;       // M_pad <= 4096 (real)
+constexpr int MAX_V_CPLX = 16;       // M_pad <= 2048 (complex, two planes)
+// warps (samples / chains in flight) per CTA of the warp-per-sample kernels: 16 while a lane's share of theta fits 64
+// registers (128 registers x 512 threads = the register file); the wide variants (up to 128 registers of theta per lane)
+// run 8 warps with 255 registers per thread
+__host__ __device__ constexpr int lane_state_warps(int V, bool cplx) { return ((cplx ? 2 : 1) * V > 16) ? 8 : 16; }
 
 // One row of the bond-difference table D: which sites it touches and the scalar data the fused kernel needs.
 struct __align__(32) RowInfo {
@@ -76,7 +80,7 @@ struct Geometry {
     bool ok;                                 // false: sizes beyond what this version supports
 };
 int fused_ctas_per_sm(int M_pad, bool cplx);
-int fused_consumer_warps();
+int fused_consumer_warps(int M_pad, bool cplx);
 Geometry make_geometry(const Operator* op, int N, int M, int dtype);
 
 // ---- launchers (each returns cudaGetLastError() of its launches) -----------------------------------------

@@ -18,6 +18,12 @@ __device__ __forceinline__ float warp_prod_f(float v) {
     return v;
 }
 
+// A lane multiplies up to 4 V factors (1 + e) in [1, 2] into four running products and then these together: at V = 32
+// (M_pad = 4096) that is 2^128 when every theta is 0 — the uniform state.  The wide variants therefore scale each
+// running product by 2^-16 at the middle of the lane's share, in the base product and in every row's product alike,
+// so the power of two cancels exactly in every ratio.
+constexpr float WIDE_RESCALE = 1.52587890625e-05f;          // 2^-16
+
 // ---- per-row inner loops ---------------------------------------------------------------------------------
 template <int V>
 struct RealState {
@@ -35,6 +41,7 @@ struct RealState {
             p1 = fmaf(p1, ex2_approx(-fabsf(t.y)), p1);
             p2 = fmaf(p2, ex2_approx(-fabsf(t.z)), p2);
             p3 = fmaf(p3, ex2_approx(-fabsf(t.w)), p3);
+            if (V > 16 && v == 15) { p0 *= WIDE_RESCALE; p1 *= WIDE_RESCALE; p2 *= WIDE_RESCALE; p3 *= WIDE_RESCALE; }
         }
         qinv = 1.f / ((p0 * p1) * (p2 * p3));
     }
@@ -57,6 +64,7 @@ struct RealState {
             acc1 += fabsf(x1) - fabsf(t.y);
             acc0 += fabsf(x2) - fabsf(t.z);
             acc1 += fabsf(x3) - fabsf(t.w);
+            if (V > 16 && v == 15) { p0 *= WIDE_RESCALE; p1 *= WIDE_RESCALE; p2 *= WIDE_RESCALE; p3 *= WIDE_RESCALE; }
         }
         p = (p0 * p1) * (p2 * p3);
         acc = acc0 + acc1;
@@ -149,6 +157,7 @@ struct CplxState {
             factor(x.y, y.y, p, q); cmul(br, bi, p, q);
             factor(x.z, y.z, p, q); cmul(ar, ai, p, q);
             factor(x.w, y.w, p, q); cmul(br, bi, p, q);
+            if (V > 8 && v == 7) { ar *= WIDE_RESCALE; ai *= WIDE_RESCALE; br *= WIDE_RESCALE; bi *= WIDE_RESCALE; }
         }
         cmul(ar, ai, br, bi);
         const float inv = 1.f / fmaf(ar, ar, ai * ai);
@@ -174,6 +183,7 @@ struct CplxState {
             factor(x3, fmaf(s, dy.w, y.w), p, q); cmul(br, bi, p, q);
             acc += (fabsf(x0) - fabsf(x.x)) + (fabsf(x1) - fabsf(x.y));
             acc += (fabsf(x2) - fabsf(x.z)) + (fabsf(x3) - fabsf(x.w));
+            if (V > 8 && v == 7) { ar *= WIDE_RESCALE; ai *= WIDE_RESCALE; br *= WIDE_RESCALE; bi *= WIDE_RESCALE; }
         }
         cmul(ar, ai, br, bi);
     }

@@ -61,8 +61,14 @@ constexpr int sampler_min_blocks() { return ((CPLX ? 8 : 4) * V <= 16) ? 2 : 1; 
 // Rows are staged through shared memory (STAGED) only where that was measured to win: rows of 8 KB (config 5:
 // 40.3 -> 35.6 ms per sweep, with 12 warps); for rows of <= 4 KB the direct L2 reads of 16 warps were faster
 // (configs 3, 4: 1.51 vs 1.68 ms, 0.66 vs 0.71 ms).
+// The wide variants (a lane's theta beyond 64 registers: M_pad > 2048 real, > 1024 complex) run 8 warps with 255 registers
+// and read their rows straight from L2.
 template <int V, bool CPLX>
-__host__ __device__ constexpr int sampler_warps() { return (16 * 2 * V * 512 * (CPLX ? 2 : 1) <= 216 * 1024) ? 16 : 12; }
+__host__ __device__ constexpr int sampler_warps() {
+    return lane_state_warps(V, CPLX) == 8 ? 8 : ((16 * 2 * V * 512 * (CPLX ? 2 : 1) <= 216 * 1024) ? 16 : 12);
+}
+template <int V, bool CPLX>
+__host__ __device__ constexpr bool sampler_staged() { return sampler_warps<V, CPLX>() == 12; }
 
 template <int V, bool CPLX>
 __global__ void __launch_bounds__(sampler_warps<V, CPLX>() * 32, (sampler_min_blocks<V, CPLX>())) metropolis_kernel(const SamplerParams p) {
@@ -72,13 +78,13 @@ __global__ void __launch_bounds__(sampler_warps<V, CPLX>() * 32, (sampler_min_bl
     if (c_loc >= p.nb) return;                         // no CTA-wide synchronisation below
     // shared memory: [sw warps][2 row buffers][M_eff floats] | [sw][n_words] spin bits | [sw][2] mbarriers
     const uint32_t row_bytes = (uint32_t)p.M_eff * 4u;
-    const size_t rows_bytes = (sampler_warps<V, CPLX>() < 16) ? (size_t)p.sw * 2 * row_bytes : 0;
+    const size_t rows_bytes = sampler_staged<V, CPLX>() ? (size_t)p.sw * 2 * row_bytes : 0;
     float* rowbuf = reinterpret_cast<float*>(smem_s) + (size_t)warp * 2 * p.M_eff;
     uint32_t* bits = reinterpret_cast<uint32_t*>(smem_s + rows_bytes) + (size_t)warp * p.n_words;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_s + rows_bytes + (size_t)p.sw * p.n_words * 4) +
                      warp * 2;                          // bit i of `bits` set <=> sigma_i = -1
     const uint32_t bar0 = smem_u32(bars), row0 = smem_u32(rowbuf);
-    constexpr bool STAGED = sampler_warps<V, CPLX>() < 16;
+    constexpr bool STAGED = sampler_staged<V, CPLX>();
     if (STAGED && lane == 0) {
         mbar_init(bar0, 1);
         mbar_init(bar0 + 8, 1);
@@ -234,8 +240,8 @@ cudaError_t launch_metropolis(const Geometry& g, int dtype, int8_t* sigma, int64
     SamplerFn fn = cplx ? pick_scplx<1>(V) : pick_sreal<1>(V);
     if (fn == nullptr) return cudaErrorInvalidValue;
     // as many warps per CTA (a multiple of 4, one chain each) as fit with two row buffers per warp
-    int sw = (16 * 2 * (size_t)g.M_eff * 4 <= (size_t)216 * 1024) ? 16 : 12;      // = sampler_warps<V, CPLX>()
-    const bool staged = sw < 16;
+    int sw = lane_state_warps(V, cplx) == 8 ? 8 : ((16 * 2 * (size_t)g.M_eff * 4 <= (size_t)216 * 1024) ? 16 : 12);   // = sampler_warps<V, CPLX>()
+    const bool staged = sw == 12;
     const size_t per_warp = (staged ? (size_t)2 * g.M_eff * 4 : 0) + (size_t)g.n_words * 4 + 16;
     while (sw > 4 && sw * per_warp + 128 > (size_t)220 * 1024) sw -= 4;
     const size_t smem = sw * per_warp + 128;

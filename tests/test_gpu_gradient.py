@@ -58,6 +58,8 @@ def test_gradient_parity_configs(nk, cfg, n, chunk):
     dict(kind=1, lattice="square", L=4, M=129, B=65, h=1.1, complex_params=True),
     dict(kind=0, lattice="square", L=6, M=300, B=200, complex_params=True),
     dict(kind=0, lattice="chain", L=16, M=40, B=300, scale=1e-3),     # |tanh theta| ~ 1e-3: far below the scale bound
+    dict(kind=0, lattice="chain", L=16, M=4096, B=150, scale=0.02),   # the width limit of this version, real
+    dict(kind=0, lattice="chain", L=16, M=2048, B=150, scale=0.02, complex_params=True),   # ... and complex
 ])
 def test_gradient_edge_cases(nk, case):
     case = dict(case)

@@ -262,7 +262,7 @@ def test_errors_are_loud(nk):
     op = nk.Operator.from_problem(p)
     with pytest.raises(nk.NkError, match="INVALID_ARG"):                 # N does not match the operator
         nk.local_energy(op, dev(np.ones((4, 8), np.int8)), dev(np.zeros((4, 8), np.float32)))
-    big = inp.draw_params(np.random.default_rng(0), 6, 2049, 0.1, False)
+    big = inp.draw_params(np.random.default_rng(0), 6, 4097, 0.1, False)
     with pytest.raises(nk.NkError):                                      # M beyond the supported width
         nk.local_energy(op, dev(p.sigma), dev(big[0]), None, None)
     lib = nk.load()
@@ -282,22 +282,28 @@ def test_errors_are_loud(nk):
 @pytest.mark.parametrize("case", [
     dict(kind=0, lattice="chain", L=3000, M=128, B=6),                       # N = 3000: 94 spin words, 3000 table rows
     dict(kind=1, lattice="chain", L=2100, M=100, B=5, h=0.9),                # long Ising chain, N + 1 = 2101 slots
-    dict(kind=0, lattice="chain", L=16, M=2048, B=40),                       # widest real RBM (V = 16) on a tiny lattice
-    dict(kind=0, lattice="square", L=4, M=1024, B=40, complex_params=True),  # widest complex RBM (V = 8)
+    dict(kind=0, lattice="chain", L=16, M=2048, B=40),                       # widest 16-warp real RBM (V = 16) on a tiny lattice
+    dict(kind=0, lattice="square", L=4, M=1024, B=40, complex_params=True),  # widest 16-warp complex RBM (V = 8)
+    dict(kind=0, lattice="chain", L=16, M=4096, B=40),                       # the limit: V = 32, the 8-warp variants
+    dict(kind=0, lattice="square", L=4, M=2048, B=40, complex_params=True),  # the limit, complex: V = 16
+    dict(kind=0, lattice="chain", L=12, M=2900, B=33, scale=0.0),            # uniform psi at V = 23: every factor is 2
 ])
 def test_maximum_sizes(nk, case):
-    """The limits of this version (include/nkb200.h): M = 2048 real, M = 1024 complex, and N well beyond the 1024 of
-    config 5 (several shared-memory words of spins per lane, thousands of table rows), both forms of the kernel."""
+    """The limits of this version (include/nkb200.h): M = 4096 real, M = 2048 complex (the 8-warp variants of the
+    warp-per-sample kernels, with their running products rescaled half-way), and N well beyond the 1024 of config 5
+    (several shared-memory words of spins per lane, thousands of table rows), both SIMT forms of the kernel."""
     case = dict(case)
+    scale = case.pop("scale", 0.02)
     p = inp.make_problem(case.pop("kind"), case.pop("lattice"), case.pop("L"), case.pop("M"), case.pop("B"),
-                         seed=44, scale=0.02, **case)
+                         seed=44, scale=scale, **case)
     e_ref, lp_ref = run_oracle(p)
     e, lp, _ = run_gpu(nk, p)
     assert_eloc(e, e_ref)
     assert_logpsi(lp, lp_ref)
     op = nk.Operator.from_problem(p)
-    e2, _, _ = nk.local_energy(op, dev(p.sigma), dev(p.W), dev(p.a), dev(p.b), flags=nk.NK_FORM_PRODUCT)
-    assert_eloc(e2.cpu().numpy(), e_ref)
+    for form in (nk.NK_FORM_PRODUCT, nk.NK_FORM_LOGCOSH):
+        e2, _, _ = nk.local_energy(op, dev(p.sigma), dev(p.W), dev(p.a), dev(p.b), flags=form)
+        assert_eloc(e2.cpu().numpy(), e_ref)
     op.close()
 
 

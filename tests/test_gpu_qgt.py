@@ -58,6 +58,13 @@ def test_qgt_matvec_parity_configs(nk, cfg, n, chunk):
     print(f"cfg{cfg}: max QGT-vector error / max|out| = {worst:.2e}")
 
 
+def test_qgt_matvec_at_the_width_limit(nk):
+    """M = 4096 real / 2048 complex (include/nkb200.h): the contractions are size-generic, only the limit moved."""
+    for kw in (dict(M=4096), dict(M=2048, complex_params=True)):
+        p = inp.make_problem(inp.KIND_HEISENBERG, "chain", 16, kw.pop("M"), 120, seed=9, scale=0.02, **kw)
+        check(nk, p, draw_v(p, 77), 0.01, 64)
+
+
 def test_qgt_matvec_properties(nk):
     p = inp.make_config(2, n_samples=256)
     v, u = draw_v(p, 1), draw_v(p, 2)

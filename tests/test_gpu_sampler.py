@@ -160,3 +160,9 @@ def test_sampler_long_chain_and_widest_rbm(nk):
     for r in (nk.NK_RULE_LOCAL, nk.NK_RULE_EXCHANGE):
         got, gacc, ref, racc, margin = run_both(nk, p, r, 77)
         assert_chains(p, r, got, gacc, ref, racc, margin, min_clear=0.7)
+    # the limits of this version: M = 4096 real, M = 2048 complex (the 8-warp variants, rows read straight from L2)
+    for kw in (dict(n_hidden=4096), dict(n_hidden=2048, complex_params=True)):
+        p = inp.make_problem(inp.KIND_HEISENBERG, "chain", 16, kw.pop("n_hidden"), 30, seed=8, scale=0.01, **kw)
+        for r in (nk.NK_RULE_LOCAL, nk.NK_RULE_EXCHANGE):
+            got, gacc, ref, racc, margin = run_both(nk, p, r, 45)
+            assert_chains(p, r, got, gacc, ref, racc, margin, min_clear=0.7)

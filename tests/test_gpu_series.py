@@ -154,3 +154,16 @@ def test_plan_replay_equals_the_eager_call(nk, cfg, n, chunk):
         bad.run_graph(sig, W, a, b)
     plan.close_plan()
     op.close()
+
+
+def test_series_wide_rbm_beyond_the_register_resident_limit(nk):
+    """N = 256 (16 x 16), M = 4096 = the limit of this version (alpha = 16): the series form has no register-resident
+    theta, the SIMT forms run their 8-warp variants; all three against the incremental oracle."""
+    p = inp.make_problem(inp.KIND_HEISENBERG, "square", 16, 4096, 200, seed=21, scale=0.01)
+    e_ref, lp_ref = inc.local_energy(p.kind, p.sigma, p.bonds, p.colors, p.J, p.h, p.W, p.a, p.b)
+    for form in (0, nk.NK_FORM_SERIES, nk.NK_FORM_PRODUCT, nk.NK_FORM_LOGCOSH):
+        (e, lp, st), took, terms = run_form(nk, p, form, chunk=128)
+        assert_eloc(e, e_ref)
+        assert_logpsi(lp, lp_ref)
+        if form == 0:
+            assert took == nk.NK_FORM_SERIES
