@@ -74,7 +74,7 @@ def test_argument_errors_are_reported_before_any_launch(lib):
     assert lib.nk_metropolis_sample(0, None, 0, P, 4, 10, 10, 0, P, None, None, -1, 0, 0, 0, 0, None, P, 1 << 20, None) == -1
     assert lib.nk_rbmsymm_expand(0, 4, 10, 0, P, None, P, P, None, None) == -1
     assert lib.nk_rbmsymm_reduce_gradient(2, 4, 10, 3, P, None, P, P, None, None) == -1
-    assert lib.nk_rbm_logpsi(P, 4, 10, 4096, 0, P, None, None, P, None, 0, P, 1 << 30, None) == -4               # M too large
+    assert lib.nk_rbm_logpsi(P, 4, 10, 4097, 0, P, None, None, P, None, 0, P, 1 << 30, None) == -4               # M too large
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
