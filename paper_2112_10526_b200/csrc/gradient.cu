@@ -9,6 +9,7 @@
 // and contracted with sigma^T by the same tcgen05 kernel, accumulating [N][M_eff] in fp32 across chunks.
 // g_a and g_b are fp64 column sums with a fixed order (bit-reproducible).
 
+#include "lncosh.cuh"
 #include "nk_internal.h"
 
 namespace nk {
@@ -194,25 +195,6 @@ __global__ void grad_split_T_kernel(const float* __restrict__ v, int64_t nb, int
     }
     if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && threadIdx.y == 0)
         *reinterpret_cast<float*>(TwT + 3 * plane) = poison ? __int_as_float(0x7fc00000) : ldexpf(1.f, ex - 23);
-}
-
-// tanh in fp32 without branches: |x| < 1 by x + x^3 P(x^2) (P = degree-6 least-squares fit of (tanh x - x) / x^3 in x^2,
-// relative error < 1e-7 in fp32), else 1 - 2 / (e^{2x} + 1) with one MUFU.EX2 and one MUFU.RCP (< 2e-7 relative)
-__device__ __forceinline__ float tanh_f32(float x) {
-    const float x2 = x * x;
-    float p = -0.0003552270936779678f;
-    p = fmaf(p, x2, 0.002289985306560993f);
-    p = fmaf(p, x2, -0.007930326275527477f);
-    p = fmaf(p, x2, 0.021475814282894135f);
-    p = fmaf(p, x2, -0.05387599393725395f);
-    p = fmaf(p, x2, 0.1333228200674057f);
-    p = fmaf(p, x2, -0.33333292603492737f);
-    const float small = fmaf(x * x2, p, x);
-    float E, rc;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(E) : "f"(x * 2.8853900817779268f));
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rc) : "f"(E + 1.f));
-    const float big = fmaf(-2.f, rc, 1.f);
-    return fabsf(x) < 1.f ? small : big;
 }
 
 // Real parameters, one pass: theta[s][.] -> v = real_scale tanh(theta) w_s -> the three int8 digit planes of

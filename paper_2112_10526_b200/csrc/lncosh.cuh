@@ -1,4 +1,4 @@
-// ln cosh for small arguments (shared by logpsi.cu and pack.cu).
+// ln cosh for small arguments and a branch-free fp32 tanh (shared by logpsi.cu, pack.cu and gradient.cu).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -39,6 +39,25 @@ __device__ __forceinline__ float ln_cosh_small_f(float t) {
     p = fmaf(p, u, -0.08333333333333333f);
     p = fmaf(p, u, 0.5f);
     return p * u;
+}
+
+// tanh in fp32 without branches: |x| < 1 by x + x^3 P(x^2) (P = degree-6 least-squares fit of (tanh x - x) / x^3 in x^2,
+// relative error < 1e-7 in fp32), else 1 - 2 / (e^{2x} + 1) with one MUFU.EX2 and one MUFU.RCP (< 2e-7 relative)
+__device__ __forceinline__ float tanh_f32(float x) {
+    const float x2 = x * x;
+    float p = -0.0003552270936779678f;
+    p = fmaf(p, x2, 0.002289985306560993f);
+    p = fmaf(p, x2, -0.007930326275527477f);
+    p = fmaf(p, x2, 0.021475814282894135f);
+    p = fmaf(p, x2, -0.05387599393725395f);
+    p = fmaf(p, x2, 0.1333228200674057f);
+    p = fmaf(p, x2, -0.33333292603492737f);
+    const float small = fmaf(x * x2, p, x);
+    float E, rc;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(E) : "f"(x * 2.8853900817779268f));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rc) : "f"(E + 1.f));
+    const float big = fmaf(-2.f, rc, 1.f);
+    return fabsf(x) < 1.f ? small : big;
 }
 
 }  // namespace nk
