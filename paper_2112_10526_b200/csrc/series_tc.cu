@@ -373,10 +373,12 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
                 if (n0 + c < p.n_rows) {
                     const RowInfo ri = p.rows[n0 + c];
                     if (ri.i >= 0) {
-                        const uint32_t wi = p.sigT[(size_t)ri.i * p.w32 + mt * 4 + q];
-                        const uint32_t wj = ri.j >= 0 ? p.sigT[(size_t)ri.j * p.w32 + mt * 4 + q] : ~wi;
-                        m = make_uint2(wi ^ wj, wi);       // antiparallel <=> active; sigma_i = -1 <=> s = +1
-                        t = make_float4(ri.coef, ri.jdiag, ri.a2_re, ri.c2_re);
+                        t = make_float4(ri.coef, ri.jdiag, ri.a2_re, ri.c2_re);   // (shared by the four warps)
+                        if ((int64_t)mt * BM + q * 32 < p.nb) {   // a pair's second tile may lie beyond the samples
+                            const uint32_t wi = p.sigT[(size_t)ri.i * p.w32 + mt * 4 + q];
+                            const uint32_t wj = ri.j >= 0 ? p.sigT[(size_t)ri.j * p.w32 + mt * 4 + q] : ~wi;
+                            m = make_uint2(wi ^ wj, wi);   // antiparallel <=> active; sigma_i = -1 <=> s = +1
+                        }
                     }
                 }
                 if ((c >> 6) == wq) tab[c] = t;
