@@ -28,6 +28,8 @@ CONFIG_TEXT = {
     3: "configs[2]: 2D TFIM 20x20 h=3, real RBM alpha=2, 8192 samples",
     4: "configs[3]: 2D J1-J2 10x10, complex RBM alpha=4, 16384 samples",
     5: "configs[4]: 2D Heisenberg 32x32, real RBM alpha=2, 65536 samples in chunks of 4096",
+    6: "widening case, not a BASELINE.json config: 2D Heisenberg 32x32, real RBM alpha=4 (M = 4096, the width limit), "
+       "16384 samples in chunks of 4096",
 }
 
 N_SMS = 148
@@ -102,7 +104,7 @@ def blas_threads():
         return os.cpu_count() or 1
 
 
-ORACLE_ROWS_PER_STEP = {1: 1024, 2: 256, 3: 16, 4: 64, 5: 4}
+ORACLE_ROWS_PER_STEP = {1: 1024, 2: 256, 3: 16, 4: 64, 5: 4, 6: 2}
 
 
 def run_reference(args):
@@ -608,7 +610,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5, 6])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the sampler / gradient timings")
     ap.add_argument("--call", default="plan", choices=["plan", "eager"],

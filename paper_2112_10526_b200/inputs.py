@@ -116,11 +116,14 @@ _CONFIGS = {
     3: ("tfim2d_20x20_real_a2", KIND_ISING, "square", 20, 1, 2, False, 0.02, 8192, False, (1.0,), 3.0, 0),
     4: ("j1j2_10x10_complex_a4", KIND_HEISENBERG, "square", 10, 2, 4, True, 0.03, 16384, True, (1.0, 0.5), 0.0, 0),
     5: ("heis2d_32x32_real_a2", KIND_HEISENBERG, "square", 32, 1, 2, False, 0.01, 65536, True, (1.0,), 0.0, 4096),
+    # not a BASELINE.json config: the widest real RBM the library takes (M = alpha N = 4096), config 5's
+    # lattice and recipe, for the width-limit bench line (`bench.py --config 6`) and tests
+    6: ("heis2d_32x32_real_a4", KIND_HEISENBERG, "square", 32, 1, 4, False, 0.01, 16384, True, (1.0,), 0.0, 4096),
 }
 
 
 def make_config(c: int, n_samples: int | None = None, sample_seed_offset: int = 0) -> Problem:
-    """BASELINE.json `configs[c-1]` (c = 1..5).  `n_samples` overrides the batch size (bench shards,
+    """BASELINE.json `configs[c-1]` (c = 1..5; 6 = the alpha = 4 widening of config 5).  `n_samples` overrides the batch size (bench shards,
     oracle subsets); `sample_seed_offset` gives ranks of a weak-scaling run distinct batches."""
     name, kind, lat, L, order, alpha, cplx, scale, B, sz0, J, h, chunk = _CONFIGS[c]
     bonds, colors = chain_bonds(L) if lat == "chain" else square_bonds(L, order)
