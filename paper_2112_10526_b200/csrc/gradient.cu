@@ -114,17 +114,23 @@ __global__ void grad_a_partial_kernel(const int8_t* __restrict__ sigma, int64_t 
     if (k >= N) return;
     double ar = 0.0, ai = 0.0;
     const int n = (int)(s1 - s0);
-    for (int t = 0; t < n; ++t) {
-        const double sg = (double)sigma[(s0 + t) * N + k];
-        ar += sg * wr_s[t];
-        ai += sg * wi_s[t];
+    const int8_t* col = sigma + s0 * N + k;
+    if (cplx) {
+        for (int t = 0; t < n; ++t) {
+            const double sg = (double)col[(size_t)t * N];
+            ar += sg * wr_s[t];
+            ai += sg * wi_s[t];
+        }
+    } else {
+#pragma unroll 8
+        for (int t = 0; t < n; ++t) ar += (double)col[(size_t)t * N] * wr_s[t];
     }
     part[(size_t)blockIdx.y * 2 * N + k] = ar;
     part[(size_t)blockIdx.y * 2 * N + N + k] = ai;
 }
 
-// acc[c] (+)= sum_slab part[slab][c] in a fixed order: block = 32 columns x 8 slab ranges (blockDim = (32, 8)); range r
-// adds its contiguous share of the slabs in order, then the eight range sums are added in order
+// acc[c] (+)= sum_slab part[slab][c] in a fixed order: block = 32 columns x blockDim.y <= 32 slab ranges; range r adds
+// its contiguous share of the slabs in order, then the range sums are added in order
 // scale_io (optional): [0] = max |v| bound as float bits (in) -> [2] = 2^(23 - ex), [3] = q = 2^(ex - 23) as floats (out)
 __global__ void grad_slab_reduce_kernel(const double* __restrict__ part, int n_slabs, int n_cols,
                                         double* __restrict__ acc, int first, unsigned* scale_io) {
@@ -143,9 +149,9 @@ __global__ void grad_slab_reduce_kernel(const double* __restrict__ part, int n_s
             scale_io[3] = 0x7fc00000u;
         }
     }
-    __shared__ double sh[8][32];
+    __shared__ double sh[32][32];
     const int c = blockIdx.x * 32 + threadIdx.x;
-    const int per = (n_slabs + 7) / 8;
+    const int per = (n_slabs + (int)blockDim.y - 1) / (int)blockDim.y;
     const int sl0 = threadIdx.y * per, sl1 = min(n_slabs, sl0 + per);
     double a = 0.0;
     if (c < n_cols)
@@ -154,8 +160,7 @@ __global__ void grad_slab_reduce_kernel(const double* __restrict__ part, int n_s
     __syncthreads();
     if (threadIdx.y == 0 && c < n_cols) {
         double t = first ? 0.0 : acc[c];
-#pragma unroll
-        for (int r = 0; r < 8; ++r) t += sh[r][threadIdx.x];
+        for (int r = 0; r < (int)blockDim.y; ++r) t += sh[r][threadIdx.x];
         acc[c] = t;
     }
 }
@@ -240,10 +245,21 @@ grad_tv_split_kernel(const float* __restrict__ theta, int64_t nb, int k_len, int
         }
         ptr += 32 * M_eff;
         // rint(v / q) = d2 2^16 + d1 2^8 + d0 with balanced digits: the low bytes of I, (I + 128) >> 8 and of that again
+        // |theta| < 1 almost everywhere at the configs' parameter scale: the polynomial alone, unless a lane of the warp
+        // holds a larger argument (a NaN passes the max and propagates through the polynomial)
+        float tv[4];
+        const float amax = fmaxf(fmaxf(fabsf(th[0]), fabsf(th[1])), fmaxf(fabsf(th[2]), fabsf(th[3])));
+        if (__any_sync(0xffffffffu, amax >= 1.f)) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) tv[i] = tanh_f32(th[i]);
+        } else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) tv[i] = tanh_unit_f(th[i]);
+        }
         unsigned w0 = 0, w1 = 0, w2 = 0;
 #define NK_DIGITS(i, sel)                                                         \
         {                                                                         \
-            const int I = __float2int_rn(tanh_f32(th[i]) * w_s[sl + i]);          \
+            const int I = __float2int_rn(tv[i] * w_s[sl + i]);                    \
             const int I1 = (I + 128) >> 8;                                        \
             const int I2 = (I1 + 128) >> 8;                                       \
             acc += I;                                                             \
@@ -371,7 +387,8 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
     const float* th_in = theta_in ? theta_in : w.theta;
     grad_a_partial_kernel<<<dim3((g.N + 127) / 128, n_slabs), 128, 0, st>>>(
         sigma, nb, g.N, (const float*)eloc, stats, inv_B, cplx, (double)real_scale, w.part, cplx ? nullptr : w.absmax);
-    grad_slab_reduce_kernel<<<(2 * g.N + 31) / 32, dim3(32, 8), 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk,
+    const dim3 red_block(32, n_slabs >= 128 ? 32 : 8);
+    grad_slab_reduce_kernel<<<(2 * g.N + 31) / 32, red_block, 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk,
                                                                    cplx ? nullptr : w.absmax);
     if (!cplx) {
         // k_len / GRAD_SLAB == n_slabs (both round nb up to 128)
@@ -388,7 +405,7 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
             w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (int8_t*)w.TwT);
         count_launch(sigT_ready ? 6 : 7);
     }
-    grad_slab_reduce_kernel<<<(g.M_eff + 31) / 32, dim3(32, 8), 0, st>>>(w.part, n_slabs, g.M_eff, w.gb_acc, first_chunk,
+    grad_slab_reduce_kernel<<<(g.M_eff + 31) / 32, red_block, 0, st>>>(w.part, n_slabs, g.M_eff, w.gb_acc, first_chunk,
                                                                    nullptr);
     if (sigT_ready == nullptr)
         grad_sigma_T_kernel<<<dim3(k_len / 128, (g.N + 127) / 128), 256, 0, st>>>(sigma, nb, k_len, g.N, w.ld,
