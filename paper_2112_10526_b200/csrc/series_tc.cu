@@ -46,16 +46,18 @@ namespace ser {
 constexpr int BM = 128, BN = 256, BK = 64;                // BK 16-bit elements = one 128-B swizzle row
 constexpr int A_TILE = BM * BK * 2;                       // 16 KB
 constexpr int NA = 4;                                     // ring depths (3 + 3 measured: GEMM 181 -> 207 us per chunk)
-constexpr int THREADS = 224;                              // warps: A producer, MMA, B producer, 4 x epilogue
-constexpr int TAB_BYTES = BN * 16, MSK_BYTES = BN * 8;    // (coef, jdiag, a2, c2) per column, shared by the epilogue warps;
-                                                          // (act, neg) spin masks per column and epilogue warp
+constexpr int EPI_HALVES = 2;                             // epilogue warps per TMEM lane quarter: each drains BN / 2 columns
+constexpr int EPI_WARPS = 4 * EPI_HALVES, EPI_COLS = BN / EPI_HALVES;
+constexpr int THREADS = 96 + 32 * EPI_WARPS;              // warps: A producer, MMA, B producer, 8 x epilogue
+constexpr int TAB_BYTES = BN * 16, MSK_BYTES = EPI_COLS * 8;   // (coef, jdiag, a2, c2) per column, shared by the epilogue
+                                                          // warps; (act, neg) spin masks per column of each epilogue warp
 // CG = CTAs per tile: 1 (a CTA owns a 128 x 256 tile) or 2 (a CTA PAIR owns 256 x 256 through tcgen05 cta_group::2: each
 // CTA holds its 128 samples' A tiles and HALF of every B tile, so the table-row operand crosses L2 -> shared memory and
 // shared memory -> tensor core once per 256 samples instead of once per 128)
 template <int CG> struct Cfg {
     static constexpr int B_TILE = (BN / CG) * BK * 2;     // 32 KB, or 16 KB per CTA of a pair
     static constexpr int NB = CG == 2 ? 6 : 4;
-    static constexpr int SMEM_BYTES = NA * A_TILE + NB * B_TILE + TAB_BYTES + 4 * MSK_BYTES + 256 /*barriers*/ + 1024 /*alignment*/;
+    static constexpr int SMEM_BYTES = NA * A_TILE + NB * B_TILE + TAB_BYTES + EPI_WARPS * MSK_BYTES + 256 /*barriers*/ + 1024 /*alignment*/;
 };
 constexpr uint32_t TMEM_COLS = 512;                       // odd at column 0, even at column 256
 // instruction descriptors of kind::f16 (the cute::UMMA::InstrDescriptor bit layout): D = F32 (c_format 1 at bit 4),
@@ -164,7 +166,7 @@ struct SeriesParams {
     int64_t nb;                   // samples of this chunk
     int n_rows, M_pad;
     int n_mt, n_nt;               // tiles along samples / table rows
-    float* part;                  // [n_nt][part_stride]
+    float* part;                  // [n_nt * EPI_HALVES][part_stride]
     int64_t part_stride;
 };
 
@@ -205,7 +207,7 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
     uint8_t* smem_al = smem_raw + (smem_base - smem_u32(smem_raw));
     const uint32_t a_ring = smem_base, b_ring = smem_base + NA * A_TILE;
     const uint32_t epi_off = NA * A_TILE + NB * B_TILE;
-    const uint32_t bars = smem_base + epi_off + TAB_BYTES + 4 * MSK_BYTES;
+    const uint32_t bars = smem_base + epi_off + TAB_BYTES + EPI_WARPS * MSK_BYTES;
     const uint32_t a_full = bars, a_empty = bars + 8 * NA, b_full = bars + 16 * NA, b_empty = b_full + 8 * NB;
     const uint32_t t_full = b_empty + 8 * NB, t_empty = t_full + 8, tmem_slot = t_empty + 8;
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_al + (tmem_slot - smem_base));
@@ -225,7 +227,7 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
         for (int s = 0; s < NA; ++s) { mbar_init(a_full + 8 * s, 1); mbar_init(a_empty + 8 * s, 1); }
         for (int s = 0; s < NB; ++s) { mbar_init(b_full + 8 * s, 1); mbar_init(b_empty + 8 * s, 1); }
         mbar_init(t_full, 1);
-        mbar_init(t_empty, 128 * CG);
+        mbar_init(t_empty, 32 * EPI_WARPS * CG);
         mbar_fence_init();
     }
     if (warp == 1) {                                       // the same warp in both CTAs of a pair
@@ -354,26 +356,29 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
             }
         }
     } else {
-        // ===== epilogue: warps 3..6, TMEM lane quarter q = warp % 4 =====
+        // ===== epilogue: warps 3..10; TMEM lane quarter q = warp % 4, column half h (two warps drain a quarter's 256
+        // columns side by side: the tensor pipe idles from the last MMA of a tile until the accumulators are handed back,
+        // so the drain time is what the tile pays for having one accumulator set) =====
         const int q = warp & 3;
+        const int we = warp - 3, h = we >> 2;              // 0..7; this warp's columns are [h EPI_COLS, (h + 1) EPI_COLS)
         float4* tab = reinterpret_cast<float4*>(smem_al + epi_off);
-        uint2* msk = reinterpret_cast<uint2*>(smem_al + epi_off + TAB_BYTES + q * MSK_BYTES);
-        const int wq = warp - 3;                           // 0..3: which quarter of the row records this warp stages
+        uint2* msk = reinterpret_cast<uint2*>(smem_al + epi_off + TAB_BYTES + we * MSK_BYTES);
         const float inv = __uint_as_float(p.ctl[1]);
         uint32_t n_done = 0;
         for (int tile = unit; tile < n_tiles; tile += n_units, ++n_done) {
             const int nt = tile % p.n_nt, mt = (tile / p.n_nt) * CG + (int)rank;     // this CTA's 128 samples
             const int n0 = nt * BN;
-            // per column: matrix element, diagonal coupling and exponents (staged once for the four warps) and this warp's
-            // 32 samples' two spin masks
-            asm volatile("bar.sync 1, 128;" ::: "memory");  // every epilogue warp is done with the previous tile's records
-            for (int c = lane; c < BN; c += 32) {
+            // per column: matrix element, diagonal coupling and exponents (the warp stages the records of the 32 columns
+            // q of its half for everyone) and the two spin masks of this warp's 32 samples
+            asm volatile("bar.sync 1, %0;" ::"n"(32 * EPI_WARPS) : "memory");   // all are done with the previous tile's records
+            for (int cc = lane; cc < EPI_COLS; cc += 32) {
+                const int c = h * EPI_COLS + cc;
                 uint2 m = make_uint2(0u, 0u);
                 float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (n0 + c < p.n_rows) {
                     const RowInfo ri = p.rows[n0 + c];
                     if (ri.i >= 0) {
-                        t = make_float4(ri.coef, ri.jdiag, ri.a2_re, ri.c2_re);   // (shared by the four warps)
+                        t = make_float4(ri.coef, ri.jdiag, ri.a2_re, ri.c2_re);
                         if ((int64_t)mt * BM + q * 32 < p.nb) {   // a pair's second tile may lie beyond the samples
                             const uint32_t wi = p.sigT[(size_t)ri.i * p.w32 + mt * 4 + q];
                             const uint32_t wj = ri.j >= 0 ? p.sigT[(size_t)ri.j * p.w32 + mt * 4 + q] : ~wi;
@@ -381,28 +386,28 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
                         }
                     }
                 }
-                if ((c >> 6) == wq) tab[c] = t;
-                msk[c] = m;
+                if (((cc >> 5) & 3) == q) tab[c] = t;
+                msk[cc] = m;
             }
-            asm volatile("bar.sync 1, 128;" ::: "memory");
+            asm volatile("bar.sync 1, %0;" ::"n"(32 * EPI_WARPS) : "memory");
             const int64_t row = (int64_t)mt * BM + q * 32 + lane;
             float E = 0.f;
             mbar_wait(t_full, n_done & 1u);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
-            for (int c0 = 0; c0 < BN; c0 += 32) {
+            for (int c0 = 0; c0 < EPI_COLS; c0 += 32) {
                 float od[32], ev[32];
-                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + c0;
+                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + h * EPI_COLS + c0;
                 tmem_ld32(taddr, od);
                 tmem_ld32(taddr + BN, ev);
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                if (c0 + 32 == BN) {                       // both accumulators are in registers: hand them back
+                if (c0 + 32 == EPI_COLS) {                 // both accumulators are in registers: hand them back
                     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
                     if (CG == 2) mbar_arrive_cluster(t_empty_l); else mbar_arrive(t_empty);
                 }
 #pragma unroll
                 for (int jj = 0; jj < 32; ++jj) {
-                    const float4 t = tab[c0 + jj];
+                    const float4 t = tab[h * EPI_COLS + c0 + jj];
                     const uint2 m = msk[c0 + jj];
                     const float u = fmaf(inv, od[jj], t.z);                 // da + odd        (log2 units)
                     const float v = fmaf(inv, ev[jj], t.w);                 // c + even
@@ -411,7 +416,7 @@ series_gemm_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
                     E += ((m.x >> lane) & 1u) ? term : t.y;                 // parallel bond: + J, no connected state
                 }
             }
-            if (row < p.nb) p.part[(size_t)nt * p.part_stride + row] = E;
+            if (row < p.nb) p.part[(size_t)(nt * EPI_HALVES + h) * p.part_stride + row] = E;
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -561,7 +566,7 @@ SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chu
             w.sigT[k] = (uint32_t*)take((size_t)g.N * w.w32 * 4);
         } else { w.Ap[k] = w.Ap[0]; w.sigT[k] = w.sigT[0]; }
     }
-    w.part = (float*)take((size_t)w.n_nt * w.part_stride * 4);
+    w.part = (float*)take((size_t)w.n_nt * ser::EPI_HALVES * w.part_stride * 4);
     return w;
 }
 
@@ -638,7 +643,7 @@ cudaError_t launch_series_gemm(const Geometry& g, int64_t s0, int64_t nb, const 
 cudaError_t launch_series_finish(const Operator* op, const Geometry& g, const int8_t* sigma, int64_t B, const SeriesWs& w,
                                  float* eloc_out, cudaStream_t st) {
     if (B <= 0) return cudaSuccess;
-    series_finish_kernel<<<(unsigned)((B + 7) / 8), 256, 0, st>>>(w.part, w.n_nt, w.part_stride, sigma, B, g.N, op->kind,
+    series_finish_kernel<<<(unsigned)((B + 7) / 8), 256, 0, st>>>(w.part, w.n_nt * ser::EPI_HALVES, w.part_stride, sigma, B, g.N, op->kind,
                                                                  op->d_bonds, op->d_colors, op->d_Jf, op->n_bonds,
                                                                  w.ctl, eloc_out);
     count_launch();
