@@ -144,13 +144,15 @@ static LogpsiWs carve_logpsi(void* ws, const Geometry& g, int64_t rows) {
     w.bytes = c.off;
     return w;
 }
+constexpr int64_t THETA_WINDOW_BYTES = int64_t(1) << 30;
 struct ElocWs {
     float *Wg, *bg, *Wt, *Dtab, *Ttab;                // Dtab: log-cosh form, Ttab: product form (both when automatic)
     float* theta;                                     // per-chunk buffers
     uint16_t *A, *Ws;
     unsigned *absmax, *taumax;                        // taumax: max |tanh delta| of Ttab as float bits (the form gate)
     RowInfo* rows;
-    int64_t unit_rows;                                // rows of theta / A: one chunk, or one group of chunks (series form)
+    int64_t unit_rows;                                // rows the kernels work on: one chunk, or one group of chunks (series form)
+    int64_t theta_rows;                               // rows of theta / A: unit_rows times the groups of one theta window
     bool has_series;                                  // the tensor-core series form is possible for these sizes
     SeriesWs ser;
     size_t bytes;
@@ -171,8 +173,19 @@ static ElocWs carve_eloc(void* ws, const Geometry& g, int64_t chunk, int dtype, 
     if (w.has_series) w.ser = carve_series(c.base, &c.off, g, chunk, B);
     // the unit the chunk loop works in: a chunk, or (series form possible) the group of chunks one tensor-core launch covers
     w.unit_rows = w.has_series ? w.ser.group_rows : chunk;
-    w.theta = c.take<float>((size_t)w.unit_rows * g.M_eff);
-    w.A = c.take<uint16_t>((size_t)w.unit_rows * g.K_pad);
+    // Series form: theta is contracted for a WINDOW of groups in one launch (as many as keep theta under
+    // THETA_WINDOW_BYTES — the whole batch at config 5, 512 MiB): the contraction and the series launches each need
+    // whole SMs, so a per-group theta launch only ever ran between two series launches; one launch per window runs at
+    // the large-launch rate and leaves nothing but the light ln psi / operand pass to run beside the tensor-core work.
+    w.theta_rows = w.unit_rows;
+    if (w.has_series) {
+        const int64_t n_groups = (B + w.unit_rows - 1) / w.unit_rows;
+        int64_t win = THETA_WINDOW_BYTES / ((int64_t)w.unit_rows * g.M_eff * 4);
+        win = win < 1 ? 1 : (win > n_groups ? n_groups : win);
+        w.theta_rows = w.unit_rows * win;
+    }
+    w.theta = c.take<float>((size_t)w.theta_rows * g.M_eff);
+    w.A = c.take<uint16_t>((size_t)w.theta_rows * g.K_pad);
     w.bytes = c.off;
     return w;
 }
@@ -797,6 +810,8 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
     // four launches of each per step at config 5 instead of sixteen (also when a SIMT form is forced there).
     const int64_t group_rows = w.unit_rows;
     const int64_t copy_chunk = chunk;                                 // granularity of the host path's arrival events
+    // groups per theta launch (carve_eloc); the host path keeps one, so that theta of a group waits for its own chunks only
+    const int64_t win = (series && tl_chunk_ready == nullptr) ? w.theta_rows / group_rows : 1;
     int64_t gi = 0;
     for (int64_t g0 = 0; g0 < B; g0 += group_rows, ++gi) {
         const int64_t gn = (B - g0 < group_rows) ? (B - g0) : group_rows;
@@ -809,14 +824,16 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
             if (tl_chunk_ready != nullptr)                            // every chunk of the group has arrived
                 for (int64_t c0 = s0; c0 < s0 + nb; c0 += copy_chunk)
                     NK_CUDA(cudaStreamWaitEvent(ps, (*tl_chunk_ready)[(size_t)(c0 / copy_chunk)], 0));
-            {
+            const float* th = w.theta + (size_t)((gi % win) * group_rows) * g.M_eff;
+            if (gi % win == 0) {               // theta of the whole window (of this group alone when win = 1)
                 Scope sc(PH_GEMM, ps);
-                NK_CUDA(run_theta(g, sg, nb, w.Wg, w.bg, w.Ws, w.A, w.theta, ps));
+                const int64_t wn = (B - s0 < win * group_rows) ? (B - s0) : win * group_rows;
+                NK_CUDA(run_theta(g, sg, wn, w.Wg, w.bg, w.Ws, w.A, w.theta, ps));
             }
             if (logpsi_out || series) {        // ln psi and, in the same pass over theta, the series form's operand rows
                 Scope sc(PH_LOGPSI, ps);
                 uint16_t* ap = series ? w.ser.Ap[set] : nullptr;
-                NK_CUDA(launch_logpsi(sg, nb, g, dtype, w.theta, a, logpsi_out ? (uint8_t*)logpsi_out + s0 * esz : nullptr,
+                NK_CUDA(launch_logpsi(sg, nb, g, dtype, th, a, logpsi_out ? (uint8_t*)logpsi_out + s0 * esz : nullptr,
                                       false, nullptr, ps, series ? w.ser.ctl : nullptr, ap));
             }
             {
@@ -827,10 +844,10 @@ int nk_local_energy_ex(nk_operator_t h, const int8_t* sigma, int64_t B, int N, i
                 void* out = (uint8_t*)eloc_out + s0 * esz;
                 if (automatic) {
                     const unsigned* sctl = series ? w.ser.ctl : nullptr;
-                    NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Ttab, w.rows, out, true, ps, w.taumax, 1, sctl));
-                    NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, w.Dtab, w.rows, out, false, ps, w.taumax, 2, sctl));
+                    NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, th, w.Ttab, w.rows, out, true, ps, w.taumax, 1, sctl));
+                    NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, th, w.Dtab, w.rows, out, false, ps, w.taumax, 2, sctl));
                 } else if (!force_series) {
-                    NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, w.theta, force_product ? w.Ttab : w.Dtab, w.rows, out,
+                    NK_CUDA(launch_fused_eloc(op, g, dtype, sg, nb, th, force_product ? w.Ttab : w.Dtab, w.rows, out,
                                               force_product, ps));
                 }
             }
