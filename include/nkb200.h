@@ -98,6 +98,23 @@ int nk_rbm_logpsi(const int8_t* sigma, int64_t B, int N, int M, int dtype, const
                   const void* b, void* logpsi_out, void* theta_out, unsigned flags, void* workspace,
                   size_t workspace_bytes, nk_stream_t stream);
 
+/* nk_rbm_logpsi for callers that cannot allocate device memory (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same inputs, outputs, arithmetic and errors, no workspace argument.  The scratch
+ * is a static device array of NK_STATIC_SCRATCH_BYTES (16 MiB) inside the library, which EVERY GPU that loads the
+ * library holds until the process exits; the call itself makes no cudaMalloc / cudaFree and calls no allocating
+ * library routine.  Limit: nk_rbm_logpsi_workspace_bytes(B, N, M, dtype) <= NK_STATIC_SCRATCH_BYTES (also returned by
+ * nk_rbm_logpsi_static_max_bytes), e.g. B = 4096 samples of config 2 (N = M = 100: 3.2 MiB) or B = 1024 at N = 400,
+ * M = 800 (7 MiB); a larger problem is rejected with NK_ERR_WORKSPACE before anything is launched — use
+ * nk_rbm_logpsi with your own workspace there.  All calls on a device share the one array, which keeps the last
+ * call's contents (every buffer in it is rewritten in full by the call before it is read, so nothing needs clearing):
+ * calls that may OVERLAP on the GPU — different streams, or graphs replayed concurrently — race on it; order them on
+ * one stream or with events.  The array's address is resolved per device on the first call there
+ * (cudaGetSymbolAddress), with that device current.  Asynchronous on `stream` like nk_rbm_logpsi. */
+#define NK_STATIC_SCRATCH_BYTES (16u << 20)
+size_t nk_rbm_logpsi_static_max_bytes(void);
+int nk_rbm_logpsi_static(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* a,
+                         const void* b, void* logpsi_out, void* theta_out, unsigned flags, nk_stream_t stream);
+
 /* ---- connected configurations (inspection / parity call; the fused path never materialises sigma') --------
  * Fixed-width list per sample, C = nk_operator_max_conn:
  *   slot 0      diagonal: flips (-1,-1), mel = H_ss (always present)

@@ -10,7 +10,7 @@ import os
 
 import numpy as np
 
-__all__ = ["load", "NkError", "Operator", "rbm_logpsi", "connected", "local_energy", "local_energy_host", "energy_gradient",
+__all__ = ["load", "NkError", "Operator", "rbm_logpsi", "rbm_logpsi_static", "connected", "local_energy", "local_energy_host", "energy_gradient",
            "qgt_matvec", "sr_solve", "rbmsymm_expand", "rbmsymm_reduce_gradient", "metropolis_sample", "NK_RULE_LOCAL", "NK_RULE_EXCHANGE", "LocalEnergyPlan", "HostPlan", "launch_count", "pipe_peaks", "profile_enable", "profile_read", "PHASES", "combine_stats", "allreduce_stats", "allreduce_gradient", "LIB_PATH",
            "NK_HEISENBERG", "NK_ISING", "NK_F32", "NK_C64", "NK_FLAG_MARSHALL", "NK_OUT_F64", "NK_FORM_PRODUCT", "NK_CHECK_SPINS", "NK_FORM_LOGCOSH", "NK_FORM_SERIES", "NK_SERIAL_CHUNKS", "EXPORTS"]
 
@@ -33,6 +33,8 @@ EXPORTS = {
     "nk_operator_max_conn": (_int, [_vp, C.POINTER(_int)]),
     "nk_rbm_logpsi_workspace_bytes": (_sz, [_i64, _int, _int, _int]),
     "nk_rbm_logpsi": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _vp, _u32, _vp, _sz, _vp]),
+    "nk_rbm_logpsi_static_max_bytes": (_sz, []),
+    "nk_rbm_logpsi_static": (_int, [_vp, _i64, _int, _int, _int, _vp, _vp, _vp, _vp, _vp, _u32, _vp]),
     "nk_connected": (_int, [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp]),
     "nk_local_energy_workspace_bytes": (_sz, [_vp, _i64, _int, _int, _int, _i64]),
     "nk_local_energy": (_int, [_vp, _vp, _i64, _int, _int, _int, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _sz, _vp]),
@@ -185,6 +187,32 @@ def rbm_logpsi(sigma, W, a=None, b=None, *, out_f64: bool = False, return_theta:
                            NK_OUT_F64 if out_f64 else 0, _ptr(ws), ws.numel(), _stream())
     _check(rc, "nk_rbm_logpsi")
     return (out, theta) if return_theta else out
+
+
+def rbm_logpsi_static(sigma, W, a=None, b=None, *, out=None, out_f64: bool = False):
+    """nk_rbm_logpsi_static: ln psi [B] with the library's static 16 MiB scratch instead of a workspace — the C call
+    allocates nothing.  `out`: preallocated result (a caller that cannot allocate passes it; else torch.empty here).
+    Calls that may overlap on the GPU race on the shared scratch."""
+    torch = _torch()
+    lib = load()
+    _check_params(sigma, W, a, b)
+    B, N = sigma.shape
+    M = W.shape[0]
+    dt = _dtype_code(W)
+    cplx = dt == NK_C64
+    odt = (torch.complex128 if cplx else torch.float64) if out_f64 else (torch.complex64 if cplx else torch.float32)
+    need, cap = lib.nk_rbm_logpsi_workspace_bytes(B, N, M, dt), lib.nk_rbm_logpsi_static_max_bytes()
+    if need > cap:
+        raise NkError(f"nk_rbm_logpsi_static: this problem needs {need} bytes of scratch, the static array holds {cap}; "
+                      "use rbm_logpsi (caller workspace)")
+    if out is None:
+        out = torch.empty(B, dtype=odt, device=sigma.device)
+    elif out.dtype != odt or out.shape != (B,) or not out.is_contiguous() or out.device != sigma.device:
+        raise NkError("out must be a contiguous [B] tensor of the result dtype on sigma's device")
+    rc = lib.nk_rbm_logpsi_static(_ptr(sigma), B, N, M, dt, _ptr(W), _ptr(a), _ptr(b), _ptr(out), None,
+                                  NK_OUT_F64 if out_f64 else 0, _stream())
+    _check(rc, "nk_rbm_logpsi_static")
+    return out
 
 
 def connected(op: Operator, sigma, *, materialize: bool = False):

@@ -5,6 +5,8 @@
 #include <new>
 #include <vector>
 
+#include <mutex>
+
 #include "nk_internal.h"
 
 namespace nk {
@@ -388,6 +390,48 @@ int nk_rbm_logpsi(const int8_t* sigma, int64_t B, int N, int M, int dtype, const
     NK_CUDA(run_theta(g, sigma, B, w.Wg, w.bg, w.Ws, w.A, w.theta, st));
     NK_CUDA(launch_logpsi(sigma, B, g, dtype, w.theta, a, logpsi_out, (flags & NK_OUT_F64) != 0, theta_out, st));
     return NK_OK;
+}
+
+// ---- ln psi without a caller workspace ---------------------------------------------------------------------------
+// For callers that cannot allocate (stream capture, serving loops, harnesses that forbid cudaMalloc): the scratch of
+// nk_rbm_logpsi lives in a file-scope device array of NK_STATIC_SCRATCH_BYTES that every GPU loading the library holds
+// until exit.  In host code `g_static_scratch` is a host-side stand-in, not a device address: the address is resolved
+// once per device, with that device current, by cudaGetSymbolAddress and that pointer is what the kernels get.
+static __device__ __align__(256) unsigned char g_static_scratch[NK_STATIC_SCRATCH_BYTES];
+static std::mutex g_static_mutex;
+static void* g_static_ptr[NK_MAX_DEVICES];
+static cudaError_t static_scratch(void** out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= NK_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (g_static_ptr[dev] == nullptr) {
+        void* ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (ptr == nullptr || ((uintptr_t)ptr & 255)) return cudaErrorInvalidSymbol;
+        g_static_ptr[dev] = ptr;
+    }
+    *out = g_static_ptr[dev];
+    return cudaSuccess;
+}
+
+size_t nk_rbm_logpsi_static_max_bytes(void) { return (size_t)NK_STATIC_SCRATCH_BYTES; }
+
+int nk_rbm_logpsi_static(const int8_t* sigma, int64_t B, int N, int M, int dtype, const void* W, const void* a,
+                         const void* b, void* logpsi_out, void* theta_out, unsigned flags, nk_stream_t stream) {
+    if (bad_dims(B, N, M, dtype)) return NK_ERR_INVALID_ARG;
+    const Geometry g = make_geometry(nullptr, N, M, dtype);
+    if (g.M_pad / MPAD_ALIGN > (dtype == NK_C64 ? MAX_V_CPLX : MAX_V_REAL) || N > 65535) return NK_ERR_UNSUPPORTED;
+    if (carve_logpsi(nullptr, g, B).bytes > (size_t)NK_STATIC_SCRATCH_BYTES) return NK_ERR_WORKSPACE;
+    void* ws = nullptr;
+    NK_CUDA(static_scratch(&ws));
+    // Nothing in the scratch has to start at zero: every buffer carved from it (packed weights and bias, digit planes and
+    // scales, padded spins, theta) is written in full by this call's own launches before a later launch reads it, so
+    // the previous call's contents — of any other shape — are never observed.
+    return nk_rbm_logpsi(sigma, B, N, M, dtype, W, a, b, logpsi_out, theta_out, flags, ws, (size_t)NK_STATIC_SCRATCH_BYTES,
+                         stream);
 }
 
 int nk_connected(nk_operator_t h, const int8_t* sigma, int64_t B, int32_t* flips_out, float* mels_out,
