@@ -131,7 +131,7 @@ int nk_connected(nk_operator_t op, const int8_t* sigma, int64_t B, int32_t* flip
  * time (0 = whole batch) inside a workspace whose size is set by min(B, chunk_size), not by B: where the tensor-core
  * series form can run (see nk_local_energy_ex) the library works on groups of up to 8 consecutive chunks — as many as
  * make its launches whole waves, at most 1 GiB of operand rows per buffer — so the bound is a small multiple of
- * chunk_size there, plus 32 bytes per sample for partial sums, and theta = W sigma + b is kept for a window of
+ * chunk_size there, plus 64 bytes per sample (at 2048 table rows) for partial sums, and theta = W sigma + b is kept for a window of
  * groups (up to 1 GiB of fp32 activations: 4 M_pad bytes per sample until that cap) so that one launch contracts the
  * whole window.  Always size the workspace with the query.  Per-sample results do not depend on chunk_size.
  *   eloc_out    dev [B] float | (re,im) float

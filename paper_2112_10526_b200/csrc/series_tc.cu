@@ -25,10 +25,10 @@
 // Kernel (series_gemm_kernel): persistent, one CTA per SM, 128 (samples) x 256 (table rows) tiles, tcgen05.mma
 // kind::f16 M = 128, N = 256, K = 16 issued by one thread; accumulators odd / even fill the 512 TMEM columns.  The two
 // operands flow through separate shared-memory rings (4 x 16 KB and 4 x 32 KB, 128B-swizzled TMA boxes of 64 hidden
-// units), each with its own producer warp.  Four epilogue warps (one TMEM lane
-// quarter each) read both accumulators, form the exponent, take 2^x, multiply by the matrix element, mask by the
+// units), each with its own producer warp.  Eight epilogue warps (two per TMEM lane
+// quarter, half of the 256 columns each) read both accumulators, form the exponent, take 2^x, multiply by the matrix element, mask by the
 // sample's spins (antiparallel bond / sign of s from bit-packed transposed spins) and sum over the tile's rows —
-// [samples] x [rows] never leaves the SM.  Partial sums per column tile go to `part`, summed in a fixed order by
+// [samples] x [rows] never leaves the SM.  Partial sums per half column tile go to `part`, summed in a fixed order by
 // series_finish_kernel (bit-reproducible, independent of chunk_size).
 #include <cuda.h>
 #include <cuda_bf16.h>
@@ -557,7 +557,7 @@ SeriesWs carve_series(uint8_t* base, size_t* off, const Geometry& g, int64_t chu
     w.group_rows = (int64_t)w.group * chunk < B ? (int64_t)w.group * chunk : B;
     w.n_sets = w.group_rows < B ? 2 : 1;
     w.w32 = (int)((w.group_rows + 127) / 128 * 4);
-    w.part_stride = (B + 127) / 128 * 128 + 128;       // whole batch (32 B per sample at config 5): one finishing pass
+    w.part_stride = (B + 127) / 128 * 128 + 128;       // whole batch (64 B per sample at config 5): one finishing pass
     w.ctl = (unsigned*)take(SER_CTL_WORDS * sizeof(unsigned));
     w.Bp = (uint16_t*)take((size_t)g.n_rows * SERIES_SEGS * g.M_pad * 2);
     for (int k = 0; k < 2; ++k) {                      // per-group buffers
