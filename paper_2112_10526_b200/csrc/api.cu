@@ -206,8 +206,9 @@ static GradWs carve_grad(void* ws, const Geometry& g, int64_t chunk, size_t* byt
     w.sigT = c.take<uint16_t>((size_t)g.N * w.ld);
     w.gb_acc = c.take<double>(g.M_eff);
     w.ga_acc = c.take<double>((size_t)2 * g.N);
-    w.part = c.take<double>((size_t)((chunk + grad_slab() - 1) / grad_slab()) *
-                            (size_t)(g.M_eff > 2 * g.N ? g.M_eff : 2 * g.N));
+    const size_t n_slabs = (size_t)((chunk + grad_slab() - 1) / grad_slab());
+    w.part = c.take<double>(n_slabs * (size_t)g.M_eff);
+    w.part_a = c.take<double>(n_slabs * (size_t)(2 * g.N));
     w.absmax = c.take<unsigned>(1);
     *bytes = c.off;
     return w;
@@ -477,15 +478,27 @@ int nk_energy_gradient_sharded(const int8_t* sigma, int64_t B, int64_t B_global,
     const GradWs w = carve_grad(workspace, g, chunk, &need);
     cudaStream_t st = (cudaStream_t)stream;
     const size_t esz = dtype == NK_C64 ? 8 : 4;
-    NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.Wg, w.bg, st));
-    NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, st));
+    // The part of a chunk that does not read theta (sample weights into grad_a, the scale of the split, the transposed
+    // spins) runs on the internal stream beside the packing and the theta contraction of the same chunk; the caller's
+    // stream waits for it before the part that needs both.  Everything the caller observes is ordered on `stream`.
+    NK_CUDA(pipeline_objects());
+    cudaStream_t side = tl_prep_stream;
     int first = 1;
     for (int64_t s0 = 0; s0 < B; s0 += chunk) {
         const int64_t nb = (B - s0 < chunk) ? (B - s0) : chunk;
         const int8_t* sg = sigma + s0 * N;
+        const void* el = (const uint8_t*)eloc + s0 * esz;
+        NK_CUDA(cudaEventRecord(tl_pipe_events[0], st));              // earlier work (the previous chunk) is done with the buffers
+        NK_CUDA(cudaStreamWaitEvent(side, tl_pipe_events[0], 0));
+        NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B_global, el, stats, w, first, 2.f, side, nullptr, nullptr, 1));
+        NK_CUDA(cudaEventRecord(tl_pipe_events[1], side));
+        if (first) {
+            NK_CUDA(launch_pack_gemm_only(g, dtype, W, b, w.Wg, w.bg, st));
+            NK_CUDA(launch_split_w(w.Wg, g.M_eff, N, g.K_pad, w.Ws, st));
+        }
         NK_CUDA(launch_theta_tc(sg, nb, N, g.M_eff, g.K_pad, w.Ws, w.A, w.bg, w.theta, st));
-        NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B_global, (const uint8_t*)eloc + s0 * esz, stats, w, first, 2.f,
-                                      st));
+        NK_CUDA(cudaStreamWaitEvent(st, tl_pipe_events[1], 0));
+        NK_CUDA(launch_gradient_chunk(g, dtype, sg, nb, B_global, el, stats, w, first, 2.f, st, nullptr, nullptr, 2));
         first = 0;
     }
     NK_CUDA(launch_gradient_finalize(g, dtype, w, grad_a_out, grad_b_out, grad_W_out, st));

@@ -374,28 +374,45 @@ __global__ void grad_finalize_ab_kernel(const double* __restrict__ ga_acc, const
 
 int grad_slab() { return GRAD_SLAB; }
 
+// phase: 0 = the whole chunk on `st`; 1 = only the part that does not read theta (sample weights into grad_a, the
+// power-of-two scale of the split, the transposed spins); 2 = the rest.  nk_energy_gradient runs phase 1 on a second
+// stream beside the theta contraction of the same chunk (71 us of small kernels at config 5) and phase 2 after both.
 cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, int64_t B_total,
                                   const void* eloc, const double* stats, const GradWs& w, int first_chunk,
-                                  float real_scale, cudaStream_t st, const float* theta_in, const void* sigT_ready) {
+                                  float real_scale, cudaStream_t st, const float* theta_in, const void* sigT_ready,
+                                  int phase) {
     if (nb <= 0) return cudaSuccess;
     const bool cplx = dtype == NK_C64;
     const double inv_B = 1.0 / (double)B_total;
     const int k_len = (int)((nb + 127) / 128 * 128);
-    cudaError_t e = cudaMemsetAsync(w.absmax, 0, sizeof(unsigned), st);
-    if (e != cudaSuccess) return e;
     const int n_slabs = (int)((nb + GRAD_SLAB - 1) / GRAD_SLAB);
-    const float* th_in = theta_in ? theta_in : w.theta;
-    grad_a_partial_kernel<<<dim3((g.N + 127) / 128, n_slabs), 128, 0, st>>>(
-        sigma, nb, g.N, (const float*)eloc, stats, inv_B, cplx, (double)real_scale, w.part, cplx ? nullptr : w.absmax);
     const dim3 red_block(32, n_slabs >= 128 ? 32 : 8);
-    grad_slab_reduce_kernel<<<(2 * g.N + 31) / 32, red_block, 0, st>>>(w.part, n_slabs, 2 * g.N, w.ga_acc, first_chunk,
-                                                                   cplx ? nullptr : w.absmax);
+    cudaError_t e;
+    if (phase != 2) {
+        e = cudaMemsetAsync(w.absmax, 0, sizeof(unsigned), st);
+        if (e != cudaSuccess) return e;
+        // (grad_a's partial sums go to the upper part of `part`'s allocation when the phases run side by side: see carve_grad)
+        grad_a_partial_kernel<<<dim3((g.N + 127) / 128, n_slabs), 128, 0, st>>>(
+            sigma, nb, g.N, (const float*)eloc, stats, inv_B, cplx, (double)real_scale, w.part_a,
+            cplx ? nullptr : w.absmax);
+        grad_slab_reduce_kernel<<<(2 * g.N + 31) / 32, red_block, 0, st>>>(w.part_a, n_slabs, 2 * g.N, w.ga_acc,
+                                                                       first_chunk, cplx ? nullptr : w.absmax);
+        count_launch(2);
+        if (sigT_ready == nullptr) {
+            grad_sigma_T_kernel<<<dim3(k_len / 128, (g.N + 127) / 128), 256, 0, st>>>(sigma, nb, k_len, g.N, w.ld,
+                                                                                         (int8_t*)w.sigT);
+            count_launch();
+        }
+        e = cudaGetLastError();
+        if (e != cudaSuccess || phase == 1) return e;
+    }
+    const float* th_in = theta_in ? theta_in : w.theta;
     if (!cplx) {
         // k_len / GRAD_SLAB == n_slabs (both round nb up to 128)
         grad_tv_split_kernel<<<(unsigned)n_slabs * (unsigned)(g.M_eff / 32), 256, 0, st>>>(
             th_in, nb, k_len, g.M, g.M_eff, w.ld, (const float*)eloc, stats, inv_B, real_scale, w.absmax,
             (int8_t*)w.TwT, w.part);
-        count_launch(sigT_ready ? 4 : 5);
+        count_launch(2);
     } else {
         dim3 gtv((g.M_pad + 255) / 256, (unsigned)(nb < 1184 ? nb : 1184));
         grad_tv_kernel<true><<<gtv, 256, 0, st>>>(th_in, w.theta, nb, g.M, g.M_pad, g.M_eff, (const float*)eloc, stats,
@@ -403,13 +420,10 @@ cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* si
         grad_colsum_partial_kernel<<<dim3((g.M_eff + 127) / 128, n_slabs), 128, 0, st>>>(w.theta, nb, g.M_eff, w.part);
         grad_split_T_kernel<<<dim3(k_len / 32, g.M_eff / 32), dim3(32, 8), 0, st>>>(
             w.theta, nb, k_len, g.M_eff, w.ld, w.absmax, (int8_t*)w.TwT);
-        count_launch(sigT_ready ? 6 : 7);
+        count_launch(4);
     }
     grad_slab_reduce_kernel<<<(g.M_eff + 31) / 32, red_block, 0, st>>>(w.part, n_slabs, g.M_eff, w.gb_acc, first_chunk,
                                                                    nullptr);
-    if (sigT_ready == nullptr)
-        grad_sigma_T_kernel<<<dim3(k_len / 128, (g.N + 127) / 128), 256, 0, st>>>(sigma, nb, k_len, g.N, w.ld,
-                                                                                     (int8_t*)w.sigT);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     return launch_tc_gemm_pieces(sigT_ready ? sigT_ready : (const void*)w.sigT, g.N, w.TwT, g.M_eff, w.ld, k_len, w.Gacc,

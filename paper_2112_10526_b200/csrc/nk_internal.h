@@ -120,7 +120,8 @@ struct GradWs {
     float *Wg, *bg, *theta, *Gacc;
     uint16_t *Ws, *A, *TwT, *sigT;
     double *gb_acc, *ga_acc;
-    double* part;               // [ceil(chunk / grad_slab())][max(M_eff, 2 N)] per-slab partial column sums
+    double* part;               // [ceil(chunk / grad_slab())][M_eff] per-slab partial column sums (grad_b)
+    double* part_a;             // [ceil(chunk / grad_slab())][2 N] the same for grad_a
     unsigned* absmax;
     int ld;                     // k extent (samples per chunk, rounded up to 64) of TwT / sigT
 };
@@ -128,7 +129,7 @@ int grad_slab();
 cudaError_t launch_gradient_chunk(const Geometry& g, int dtype, const int8_t* sigma, int64_t nb, int64_t B_total,
                                   const void* eloc, const double* stats, const GradWs& w, int first_chunk,
                                   float real_scale, cudaStream_t st, const float* theta_in = nullptr,
-                                  const void* sigT_ready = nullptr);
+                                  const void* sigT_ready = nullptr, int phase = 0);
 // real_scale: 2 (gradient 2 Re f~) | 1 (QGT).  theta_in: read theta from there (w.theta receives v) instead of in
 // place; sigT_ready: the chunk's transposed bf16 spins prepared earlier by launch_sigma_T (w.sigT is not touched).
 cudaError_t launch_sigma_T(const int8_t* sigma, int64_t nb, int N, int ld, void* sigT, cudaStream_t st);
