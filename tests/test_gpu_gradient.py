@@ -51,6 +51,19 @@ def test_gradient_parity_configs(nk, cfg, n, chunk):
     print(f"cfg{cfg}: max gradient error / max|g| = {worst:.2e}")
 
 
+@pytest.mark.parametrize("chunk", [0, 16384])
+def test_gradient_full_batch_config5(nk, chunk):
+    """All 65536 samples of config 5 in the launch configuration bench.py times (the whole batch as one chunk) and in
+    four chunks, against the float64 oracle on the same inputs.  The local energies are an INPUT of this call: seeded
+    normal numbers with the mean and spread of config 5's (they need not come from any local-energy routine)."""
+    p = inp.make_config(5)
+    rng = np.random.default_rng(77)
+    e32 = (-2197.8 + 4.6 * rng.standard_normal(p.n_samples)).astype(np.float32)
+    st = np.array(orc.stats(e32.astype(np.float64)))
+    worst = check(nk, p, e32, st, chunk)
+    print(f"cfg5 full batch, chunk {chunk}: max gradient error / max|g| = {worst:.2e}")
+
+
 @pytest.mark.parametrize("case", [
     dict(kind=0, lattice="chain", L=4, M=1, B=1),
     dict(kind=1, lattice="chain", L=7, M=5, B=31, h=0.8),
