@@ -275,6 +275,30 @@ def qgt_matvec(sigma, W, b, v_a, v_b, v_W, diag_shift=0.0):
     return unpack_params(out, N, M)
 
 
+def qgt_matvec_batched(sigma, W, b, v_a, v_b, v_W, diag_shift=0.0, return_w=False):
+    """Same numbers as `qgt_matvec` without the [B][P] Jacobian (needed at full batch size): with O_a = s,
+    O_b = tanh theta, O_W = tanh theta s^T (Eq. (13)) the three steps of Eq. (75) L2219 are
+        (J v)_s = s_s . v_a + sum_j tanh(theta_sj) (v_b,j + (V_W s_s)_j),
+        dw = (J v) / N_s - <(J v) / N_s>,
+        v~_a = s^T dw,   v~_b = conj(tanh theta)^T dw,   v~_W = (conj(tanh theta) * dw)^T s,
+    as library matmuls; + eps v (Eq. (25)).  return_w: also return J v (the tests' error scale)."""
+    cplx = np.iscomplexobj(W)
+    sigma = np.atleast_2d(np.asarray(sigma))
+    dt = np.complex128 if cplx else np.float64
+    T = np.tanh(rbm_theta(sigma, W, b))
+    s = sigma.astype(dt)
+    v_a, v_b, v_W = (np.asarray(x).astype(dt) for x in (v_a, v_b, v_W))
+    Jv = s @ v_a + np.sum(T * (v_b[None, :] + s @ v_W.T), axis=1)
+    w = Jv / sigma.shape[0]
+    dw = w - w.mean()
+    out_a = s.T @ dw + diag_shift * v_a
+    out_b = np.conj(T).T @ dw + diag_shift * v_b
+    out_W = (np.conj(T) * dw[:, None]).T @ s + diag_shift * v_W
+    if not cplx:
+        out_a, out_b, out_W = out_a.real, out_b.real, out_W.real
+    return (out_a, out_b, out_W, Jv) if return_w else (out_a, out_b, out_W)
+
+
 def sr_solve(sigma, W, b, f_a, f_b, f_W, diag_shift):
     """Stochastic reconfiguration: the solution delta of sum_j (G_ij + eps delta_ij) delta_j = f_i
     (Eq. (25) L886 with Eq. (30)/(31) L961-967), by a dense direct solve of the definition."""

@@ -58,6 +58,25 @@ def test_qgt_matvec_parity_configs(nk, cfg, n, chunk):
     print(f"cfg{cfg}: max QGT-vector error / max|out| = {worst:.2e}")
 
 
+@pytest.mark.parametrize("chunk", [0, 16384])
+def test_qgt_matvec_full_batch_config5(nk, chunk):
+    """All 65536 samples of config 5 (the launch configuration bench.py times, and four chunks) against the oracle's
+    Jacobian-free route `qgt_matvec_batched` (pinned to the dense covariance matrix in tests/test_oracle_qgt.py)."""
+    p = inp.make_config(5)
+    rng = np.random.default_rng(91)
+    va = rng.standard_normal(p.n_sites).astype(np.float32)
+    vb = rng.standard_normal(p.n_hidden).astype(np.float32)
+    vW = rng.standard_normal((p.n_hidden, p.n_sites)).astype(np.float32)
+    out = nk.qgt_matvec(dev(p.sigma), dev(p.W), dev(p.b), dev(va), dev(vb), dev(vW), diag_shift=0.01, chunk_size=chunk)
+    torch.cuda.synchronize()
+    ra, rb, rW, Jv = orc.qgt_matvec_batched(p.sigma, p.W, p.b, va, vb, vW, 0.01, return_w=True)
+    bound = 1e-6 * np.abs(Jv - Jv.mean()).max()                         # as in check(): the scale of the sample weights
+    for name, g, r, vv in (("a", out[0], ra, va), ("b", out[1], rb, vb), ("W", out[2], rW, vW)):
+        err = np.abs(g.cpu().numpy().astype(np.float64) - r).max()
+        assert err <= bound + 2e-7 * np.abs(r).max() + 1e-9 * np.abs(vv).max(), f"out_{name}: err {err}, bound {bound}"
+        print(f"cfg5 full batch chunk {chunk} out_{name}: err / max|out| = {err / np.abs(r).max():.2e}")
+
+
 def test_qgt_matvec_at_the_width_limit(nk):
     """M = 4096 real / 2048 complex (include/nkb200.h): the contractions are size-generic, only the limit moved."""
     for kw in (dict(M=4096), dict(M=2048, complex_params=True)):

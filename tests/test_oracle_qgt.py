@@ -86,3 +86,23 @@ def test_matvec_and_sr_solve_against_the_dense_matrix(cplx):
     const_sigma = np.tile(sigma[:1], (8, 1))
     z = orc.pack_params(*orc.qgt_matvec(const_sigma, W, b, va, vb, vW))
     assert np.abs(z).max() < 1e-12
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_batched_matvec_equals_the_dense_matrix_and_the_jacobian_route(cplx):
+    """`qgt_matvec_batched` (no [B][P] Jacobian; used at full batch size) is pinned to the DEFINITION, the dense
+    covariance matrix of Eq. (23) built by np.cov above, not only to `qgt_matvec`; M != N guards a transposed v_W."""
+    N, M, B = 5, 7, 150
+    W, a, b = _params(N, M, 0.4, 21, cplx)
+    rng = np.random.default_rng(5)
+    sigma = (1 - 2 * rng.integers(0, 2, size=(B, N))).astype(np.int8)
+    vW, va, vb = _params(N, M, 1.0, 23, cplx)
+    J = orc.rbm_jacobian(sigma, W, b)
+    G = np.cov(np.conj(J).T, bias=True)
+    v = orc.pack_params(va, vb, vW)
+    oa, ob, oW, Jv = orc.qgt_matvec_batched(sigma, W, b, va, vb, vW, diag_shift=0.02, return_w=True)
+    out = orc.pack_params(oa, ob, oW)
+    np.testing.assert_allclose(out, (G if cplx else G.real) @ v + 0.02 * v, atol=1e-12)
+    np.testing.assert_allclose(out, orc.pack_params(*orc.qgt_matvec(sigma, W, b, va, vb, vW, diag_shift=0.02)), atol=1e-12)
+    np.testing.assert_allclose(Jv, J @ v.astype(J.dtype), atol=1e-12)
+    assert np.iscomplexobj(out) == cplx
