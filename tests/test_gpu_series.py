@@ -127,6 +127,30 @@ def test_config5_full_batch_every_sample(nk, cfg5_full, form_name):
     print(f"config 5, all {p.n_samples} samples, {form_name}: max rel err E_loc {worst:.2e}")
 
 
+def test_series_more_than_one_theta_window(nk):
+    """theta is contracted once per WINDOW of groups (api.cu carve_eloc: as many groups as keep it under 1 GiB — 8 at
+    config 5's width).  136072 samples of config 5 are nine groups of 16384 (the last one ragged) = two windows, the
+    second holding one partial group; sampled rows of every region against the incremental oracle, the per-sample
+    results bit-equal to those of a batch that fits one window, and the eager call bit-equal to the host-buffer call
+    (which keeps one group per window)."""
+    B = 8 * 16384 + 5000
+    p = inp.make_config(5, n_samples=B)
+    (e, lp, st), form, terms = run_form(nk, p, 0)
+    assert form == nk.NK_FORM_SERIES and terms == 5 and st[3] == B
+    rows = np.concatenate([np.arange(0, 24), np.arange(16384 - 12, 16384 + 12), np.arange(7 * 16384 - 8, 7 * 16384 + 8),
+                           np.arange(8 * 16384 - 16, 8 * 16384 + 16), np.arange(B - 24, B)])
+    e_ref, lp_ref = inc.local_energy(p.kind, p.sigma[rows], p.bonds, p.colors, p.J, p.h, p.W, p.a, p.b)
+    assert_eloc(e[rows], e_ref)
+    assert_logpsi(lp[rows], lp_ref)
+    # the tail of the second window as a batch of its own (one window): per-sample results do not depend on the split
+    q = inp.make_config(5, n_samples=16)
+    q.sigma = p.sigma[8 * 16384: 8 * 16384 + 5000].copy()
+    (e_tail, lp_tail, _), _, _ = run_form(nk, q, 0)
+    assert np.array_equal(e_tail, e[8 * 16384:]) and np.array_equal(lp_tail, lp[8 * 16384:])
+    m = orc.stats(e.astype(np.float64))
+    assert abs(st[0] - m[0]) <= 1e-9 * abs(m[0]) and abs(st[2] - m[2]) <= 1e-9 * m[2]
+
+
 @pytest.mark.parametrize("cfg,n,chunk", [(5, 700, 256), (2, 300, 128), (4, 200, 0)])
 def test_plan_replay_equals_the_eager_call(nk, cfg, n, chunk):
     """nk_local_energy_plan_*: the captured graph replays the same kernels — bit-identical outputs, new CONTENTS of the
